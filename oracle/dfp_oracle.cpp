@@ -1,0 +1,612 @@
+// dfp_oracle.cpp - TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+//
+// Plain, slow, fp64 CPU statement of what the dfp hot path computes, written from
+// /root/reference/PAPER.md (arXiv 2508.13304) and the readings in SURVEY.md §8(c) / DESIGN.md.
+// It shares no code, header, table or helper with the CUDA path (paper_2508_13304_b200/csrc) and
+// neither imports the other.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+// `--impl reference` leg may load it.  OpenMP is used only to spread independent rays / voxels
+// over cores; there is no blocking, fusion or reordering inside a ray or a voxel.
+//
+// Pins (tests/test_oracle_*.py, all `-m "not gpu"`): closed-form ellipsoid and Gaussian line
+// integrals, explicit-transpose adjointness, central finite differences in all six pose
+// parameters, the translation invariant dL/dt = -R A[grad mu], 6-accumulator vs the paper's
+// 12-element G route, stored-G literal algorithm, brute-force back-projection on tiny grids.
+// No function here is "parity unpinned".
+//
+// Conventions:
+//   vol[iz][iy][ix], x fastest; proj[view][iv][iu], u fastest; pose = (tx,ty,tz,gx,gy,gz) mm / rad.
+//   O1  voxel centre r'_j = c + ((ix-(nx-1)/2)vx, (iy-(ny-1)/2)vy, (iz-(nz-1)/2)vz)
+//   O2  f~ = trilinear interpolant between voxel centres, out-of-range voxels read as 0
+//   O4  R = Rz(gz) Ry(gy) Rx(gx);  r = R r' + t;  r' = R^T (r - t)         (Table I :29-36)
+//   O5  view angle b: n=(cos b, sin b,0); source s = SAD n; detector centre -(SDD-SAD) n;
+//       e_u=(-sin b, cos b, 0); e_v=(0,0,1); P in pixel-index units         (Eq.1 :60-63)
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+#include <algorithm>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+extern "C" {
+struct ora_geom {
+  int32_t nx, ny, nz;
+  double vx, vy, vz;
+  double cx, cy, cz;
+  int32_t nu, nv;
+  double du, dv, u0, v0;
+  double sad, sdd;
+  double step_mm;
+  int32_t bp_weight;
+  int32_t flags;
+};
+}
+
+namespace {
+
+struct V3 { double x, y, z; };
+inline V3 operator+(V3 a, V3 b) { return {a.x + b.x, a.y + b.y, a.z + b.z}; }
+inline V3 operator-(V3 a, V3 b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
+inline V3 operator*(double s, V3 a) { return {s * a.x, s * a.y, s * a.z}; }
+inline double dot(V3 a, V3 b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
+inline V3 cross(V3 a, V3 b) { return {a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x}; }
+inline double comp(V3 a, int k) { return k == 0 ? a.x : (k == 1 ? a.y : a.z); }
+
+struct M3 { double m[3][3]; };
+inline M3 mul(const M3& a, const M3& b) {
+  M3 c;
+  for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) {
+    double s = 0; for (int k = 0; k < 3; ++k) s += a.m[i][k] * b.m[k][j]; c.m[i][j] = s; }
+  return c;
+}
+inline V3 mul(const M3& a, V3 v) {
+  return {a.m[0][0] * v.x + a.m[0][1] * v.y + a.m[0][2] * v.z,
+          a.m[1][0] * v.x + a.m[1][1] * v.y + a.m[1][2] * v.z,
+          a.m[2][0] * v.x + a.m[2][1] * v.y + a.m[2][2] * v.z};
+}
+inline V3 mulT(const M3& a, V3 v) {   // a^T v
+  return {a.m[0][0] * v.x + a.m[1][0] * v.y + a.m[2][0] * v.z,
+          a.m[0][1] * v.x + a.m[1][1] * v.y + a.m[2][1] * v.z,
+          a.m[0][2] * v.x + a.m[1][2] * v.y + a.m[2][2] * v.z};
+}
+inline M3 Rx(double a) { double c = cos(a), s = sin(a); return {{{1, 0, 0}, {0, c, -s}, {0, s, c}}}; }
+inline M3 Ry(double a) { double c = cos(a), s = sin(a); return {{{c, 0, s}, {0, 1, 0}, {-s, 0, c}}}; }
+inline M3 Rz(double a) { double c = cos(a), s = sin(a); return {{{c, -s, 0}, {s, c, 0}, {0, 0, 1}}}; }
+inline M3 dRx(double a) { double c = cos(a), s = sin(a); return {{{0, 0, 0}, {0, -s, -c}, {0, c, -s}}}; }
+inline M3 dRy(double a) { double c = cos(a), s = sin(a); return {{{-s, 0, c}, {0, 0, 0}, {-c, 0, -s}}}; }
+inline M3 dRz(double a) { double c = cos(a), s = sin(a); return {{{-s, -c, 0}, {c, -s, 0}, {0, 0, 0}}}; }
+
+// O4 + U4: pose -> R, t and dR/dgamma_k (PAPER.md :79 "has an explicit expression").
+struct Pose {
+  M3 R; V3 t; M3 dR[3];
+  explicit Pose(const double* th) {
+    t = {th[0], th[1], th[2]};
+    M3 rx = Rx(th[3]), ry = Ry(th[4]), rz = Rz(th[5]);
+    R = mul(rz, mul(ry, rx));
+    dR[0] = mul(rz, mul(ry, dRx(th[3])));
+    dR[1] = mul(rz, mul(dRy(th[4]), rx));
+    dR[2] = mul(dRz(th[5]), mul(ry, rx));
+  }
+};
+
+// O5: one view of the circular cone-beam scanner.
+struct View {
+  V3 n, s, dc, eu, ev; double P[3][4]; double cu, cv;
+  View(const ora_geom& g, double beta) {
+    n = {cos(beta), sin(beta), 0.0};
+    s = g.sad * n;
+    dc = -(g.sdd - g.sad) * n;
+    eu = {-sin(beta), cos(beta), 0.0};
+    ev = {0.0, 0.0, 1.0};
+    cu = (g.nu - 1) / 2.0 + g.u0;
+    cv = (g.nv - 1) / 2.0 + g.v0;
+    double P3[4] = {-n.x, -n.y, -n.z, g.sad};
+    double e1[4] = {eu.x, eu.y, eu.z, 0.0}, e2[4] = {ev.x, ev.y, ev.z, 0.0};
+    for (int k = 0; k < 4; ++k) {
+      P[2][k] = P3[k];
+      P[0][k] = (g.sdd / g.du) * e1[k] + cu * P3[k];
+      P[1][k] = (g.sdd / g.dv) * e2[k] + cv * P3[k];
+    }
+  }
+  V3 pixel(const ora_geom& g, int iu, int iv) const {
+    return dc + ((iu - cu) * g.du) * eu + ((iv - cv) * g.dv) * ev;
+  }
+};
+
+inline double step_of(const ora_geom& g) {
+  return g.step_mm > 0 ? g.step_mm : std::min(g.vx, std::min(g.vy, g.vz));
+}
+
+// O1: object-frame mm -> continuous voxel index.
+inline V3 to_index(const ora_geom& g, V3 rp) {
+  return {(rp.x - g.cx) / g.vx + (g.nx - 1) / 2.0, (rp.y - g.cy) / g.vy + (g.ny - 1) / 2.0,
+          (rp.z - g.cz) / g.vz + (g.nz - 1) / 2.0};
+}
+inline V3 voxel_centre(const ora_geom& g, int ix, int iy, int iz) {
+  return {g.cx + (ix - (g.nx - 1) / 2.0) * g.vx, g.cy + (iy - (g.ny - 1) / 2.0) * g.vy,
+          g.cz + (iz - (g.nz - 1) / 2.0) * g.vz};
+}
+
+template <typename T>
+struct Vol {
+  const T* v; int nx, ny, nz;
+  double at(long ix, long iy, long iz) const {
+    if (ix < 0 || iy < 0 || iz < 0 || ix >= nx || iy >= ny || iz >= nz) return 0.0;
+    return (double)v[((size_t)iz * ny + iy) * nx + ix];
+  }
+};
+
+// O2: zero-extended trilinear interpolant at continuous index p.
+template <typename T>
+inline double trilin(const Vol<T>& V, V3 p) {
+  double fx = floor(p.x), fy = floor(p.y), fz = floor(p.z);
+  long ix = (long)fx, iy = (long)fy, iz = (long)fz;
+  double ax = p.x - fx, ay = p.y - fy, az = p.z - fz;
+  double s = 0.0;
+  for (int dz = 0; dz < 2; ++dz) for (int dy = 0; dy < 2; ++dy) for (int dx = 0; dx < 2; ++dx) {
+    double w = (dx ? ax : 1 - ax) * (dy ? ay : 1 - ay) * (dz ? az : 1 - az);
+    s += w * V.at(ix + dx, iy + dy, iz + dz);
+  }
+  return s;
+}
+
+// O3: volume gradient at a sample (per mm).
+//  mode 0 CENTRAL (the paper's "central finite difference", PAPER.md :183):
+//         g_a = [f~(r' + v_a e_a) - f~(r' - v_a e_a)] / (2 v_a)
+//  mode 1 INTERP: exact derivative of the trilinear interpolant (test aid).
+template <typename T>
+inline V3 vol_grad(const Vol<T>& V, const ora_geom& g, V3 p, int mode) {
+  if (mode == 0) {
+    V3 ex = {1, 0, 0}, ey = {0, 1, 0}, ez = {0, 0, 1};
+    return {(trilin(V, p + ex) - trilin(V, p - ex)) / (2 * g.vx),
+            (trilin(V, p + ey) - trilin(V, p - ey)) / (2 * g.vy),
+            (trilin(V, p + ez) - trilin(V, p - ez)) / (2 * g.vz)};
+  }
+  double fx = floor(p.x), fy = floor(p.y), fz = floor(p.z);
+  long ix = (long)fx, iy = (long)fy, iz = (long)fz;
+  double a[3] = {p.x - fx, p.y - fy, p.z - fz};
+  double gx = 0, gy = 0, gz = 0;
+  for (int dz = 0; dz < 2; ++dz) for (int dy = 0; dy < 2; ++dy) for (int dx = 0; dx < 2; ++dx) {
+    double val = V.at(ix + dx, iy + dy, iz + dz);
+    double wx = dx ? a[0] : 1 - a[0], wy = dy ? a[1] : 1 - a[1], wz = dz ? a[2] : 1 - a[2];
+    gx += (dx ? 1.0 : -1.0) * wy * wz * val;
+    gy += wx * (dy ? 1.0 : -1.0) * wz * val;
+    gz += wx * wy * (dz ? 1.0 : -1.0) * val;
+  }
+  return {gx / g.vx, gy / g.vy, gz / g.vz};
+}
+
+// Sample index range [k0,k1] that is a SUPERSET of the samples whose object-frame position can
+// fall inside the volume padded by `pad` voxels (O6: "clipping the range never changes the value").
+inline bool k_range(const ora_geom& g, V3 ps, V3 pe_per_mm, double step, double pad, long& k0, long& k1) {
+  double lo = -1e300, hi = 1e300;
+  double n[3] = {(double)g.nx, (double)g.ny, (double)g.nz};
+  for (int a = 0; a < 3; ++a) {
+    double o = comp(ps, a), d = comp(pe_per_mm, a);
+    double bmin = -pad, bmax = n[a] - 1 + pad;
+    if (fabs(d) < 1e-300) { if (o < bmin || o > bmax) return false; continue; }
+    double t0 = (bmin - o) / d, t1 = (bmax - o) / d;
+    if (t0 > t1) std::swap(t0, t1);
+    lo = std::max(lo, t0); hi = std::min(hi, t1);
+  }
+  if (hi < lo || hi < 0) return false;
+  k0 = (long)floor(lo / step) - 2; if (k0 < 0) k0 = 0;
+  k1 = (long)ceil(hi / step) + 2;
+  return true;
+}
+inline bool in_padded_box(const ora_geom& g, V3 p, double pad) {
+  return p.x >= -pad && p.x <= g.nx - 1 + pad && p.y >= -pad && p.y <= g.ny - 1 + pad &&
+         p.z >= -pad && p.z <= g.nz - 1 + pad;
+}
+
+// ------------------------------------------------------------------------------------------------
+// O6: forward projection, Eq.2a :67-69 discretised as Eq.18 :172-177 with a fixed-step
+// trilinear ray-march (reading U1):  l_i = D * sum_k f~(R^T (s + tau_k e - t)),  tau_k=(k+1/2) D.
+template <typename T>
+void forward_impl(const ora_geom& g, int n_views, const double* angles, const double* poses, const T* vol,
+                  double* proj, int64_t* ray_steps) {
+  Vol<T> V{vol, g.nx, g.ny, g.nz};
+  const double D = step_of(g);
+  int64_t total_steps = 0;
+  for (int v = 0; v < n_views; ++v) {
+    View view(g, angles[v]);
+    Pose pose(poses + 6 * v);
+    int64_t steps_v = 0;
+#pragma omp parallel for schedule(dynamic, 4) reduction(+ : steps_v)
+    for (int iv = 0; iv < g.nv; ++iv) {
+      for (int iu = 0; iu < g.nu; ++iu) {
+        V3 d = view.pixel(g, iu, iv) - view.s;
+        V3 e = (1.0 / sqrt(dot(d, d))) * d;
+        // range of k worth visiting (object-frame line: s' + tau e')
+        V3 ps = to_index(g, mulT(pose.R, view.s - pose.t));
+        V3 eo = mulT(pose.R, e);
+        V3 pe = {eo.x / g.vx, eo.y / g.vy, eo.z / g.vz};
+        long k0, k1;
+        double sum = 0.0;
+        if (k_range(g, ps, pe, D, 3.0, k0, k1)) {
+          for (long k = k0; k <= k1; ++k) {
+            double tau = (k + 0.5) * D;
+            V3 r = view.s + tau * e;                 // world sample, fixed in the world
+            V3 rp = mulT(pose.R, r - pose.t);        // r' = R^T (r - t)
+            V3 p = to_index(g, rp);
+            sum += trilin(V, p);
+            if (in_padded_box(g, p, 2.0)) ++steps_v;
+          }
+        }
+        proj[((size_t)v * g.nv + iv) * g.nu + iu] = D * sum;
+      }
+    }
+    total_steps += steps_v;
+  }
+  if (ray_steps) *ray_steps = total_steps;
+}
+
+// O10: explicit transpose of the forward projector (adjointness pin only).
+template <typename T>
+void forward_T_impl(const ora_geom& g, int n_views, const double* angles, const double* poses, const T* y,
+                    double* vol_out) {
+  const double D = step_of(g);
+  size_t nvox = (size_t)g.nx * g.ny * g.nz;
+  for (size_t i = 0; i < nvox; ++i) vol_out[i] = 0.0;
+  for (int v = 0; v < n_views; ++v) {
+    View view(g, angles[v]);
+    Pose pose(poses + 6 * v);
+    for (int iv = 0; iv < g.nv; ++iv) for (int iu = 0; iu < g.nu; ++iu) {
+      double yi = (double)y[((size_t)v * g.nv + iv) * g.nu + iu];
+      V3 d = view.pixel(g, iu, iv) - view.s;
+      V3 e = (1.0 / sqrt(dot(d, d))) * d;
+      V3 ps = to_index(g, mulT(pose.R, view.s - pose.t));
+      V3 eo = mulT(pose.R, e);
+      V3 pe = {eo.x / g.vx, eo.y / g.vy, eo.z / g.vz};
+      long k0, k1;
+      if (!k_range(g, ps, pe, D, 3.0, k0, k1)) continue;
+      for (long k = k0; k <= k1; ++k) {
+        V3 p = to_index(g, mulT(pose.R, view.s + ((k + 0.5) * D) * e - pose.t));
+        double fx = floor(p.x), fy = floor(p.y), fz = floor(p.z);
+        long ix = (long)fx, iy = (long)fy, iz = (long)fz;
+        double ax = p.x - fx, ay = p.y - fy, az = p.z - fz;
+        for (int dz = 0; dz < 2; ++dz) for (int dy = 0; dy < 2; ++dy) for (int dx = 0; dx < 2; ++dx) {
+          long X = ix + dx, Y = iy + dy, Z = iz + dz;
+          if (X < 0 || Y < 0 || Z < 0 || X >= g.nx || Y >= g.ny || Z >= g.nz) continue;
+          double w = (dx ? ax : 1 - ax) * (dy ? ay : 1 - ay) * (dz ? az : 1 - az);
+          vol_out[((size_t)Z * g.ny + Y) * g.nx + X] += D * w * yi;
+        }
+      }
+    }
+  }
+}
+
+// dL/dtheta_k = sum_ab (dM_ab/dtheta_k) (grad_M L)_ab, M = [R | t]   (PAPER.md :79, reading U4).
+inline void contract_M(const Pose& pose, const double GM[3][4], double* out6) {
+  for (int k = 0; k < 3; ++k) out6[k] = GM[k][3];
+  for (int k = 0; k < 3; ++k) {
+    double s = 0;
+    for (int a = 0; a < 3; ++a) for (int b = 0; b < 3; ++b) s += pose.dR[k].m[a][b] * GM[a][b];
+    out6[3 + k] = s;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// O7: forward pose gradient, Eq.3-8 :81-113 and Eq.19-20 :179-191.
+//  lever_arm 0 SAMPLE: G_f evaluated at the interpolated sample (reading U2, default)
+//            1 VOXEL : per-voxel G_f^j (central-difference gradient and lever arm at voxel centres,
+//                      "Compute matrix G_f^j for each voxel", :189) projected with the weights a^ij
+//  grad_mode 0 CENTRAL | 1 INTERP (SAMPLE only)
+//  route 0: six accumulators  A_i = D sum g~,  B_i = D sum r' x g~;  dL/dt = -R S_A, dL/dgamma_k = -w_k.S_B
+//        1: the paper's 12-element route  G_f = [ (r-t) g~^T | -R g~ ]  (Eq.6/8), contracted with dM/dtheta
+template <typename T>
+void forward_grad_impl(const ora_geom& g, int n_views, const double* angles, const double* poses, const T* vol,
+                       const float* upstream, double* grad, int lever_arm, int grad_mode, int route) {
+  Vol<T> V{vol, g.nx, g.ny, g.nz};
+  const double D = step_of(g);
+  for (int v = 0; v < n_views; ++v) {
+    View view(g, angles[v]);
+    Pose pose(poses + 6 * v);
+    // per-row partial sums, added in row order afterwards (deterministic)
+    std::vector<double> rowacc((size_t)g.nv * 12, 0.0);
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int iv = 0; iv < g.nv; ++iv) {
+      double acc[12] = {0};
+      for (int iu = 0; iu < g.nu; ++iu) {
+        double w = (double)upstream[((size_t)v * g.nv + iv) * g.nu + iu];
+        V3 d = view.pixel(g, iu, iv) - view.s;
+        V3 e = (1.0 / sqrt(dot(d, d))) * d;
+        V3 ps = to_index(g, mulT(pose.R, view.s - pose.t));
+        V3 eo = mulT(pose.R, e);
+        V3 pe = {eo.x / g.vx, eo.y / g.vy, eo.z / g.vz};
+        long k0, k1;
+        if (!k_range(g, ps, pe, D, 3.0, k0, k1)) continue;
+        V3 A = {0, 0, 0}, B = {0, 0, 0};
+        double GM[3][4] = {{0}};
+        for (long k = k0; k <= k1; ++k) {
+          V3 r = view.s + ((k + 0.5) * D) * e;
+          V3 rp = mulT(pose.R, r - pose.t);
+          V3 p = to_index(g, rp);
+          if (lever_arm == 0) {
+            V3 gr = vol_grad(V, g, p, grad_mode);
+            if (route == 0) {
+              A = A + gr;
+              B = B + cross(rp, gr);
+            } else {
+              V3 lever = r - pose.t;              // (x-tx, y-ty, z-tz), Eq.6
+              V3 Rg = mul(pose.R, gr);
+              for (int a = 0; a < 3; ++a) {
+                GM[a][0] += comp(lever, a) * gr.x;
+                GM[a][1] += comp(lever, a) * gr.y;
+                GM[a][2] += comp(lever, a) * gr.z;
+                GM[a][3] += -comp(Rg, a);
+              }
+            }
+          } else {
+            // VOXEL: sum_j a^ij G_f^j, a^ij = trilinear weight of voxel j (including the one-voxel
+            // ring where the central difference of the zero-extended volume is still non-zero).
+            double fx = floor(p.x), fy = floor(p.y), fz = floor(p.z);
+            long ix = (long)fx, iy = (long)fy, iz = (long)fz;
+            double ax = p.x - fx, ay = p.y - fy, az = p.z - fz;
+            for (int dz = 0; dz < 2; ++dz) for (int dy = 0; dy < 2; ++dy) for (int dx = 0; dx < 2; ++dx) {
+              long X = ix + dx, Y = iy + dy, Z = iz + dz;
+              double wt = (dx ? ax : 1 - ax) * (dy ? ay : 1 - ay) * (dz ? az : 1 - az);
+              V3 gj = {(V.at(X + 1, Y, Z) - V.at(X - 1, Y, Z)) / (2 * g.vx),
+                       (V.at(X, Y + 1, Z) - V.at(X, Y - 1, Z)) / (2 * g.vy),
+                       (V.at(X, Y, Z + 1) - V.at(X, Y, Z - 1)) / (2 * g.vz)};
+              V3 rj = voxel_centre(g, (int)X, (int)Y, (int)Z);   // r'_j
+              V3 lever = mul(pose.R, rj);                          // r_j - t = R r'_j
+              V3 Rg = mul(pose.R, gj);
+              for (int a = 0; a < 3; ++a) {
+                GM[a][0] += wt * comp(lever, a) * gj.x;
+                GM[a][1] += wt * comp(lever, a) * gj.y;
+                GM[a][2] += wt * comp(lever, a) * gj.z;
+                GM[a][3] += -wt * comp(Rg, a);
+              }
+            }
+          }
+        }
+        if (lever_arm == 0 && route == 0) {
+          acc[0] += w * D * A.x; acc[1] += w * D * A.y; acc[2] += w * D * A.z;
+          acc[3] += w * D * B.x; acc[4] += w * D * B.y; acc[5] += w * D * B.z;
+        } else {
+          for (int a = 0; a < 3; ++a) for (int b = 0; b < 4; ++b) acc[a * 4 + b] += w * D * GM[a][b];
+        }
+      }
+      for (int q = 0; q < 12; ++q) rowacc[(size_t)iv * 12 + q] = acc[q];
+    }
+    double tot[12] = {0};
+    for (int iv = 0; iv < g.nv; ++iv) for (int q = 0; q < 12; ++q) tot[q] += rowacc[(size_t)iv * 12 + q];
+    double* out = grad + 6 * v;
+    if (lever_arm == 0 && route == 0) {
+      V3 SA = {tot[0], tot[1], tot[2]}, SB = {tot[3], tot[4], tot[5]};
+      V3 dt = mul(pose.R, SA);
+      out[0] = -dt.x; out[1] = -dt.y; out[2] = -dt.z;
+      // axial vectors of R^T dR/dgamma_k:  w_x = e_x, w_y = Rx^T e_y, w_z = (Ry Rx)^T e_z
+      const double* th = poses + 6 * v;
+      V3 wx = {1, 0, 0};
+      V3 wy = mulT(Rx(th[3]), V3{0, 1, 0});
+      V3 wz = mulT(mul(Ry(th[4]), Rx(th[3])), V3{0, 0, 1});
+      out[3] = -dot(wx, SB); out[4] = -dot(wy, SB); out[5] = -dot(wz, SB);
+    } else {
+      double GM[3][4];
+      for (int a = 0; a < 3; ++a) for (int b = 0; b < 4; ++b) GM[a][b] = tot[a * 4 + b];
+      contract_M(pose, GM, out);
+    }
+  }
+}
+
+// zero-extended bilinear interpolant of one projection at pixel-index coordinates (u,v).  O8.
+struct Img {
+  const float* p; int nu, nv;
+  double at(long iu, long iv) const {
+    if (iu < 0 || iv < 0 || iu >= nu || iv >= nv) return 0.0;
+    return (double)p[(size_t)iv * nu + iu];
+  }
+};
+inline double bilin(const Img& I, double u, double v) {
+  double fu = floor(u), fv = floor(v);
+  long iu = (long)fu, iv = (long)fv;
+  double a = u - fu, b = v - fv;
+  return (1 - b) * ((1 - a) * I.at(iu, iv) + a * I.at(iu + 1, iv)) +
+         b * ((1 - a) * I.at(iu, iv + 1) + a * I.at(iu + 1, iv + 1));
+}
+
+// ------------------------------------------------------------------------------------------------
+// O8: voxel-driven back-projection, Eq.2b :71-75 / Eq.21 :193-196.
+//   r_j = R_v r'_j + t_v; (u',v',w') = P_v (r_j;1); mu_j = sum_v W b~_v(u'/w', v'/w'); W = 1 | (SAD/w')^2.
+void backproject_impl(const ora_geom& g, int n_views, const double* angles, const double* poses,
+                      const float* proj, double* vol_out, int iz0, int iz1) {
+  std::vector<View> views; std::vector<Pose> ps;
+  for (int v = 0; v < n_views; ++v) { views.emplace_back(g, angles[v]); ps.emplace_back(poses + 6 * v); }
+#pragma omp parallel for schedule(dynamic, 1) collapse(2)
+  for (int iz = iz0; iz < iz1; ++iz) for (int iy = 0; iy < g.ny; ++iy) for (int ix = 0; ix < g.nx; ++ix) {
+    V3 rp = voxel_centre(g, ix, iy, iz);
+    double s = 0.0;
+    for (int v = 0; v < n_views; ++v) {
+      V3 r = mul(ps[v].R, rp) + ps[v].t;
+      const double(*P)[4] = views[v].P;
+      double up = P[0][0] * r.x + P[0][1] * r.y + P[0][2] * r.z + P[0][3];
+      double vp = P[1][0] * r.x + P[1][1] * r.y + P[1][2] * r.z + P[1][3];
+      double wp = P[2][0] * r.x + P[2][1] * r.y + P[2][2] * r.z + P[2][3];
+      if (wp <= 0) continue;
+      Img I{proj + (size_t)v * g.nu * g.nv, g.nu, g.nv};
+      double W = g.bp_weight ? (g.sad / wp) * (g.sad / wp) : 1.0;
+      s += W * bilin(I, up / wp, vp / wp);
+    }
+    vol_out[((size_t)(iz - iz0) * g.ny + iy) * g.nx + ix] = s;
+  }
+}
+
+// O10: explicit transpose of the back-projector (splat), adjointness pin only.
+void backproject_T_impl(const ora_geom& g, int n_views, const double* angles, const double* poses,
+                        const double* x, double* proj_out) {
+  size_t np = (size_t)n_views * g.nu * g.nv;
+  for (size_t i = 0; i < np; ++i) proj_out[i] = 0.0;
+  for (int v = 0; v < n_views; ++v) {
+    View view(g, angles[v]); Pose pose(poses + 6 * v);
+    double* out = proj_out + (size_t)v * g.nu * g.nv;
+    for (int iz = 0; iz < g.nz; ++iz) for (int iy = 0; iy < g.ny; ++iy) for (int ix = 0; ix < g.nx; ++ix) {
+      V3 r = mul(pose.R, voxel_centre(g, ix, iy, iz)) + pose.t;
+      const double(*P)[4] = view.P;
+      double up = P[0][0] * r.x + P[0][1] * r.y + P[0][2] * r.z + P[0][3];
+      double vp = P[1][0] * r.x + P[1][1] * r.y + P[1][2] * r.z + P[1][3];
+      double wp = P[2][0] * r.x + P[2][1] * r.y + P[2][2] * r.z + P[2][3];
+      if (wp <= 0) continue;
+      double W = g.bp_weight ? (g.sad / wp) * (g.sad / wp) : 1.0;
+      double u = up / wp, vv = vp / wp;
+      double fu = floor(u), fv = floor(vv);
+      long iu = (long)fu, iw = (long)fv;
+      double a = u - fu, b = vv - fv;
+      double xv = x[((size_t)iz * g.ny + iy) * g.nx + ix] * W;
+      for (int dv = 0; dv < 2; ++dv) for (int du = 0; du < 2; ++du) {
+        long U = iu + du, Vv = iw + dv;
+        if (U < 0 || Vv < 0 || U >= g.nu || Vv >= g.nv) continue;
+        out[(size_t)Vv * g.nu + U] += (du ? a : 1 - a) * (dv ? b : 1 - b) * xv;
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// O9: back-projection pose gradient, Eq.9-17 :115-168 and Eq.22 :198-206.
+//  d~_u l = [b~(u+1,v) - b~(u-1,v)]/2 (central difference in pixel units, :202); J from Eq.13 :143-146;
+//  q = W (d~_u l J_u + d~_v l J_v)  [+ b~ dW/dr, dW/dr = -2 W/w' P_3[0:3], if flags&1];
+//  route 0: S_q = sum_j w_j q_j, S_c = sum_j w_j (r_j - t) x q_j; dL/dt = S_q; dL/dgamma_k = a_k . S_c,
+//           a_x = R e_x, a_y = Rz e_y, a_z = e_z  (axial vectors of dR/dgamma_k R^T)
+//  route 1: the paper's 12-element  G_b = q^T (x) (x',y',z',1)  (Eq.15/17) contracted with dM/dtheta.
+//  grad_mode 0 CENTRAL | 1 INTERP (exact derivative of the bilinear interpolant; test aid)
+void backproject_grad_impl(const ora_geom& g, int n_views, const double* angles, const double* poses,
+                           const float* proj, const float* upstream, double* grad, int grad_mode, int route) {
+  for (int v = 0; v < n_views; ++v) {
+    View view(g, angles[v]); Pose pose(poses + 6 * v);
+    Img I{proj + (size_t)v * g.nu * g.nv, g.nu, g.nv};
+    const double(*P)[4] = view.P;
+    std::vector<double> slab((size_t)g.nz * 12, 0.0);
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int iz = 0; iz < g.nz; ++iz) {
+      double acc[12] = {0};
+      for (int iy = 0; iy < g.ny; ++iy) for (int ix = 0; ix < g.nx; ++ix) {
+        double wj = (double)upstream[((size_t)iz * g.ny + iy) * g.nx + ix];
+        V3 rp = voxel_centre(g, ix, iy, iz);
+        V3 r = mul(pose.R, rp) + pose.t;
+        double up = P[0][0] * r.x + P[0][1] * r.y + P[0][2] * r.z + P[0][3];
+        double vp = P[1][0] * r.x + P[1][1] * r.y + P[1][2] * r.z + P[1][3];
+        double wp = P[2][0] * r.x + P[2][1] * r.y + P[2][2] * r.z + P[2][3];
+        if (wp <= 0) continue;
+        double u = up / wp, vv = vp / wp;
+        double W = g.bp_weight ? (g.sad / wp) * (g.sad / wp) : 1.0;
+        double dlu, dlv;
+        if (grad_mode == 0) {
+          dlu = 0.5 * (bilin(I, u + 1, vv) - bilin(I, u - 1, vv));
+          dlv = 0.5 * (bilin(I, u, vv + 1) - bilin(I, u, vv - 1));
+        } else {
+          double fu = floor(u), fv = floor(vv);
+          long iu = (long)fu, iw = (long)fv;
+          double a = u - fu, b = vv - fv;
+          dlu = (1 - b) * (I.at(iu + 1, iw) - I.at(iu, iw)) + b * (I.at(iu + 1, iw + 1) - I.at(iu, iw + 1));
+          dlv = (1 - a) * (I.at(iu, iw + 1) - I.at(iu, iw)) + a * (I.at(iu + 1, iw + 1) - I.at(iu + 1, iw));
+        }
+        V3 Ju = {(P[0][0] * wp - P[2][0] * up) / (wp * wp), (P[0][1] * wp - P[2][1] * up) / (wp * wp),
+                 (P[0][2] * wp - P[2][2] * up) / (wp * wp)};
+        V3 Jv = {(P[1][0] * wp - P[2][0] * vp) / (wp * wp), (P[1][1] * wp - P[2][1] * vp) / (wp * wp),
+                 (P[1][2] * wp - P[2][2] * vp) / (wp * wp)};
+        V3 q = W * ((dlu * Ju) + (dlv * Jv));
+        if ((g.flags & 1) && g.bp_weight) {
+          V3 dW = (-2.0 * W / wp) * V3{P[2][0], P[2][1], P[2][2]};
+          q = q + bilin(I, u, vv) * dW;
+        }
+        if (route == 0) {
+          V3 c = cross(r - pose.t, q);
+          acc[0] += wj * q.x; acc[1] += wj * q.y; acc[2] += wj * q.z;
+          acc[3] += wj * c.x; acc[4] += wj * c.y; acc[5] += wj * c.z;
+        } else {
+          double h[4] = {rp.x, rp.y, rp.z, 1.0};
+          for (int a = 0; a < 3; ++a) for (int b = 0; b < 4; ++b) acc[a * 4 + b] += wj * comp(q, a) * h[b];
+        }
+      }
+      for (int k = 0; k < 12; ++k) slab[(size_t)iz * 12 + k] = acc[k];
+    }
+    double tot[12] = {0};
+    for (int iz = 0; iz < g.nz; ++iz) for (int k = 0; k < 12; ++k) tot[k] += slab[(size_t)iz * 12 + k];
+    double* out = grad + 6 * v;
+    if (route == 0) {
+      const double* th = poses + 6 * v;
+      V3 Sq = {tot[0], tot[1], tot[2]}, Sc = {tot[3], tot[4], tot[5]};
+      V3 ax = mul(pose.R, V3{1, 0, 0});
+      V3 ay = mul(Rz(th[5]), V3{0, 1, 0});
+      V3 az = {0, 0, 1};
+      out[0] = Sq.x; out[1] = Sq.y; out[2] = Sq.z;
+      out[3] = dot(ax, Sc); out[4] = dot(ay, Sc); out[5] = dot(az, Sc);
+    } else {
+      double GM[3][4];
+      for (int a = 0; a < 3; ++a) for (int b = 0; b < 4; ++b) GM[a][b] = tot[a * 4 + b];
+      contract_M(pose, GM, out);
+    }
+  }
+}
+
+}  // namespace
+
+extern "C" {
+
+int ora_num_threads() {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+void ora_set_num_threads(int n) {
+#ifdef _OPENMP
+  if (n > 0) omp_set_num_threads(n);
+#else
+  (void)n;
+#endif
+}
+
+void ora_forward_f32(const ora_geom* g, int n_views, const double* angles, const double* poses, const float* vol,
+                     double* proj, int64_t* ray_steps) {
+  forward_impl<float>(*g, n_views, angles, poses, vol, proj, ray_steps);
+}
+void ora_forward_f64(const ora_geom* g, int n_views, const double* angles, const double* poses, const double* vol,
+                     double* proj, int64_t* ray_steps) {
+  forward_impl<double>(*g, n_views, angles, poses, vol, proj, ray_steps);
+}
+void ora_forward_T(const ora_geom* g, int n_views, const double* angles, const double* poses, const double* y,
+                   double* vol_out) {
+  forward_T_impl<double>(*g, n_views, angles, poses, y, vol_out);
+}
+void ora_forward_pose_grad_f32(const ora_geom* g, int n_views, const double* angles, const double* poses,
+                               const float* vol, const float* upstream, double* grad, int lever_arm,
+                               int grad_mode, int route) {
+  forward_grad_impl<float>(*g, n_views, angles, poses, vol, upstream, grad, lever_arm, grad_mode, route);
+}
+void ora_forward_pose_grad_f64(const ora_geom* g, int n_views, const double* angles, const double* poses,
+                               const double* vol, const float* upstream, double* grad, int lever_arm,
+                               int grad_mode, int route) {
+  forward_grad_impl<double>(*g, n_views, angles, poses, vol, upstream, grad, lever_arm, grad_mode, route);
+}
+void ora_backproject(const ora_geom* g, int n_views, const double* angles, const double* poses, const float* proj,
+                     double* vol_out, int iz0, int iz1) {
+  backproject_impl(*g, n_views, angles, poses, proj, vol_out, iz0, iz1);
+}
+void ora_backproject_T(const ora_geom* g, int n_views, const double* angles, const double* poses, const double* x,
+                       double* proj_out) {
+  backproject_T_impl(*g, n_views, angles, poses, x, proj_out);
+}
+void ora_backproject_pose_grad(const ora_geom* g, int n_views, const double* angles, const double* poses,
+                               const float* proj, const float* upstream, double* grad, int grad_mode, int route) {
+  backproject_grad_impl(*g, n_views, angles, poses, proj, upstream, grad, grad_mode, route);
+}
+// R(gamma) and dR/dgamma_k, exposed so the tests can pin them (finite differences, orthogonality).
+void ora_rotation(const double* pose6, double* R9, double* dR27) {
+  Pose p(pose6);
+  for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) {
+    R9[i * 3 + j] = p.R.m[i][j];
+    for (int k = 0; k < 3; ++k) dR27[k * 9 + i * 3 + j] = p.dR[k].m[i][j];
+  }
+}
+// Projection matrix P (pixel-index units) of a view, exposed so the tests can pin Eq.1.
+void ora_projection_matrix(const ora_geom* g, double angle, double* P12) {
+  View v(*g, angle);
+  for (int i = 0; i < 3; ++i) for (int j = 0; j < 4; ++j) P12[i * 4 + j] = v.P[i][j];
+}
+
+}  // extern "C"

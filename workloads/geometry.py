@@ -1,0 +1,57 @@
+"""Scanner / grid description as plain numbers (the fields of `dfp_geometry`, include/dfp.h).
+
+No projector arithmetic lives here: each implementation (oracle, CUDA host code,
+closed-form renderer) builds its own rays and matrices from these numbers.
+"""
+import dataclasses
+import math
+
+import torch
+
+
+@dataclasses.dataclass
+class Geometry:
+    nx: int
+    ny: int
+    nz: int
+    vx: float
+    vy: float
+    vz: float
+    nu: int
+    nv: int
+    du: float
+    dv: float
+    sad: float
+    sdd: float
+    cx: float = 0.0
+    cy: float = 0.0
+    cz: float = 0.0
+    u0: float = 0.0
+    v0: float = 0.0
+    step_mm: float = 0.0      # <=0: min(vx,vy,vz)
+    bp_weight: int = 0        # 0 unit, 1 FDK (sad/w')^2
+    flags: int = 0            # bit0: add dW/dtheta term in backproject_pose_grad
+
+    def replace(self, **kw) -> "Geometry":
+        return dataclasses.replace(self, **kw)
+
+    def as_dict(self) -> dict:
+        return dataclasses.asdict(self)
+
+    @property
+    def step(self) -> float:
+        return self.step_mm if self.step_mm > 0 else min(self.vx, self.vy, self.vz)
+
+    @property
+    def vol_shape(self):
+        return (self.nz, self.ny, self.nx)
+
+    @property
+    def det_shape(self):
+        return (self.nv, self.nu)
+
+
+def view_angles(n_views: int, arc_deg: float = 360.0, start_deg: float = 0.0) -> torch.Tensor:
+    """Gantry angles in radians, evenly spaced over `arc_deg` (end point excluded), float64."""
+    k = torch.arange(n_views, dtype=torch.float64)
+    return (start_deg + arc_deg * k / n_views) * (math.pi / 180.0)
