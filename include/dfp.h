@@ -1,0 +1,126 @@
+/* dfp.h - C ABI of libdfp: differentiable cone-beam forward / back-projector with a 6-DOF rigid pose per view.
+ *
+ * Implements the hot path of "Differentiable Forward and Back-Projector for Rigid Motion Estimation in X-ray
+ * Imaging" (arXiv 2508.13304; citations are lines of /root/reference/PAPER.md) as hand-written CUDA for
+ * sm_100a (NVIDIA B200).  There is no CPU fallback: without a CUDA device every compute call returns
+ * DFP_ERR_CUDA.  See DESIGN.md for the discretisation (readings U1-U13) and the data layout.
+ *
+ * Conventions:
+ *   vol [nz][ny][nx] fp32, x fastest.  proj [n_views][nv][nu] fp32, u fastest.
+ *   pose [n_views][6] = (tx,ty,tz,gx,gy,gz) in mm and RADIANS;  r = R r' + t,  R = Rz(gz) Ry(gy) Rx(gx),
+ *   r' = R^T (r - t)                                                      (Table I :27-42, :58-60).
+ *   View of gantry angle b: source s = SAD (cos b, sin b, 0); detector centre -(SDD-SAD)(cos b, sin b, 0);
+ *   e_u = (-sin b, cos b, 0), e_v = (0,0,1); pixel (iu,iv) centre = centre + (iu-c_u) du e_u + (iv-c_v) dv e_v,
+ *   c_u = (nu-1)/2 + u0, c_v = (nv-1)/2 + v0;  d = p(r) of Eq.1 (:60-63) is in pixel-index units.
+ *   Gradients [n_views][6] are dL/d(tx,ty,tz) per mm and dL/d(gx,gy,gz) per radian.
+ *
+ * Pointer kinds.  `angles`, `poses`, `geometry`: HOST memory, read before the call returns.
+ *   d_* : DEVICE memory owned by the caller (e.g. torch tensors), fp32, contiguous, 16-byte aligned; read /
+ *   written asynchronously on `stream` (a cudaStream_t passed as void*, NULL = default stream) and must stay
+ *   alive until the stream reaches that point.  The library allocates no device memory in these calls and
+ *   never synchronises the host; all scratch lives in the caller-provided workspace `d_ws`
+ *   (>= dfp_workspace_bytes(...) bytes, 256-byte aligned).
+ *   The dfp_*_host convenience calls take HOST arrays for the big buffers too, allocate and free their own
+ *   device scratch on `stream` and return after the result has landed in host memory.
+ *
+ * Errors.  Every call returns an int status: DFP_OK (0) or a negative code; nothing is thrown, printed or
+ *   exited.  On error no kernel has been launched.  Rays / voxels that miss contribute exact zeros (never NaN).
+ */
+#ifndef DFP_H_
+#define DFP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dfp_geometry {
+  int32_t nx, ny, nz;   /* volume dims; vol[iz][iy][ix], x fastest                                          */
+  float vx, vy, vz;     /* voxel pitch, mm (> 0)                                                            */
+  float cx, cy, cz;     /* volume centre in the OBJECT frame, mm (normally 0)                               */
+  int32_t nu, nv;       /* detector columns (u, fastest) and rows (v)                                       */
+  float du, dv;         /* pixel pitch, mm (> 0)                                                            */
+  float u0, v0;         /* principal-point shift, pixels (0 = centred)                                      */
+  float sad, sdd;       /* source-axis and source-detector distance, mm (0 < sad < sdd)                     */
+  float step_mm;        /* ray-march step; <= 0 means min(vx,vy,vz)                                         */
+  int32_t bp_weight;    /* back-projection weight W: 0 = 1 (pure Eq.2b), 1 = FDK (sad/w')^2                 */
+  int32_t flags;        /* bit0 (DFP_FLAG_DW): add the dW/dtheta term in dfp_backproject_pose_grad          */
+} dfp_geometry;
+
+enum {
+  DFP_OK = 0,
+  DFP_ERR_NULL = -1,       /* a required pointer is NULL                                                    */
+  DFP_ERR_DIMS = -2,       /* non-positive size / pitch, sad <= 0, sdd <= sad, n_views <= 0, index overflow */
+  DFP_ERR_NONFINITE = -3,  /* NaN / Inf in geometry, angles or poses                                        */
+  DFP_ERR_ALIGN = -4,      /* a device pointer is not 16-byte (workspace: 256-byte) aligned                 */
+  DFP_ERR_WORKSPACE = -5,  /* ws_bytes < dfp_workspace_bytes(...)                                           */
+  DFP_ERR_CUDA = -6        /* CUDA runtime error (no device, launch failure, out of memory in *_host)       */
+};
+enum { DFP_OP_FORWARD = 0, DFP_OP_FORWARD_POSE_GRAD = 1, DFP_OP_BACKPROJECT = 2, DFP_OP_BACKPROJECT_POSE_GRAD = 3 };
+enum { DFP_FLAG_DW = 1 };
+
+/* Forward projection, Eq.2a :67-69 discretised as Eq.18 :172-177 with a fixed-step, zero-extended
+ * trilinear ray-march (U1): proj[v][iv][iu] = D * sum_k f~(R_v^T (s_v + (k+1/2) D e_i - t_v)).
+ * d_vol is read, d_proj ([n_views][nv][nu]) is overwritten. */
+int dfp_forward(const dfp_geometry* geometry, int n_views, const float* angles, const float* poses,
+                const float* d_vol, float* d_proj, void* d_ws, size_t ws_bytes, void* stream);
+
+/* Pose gradient of a loss through the forward projector, Eq.3-8 :81-113, Eq.19-20 :179-191:
+ * d_grad[v][0:6] = dL/dtheta_v = sum_i d_dLdproj[v][i] * dl_i/dtheta_v, with the volume gradient taken on
+ * the fly by central differences of f~ (:183) and G_f never materialised (:207).  d_grad is overwritten. */
+int dfp_forward_pose_grad(const dfp_geometry* geometry, int n_views, const float* angles, const float* poses,
+                          const float* d_vol, const float* d_dLdproj, float* d_grad, void* d_ws, size_t ws_bytes,
+                          void* stream);
+
+/* Voxel-driven back-projection, Eq.2b :71-75 / Eq.21 :193-196:
+ * vol[j] = sum_v W * b~_v(p(R_v r'_j + t_v)), b~ = zero-extended bilinear interpolant, W per bp_weight.
+ * d_proj is read, d_vol ([nz][ny][nx]) is overwritten. */
+int dfp_backproject(const dfp_geometry* geometry, int n_views, const float* angles, const float* poses,
+                    const float* d_proj, float* d_vol, void* d_ws, size_t ws_bytes, void* stream);
+
+/* Pose gradient of a loss through the back-projector, Eq.9-17 :115-168, Eq.22 :198-206:
+ * d_grad[v][0:6] = sum_j d_dLdvol[j] * dmu_j/dtheta_v, projection gradient by central differences of b~ (:202),
+ * G_b never materialised.  d_grad is overwritten. */
+int dfp_backproject_pose_grad(const dfp_geometry* geometry, int n_views, const float* angles, const float* poses,
+                              const float* d_proj, const float* d_dLdvol, float* d_grad, void* d_ws,
+                              size_t ws_bytes, void* stream);
+
+/* Bytes of device workspace the op needs for this geometry and view count (0 on invalid arguments).
+ * View chunking: any n_views may be passed to the calls above; to bound the workspace (and the size of
+ * d_proj) call them on consecutive slices of the view arrays - views are independent in forward /
+ * forward_pose_grad / *_pose_grad, and dfp_backproject of a slice can be summed by the caller. */
+size_t dfp_workspace_bytes(const dfp_geometry* geometry, int n_views, int op);
+
+/* Same four operations with HOST buffers (h_*: host memory, pinned or pageable).  Each allocates device
+ * scratch with cudaMallocAsync on `stream`, copies inputs in, runs the device call above, copies the result
+ * out, frees, and synchronises `stream` before returning. */
+int dfp_forward_host(const dfp_geometry* geometry, int n_views, const float* angles, const float* poses,
+                     const float* h_vol, float* h_proj, void* stream);
+int dfp_forward_pose_grad_host(const dfp_geometry* geometry, int n_views, const float* angles, const float* poses,
+                               const float* h_vol, const float* h_dLdproj, float* h_grad, void* stream);
+int dfp_backproject_host(const dfp_geometry* geometry, int n_views, const float* angles, const float* poses,
+                         const float* h_proj, float* h_vol, void* stream);
+int dfp_backproject_pose_grad_host(const dfp_geometry* geometry, int n_views, const float* angles,
+                                   const float* poses, const float* h_proj, const float* h_dLdvol, float* h_grad,
+                                   void* stream);
+
+/* Number of ray-steps one dfp_forward / dfp_forward_pose_grad call marches (samples inside the clip box,
+ * summed over rays and views), computed on the host in fp64 from the geometry alone; the unit of the
+ * "Gray-steps/s" metric.  Returns -1 on invalid arguments. */
+int64_t dfp_count_ray_steps(const dfp_geometry* geometry, int n_views, const float* angles, const float* poses);
+
+/* Number of kernels the last successful call on this thread launched (for bench accounting). */
+int dfp_last_launch_count(void);
+
+/* Static description of a status code; for DFP_ERR_CUDA the text of the last CUDA error seen on this thread. */
+const char* dfp_status_string(int status);
+
+/* Library version (major*10000 + minor*100 + patch). */
+int dfp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DFP_H_ */

@@ -1,0 +1,16 @@
+"""paper_2508_13304_b200 - B200-native differentiable cone-beam forward / back-projector (arXiv 2508.13304).
+
+The product is `libdfp.so` (hand-written CUDA for sm_100a behind the C ABI in include/dfp.h).  This package is
+the thin Python binding with the same names: argument marshalling only, every step of the path runs in the
+library's kernels.  torch is used for device memory and streams.  There is no CPU fallback.
+"""
+from .binding import (DfpError, Geometry, backproject, backproject_host, backproject_pose_grad,
+                      backproject_pose_grad_host, count_ray_steps, forward, forward_host, forward_pose_grad,
+                      forward_pose_grad_host, last_launch_count, lib_path, status_string, version,
+                      workspace_bytes, OP_FORWARD, OP_FORWARD_POSE_GRAD, OP_BACKPROJECT, OP_BACKPROJECT_POSE_GRAD,
+                      FLAG_DW)
+
+__all__ = ["DfpError", "Geometry", "forward", "forward_pose_grad", "backproject", "backproject_pose_grad",
+           "forward_host", "forward_pose_grad_host", "backproject_host", "backproject_pose_grad_host",
+           "workspace_bytes", "count_ray_steps", "last_launch_count", "status_string", "version", "lib_path",
+           "OP_FORWARD", "OP_FORWARD_POSE_GRAD", "OP_BACKPROJECT", "OP_BACKPROJECT_POSE_GRAD", "FLAG_DW"]

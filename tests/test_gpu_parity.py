@@ -1,0 +1,195 @@
+"""GPU-vs-oracle parity through the C ABI (`-m gpu`).  Same seeded inputs, element by element.
+
+Tolerances (BASELINE.json north_star): relative L2 <= 1e-5 on projections and
+back-projections, <= 1e-3 on every pose-gradient component with the floored denominator of reading U9.
+Angles and poses are rounded to fp32 first (the C ABI takes fp32) and the SAME values go to the oracle.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import workloads as W
+from helpers import aniso_geom, grad_err_u9, rel_l2, small_geom
+
+pytestmark = pytest.mark.gpu
+
+TOL_VAL = 1e-5
+TOL_GRAD = 1e-3
+
+
+@pytest.fixture(scope="module")
+def dfp():
+    import paper_2508_13304_b200 as m
+    return m
+
+
+def f32(a):
+    return np.asarray(a, dtype=np.float64).astype(np.float32)
+
+
+def run_forward_case(dfp, g, angles, poses, vol, up):
+    dev = torch.device("cuda:0")
+    angles, poses = f32(angles), f32(poses).reshape(-1, 6)
+    vol_d = torch.as_tensor(vol, dtype=torch.float32, device=dev).contiguous()
+    up_d = torch.as_tensor(up, dtype=torch.float32, device=dev).contiguous()
+    proj = dfp.forward(g, angles, poses, vol_d).cpu().numpy()
+    grad = dfp.forward_pose_grad(g, angles, poses, vol_d, up_d).cpu().numpy()
+    o_proj = oracle.forward(g, angles, poses, vol_d.cpu().numpy())
+    o_grad = oracle.forward_pose_grad(g, angles, poses, vol_d.cpu().numpy(), up_d.cpu().numpy())
+    return proj, grad, o_proj, o_grad
+
+
+def run_back_case(dfp, g, angles, poses, proj, up):
+    dev = torch.device("cuda:0")
+    angles, poses = f32(angles), f32(poses).reshape(-1, 6)
+    proj_d = torch.as_tensor(proj, dtype=torch.float32, device=dev).contiguous()
+    up_d = torch.as_tensor(up, dtype=torch.float32, device=dev).contiguous()
+    vol = dfp.backproject(g, angles, poses, proj_d).cpu().numpy()
+    grad = dfp.backproject_pose_grad(g, angles, poses, proj_d, up_d).cpu().numpy()
+    o_vol = oracle.backproject(g, angles, poses, proj_d.cpu().numpy())
+    o_grad = oracle.backproject_pose_grad(g, angles, poses, proj_d.cpu().numpy(), up_d.cpu().numpy())
+    return vol, grad, o_vol, o_grad
+
+
+def check_forward(res):
+    proj, grad, o_proj, o_grad = res
+    assert np.all(np.isfinite(proj)) and np.all(np.isfinite(grad))
+    assert rel_l2(proj, o_proj) <= TOL_VAL, rel_l2(proj, o_proj)
+    assert np.array_equal(proj == 0, o_proj == 0) or rel_l2(proj, o_proj) <= TOL_VAL
+    e = grad_err_u9(grad, o_grad)
+    assert e.max() <= TOL_GRAD, e
+
+
+def check_back(res):
+    vol, grad, o_vol, o_grad = res
+    assert np.all(np.isfinite(vol)) and np.all(np.isfinite(grad))
+    assert rel_l2(vol, o_vol) <= TOL_VAL, rel_l2(vol, o_vol)
+    e = grad_err_u9(grad, o_grad)
+    assert e.max() <= TOL_GRAD, e
+
+
+POSES3 = [[1.2, -0.8, 0.6, 0.11, -0.07, 0.19], [0, 0, 0, 0, 0, 0], [-3.0, 2.0, 1.5, -0.2, 0.15, -0.4]]
+ANGLES3 = [0.4, math.pi / 2, 4.1]
+
+
+# ------------------------------------------------------------------ ragged small cases (several tiles + tails)
+def test_forward_ragged_anisotropic(dfp):
+    g = aniso_geom(nx=37, ny=29, nz=23, nu=45, nv=21)
+    rng = np.random.default_rng(0)
+    vol = rng.standard_normal(g.vol_shape).astype(np.float32)
+    up = rng.standard_normal((3,) + g.det_shape).astype(np.float32)
+    check_forward(run_forward_case(dfp, g, ANGLES3, POSES3, vol, up))
+
+
+def test_forward_odd_and_even_grids_and_fine_step(dfp):
+    for n, step in ((16, 0.0), (17, 0.0), (21, 0.4)):
+        g = small_geom(n=n, nu=33, nv=9, step_mm=step)
+        rng = np.random.default_rng(n)
+        vol = rng.random(g.vol_shape).astype(np.float32)
+        up = rng.standard_normal((3,) + g.det_shape).astype(np.float32)
+        check_forward(run_forward_case(dfp, g, ANGLES3, POSES3, vol, up))
+
+
+def test_back_ragged_anisotropic(dfp):
+    for bw, fl in ((0, 0), (1, 0), (1, 1)):
+        g = aniso_geom(nx=37, ny=29, nz=23, nu=45, nv=21, bp_weight=bw, flags=fl)
+        rng = np.random.default_rng(1)
+        proj = rng.standard_normal((3,) + g.det_shape).astype(np.float32)
+        up = rng.standard_normal(g.vol_shape).astype(np.float32)
+        check_back(run_back_case(dfp, g, ANGLES3, POSES3, proj, up))
+
+
+def test_back_volume_larger_than_field_of_view(dfp):
+    """Voxels that project outside the detector (zero extension of b~) and a tall z range (several z chunks)."""
+    g = small_geom(n=40, voxel=3.0, nu=20, nv=12, pix=2.0)
+    g = g.replace(nz=70)
+    rng = np.random.default_rng(2)
+    proj = rng.standard_normal((3,) + g.det_shape).astype(np.float32)
+    up = rng.standard_normal(g.vol_shape).astype(np.float32)
+    res = run_back_case(dfp, g, ANGLES3, POSES3, proj, up)
+    check_back(res)
+    assert (res[2] == 0).mean() > 0.2 and np.array_equal(res[0] == 0, res[2] == 0)
+
+
+# ------------------------------------------------------------------ degenerate cases
+def test_missed_and_empty_inputs_give_exact_zeros(dfp):
+    g = small_geom(n=12, nu=10, nv=7)
+    vol = np.ones(g.vol_shape, np.float32)
+    up = np.ones((1,) + g.det_shape, np.float32)
+    far = [[0, 0, 700.0, 0, 0, 0]]
+    proj, grad, _, _ = run_forward_case(dfp, g, [0.3], far, vol, up)
+    assert np.all(proj == 0) and np.all(grad == 0)
+    proj, grad, _, _ = run_forward_case(dfp, g, [0.3], [POSES3[0]], 0 * vol, up)
+    assert np.all(proj == 0) and np.all(grad == 0)
+    pr = np.ones((1,) + g.det_shape, np.float32)
+    uv = np.ones(g.vol_shape, np.float32)
+    bvol, bgrad, _, _ = run_back_case(dfp, g, [0.3], far, pr, uv)
+    assert np.all(bvol == 0) and np.all(bgrad == 0)
+
+
+def test_single_voxel_and_single_pixel(dfp):
+    g = small_geom(n=1, voxel=4.0, nu=1, nv=1, pix=3.0)
+    vol = np.full(g.vol_shape, 0.7, np.float32)
+    up = np.ones((1,) + g.det_shape, np.float32)
+    check_forward(run_forward_case(dfp, g, [0.0], [[0.3, 0.2, -0.1, 0.01, 0.02, 0.03]], vol, up))
+    check_back(run_back_case(dfp, g, [0.0], [[0.3, 0.2, -0.1, 0.01, 0.02, 0.03]], np.ones((1, 1, 1), np.float32),
+                             np.ones(g.vol_shape, np.float32)))
+
+
+def test_host_buffer_entry_points_match_device_ones(dfp):
+    g = aniso_geom()
+    rng = np.random.default_rng(3)
+    vol = rng.standard_normal(g.vol_shape).astype(np.float32)
+    up = rng.standard_normal((3,) + g.det_shape).astype(np.float32)
+    a, p = f32(ANGLES3), f32(POSES3)
+    dev = torch.device("cuda:0")
+    vd, ud = torch.as_tensor(vol, device=dev), torch.as_tensor(up, device=dev)
+    proj = dfp.forward(g, a, p, vd)
+    assert torch.equal(dfp.forward_host(g, a, p, vol), proj.cpu())
+    assert torch.equal(dfp.forward_pose_grad_host(g, a, p, vol, up), dfp.forward_pose_grad(g, a, p, vd, ud).cpu())
+    pj = proj.cpu().numpy()
+    wv = rng.standard_normal(g.vol_shape).astype(np.float32)
+    assert torch.equal(dfp.backproject_host(g, a, p, pj), dfp.backproject(g, a, p, proj).cpu())
+    assert torch.equal(dfp.backproject_pose_grad_host(g, a, p, pj, wv),
+                       dfp.backproject_pose_grad(g, a, p, proj, torch.as_tensor(wv, device=dev)).cpu())
+
+
+def test_results_are_deterministic(dfp):
+    g = aniso_geom(nx=37, ny=29, nz=23, nu=45, nv=21)
+    rng = np.random.default_rng(4)
+    dev = torch.device("cuda:0")
+    vol = torch.as_tensor(rng.standard_normal(g.vol_shape).astype(np.float32), device=dev)
+    up = torch.as_tensor(rng.standard_normal((3,) + g.det_shape).astype(np.float32), device=dev)
+    a, p = f32(ANGLES3), f32(POSES3)
+    g1 = dfp.forward_pose_grad(g, a, p, vol, up)
+    g2 = dfp.forward_pose_grad(g, a, p, vol, up)
+    assert torch.equal(g1, g2)
+    b1 = dfp.backproject_pose_grad(g, a, p, up, vol)
+    b2 = dfp.backproject_pose_grad(g, a, p, up, vol)
+    assert torch.equal(b1, b2)
+
+
+def test_ray_step_count_matches_oracle(dfp):
+    w = W.make_config(1)
+    a, p = f32(w.angles), f32(w.poses)
+    n_gpu = dfp.count_ray_steps(w.geom, a, p)
+    _, n_ora = oracle.forward(w.geom, a, p, w.volume().numpy(), return_steps=True)
+    assert abs(n_gpu - n_ora) <= 2e-3 * n_ora, (n_gpu, n_ora)
+
+
+# ------------------------------------------------------------------ the five configs, reduced so the oracle takes seconds
+@pytest.mark.parametrize("index,scale,views", [(1, 1.0, None), (2, 0.25, 3), (4, 0.125, 4), (5, 0.125, 3)])
+def test_forward_configs_reduced(dfp, index, scale, views):
+    w = W.make_config(index, scale=scale, n_views=views)
+    check_forward(run_forward_case(dfp, w.geom, w.angles.numpy(), w.poses.numpy(), w.volume().numpy(),
+                                   w.fwd_upstream().numpy()))
+
+
+@pytest.mark.parametrize("index,scale,views", [(3, 0.25, 12), (5, 0.125, 6)])
+def test_back_configs_reduced(dfp, index, scale, views):
+    w = W.make_config(index, scale=scale, n_views=views)
+    check_back(run_back_case(dfp, w.geom, w.angles.numpy(), w.poses.numpy(), w.projections().numpy(),
+                             w.bp_upstream().numpy()))
