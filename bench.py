@@ -1,0 +1,359 @@
+#!/usr/bin/env python
+"""bench.py - throughput of the dfp hot path on B200, one JSON line (contract: see the task statement / DESIGN.md).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 2]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N --steps K --warmup W
+
+A STEP is one pass of the whole hot path over one batch of synthetic input: dfp_forward, dfp_forward_pose_grad,
+dfp_backproject and dfp_backproject_pose_grad on the workload (default: BASELINE.json configs[1], the 2D/3D
+registration batch - 256^3 volume, 64 pose candidates, 512x512 detector).  `value` is the headline metric
+"fwd+pose-grad Gray-steps/s" = 2 * ray_steps / (t_forward + t_forward_pose_grad), with inputs resident in
+HBM; the back-projection half of the step is reported in `extra` as Gvoxel-views/s.  N > 1: every rank runs
+its own copy of the batch (independent problems, no data-path collective) -> weak scaling.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as W  # noqa: E402
+
+METRIC = "fwd+pose-grad Gray-steps/s"
+UNIT = "Gray-steps/s"
+
+# Algorithmic work per unit: thread-level arithmetic + load operations the method itself
+# needs per ray-step / voxel-view, FMA counted as one op.  ALU peak = SMs x 128 lanes x clock.
+OPS_PER_UNIT = {"fwd_project": 38, "fwd_grad": 113, "bp": 30, "bp_grad": 78}
+N_SM = 148
+LANES_PER_SM = 128
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return d, "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(w, rows=32):
+    """A bounded sample of the workload for the CPU oracle: ONE view, the central `rows` detector rows
+    (v0 shifts the principal point so that the rays are exactly rays of the full detector)."""
+    g = w.geom
+    rows = min(rows, g.nv)
+    r0 = (g.nv - rows) // 2
+    # c_v' = (rows-1)/2 + v0' must equal c_v - r0
+    v0 = (g.nv - 1) / 2.0 + g.v0 - r0 - (rows - 1) / 2.0
+    gs = g.replace(nv=rows, v0=v0)
+    return gs, r0, rows
+
+
+def time_oracle(w, vol_cpu, up_cpu_view0, steps=1, warmup=0, rows=128):
+    """Oracle forward + forward_pose_grad on the sample; returns (Gray-steps/s, seconds per step, cores, text)."""
+    import oracle
+    gs, r0, rows = oracle_sample(w, rows)
+    a = w.angles[:1].float().numpy()
+    p = w.poses[:1].float().numpy()
+    up = np.ascontiguousarray(up_cpu_view0[None, r0:r0 + rows, :])
+    times, n_steps = [], 0
+    for i in range(warmup + steps):
+        t0 = time.perf_counter()
+        _, n_steps = oracle.forward(gs, a, p, vol_cpu, return_steps=True)
+        oracle.forward_pose_grad(gs, a, p, vol_cpu, up)
+        dt = time.perf_counter() - t0
+        if i >= warmup:
+            times.append(dt)
+    sec = float(np.mean(times))
+    val = 2.0 * n_steps / sec / 1e9
+    txt = (f"view 0 of {w.n_views}, central {rows} of {g_nv(w)} detector rows x {w.geom.nu} columns "
+           f"({n_steps} ray-steps per pass), oracle.forward + oracle.forward_pose_grad, fp64, OpenMP")
+    return val, sec, oracle.num_threads(), txt
+
+
+def g_nv(w):
+    return w.geom.nv
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the fp64 CPU oracle, as it stands, on the host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    w = W.make_config(args.config)
+    vol = w.volume("cpu").numpy()
+    up0 = w.fwd_upstream("cpu", views=[0])[0].numpy()
+    val, sec, cores, txt = time_oracle(w, vol, up0, steps=args.steps, warmup=args.warmup)
+    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": f"{w.name} (BASELINE.json configs[{args.config - 1}])", "sample": txt},
+           "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": txt},
+           "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index 1..5 (default 2)")
+    ap.add_argument("--views", type=int, default=None, help="override the view count (debugging)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import paper_2508_13304_b200 as dfp   # fails loudly if libdfp.so is missing: no CPU fallback
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---------------------------------------------------------------- workload, resident in HBM
+    w = W.make_config(args.config, n_views=args.views)
+    g = w.geom
+    V = w.n_views
+    angles = w.angles.float().numpy()
+    poses = w.poses.float().numpy()
+    vol = w.volume(dev)
+    up = w.fwd_upstream(dev)
+    bp_up = W.normal_field(w.seed * 4096 + 5, g.nx * g.ny * g.nz, dev).reshape(g.vol_shape).contiguous()
+    proj = torch.empty((V, g.nv, g.nu), dtype=torch.float32, device=dev)
+    grad = torch.empty((V, 6), dtype=torch.float32, device=dev)
+    bvol = torch.empty(g.vol_shape, dtype=torch.float32, device=dev)
+    bgrad = torch.empty((V, 6), dtype=torch.float32, device=dev)
+    ws = torch.empty(max(dfp.workspace_bytes(g, V, op) for op in range(4)), dtype=torch.uint8, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)        # > 126 MB L2
+    ray_steps = dfp.count_ray_steps(g, angles, poses)
+    voxel_views = g.nx * g.ny * g.nz * V
+    dfp.set_kernel_timing(True)
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    kern_ms = {k: [] for k in OPS_PER_UNIT}
+    launches = [0]
+
+    def step(record=False):
+        e = [ev() for _ in range(5)]
+        e[0].record()
+        dfp.forward(g, angles, poses, vol, out=proj, ws=ws)
+        launches[0] += dfp.last_launch_count()
+        k0 = dfp.last_kernel_ms() if record else None
+        e[1].record()
+        dfp.forward_pose_grad(g, angles, poses, vol, up, out=grad, ws=ws)
+        launches[0] += dfp.last_launch_count()
+        k1 = dfp.last_kernel_ms() if record else None
+        e[2].record()
+        dfp.backproject(g, angles, poses, proj, out=bvol, ws=ws)
+        launches[0] += dfp.last_launch_count()
+        k2 = dfp.last_kernel_ms() if record else None
+        e[3].record()
+        dfp.backproject_pose_grad(g, angles, poses, proj, bp_up, out=bgrad, ws=ws)
+        launches[0] += dfp.last_launch_count()
+        k3 = dfp.last_kernel_ms() if record else None
+        e[4].record()
+        if record:
+            for k, v in zip(OPS_PER_UNIT, (k0, k1, k2, k3)):
+                kern_ms[k].append(v)
+        return e
+
+    for _ in range(args.warmup):
+        step()
+        flush.zero_()
+    barrier()
+    launches[0] = 0
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    evs = []
+    for _ in range(args.steps):
+        flush.zero_()                      # L2 flush between timed iterations (outside the per-step events)
+        evs.append(step(record=True))
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    seg = np.array([[a.elapsed_time(b) for a, b in zip(e[:-1], e[1:])] for e in evs])   # ms, [K,4]
+    t = seg.sum(axis=0) / 1e3                                                            # s per call, over K steps
+    tt = torch.tensor([t[0] + t[1], t[2] + t[3], t.sum()], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    t_fg, t_bp, t_all = [float(x) for x in tt.cpu()]
+    K = args.steps
+    value = 2.0 * ray_steps * K * world / t_fg / 1e9
+    bp_value = 2.0 * voxel_views * K * world / t_bp / 1e9
+    n_launch = launches[0]
+
+    # ---------------------------------------------------------------- end to end through the host-buffer C ABI
+    e2e = None
+    if not args.no_e2e:
+        pin = lambda t_: t_.cpu().pin_memory()
+        h_vol, h_up, h_bpup = pin(vol), pin(up), pin(bp_up)
+        h_proj = torch.empty((V, g.nv, g.nu), dtype=torch.float32).pin_memory()
+        h_grad = torch.empty((V, 6), dtype=torch.float32).pin_memory()
+        h_bvol = torch.empty(g.vol_shape, dtype=torch.float32).pin_memory()
+        h_bgrad = torch.empty((V, 6), dtype=torch.float32).pin_memory()
+
+        def e2e_step():
+            t0 = time.perf_counter()
+            dfp.forward_host(g, angles, poses, h_vol, out=h_proj)
+            dfp.forward_pose_grad_host(g, angles, poses, h_vol, h_up, out=h_grad)
+            t1 = time.perf_counter()
+            dfp.backproject_host(g, angles, poses, h_proj, out=h_bvol)
+            dfp.backproject_pose_grad_host(g, angles, poses, h_proj, h_bpup, out=h_bgrad)
+            return t1 - t0, time.perf_counter() - t1
+
+        for _ in range(2):
+            e2e_step()
+        barrier()
+        tf = tb = 0.0
+        for _ in range(K):
+            a_, b_ = e2e_step()
+            tf += a_
+            tb += b_
+        barrier()
+        te = torch.tensor([tf, tb], dtype=torch.float64, device=dev)
+        if dist is not None:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        tf, tb = [float(x) for x in te.cpu()]
+        nb = lambda t_: t_.numel() * t_.element_size()
+        e2e = {"value": 2.0 * ray_steps * K * world / tf / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": 2 * nb(h_vol) + nb(h_up) + 2 * nb(h_proj) + nb(h_bpup),
+               "d2h_bytes_per_step": nb(h_proj) + nb(h_grad) + nb(h_bvol) + nb(h_bgrad),
+               "backproject_gvoxel_views_per_s": 2.0 * voxel_views * K * world / tb / 1e9,
+               "api": "dfp_*_host (pinned host buffers; cudaMallocAsync + H2D + kernels + D2H + sync per call)"}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---------------------------------------------------------------- roofline of the dominant kernel
+    pk, pk_kind = peaks()
+    mean_ms = {k: float(np.mean(v)) for k, v in kern_ms.items()}
+    dom = max(mean_ms, key=mean_ms.get)
+    units = {"fwd_project": ray_steps, "fwd_grad": ray_steps, "bp": voxel_views, "bp_grad": voxel_views}
+    alu_peak = N_SM * LANES_PER_SM * pk.get("sm_max_mhz", 1965.0) * 1e6 / 1e12          # Tera lane-ops/s
+    achieved = OPS_PER_UNIT[dom] * units[dom] / (mean_ms[dom] * 1e-3) / 1e12
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        traffic = json.load(open(tp)).get(f"C{args.config}", {}).get(dom)
+    roofline = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": alu_peak, "unit": "Tlane-op/s",
+                "frac": achieved / alu_peak, "traffic": traffic,
+                "peak_source": f"148 SMs x 128 fp32 lanes x sm_max_mhz ({pk_kind} MEASURED_PEAKS.json clock)",
+                "ops_per_unit": OPS_PER_UNIT[dom], "units_per_launch": units[dom], "kernel_ms": mean_ms,
+                "kernel_share_of_step": {k: v * K / 1e3 / t_all for k, v in mean_ms.items()},
+                "hbm_compulsory_frac": None}
+    # compulsory HBM bytes of the dominant kernel vs the measured copy peak (expected to be small)
+    comp = {"fwd_project": vol.numel() * 8 + proj.numel() * 4, "fwd_grad": vol.numel() * 8 + up.numel() * 4,
+            "bp": proj.numel() * 16 + bvol.numel() * 4, "bp_grad": proj.numel() * 16 + bvol.numel() * 4}[dom]
+    roofline["hbm_compulsory_frac"] = comp / (mean_ms[dom] * 1e-3) / 1e9 / pk["hbm_gbs"]
+
+    # ---------------------------------------------------------------- CPU baseline: the oracle on the host cores
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        val, sec, cores, txt = time_oracle(w, vol.cpu().numpy(), up[0].cpu().numpy(), rows=g.nv)
+        cpu = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": txt, "seconds": sec}
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+           "ms_per_step": t_all / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f32", "data": "synthetic",
+           "config": {"workload": f"{w.name} (BASELINE.json configs[{args.config - 1}]): {g.nx}^3 volume, {V} views of "
+                                  f"{g.nu}x{g.nv}, all four calls per step", "ray_steps_per_pass": ray_steps,
+                      "voxel_views_per_pass": voxel_views, "l2": "256 MiB flush write between timed steps",
+                      "parallelism": f"replicated batch x{world}, no collective"},
+           "extra": {"backproject+grad_gvoxel_views_per_s": bp_value,
+                     "forward_gray_steps_per_s": ray_steps * K * world / float(seg[:, 0].sum() / 1e3) / 1e9,
+                     "forward_pose_grad_gray_steps_per_s": ray_steps * K * world / float(seg[:, 1].sum() / 1e3) / 1e9,
+                     "backproject_gvoxel_views_per_s": voxel_views * K * world / float(seg[:, 2].sum() / 1e3) / 1e9,
+                     "backproject_pose_grad_gvoxel_views_per_s":
+                         voxel_views * K * world / float(seg[:, 3].sum() / 1e3) / 1e9,
+                     "ms_per_call": {"forward": float(seg[:, 0].mean()), "forward_pose_grad": float(seg[:, 1].mean()),
+                                     "backproject": float(seg[:, 2].mean()),
+                                     "backproject_pose_grad": float(seg[:, 3].mean())}},
+           "clocks": clocks, "e2e": e2e, "gpu_launches": n_launch, "roofline": roofline, "cpu_baseline": cpu}
+    print(json.dumps(out), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

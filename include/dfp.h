@@ -111,6 +111,14 @@ int dfp_backproject_pose_grad_host(const dfp_geometry* geometry, int n_views, co
  * "Gray-steps/s" metric.  Returns -1 on invalid arguments. */
 int64_t dfp_count_ray_steps(const dfp_geometry* geometry, int n_views, const float* angles, const float* poses);
 
+/* Kernel timing for roofline accounting.  dfp_set_kernel_timing(1) makes every later device-pointer call on
+ * this thread bracket its DOMINANT kernel (fwd_project / fwd_grad / bp / bp_grad; not the packing or the
+ * contraction kernels) with two CUDA events recorded on `stream`; dfp_last_kernel_ms() waits for the second
+ * event and returns the elapsed milliseconds of that one launch (-1 if timing is off or nothing ran).
+ * Off by default; costs two event records per call when on. */
+int dfp_set_kernel_timing(int enable);
+float dfp_last_kernel_ms(void);
+
 /* Number of kernels the last successful call on this thread launched (for bench accounting). */
 int dfp_last_launch_count(void);
 

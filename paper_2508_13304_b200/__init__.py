@@ -6,11 +6,11 @@ library's kernels.  torch is used for device memory and streams.  There is no CP
 """
 from .binding import (DfpError, Geometry, backproject, backproject_host, backproject_pose_grad,
                       backproject_pose_grad_host, count_ray_steps, forward, forward_host, forward_pose_grad,
-                      forward_pose_grad_host, last_launch_count, lib_path, status_string, version,
+                      forward_pose_grad_host, last_kernel_ms, last_launch_count, set_kernel_timing, lib_path, status_string, version,
                       workspace_bytes, OP_FORWARD, OP_FORWARD_POSE_GRAD, OP_BACKPROJECT, OP_BACKPROJECT_POSE_GRAD,
                       FLAG_DW)
 
 __all__ = ["DfpError", "Geometry", "forward", "forward_pose_grad", "backproject", "backproject_pose_grad",
            "forward_host", "forward_pose_grad_host", "backproject_host", "backproject_pose_grad_host",
-           "workspace_bytes", "count_ray_steps", "last_launch_count", "status_string", "version", "lib_path",
+           "workspace_bytes", "count_ray_steps", "last_launch_count", "set_kernel_timing", "last_kernel_ms", "status_string", "version", "lib_path",
            "OP_FORWARD", "OP_FORWARD_POSE_GRAD", "OP_BACKPROJECT", "OP_BACKPROJECT_POSE_GRAD", "FLAG_DW"]

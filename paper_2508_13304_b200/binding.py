@@ -43,13 +43,16 @@ class Geometry(ctypes.Structure):
 
 
 def _load():
-    if not os.path.exists(_LIB_PATH):
+    # (re)build when the library is missing or older than its sources and nvcc is here; on a box without nvcc
+    # a prebuilt in-tree library is used as is.  Never fall back to anything else.
+    from .build import build, stale
+    import shutil
+    if stale() and (shutil.which("nvcc") or os.path.exists("/usr/local/cuda/bin/nvcc") or not os.path.exists(_LIB_PATH)):
         try:
-            from .build import build
             build()
-        except Exception as e:   # no nvcc here and no prebuilt library: fail loudly, never fall back
-            raise ImportError(f"libdfp.so is missing and could not be built ({e}); the dfp CUDA library is "
-                              "required - there is no CPU fallback") from e
+        except Exception as e:
+            raise ImportError(f"libdfp.so is missing or stale and could not be built ({e}); the dfp CUDA library "
+                              "is required - there is no CPU fallback") from e
     lib = ctypes.CDLL(_LIB_PATH)
     vp, cp, sz, ci = ctypes.c_void_p, ctypes.c_char_p, ctypes.c_size_t, ctypes.c_int
     gp = ctypes.POINTER(Geometry)
@@ -71,6 +74,10 @@ def _load():
     lib.dfp_workspace_bytes.restype = sz
     lib.dfp_count_ray_steps.argtypes = [gp, ci, vp, vp]
     lib.dfp_count_ray_steps.restype = ctypes.c_int64
+    lib.dfp_set_kernel_timing.argtypes = [ci]
+    lib.dfp_set_kernel_timing.restype = ci
+    lib.dfp_last_kernel_ms.argtypes = []
+    lib.dfp_last_kernel_ms.restype = ctypes.c_float
     lib.dfp_status_string.argtypes = [ci]
     lib.dfp_status_string.restype = cp
     return lib
@@ -93,6 +100,15 @@ def status_string(status: int) -> str:
 
 def last_launch_count() -> int:
     return int(_lib.dfp_last_launch_count())
+
+
+def set_kernel_timing(enable: bool) -> None:
+    _lib.dfp_set_kernel_timing(1 if enable else 0)
+
+
+def last_kernel_ms() -> float:
+    """Milliseconds of the dominant kernel of the last device-pointer call (waits for it); -1 if timing is off."""
+    return float(_lib.dfp_last_kernel_ms())
 
 
 def _check(status):

