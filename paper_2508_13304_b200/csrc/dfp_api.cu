@@ -90,7 +90,7 @@ FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad) {
   size_t o = 0;
   w.off_views = o; o += align_up(sizeof(FwdView) * (size_t)V);
   w.off_con = o;   o += grad ? align_up(sizeof(FwdContract) * (size_t)V) : 0;
-  w.off_pvol = o;  o += align_up(sizeof(float2) * (size_t)L.px * L.py * L.pz);
+  w.off_pvol = o;  o += align_up(sizeof(float4) * (size_t)L.px * L.py * L.pz);
   w.off_part = o;  o += grad ? align_up(sizeof(float) * 6 * (size_t)V * w.gx * w.gy) : 0;
   w.total = o;
   return w;
@@ -149,7 +149,7 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
   char* base = static_cast<char*>(d_ws);
   FwdView* dv = reinterpret_cast<FwdView*>(base + w.off_views);
   FwdContract* dc = reinterpret_cast<FwdContract*>(base + w.off_con);
-  float2* pvol = reinterpret_cast<float2*>(base + w.off_pvol);
+  float4* pvol = reinterpret_cast<float4*>(base + w.off_pvol);
   float* part = reinterpret_cast<float*>(base + w.off_part);
   g_launches = 0;
   DFP_CUDA(cudaMemcpyAsync(dv, hv.data(), sizeof(FwdView) * V, cudaMemcpyHostToDevice, s), "view upload");

@@ -38,17 +38,26 @@ __device__ __forceinline__ float4 ldg4(const float4* p) { return __ldg(p); }
 
 // ------------------------------------------------------------------------------------------------ packing
 __global__ void __launch_bounds__(256) pack_volume_kernel(VolLayout L, const float* __restrict__ vol,
-                                                          float2* __restrict__ pvol) {
+                                                          float4* __restrict__ pvol) {
   const size_t n = (size_t)L.px * L.py * L.pz;
+  const unsigned nbxy = (unsigned)L.nbx * L.nby;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-    const int x = (int)(i % L.px) - kPad;
-    const int y = (int)((i / L.px) % L.py) - kPad;
-    const int z = (int)(i / ((size_t)L.px * L.py)) - kPad;
-    float2 c = make_float2(0.f, 0.f);
-    if (y >= 0 && y < L.ny && z >= 0 && z < L.nz) {
-      const float* row = vol + ((size_t)z * L.ny + y) * L.nx;
-      if (x >= 0 && x < L.nx) c.x = __ldg(row + x);
-      if (x + 1 >= 0 && x + 1 < L.nx) c.y = __ldg(row + x + 1);
+    // output order = memory order: brick-major, 8 cells per brick (x fastest, then y, then z)
+    const unsigned within = (unsigned)(i & 7), brick = (unsigned)(i >> 3);
+    const unsigned bz = brick / nbxy, rem = brick - bz * nbxy;
+    const unsigned by = rem / L.nbx, bx = rem - by * L.nbx;
+    const int x = (int)(2 * bx + (within & 1)) - L.lx;
+    const int y = (int)(2 * by + ((within >> 1) & 1)) - L.ly;
+    const int z = (int)(2 * bz + (within >> 2)) - L.lz;
+    float4 c = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (z >= 0 && z < L.nz) {
+      const float* sl = vol + (size_t)z * L.ny * L.nx;
+      const bool x0 = x >= 0 && x < L.nx, x1 = x + 1 >= 0 && x + 1 < L.nx;
+      const bool y0 = y >= 0 && y < L.ny, y1 = y + 1 >= 0 && y + 1 < L.ny;
+      if (x0 && y0) c.x = __ldg(sl + (size_t)y * L.nx + x);
+      if (x1 && y0) c.y = __ldg(sl + (size_t)y * L.nx + x + 1);
+      if (x0 && y1) c.z = __ldg(sl + (size_t)(y + 1) * L.nx + x);
+      if (x1 && y1) c.w = __ldg(sl + (size_t)(y + 1) * L.nx + x + 1);
     }
     pvol[i] = c;
   }
@@ -141,30 +150,32 @@ __device__ __forceinline__ void fwd_pixel(int& iu, int& iv) {
 
 // ------------------------------------------------------------------------------------------------ a3 forward
 // l_i = D sum_k f~(r'_k)  (Eq.18 :172-177 with a^ij = D * trilinear weight; U1).
+// Cell index of the sample's base voxel from the magic-rounded coordinates (VolLayout): 3 LOP + 6 IMAD/LEA.
+__device__ __forceinline__ unsigned brick_index(const VolLayout& L, float tx, float ty, float tz) {
+  const unsigned X = (unsigned)__float_as_int(tx), Y = (unsigned)__float_as_int(ty), Z = (unsigned)__float_as_int(tz);
+  return X + 3u * (X & ~1u) + 2u * Y + L.by * (Y & ~1u) + 4u * Z + L.bz * (Z & ~1u) + L.c0;
+}
+
 __global__ void __launch_bounds__(kFwdThreads) fwd_project_kernel(FwdGeom G, const FwdView* __restrict__ views,
-                                                                  const float2* __restrict__ pvol,
+                                                                  const float4* __restrict__ pvol,
                                                                   float* __restrict__ proj) {
   int iu, iv;
   fwd_pixel(iu, iv);
   const int view = blockIdx.z;
   if (iu >= G.nu || iv >= G.nv) return;
   const Ray r = setup_ray(G, views[view], iu, iv, nullptr, nullptr);
-  const unsigned S1 = G.L.px, S2 = (unsigned)G.L.px * G.L.py;
-  // cell index = (iz+hz+kPad)*S2 + (iy+hy+kPad)*S1 + (ix+hx+kPad), i* = float bits of t* minus kMagicBits
-  const unsigned C0 = (unsigned)(G.L.hz + kPad) * S2 + (unsigned)(G.L.hy + kPad) * S1 + (unsigned)(G.L.hx + kPad) -
-                      (unsigned)kMagicBits * (S2 + S1 + 1u);
+  const unsigned dz1 = 2u * G.L.bz + 4u;     // FZ(Z+1) - FZ(Z) for odd Z (4 for even Z)
   float sum = 0.f;
   float kf = (float)r.k0;
   for (int i = 0; i < r.n; ++i) {
     const float qx = fmaf(kf, r.dpx, r.pmx), qy = fmaf(kf, r.dpy, r.pmy), qz = fmaf(kf, r.dpz, r.pmz);
     const float tx = qx + kMagic, ty = qy + kMagic, tz = qz + kMagic;
     const float ax = (qx - (tx - kMagic)) + 0.5f, ay = (qy - (ty - kMagic)) + 0.5f, az = (qz - (tz - kMagic)) + 0.5f;
-    const unsigned idx = (unsigned)__float_as_int(tz) * S2 + (unsigned)__float_as_int(ty) * S1 +
-                         (unsigned)__float_as_int(tx) + C0;
-    const float2* c = pvol + idx;
-    const float2 c00 = ldg2(c), c10 = ldg2(c + S1), c01 = ldg2(c + S2), c11 = ldg2(c + S2 + S1);
-    const float r00 = lerp(ax, c00.x, c00.y), r10 = lerp(ax, c10.x, c10.y);
-    const float r01 = lerp(ax, c01.x, c01.y), r11 = lerp(ax, c11.x, c11.y);
+    const unsigned idx = brick_index(G.L, tx, ty, tz);
+    const unsigned up = (__float_as_int(tz) & 1) ? dz1 : 4u;
+    const float4 c0 = ldg4(pvol + idx), c1 = ldg4(pvol + (idx + up));
+    const float r00 = lerp(ax, c0.x, c0.y), r10 = lerp(ax, c0.z, c0.w);
+    const float r01 = lerp(ax, c1.x, c1.y), r11 = lerp(ax, c1.z, c1.w);
     sum += lerp(az, lerp(ay, r00, r10), lerp(ay, r01, r11));
     kf += 1.0f;
   }
@@ -179,7 +190,7 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_project_kernel(FwdGeom G, con
 //   B_i = D [ r_ref x sum g + D e x sum kappa g ]     -> six running sums (sum g, sum kappa g) per ray.
 // Block result: sum_i w_i A_i, sum_i w_i B_i over the block's rays -> partials[view][block][6]   (Eq.20 :185).
 __global__ void __launch_bounds__(kFwdThreads) fwd_grad_kernel(FwdGeom G, const FwdView* __restrict__ views,
-                                                               const float2* __restrict__ pvol,
+                                                               const float4* __restrict__ pvol,
                                                                const float* __restrict__ upstream,
                                                                float* __restrict__ partials) {
   int iu, iv;
@@ -190,9 +201,8 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_grad_kernel(FwdGeom G, const 
   if (live) {
     double e_mm[3], ref_mm[3];
     const Ray r = setup_ray(G, views[view], iu, iv, e_mm, ref_mm);
-    const unsigned S1 = G.L.px, S2 = (unsigned)G.L.px * G.L.py;
-    const unsigned C0 = (unsigned)(G.L.hz + kPad) * S2 + (unsigned)(G.L.hy + kPad) * S1 + (unsigned)(G.L.hx + kPad) -
-                        (unsigned)kMagicBits * (S2 + S1 + 1u);
+    const unsigned by8 = 2u * G.L.by + 4u;          // 8*nbx:     FY(Y+2) - FY(Y)
+    const unsigned bz8 = 2u * G.L.bz + 8u;          // 8*nbx*nby: FZ(Z+2) - FZ(Z)
     float gx = 0.f, gy = 0.f, gz = 0.f, hx = 0.f, hy = 0.f, hz = 0.f;
     float kf = (float)r.k0;
     for (int i = 0; i < r.n; ++i) {
@@ -200,33 +210,31 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_grad_kernel(FwdGeom G, const 
       const float tx = qx + kMagic, ty = qy + kMagic, tz = qz + kMagic;
       const float ax = (qx - (tx - kMagic)) + 0.5f, ay = (qy - (ty - kMagic)) + 0.5f,
                   az = (qz - (tz - kMagic)) + 0.5f;
-      const unsigned idx = (unsigned)__float_as_int(tz) * S2 + (unsigned)__float_as_int(ty) * S1 +
-                           (unsigned)__float_as_int(tx) + C0;
-      const float2* c = pvol + idx;
-      // core rows (y+j, z+k): cells x-1 and x+1 give v[x-1..x+2]
-      float rv[2][2], rdx[2][2];
-#pragma unroll
-      for (int k = 0; k < 2; ++k)
-#pragma unroll
-        for (int j = 0; j < 2; ++j) {
-          const float2* row = c + k * S2 + j * S1;
-          const float2 lo = ldg2(row - 1), hi = ldg2(row + 1);     // (v[x-1], v[x]), (v[x+1], v[x+2])
-          rv[j][k] = lerp(ax, lo.y, hi.x);
-          rdx[j][k] = lerp(ax, hi.x - lo.x, hi.y - lo.y);
-        }
-      // ring rows in y: (y-1, z+k), (y+2, z+k); ring rows in z: (y+j, z-1), (y+j, z+2)
-      float rym[2], ryp[2], rzm[2], rzp[2];
+      const unsigned idx = brick_index(G.L, tx, ty, tz);
+      // neighbour cells: +-1 along an axis stays inside the brick or hops to the next one, by parity
+      const unsigned ox = (unsigned)__float_as_int(tx) & 1u, oy = (unsigned)__float_as_int(ty) & 1u,
+                     oz = (unsigned)__float_as_int(tz) & 1u;
+      const unsigned dxp = 1u + 6u * ox, dxm = dxp - 8u;
+      const unsigned dyp = 2u + (by8 - 4u) * oy, dym = dyp - by8;
+      const unsigned dzp = 4u + (bz8 - 8u) * oz, dzm = dzp - bz8;
+      float rv[2][2], rdx[2][2], rym[2], ryp[2];
 #pragma unroll
       for (int k = 0; k < 2; ++k) {
-        const float2 m = ldg2(c + k * S2 - S1), p = ldg2(c + k * S2 + 2 * S1);
-        rym[k] = lerp(ax, m.x, m.y);
-        ryp[k] = lerp(ax, p.x, p.y);
+        const unsigned b = k ? idx + dzp : idx;
+        const float4 A = ldg4(pvol + (b + dxm)), B = ldg4(pvol + (b + dxp));   // x-1,x | x+1,x+2 ; rows y, y+1
+        const float4 C = ldg4(pvol + (b + dym)), D = ldg4(pvol + (b + dyp));   // x,x+1 ; rows y-1,y | y+1,y+2
+        rv[0][k] = lerp(ax, A.y, B.x);
+        rv[1][k] = lerp(ax, A.w, B.z);
+        rdx[0][k] = lerp(ax, B.x - A.x, B.y - A.y);
+        rdx[1][k] = lerp(ax, B.z - A.z, B.w - A.w);
+        rym[k] = lerp(ax, C.x, C.y);
+        ryp[k] = lerp(ax, D.z, D.w);
       }
-#pragma unroll
-      for (int j = 0; j < 2; ++j) {
-        const float2 m = ldg2(c + j * S1 - S2), p = ldg2(c + j * S1 + 2 * S2);
-        rzm[j] = lerp(ax, m.x, m.y);
-        rzp[j] = lerp(ax, p.x, p.y);
+      float rzm[2], rzp[2];
+      {
+        const float4 E = ldg4(pvol + (idx + dzm)), F = ldg4(pvol + (idx + bz8));  // slices z-1, z+2; rows y, y+1
+        rzm[0] = lerp(ax, E.x, E.y); rzm[1] = lerp(ax, E.z, E.w);
+        rzp[0] = lerp(ax, F.x, F.y); rzp[1] = lerp(ax, F.z, F.w);
       }
       const float ddx = lerp(az, lerp(ay, rdx[0][0], rdx[1][0]), lerp(ay, rdx[0][1], rdx[1][1]));
       const float dy0 = lerp(ay, rv[1][0] - rym[0], ryp[0] - rv[0][0]);

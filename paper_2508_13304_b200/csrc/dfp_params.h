@@ -20,11 +20,22 @@ constexpr int kPad = 4;          // zero border (voxels / pixels) around the pac
 constexpr int kPadDet = 4;
 
 // ---------------------------------------------------------------- geometry shared by all views of a call
-struct VolLayout {               // packed volume: float2 cell (v[x], v[x+1]) at [z+kPad][y+kPad][x+kPad]
+// Packed volume: one float4 QUAD cell per padded voxel position (X,Y,Z) = (ix+lx, iy+ly, iz+lz),
+//   cell = (v[ix][iy], v[ix+1][iy], v[ix][iy+1], v[ix+1][iy+1]) at slice iz   (out-of-range voxels = 0),
+// stored in 2x2x2-cell BRICKS of 128 bytes (one L1 line):
+//   cell index = FX(X) + FY(Y) + FZ(Z),  FX = (X>>1)*8 + (X&1),  FY = (Y>>1)*8*nbx + (Y&1)*2,
+//                                        FZ = (Z>>1)*8*nbx*nby + (Z&1)*4
+// so that the 32 rays of a warp (a compact patch perpendicular to the ray, whatever its direction) touch
+// few distinct lines per load.
+struct VolLayout {
   int nx, ny, nz;
-  int px, py, pz;                // padded dims (px even)
+  int px, py, pz;                // padded dims (all even)
+  int nbx, nby;                  // bricks per row / per slab row
+  int lx, ly, lz;                // low-side pad (kPad or kPad+1, chosen so that H_a + l_a is even)
   int hx, hy, hz;                // H_a = floor((n_a - 1)/2): integer part of the centre index
   float fx, fy, fz;              // (n_a-1)/2 - H_a  in {0, 0.5}
+  unsigned by, bz;               // 4*nbx - 2, 4*nbx*nby - 4: multipliers of (Y & ~1), (Z & ~1)
+  unsigned c0;                   // folds (H_a + l_a) and the magic-number bias into the cell index
 };
 
 struct FwdGeom {
@@ -101,10 +112,21 @@ inline float step_of(const dfp_geometry& g) {
 inline VolLayout make_layout(const dfp_geometry& g) {
   VolLayout L;
   L.nx = g.nx; L.ny = g.ny; L.nz = g.nz;
-  L.px = (g.nx + 2 * kPad + 1) & ~1;
-  L.py = g.ny + 2 * kPad;
-  L.pz = g.nz + 2 * kPad;
   L.hx = (g.nx - 1) / 2; L.hy = (g.ny - 1) / 2; L.hz = (g.nz - 1) / 2;
+  L.lx = kPad + ((L.hx + kPad) & 1); L.ly = kPad + ((L.hy + kPad) & 1); L.lz = kPad + ((L.hz + kPad) & 1);
+  L.px = (g.nx + L.lx + kPad + 1) & ~1;
+  L.py = (g.ny + L.ly + kPad + 1) & ~1;
+  L.pz = (g.nz + L.lz + kPad + 1) & ~1;
+  L.nbx = L.px / 2; L.nby = L.py / 2;
+  L.by = 4u * (unsigned)L.nbx - 2u;
+  L.bz = 4u * (unsigned)L.nbx * (unsigned)L.nby - 4u;
+  // index = sum_a [ w_a*T_a + b_a*(T_a & ~1) ] + c0 with T_a = float bits of the magic-rounded coordinate
+  // = kMagicBits + i_a (i_a = centred index), X = i_a + H_a + l_a (even offset keeps the parity of T_a).
+  {
+    const unsigned mb = 0x4B400000u;
+    const unsigned ox = (unsigned)(L.hx + L.lx) - mb, oy = (unsigned)(L.hy + L.ly) - mb, oz = (unsigned)(L.hz + L.lz) - mb;
+    L.c0 = ox * 4u + oy * (2u + L.by) + oz * (4u + L.bz);
+  }
   L.fx = (float)((g.nx - 1) * 0.5 - L.hx); L.fy = (float)((g.ny - 1) * 0.5 - L.hy);
   L.fz = (float)((g.nz - 1) * 0.5 - L.hz);
   return L;
