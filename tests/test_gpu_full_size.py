@@ -1,0 +1,125 @@
+"""GPU-vs-oracle parity at BASELINE.json's FULL sizes (`-m gpu`), in the launch configuration `bench.py` times.
+
+The CUDA path runs the whole config (all views, full grids) through the C ABI; the fp64 oracle recomputes
+SAMPLED outputs one by one on the same seeded inputs:
+  * projections: seeded views x a band of detector rows (the band is an exact sub-detector: `v0` shifts the
+    principal point so that its rays are rays of the full detector);
+  * forward pose gradients: seeded views, the full 6-vector (every ray of the view enters the sum);
+  * back-projections: seeded z-slabs, all views;
+  * back-projection pose gradients: seeded views, all voxels.
+Tolerances as in test_gpu_parity.py (BASELINE.json north_star; U9).
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import workloads as W
+from helpers import grad_err_u9, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+TOL_VAL = 1e-5
+TOL_GRAD = 1e-3
+
+
+@pytest.fixture(scope="module")
+def dfp():
+    import paper_2508_13304_b200 as m
+    return m
+
+
+def row_band(g, r0, rows):
+    """Sub-detector made of rows [r0, r0+rows) of g: c_v' = c_v - r0."""
+    v0 = (g.nv - 1) / 2.0 + g.v0 - r0 - (rows - 1) / 2.0
+    return g.replace(nv=rows, v0=v0)
+
+
+def pick(seed, n, k):
+    rng = W.SplitMix64(seed)
+    out = []
+    while len(out) < k:
+        v = int(rng.uniform(0.0, n)) % n
+        if v not in out:
+            out.append(v)
+    return out
+
+
+def check_forward_full(dfp, index, n_check_views, band_rows, n_grad_views):
+    dev = torch.device("cuda:0")
+    w = W.make_config(index)
+    g = w.geom
+    a = w.angles.float().numpy()
+    p = w.poses.float().numpy()
+    vol = w.volume(dev)
+    up = w.fwd_upstream(dev)
+    proj = dfp.forward(g, a, p, vol)
+    grad = dfp.forward_pose_grad(g, a, p, vol, up).cpu().numpy()
+    torch.cuda.synchronize()
+    assert torch.isfinite(proj).all() and np.isfinite(grad).all()
+    vol_c = vol.cpu().numpy()
+    views = pick(w.seed + 101, w.n_views, n_check_views)
+    for i, v in enumerate(views):
+        r0 = pick(w.seed + 211 + v, g.nv - band_rows + 1, 1)[0]
+        gb = row_band(g, r0, band_rows)
+        o = oracle.forward(gb, a[v:v + 1], p[v:v + 1], vol_c)[0]
+        got = proj[v, r0:r0 + band_rows].cpu().numpy()
+        assert np.linalg.norm(o) > 0
+        e = rel_l2(got, o)
+        assert e <= TOL_VAL, (index, v, r0, e)
+        assert np.array_equal(got == 0, o == 0) or e <= TOL_VAL
+    for v in views[:n_grad_views]:
+        o = oracle.forward_pose_grad(g, a[v:v + 1], p[v:v + 1], vol_c, up[v:v + 1].cpu().numpy())
+        e = grad_err_u9(grad[v:v + 1], o)
+        assert e.max() <= TOL_GRAD, (index, v, e)
+    return w
+
+
+def check_back_full(dfp, index, n_slabs, slab, n_grad_views):
+    dev = torch.device("cuda:0")
+    w = W.make_config(index)
+    g = w.geom
+    a = w.angles.float().numpy()
+    p = w.poses.float().numpy()
+    proj = w.projections(dev)
+    up = w.bp_upstream(dev)
+    vol = dfp.backproject(g, a, p, proj)
+    grad = dfp.backproject_pose_grad(g, a, p, proj, up).cpu().numpy()
+    torch.cuda.synchronize()
+    assert torch.isfinite(vol).all() and np.isfinite(grad).all()
+    proj_c = proj.cpu().numpy()
+    # the back-projection tolerance is on the whole volume: accumulate the sampled slabs into one relative L2
+    num = den = 0.0
+    for z0 in pick(w.seed + 307, g.nz - slab + 1, n_slabs):
+        o = oracle.backproject(g, a, p, proj_c, z0, z0 + slab)
+        d = vol[z0:z0 + slab].cpu().numpy().astype(np.float64) - o
+        num += float((d * d).sum())
+        den += float((o * o).sum())
+    assert den > 0 and (num / den) ** 0.5 <= TOL_VAL, (index, (num / den) ** 0.5)
+    up_c = up.cpu().numpy()
+    for v in pick(w.seed + 401, w.n_views, n_grad_views):
+        o = oracle.backproject_pose_grad(g, a[v:v + 1], p[v:v + 1], proj_c[v:v + 1], up_c)
+        e = grad_err_u9(grad[v:v + 1], o)
+        assert e.max() <= TOL_GRAD, (index, v, e)
+
+
+def test_c2_registration_full(dfp):
+    """The workload bench.py times: 256^3, 64 candidate poses, 512x512 detector."""
+    check_forward_full(dfp, 2, n_check_views=3, band_rows=64, n_grad_views=2)
+
+
+def test_c3_mcfdk_full(dfp):
+    """256^3, 360 ramp-filtered views of 512x384, FDK weight."""
+    check_back_full(dfp, 3, n_slabs=3, slab=2, n_grad_views=2)
+
+
+def test_c4_calibration_full(dfp):
+    """512^3, 720 views of 768x768."""
+    check_forward_full(dfp, 4, n_check_views=2, band_rows=32, n_grad_views=1)
+
+
+def test_c5_sweep_full(dfp):
+    """512^3, 360 views of 1024x1024: all four calls (the largest config; everything resident at once)."""
+    check_forward_full(dfp, 5, n_check_views=2, band_rows=24, n_grad_views=1)
+    torch.cuda.empty_cache()
+    check_back_full(dfp, 5, n_slabs=2, slab=1, n_grad_views=1)
