@@ -174,6 +174,7 @@ def main():
         return
 
     import paper_2508_13304_b200 as dfp   # fails loudly if libdfp.so is missing: no CPU fallback
+    from paper_2508_13304_b200.sharding import max_over_ranks, shard_range, sum_over_ranks
 
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
     torch.cuda.set_device(local_rank)
@@ -190,13 +191,17 @@ def main():
         torch.cuda.synchronize()
 
     # ---------------------------------------------------------------- workload, resident in HBM
-    w = W.make_config(args.config, n_views=args.views)
+    # N ranks: a global batch of N x (the config's views), sharded by views, one shard per GPU (weak scaling);
+    # rank 0's shard is exactly the N=1 workload.  No data-path collective.
+    V1 = args.views if args.views is not None else W.CONFIGS[args.config]["views"]
+    w = W.make_config(args.config, n_views=V1 * world)
     g = w.geom
-    V = w.n_views
-    angles = w.angles.float().numpy()
-    poses = w.poses.float().numpy()
+    lo, hi = shard_range(w.n_views, rank, world)
+    V = hi - lo
+    angles = np.ascontiguousarray(w.angles.float().numpy()[lo:hi])
+    poses = np.ascontiguousarray(w.poses.float().numpy()[lo:hi])
     vol = w.volume(dev)
-    up = w.fwd_upstream(dev)
+    up = w.fwd_upstream(dev, views=range(lo, hi))
     bp_up = W.normal_field(w.seed * 4096 + 5, g.nx * g.ny * g.nz, dev).reshape(g.vol_shape).contiguous()
     proj = torch.empty((V, g.nv, g.nu), dtype=torch.float32, device=dev)
     grad = torch.empty((V, 6), dtype=torch.float32, device=dev)
@@ -252,13 +257,14 @@ def main():
     clocks = sampler.stop() if rank == 0 else None
     seg = np.array([[a.elapsed_time(b) for a, b in zip(e[:-1], e[1:])] for e in evs])   # ms, [K,4]
     t = seg.sum(axis=0) / 1e3                                                            # s per call, over K steps
-    tt = torch.tensor([t[0] + t[1], t[2] + t[3], t.sum()], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    tt = max_over_ranks(torch.tensor([t[0] + t[1], t[2] + t[3], t.sum()], dtype=torch.float64, device=dev))
     t_fg, t_bp, t_all = [float(x) for x in tt.cpu()]
+    t_call = [float(x) for x in max_over_ranks(torch.tensor(t, dtype=torch.float64, device=dev)).cpu()]
+    uu = sum_over_ranks(torch.tensor([ray_steps, voxel_views], dtype=torch.float64, device=dev))
+    job_ray_steps, job_voxel_views = [float(x) for x in uu.cpu()]      # units all ranks processed per pass
     K = args.steps
-    value = 2.0 * ray_steps * K * world / t_fg / 1e9
-    bp_value = 2.0 * voxel_views * K * world / t_bp / 1e9
+    value = 2.0 * job_ray_steps * K / t_fg / 1e9
+    bp_value = 2.0 * job_voxel_views * K / t_bp / 1e9
     n_launch = launches[0]
 
     # ---------------------------------------------------------------- end to end through the host-buffer C ABI
@@ -289,15 +295,13 @@ def main():
             tf += a_
             tb += b_
         barrier()
-        te = torch.tensor([tf, tb], dtype=torch.float64, device=dev)
-        if dist is not None:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        te = max_over_ranks(torch.tensor([tf, tb], dtype=torch.float64, device=dev))
         tf, tb = [float(x) for x in te.cpu()]
         nb = lambda t_: t_.numel() * t_.element_size()
-        e2e = {"value": 2.0 * ray_steps * K * world / tf / 1e9, "unit": UNIT,
+        e2e = {"value": 2.0 * job_ray_steps * K / tf / 1e9, "unit": UNIT,
                "h2d_bytes_per_step": 2 * nb(h_vol) + nb(h_up) + 2 * nb(h_proj) + nb(h_bpup),
                "d2h_bytes_per_step": nb(h_proj) + nb(h_grad) + nb(h_bvol) + nb(h_bgrad),
-               "backproject_gvoxel_views_per_s": 2.0 * voxel_views * K * world / tb / 1e9,
+               "backproject_gvoxel_views_per_s": 2.0 * job_voxel_views * K / tb / 1e9,
                "api": "dfp_*_host (pinned host buffers; cudaMallocAsync + H2D + kernels + D2H + sync per call)"}
 
     if rank != 0:
@@ -323,7 +327,7 @@ def main():
                 "kernel_share_of_step": {k: v * K / 1e3 / t_all for k, v in mean_ms.items()},
                 "hbm_compulsory_frac": None}
     # compulsory HBM bytes of the dominant kernel vs the measured copy peak (expected to be small)
-    comp = {"fwd_project": vol.numel() * 8 + proj.numel() * 4, "fwd_grad": vol.numel() * 8 + up.numel() * 4,
+    comp = {"fwd_project": vol.numel() * 16 + proj.numel() * 4, "fwd_grad": vol.numel() * 16 + up.numel() * 4,
             "bp": proj.numel() * 16 + bvol.numel() * 4, "bp_grad": proj.numel() * 16 + bvol.numel() * 4}[dom]
     roofline["hbm_compulsory_frac"] = comp / (mean_ms[dom] * 1e-3) / 1e9 / pk["hbm_gbs"]
 
@@ -337,15 +341,15 @@ def main():
            "ms_per_step": t_all / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f32", "data": "synthetic",
            "config": {"workload": f"{w.name} (BASELINE.json configs[{args.config - 1}]): {g.nx}^3 volume, {V} views of "
-                                  f"{g.nu}x{g.nv}, all four calls per step", "ray_steps_per_pass": ray_steps,
-                      "voxel_views_per_pass": voxel_views, "l2": "256 MiB flush write between timed steps",
-                      "parallelism": f"replicated batch x{world}, no collective"},
+                                  f"{g.nu}x{g.nv}, all four calls per step", "ray_steps_per_pass": int(job_ray_steps),
+                      "voxel_views_per_pass": int(job_voxel_views), "l2": "256 MiB flush write between timed steps",
+                      "parallelism": f"views sharded over {world} rank(s), {V} views per GPU, no data-path collective"},
            "extra": {"backproject+grad_gvoxel_views_per_s": bp_value,
-                     "forward_gray_steps_per_s": ray_steps * K * world / float(seg[:, 0].sum() / 1e3) / 1e9,
-                     "forward_pose_grad_gray_steps_per_s": ray_steps * K * world / float(seg[:, 1].sum() / 1e3) / 1e9,
-                     "backproject_gvoxel_views_per_s": voxel_views * K * world / float(seg[:, 2].sum() / 1e3) / 1e9,
+                     "forward_gray_steps_per_s": job_ray_steps * K / t_call[0] / 1e9,
+                     "forward_pose_grad_gray_steps_per_s": job_ray_steps * K / t_call[1] / 1e9,
+                     "backproject_gvoxel_views_per_s": job_voxel_views * K / t_call[2] / 1e9,
                      "backproject_pose_grad_gvoxel_views_per_s":
-                         voxel_views * K * world / float(seg[:, 3].sum() / 1e3) / 1e9,
+                         job_voxel_views * K / t_call[3] / 1e9,
                      "ms_per_call": {"forward": float(seg[:, 0].mean()), "forward_pose_grad": float(seg[:, 1].mean()),
                                      "backproject": float(seg[:, 2].mean()),
                                      "backproject_pose_grad": float(seg[:, 3].mean())}},

@@ -46,7 +46,9 @@ typedef struct dfp_geometry {
   float sad, sdd;       /* source-axis and source-detector distance, mm (0 < sad < sdd)                     */
   float step_mm;        /* ray-march step; <= 0 means min(vx,vy,vz)                                         */
   int32_t bp_weight;    /* back-projection weight W: 0 = 1 (pure Eq.2b), 1 = FDK (sad/w')^2                 */
-  int32_t flags;        /* bit0 (DFP_FLAG_DW): add the dW/dtheta term in dfp_backproject_pose_grad          */
+  int32_t flags;        /* bit0 (DFP_FLAG_DW): add the dW/dtheta term in dfp_backproject_pose_grad;
+                           bit1 (DFP_FLAG_NO_TMA): forward paths use the global-memory gather kernels even where
+                           the TMA-staged kernels apply (same results bit for bit; a testing / profiling switch) */
 } dfp_geometry;
 
 enum {
@@ -59,7 +61,7 @@ enum {
   DFP_ERR_CUDA = -6        /* CUDA runtime error (no device, launch failure, out of memory in *_host)       */
 };
 enum { DFP_OP_FORWARD = 0, DFP_OP_FORWARD_POSE_GRAD = 1, DFP_OP_BACKPROJECT = 2, DFP_OP_BACKPROJECT_POSE_GRAD = 3 };
-enum { DFP_FLAG_DW = 1 };
+enum { DFP_FLAG_DW = 1, DFP_FLAG_NO_TMA = 2 };
 
 /* Forward projection, Eq.2a :67-69 discretised as Eq.18 :172-177 with a fixed-step, zero-extended
  * trilinear ray-march (U1): proj[v][iv][iu] = D * sum_k f~(R_v^T (s_v + (k+1/2) D e_i - t_v)).
@@ -121,6 +123,13 @@ float dfp_last_kernel_ms(void);
 
 /* Number of kernels the last successful call on this thread launched (for bench accounting). */
 int dfp_last_launch_count(void);
+
+/* Kernel path the last successful device-pointer call on this thread took: DFP_PATH_GATHER (global-memory
+ * gathers from a packed copy of the input) or DFP_PATH_TMA (input staged tile by tile in shared memory by TMA;
+ * forward calls only, taken when nx % 4 == 0 and every view's pixel tiles fit the staging box).  The two paths
+ * give bit-identical results. */
+enum { DFP_PATH_GATHER = 0, DFP_PATH_TMA = 1 };
+int dfp_last_path(void);
 
 /* Static description of a status code; for DFP_ERR_CUDA the text of the last CUDA error seen on this thread. */
 const char* dfp_status_string(int status);

@@ -15,6 +15,8 @@ _LIB_PATH = os.path.join(_HERE, "libdfp.so")
 
 OP_FORWARD, OP_FORWARD_POSE_GRAD, OP_BACKPROJECT, OP_BACKPROJECT_POSE_GRAD = 0, 1, 2, 3
 FLAG_DW = 1
+FLAG_NO_TMA = 2
+PATH_GATHER, PATH_TMA = 0, 1
 
 
 class DfpError(RuntimeError):
@@ -68,7 +70,7 @@ def _load():
     lib.dfp_backproject_pose_grad_host.argtypes = [gp, ci, vp, vp, vp, vp, vp, vp]
     for f in (lib.dfp_forward, lib.dfp_backproject, lib.dfp_forward_pose_grad, lib.dfp_backproject_pose_grad,
               lib.dfp_forward_host, lib.dfp_backproject_host, lib.dfp_forward_pose_grad_host,
-              lib.dfp_backproject_pose_grad_host, lib.dfp_last_launch_count, lib.dfp_version):
+              lib.dfp_backproject_pose_grad_host, lib.dfp_last_launch_count, lib.dfp_last_path, lib.dfp_version):
         f.restype = ci
     lib.dfp_workspace_bytes.argtypes = [gp, ci, ci]
     lib.dfp_workspace_bytes.restype = sz
@@ -100,6 +102,11 @@ def status_string(status: int) -> str:
 
 def last_launch_count() -> int:
     return int(_lib.dfp_last_launch_count())
+
+
+def last_path() -> int:
+    """PATH_GATHER or PATH_TMA: which kernels the last device-pointer call on this thread ran."""
+    return int(_lib.dfp_last_path())
 
 
 def set_kernel_timing(enable: bool) -> None:

@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "../../include/dfp.h"
+#include "dfp_fwd_tma.cuh"
 #include "dfp_kernels.cuh"
 #include "dfp_params.h"
 
@@ -19,6 +20,7 @@ using namespace dfp;
 
 thread_local char g_cuda_msg[256] = "no CUDA error recorded";
 thread_local int g_launches = 0;
+thread_local int g_path = DFP_PATH_GATHER;
 
 thread_local bool g_timing = false;
 thread_local cudaEvent_t g_ev[2] = {nullptr, nullptr};
@@ -75,6 +77,78 @@ int validate_views(int n_views, const float* angles, const float* poses) {
       if (!std::isfinite(poses[6 * v + k])) return DFP_ERR_NONFINITE;
   }
   return DFP_OK;
+}
+
+// ---- TMA path of the forward kernels (dfp_fwd_tma.cuh) -------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = []() -> EncodeTiledFn {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      return nullptr;
+    return reinterpret_cast<EncodeTiledFn>(p);
+  }();
+  return fn;
+}
+
+// Tensor map over the caller's volume [nz][ny][nx] fp32 with the staging box of dfp_fwd_tma.cuh; elements
+// outside the volume read as zero (the zero extension of f~, U7).
+bool make_volume_map(const dfp_geometry& g, const float* d_vol, CUtensorMap* map) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc || (g.nx % 4) != 0) return false;           // global strides must be multiples of 16 bytes
+  const cuuint64_t dims[3] = {(cuuint64_t)g.nx, (cuuint64_t)g.ny, (cuuint64_t)g.nz};
+  const cuuint64_t strides[2] = {(cuuint64_t)g.nx * 4, (cuuint64_t)g.nx * g.ny * 4};
+  const cuuint32_t box[3] = {kBX, kBY, kBZ};
+  const cuuint32_t es[3] = {1, 1, 1};
+  return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(d_vol), dims, strides, box, es,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// Conservative host-side bound: can every 16x16-pixel tile of this view march in chunks of >= kMinChunk samples
+// inside the staging box?  (The kernel computes the exact chunk length per block; this only picks the path.)
+// Positions at path length tau: p = s' + tau e, so a tile's extent along axis a is tau |De_a| with
+// |De_a| <= (|Dd_a| + |e_a| (rho_max/|d|) |Dd|) / SDD  for pixel offsets Dd on a detector at distance >= SDD.
+constexpr int kMinChunk = 4;
+bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V, bool grad) {
+  const double v3[3] = {g.vx, g.vy, g.vz}, c3[3] = {g.cx, g.cy, g.cz};
+  const double half[3] = {0.5 * g.nx * g.vx + 3 * g.vx, 0.5 * g.ny * g.vy + 3 * g.vy, 0.5 * g.nz * g.vz + 3 * g.vz};
+  double tau_max = 0;
+  for (int c = 0; c < 8; ++c) {
+    double d2 = 0;
+    for (int a = 0; a < 3; ++a) {
+      const double x = c3[a] + ((c >> a) & 1 ? half[a] : -half[a]) - V.src[a];
+      d2 += x * x;
+    }
+    tau_max = std::fmax(tau_max, std::sqrt(d2));
+  }
+  double emax[3] = {0, 0, 0}, dmax = 0;
+  for (int c = 0; c < 4; ++c) {
+    const double iu = (c & 1) ? g.nu - 1 : 0, iv = (c & 2) ? g.nv - 1 : 0;
+    double d[3], n2 = 0;
+    for (int a = 0; a < 3; ++a) { d[a] = V.d0[a] + iu * V.du[a] + iv * V.dv[a]; n2 += d[a] * d[a]; }
+    const double n = std::sqrt(n2);
+    dmax = std::fmax(dmax, n);
+    for (int a = 0; a < 3; ++a) emax[a] = std::fmax(emax[a], std::fabs(d[a]) / n);
+  }
+  const double sdd = g.sdd;
+  const double rho = std::sqrt(std::fmax(dmax * dmax - sdd * sdd, 0.0)) / sdd;
+  const double tu = kFwdTU - 1, tv = kFwdTV - 1;
+  const double dnorm = std::hypot(tu * (double)g.du, tv * (double)g.dv);
+  const int box[3] = {kBX, kBY, kBZ};
+  for (int a = 0; a < 3; ++a) {
+    const double dd = tu * std::fabs(V.du[a]) + tv * std::fabs(V.dv[a]);
+    const double span = tau_max * (dd + emax[a] * rho * dnorm) / sdd / v3[a];
+    const double slope = (double)G.step * emax[a] / v3[a];
+    const double avail = box[a] - 4 - (grad ? 2 : 0) - (a == 0 ? kBoxAlignLoss : 0) - 2.0 * kBoxMargin - 1.05 * span - 0.05;
+    if (avail < (kMinChunk - 1) * slope) return false;
+  }
+  return true;
 }
 
 // ---- workspace carving ---------------------------------------------------------------------------
@@ -154,10 +228,34 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
   g_launches = 0;
   DFP_CUDA(cudaMemcpyAsync(dv, hv.data(), sizeof(FwdView) * V, cudaMemcpyHostToDevice, s), "view upload");
   if (grad) DFP_CUDA(cudaMemcpyAsync(dc, hc.data(), sizeof(FwdContract) * V, cudaMemcpyHostToDevice, s), "view upload");
+  const dim3 grid(w.gx, w.gy, V);
+  // TMA-staged path when the volume admits a tensor map and every view's tiles fit the staging box
+  CUtensorMap vol_map;
+  bool tma = !(g->flags & DFP_FLAG_NO_TMA) && make_volume_map(*g, d_vol, &vol_map);
+  for (int v = 0; tma && v < V; ++v) tma = tma_view_fits(*g, G, hv[v], grad);
+  g_path = tma ? DFP_PATH_TMA : DFP_PATH_GATHER;
+  if (tma) {
+    static const cudaError_t attr_f = cudaFuncSetAttribute(fwd_tma_kernel<false>,
+                                                           cudaFuncAttributeMaxDynamicSharedMemorySize, kTmaSmemBytes);
+    static const cudaError_t attr_g = cudaFuncSetAttribute(fwd_tma_kernel<true>,
+                                                           cudaFuncAttributeMaxDynamicSharedMemorySize, kTmaSmemBytes);
+    DFP_CUDA(attr_f, "cudaFuncSetAttribute");
+    DFP_CUDA(attr_g, "cudaFuncSetAttribute");
+    time_begin(s);
+    if (!grad) fwd_tma_kernel<false><<<grid, kFwdThreads, kTmaSmemBytes, s>>>(G, dv, vol_map, nullptr, d_out);
+    else fwd_tma_kernel<true><<<grid, kFwdThreads, kTmaSmemBytes, s>>>(G, dv, vol_map, d_up, part);
+    time_end(s);
+    ++g_launches;
+    if (grad) {
+      fwd_contract_kernel<<<V, 256, 0, s>>>(w.gx * w.gy, part, dc, d_out);
+      ++g_launches;
+    }
+    DFP_CUDA(cudaGetLastError(), "forward launch (TMA path)");
+    return DFP_OK;
+  }
   const size_t ncell = (size_t)G.L.px * G.L.py * G.L.pz;
   pack_volume_kernel<<<grid_1d(ncell, 256), 256, 0, s>>>(G.L, d_vol, pvol);
   ++g_launches;
-  const dim3 grid(w.gx, w.gy, V);
   if (!grad) {
     time_begin(s);
     fwd_project_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, pvol, d_out);
@@ -193,6 +291,7 @@ int run_backproject(const dfp_geometry* g, int V, const float* angles, const flo
   float4* q = reinterpret_cast<float4*>(base + w.off_q);
   float* part = reinterpret_cast<float*>(base + w.off_part);
   g_launches = 0;
+  g_path = DFP_PATH_GATHER;
   DFP_CUDA(cudaMemcpyAsync(dv, hv.data(), sizeof(BpView) * V, cudaMemcpyHostToDevice, s), "view upload");
   if (grad) DFP_CUDA(cudaMemcpyAsync(dc, hc.data(), sizeof(BpContract) * V, cudaMemcpyHostToDevice, s), "view upload");
   const size_t ncell = (size_t)V * G.pu * G.pv;
@@ -358,6 +457,8 @@ float dfp_last_kernel_ms(void) {
 }
 
 int dfp_last_launch_count(void) { return g_launches; }
+
+int dfp_last_path(void) { return g_path; }
 
 const char* dfp_status_string(int status) {
   switch (status) {

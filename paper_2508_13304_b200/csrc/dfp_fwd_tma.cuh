@@ -1,0 +1,287 @@
+// dfp_fwd_tma.cuh - a3 / a4 with the volume staged in shared memory by TMA (sm_100a).
+//
+// Same arithmetic, sample for sample, as fwd_project_kernel / fwd_grad_kernel (dfp_kernels.cuh) - the two paths
+// are bit-identical - but the 8 (forward) or 32 (gradient) voxel reads of a sample are LDS from a box of the
+// volume that the block's 16x16-pixel frustum crosses during one CHUNK of consecutive samples:
+//
+//   * the block's rays share one kappa axis (sample k = kref + kappa, tau_k = (k + 1/2) D, fixed in the world:
+//     DESIGN.md O6), so a chunk [kappa0, kappa0 + Kc) is a slab of the frustum; its bounding box in voxel
+//     indices is found from the tile's four corner rays (positions are convex in the pixel index up to the
+//     sagitta of the sphere |r - s| = tau, < 0.01 voxel for a 16-pixel tile; kBoxMargin covers it);
+//   * one elected thread issues `cp.async.bulk.tensor.3d` (TMA, SASS UTMALDG) for the box [kBX x kBY x kBZ]
+//     straight from the caller's volume: out-of-range elements are ZERO-FILLED by the TMA unit, which is the
+//     zero extension of f~ (U7) - no padded / packed copy of the volume is made on this path;
+//   * two stages, mbarrier (complete_tx) as the "full" signal, __syncthreads as the "empty" signal;
+//   * the box origin is rounded down to a multiple of 4 floats along x (TMA: 16-byte inner alignment);
+//   * Kc is chosen per block so that the box always fits (oblique tiles get shorter chunks).
+// PAPER.md Eq.18 :172-177 (forward), Eq.7-8 :101-113, Eq.19-20 :179-191 (gradient), :207 (on the fly, weights once).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include "dfp_kernels.cuh"
+
+namespace dfp {
+
+constexpr int kBX = 20, kBY = 20, kBZ = 16;            // staged box (floats); kBX*4 bytes is a multiple of 16
+constexpr int kBXY = kBX * kBY;
+constexpr int kBoxWords = kBX * kBY * kBZ;
+constexpr int kBoxBytes = kBoxWords * 4;               // 25600 = 200 * 128
+constexpr int kStages = 2;
+constexpr int kTmaSmemBytes = kStages * kBoxBytes;     // dynamic shared memory of fwd_tma_kernel
+constexpr float kBoxMargin = 0.05f;                    // voxels: sagitta of the tile + fp32 rounding
+constexpr int kBoxAlignLoss = 3;                       // x cells lost to the 16-byte alignment of the box origin
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap* map, int x, int y, int z, unsigned bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+      ::"r"(dst), "l"(reinterpret_cast<unsigned long long>(map)), "r"(x), "r"(y), "r"(z), "r"(bar)
+      : "memory");
+}
+
+struct TmaBlock {              // block-wide state in shared memory
+  float pm[4][3], dp[4][3];    // the tile's corner rays (centred-index coordinates, as in struct Ray)
+  int kA, kB;                  // union of the live rays' kappa ranges [kA, kB)
+  int Kc;                      // samples per chunk (0: nothing to do, -1: the box cannot hold the tile)
+  unsigned c0[kStages];        // per-stage index constant: word index = Tx + kBX*Ty + kBXY*Tz + c0
+};
+
+// One chunk's box: origin (voxel indices, for the TMA) and the index constant of the stage it lands in.
+template <bool GRAD>
+__device__ __forceinline__ void issue_chunk(const VolLayout& L, TmaBlock& B, const CUtensorMap* map, int chunk,
+                                            unsigned tiles_addr, unsigned bar_addr) {
+  const int s = chunk % kStages;
+  const int k0 = B.kA + chunk * B.Kc;
+  const int k1 = min(k0 + B.Kc, B.kB) - 1;
+  const float f0 = (float)k0, f1 = (float)k1;
+  int oc[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    float lo = 3.0e38f;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) lo = fminf(lo, fminf(fmaf(f0, B.dp[r][a], B.pm[r][a]), fmaf(f1, B.dp[r][a], B.pm[r][a])));
+    oc[a] = (int)floorf(lo - 0.5f - kBoxMargin) - (GRAD ? 1 : 0);      // centred index of the box's first cell
+  }
+  // the TMA unit wants the innermost coordinate on a 16-byte boundary (measured on B200: an x origin that is
+  // not a multiple of 4 floats raises an illegal-instruction fault): round the x origin down, kBoxAlignLoss
+  oc[0] = (((oc[0] + L.hx) >> 2) << 2) - L.hx;
+  const unsigned mb = (unsigned)kMagicBits;
+  B.c0[s] = (unsigned)(s * kBoxWords) - ((unsigned)oc[0] + mb) - (unsigned)kBX * ((unsigned)oc[1] + mb) -
+            (unsigned)kBXY * ((unsigned)oc[2] + mb);
+  const unsigned bar = bar_addr + 8u * s;
+  mbar_expect_tx(bar, kBoxBytes);
+  tma_load_3d(tiles_addr + (unsigned)(s * kBoxBytes), map, oc[0] + L.hx, oc[1] + L.hy, oc[2] + L.hz, bar);
+}
+
+template <bool GRAD>
+__global__ void __launch_bounds__(kFwdThreads) fwd_tma_kernel(FwdGeom G, const FwdView* __restrict__ views,
+                                                              const __grid_constant__ CUtensorMap vol_map,
+                                                              const float* __restrict__ upstream,
+                                                              float* __restrict__ out) {
+  extern __shared__ __align__(128) float tiles[];      // kStages boxes
+  __shared__ __align__(8) unsigned long long full_bar[kStages];
+  __shared__ TmaBlock B;
+  __shared__ float red[kFwdThreads / 32][6];
+
+  int iu, iv;
+  fwd_pixel(iu, iv);
+  const int view = blockIdx.z;
+  const bool live = iu < G.nu && iv < G.nv;
+  const unsigned tiles_addr = smem_u32(tiles), bar_addr = smem_u32(full_bar);
+
+  double e_mm[3], ref_mm[3];
+  Ray r = setup_ray(G, views[view], iu, iv, GRAD ? e_mm : nullptr, GRAD ? ref_mm : nullptr);
+  if (!live) r.n = 0;
+
+  if (threadIdx.x == 0) {
+    B.kA = 0x7fffffff;
+    B.kB = -0x7fffffff;
+#pragma unroll
+    for (int s = 0; s < kStages; ++s) mbar_init(bar_addr + 8u * s, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  {  // corner rays of the tile: pixels (0,0), (TU-1,0), (0,TV-1), (TU-1,TV-1) of the block
+    const int cu = iu - blockIdx.x * kFwdTU, cv = iv - blockIdx.y * kFwdTV;
+    if ((cu == 0 || cu == kFwdTU - 1) && (cv == 0 || cv == kFwdTV - 1)) {
+      const int c = (cu ? 1 : 0) + (cv ? 2 : 0);
+      B.pm[c][0] = r.pmx; B.pm[c][1] = r.pmy; B.pm[c][2] = r.pmz;
+      B.dp[c][0] = r.dpx; B.dp[c][1] = r.dpy; B.dp[c][2] = r.dpz;
+    }
+  }
+  __syncthreads();
+  {  // union of the live kappa ranges
+    int lo = r.n > 0 ? r.k0 : 0x7fffffff, hi = r.n > 0 ? r.k0 + r.n : -0x7fffffff;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+      hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+    }
+    if ((threadIdx.x & 31) == 0 && lo < hi) {
+      atomicMin(&B.kA, lo);
+      atomicMax(&B.kB, hi);
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int Kc = 0;
+    if (B.kA < B.kB) {
+      // chunk length: extent_a <= span_a + (Kc - 1) slope_a must leave room for the floor / stencil cells
+      const float fa = (float)B.kA, fb = (float)(B.kB - 1);
+      const int box[3] = {kBX, kBY, kBZ};
+      Kc = 4096;
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        float lo0 = 3e38f, hi0 = -3e38f, lo1 = 3e38f, hi1 = -3e38f, slope = 0.f;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          const float q0 = fmaf(fa, B.dp[c][a], B.pm[c][a]), q1 = fmaf(fb, B.dp[c][a], B.pm[c][a]);
+          lo0 = fminf(lo0, q0); hi0 = fmaxf(hi0, q0);
+          lo1 = fminf(lo1, q1); hi1 = fmaxf(hi1, q1);
+          slope = fmaxf(slope, fabsf(B.dp[c][a]));
+        }
+        const float span = fmaxf(hi0 - lo0, hi1 - lo1);
+        const float avail = (float)(box[a] - 4 - (GRAD ? 2 : 0) - (a == 0 ? kBoxAlignLoss : 0)) - 2.f * kBoxMargin - span;
+        if (avail < 0.f) Kc = -1;
+        else if (Kc > 0 && slope > 1e-7f) Kc = min(Kc, (int)floorf(avail / slope) + 1);
+      }
+    }
+    B.Kc = Kc;
+    if (Kc > 0) {
+      const int n_chunks = (B.kB - B.kA + Kc - 1) / Kc;
+      issue_chunk<GRAD>(G.L, B, &vol_map, 0, tiles_addr, bar_addr);
+      if (n_chunks > 1) issue_chunk<GRAD>(G.L, B, &vol_map, 1, tiles_addr, bar_addr);
+    }
+  }
+  __syncthreads();
+  const int Kc = B.Kc, kA = B.kA, kB = B.kB;
+  const int n_chunks = Kc > 0 ? (kB - kA + Kc - 1) / Kc : 0;
+  const int kend = r.k0 + r.n;
+
+  float sum = 0.f;
+  float gx = 0.f, gy = 0.f, gz = 0.f, hx = 0.f, hy = 0.f, hz = 0.f;
+  for (int chunk = 0; chunk < n_chunks; ++chunk) {
+    const int s = chunk % kStages;
+    mbar_wait(bar_addr + 8u * s, (unsigned)(chunk / kStages) & 1u);
+    const unsigned c0 = B.c0[s];
+    const int c_lo = kA + chunk * Kc;
+    const int ka = max(c_lo, r.k0), kb = min(min(c_lo + Kc, kB), kend);
+    float kf = (float)ka;
+    for (int k = ka; k < kb; ++k) {
+      const float qx = fmaf(kf, r.dpx, r.pmx), qy = fmaf(kf, r.dpy, r.pmy), qz = fmaf(kf, r.dpz, r.pmz);
+      const float tx = qx + kMagic, ty = qy + kMagic, tz = qz + kMagic;
+      const float ax = (qx - (tx - kMagic)) + 0.5f, ay = (qy - (ty - kMagic)) + 0.5f, az = (qz - (tz - kMagic)) + 0.5f;
+      const unsigned idx = (unsigned)__float_as_int(tx) + (unsigned)kBX * (unsigned)__float_as_int(ty) +
+                           (unsigned)kBXY * (unsigned)__float_as_int(tz) + c0;
+      const float* c = tiles + idx;
+      if (!GRAD) {
+        const float r00 = lerp(ax, c[0], c[1]), r10 = lerp(ax, c[kBX], c[kBX + 1]);
+        const float r01 = lerp(ax, c[kBXY], c[kBXY + 1]), r11 = lerp(ax, c[kBXY + kBX], c[kBXY + kBX + 1]);
+        sum += lerp(az, lerp(ay, r00, r10), lerp(ay, r01, r11));
+      } else {
+        float rv[2][2], rdx[2][2];
+#pragma unroll
+        for (int kk = 0; kk < 2; ++kk)
+#pragma unroll
+          for (int j = 0; j < 2; ++j) {
+            const float* row = c + kk * kBXY + j * kBX;
+            const float m1 = row[-1], v0 = row[0], v1 = row[1], v2 = row[2];
+            rv[j][kk] = lerp(ax, v0, v1);
+            rdx[j][kk] = lerp(ax, v1 - m1, v2 - v0);
+          }
+        float rym[2], ryp[2], rzm[2], rzp[2];
+#pragma unroll
+        for (int kk = 0; kk < 2; ++kk) {
+          const float* m = c + kk * kBXY - kBX;
+          const float* p = c + kk * kBXY + 2 * kBX;
+          rym[kk] = lerp(ax, m[0], m[1]);
+          ryp[kk] = lerp(ax, p[0], p[1]);
+        }
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+          const float* m = c + j * kBX - kBXY;
+          const float* p = c + j * kBX + 2 * kBXY;
+          rzm[j] = lerp(ax, m[0], m[1]);
+          rzp[j] = lerp(ax, p[0], p[1]);
+        }
+        const float ddx = lerp(az, lerp(ay, rdx[0][0], rdx[1][0]), lerp(ay, rdx[0][1], rdx[1][1]));
+        const float dy0 = lerp(ay, rv[1][0] - rym[0], ryp[0] - rv[0][0]);
+        const float dy1 = lerp(ay, rv[1][1] - rym[1], ryp[1] - rv[0][1]);
+        const float ddy = lerp(az, dy0, dy1);
+        const float dz0 = lerp(az, rv[0][1] - rzm[0], rzp[0] - rv[0][0]);
+        const float dz1 = lerp(az, rv[1][1] - rzm[1], rzp[1] - rv[1][0]);
+        const float ddz = lerp(ay, dz0, dz1);
+        gx += ddx; gy += ddy; gz += ddz;
+        hx = fmaf(kf, ddx, hx); hy = fmaf(kf, ddy, hy); hz = fmaf(kf, ddz, hz);
+      }
+      kf += 1.0f;
+    }
+    __syncthreads();                                   // every thread is done with stage s ("empty")
+    if (threadIdx.x == 0 && chunk + kStages < n_chunks)
+      issue_chunk<GRAD>(G.L, B, &vol_map, chunk + kStages, tiles_addr, bar_addr);
+  }
+
+  const float bad = Kc < 0 ? __int_as_float(0x7fc00000) : 0.f;   // NaN marks "box cannot hold the tile" (host bound wrong)
+  if (!GRAD) {
+    if (live) out[((size_t)view * G.nv + iv) * G.nu + iu] = G.step * sum + bad;
+    return;
+  }
+  float o6[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  if (live) {
+    const float w = __ldg(upstream + ((size_t)view * G.nv + iv) * G.nu + iu);
+    const float D = G.step;
+    const float sx = gx * G.sgx, sy = gy * G.sgy, sz = gz * G.sgz;
+    const float mx = hx * G.sgx * D, my = hy * G.sgy * D, mz = hz * G.sgz * D;
+    const float ex = (float)e_mm[0], ey = (float)e_mm[1], ez = (float)e_mm[2];
+    const float px = (float)ref_mm[0], py = (float)ref_mm[1], pz = (float)ref_mm[2];
+    const float wd = w * D;
+    o6[0] = wd * sx + bad; o6[1] = wd * sy; o6[2] = wd * sz;
+    o6[3] = wd * ((py * sz - pz * sy) + (ey * mz - ez * my));
+    o6[4] = wd * ((pz * sx - px * sz) + (ez * mx - ex * mz));
+    o6[5] = wd * ((px * sy - py * sx) + (ex * my - ey * mx));
+  }
+#pragma unroll
+  for (int q = 0; q < 6; ++q) {
+    float v = o6[q];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    o6[q] = v;
+  }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (lane == 0) {
+#pragma unroll
+    for (int q = 0; q < 6; ++q) red[warp][q] = o6[q];
+  }
+  __syncthreads();
+  if (threadIdx.x < 6) {
+    float t = 0.f;
+#pragma unroll
+    for (int wI = 0; wI < kFwdThreads / 32; ++wI) t += red[wI][threadIdx.x];
+    const size_t blk = (size_t)blockIdx.y * gridDim.x + blockIdx.x;
+    const size_t nblk = (size_t)gridDim.x * gridDim.y;
+    out[((size_t)view * nblk + blk) * 6 + threadIdx.x] = t;
+  }
+}
+
+}  // namespace dfp

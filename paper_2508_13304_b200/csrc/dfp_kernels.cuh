@@ -25,7 +25,7 @@ namespace dfp {
 constexpr float kMagic = 12582912.0f;        // 1.5 * 2^23: (x + kMagic) - kMagic == rint(x) for |x| < 2^22
 constexpr int kMagicBits = 0x4B400000;       // __float_as_int(kMagic)
 
-constexpr int kFwdTU = 32, kFwdTV = 8;       // block tile of detector pixels (8 warps, each an 8x4 pixel patch)
+constexpr int kFwdTU = 16, kFwdTV = 16;      // block tile of detector pixels (8 warps, each an 8x4 pixel patch)
 constexpr int kFwdThreads = kFwdTU * kFwdTV;
 constexpr int kBpTX = 32, kBpTY = 8;         // block tile of voxels in (x, y)
 constexpr int kBpThreads = kBpTX * kBpTY;
@@ -141,11 +141,11 @@ __device__ __forceinline__ Ray setup_ray(const FwdGeom& G, const FwdView& V, int
   return r;
 }
 
-// pixel of this thread: warps are 8(u) x 4(v) patches, 4 x 2 warps per block
+// pixel of this thread: warps are 8(u) x 4(v) patches, (kFwdTU/8) x (kFwdTV/4) warps per block
 __device__ __forceinline__ void fwd_pixel(int& iu, int& iv) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  iu = blockIdx.x * kFwdTU + (warp & 3) * 8 + (lane & 7);
-  iv = blockIdx.y * kFwdTV + (warp >> 2) * 4 + (lane >> 3);
+  iu = blockIdx.x * kFwdTU + (warp % (kFwdTU / 8)) * 8 + (lane & 7);
+  iv = blockIdx.y * kFwdTV + (warp / (kFwdTU / 8)) * 4 + (lane >> 3);
 }
 
 // ------------------------------------------------------------------------------------------------ a3 forward

@@ -193,3 +193,56 @@ def test_back_configs_reduced(dfp, index, scale, views):
     w = W.make_config(index, scale=scale, n_views=views)
     check_back(run_back_case(dfp, w.geom, w.angles.numpy(), w.poses.numpy(), w.projections().numpy(),
                              w.bp_upstream().numpy()))
+
+
+# ------------------------------------------------------------------ the two forward kernel paths (gather / TMA-staged)
+def _both_paths(dfp, g, angles, poses, vol, up):
+    dev = torch.device("cuda:0")
+    a, p = f32(angles), f32(poses).reshape(-1, 6)
+    vd = torch.as_tensor(vol, dtype=torch.float32, device=dev).contiguous()
+    ud = torch.as_tensor(up, dtype=torch.float32, device=dev).contiguous()
+    out = {}
+    for name, gg in (("tma", g), ("gather", g.replace(flags=g.flags | dfp.FLAG_NO_TMA))):
+        proj = dfp.forward(gg, a, p, vd)
+        path_f = dfp.last_path()
+        grad = dfp.forward_pose_grad(gg, a, p, vd, ud)
+        out[name] = (proj.cpu(), grad.cpu(), path_f, dfp.last_path())
+    return out
+
+
+def test_tma_path_is_taken_and_matches_gather_path_bit_for_bit(dfp):
+    """nx % 4 == 0 and clinical magnification: the TMA-staged kernels run; same arithmetic => same bits."""
+    w = W.make_config(2, scale=0.25, n_views=3)
+    o = _both_paths(dfp, w.geom, w.angles.numpy(), w.poses.numpy(), w.volume().numpy(), w.fwd_upstream().numpy())
+    assert o["tma"][2] == dfp.PATH_TMA and o["tma"][3] == dfp.PATH_TMA
+    assert o["gather"][2] == dfp.PATH_GATHER and o["gather"][3] == dfp.PATH_GATHER
+    assert torch.equal(o["tma"][0], o["gather"][0])
+    assert torch.equal(o["tma"][1], o["gather"][1])
+    w = W.make_config(4, scale=0.125, n_views=5)          # views around the circle: oblique frusta, short chunks
+    o = _both_paths(dfp, w.geom, w.angles.numpy(), w.poses.numpy(), w.volume().numpy(), w.fwd_upstream().numpy())
+    assert o["tma"][2] == dfp.PATH_TMA and o["tma"][3] == dfp.PATH_TMA
+    assert torch.equal(o["tma"][0], o["gather"][0]) and torch.equal(o["tma"][1], o["gather"][1])
+
+
+def test_tma_path_ragged_detector_and_partial_misses(dfp):
+    """Detector not a multiple of the 16x16 tile, volume partly outside the fan (zero fill by the TMA unit)."""
+    g = aniso_geom(nx=40, ny=29, nz=23, nu=45, nv=21, vx=0.9, vy=1.0, vz=1.1, du=0.8, dv=0.7, sad=400.0, sdd=600.0)
+    rng = np.random.default_rng(11)
+    vol = rng.standard_normal(g.vol_shape).astype(np.float32)
+    up = rng.standard_normal((3,) + g.det_shape).astype(np.float32)
+    o = _both_paths(dfp, g, ANGLES3, POSES3, vol, up)
+    assert o["tma"][2] == dfp.PATH_TMA and o["tma"][3] == dfp.PATH_TMA
+    assert torch.equal(o["tma"][0], o["gather"][0]) and torch.equal(o["tma"][1], o["gather"][1])
+    check_forward(run_forward_case(dfp, g, ANGLES3, POSES3, vol, up))
+
+
+def test_tma_path_falls_back_when_it_does_not_apply(dfp):
+    """nx % 4 != 0 (no tensor map) or coarse pixels on fine voxels (a tile's frustum exceeds the staging box)."""
+    rng = np.random.default_rng(12)
+    for g in (aniso_geom(nx=37, ny=29, nz=23), small_geom(n=64, voxel=0.25, nu=20, nv=18, pix=2.4)):
+        vol = rng.standard_normal(g.vol_shape).astype(np.float32)
+        up = rng.standard_normal((1,) + g.det_shape).astype(np.float32)
+        dev = torch.device("cuda:0")
+        dfp.forward(g, f32([0.3]), f32([POSES3[0]]), torch.as_tensor(vol, device=dev))
+        assert dfp.last_path() == dfp.PATH_GATHER
+        check_forward(run_forward_case(dfp, g, [0.3], [POSES3[0]], vol, up))
