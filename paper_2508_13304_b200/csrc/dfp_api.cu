@@ -98,12 +98,12 @@ EncodeTiledFn encode_tiled_fn() {
 
 // Tensor map over the caller's volume [nz][ny][nx] fp32 with the staging box of dfp_fwd_tma.cuh; elements
 // outside the volume read as zero (the zero extension of f~, U7).
-bool make_volume_map(const dfp_geometry& g, const float* d_vol, CUtensorMap* map) {
+bool make_volume_map(const dfp_geometry& g, const float* d_vol, int bx, int by, int bz, CUtensorMap* map) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc || (g.nx % 4) != 0) return false;           // global strides must be multiples of 16 bytes
   const cuuint64_t dims[3] = {(cuuint64_t)g.nx, (cuuint64_t)g.ny, (cuuint64_t)g.nz};
   const cuuint64_t strides[2] = {(cuuint64_t)g.nx * 4, (cuuint64_t)g.nx * g.ny * 4};
-  const cuuint32_t box[3] = {kBX, kBY, kBZ};
+  const cuuint32_t box[3] = {(cuuint32_t)bx, (cuuint32_t)by, (cuuint32_t)bz};
   const cuuint32_t es[3] = {1, 1, 1};
   return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(d_vol), dims, strides, box, es,
              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
@@ -115,7 +115,9 @@ bool make_volume_map(const dfp_geometry& g, const float* d_vol, CUtensorMap* map
 // Positions at path length tau: p = s' + tau e, so a tile's extent along axis a is tau |De_a| with
 // |De_a| <= (|Dd_a| + |e_a| (rho_max/|d|) |Dd|) / SDD  for pixel offsets Dd on a detector at distance >= SDD.
 constexpr int kMinChunk = 4;
-bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V, bool grad) {
+template <bool GRAD>
+bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V) {
+  const bool grad = GRAD;
   const double v3[3] = {g.vx, g.vy, g.vz}, c3[3] = {g.cx, g.cy, g.cz};
   const double half[3] = {0.5 * g.nx * g.vx + 3 * g.vx, 0.5 * g.ny * g.vy + 3 * g.vy, 0.5 * g.nz * g.vz + 3 * g.vz};
   double tau_max = 0;
@@ -140,13 +142,19 @@ bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V, bo
   const double rho = std::sqrt(std::fmax(dmax * dmax - sdd * sdd, 0.0)) / sdd;
   const double tu = kFwdTU - 1, tv = kFwdTV - 1;
   const double dnorm = std::hypot(tu * (double)g.du, tv * (double)g.dv);
-  const int box[3] = {kBX, kBY, kBZ};
+  // the kernel picks the box by the first tile's ray direction; a view must fit whichever its tiles may pick
+  const bool may_x = emax[0] >= 0.5 * emax[1] || !GRAD, may_y = GRAD && emax[1] >= 0.5 * emax[0];
+  for (int cls = 0; cls < 2; ++cls) {
+    if ((cls == 0 && !may_x) || (cls == 1 && !may_y)) continue;
+    const int box[3] = {cls ? BoxShape<GRAD, 1>::X : BoxShape<GRAD, 0>::X, cls ? BoxShape<GRAD, 1>::Y : BoxShape<GRAD, 0>::Y,
+                        BoxShape<GRAD, 0>::Z};
   for (int a = 0; a < 3; ++a) {
     const double dd = tu * std::fabs(V.du[a]) + tv * std::fabs(V.dv[a]);
     const double span = tau_max * (dd + emax[a] * rho * dnorm) / sdd / v3[a];
     const double slope = (double)G.step * emax[a] / v3[a];
     const double avail = box[a] - 4 - (grad ? 2 : 0) - (a == 0 ? kBoxAlignLoss : 0) - 2.0 * kBoxMargin - 1.05 * span - 0.05;
     if (avail < (kMinChunk - 1) * slope) return false;
+  }
   }
   return true;
 }
@@ -230,20 +238,28 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
   if (grad) DFP_CUDA(cudaMemcpyAsync(dc, hc.data(), sizeof(FwdContract) * V, cudaMemcpyHostToDevice, s), "view upload");
   const dim3 grid(w.gx, w.gy, V);
   // TMA-staged path when the volume admits a tensor map and every view's tiles fit the staging box
-  CUtensorMap vol_map;
-  bool tma = !(g->flags & DFP_FLAG_NO_TMA) && make_volume_map(*g, d_vol, &vol_map);
-  for (int v = 0; tma && v < V; ++v) tma = tma_view_fits(*g, G, hv[v], grad);
+  CUtensorMap map_x, map_y;
+  bool tma = !(g->flags & DFP_FLAG_NO_TMA);
+  if (tma && !grad)
+    tma = make_volume_map(*g, d_vol, BoxShape<false, 0>::X, BoxShape<false, 0>::Y, BoxShape<false, 0>::Z, &map_x) &&
+          make_volume_map(*g, d_vol, BoxShape<false, 1>::X, BoxShape<false, 1>::Y, BoxShape<false, 1>::Z, &map_y);
+  if (tma && grad)
+    tma = make_volume_map(*g, d_vol, BoxShape<true, 0>::X, BoxShape<true, 0>::Y, BoxShape<true, 0>::Z, &map_x) &&
+          make_volume_map(*g, d_vol, BoxShape<true, 1>::X, BoxShape<true, 1>::Y, BoxShape<true, 1>::Z, &map_y);
+  for (int v = 0; tma && v < V; ++v) tma = grad ? tma_view_fits<true>(*g, G, hv[v]) : tma_view_fits<false>(*g, G, hv[v]);
   g_path = tma ? DFP_PATH_TMA : DFP_PATH_GATHER;
   if (tma) {
-    static const cudaError_t attr_f = cudaFuncSetAttribute(fwd_tma_kernel<false>,
-                                                           cudaFuncAttributeMaxDynamicSharedMemorySize, kTmaSmemBytes);
-    static const cudaError_t attr_g = cudaFuncSetAttribute(fwd_tma_kernel<true>,
-                                                           cudaFuncAttributeMaxDynamicSharedMemorySize, kTmaSmemBytes);
+    static const cudaError_t attr_f = cudaFuncSetAttribute(
+        fwd_tma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<false>());
+    static const cudaError_t attr_g = cudaFuncSetAttribute(
+        fwd_tma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<true>());
     DFP_CUDA(attr_f, "cudaFuncSetAttribute");
     DFP_CUDA(attr_g, "cudaFuncSetAttribute");
     time_begin(s);
-    if (!grad) fwd_tma_kernel<false><<<grid, kFwdThreads, kTmaSmemBytes, s>>>(G, dv, vol_map, nullptr, d_out);
-    else fwd_tma_kernel<true><<<grid, kFwdThreads, kTmaSmemBytes, s>>>(G, dv, vol_map, d_up, part);
+    if (!grad)
+      fwd_tma_kernel<false><<<grid, kFwdThreads, tma_smem_bytes<false>(), s>>>(G, dv, map_x, map_y, nullptr, d_out);
+    else
+      fwd_tma_kernel<true><<<grid, kFwdThreads, tma_smem_bytes<true>(), s>>>(G, dv, map_x, map_y, d_up, part);
     time_end(s);
     ++g_launches;
     if (grad) {

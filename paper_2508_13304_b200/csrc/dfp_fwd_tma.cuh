@@ -8,7 +8,7 @@
 //     DESIGN.md O6), so a chunk [kappa0, kappa0 + Kc) is a slab of the frustum; its bounding box in voxel
 //     indices is found from the tile's four corner rays (positions are convex in the pixel index up to the
 //     sagitta of the sphere |r - s| = tau, < 0.01 voxel for a 16-pixel tile; kBoxMargin covers it);
-//   * one elected thread issues `cp.async.bulk.tensor.3d` (TMA, SASS UTMALDG) for the box [kBX x kBY x kBZ]
+//   * one elected thread issues `cp.async.bulk.tensor.3d` (TMA, SASS UTMALDG) for the chunk's box (BoxShape)
 //     straight from the caller's volume: out-of-range elements are ZERO-FILLED by the TMA unit, which is the
 //     zero extension of f~ (U7) - no padded / packed copy of the volume is made on this path;
 //   * two stages, mbarrier (complete_tx) as the "full" signal, __syncthreads as the "empty" signal;
@@ -23,12 +23,21 @@
 
 namespace dfp {
 
-constexpr int kBX = 20, kBY = 20, kBZ = 16;            // staged box (floats); kBX*4 bytes is a multiple of 16
-constexpr int kBXY = kBX * kBY;
-constexpr int kBoxWords = kBX * kBY * kBZ;
-constexpr int kBoxBytes = kBoxWords * 4;               // 25600 = 200 * 128
-constexpr int kStages = 2;
-constexpr int kTmaSmemBytes = kStages * kBoxBytes;     // dynamic shared memory of fwd_tma_kernel
+// Staging boxes (floats).  The x extent times 4 bytes must be a multiple of 16 (TMA inner box).  Pitches of
+// 20 / 28 words spread the rows of a warp's 8x4-pixel footprint over distinct banks (measured 1.4 LDS
+// wavefronts per warp load on C2).
+//   forward : one shape, two stages (a chunk is short: ~12 cycles per warp-sample);
+//   gradient: the stencil needs 2 more cells per axis and a chunk lasts 4x longer, so ONE stage of a longer
+//             box, elongated along the axis the view's rays mostly follow (x- or y-dominant, chosen per view).
+template <bool GRAD, int CLS> struct BoxShape;
+template <> struct BoxShape<false, 0> { static constexpr int X = 20, Y = 20, Z = 16, STAGES = 2; };
+template <> struct BoxShape<false, 1> { static constexpr int X = 20, Y = 20, Z = 16, STAGES = 2; };
+template <> struct BoxShape<true, 0>  { static constexpr int X = 28, Y = 20, Z = 20, STAGES = 1; };
+template <> struct BoxShape<true, 1>  { static constexpr int X = 20, Y = 28, Z = 20, STAGES = 1; };
+template <bool GRAD> constexpr int tma_smem_bytes() {
+  return BoxShape<GRAD, 0>::X * BoxShape<GRAD, 0>::Y * BoxShape<GRAD, 0>::Z * 4 * BoxShape<GRAD, 0>::STAGES;
+}
+constexpr int kMaxStages = 2;
 constexpr float kBoxMargin = 0.05f;                    // voxels: sagitta of the tile + fp32 rounding
 constexpr int kBoxAlignLoss = 3;                       // x cells lost to the 16-byte alignment of the box origin
 
@@ -64,14 +73,16 @@ struct TmaBlock {              // block-wide state in shared memory
   float pm[4][3], dp[4][3];    // the tile's corner rays (centred-index coordinates, as in struct Ray)
   int kA, kB;                  // union of the live rays' kappa ranges [kA, kB)
   int Kc;                      // samples per chunk (0: nothing to do, -1: the box cannot hold the tile)
-  unsigned c0[kStages];        // per-stage index constant: word index = Tx + kBX*Ty + kBXY*Tz + c0
+  unsigned c0[kMaxStages];     // per-stage index constant: word index = Tx + X*Ty + X*Y*Tz + c0
 };
 
 // One chunk's box: origin (voxel indices, for the TMA) and the index constant of the stage it lands in.
-template <bool GRAD>
+template <bool GRAD, int CLS>
 __device__ __forceinline__ void issue_chunk(const VolLayout& L, TmaBlock& B, const CUtensorMap* map, int chunk,
                                             unsigned tiles_addr, unsigned bar_addr) {
-  const int s = chunk % kStages;
+  using S = BoxShape<GRAD, CLS>;
+  constexpr int kWords = S::X * S::Y * S::Z;
+  const int s = chunk % S::STAGES;
   const int k0 = B.kA + chunk * B.Kc;
   const int k1 = min(k0 + B.Kc, B.kB) - 1;
   const float f0 = (float)k0, f1 = (float)k1;
@@ -87,20 +98,133 @@ __device__ __forceinline__ void issue_chunk(const VolLayout& L, TmaBlock& B, con
   // not a multiple of 4 floats raises an illegal-instruction fault): round the x origin down, kBoxAlignLoss
   oc[0] = (((oc[0] + L.hx) >> 2) << 2) - L.hx;
   const unsigned mb = (unsigned)kMagicBits;
-  B.c0[s] = (unsigned)(s * kBoxWords) - ((unsigned)oc[0] + mb) - (unsigned)kBX * ((unsigned)oc[1] + mb) -
-            (unsigned)kBXY * ((unsigned)oc[2] + mb);
+  B.c0[s] = (unsigned)(s * kWords) - ((unsigned)oc[0] + mb) - (unsigned)S::X * ((unsigned)oc[1] + mb) -
+            (unsigned)(S::X * S::Y) * ((unsigned)oc[2] + mb);
   const unsigned bar = bar_addr + 8u * s;
-  mbar_expect_tx(bar, kBoxBytes);
-  tma_load_3d(tiles_addr + (unsigned)(s * kBoxBytes), map, oc[0] + L.hx, oc[1] + L.hy, oc[2] + L.hz, bar);
+  mbar_expect_tx(bar, kWords * 4);
+  tma_load_3d(tiles_addr + (unsigned)(s * kWords * 4), map, oc[0] + L.hx, oc[1] + L.hy, oc[2] + L.hz, bar);
+}
+
+// The chunk loop of one block for one box shape.  acc = {sum} (forward) or {gx,gy,gz,hx,hy,hz} (gradient).
+template <bool GRAD, int CLS>
+__device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* map, const Ray& r, TmaBlock& B,
+                                          const float* tiles, unsigned tiles_addr, unsigned bar_addr, float* acc) {
+  using S = BoxShape<GRAD, CLS>;
+  constexpr int BX = S::X, BXY = S::X * S::Y;
+  if (threadIdx.x == 0) {
+    int Kc = 0;
+    if (B.kA < B.kB) {
+      // chunk length: extent_a <= span_a + (Kc - 1) slope_a must leave room for the floor / stencil cells
+      const float fa = (float)B.kA, fb = (float)(B.kB - 1);
+      const int box[3] = {S::X, S::Y, S::Z};
+      Kc = 4096;
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        float lo0 = 3e38f, hi0 = -3e38f, lo1 = 3e38f, hi1 = -3e38f, slope = 0.f;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          const float q0 = fmaf(fa, B.dp[c][a], B.pm[c][a]), q1 = fmaf(fb, B.dp[c][a], B.pm[c][a]);
+          lo0 = fminf(lo0, q0); hi0 = fmaxf(hi0, q0);
+          lo1 = fminf(lo1, q1); hi1 = fmaxf(hi1, q1);
+          slope = fmaxf(slope, fabsf(B.dp[c][a]));
+        }
+        const float span = fmaxf(hi0 - lo0, hi1 - lo1);
+        const float avail =
+            (float)(box[a] - 4 - (GRAD ? 2 : 0) - (a == 0 ? kBoxAlignLoss : 0)) - 2.f * kBoxMargin - span;
+        if (avail < 0.f) Kc = -1;
+        else if (Kc > 0 && slope > 1e-7f) Kc = min(Kc, (int)floorf(avail / slope) + 1);
+      }
+    }
+    B.Kc = Kc;
+    if (Kc > 0) {
+      const int n_chunks = (B.kB - B.kA + Kc - 1) / Kc;
+#pragma unroll
+      for (int c = 0; c < S::STAGES; ++c)
+        if (c < n_chunks) issue_chunk<GRAD, CLS>(G.L, B, map, c, tiles_addr, bar_addr);
+    }
+  }
+  __syncthreads();
+  const int Kc = B.Kc, kA = B.kA, kB = B.kB;
+  const int n_chunks = Kc > 0 ? (kB - kA + Kc - 1) / Kc : 0;
+  const int kend = r.k0 + r.n;
+
+  float sum = 0.f;
+  float gx = 0.f, gy = 0.f, gz = 0.f, hx = 0.f, hy = 0.f, hz = 0.f;
+  for (int chunk = 0; chunk < n_chunks; ++chunk) {
+    const int s = chunk % S::STAGES;
+    mbar_wait(bar_addr + 8u * s, (unsigned)(chunk / S::STAGES) & 1u);
+    const unsigned c0 = B.c0[s];
+    const int c_lo = kA + chunk * Kc;
+    const int ka = max(c_lo, r.k0), kb = min(min(c_lo + Kc, kB), kend);
+    float kf = (float)ka;
+    for (int k = ka; k < kb; ++k) {
+      const float qx = fmaf(kf, r.dpx, r.pmx), qy = fmaf(kf, r.dpy, r.pmy), qz = fmaf(kf, r.dpz, r.pmz);
+      const float tx = qx + kMagic, ty = qy + kMagic, tz = qz + kMagic;
+      const float ax = (qx - (tx - kMagic)) + 0.5f, ay = (qy - (ty - kMagic)) + 0.5f, az = (qz - (tz - kMagic)) + 0.5f;
+      const unsigned idx = (unsigned)__float_as_int(tx) + (unsigned)BX * (unsigned)__float_as_int(ty) +
+                           (unsigned)BXY * (unsigned)__float_as_int(tz) + c0;
+      const float* c = tiles + idx;
+      if (!GRAD) {
+        const float r00 = lerp(ax, c[0], c[1]), r10 = lerp(ax, c[BX], c[BX + 1]);
+        const float r01 = lerp(ax, c[BXY], c[BXY + 1]), r11 = lerp(ax, c[BXY + BX], c[BXY + BX + 1]);
+        sum += lerp(az, lerp(ay, r00, r10), lerp(ay, r01, r11));
+      } else {
+        float rv[2][2], rdx[2][2];
+#pragma unroll
+        for (int kk = 0; kk < 2; ++kk)
+#pragma unroll
+          for (int j = 0; j < 2; ++j) {
+            const float* row = c + kk * BXY + j * BX;
+            const float m1 = row[-1], v0 = row[0], v1 = row[1], v2 = row[2];
+            rv[j][kk] = lerp(ax, v0, v1);
+            rdx[j][kk] = lerp(ax, v1 - m1, v2 - v0);
+          }
+        float rym[2], ryp[2], rzm[2], rzp[2];
+#pragma unroll
+        for (int kk = 0; kk < 2; ++kk) {
+          const float* m = c + kk * BXY - BX;
+          const float* p = c + kk * BXY + 2 * BX;
+          rym[kk] = lerp(ax, m[0], m[1]);
+          ryp[kk] = lerp(ax, p[0], p[1]);
+        }
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+          const float* m = c + j * BX - BXY;
+          const float* p = c + j * BX + 2 * BXY;
+          rzm[j] = lerp(ax, m[0], m[1]);
+          rzp[j] = lerp(ax, p[0], p[1]);
+        }
+        const float ddx = lerp(az, lerp(ay, rdx[0][0], rdx[1][0]), lerp(ay, rdx[0][1], rdx[1][1]));
+        const float dy0 = lerp(ay, rv[1][0] - rym[0], ryp[0] - rv[0][0]);
+        const float dy1 = lerp(ay, rv[1][1] - rym[1], ryp[1] - rv[0][1]);
+        const float ddy = lerp(az, dy0, dy1);
+        const float dz0 = lerp(az, rv[0][1] - rzm[0], rzp[0] - rv[0][0]);
+        const float dz1 = lerp(az, rv[1][1] - rzm[1], rzp[1] - rv[1][0]);
+        const float ddz = lerp(ay, dz0, dz1);
+        gx += ddx; gy += ddy; gz += ddz;
+        hx = fmaf(kf, ddx, hx); hy = fmaf(kf, ddy, hy); hz = fmaf(kf, ddz, hz);
+      }
+      kf += 1.0f;
+    }
+    __syncthreads();                                   // every thread is done with stage s ("empty")
+    if (threadIdx.x == 0 && chunk + S::STAGES < n_chunks)
+      issue_chunk<GRAD, CLS>(G.L, B, map, chunk + S::STAGES, tiles_addr, bar_addr);
+  }
+  if (!GRAD) {
+    acc[0] = sum;
+  } else {
+    acc[0] = gx; acc[1] = gy; acc[2] = gz; acc[3] = hx; acc[4] = hy; acc[5] = hz;
+  }
 }
 
 template <bool GRAD>
 __global__ void __launch_bounds__(kFwdThreads) fwd_tma_kernel(FwdGeom G, const FwdView* __restrict__ views,
-                                                              const __grid_constant__ CUtensorMap vol_map,
+                                                              const __grid_constant__ CUtensorMap map_x,
+                                                              const __grid_constant__ CUtensorMap map_y,
                                                               const float* __restrict__ upstream,
                                                               float* __restrict__ out) {
-  extern __shared__ __align__(128) float tiles[];      // kStages boxes
-  __shared__ __align__(8) unsigned long long full_bar[kStages];
+  extern __shared__ __align__(128) float tiles[];      // STAGES boxes
+  __shared__ __align__(8) unsigned long long full_bar[kMaxStages];
   __shared__ TmaBlock B;
   __shared__ float red[kFwdThreads / 32][6];
 
@@ -118,7 +242,7 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_tma_kernel(FwdGeom G, const F
     B.kA = 0x7fffffff;
     B.kB = -0x7fffffff;
 #pragma unroll
-    for (int s = 0; s < kStages; ++s) mbar_init(bar_addr + 8u * s, 1);
+    for (int s = 0; s < kMaxStages; ++s) mbar_init(bar_addr + 8u * s, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
@@ -144,111 +268,20 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_tma_kernel(FwdGeom G, const F
     }
   }
   __syncthreads();
-  if (threadIdx.x == 0) {
-    int Kc = 0;
-    if (B.kA < B.kB) {
-      // chunk length: extent_a <= span_a + (Kc - 1) slope_a must leave room for the floor / stencil cells
-      const float fa = (float)B.kA, fb = (float)(B.kB - 1);
-      const int box[3] = {kBX, kBY, kBZ};
-      Kc = 4096;
-#pragma unroll
-      for (int a = 0; a < 3; ++a) {
-        float lo0 = 3e38f, hi0 = -3e38f, lo1 = 3e38f, hi1 = -3e38f, slope = 0.f;
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-          const float q0 = fmaf(fa, B.dp[c][a], B.pm[c][a]), q1 = fmaf(fb, B.dp[c][a], B.pm[c][a]);
-          lo0 = fminf(lo0, q0); hi0 = fmaxf(hi0, q0);
-          lo1 = fminf(lo1, q1); hi1 = fmaxf(hi1, q1);
-          slope = fmaxf(slope, fabsf(B.dp[c][a]));
-        }
-        const float span = fmaxf(hi0 - lo0, hi1 - lo1);
-        const float avail = (float)(box[a] - 4 - (GRAD ? 2 : 0) - (a == 0 ? kBoxAlignLoss : 0)) - 2.f * kBoxMargin - span;
-        if (avail < 0.f) Kc = -1;
-        else if (Kc > 0 && slope > 1e-7f) Kc = min(Kc, (int)floorf(avail / slope) + 1);
-      }
-    }
-    B.Kc = Kc;
-    if (Kc > 0) {
-      const int n_chunks = (B.kB - B.kA + Kc - 1) / Kc;
-      issue_chunk<GRAD>(G.L, B, &vol_map, 0, tiles_addr, bar_addr);
-      if (n_chunks > 1) issue_chunk<GRAD>(G.L, B, &vol_map, 1, tiles_addr, bar_addr);
-    }
-  }
-  __syncthreads();
-  const int Kc = B.Kc, kA = B.kA, kB = B.kB;
-  const int n_chunks = Kc > 0 ? (kB - kA + Kc - 1) / Kc : 0;
-  const int kend = r.k0 + r.n;
+  float acc[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  // box elongated along the axis the tile's rays mostly follow (block-uniform choice)
+  const bool y_dominant = GRAD && fabsf(B.dp[0][1]) > fabsf(B.dp[0][0]);
+  if (!y_dominant) tma_march<GRAD, 0>(G, &map_x, r, B, tiles, tiles_addr, bar_addr, acc);
+  else tma_march<GRAD, 1>(G, &map_y, r, B, tiles, tiles_addr, bar_addr, acc);
 
-  float sum = 0.f;
-  float gx = 0.f, gy = 0.f, gz = 0.f, hx = 0.f, hy = 0.f, hz = 0.f;
-  for (int chunk = 0; chunk < n_chunks; ++chunk) {
-    const int s = chunk % kStages;
-    mbar_wait(bar_addr + 8u * s, (unsigned)(chunk / kStages) & 1u);
-    const unsigned c0 = B.c0[s];
-    const int c_lo = kA + chunk * Kc;
-    const int ka = max(c_lo, r.k0), kb = min(min(c_lo + Kc, kB), kend);
-    float kf = (float)ka;
-    for (int k = ka; k < kb; ++k) {
-      const float qx = fmaf(kf, r.dpx, r.pmx), qy = fmaf(kf, r.dpy, r.pmy), qz = fmaf(kf, r.dpz, r.pmz);
-      const float tx = qx + kMagic, ty = qy + kMagic, tz = qz + kMagic;
-      const float ax = (qx - (tx - kMagic)) + 0.5f, ay = (qy - (ty - kMagic)) + 0.5f, az = (qz - (tz - kMagic)) + 0.5f;
-      const unsigned idx = (unsigned)__float_as_int(tx) + (unsigned)kBX * (unsigned)__float_as_int(ty) +
-                           (unsigned)kBXY * (unsigned)__float_as_int(tz) + c0;
-      const float* c = tiles + idx;
-      if (!GRAD) {
-        const float r00 = lerp(ax, c[0], c[1]), r10 = lerp(ax, c[kBX], c[kBX + 1]);
-        const float r01 = lerp(ax, c[kBXY], c[kBXY + 1]), r11 = lerp(ax, c[kBXY + kBX], c[kBXY + kBX + 1]);
-        sum += lerp(az, lerp(ay, r00, r10), lerp(ay, r01, r11));
-      } else {
-        float rv[2][2], rdx[2][2];
-#pragma unroll
-        for (int kk = 0; kk < 2; ++kk)
-#pragma unroll
-          for (int j = 0; j < 2; ++j) {
-            const float* row = c + kk * kBXY + j * kBX;
-            const float m1 = row[-1], v0 = row[0], v1 = row[1], v2 = row[2];
-            rv[j][kk] = lerp(ax, v0, v1);
-            rdx[j][kk] = lerp(ax, v1 - m1, v2 - v0);
-          }
-        float rym[2], ryp[2], rzm[2], rzp[2];
-#pragma unroll
-        for (int kk = 0; kk < 2; ++kk) {
-          const float* m = c + kk * kBXY - kBX;
-          const float* p = c + kk * kBXY + 2 * kBX;
-          rym[kk] = lerp(ax, m[0], m[1]);
-          ryp[kk] = lerp(ax, p[0], p[1]);
-        }
-#pragma unroll
-        for (int j = 0; j < 2; ++j) {
-          const float* m = c + j * kBX - kBXY;
-          const float* p = c + j * kBX + 2 * kBXY;
-          rzm[j] = lerp(ax, m[0], m[1]);
-          rzp[j] = lerp(ax, p[0], p[1]);
-        }
-        const float ddx = lerp(az, lerp(ay, rdx[0][0], rdx[1][0]), lerp(ay, rdx[0][1], rdx[1][1]));
-        const float dy0 = lerp(ay, rv[1][0] - rym[0], ryp[0] - rv[0][0]);
-        const float dy1 = lerp(ay, rv[1][1] - rym[1], ryp[1] - rv[0][1]);
-        const float ddy = lerp(az, dy0, dy1);
-        const float dz0 = lerp(az, rv[0][1] - rzm[0], rzp[0] - rv[0][0]);
-        const float dz1 = lerp(az, rv[1][1] - rzm[1], rzp[1] - rv[1][0]);
-        const float ddz = lerp(ay, dz0, dz1);
-        gx += ddx; gy += ddy; gz += ddz;
-        hx = fmaf(kf, ddx, hx); hy = fmaf(kf, ddy, hy); hz = fmaf(kf, ddz, hz);
-      }
-      kf += 1.0f;
-    }
-    __syncthreads();                                   // every thread is done with stage s ("empty")
-    if (threadIdx.x == 0 && chunk + kStages < n_chunks)
-      issue_chunk<GRAD>(G.L, B, &vol_map, chunk + kStages, tiles_addr, bar_addr);
-  }
-
-  const float bad = Kc < 0 ? __int_as_float(0x7fc00000) : 0.f;   // NaN marks "box cannot hold the tile" (host bound wrong)
+  const float bad = B.Kc < 0 ? __int_as_float(0x7fc00000) : 0.f;   // NaN: the box cannot hold the tile (host bound wrong)
   if (!GRAD) {
-    if (live) out[((size_t)view * G.nv + iv) * G.nu + iu] = G.step * sum + bad;
+    if (live) out[((size_t)view * G.nv + iv) * G.nu + iu] = G.step * acc[0] + bad;
     return;
   }
   float o6[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   if (live) {
+    const float gx = acc[0], gy = acc[1], gz = acc[2], hx = acc[3], hy = acc[4], hz = acc[5];
     const float w = __ldg(upstream + ((size_t)view * G.nv + iv) * G.nu + iu);
     const float D = G.step;
     const float sx = gx * G.sgx, sy = gy * G.sgy, sz = gz * G.sgz;
