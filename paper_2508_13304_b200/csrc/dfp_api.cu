@@ -115,9 +115,7 @@ bool make_volume_map(const dfp_geometry& g, const float* d_vol, int bx, int by, 
 // Positions at path length tau: p = s' + tau e, so a tile's extent along axis a is tau |De_a| with
 // |De_a| <= (|Dd_a| + |e_a| (rho_max/|d|) |Dd|) / SDD  for pixel offsets Dd on a detector at distance >= SDD.
 constexpr int kMinChunk = 4;
-template <bool GRAD>
-bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V) {
-  const bool grad = GRAD;
+bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V, bool grad, const int* box) {
   const double v3[3] = {g.vx, g.vy, g.vz}, c3[3] = {g.cx, g.cy, g.cz};
   const double half[3] = {0.5 * g.nx * g.vx + 3 * g.vx, 0.5 * g.ny * g.vy + 3 * g.vy, 0.5 * g.nz * g.vz + 3 * g.vz};
   double tau_max = 0;
@@ -142,19 +140,12 @@ bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V) {
   const double rho = std::sqrt(std::fmax(dmax * dmax - sdd * sdd, 0.0)) / sdd;
   const double tu = kFwdTU - 1, tv = kFwdTV - 1;
   const double dnorm = std::hypot(tu * (double)g.du, tv * (double)g.dv);
-  // the kernel picks the box by the first tile's ray direction; a view must fit whichever its tiles may pick
-  const bool may_x = emax[0] >= 0.5 * emax[1] || !GRAD, may_y = GRAD && emax[1] >= 0.5 * emax[0];
-  for (int cls = 0; cls < 2; ++cls) {
-    if ((cls == 0 && !may_x) || (cls == 1 && !may_y)) continue;
-    const int box[3] = {cls ? BoxShape<GRAD, 1>::X : BoxShape<GRAD, 0>::X, cls ? BoxShape<GRAD, 1>::Y : BoxShape<GRAD, 0>::Y,
-                        BoxShape<GRAD, 0>::Z};
   for (int a = 0; a < 3; ++a) {
     const double dd = tu * std::fabs(V.du[a]) + tv * std::fabs(V.dv[a]);
     const double span = tau_max * (dd + emax[a] * rho * dnorm) / sdd / v3[a];
     const double slope = (double)G.step * emax[a] / v3[a];
     const double avail = box[a] - 4 - (grad ? 2 : 0) - (a == 0 ? kBoxAlignLoss : 0) - 2.0 * kBoxMargin - 1.05 * span - 0.05;
     if (avail < (kMinChunk - 1) * slope) return false;
-  }
   }
   return true;
 }
@@ -238,28 +229,37 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
   if (grad) DFP_CUDA(cudaMemcpyAsync(dc, hc.data(), sizeof(FwdContract) * V, cudaMemcpyHostToDevice, s), "view upload");
   const dim3 grid(w.gx, w.gy, V);
   // TMA-staged path when the volume admits a tensor map and every view's tiles fit the staging box
-  CUtensorMap map_x, map_y;
-  bool tma = !(g->flags & DFP_FLAG_NO_TMA);
-  if (tma && !grad)
-    tma = make_volume_map(*g, d_vol, BoxShape<false, 0>::X, BoxShape<false, 0>::Y, BoxShape<false, 0>::Z, &map_x) &&
-          make_volume_map(*g, d_vol, BoxShape<false, 1>::X, BoxShape<false, 1>::Y, BoxShape<false, 1>::Z, &map_y);
-  if (tma && grad)
-    tma = make_volume_map(*g, d_vol, BoxShape<true, 0>::X, BoxShape<true, 0>::Y, BoxShape<true, 0>::Z, &map_x) &&
-          make_volume_map(*g, d_vol, BoxShape<true, 1>::X, BoxShape<true, 1>::Y, BoxShape<true, 1>::Z, &map_y);
-  for (int v = 0; tma && v < V; ++v) tma = grad ? tma_view_fits<true>(*g, G, hv[v]) : tma_view_fits<false>(*g, G, hv[v]);
+  // the smallest staging box (dfp_fwd_tma.cuh) that holds every view's tiles; the gradient uses shape 2 only
+  CUtensorMap vol_map;
+  static const int kBoxes[kNumShapes][3] = {{BoxShape<0>::X, BoxShape<0>::Y, BoxShape<0>::Z},
+                                            {BoxShape<1>::X, BoxShape<1>::Y, BoxShape<1>::Z},
+                                            {BoxShape<2>::X, BoxShape<2>::Y, BoxShape<2>::Z}};
+  int shape = -1;
+  if (!(g->flags & DFP_FLAG_NO_TMA) && (g->nx % 4) == 0) {
+    for (int c = grad ? 2 : 0; c < kNumShapes && shape < 0; ++c) {
+      bool fits = true;
+      for (int v = 0; fits && v < V; ++v) fits = tma_view_fits(*g, G, hv[v], grad, kBoxes[c]);
+      if (fits) shape = c;
+    }
+  }
+  const bool tma = shape >= 0 && make_volume_map(*g, d_vol, kBoxes[shape][0], kBoxes[shape][1], kBoxes[shape][2], &vol_map);
   g_path = tma ? DFP_PATH_TMA : DFP_PATH_GATHER;
   if (tma) {
-    static const cudaError_t attr_f = cudaFuncSetAttribute(
-        fwd_tma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<false>());
-    static const cudaError_t attr_g = cudaFuncSetAttribute(
-        fwd_tma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<true>());
-    DFP_CUDA(attr_f, "cudaFuncSetAttribute");
-    DFP_CUDA(attr_g, "cudaFuncSetAttribute");
+    static const cudaError_t attr[4] = {
+        cudaFuncSetAttribute(fwd_tma_kernel<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<0>()),
+        cudaFuncSetAttribute(fwd_tma_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<1>()),
+        cudaFuncSetAttribute(fwd_tma_kernel<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<2>()),
+        cudaFuncSetAttribute(fwd_tma_kernel<true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<2>())};
+    for (cudaError_t e : attr) DFP_CUDA(e, "cudaFuncSetAttribute");
     time_begin(s);
-    if (!grad)
-      fwd_tma_kernel<false><<<grid, kFwdThreads, tma_smem_bytes<false>(), s>>>(G, dv, map_x, map_y, nullptr, d_out);
+    if (grad)
+      fwd_tma_kernel<true, 2><<<grid, kFwdThreads, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, d_up, part);
+    else if (shape == 0)
+      fwd_tma_kernel<false, 0><<<grid, kFwdThreads, tma_smem_bytes<0>(), s>>>(G, dv, vol_map, nullptr, d_out);
+    else if (shape == 1)
+      fwd_tma_kernel<false, 1><<<grid, kFwdThreads, tma_smem_bytes<1>(), s>>>(G, dv, vol_map, nullptr, d_out);
     else
-      fwd_tma_kernel<true><<<grid, kFwdThreads, tma_smem_bytes<true>(), s>>>(G, dv, map_x, map_y, d_up, part);
+      fwd_tma_kernel<false, 2><<<grid, kFwdThreads, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, nullptr, d_out);
     time_end(s);
     ++g_launches;
     if (grad) {

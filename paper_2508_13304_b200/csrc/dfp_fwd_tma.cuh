@@ -26,16 +26,20 @@ namespace dfp {
 // Staging boxes (floats).  The x extent times 4 bytes must be a multiple of 16 (TMA inner box).  Pitches of
 // 20 / 28 words spread the rows of a warp's 8x4-pixel footprint over distinct banks (measured 1.4 LDS
 // wavefronts per warp load on C2).
-//   forward : one shape, two stages (a chunk is short: ~12 cycles per warp-sample);
-//   gradient: the stencil needs 2 more cells per axis and a chunk lasts 4x longer, so ONE stage of a longer
-//             box, elongated along the axis the view's rays mostly follow (x- or y-dominant, chosen per view).
-template <bool GRAD, int CLS> struct BoxShape;
-template <> struct BoxShape<false, 0> { static constexpr int X = 20, Y = 20, Z = 16, STAGES = 2; };
-template <> struct BoxShape<false, 1> { static constexpr int X = 20, Y = 20, Z = 16, STAGES = 2; };
-template <> struct BoxShape<true, 0>  { static constexpr int X = 28, Y = 20, Z = 20, STAGES = 1; };
-template <> struct BoxShape<true, 1>  { static constexpr int X = 20, Y = 28, Z = 20, STAGES = 1; };
-template <bool GRAD> constexpr int tma_smem_bytes() {
-  return BoxShape<GRAD, 0>::X * BoxShape<GRAD, 0>::Y * BoxShape<GRAD, 0>::Z * 4 * BoxShape<GRAD, 0>::STAGES;
+// The host picks, per call, the smallest shape every view's tiles fit with chunks of >= kMinChunk samples:
+//   shape 0  20 x 20 x 16, two stages : forward, clinical magnification and small pose angles (C2, C4)
+//   shape 1  28 x 20 x 20, two stages : forward, wider tiles / larger tilts (C5)
+//   shape 2  28 x 28 x 20, one stage  : gradient (the stencil needs 2 more cells per axis and a chunk lasts 4x
+//            longer, so one stage suffices; long enough along x and y that views at 45 degrees in the xy plane
+//            still get ~10-sample chunks), and the forward fallback before the gather path.
+// Measured on B200 (Gray-steps/s, forward): C2 625 / 591 / 557, C4 607 / 560 / 548 for shapes 0 / 1 / 2.
+template <int SHAPE> struct BoxShape;
+template <> struct BoxShape<0> { static constexpr int X = 20, Y = 20, Z = 16, STAGES = 2; };
+template <> struct BoxShape<1> { static constexpr int X = 28, Y = 20, Z = 20, STAGES = 2; };
+template <> struct BoxShape<2> { static constexpr int X = 28, Y = 28, Z = 20, STAGES = 1; };
+constexpr int kNumShapes = 3;
+template <int SHAPE> constexpr int tma_smem_bytes() {
+  return BoxShape<SHAPE>::X * BoxShape<SHAPE>::Y * BoxShape<SHAPE>::Z * 4 * BoxShape<SHAPE>::STAGES;
 }
 constexpr int kMaxStages = 2;
 constexpr float kBoxMargin = 0.05f;                    // voxels: sagitta of the tile + fp32 rounding
@@ -77,10 +81,10 @@ struct TmaBlock {              // block-wide state in shared memory
 };
 
 // One chunk's box: origin (voxel indices, for the TMA) and the index constant of the stage it lands in.
-template <bool GRAD, int CLS>
+template <bool GRAD, int SHAPE>
 __device__ __forceinline__ void issue_chunk(const VolLayout& L, TmaBlock& B, const CUtensorMap* map, int chunk,
                                             unsigned tiles_addr, unsigned bar_addr) {
-  using S = BoxShape<GRAD, CLS>;
+  using S = BoxShape<SHAPE>;
   constexpr int kWords = S::X * S::Y * S::Z;
   const int s = chunk % S::STAGES;
   const int k0 = B.kA + chunk * B.Kc;
@@ -106,10 +110,10 @@ __device__ __forceinline__ void issue_chunk(const VolLayout& L, TmaBlock& B, con
 }
 
 // The chunk loop of one block for one box shape.  acc = {sum} (forward) or {gx,gy,gz,hx,hy,hz} (gradient).
-template <bool GRAD, int CLS>
+template <bool GRAD, int SHAPE>
 __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* map, const Ray& r, TmaBlock& B,
                                           const float* tiles, unsigned tiles_addr, unsigned bar_addr, float* acc) {
-  using S = BoxShape<GRAD, CLS>;
+  using S = BoxShape<SHAPE>;
   constexpr int BX = S::X, BXY = S::X * S::Y;
   if (threadIdx.x == 0) {
     int Kc = 0;
@@ -140,7 +144,7 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
       const int n_chunks = (B.kB - B.kA + Kc - 1) / Kc;
 #pragma unroll
       for (int c = 0; c < S::STAGES; ++c)
-        if (c < n_chunks) issue_chunk<GRAD, CLS>(G.L, B, map, c, tiles_addr, bar_addr);
+        if (c < n_chunks) issue_chunk<GRAD, SHAPE>(G.L, B, map, c, tiles_addr, bar_addr);
     }
   }
   __syncthreads();
@@ -208,7 +212,7 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
     }
     __syncthreads();                                   // every thread is done with stage s ("empty")
     if (threadIdx.x == 0 && chunk + S::STAGES < n_chunks)
-      issue_chunk<GRAD, CLS>(G.L, B, map, chunk + S::STAGES, tiles_addr, bar_addr);
+      issue_chunk<GRAD, SHAPE>(G.L, B, map, chunk + S::STAGES, tiles_addr, bar_addr);
   }
   if (!GRAD) {
     acc[0] = sum;
@@ -217,10 +221,9 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
   }
 }
 
-template <bool GRAD>
+template <bool GRAD, int SHAPE>
 __global__ void __launch_bounds__(kFwdThreads) fwd_tma_kernel(FwdGeom G, const FwdView* __restrict__ views,
-                                                              const __grid_constant__ CUtensorMap map_x,
-                                                              const __grid_constant__ CUtensorMap map_y,
+                                                              const __grid_constant__ CUtensorMap vol_map,
                                                               const float* __restrict__ upstream,
                                                               float* __restrict__ out) {
   extern __shared__ __align__(128) float tiles[];      // STAGES boxes
@@ -269,10 +272,7 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_tma_kernel(FwdGeom G, const F
   }
   __syncthreads();
   float acc[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-  // box elongated along the axis the tile's rays mostly follow (block-uniform choice)
-  const bool y_dominant = GRAD && fabsf(B.dp[0][1]) > fabsf(B.dp[0][0]);
-  if (!y_dominant) tma_march<GRAD, 0>(G, &map_x, r, B, tiles, tiles_addr, bar_addr, acc);
-  else tma_march<GRAD, 1>(G, &map_y, r, B, tiles, tiles_addr, bar_addr, acc);
+  tma_march<GRAD, SHAPE>(G, &vol_map, r, B, tiles, tiles_addr, bar_addr, acc);
 
   const float bad = B.Kc < 0 ? __int_as_float(0x7fc00000) : 0.f;   // NaN: the box cannot hold the tile (host bound wrong)
   if (!GRAD) {
