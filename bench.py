@@ -317,9 +317,12 @@ def main():
     alu_peak = N_SM * LANES_PER_SM * pk.get("sm_max_mhz", 1965.0) * 1e6 / 1e12          # Tera lane-ops/s
     achieved = OPS_PER_UNIT[dom] * units[dom] / (mean_ms[dom] * 1e-3) / 1e12
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    tp = os.path.join(ROOT, "profiles", "traffic.csv")     # dram__bytes_read+write per launch from the ncu --set full capture
     if os.path.exists(tp):
-        traffic = json.load(open(tp)).get(f"C{args.config}", {}).get(dom)
+        import csv
+        for row in csv.DictReader(open(tp)):
+            if row["config"] == f"C{args.config}" and row["kernel"] == dom:
+                traffic = int(row["dram_bytes_per_launch"])
     roofline = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": alu_peak, "unit": "Tlane-op/s",
                 "frac": achieved / alu_peak, "traffic": traffic,
                 "peak_source": f"148 SMs x 128 fp32 lanes x sm_max_mhz ({pk_kind} MEASURED_PEAKS.json clock)",
