@@ -169,7 +169,7 @@ FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad) {
   return w;
 }
 
-constexpr int kBpGradZChunk = 64;
+constexpr int kBpGradZChunk = 16;
 struct BpWs {
   size_t off_views, off_con, off_q, off_part, total;
   int gx, gy, gz;  // voxel tiles
