@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "../../include/dfp.h"
+#include "dfp_bp_tma.cuh"
 #include "dfp_fwd_tma.cuh"
 #include "dfp_kernels.cuh"
 #include "dfp_params.h"
@@ -150,6 +151,55 @@ bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V, bo
   return true;
 }
 
+// ---- TMA path of the back-projection kernels (dfp_bp_tma.cuh) -----------------------------------
+// Tensor maps over the caller's projections [V][nv][nu] fp32, one per patch of the menu up to kmax.
+bool make_proj_maps(const dfp_geometry& g, int V, const float* d_proj, int kmax, PatchMaps* maps) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc || (g.nu % 4) != 0) return false;
+  const cuuint64_t dims[3] = {(cuuint64_t)g.nu, (cuuint64_t)g.nv, (cuuint64_t)V};
+  const cuuint64_t strides[2] = {(cuuint64_t)g.nu * 4, (cuuint64_t)g.nu * g.nv * 4};
+  const cuuint32_t es[3] = {1, 1, 1};
+  for (int k = 0; k < kNumPatches; ++k) {
+    const int kk = k <= kmax ? k : kmax;                 // unused slots repeat the largest map
+    const cuuint32_t box[3] = {(cuuint32_t)kPatchUHost[kk], (cuuint32_t)kPatchVHost[kk], 1};
+    if (enc(&maps->m[k], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(d_proj), dims, strides, box, es,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return false;
+  }
+  return true;
+}
+
+// Smallest patch of the menu that is guaranteed to hold the footprint of every 16 x 16 x tz voxel tile in this
+// view (-1: none, or a voxel is not in front of the source - then the gather path, which handles w' <= 0, runs).
+// For two voxels r, r+D of a tile: |Du| <= (|A0.D| + |u| |A2.D|) / w'(r+D)  with u = A0.r / A2.r  (exact).
+int bp_view_patch(const BpGeom& G, const BpView& Vw, int tz, int halo) {
+  const double lo[3] = {-(double)G.hx, -(double)G.hy, -(double)G.hz};
+  const double hi[3] = {G.nx - 1 - (double)G.hx, G.ny - 1 - (double)G.hy, G.nz - 1 - (double)G.hz};
+  double wmin = 1e300, umax = 0, vmax = 0, wmax = 0;
+  for (int c = 0; c < 8; ++c) {
+    const double x = (c & 1) ? hi[0] : lo[0], y = (c & 2) ? hi[1] : lo[1], z = (c & 4) ? hi[2] : lo[2];
+    const double u = Vw.A[0][0] * x + Vw.A[0][1] * y + Vw.A[0][2] * z + Vw.A[0][3];
+    const double v = Vw.A[1][0] * x + Vw.A[1][1] * y + Vw.A[1][2] * z + Vw.A[1][3];
+    const double w = Vw.A[2][0] * x + Vw.A[2][1] * y + Vw.A[2][2] * z + Vw.A[2][3];
+    if (!(w > 0)) return -1;
+    wmin = std::fmin(wmin, w); wmax = std::fmax(wmax, w);
+    umax = std::fmax(umax, std::fabs(u / w)); vmax = std::fmax(vmax, std::fabs(v / w));
+  }
+  if (!(wmin > 0.02 * wmax)) return -1;
+  const double T[3] = {(double)(kBpT - 1), (double)(kBpT - 1), (double)(tz - 1)};
+  double eu = 0, ev = 0;
+  for (int a = 0; a < 3; ++a) {
+    eu += (std::fabs(Vw.A[0][a]) + umax * std::fabs(Vw.A[2][a])) * T[a] / wmin;
+    ev += (std::fabs(Vw.A[1][a]) + vmax * std::fabs(Vw.A[2][a])) * T[a] / wmin;
+  }
+  const int need_u = (int)std::ceil(eu + 2 * kPatchMargin) + 3 + 2 * halo + 3;   // floor cells, stencil, alignment
+  const int need_v = (int)std::ceil(ev + 2 * kPatchMargin) + 3 + 2 * halo;
+  for (int k = 0; k < kNumPatches; ++k)
+    if (need_u <= kPatchUHost[k] && need_v <= kPatchVHost[k]) return k;
+  return -1;
+}
+
 // ---- workspace carving ---------------------------------------------------------------------------
 struct FwdWs {
   size_t off_views, off_con, off_pvol, off_part, total;
@@ -172,18 +222,27 @@ FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad) {
 constexpr int kBpGradZChunk = 16;
 struct BpWs {
   size_t off_views, off_con, off_q, off_part, total;
-  int gx, gy, gz;  // voxel tiles
+  int gx, gy, gz;  // voxel tiles (gather path)
+  int tx, ty, tz;  // voxel tiles (TMA path)
 };
 BpWs bp_ws(const dfp_geometry& g, int V, bool grad) {
   BpWs w;
   w.gx = (g.nx + kBpTX - 1) / kBpTX;
   w.gy = (g.ny + kBpTY - 1) / kBpTY;
   w.gz = grad ? (g.nz + kBpGradZChunk - 1) / kBpGradZChunk : (g.nz + kBpZ - 1) / kBpZ;
+  // tiles of the TMA path: 16 x 16 x (16 or 8) voxels; sized for the finer tiling
+  w.tx = (g.nx + kBpT - 1) / kBpT;
+  w.ty = (g.ny + kBpT - 1) / kBpT;
+  w.tz = (g.nz + 7) / 8;
   size_t o = 0;
   w.off_views = o; o += align_up(sizeof(BpView) * (size_t)V);
   w.off_con = o;   o += grad ? align_up(sizeof(BpContract) * (size_t)V) : 0;
   w.off_q = o;     o += align_up(sizeof(float4) * (size_t)V * (g.nu + 2 * kPadDet) * (g.nv + 2 * kPadDet));
-  w.off_part = o;  o += grad ? align_up(sizeof(float) * 6 * (size_t)V * w.gx * w.gy * w.gz) : 0;
+  w.off_part = o;
+  {
+    const size_t t_gather = (size_t)w.gx * w.gy * w.gz, t_tma = (size_t)w.tx * w.ty * w.tz;
+    o += grad ? align_up(sizeof(float) * 6 * (size_t)V * (t_gather > t_tma ? t_gather : t_tma)) : 0;
+  }
   w.total = o;
   return w;
 }
@@ -310,6 +369,58 @@ int run_backproject(const dfp_geometry* g, int V, const float* angles, const flo
   g_path = DFP_PATH_GATHER;
   DFP_CUDA(cudaMemcpyAsync(dv, hv.data(), sizeof(BpView) * V, cudaMemcpyHostToDevice, s), "view upload");
   if (grad) DFP_CUDA(cudaMemcpyAsync(dc, hc.data(), sizeof(BpContract) * V, cudaMemcpyHostToDevice, s), "view upload");
+  // TMA-staged path: projections admit a tensor map, every voxel in front of the source, patches fit the menu
+  int kmax = -1, TZ = 16;
+  if (!(g->flags & DFP_FLAG_NO_TMA) && (g->nu % 4) == 0) {
+    for (TZ = 16; TZ >= 8 && kmax < 0; TZ >>= 1) {
+      kmax = 0;
+      for (int v = 0; v < V && kmax >= 0; ++v) {
+        const int k = bp_view_patch(G, hv[v], TZ, grad ? 1 : 0);
+        kmax = k < 0 ? -1 : (k > kmax ? k : kmax);
+      }
+      if (kmax >= 0 && bp_num_stages(kmax) < 2) kmax = -1;      // a single stage would serialise TMA and compute
+      if (kmax >= 0) break;
+    }
+  }
+  PatchMaps maps;
+  if (kmax >= 0 && make_proj_maps(*g, V, d_proj, kmax, &maps)) {
+    const int stage_words = bp_stage_words(kmax), n_stages = bp_num_stages(kmax);
+    const int smem = stage_words * 4 * n_stages;
+#define DFP_BP_ATTR(k) cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, kBpSmemBudget)
+    static const cudaError_t attr[10] = {
+        DFP_BP_ATTR((bp_tma_kernel<0, 16>)), DFP_BP_ATTR((bp_tma_kernel<1, 16>)), DFP_BP_ATTR((bp_tma_kernel<0, 8>)),
+        DFP_BP_ATTR((bp_tma_kernel<1, 8>)), DFP_BP_ATTR((bp_grad_tma_kernel<0, 0, 16>)),
+        DFP_BP_ATTR((bp_grad_tma_kernel<1, 0, 16>)), DFP_BP_ATTR((bp_grad_tma_kernel<1, 1, 16>)),
+        DFP_BP_ATTR((bp_grad_tma_kernel<0, 0, 8>)), DFP_BP_ATTR((bp_grad_tma_kernel<1, 0, 8>)),
+        DFP_BP_ATTR((bp_grad_tma_kernel<1, 1, 8>))};
+#undef DFP_BP_ATTR
+    for (cudaError_t e : attr) DFP_CUDA(e, "cudaFuncSetAttribute");
+    const dim3 tgrid(w.tx, w.ty, (g->nz + TZ - 1) / TZ);
+    g_path = DFP_PATH_TMA;
+#define DFP_BP_ARGS <<<tgrid, kBpTmaThreads, smem, s>>>(G, V, dv, maps, kmax, stage_words, n_stages
+    time_begin(s);
+    if (!grad) {
+      if (G.bp_weight) { if (TZ == 16) bp_tma_kernel<1, 16> DFP_BP_ARGS, d_out); else bp_tma_kernel<1, 8> DFP_BP_ARGS, d_out); }
+      else { if (TZ == 16) bp_tma_kernel<0, 16> DFP_BP_ARGS, d_out); else bp_tma_kernel<0, 8> DFP_BP_ARGS, d_out); }
+      time_end(s);
+      ++g_launches;
+    } else {
+      const bool dw = G.bp_weight && (G.flags & DFP_FLAG_DW);
+      if (!G.bp_weight) {
+        if (TZ == 16) bp_grad_tma_kernel<0, 0, 16> DFP_BP_ARGS, d_up, part); else bp_grad_tma_kernel<0, 0, 8> DFP_BP_ARGS, d_up, part);
+      } else if (!dw) {
+        if (TZ == 16) bp_grad_tma_kernel<1, 0, 16> DFP_BP_ARGS, d_up, part); else bp_grad_tma_kernel<1, 0, 8> DFP_BP_ARGS, d_up, part);
+      } else {
+        if (TZ == 16) bp_grad_tma_kernel<1, 1, 16> DFP_BP_ARGS, d_up, part); else bp_grad_tma_kernel<1, 1, 8> DFP_BP_ARGS, d_up, part);
+      }
+      time_end(s);
+      bp_contract_kernel<<<V, 256, 0, s>>>(tgrid.x * tgrid.y * tgrid.z, V, part, dc, d_out);
+      g_launches += 2;
+    }
+#undef DFP_BP_ARGS
+    DFP_CUDA(cudaGetLastError(), "back-projection launch (TMA path)");
+    return DFP_OK;
+  }
   const size_t ncell = (size_t)V * G.pu * G.pv;
   pack_proj_kernel<<<grid_1d(ncell, 256), 256, 0, s>>>(G.nu, G.nv, G.pu, G.pv, (size_t)V, d_proj, q);
   ++g_launches;

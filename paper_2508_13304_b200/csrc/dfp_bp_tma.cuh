@@ -1,0 +1,348 @@
+// dfp_bp_tma.cuh - a6 / a7 with the detector patch of each (voxel tile, view) staged in shared memory by TMA.
+//
+// Same arithmetic, voxel for voxel, as bp_kernel / bp_grad_kernel (dfp_kernels.cuh), but the 4 (back-projection)
+// or 12 (gradient) pixel reads of a (voxel, view) pair are LDS from a box of that view's projection:
+//
+//   * a block owns a tile of 16 x 16 x TZ voxels and loops over ALL views (the volume is written once, a6; the
+//     per-view 6-vectors of the tile are reduced in the block, a7/a8);
+//   * the image of a convex box under the projective map of Eq.1 is the convex hull of its 8 projected corners
+//     (all w' > 0 - the host takes this path only then), so the tile's footprint on the detector is the min/max
+//     of 8 corner projections: a PRODUCER warp computes it per view (lanes 0-7 one corner each, shuffle min/max),
+//     copies the view's P_eff rows next to the stage and issues ONE `cp.async.bulk.tensor.3d` (SASS UTMALDG) for
+//     the box [1][BV][BU] of the caller's projections - out-of-detector pixels are ZERO-FILLED by the TMA unit,
+//     which is the zero extension of b~ (U7): no packed copy, no clamps in the inner loop;
+//   * STAGES boxes in flight; "full" = mbarrier with complete_tx, "empty" = mbarrier the 8 consumer warps arrive on.
+// PAPER.md Eq.1 :60-63, Eq.21 :193-196 (back-projection); Eq.12-17 :139-168, Eq.22 :198-206 (its pose gradient).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include "dfp_fwd_tma.cuh"
+#include "dfp_kernels.cuh"
+
+namespace dfp {
+
+constexpr int kBpT = 16;                         // voxel tile in x and in y (one consumer thread per column)
+constexpr int kBpConsumers = kBpT * kBpT;        // 256 consumer threads = 8 warps
+constexpr int kBpTmaThreads = kBpConsumers + 32; // + 1 producer warp
+constexpr float kPatchMargin = 0.05f;            // pixels: fp32 rounding of the per-voxel projection
+
+// Detector patch menu (floats): U x V, every U a multiple of 4 (TMA inner box) and = 4 or 20 mod 32, so that
+// consecutive detector rows of a patch start 4 banks apart (U = 32, 64, 96 put all rows on the same banks:
+// measured 1.97 LDS wavefronts per warp load on C3 against 1.3 with these pitches).  The host bounds the largest
+// patch any (tile, view) of the call can need and sizes the stages for it; the producer then picks, per (tile,
+// view), the SMALLEST patch that holds the actual footprint, so the bytes the TMA unit moves follow the local
+// magnification instead of the worst case (near-source tiles and rotated views need 2-4x the median patch).
+constexpr int kNumPatches = 6;
+__device__ __constant__ int kPatchU[kNumPatches] = {36, 52, 68, 68, 100, 100};
+__device__ __constant__ int kPatchV[kNumPatches] = {16, 24, 32, 48, 64, 80};
+static const int kPatchUHost[kNumPatches] = {36, 52, 68, 68, 100, 100};
+static const int kPatchVHost[kNumPatches] = {16, 24, 32, 48, 64, 80};
+struct alignas(64) PatchMaps { CUtensorMap m[kNumPatches]; };
+constexpr int kPatchHeader = 32;                 // floats per stage in front of the patch: P_eff rows, c0, pitch, status
+constexpr int kBpMaxStages = 4;
+constexpr int kBpSmemBudget = 72 * 1024;         // dynamic shared memory per block: 3 blocks per SM
+inline int bp_stage_words(int kmax) { return kPatchUHost[kmax] * kPatchVHost[kmax] + kPatchHeader; }
+inline int bp_num_stages(int kmax) {
+  const int n = kBpSmemBudget / (bp_stage_words(kmax) * 4);
+  return n > kBpMaxStages ? kBpMaxStages : n;
+}
+
+__device__ __forceinline__ void mbar_arrive(unsigned bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kBpConsumers) : "memory"); }
+
+// Stage header layout (floats): [0..11] A rows (P_eff on centred voxel indices, u and v rows minus half the w row),
+// [12..20] J rows (gradient only), [24] c0b (as bits; see patch_locate), [25] status (as bits: 0 ok, 1 no patch
+// of the menu fits), [26] row pitch of the patch in BYTES (as bits).
+struct BpTile {
+  int x0, y0, z0, tz;          // first voxel of the tile and its z extent (<= TZ)
+};
+
+// Producer: footprint of the tile in view `view`, header, TMA.  Called by the whole producer warp.
+template <int HALO>
+__device__ __forceinline__ void bp_issue_view(const BpGeom& G, const BpTile& T, const BpView* __restrict__ views,
+                                              const PatchMaps* maps, int kmax, int stage_words, int view, int stage,
+                                              float* smem, unsigned smem_addr, unsigned full_addr) {
+  const int lane = threadIdx.x & 31;
+  float* hdr = smem + stage * stage_words;
+  const float* src = reinterpret_cast<const float*>(views + view);
+  if (lane < (int)(sizeof(BpView) / 4)) hdr[lane] = __ldg(src + lane);
+  // corner (lane & 7) of the tile, centred voxel indices
+  const int cx = T.x0 + ((lane & 1) ? kBpT - 1 : 0), cy = T.y0 + ((lane & 2) ? kBpT - 1 : 0),
+            cz = T.z0 + ((lane & 4) ? T.tz - 1 : 0);
+  const float xf = (float)min(cx, G.nx - 1) - G.hx, yf = (float)min(cy, G.ny - 1) - G.hy, zf = (float)cz - G.hz;
+  const float* A = src;
+  const float up = fmaf(__ldg(A + 0), xf, fmaf(__ldg(A + 1), yf, fmaf(__ldg(A + 2), zf, __ldg(A + 3))));
+  const float vp = fmaf(__ldg(A + 4), xf, fmaf(__ldg(A + 5), yf, fmaf(__ldg(A + 6), zf, __ldg(A + 7))));
+  const float wp = fmaf(__ldg(A + 8), xf, fmaf(__ldg(A + 9), yf, fmaf(__ldg(A + 10), zf, __ldg(A + 11))));
+  const float rw = fast_rcp(wp);
+  float ulo = up * rw, vlo = vp * rw, uhi = ulo, vhi = vlo;
+#pragma unroll
+  for (int o = 4; o > 0; o >>= 1) {
+    ulo = fminf(ulo, __shfl_xor_sync(0xffffffffu, ulo, o));
+    uhi = fmaxf(uhi, __shfl_xor_sync(0xffffffffu, uhi, o));
+    vlo = fminf(vlo, __shfl_xor_sync(0xffffffffu, vlo, o));
+    vhi = fmaxf(vhi, __shfl_xor_sync(0xffffffffu, vhi, o));
+  }
+  __syncwarp();                                                  // header words written by lanes 0..20
+  if (lane == 0) {
+    // cells floor(u - CU) = rint(uq) in [rint(lo), rint(hi)], stencil [-HALO, 1 + HALO]
+    int ou = (int)floorf(ulo - 0.5f - kPatchMargin) - HALO, ov = (int)floorf(vlo - 0.5f - kPatchMargin) - HALO;
+    ou = (((ou + G.CU) >> 2) << 2) - G.CU;                       // 16-byte alignment of the TMA inner coordinate
+    const int eu = (int)floorf(uhi + 0.5f + kPatchMargin) + 1 + HALO - ou + 1;
+    const int ev = (int)floorf(vhi + 0.5f + kPatchMargin) + 1 + HALO - ov + 1;
+    int k = 0;
+    while (k <= kmax && (eu > kPatchU[k] || ev > kPatchV[k])) ++k;
+    const bool ok = k <= kmax && ulo == ulo && vlo == vlo;
+    if (!ok) k = 0;
+    const int U = kPatchU[k], V = kPatchV[k];
+    const unsigned mb = (unsigned)kMagicBits;
+    const unsigned c0b = smem_addr + 4u * ((unsigned)(stage * stage_words + kPatchHeader) - ((unsigned)ou + mb) -
+                                           (unsigned)U * ((unsigned)ov + mb));
+    hdr[24] = __uint_as_float(c0b);
+    hdr[25] = __uint_as_float(ok ? 0u : 1u);
+    hdr[26] = __uint_as_float(4u * (unsigned)U);
+    const unsigned bar = full_addr + 8u * stage;
+    mbar_expect_tx(bar, U * V * 4);
+    // a footprint no patch holds (host bound wrong; never in the tested configs) still loads a patch - from a
+    // far corner, all zeros - so that the barrier protocol stays uniform; the consumers write NaN for it
+    tma_load_3d(smem_addr + (unsigned)((stage * stage_words + kPatchHeader) * 4), &maps->m[k],
+                ok ? ou + G.CU : -4096, ok ? ov + G.CV : -4096, view, bar);
+  }
+}
+
+// Pixel cell and fractions of one (voxel, view) pair inside the staged patch (no clamps: the patch holds the
+// tile's whole footprint plus the stencil halo, and out-of-detector pixels were zero-filled).
+// `addr` is the SHARED-space byte address of pixel (floor u, floor v): 4*Tu + 4*pitch*Tv + c0b, two IMADs on the
+// magic-rounded float bits (c0b folds the stage base, the patch origin and the magic bias).
+struct PatchPix {
+  float a, b, rw, uq, vq;
+  unsigned addr;
+};
+__device__ __forceinline__ PatchPix patch_locate(float up, float vp, float wp, unsigned c0b, unsigned pitch4) {
+  PatchPix o;
+  o.rw = fast_rcp(wp);
+  o.uq = up * o.rw;
+  o.vq = vp * o.rw;
+  const float tu = o.uq + kMagic, tv = o.vq + kMagic;
+  o.a = (o.uq - (tu - kMagic)) + 0.5f;
+  o.b = (o.vq - (tv - kMagic)) + 0.5f;
+  o.addr = 4u * (unsigned)__float_as_int(tu) + pitch4 * (unsigned)__float_as_int(tv) + c0b;
+  return o;
+}
+template <int OFF>
+__device__ __forceinline__ float lds_f32(unsigned addr) {
+  float v;
+  asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v) : "r"(addr), "n"(OFF));
+  return v;
+}
+
+// ------------------------------------------------------------------------------------------------ a6 back
+// TZ = voxels along z per thread (register accumulators): 16, or 8 where the magnification is so large that a
+// 16-deep tile's footprint exceeds the patch menu (C2: 2.5-3 pixels per voxel).
+template <int WEIGHT, int TZ>
+__global__ void __launch_bounds__(kBpTmaThreads) bp_tma_kernel(BpGeom G, int n_views, const BpView* __restrict__ views,
+                                                               const __grid_constant__ PatchMaps maps, int kmax,
+                                                               int stage_words, int n_stages, float* __restrict__ vol) {
+  extern __shared__ __align__(128) float smem[];
+  __shared__ __align__(8) unsigned long long bars[2 * kBpMaxStages];  // full[], empty[]
+  const unsigned smem_addr = smem_u32(smem), full_addr = smem_u32(bars), empty_addr = full_addr + 8u * kBpMaxStages;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  BpTile T;
+  T.x0 = blockIdx.x * kBpT; T.y0 = blockIdx.y * kBpT; T.z0 = blockIdx.z * TZ;
+  T.tz = min(TZ, G.nz - T.z0);
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int s = 0; s < kBpMaxStages; ++s) {
+      mbar_init(full_addr + 8u * s, 1);
+      mbar_init(empty_addr + 8u * s, kBpConsumers / 32);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+  if (warp == kBpConsumers / 32) {                      // ---- producer warp
+    for (int view = 0; view < n_views; ++view) {
+      const int s = view % n_stages;
+      mbar_wait(empty_addr + 8u * s, ((unsigned)(view / n_stages) & 1u) ^ 1u);
+      bp_issue_view<0>(G, T, views, &maps, kmax, stage_words, view, s, smem, smem_addr, full_addr);
+    }
+    return;
+  }
+  // ---- consumers: thread = one (x, y) column of the tile, TZ voxels along z in registers
+  const int ix = T.x0 + (threadIdx.x & (kBpT - 1)), iy = T.y0 + threadIdx.x / kBpT;
+  const bool live = ix < G.nx && iy < G.ny;
+  const float xf = (float)ix - G.hx, yf = (float)iy - G.hy, zf = (float)T.z0 - G.hz;
+  float acc[TZ];
+#pragma unroll
+  for (int m = 0; m < TZ; ++m) acc[m] = 0.f;
+  bool bad = false;
+  for (int view = 0; view < n_views; ++view) {
+    const int s = view % n_stages;
+    mbar_wait(full_addr + 8u * s, (unsigned)(view / n_stages) & 1u);
+    const float* hdr = smem + s * stage_words;
+    const unsigned c0 = __float_as_uint(hdr[24]), BU = __float_as_uint(hdr[26]);
+    bad |= __float_as_uint(hdr[25]) != 0u;
+    if (live) {
+      const float a02 = hdr[2], a12 = hdr[6], a22 = hdr[10];
+      const float ub = fmaf(hdr[0], xf, fmaf(hdr[1], yf, fmaf(a02, zf, hdr[3])));
+      const float vb = fmaf(hdr[4], xf, fmaf(hdr[5], yf, fmaf(a12, zf, hdr[7])));
+      const float wb = fmaf(hdr[8], xf, fmaf(hdr[9], yf, fmaf(a22, zf, hdr[11])));
+#pragma unroll
+      for (int m = 0; m < TZ; ++m) {
+        if (m < T.tz) {
+          const float mf = (float)m;
+          const PatchPix p = patch_locate(fmaf(mf, a02, ub), fmaf(mf, a12, vb), fmaf(mf, a22, wb), c0, BU);
+          const unsigned a1 = p.addr + BU;
+          const float val = lerp(p.b, lerp(p.a, lds_f32<0>(p.addr), lds_f32<4>(p.addr)),
+                                 lerp(p.a, lds_f32<0>(a1), lds_f32<4>(a1)));
+          const float wgt = WEIGHT ? G.sad2 * p.rw * p.rw : 1.f;
+          acc[m] = fmaf(wgt, val, acc[m]);
+        }
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(empty_addr + 8u * s);
+  }
+  if (live) {
+    const float nanv = bad ? __int_as_float(0x7fc00000) : 0.f;
+#pragma unroll
+    for (int m = 0; m < TZ; ++m)
+      if (m < T.tz) vol[((size_t)(T.z0 + m) * G.ny + iy) * G.nx + ix] = acc[m] + nanv;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ a7 back gradient
+// Per (voxel j, view), as bp_grad_kernel: q' = W [ d~_u l (J1 - u J3) + d~_v l (J2 - v J3) ] / w' (+ b~ dW/dr'),
+// six running sums per (thread, view) along the thread's z column with the lever arm factored out.  Per view the
+// warp's sums are shuffled together; the 8 warps' results wait in shared memory (two buffers of kBpGradGroup views)
+// and are added in fixed order once per group -> partials[tile][view][6]: one consumer barrier per group, not per view.
+constexpr int kBpGradGroup = 8;                  // views per cross-warp reduction
+
+template <int WEIGHT, int DW, int TZ>
+__global__ void __launch_bounds__(kBpTmaThreads) bp_grad_tma_kernel(BpGeom G, int n_views,
+                                                                    const BpView* __restrict__ views,
+                                                                    const __grid_constant__ PatchMaps maps, int kmax,
+                                                                    int stage_words, int n_stages,
+                                                                    const float* __restrict__ upstream,
+                                                                    float* __restrict__ partials) {
+  constexpr int NW = kBpConsumers / 32;
+  extern __shared__ __align__(128) float smem[];
+  __shared__ __align__(8) unsigned long long bars[2 * kBpMaxStages];
+  __shared__ float wpart[2][kBpGradGroup][NW][6];
+  const unsigned smem_addr = smem_u32(smem), full_addr = smem_u32(bars), empty_addr = full_addr + 8u * kBpMaxStages;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  BpTile T;
+  T.x0 = blockIdx.x * kBpT; T.y0 = blockIdx.y * kBpT; T.z0 = blockIdx.z * TZ;
+  T.tz = min(TZ, G.nz - T.z0);
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int s = 0; s < kBpMaxStages; ++s) {
+      mbar_init(full_addr + 8u * s, 1);
+      mbar_init(empty_addr + 8u * s, NW);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+  if (warp == NW) {                                     // ---- producer warp
+    for (int view = 0; view < n_views; ++view) {
+      const int s = view % n_stages;
+      mbar_wait(empty_addr + 8u * s, ((unsigned)(view / n_stages) & 1u) ^ 1u);
+      bp_issue_view<1>(G, T, views, &maps, kmax, stage_words, view, s, smem, smem_addr, full_addr);
+    }
+    return;
+  }
+  // ---- consumers
+  const int ix = T.x0 + (threadIdx.x & (kBpT - 1)), iy = T.y0 + threadIdx.x / kBpT;
+  const bool live = ix < G.nx && iy < G.ny;
+  const float xf = (float)ix - G.hx, yf = (float)iy - G.hy, zf = (float)T.z0 - G.hz;
+  const float rx = G.cx + xf * G.vx, ry = G.cy + yf * G.vy, rz = G.cz + zf * G.vz;   // object-frame mm, first voxel
+  const float* wcol = upstream + ((size_t)T.z0 * G.ny + (live ? iy : 0)) * G.nx + (live ? ix : 0);
+  const size_t wstride = (size_t)G.ny * G.nx;
+  const size_t tile = ((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+  bool bad = false;
+  const int n_groups = (n_views + kBpGradGroup - 1) / kBpGradGroup;
+  for (int grp = 0; grp < n_groups; ++grp) {
+    const int v_lo = grp * kBpGradGroup, v_hi = min(v_lo + kBpGradGroup, n_views);
+    for (int view = v_lo; view < v_hi; ++view) {
+      const int s = view % n_stages;
+      mbar_wait(full_addr + 8u * s, (unsigned)(view / n_stages) & 1u);
+      const float* hdr = smem + s * stage_words;
+      const unsigned c0 = __float_as_uint(hdr[24]), BU = __float_as_uint(hdr[26]);
+      bad |= __float_as_uint(hdr[25]) != 0u;
+      float sm[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+      if (live) {
+        const float a02 = hdr[2], a12 = hdr[6], a22 = hdr[10];
+        const float ub = fmaf(hdr[0], xf, fmaf(hdr[1], yf, fmaf(a02, zf, hdr[3])));
+        const float vb = fmaf(hdr[4], xf, fmaf(hdr[5], yf, fmaf(a12, zf, hdr[7])));
+        const float wb = fmaf(hdr[8], xf, fmaf(hdr[9], yf, fmaf(a22, zf, hdr[11])));
+        const float j00 = hdr[12], j01 = hdr[13], j02 = hdr[14], j10 = hdr[15], j11 = hdr[16], j12 = hdr[17],
+                    j20 = hdr[18], j21 = hdr[19], j22 = hdr[20];
+        float mf = 0.f;
+        for (int m = 0; m < T.tz; ++m) {
+          const PatchPix p = patch_locate(fmaf(mf, a02, ub), fmaf(mf, a12, vb), fmaf(mf, a22, wb), c0, BU);
+          // rows v, v+1: columns u-1 .. u+2; rows v-1, v+2: columns u, u+1
+          const unsigned a0 = p.addr, a1 = a0 + BU, am = a0 - BU, a2 = a1 + BU;
+          const float l0m = lds_f32<-4>(a0), l00 = lds_f32<0>(a0), l01 = lds_f32<4>(a0), l02 = lds_f32<8>(a0);
+          const float l1m = lds_f32<-4>(a1), l10 = lds_f32<0>(a1), l11 = lds_f32<4>(a1), l12 = lds_f32<8>(a1);
+          const float lm0 = lds_f32<0>(am), lm1 = lds_f32<4>(am), l20 = lds_f32<0>(a2), l21 = lds_f32<4>(a2);
+          const float du0 = lerp(p.a, l01 - l0m, l02 - l00);
+          const float du1 = lerp(p.a, l11 - l1m, l12 - l10);
+          const float dlu = lerp(p.b, du0, du1);
+          const float dv0 = lerp(p.b, l10 - lm0, l20 - l00);
+          const float dv1 = lerp(p.b, l11 - lm1, l21 - l01);
+          const float dlv = lerp(p.a, dv0, dv1);
+          const float wj = __ldg(wcol + (size_t)m * wstride);
+          const float W = WEIGHT ? G.sad2 * p.rw * p.rw : 1.f;
+          const float cc = fmaf(dlu, p.uq, dlv * p.vq);
+          float qx = fmaf(dlu, j00, fmaf(dlv, j10, -cc * j20));
+          float qy = fmaf(dlu, j01, fmaf(dlv, j11, -cc * j21));
+          float qz = fmaf(dlu, j02, fmaf(dlv, j12, -cc * j22));
+          const float sc = 0.5f * W * p.rw * wj;
+          if (DW) {
+            const float b0 = lerp(p.a, l00, l01), b1 = lerp(p.a, l10, l11);
+            const float bv = lerp(p.b, b0, b1);
+            const float k = -4.f * bv;
+            qx = fmaf(k, j20, qx); qy = fmaf(k, j21, qy); qz = fmaf(k, j22, qz);
+          }
+          sm[0] = fmaf(sc, qx, sm[0]); sm[1] = fmaf(sc, qy, sm[1]); sm[2] = fmaf(sc, qz, sm[2]);
+          const float scm = sc * mf;
+          sm[3] = fmaf(scm, qx, sm[3]); sm[4] = fmaf(scm, qy, sm[4]); sm[5] = fmaf(scm, qz, sm[5]);
+          mf += 1.0f;
+        }
+        const float mx = sm[3] * G.vz, my = sm[4] * G.vz;
+        const float cx = ry * sm[2] - rz * sm[1] - my;
+        const float cy = rz * sm[0] - rx * sm[2] + mx;
+        const float cz = rx * sm[1] - ry * sm[0];
+        sm[3] = cx; sm[4] = cy; sm[5] = cz;
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty_addr + 8u * s);     // the patch is free; the sums are in registers
+#pragma unroll
+      for (int k = 0; k < 6; ++k) {
+        float v = sm[k];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        sm[k] = v;
+      }
+      if (lane == 0) {
+#pragma unroll
+        for (int k = 0; k < 6; ++k) wpart[grp & 1][view - v_lo][warp][k] = sm[k];
+      }
+    }
+    consumer_sync();        // group grp complete in wpart[grp & 1]; also: the reducers of group grp-1 are done
+    if (threadIdx.x < (v_hi - v_lo) * 6) {
+      const int vv = threadIdx.x / 6, k = threadIdx.x % 6;
+      float t = 0.f;
+#pragma unroll
+      for (int w = 0; w < NW; ++w) t += wpart[grp & 1][vv][w][k];
+      if (bad) t = __int_as_float(0x7fc00000);
+      partials[(tile * n_views + (v_lo + vv)) * 6 + k] = t;
+    }
+  }
+}
+
+}  // namespace dfp

@@ -33,6 +33,14 @@ constexpr int kBpZ = 8;                      // voxels along z per thread in bp_
 
 __device__ __forceinline__ float lerp(float a, float v0, float v1) { return fmaf(a, v1 - v0, v0); }
 
+// 1 / w' for the perspective divide: MUFU.RCP plus one Newton step (relative error < 2^-23, no range check or
+// slow path: w' is a source-to-voxel depth in mm, far inside the normal range).  __frcp_rn costs ~11 instructions.
+__device__ __forceinline__ float fast_rcp(float w) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(w));
+  return fmaf(r, fmaf(-w, r, 1.0f), r);
+}
+
 __device__ __forceinline__ float2 ldg2(const float2* p) { return __ldg(p); }
 __device__ __forceinline__ float4 ldg4(const float4* p) { return __ldg(p); }
 
@@ -349,7 +357,7 @@ struct BpPix {
 __device__ __forceinline__ BpPix bp_locate(float up, float vp, float wp, float ulo, float uhi, float vlo, float vhi,
                                            unsigned pu, unsigned C0) {
   BpPix o;
-  float r = __frcp_rn(wp);
+  float r = fast_rcp(wp);
   o.front = wp > 0.f;
   o.rw = r;
   // fminf/fmaxf drop NaNs, so a degenerate w' cannot produce an out-of-range index

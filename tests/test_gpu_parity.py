@@ -246,3 +246,69 @@ def test_tma_path_falls_back_when_it_does_not_apply(dfp):
         dfp.forward(g, f32([0.3]), f32([POSES3[0]]), torch.as_tensor(vol, device=dev))
         assert dfp.last_path() == dfp.PATH_GATHER
         check_forward(run_forward_case(dfp, g, [0.3], [POSES3[0]], vol, up))
+
+
+# ------------------------------------------------------------------ the two back-projection kernel paths
+def _both_bp_paths(dfp, g, angles, poses, proj, up):
+    dev = torch.device("cuda:0")
+    a, p = f32(angles), f32(poses).reshape(-1, 6)
+    pd = torch.as_tensor(proj, dtype=torch.float32, device=dev).contiguous()
+    ud = torch.as_tensor(up, dtype=torch.float32, device=dev).contiguous()
+    out = {}
+    for name, gg in (("tma", g), ("gather", g.replace(flags=g.flags | dfp.FLAG_NO_TMA))):
+        vol = dfp.backproject(gg, a, p, pd)
+        path_b = dfp.last_path()
+        grad = dfp.backproject_pose_grad(gg, a, p, pd, ud)
+        out[name] = (vol.cpu().numpy(), grad.cpu().numpy(), path_b, dfp.last_path())
+    return out
+
+
+@pytest.mark.parametrize("bw,fl", [(0, 0), (1, 0), (1, 1)])
+def test_bp_tma_path_is_taken_and_agrees_with_gather_path(dfp, bw, fl):
+    """nu % 4 == 0, every voxel in front of the source: detector patches staged by TMA.  Same per-voxel formulae;
+    the TMA kernels need no clamp of (u, v), so the compiler fuses u'/w' into the floor / fraction FMAs (one rounding
+    less), and the per-view partial sums of the gradient are grouped by different voxel tiles: agreement to a few
+    1e-6 (ramp-filtered data: sign-cancelling sums), both within 1e-5 of the oracle (the config tests)."""
+    w = W.make_config(3, scale=0.25, n_views=12)
+    g = w.geom.replace(bp_weight=bw, flags=fl)
+    o = _both_bp_paths(dfp, g, w.angles.numpy(), w.poses.numpy(), w.projections().numpy(), w.bp_upstream().numpy())
+    assert o["tma"][2] == dfp.PATH_TMA and o["tma"][3] == dfp.PATH_TMA
+    assert o["gather"][2] == dfp.PATH_GATHER and o["gather"][3] == dfp.PATH_GATHER
+    assert rel_l2(o["tma"][0], o["gather"][0]) <= 5e-6
+    assert np.array_equal(o["tma"][0] == 0, o["gather"][0] == 0)
+    assert grad_err_u9(o["tma"][1], o["gather"][1]).max() <= 1e-4
+
+
+def test_bp_tma_path_ragged_volume_off_detector_voxels_and_many_views(dfp):
+    """Volume not a multiple of the 16x16x16 tile, wider than the fan (zero fill by the TMA unit), and more views
+    than pipeline stages and reduction groups (17 = 2 groups of 8 + 1)."""
+    g = aniso_geom(nx=37, ny=29, nz=23, nu=44, nv=21, vx=2.2, vy=2.0, vz=1.9, du=1.1, dv=1.3, sad=400.0, sdd=600.0)
+    rng = np.random.default_rng(21)
+    V = 17
+    angles = rng.uniform(0, 2 * math.pi, V)
+    poses = np.concatenate([rng.uniform(-3, 3, (V, 3)), rng.uniform(-0.15, 0.15, (V, 3))], axis=1)
+    proj = rng.standard_normal((V,) + g.det_shape).astype(np.float32)
+    up = rng.standard_normal(g.vol_shape).astype(np.float32)
+    for bw in (0, 1):
+        gg = g.replace(bp_weight=bw)
+        o = _both_bp_paths(dfp, gg, angles, poses, proj, up)
+        assert o["tma"][2] == dfp.PATH_TMA and o["tma"][3] == dfp.PATH_TMA
+        assert rel_l2(o["tma"][0], o["gather"][0]) <= 5e-6
+        assert (o["tma"][0] == 0).mean() > 0.05 and np.array_equal(o["tma"][0] == 0, o["gather"][0] == 0)
+        assert grad_err_u9(o["tma"][1], o["gather"][1]).max() <= 1e-4
+        check_back(run_back_case(dfp, gg, angles, poses, proj, up))
+
+
+def test_bp_tma_path_falls_back_when_it_does_not_apply(dfp):
+    """nu % 4 != 0 (no tensor map), or a magnification so large that a tile's footprint exceeds the patch menu."""
+    rng = np.random.default_rng(22)
+    for g in (aniso_geom(nu=21, nv=17), small_geom(n=24, voxel=4.0, nu=400, nv=40, pix=0.1, sad=300.0, sdd=900.0)):
+        # smooth projections: at 120 pixels per voxel, white noise would measure the fp32 resolution of u (|u| <= 200
+        # pixels -> 2e-5 pixel) rather than the kernel
+        iv, iu = np.meshgrid(np.arange(g.nv), np.arange(g.nu), indexing="ij")
+        proj = np.stack([np.sin(0.05 * iu + 0.07 * iv + k) + 0.3 * np.cos(0.11 * iu - 0.02 * iv) for k in range(2)])
+        proj = proj.astype(np.float32)
+        up = rng.standard_normal(g.vol_shape).astype(np.float32)
+        o = _both_bp_paths(dfp, g, ANGLES3[:2], POSES3[:2], proj, up)
+        assert o["tma"][2] == dfp.PATH_GATHER and o["tma"][3] == dfp.PATH_GATHER
+        check_back(run_back_case(dfp, g, ANGLES3[:2], POSES3[:2], proj, up))
