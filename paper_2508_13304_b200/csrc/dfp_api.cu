@@ -312,13 +312,13 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
     for (cudaError_t e : attr) DFP_CUDA(e, "cudaFuncSetAttribute");
     time_begin(s);
     if (grad)
-      fwd_tma_kernel<true, 2><<<grid, kFwdThreads, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, d_up, part);
+      fwd_tma_kernel<true, 2><<<grid, TmaLanes<true>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, d_up, part);
     else if (shape == 0)
-      fwd_tma_kernel<false, 0><<<grid, kFwdThreads, tma_smem_bytes<0>(), s>>>(G, dv, vol_map, nullptr, d_out);
+      fwd_tma_kernel<false, 0><<<grid, TmaLanes<false>::THREADS, tma_smem_bytes<0>(), s>>>(G, dv, vol_map, nullptr, d_out);
     else if (shape == 1)
-      fwd_tma_kernel<false, 1><<<grid, kFwdThreads, tma_smem_bytes<1>(), s>>>(G, dv, vol_map, nullptr, d_out);
+      fwd_tma_kernel<false, 1><<<grid, TmaLanes<false>::THREADS, tma_smem_bytes<1>(), s>>>(G, dv, vol_map, nullptr, d_out);
     else
-      fwd_tma_kernel<false, 2><<<grid, kFwdThreads, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, nullptr, d_out);
+      fwd_tma_kernel<false, 2><<<grid, TmaLanes<false>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, nullptr, d_out);
     time_end(s);
     ++g_launches;
     if (grad) {

@@ -41,6 +41,26 @@ constexpr int kNumShapes = 3;
 template <int SHAPE> constexpr int tma_smem_bytes() {
   return BoxShape<SHAPE>::X * BoxShape<SHAPE>::Y * BoxShape<SHAPE>::Z * 4 * BoxShape<SHAPE>::STAGES;
 }
+// Lane mapping.  Each ray is marched by kTmaSlots = 2 lanes (even / odd samples); a warp = 8(u) x 2(v) pixels x 2
+// consecutive samples.  The 32 lanes of a warp-wide LDS then touch voxels spread over two depth steps as well as
+// the 8 x 2 patch: with row pitches 20 / 28 (= -12 / -4 mod 32) and slab pitch = 16 mod 32 these fall on distinct
+// banks almost always (simulated 1.01 wavefronts per load on C2, 1.2 on C4; the 8 x 4-pixel single-sample warp of
+// the gather kernels gives 1.39 / 1.69, measured 1.39 on C2).  Block = 16 x 16 pixels x 2 slots = 512 threads.
+// The forward kernel is issue-bound, not LDS-bound, and keeps one lane per ray (256 threads, 8 x 4-pixel warps):
+// with two slots it ran 7.0 -> 9.0 ms on C2 (twice the per-ray set-up and loop overhead).
+template <bool GRAD> struct TmaLanes { static constexpr int SLOTS = GRAD ? 2 : 1, THREADS = kFwdThreads * SLOTS; };
+template <int SLOTS>
+__device__ __forceinline__ void tma_pixel(int& iu, int& iv, int& slot) {
+  if (SLOTS == 1) {
+    slot = 0;
+    fwd_pixel(iu, iv);
+    return;
+  }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;          // 16 warps: 2 across u, 8 down v
+  slot = lane >> 4;
+  iu = blockIdx.x * kFwdTU + (warp & 1) * 8 + (lane & 7);
+  iv = blockIdx.y * kFwdTV + (warp >> 1) * 2 + ((lane >> 3) & 1);
+}
 constexpr int kMaxStages = 2;
 constexpr float kBoxMargin = 0.05f;                    // voxels: sagitta of the tile + fp32 rounding
 constexpr int kBoxAlignLoss = 3;                       // x cells lost to the 16-byte alignment of the box origin
@@ -111,8 +131,9 @@ __device__ __forceinline__ void issue_chunk(const VolLayout& L, TmaBlock& B, con
 
 // The chunk loop of one block for one box shape.  acc = {sum} (forward) or {gx,gy,gz,hx,hy,hz} (gradient).
 template <bool GRAD, int SHAPE>
-__device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* map, const Ray& r, TmaBlock& B,
-                                          const float* tiles, unsigned tiles_addr, unsigned bar_addr, float* acc) {
+__device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* map, const Ray& r, int slot,
+                                          TmaBlock& B, const float* tiles, unsigned tiles_addr, unsigned bar_addr,
+                                          float* acc) {
   using S = BoxShape<SHAPE>;
   constexpr int BX = S::X, BXY = S::X * S::Y;
   if (threadIdx.x == 0) {
@@ -160,8 +181,11 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
     const unsigned c0 = B.c0[s];
     const int c_lo = kA + chunk * Kc;
     const int ka = max(c_lo, r.k0), kb = min(min(c_lo + Kc, kB), kend);
-    float kf = (float)ka;
-    for (int k = ka; k < kb; ++k) {
+    // this lane takes the samples of its ray whose kappa has the lane's parity (the other slot takes the rest)
+    constexpr int SLOTS = TmaLanes<GRAD>::SLOTS;
+    const int kfirst = SLOTS == 1 ? ka : ka + ((ka ^ slot) & 1);
+    float kf = (float)kfirst;
+    for (int k = kfirst; k < kb; k += SLOTS) {
       const float qx = fmaf(kf, r.dpx, r.pmx), qy = fmaf(kf, r.dpy, r.pmy), qz = fmaf(kf, r.dpz, r.pmz);
       const float tx = qx + kMagic, ty = qy + kMagic, tz = qz + kMagic;
       const float ax = (qx - (tx - kMagic)) + 0.5f, ay = (qy - (ty - kMagic)) + 0.5f, az = (qz - (tz - kMagic)) + 0.5f;
@@ -208,7 +232,7 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
         gx += ddx; gy += ddy; gz += ddz;
         hx = fmaf(kf, ddx, hx); hy = fmaf(kf, ddy, hy); hz = fmaf(kf, ddz, hz);
       }
-      kf += 1.0f;
+      kf += (float)SLOTS;
     }
     __syncthreads();                                   // every thread is done with stage s ("empty")
     if (threadIdx.x == 0 && chunk + S::STAGES < n_chunks)
@@ -222,23 +246,31 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
 }
 
 template <bool GRAD, int SHAPE>
-__global__ void __launch_bounds__(kFwdThreads) fwd_tma_kernel(FwdGeom G, const FwdView* __restrict__ views,
+__global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, GRAD ? 2 : 4) fwd_tma_kernel(FwdGeom G, const FwdView* __restrict__ views,
                                                               const __grid_constant__ CUtensorMap vol_map,
                                                               const float* __restrict__ upstream,
                                                               float* __restrict__ out) {
   extern __shared__ __align__(128) float tiles[];      // STAGES boxes
   __shared__ __align__(8) unsigned long long full_bar[kMaxStages];
   __shared__ TmaBlock B;
-  __shared__ float red[kFwdThreads / 32][6];
+  __shared__ float red[TmaLanes<GRAD>::THREADS / 32][6];
 
-  int iu, iv;
-  fwd_pixel(iu, iv);
+  int iu, iv, slot;
+  tma_pixel<TmaLanes<GRAD>::SLOTS>(iu, iv, slot);
   const int view = blockIdx.z;
   const bool live = iu < G.nu && iv < G.nv;
   const unsigned tiles_addr = smem_u32(tiles), bar_addr = smem_u32(full_bar);
 
-  double e_mm[3], ref_mm[3];
-  Ray r = setup_ray(G, views[view], iu, iv, GRAD ? e_mm : nullptr, GRAD ? ref_mm : nullptr);
+  float ex = 0.f, ey = 0.f, ez = 0.f, px = 0.f, py = 0.f, pz = 0.f;    // ray direction, reference sample (mm)
+  Ray r;
+  {
+    double e_mm[3], ref_mm[3];
+    r = setup_ray(G, views[view], iu, iv, GRAD ? e_mm : nullptr, GRAD ? ref_mm : nullptr);
+    if (GRAD) {
+      ex = (float)e_mm[0]; ey = (float)e_mm[1]; ez = (float)e_mm[2];
+      px = (float)ref_mm[0]; py = (float)ref_mm[1]; pz = (float)ref_mm[2];
+    }
+  }
   if (!live) r.n = 0;
 
   if (threadIdx.x == 0) {
@@ -251,7 +283,7 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_tma_kernel(FwdGeom G, const F
   }
   {  // corner rays of the tile: pixels (0,0), (TU-1,0), (0,TV-1), (TU-1,TV-1) of the block
     const int cu = iu - blockIdx.x * kFwdTU, cv = iv - blockIdx.y * kFwdTV;
-    if ((cu == 0 || cu == kFwdTU - 1) && (cv == 0 || cv == kFwdTV - 1)) {
+    if (slot == 0 && (cu == 0 || cu == kFwdTU - 1) && (cv == 0 || cv == kFwdTV - 1)) {
       const int c = (cu ? 1 : 0) + (cv ? 2 : 0);
       B.pm[c][0] = r.pmx; B.pm[c][1] = r.pmy; B.pm[c][2] = r.pmz;
       B.dp[c][0] = r.dpx; B.dp[c][1] = r.dpy; B.dp[c][2] = r.dpz;
@@ -272,22 +304,25 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_tma_kernel(FwdGeom G, const F
   }
   __syncthreads();
   float acc[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-  tma_march<GRAD, SHAPE>(G, &vol_map, r, B, tiles, tiles_addr, bar_addr, acc);
+  tma_march<GRAD, SHAPE>(G, &vol_map, r, slot, B, tiles, tiles_addr, bar_addr, acc);
+  // the two slots of a ray: even-kappa partial sums + odd-kappa partial sums
+  if (TmaLanes<GRAD>::SLOTS == 2) {
+#pragma unroll
+    for (int q = 0; q < (GRAD ? 6 : 1); ++q) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], 16);
+  }
 
   const float bad = B.Kc < 0 ? __int_as_float(0x7fc00000) : 0.f;   // NaN: the box cannot hold the tile (host bound wrong)
   if (!GRAD) {
-    if (live) out[((size_t)view * G.nv + iv) * G.nu + iu] = G.step * acc[0] + bad;
+    if (live && slot == 0) out[((size_t)view * G.nv + iv) * G.nu + iu] = G.step * acc[0] + bad;
     return;
   }
   float o6[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-  if (live) {
+  if (live && slot == 0) {
     const float gx = acc[0], gy = acc[1], gz = acc[2], hx = acc[3], hy = acc[4], hz = acc[5];
     const float w = __ldg(upstream + ((size_t)view * G.nv + iv) * G.nu + iu);
     const float D = G.step;
     const float sx = gx * G.sgx, sy = gy * G.sgy, sz = gz * G.sgz;
     const float mx = hx * G.sgx * D, my = hy * G.sgy * D, mz = hz * G.sgz * D;
-    const float ex = (float)e_mm[0], ey = (float)e_mm[1], ez = (float)e_mm[2];
-    const float px = (float)ref_mm[0], py = (float)ref_mm[1], pz = (float)ref_mm[2];
     const float wd = w * D;
     o6[0] = wd * sx + bad; o6[1] = wd * sy; o6[2] = wd * sz;
     o6[3] = wd * ((py * sz - pz * sy) + (ey * mz - ez * my));
@@ -310,7 +345,7 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_tma_kernel(FwdGeom G, const F
   if (threadIdx.x < 6) {
     float t = 0.f;
 #pragma unroll
-    for (int wI = 0; wI < kFwdThreads / 32; ++wI) t += red[wI][threadIdx.x];
+    for (int wI = 0; wI < TmaLanes<GRAD>::THREADS / 32; ++wI) t += red[wI][threadIdx.x];
     const size_t blk = (size_t)blockIdx.y * gridDim.x + blockIdx.x;
     const size_t nblk = (size_t)gridDim.x * gridDim.y;
     out[((size_t)view * nblk + blk) * 6 + threadIdx.x] = t;

@@ -210,18 +210,25 @@ def _both_paths(dfp, g, angles, poses, vol, up):
     return out
 
 
-def test_tma_path_is_taken_and_matches_gather_path_bit_for_bit(dfp):
-    """nx % 4 == 0 and clinical magnification: the TMA-staged kernels run; same arithmetic => same bits."""
+def _same(o):
+    """The two forward paths do the same arithmetic per sample; the TMA kernels split a ray's samples between two
+    lanes (even / odd) and add the two partial sums, so the results agree to fp32 summation order."""
+    pt, pg = o["tma"][0].numpy(), o["gather"][0].numpy()
+    return (rel_l2(pt, pg) <= 2e-6 and np.array_equal(pt == 0, pg == 0) and
+            grad_err_u9(o["tma"][1].numpy(), o["gather"][1].numpy()).max() <= 2e-5)
+
+
+def test_tma_path_is_taken_and_matches_gather_path(dfp):
+    """nx % 4 == 0 and clinical magnification: the TMA-staged kernels run; same arithmetic per sample."""
     w = W.make_config(2, scale=0.25, n_views=3)
     o = _both_paths(dfp, w.geom, w.angles.numpy(), w.poses.numpy(), w.volume().numpy(), w.fwd_upstream().numpy())
     assert o["tma"][2] == dfp.PATH_TMA and o["tma"][3] == dfp.PATH_TMA
     assert o["gather"][2] == dfp.PATH_GATHER and o["gather"][3] == dfp.PATH_GATHER
-    assert torch.equal(o["tma"][0], o["gather"][0])
-    assert torch.equal(o["tma"][1], o["gather"][1])
+    assert _same(o)
     w = W.make_config(4, scale=0.125, n_views=5)          # views around the circle: oblique frusta, short chunks
     o = _both_paths(dfp, w.geom, w.angles.numpy(), w.poses.numpy(), w.volume().numpy(), w.fwd_upstream().numpy())
     assert o["tma"][2] == dfp.PATH_TMA and o["tma"][3] == dfp.PATH_TMA
-    assert torch.equal(o["tma"][0], o["gather"][0]) and torch.equal(o["tma"][1], o["gather"][1])
+    assert _same(o)
 
 
 def test_tma_path_ragged_detector_and_partial_misses(dfp):
@@ -232,7 +239,7 @@ def test_tma_path_ragged_detector_and_partial_misses(dfp):
     up = rng.standard_normal((3,) + g.det_shape).astype(np.float32)
     o = _both_paths(dfp, g, ANGLES3, POSES3, vol, up)
     assert o["tma"][2] == dfp.PATH_TMA and o["tma"][3] == dfp.PATH_TMA
-    assert torch.equal(o["tma"][0], o["gather"][0]) and torch.equal(o["tma"][1], o["gather"][1])
+    assert _same(o)
     check_forward(run_forward_case(dfp, g, ANGLES3, POSES3, vol, up))
 
 
