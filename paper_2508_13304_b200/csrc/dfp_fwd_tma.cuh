@@ -48,6 +48,10 @@ template <int SHAPE> constexpr int tma_smem_bytes() {
 // the gather kernels gives 1.39 / 1.69, measured 1.39 on C2).  Block = 16 x 16 pixels x 2 slots = 512 threads.
 // The forward kernel is issue-bound, not LDS-bound, and keeps one lane per ray (256 threads, 8 x 4-pixel warps):
 // with two slots it ran 7.0 -> 9.0 ms on C2 (twice the per-ray set-up and loop overhead).
+__device__ __forceinline__ float2 sub2(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
+// lerp on two lanes of data at once: v0 + a (v1 - v0), rounded exactly like lerp()
+__device__ __forceinline__ float2 lerp2(float2 a, float2 v0, float2 v1) { return __ffma2_rn(a, sub2(v1, v0), v0); }
+
 template <bool GRAD> struct TmaLanes { static constexpr int SLOTS = GRAD ? 2 : 1, THREADS = kFwdThreads * SLOTS; };
 template <int SLOTS>
 __device__ __forceinline__ void tma_pixel(int& iu, int& iv, int& slot) {
@@ -186,49 +190,64 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
     const int kfirst = SLOTS == 1 ? ka : ka + ((ka ^ slot) & 1);
     float kf = (float)kfirst;
     for (int k = kfirst; k < kb; k += SLOTS) {
-      const float qx = fmaf(kf, r.dpx, r.pmx), qy = fmaf(kf, r.dpy, r.pmy), qz = fmaf(kf, r.dpz, r.pmz);
-      const float tx = qx + kMagic, ty = qy + kMagic, tz = qz + kMagic;
-      const float ax = (qx - (tx - kMagic)) + 0.5f, ay = (qy - (ty - kMagic)) + 0.5f, az = (qz - (tz - kMagic)) + 0.5f;
-      const unsigned idx = (unsigned)__float_as_int(tx) + (unsigned)BX * (unsigned)__float_as_int(ty) +
+      // position, floor and fractions: x and y as one fp32x2 lane pair (same roundings as the scalar code)
+      const float2 q2 = __ffma2_rn(make_float2(kf, kf), make_float2(r.dpx, r.dpy), make_float2(r.pmx, r.pmy));
+      const float qz = fmaf(kf, r.dpz, r.pmz);
+      const float2 t2 = __fadd2_rn(q2, make_float2(kMagic, kMagic));
+      const float tz = qz + kMagic;
+      const float2 a2 = __fadd2_rn(sub2(q2, __fadd2_rn(t2, make_float2(-kMagic, -kMagic))), make_float2(0.5f, 0.5f));
+      const float ax = a2.x, ay = a2.y, az = (qz - (tz - kMagic)) + 0.5f;
+      const unsigned idx = (unsigned)__float_as_int(t2.x) + (unsigned)BX * (unsigned)__float_as_int(t2.y) +
                            (unsigned)BXY * (unsigned)__float_as_int(tz) + c0;
       const float* c = tiles + idx;
       if (!GRAD) {
-        const float r00 = lerp(ax, c[0], c[1]), r10 = lerp(ax, c[BX], c[BX + 1]);
-        const float r01 = lerp(ax, c[BXY], c[BXY + 1]), r11 = lerp(ax, c[BXY + BX], c[BXY + BX + 1]);
-        sum += lerp(az, lerp(ay, r00, r10), lerp(ay, r01, r11));
+        // pairs over the two z slices: (r00, r01), (r10, r11), then the y lerp on the pair, the z lerp scalar
+        const float2 ax2 = make_float2(ax, ax);
+        const float2 rA = lerp2(ax2, make_float2(c[0], c[BXY]), make_float2(c[1], c[BXY + 1]));
+        const float2 rB = lerp2(ax2, make_float2(c[BX], c[BXY + BX]), make_float2(c[BX + 1], c[BXY + BX + 1]));
+        const float2 ry = lerp2(make_float2(ay, ay), rA, rB);
+        sum += lerp(az, ry.x, ry.y);
       } else {
-        float rv[2][2], rdx[2][2];
-#pragma unroll
-        for (int kk = 0; kk < 2; ++kk)
-#pragma unroll
-          for (int j = 0; j < 2; ++j) {
-            const float* row = c + kk * BXY + j * BX;
-            const float m1 = row[-1], v0 = row[0], v1 = row[1], v2 = row[2];
-            rv[j][kk] = lerp(ax, v0, v1);
-            rdx[j][kk] = lerp(ax, v1 - m1, v2 - v0);
-          }
-        float rym[2], ryp[2], rzm[2], rzp[2];
-#pragma unroll
-        for (int kk = 0; kk < 2; ++kk) {
-          const float* m = c + kk * BXY - BX;
-          const float* p = c + kk * BXY + 2 * BX;
-          rym[kk] = lerp(ax, m[0], m[1]);
-          ryp[kk] = lerp(ax, p[0], p[1]);
-        }
+        // Packed fp32x2 arithmetic (sm_100 FADD2 / FFMA2: two IEEE-rounded fp32 results per issue slot, the same
+        // bits as the scalar code of fwd_grad_kernel).  Pairs run over the two z slices kk = 0, 1 of a row (y + j).
+        const float2 ax2 = make_float2(ax, ax), ay2 = make_float2(ay, ay);
+        float2 rv2[2], rdx2[2];          // rv2[j] = (rv[j][0], rv[j][1]), likewise rdx2
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
-          const float* m = c + j * BX - BXY;
-          const float* p = c + j * BX + 2 * BXY;
-          rzm[j] = lerp(ax, m[0], m[1]);
-          rzp[j] = lerp(ax, p[0], p[1]);
+          const float* r0 = c + j * BX;
+          const float* r1 = c + BXY + j * BX;
+          const float2 m1 = make_float2(r0[-1], r1[-1]), v0 = make_float2(r0[0], r1[0]);
+          const float2 v1 = make_float2(r0[1], r1[1]), v2 = make_float2(r0[2], r1[2]);
+          rv2[j] = lerp2(ax2, v0, v1);
+          rdx2[j] = lerp2(ax2, sub2(v1, m1), sub2(v2, v0));
         }
-        const float ddx = lerp(az, lerp(ay, rdx[0][0], rdx[1][0]), lerp(ay, rdx[0][1], rdx[1][1]));
-        const float dy0 = lerp(ay, rv[1][0] - rym[0], ryp[0] - rv[0][0]);
-        const float dy1 = lerp(ay, rv[1][1] - rym[1], ryp[1] - rv[0][1]);
-        const float ddy = lerp(az, dy0, dy1);
-        const float dz0 = lerp(az, rv[0][1] - rzm[0], rzp[0] - rv[0][0]);
-        const float dz1 = lerp(az, rv[1][1] - rzm[1], rzp[1] - rv[1][0]);
-        const float ddz = lerp(ay, dz0, dz1);
+        float2 rym2, ryp2;               // ring rows in y: (y-1, z+kk), (y+2, z+kk), paired over kk
+        {
+          const float* m0 = c - BX;
+          const float* m1 = c + BXY - BX;
+          const float* p0 = c + 2 * BX;
+          const float* p1 = c + BXY + 2 * BX;
+          rym2 = lerp2(ax2, make_float2(m0[0], m1[0]), make_float2(m0[1], m1[1]));
+          ryp2 = lerp2(ax2, make_float2(p0[0], p1[0]), make_float2(p0[1], p1[1]));
+        }
+        float2 rzm2, rzp2;               // ring rows in z: (y+j, z-1), (y+j, z+2), paired over j
+        {
+          const float* m0 = c - BXY;
+          const float* m1 = c + BX - BXY;
+          const float* p0 = c + 2 * BXY;
+          const float* p1 = c + BX + 2 * BXY;
+          rzm2 = lerp2(ax2, make_float2(m0[0], m1[0]), make_float2(m0[1], m1[1]));
+          rzp2 = lerp2(ax2, make_float2(p0[0], p1[0]), make_float2(p0[1], p1[1]));
+        }
+        const float2 dx2 = lerp2(ay2, rdx2[0], rdx2[1]);                           // pair over kk
+        const float ddx = lerp(az, dx2.x, dx2.y);
+        const float2 dy2 = lerp2(ay2, sub2(rv2[1], rym2), sub2(ryp2, rv2[0]));     // (dy0, dy1)
+        const float ddy = lerp(az, dy2.x, dy2.y);
+        // d/dz pairs over j: (rv[0][1], rv[1][1]) - rzm2, rzp2 - (rv[0][0], rv[1][0])
+        const float2 az2 = make_float2(az, az);
+        const float2 dz2 = lerp2(az2, sub2(make_float2(rv2[0].y, rv2[1].y), rzm2),
+                                 sub2(rzp2, make_float2(rv2[0].x, rv2[1].x)));     // (dz0, dz1)
+        const float ddz = lerp(ay, dz2.x, dz2.y);
         gx += ddx; gy += ddy; gz += ddz;
         hx = fmaf(kf, ddx, hx); hy = fmaf(kf, ddy, hy); hz = fmaf(kf, ddz, hz);
       }
