@@ -116,7 +116,8 @@ bool make_volume_map(const dfp_geometry& g, const float* d_vol, int bx, int by, 
 // Positions at path length tau: p = s' + tau e, so a tile's extent along axis a is tau |De_a| with
 // |De_a| <= (|Dd_a| + |e_a| (rho_max/|d|) |Dd|) / SDD  for pixel offsets Dd on a detector at distance >= SDD.
 constexpr int kMinChunk = 4;
-bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V, bool grad, const int* box) {
+bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V, bool grad, const int* box, int TU,
+                   int TV) {
   const double v3[3] = {g.vx, g.vy, g.vz}, c3[3] = {g.cx, g.cy, g.cz};
   const double half[3] = {0.5 * g.nx * g.vx + 3 * g.vx, 0.5 * g.ny * g.vy + 3 * g.vy, 0.5 * g.nz * g.vz + 3 * g.vz};
   double tau_max = 0;
@@ -139,7 +140,7 @@ bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V, bo
   }
   const double sdd = g.sdd;
   const double rho = std::sqrt(std::fmax(dmax * dmax - sdd * sdd, 0.0)) / sdd;
-  const double tu = kFwdTU - 1, tv = kFwdTV - 1;
+  const double tu = TU - 1, tv = TV - 1;
   const double dnorm = std::hypot(tu * (double)g.du, tv * (double)g.dv);
   for (int a = 0; a < 3; ++a) {
     const double dd = tu * std::fabs(V.du[a]) + tv * std::fabs(V.dv[a]);
@@ -203,18 +204,20 @@ int bp_view_patch(const BpGeom& G, const BpView& Vw, int tz, int halo) {
 // ---- workspace carving ---------------------------------------------------------------------------
 struct FwdWs {
   size_t off_views, off_con, off_pvol, off_part, total;
-  int gx, gy;     // blocks per view
+  int gx, gy;     // blocks per view (16 x 16-pixel tiles)
+  int gy8;        // rows of 16 x 8-pixel tiles (TMA gradient kernel)
 };
 FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad) {
   FwdWs w;
   const VolLayout L = make_layout(g);
   w.gx = (g.nu + kFwdTU - 1) / kFwdTU;
   w.gy = (g.nv + kFwdTV - 1) / kFwdTV;
+  w.gy8 = (g.nv + TmaLanes<true>::TV - 1) / TmaLanes<true>::TV;
   size_t o = 0;
   w.off_views = o; o += align_up(sizeof(FwdView) * (size_t)V);
   w.off_con = o;   o += grad ? align_up(sizeof(FwdContract) * (size_t)V) : 0;
   w.off_pvol = o;  o += align_up(sizeof(float4) * (size_t)L.px * L.py * L.pz);
-  w.off_part = o;  o += grad ? align_up(sizeof(float) * 6 * (size_t)V * w.gx * w.gy) : 0;
+  w.off_part = o;  o += grad ? align_up(sizeof(float) * 6 * (size_t)V * w.gx * w.gy8) : 0;
   w.total = o;
   return w;
 }
@@ -292,13 +295,19 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
   CUtensorMap vol_map;
   static const int kBoxes[kNumShapes][3] = {{BoxShape<0>::X, BoxShape<0>::Y, BoxShape<0>::Z},
                                             {BoxShape<1>::X, BoxShape<1>::Y, BoxShape<1>::Z},
-                                            {BoxShape<2>::X, BoxShape<2>::Y, BoxShape<2>::Z}};
+                                            {BoxShape<2>::X, BoxShape<2>::Y, BoxShape<2>::Z},
+                                            {BoxShape<3>::X, BoxShape<3>::Y, BoxShape<3>::Z}};
+  // forward: shapes 0, 1, 2 (16 x 16-pixel tiles); gradient: shapes 3, 2 (16 x 8-pixel tiles)
+  static const int kOrderFwd[3] = {0, 1, 2}, kOrderGrad[2] = {3, 2};
+  const int* order = grad ? kOrderGrad : kOrderFwd;
+  const int n_order = grad ? 2 : 3;
+  const int TU = grad ? TmaLanes<true>::TU : TmaLanes<false>::TU, TV = grad ? TmaLanes<true>::TV : TmaLanes<false>::TV;
   int shape = -1;
   if (!(g->flags & DFP_FLAG_NO_TMA) && (g->nx % 4) == 0) {
-    for (int c = grad ? 2 : 0; c < kNumShapes && shape < 0; ++c) {
+    for (int i = 0; i < n_order && shape < 0; ++i) {
       bool fits = true;
-      for (int v = 0; fits && v < V; ++v) fits = tma_view_fits(*g, G, hv[v], grad, kBoxes[c]);
-      if (fits) shape = c;
+      for (int v = 0; fits && v < V; ++v) fits = tma_view_fits(*g, G, hv[v], grad, kBoxes[order[i]], TU, TV);
+      if (fits) shape = order[i];
     }
   }
   const bool tma = shape >= 0 && make_volume_map(*g, d_vol, kBoxes[shape][0], kBoxes[shape][1], kBoxes[shape][2], &vol_map);
@@ -309,10 +318,16 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
         cudaFuncSetAttribute(fwd_tma_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<1>()),
         cudaFuncSetAttribute(fwd_tma_kernel<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<2>()),
         cudaFuncSetAttribute(fwd_tma_kernel<true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<2>())};
+    static const cudaError_t attr3 =
+        cudaFuncSetAttribute(fwd_tma_kernel<true, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<3>());
+    DFP_CUDA(attr3, "cudaFuncSetAttribute");
     for (cudaError_t e : attr) DFP_CUDA(e, "cudaFuncSetAttribute");
     time_begin(s);
-    if (grad)
-      fwd_tma_kernel<true, 2><<<grid, TmaLanes<true>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, d_up, part);
+    const dim3 ggrid(w.gx, w.gy8, V);
+    if (grad && shape == 3)
+      fwd_tma_kernel<true, 3><<<ggrid, TmaLanes<true>::THREADS, tma_smem_bytes<3>(), s>>>(G, dv, vol_map, d_up, part);
+    else if (grad)
+      fwd_tma_kernel<true, 2><<<ggrid, TmaLanes<true>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, d_up, part);
     else if (shape == 0)
       fwd_tma_kernel<false, 0><<<grid, TmaLanes<false>::THREADS, tma_smem_bytes<0>(), s>>>(G, dv, vol_map, nullptr, d_out);
     else if (shape == 1)
@@ -322,7 +337,7 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
     time_end(s);
     ++g_launches;
     if (grad) {
-      fwd_contract_kernel<<<V, 256, 0, s>>>(w.gx * w.gy, part, dc, d_out);
+      fwd_contract_kernel<<<V, 256, 0, s>>>(w.gx * w.gy8, part, dc, d_out);
       ++g_launches;
     }
     DFP_CUDA(cudaGetLastError(), "forward launch (TMA path)");

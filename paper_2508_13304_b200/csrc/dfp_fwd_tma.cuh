@@ -37,7 +37,8 @@ template <int SHAPE> struct BoxShape;
 template <> struct BoxShape<0> { static constexpr int X = 20, Y = 20, Z = 16, STAGES = 2; };
 template <> struct BoxShape<1> { static constexpr int X = 28, Y = 20, Z = 20, STAGES = 2; };
 template <> struct BoxShape<2> { static constexpr int X = 28, Y = 28, Z = 20, STAGES = 1; };
-constexpr int kNumShapes = 3;
+template <> struct BoxShape<3> { static constexpr int X = 28, Y = 28, Z = 16, STAGES = 1; };   // gradient, 16 x 8 tiles
+constexpr int kNumShapes = 4;
 template <int SHAPE> constexpr int tma_smem_bytes() {
   return BoxShape<SHAPE>::X * BoxShape<SHAPE>::Y * BoxShape<SHAPE>::Z * 4 * BoxShape<SHAPE>::STAGES;
 }
@@ -52,7 +53,11 @@ __device__ __forceinline__ float2 sub2(float2 a, float2 b) { return __fadd2_rn(a
 // lerp on two lanes of data at once: v0 + a (v1 - v0), rounded exactly like lerp()
 __device__ __forceinline__ float2 lerp2(float2 a, float2 v0, float2 v1) { return __ffma2_rn(a, sub2(v1, v0), v0); }
 
-template <bool GRAD> struct TmaLanes { static constexpr int SLOTS = GRAD ? 2 : 1, THREADS = kFwdThreads * SLOTS; };
+// Pixel tile of a block: 16 x 16 (forward), 16 x 8 (gradient: 256 threads = 128 rays x 2 slots, four blocks per SM
+// instead of two 512-thread ones hide the single-stage TMA latency better).
+template <bool GRAD> struct TmaLanes {
+  static constexpr int SLOTS = GRAD ? 2 : 1, TU = kFwdTU, TV = GRAD ? 8 : kFwdTV, THREADS = TU * TV * SLOTS;
+};
 template <int SLOTS>
 __device__ __forceinline__ void tma_pixel(int& iu, int& iv, int& slot) {
   if (SLOTS == 1) {
@@ -60,10 +65,10 @@ __device__ __forceinline__ void tma_pixel(int& iu, int& iv, int& slot) {
     fwd_pixel(iu, iv);
     return;
   }
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;          // 16 warps: 2 across u, 8 down v
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;          // warps: 2 across u, TV / 2 down v
   slot = lane >> 4;
   iu = blockIdx.x * kFwdTU + (warp & 1) * 8 + (lane & 7);
-  iv = blockIdx.y * kFwdTV + (warp >> 1) * 2 + ((lane >> 3) & 1);
+  iv = blockIdx.y * TmaLanes<true>::TV + (warp >> 1) * 2 + ((lane >> 3) & 1);
 }
 constexpr int kMaxStages = 2;
 constexpr float kBoxMargin = 0.05f;                    // voxels: sagitta of the tile + fp32 rounding
@@ -265,7 +270,7 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
 }
 
 template <bool GRAD, int SHAPE>
-__global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, GRAD ? 2 : 4) fwd_tma_kernel(FwdGeom G, const FwdView* __restrict__ views,
+__global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, 4) fwd_tma_kernel(FwdGeom G, const FwdView* __restrict__ views,
                                                               const __grid_constant__ CUtensorMap vol_map,
                                                               const float* __restrict__ upstream,
                                                               float* __restrict__ out) {
@@ -301,8 +306,9 @@ __global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, GRAD ? 2 : 4) fwd_tma
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   {  // corner rays of the tile: pixels (0,0), (TU-1,0), (0,TV-1), (TU-1,TV-1) of the block
-    const int cu = iu - blockIdx.x * kFwdTU, cv = iv - blockIdx.y * kFwdTV;
-    if (slot == 0 && (cu == 0 || cu == kFwdTU - 1) && (cv == 0 || cv == kFwdTV - 1)) {
+    constexpr int TU = TmaLanes<GRAD>::TU, TV = TmaLanes<GRAD>::TV;
+    const int cu = iu - blockIdx.x * TU, cv = iv - blockIdx.y * TV;
+    if (slot == 0 && (cu == 0 || cu == TU - 1) && (cv == 0 || cv == TV - 1)) {
       const int c = (cu ? 1 : 0) + (cv ? 2 : 0);
       B.pm[c][0] = r.pmx; B.pm[c][1] = r.pmy; B.pm[c][2] = r.pmz;
       B.dp[c][0] = r.dpx; B.dp[c][1] = r.dpy; B.dp[c][2] = r.dpz;
