@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdfp.so")
 SOURCES = [os.path.join(CSRC, "dfp_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("dfp_kernels.cuh", "dfp_params.h")] + \
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("dfp_kernels.cuh", "dfp_fwd_tma.cuh", "dfp_bp_tma.cuh", "dfp_params.h")] + \
     [os.path.join(os.path.dirname(HERE), "include", "dfp.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
@@ -33,7 +33,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
     nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
     if not os.path.exists(nvcc):
         raise RuntimeError("nvcc not found: cannot build libdfp.so (there is no CPU fallback)")
-    cmd = [nvcc] + NVCC_FLAGS + ["-o", LIB] + SOURCES
+    # DFP_NVCC_EXTRA (e.g. "-DDFP_CHECK_BOUNDS"): debug builds; the TMA kernels then verify every shared-memory index
+    extra = os.environ.get("DFP_NVCC_EXTRA", "").split()
+    cmd = [nvcc] + NVCC_FLAGS + extra + ["-o", LIB] + SOURCES
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode:
         sys.stderr.write(res.stdout + res.stderr)

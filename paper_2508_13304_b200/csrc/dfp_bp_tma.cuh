@@ -121,7 +121,8 @@ struct PatchPix {
   float a, b, rw, uq, vq;
   unsigned addr;
 };
-__device__ __forceinline__ PatchPix patch_locate(float up, float vp, float wp, unsigned c0b, unsigned pitch4) {
+__device__ __forceinline__ PatchPix patch_locate(float up, float vp, float wp, unsigned c0b, unsigned pitch4,
+                                                 unsigned chk_lo = 0u, unsigned chk_hi = 0xffffffffu) {
   PatchPix o;
   o.rw = fast_rcp(wp);
   o.uq = up * o.rw;
@@ -130,6 +131,9 @@ __device__ __forceinline__ PatchPix patch_locate(float up, float vp, float wp, u
   o.a = (o.uq - (tu - kMagic)) + 0.5f;
   o.b = (o.vq - (tv - kMagic)) + 0.5f;
   o.addr = 4u * (unsigned)__float_as_int(tu) + pitch4 * (unsigned)__float_as_int(tv) + c0b;
+#ifdef DFP_CHECK_BOUNDS   // debug build: the cell and its halo must lie inside this stage's patch area (else NaN out)
+  if (o.addr < chk_lo || o.addr > chk_hi) o.a = __int_as_float(0x7fc00000);
+#endif
   return o;
 }
 template <int OFF>
@@ -184,6 +188,8 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_tma_kernel(BpGeom G, int n_v
     mbar_wait(full_addr + 8u * s, (unsigned)(view / n_stages) & 1u);
     const float* hdr = smem + s * stage_words;
     const unsigned c0 = __float_as_uint(hdr[24]), BU = __float_as_uint(hdr[26]);
+    const unsigned chk_lo = smem_addr + 4u * (unsigned)(s * stage_words + kPatchHeader) + BU + 4u,
+                   chk_hi = smem_addr + 4u * (unsigned)((s + 1) * stage_words) - 2u * BU - 12u;
     bad |= __float_as_uint(hdr[25]) != 0u;
     if (live) {
       const float a02 = hdr[2], a12 = hdr[6], a22 = hdr[10];
@@ -194,7 +200,7 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_tma_kernel(BpGeom G, int n_v
       for (int m = 0; m < TZ; ++m) {
         if (m < T.tz) {
           const float mf = (float)m;
-          const PatchPix p = patch_locate(fmaf(mf, a02, ub), fmaf(mf, a12, vb), fmaf(mf, a22, wb), c0, BU);
+          const PatchPix p = patch_locate(fmaf(mf, a02, ub), fmaf(mf, a12, vb), fmaf(mf, a22, wb), c0, BU, chk_lo, chk_hi);
           const unsigned a1 = p.addr + BU;
           const float val = lerp(p.b, lerp(p.a, lds_f32<0>(p.addr), lds_f32<4>(p.addr)),
                                  lerp(p.a, lds_f32<0>(a1), lds_f32<4>(a1)));
@@ -272,6 +278,8 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_grad_tma_kernel(BpGeom G, in
       mbar_wait(full_addr + 8u * s, (unsigned)(view / n_stages) & 1u);
       const float* hdr = smem + s * stage_words;
       const unsigned c0 = __float_as_uint(hdr[24]), BU = __float_as_uint(hdr[26]);
+      const unsigned chk_lo = smem_addr + 4u * (unsigned)(s * stage_words + kPatchHeader) + BU + 4u,
+                     chk_hi = smem_addr + 4u * (unsigned)((s + 1) * stage_words) - 2u * BU - 12u;
       bad |= __float_as_uint(hdr[25]) != 0u;
       float sm[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
       if (live) {
@@ -283,7 +291,7 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_grad_tma_kernel(BpGeom G, in
                     j20 = hdr[18], j21 = hdr[19], j22 = hdr[20];
         float mf = 0.f;
         for (int m = 0; m < T.tz; ++m) {
-          const PatchPix p = patch_locate(fmaf(mf, a02, ub), fmaf(mf, a12, vb), fmaf(mf, a22, wb), c0, BU);
+          const PatchPix p = patch_locate(fmaf(mf, a02, ub), fmaf(mf, a12, vb), fmaf(mf, a22, wb), c0, BU, chk_lo, chk_hi);
           // rows v, v+1: columns u-1 .. u+2; rows v-1, v+2: columns u, u+1
           const unsigned a0 = p.addr, a1 = a0 + BU, am = a0 - BU, a2 = a1 + BU;
           const float l0m = lds_f32<-4>(a0), l00 = lds_f32<0>(a0), l01 = lds_f32<4>(a0), l02 = lds_f32<8>(a0);

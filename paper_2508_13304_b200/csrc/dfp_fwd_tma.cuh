@@ -205,6 +205,13 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
       const unsigned idx = (unsigned)__float_as_int(t2.x) + (unsigned)BX * (unsigned)__float_as_int(t2.y) +
                            (unsigned)BXY * (unsigned)__float_as_int(tz) + c0;
       const float* c = tiles + idx;
+#ifdef DFP_CHECK_BOUNDS   // debug build: every LDS of the sample must fall inside the stage's box (else NaN out)
+      {
+        const int local = (int)(idx - (unsigned)(s * BXY * S::Z)), halo = GRAD ? 1 : 0;
+        const int lo = local - halo * (1 + BX + BXY), hi = local + (1 + halo) * (1 + BX + BXY);
+        if (lo < 0 || hi >= BXY * S::Z) sum = gx = __int_as_float(0x7fc00000);
+      }
+#endif
       if (!GRAD) {
         // pairs over the two z slices: (r00, r01), (r10, r11), then the y lerp on the pair, the z lerp scalar
         const float2 ax2 = make_float2(ax, ax);
