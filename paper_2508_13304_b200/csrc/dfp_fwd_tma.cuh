@@ -1,8 +1,9 @@
 // dfp_fwd_tma.cuh - a3 / a4 with the volume staged in shared memory by TMA (sm_100a).
 //
-// Same arithmetic, sample for sample, as fwd_project_kernel / fwd_grad_kernel (dfp_kernels.cuh) - the two paths
-// are bit-identical - but the 8 (forward) or 32 (gradient) voxel reads of a sample are LDS from a box of the
-// volume that the block's 16x16-pixel frustum crosses during one CHUNK of consecutive samples:
+// Same arithmetic, sample for sample, as fwd_project_kernel / fwd_grad_kernel (dfp_kernels.cuh) - the forward
+// results are bit-identical, the gradient's differ only by the order in which a ray's even and odd samples are
+// added - but the 8 (forward) or 32 (gradient) voxel reads of a sample are LDS from a box of the volume that the
+// block's pixel tile (16x16 forward, 16x8 gradient) crosses during one CHUNK of consecutive samples:
 //
 //   * the block's rays share one kappa axis (sample k = kref + kappa, tau_k = (k + 1/2) D, fixed in the world:
 //     DESIGN.md O6), so a chunk [kappa0, kappa0 + Kc) is a slab of the frustum; its bounding box in voxel
@@ -11,9 +12,10 @@
 //   * one elected thread issues `cp.async.bulk.tensor.3d` (TMA, SASS UTMALDG) for the chunk's box (BoxShape)
 //     straight from the caller's volume: out-of-range elements are ZERO-FILLED by the TMA unit, which is the
 //     zero extension of f~ (U7) - no padded / packed copy of the volume is made on this path;
-//   * two stages, mbarrier (complete_tx) as the "full" signal, __syncthreads as the "empty" signal;
+//   * one or two stages (BoxShape), mbarrier (complete_tx) as the "full" signal, __syncthreads as the "empty" one;
 //   * the box origin is rounded down to a multiple of 4 floats along x (TMA: 16-byte inner alignment);
-//   * Kc is chosen per block so that the box always fits (oblique tiles get shorter chunks).
+//   * Kc is chosen per block so that the box always fits (oblique tiles get shorter chunks);
+//   * gradient: two lanes per ray (even / odd samples) and packed fp32x2 arithmetic (FFMA2 / FADD2).
 // PAPER.md Eq.18 :172-177 (forward), Eq.7-8 :101-113, Eq.19-20 :179-191 (gradient), :207 (on the fly, weights once).
 #pragma once
 #include <cuda.h>
@@ -29,9 +31,10 @@ namespace dfp {
 // The host picks, per call, the smallest shape every view's tiles fit with chunks of >= kMinChunk samples:
 //   shape 0  20 x 20 x 16, two stages : forward, clinical magnification and small pose angles (C2, C4)
 //   shape 1  28 x 20 x 20, two stages : forward, wider tiles / larger tilts (C5)
-//   shape 2  28 x 28 x 20, one stage  : gradient (the stencil needs 2 more cells per axis and a chunk lasts 4x
-//            longer, so one stage suffices; long enough along x and y that views at 45 degrees in the xy plane
-//            still get ~10-sample chunks), and the forward fallback before the gather path.
+//   shape 2  28 x 28 x 20, one stage  : forward fallback before the gather path; gradient fallback
+//   shape 3  28 x 28 x 16, one stage  : gradient, 16 x 8-pixel tiles (the stencil needs 2 more cells per axis and a
+//            chunk lasts 4x longer than the forward's, so one stage and four blocks per SM hide the TMA latency;
+//            long enough along x and y that views at 45 degrees in the xy plane still get ~10-sample chunks).
 // Measured on B200 (Gray-steps/s, forward): C2 625 / 591 / 557, C4 607 / 560 / 548 for shapes 0 / 1 / 2.
 template <int SHAPE> struct BoxShape;
 template <> struct BoxShape<0> { static constexpr int X = 20, Y = 20, Z = 16, STAGES = 2; };
