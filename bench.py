@@ -328,11 +328,16 @@ def main():
                 "peak_source": f"148 SMs x 128 fp32 lanes x sm_max_mhz ({pk_kind} MEASURED_PEAKS.json clock)",
                 "ops_per_unit": OPS_PER_UNIT[dom], "units_per_launch": units[dom], "kernel_ms": mean_ms,
                 "kernel_share_of_step": {k: v * K / 1e3 / t_all for k, v in mean_ms.items()},
-                "hbm_compulsory_frac": None}
+                "hbm_compulsory_frac": None, "lsu_floor_frac": None}
     # compulsory HBM bytes of the dominant kernel vs the measured copy peak (expected to be small)
     comp = {"fwd_project": vol.numel() * 16 + proj.numel() * 4, "fwd_grad": vol.numel() * 16 + up.numel() * 4,
             "bp": proj.numel() * 16 + bvol.numel() * 4, "bp_grad": proj.numel() * 16 + bvol.numel() * 4}[dom]
     roofline["hbm_compulsory_frac"] = comp / (mean_ms[dom] * 1e-3) / 1e9 / pk["hbm_gbs"]
+    # the unit that binds the staged kernels: the LSU issues one warp-wide shared-memory load per
+    # clock per SM; loads per unit x warp-units / (SMs x clock x time) = fraction of that floor
+    lds = {"fwd_project": 8, "fwd_grad": 32, "bp": 4, "bp_grad": 12}[dom]
+    roofline["lsu_floor_frac"] = lds * (units[dom] / 32.0) / (N_SM * pk.get("sm_max_mhz", 1965.0) * 1e6 *
+                                                                mean_ms[dom] * 1e-3)
 
     # ---------------------------------------------------------------- CPU baseline: the oracle on the host cores
     cpu = None
