@@ -267,6 +267,22 @@ def main():
     bp_value = 2.0 * job_voxel_views * K / t_bp / 1e9
     n_launch = launches[0]
 
+    # ---------------------------------------------------------------- DFP_FLAG_GRAD_INTERP variants (outside the step)
+    gi = g.replace(flags=g.flags | dfp.FLAG_GRAD_INTERP)
+    interp_ms = []
+    for fn in (lambda: dfp.forward_pose_grad(gi, angles, poses, vol, up, out=grad, ws=ws),
+               lambda: dfp.backproject_pose_grad(gi, angles, poses, proj, bp_up, out=bgrad, ws=ws)):
+        fn()
+        a_, b_ = ev(), ev()
+        a_.record()
+        for _ in range(3):
+            fn()
+        b_.record()
+        torch.cuda.synchronize()
+        interp_ms.append(a_.elapsed_time(b_) / 3)
+    dfp.forward_pose_grad(g, angles, poses, vol, up, out=grad, ws=ws)          # leave the default-mode results behind
+    dfp.backproject_pose_grad(g, angles, poses, proj, bp_up, out=bgrad, ws=ws)
+
     # ---------------------------------------------------------------- end to end through the host-buffer C ABI
     e2e = None
     if not args.no_e2e:
@@ -360,7 +376,9 @@ def main():
                          job_voxel_views * K / t_call[3] / 1e9,
                      "ms_per_call": {"forward": float(seg[:, 0].mean()), "forward_pose_grad": float(seg[:, 1].mean()),
                                      "backproject": float(seg[:, 2].mean()),
-                                     "backproject_pose_grad": float(seg[:, 3].mean())}},
+                                     "backproject_pose_grad": float(seg[:, 3].mean())},
+                     "grad_interp_mode_ms_per_call": {"forward_pose_grad": interp_ms[0],
+                                                      "backproject_pose_grad": interp_ms[1]}},
            "clocks": clocks, "e2e": e2e, "gpu_launches": n_launch, "roofline": roofline, "cpu_baseline": cpu}
     print(json.dumps(out), flush=True)
     if dist is not None:

@@ -48,7 +48,12 @@ typedef struct dfp_geometry {
   int32_t bp_weight;    /* back-projection weight W: 0 = 1 (pure Eq.2b), 1 = FDK (sad/w')^2                 */
   int32_t flags;        /* bit0 (DFP_FLAG_DW): add the dW/dtheta term in dfp_backproject_pose_grad;
                            bit1 (DFP_FLAG_NO_TMA): forward paths use the global-memory gather kernels even where
-                           the TMA-staged kernels apply (same results bit for bit; a testing / profiling switch) */
+                           the TMA-staged kernels apply (same results up to summation order; a testing / profiling
+                           switch);
+                           bit2 (DFP_FLAG_GRAD_INTERP): the two *_pose_grad calls differentiate the trilinear / bilinear
+                           INTERPOLANT exactly (8 voxels / 4 pixels per sample, what automatic differentiation of the
+                           discrete projector gives - PAPER.md :211, :346) instead of taking the paper's central finite
+                           differences of it (32 voxels / 12 pixels; Eq.19-22, :183, :202) */
 } dfp_geometry;
 
 enum {
@@ -61,7 +66,7 @@ enum {
   DFP_ERR_CUDA = -6        /* CUDA runtime error (no device, launch failure, out of memory in *_host)       */
 };
 enum { DFP_OP_FORWARD = 0, DFP_OP_FORWARD_POSE_GRAD = 1, DFP_OP_BACKPROJECT = 2, DFP_OP_BACKPROJECT_POSE_GRAD = 3 };
-enum { DFP_FLAG_DW = 1, DFP_FLAG_NO_TMA = 2 };
+enum { DFP_FLAG_DW = 1, DFP_FLAG_NO_TMA = 2, DFP_FLAG_GRAD_INTERP = 4 };
 
 /* Forward projection, Eq.2a :67-69 discretised as Eq.18 :172-177 with a fixed-step, zero-extended
  * trilinear ray-march (U1): proj[v][iv][iu] = D * sum_k f~(R_v^T (s_v + (k+1/2) D e_i - t_v)).

@@ -16,6 +16,7 @@ _LIB_PATH = os.path.join(_HERE, "libdfp.so")
 OP_FORWARD, OP_FORWARD_POSE_GRAD, OP_BACKPROJECT, OP_BACKPROJECT_POSE_GRAD = 0, 1, 2, 3
 FLAG_DW = 1
 FLAG_NO_TMA = 2
+FLAG_GRAD_INTERP = 4
 PATH_GATHER, PATH_TMA = 0, 1
 
 

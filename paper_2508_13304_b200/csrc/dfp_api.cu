@@ -212,7 +212,7 @@ FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad) {
   const VolLayout L = make_layout(g);
   w.gx = (g.nu + kFwdTU - 1) / kFwdTU;
   w.gy = (g.nv + kFwdTV - 1) / kFwdTV;
-  w.gy8 = (g.nv + TmaLanes<true>::TV - 1) / TmaLanes<true>::TV;
+  w.gy8 = (g.nv + TmaLanes<1>::TV - 1) / TmaLanes<1>::TV;
   size_t o = 0;
   w.off_views = o; o += align_up(sizeof(FwdView) * (size_t)V);
   w.off_con = o;   o += grad ? align_up(sizeof(FwdContract) * (size_t)V) : 0;
@@ -277,7 +277,8 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
   st = check_common(g, V, angles, poses, d_vol, d_out, grad ? (const void*)d_up : (const void*)d_vol, d_ws,
                         ws_bytes, w.total);
   if (st) return st;
-  const FwdGeom G = make_fwd_geom(*g, grad);
+  const bool interp = grad && (g->flags & DFP_FLAG_GRAD_INTERP);
+  const FwdGeom G = make_fwd_geom(*g, grad, interp);
   std::vector<FwdView> hv((size_t)V);
   std::vector<FwdContract> hc(grad ? (size_t)V : 0);
   for (int v = 0; v < V; ++v) make_fwd_view(*g, angles[v], poses + 6 * v, &hv[v], grad ? &hc[v] : nullptr);
@@ -301,7 +302,7 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
   static const int kOrderFwd[3] = {0, 1, 2}, kOrderGrad[2] = {3, 2};
   const int* order = grad ? kOrderGrad : kOrderFwd;
   const int n_order = grad ? 2 : 3;
-  const int TU = grad ? TmaLanes<true>::TU : TmaLanes<false>::TU, TV = grad ? TmaLanes<true>::TV : TmaLanes<false>::TV;
+  const int TU = grad ? TmaLanes<1>::TU : TmaLanes<0>::TU, TV = grad ? TmaLanes<1>::TV : TmaLanes<0>::TV;
   int shape = -1;
   if (!(g->flags & DFP_FLAG_NO_TMA) && (g->nx % 4) == 0) {
     for (int i = 0; i < n_order && shape < 0; ++i) {
@@ -314,26 +315,32 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
   g_path = tma ? DFP_PATH_TMA : DFP_PATH_GATHER;
   if (tma) {
     static const cudaError_t attr[4] = {
-        cudaFuncSetAttribute(fwd_tma_kernel<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<0>()),
-        cudaFuncSetAttribute(fwd_tma_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<1>()),
-        cudaFuncSetAttribute(fwd_tma_kernel<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<2>()),
-        cudaFuncSetAttribute(fwd_tma_kernel<true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<2>())};
-    static const cudaError_t attr3 =
-        cudaFuncSetAttribute(fwd_tma_kernel<true, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<3>());
-    DFP_CUDA(attr3, "cudaFuncSetAttribute");
+        cudaFuncSetAttribute(fwd_tma_kernel<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<0>()),
+        cudaFuncSetAttribute(fwd_tma_kernel<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<1>()),
+        cudaFuncSetAttribute(fwd_tma_kernel<0, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<2>()),
+        cudaFuncSetAttribute(fwd_tma_kernel<1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<2>())};
+    static const cudaError_t attr3[3] = {
+        cudaFuncSetAttribute(fwd_tma_kernel<1, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<3>()),
+        cudaFuncSetAttribute(fwd_tma_kernel<2, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<3>()),
+        cudaFuncSetAttribute(fwd_tma_kernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<2>())};
+    for (cudaError_t e : attr3) DFP_CUDA(e, "cudaFuncSetAttribute");
     for (cudaError_t e : attr) DFP_CUDA(e, "cudaFuncSetAttribute");
     time_begin(s);
     const dim3 ggrid(w.gx, w.gy8, V);
-    if (grad && shape == 3)
-      fwd_tma_kernel<true, 3><<<ggrid, TmaLanes<true>::THREADS, tma_smem_bytes<3>(), s>>>(G, dv, vol_map, d_up, part);
+    if (grad && interp && shape == 3)
+      fwd_tma_kernel<2, 3><<<ggrid, TmaLanes<2>::THREADS, tma_smem_bytes<3>(), s>>>(G, dv, vol_map, d_up, part);
+    else if (grad && interp)
+      fwd_tma_kernel<2, 2><<<ggrid, TmaLanes<2>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, d_up, part);
+    else if (grad && shape == 3)
+      fwd_tma_kernel<1, 3><<<ggrid, TmaLanes<1>::THREADS, tma_smem_bytes<3>(), s>>>(G, dv, vol_map, d_up, part);
     else if (grad)
-      fwd_tma_kernel<true, 2><<<ggrid, TmaLanes<true>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, d_up, part);
+      fwd_tma_kernel<1, 2><<<ggrid, TmaLanes<1>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, d_up, part);
     else if (shape == 0)
-      fwd_tma_kernel<false, 0><<<grid, TmaLanes<false>::THREADS, tma_smem_bytes<0>(), s>>>(G, dv, vol_map, nullptr, d_out);
+      fwd_tma_kernel<0, 0><<<grid, TmaLanes<0>::THREADS, tma_smem_bytes<0>(), s>>>(G, dv, vol_map, nullptr, d_out);
     else if (shape == 1)
-      fwd_tma_kernel<false, 1><<<grid, TmaLanes<false>::THREADS, tma_smem_bytes<1>(), s>>>(G, dv, vol_map, nullptr, d_out);
+      fwd_tma_kernel<0, 1><<<grid, TmaLanes<0>::THREADS, tma_smem_bytes<1>(), s>>>(G, dv, vol_map, nullptr, d_out);
     else
-      fwd_tma_kernel<false, 2><<<grid, TmaLanes<false>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, nullptr, d_out);
+      fwd_tma_kernel<0, 2><<<grid, TmaLanes<0>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, nullptr, d_out);
     time_end(s);
     ++g_launches;
     if (grad) {
@@ -353,7 +360,8 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
     ++g_launches;
   } else {
     time_begin(s);
-    fwd_grad_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, pvol, d_up, part);
+    if (interp) fwd_grad_kernel<1><<<grid, kFwdThreads, 0, s>>>(G, dv, pvol, d_up, part);
+    else fwd_grad_kernel<0><<<grid, kFwdThreads, 0, s>>>(G, dv, pvol, d_up, part);
     time_end(s);
     fwd_contract_kernel<<<V, 256, 0, s>>>(w.gx * w.gy, part, dc, d_out);
     g_launches += 2;
@@ -402,12 +410,12 @@ int run_backproject(const dfp_geometry* g, int V, const float* angles, const flo
     const int stage_words = bp_stage_words(kmax), n_stages = bp_num_stages(kmax);
     const int smem = stage_words * 4 * n_stages;
 #define DFP_BP_ATTR(k) cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, kBpSmemBudget)
-    static const cudaError_t attr[10] = {
+#define DFP_BP_ATTR_G(W, D) DFP_BP_ATTR((bp_grad_tma_kernel<W, D, 16, 0>)), DFP_BP_ATTR((bp_grad_tma_kernel<W, D, 8, 0>)), \
+                            DFP_BP_ATTR((bp_grad_tma_kernel<W, D, 16, 1>)), DFP_BP_ATTR((bp_grad_tma_kernel<W, D, 8, 1>))
+    static const cudaError_t attr[16] = {
         DFP_BP_ATTR((bp_tma_kernel<0, 16>)), DFP_BP_ATTR((bp_tma_kernel<1, 16>)), DFP_BP_ATTR((bp_tma_kernel<0, 8>)),
-        DFP_BP_ATTR((bp_tma_kernel<1, 8>)), DFP_BP_ATTR((bp_grad_tma_kernel<0, 0, 16>)),
-        DFP_BP_ATTR((bp_grad_tma_kernel<1, 0, 16>)), DFP_BP_ATTR((bp_grad_tma_kernel<1, 1, 16>)),
-        DFP_BP_ATTR((bp_grad_tma_kernel<0, 0, 8>)), DFP_BP_ATTR((bp_grad_tma_kernel<1, 0, 8>)),
-        DFP_BP_ATTR((bp_grad_tma_kernel<1, 1, 8>))};
+        DFP_BP_ATTR((bp_tma_kernel<1, 8>)), DFP_BP_ATTR_G(0, 0), DFP_BP_ATTR_G(1, 0), DFP_BP_ATTR_G(1, 1)};
+#undef DFP_BP_ATTR_G
 #undef DFP_BP_ATTR
     for (cudaError_t e : attr) DFP_CUDA(e, "cudaFuncSetAttribute");
     const dim3 tgrid(w.tx, w.ty, (g->nz + TZ - 1) / TZ);
@@ -421,13 +429,18 @@ int run_backproject(const dfp_geometry* g, int V, const float* angles, const flo
       ++g_launches;
     } else {
       const bool dw = G.bp_weight && (G.flags & DFP_FLAG_DW);
-      if (!G.bp_weight) {
-        if (TZ == 16) bp_grad_tma_kernel<0, 0, 16> DFP_BP_ARGS, d_up, part); else bp_grad_tma_kernel<0, 0, 8> DFP_BP_ARGS, d_up, part);
-      } else if (!dw) {
-        if (TZ == 16) bp_grad_tma_kernel<1, 0, 16> DFP_BP_ARGS, d_up, part); else bp_grad_tma_kernel<1, 0, 8> DFP_BP_ARGS, d_up, part);
-      } else {
-        if (TZ == 16) bp_grad_tma_kernel<1, 1, 16> DFP_BP_ARGS, d_up, part); else bp_grad_tma_kernel<1, 1, 8> DFP_BP_ARGS, d_up, part);
-      }
+      const bool interp = (G.flags & DFP_FLAG_GRAD_INTERP) != 0;
+#define DFP_BP_GRAD(W, D)                                                                            \
+  do {                                                                                               \
+    if (TZ == 16 && !interp) bp_grad_tma_kernel<W, D, 16, 0> DFP_BP_ARGS, d_up, part);               \
+    else if (TZ == 16) bp_grad_tma_kernel<W, D, 16, 1> DFP_BP_ARGS, d_up, part);                     \
+    else if (!interp) bp_grad_tma_kernel<W, D, 8, 0> DFP_BP_ARGS, d_up, part);                       \
+    else bp_grad_tma_kernel<W, D, 8, 1> DFP_BP_ARGS, d_up, part);                                    \
+  } while (0)
+      if (!G.bp_weight) DFP_BP_GRAD(0, 0);
+      else if (!dw) DFP_BP_GRAD(1, 0);
+      else DFP_BP_GRAD(1, 1);
+#undef DFP_BP_GRAD
       time_end(s);
       bp_contract_kernel<<<V, 256, 0, s>>>(tgrid.x * tgrid.y * tgrid.z, V, part, dc, d_out);
       g_launches += 2;
@@ -449,9 +462,16 @@ int run_backproject(const dfp_geometry* g, int V, const float* angles, const flo
   } else {
     const bool dw = G.bp_weight && (G.flags & DFP_FLAG_DW);
     time_begin(s);
-    if (!G.bp_weight) bp_grad_kernel<0, 0><<<grid, kBpThreads, 0, s>>>(G, V, kBpGradZChunk, dv, q, d_up, part);
-    else if (!dw) bp_grad_kernel<1, 0><<<grid, kBpThreads, 0, s>>>(G, V, kBpGradZChunk, dv, q, d_up, part);
-    else bp_grad_kernel<1, 1><<<grid, kBpThreads, 0, s>>>(G, V, kBpGradZChunk, dv, q, d_up, part);
+    const bool interp = (G.flags & DFP_FLAG_GRAD_INTERP) != 0;
+#define DFP_BP_GRAD(W, D)                                                                                       \
+  do {                                                                                                          \
+    if (interp) bp_grad_kernel<W, D, 1><<<grid, kBpThreads, 0, s>>>(G, V, kBpGradZChunk, dv, q, d_up, part);    \
+    else bp_grad_kernel<W, D, 0><<<grid, kBpThreads, 0, s>>>(G, V, kBpGradZChunk, dv, q, d_up, part);           \
+  } while (0)
+    if (!G.bp_weight) DFP_BP_GRAD(0, 0);
+    else if (!dw) DFP_BP_GRAD(1, 0);
+    else DFP_BP_GRAD(1, 1);
+#undef DFP_BP_GRAD
     time_end(s);
     bp_contract_kernel<<<V, 256, 0, s>>>(w.gx * w.gy * w.gz, V, part, dc, d_out);
     g_launches += 2;

@@ -227,7 +227,8 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_tma_kernel(BpGeom G, int n_v
 // and are added in fixed order once per group -> partials[tile][view][6]: one consumer barrier per group, not per view.
 constexpr int kBpGradGroup = 8;                  // views per cross-warp reduction
 
-template <int WEIGHT, int DW, int TZ>
+// MODE 1 (DFP_FLAG_GRAD_INTERP): exact derivatives of the bilinear interpolant, 4 LDS instead of 12.
+template <int WEIGHT, int DW, int TZ, int MODE>
 __global__ void __launch_bounds__(kBpTmaThreads) bp_grad_tma_kernel(BpGeom G, int n_views,
                                                                     const BpView* __restrict__ views,
                                                                     const __grid_constant__ PatchMaps maps, int kmax,
@@ -293,27 +294,36 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_grad_tma_kernel(BpGeom G, in
         for (int m = 0; m < T.tz; ++m) {
           const PatchPix p = patch_locate(fmaf(mf, a02, ub), fmaf(mf, a12, vb), fmaf(mf, a22, wb), c0, BU, chk_lo, chk_hi);
           // rows v, v+1: columns u-1 .. u+2; rows v-1, v+2: columns u, u+1
-          const unsigned a0 = p.addr, a1 = a0 + BU, am = a0 - BU, a2 = a1 + BU;
-          const float l0m = lds_f32<-4>(a0), l00 = lds_f32<0>(a0), l01 = lds_f32<4>(a0), l02 = lds_f32<8>(a0);
-          const float l1m = lds_f32<-4>(a1), l10 = lds_f32<0>(a1), l11 = lds_f32<4>(a1), l12 = lds_f32<8>(a1);
-          const float lm0 = lds_f32<0>(am), lm1 = lds_f32<4>(am), l20 = lds_f32<0>(a2), l21 = lds_f32<4>(a2);
-          const float du0 = lerp(p.a, l01 - l0m, l02 - l00);
-          const float du1 = lerp(p.a, l11 - l1m, l12 - l10);
-          const float dlu = lerp(p.b, du0, du1);
-          const float dv0 = lerp(p.b, l10 - lm0, l20 - l00);
-          const float dv1 = lerp(p.b, l11 - lm1, l21 - l01);
-          const float dlv = lerp(p.a, dv0, dv1);
+          float dlu, dlv, l00, l01, l10, l11;
+          if (MODE == 1) {
+            const unsigned a0 = p.addr, a1 = a0 + BU;
+            l00 = lds_f32<0>(a0); l01 = lds_f32<4>(a0); l10 = lds_f32<0>(a1); l11 = lds_f32<4>(a1);
+            dlu = lerp(p.b, l01 - l00, l11 - l10);
+            dlv = lerp(p.a, l10 - l00, l11 - l01);
+          } else {
+            const unsigned a0 = p.addr, a1 = a0 + BU, am = a0 - BU, a2 = a1 + BU;
+            const float l0m = lds_f32<-4>(a0), l02 = lds_f32<8>(a0);
+            const float l1m = lds_f32<-4>(a1), l12 = lds_f32<8>(a1);
+            l00 = lds_f32<0>(a0); l01 = lds_f32<4>(a0); l10 = lds_f32<0>(a1); l11 = lds_f32<4>(a1);
+            const float lm0 = lds_f32<0>(am), lm1 = lds_f32<4>(am), l20 = lds_f32<0>(a2), l21 = lds_f32<4>(a2);
+            const float du0 = lerp(p.a, l01 - l0m, l02 - l00);
+            const float du1 = lerp(p.a, l11 - l1m, l12 - l10);
+            dlu = lerp(p.b, du0, du1);
+            const float dv0 = lerp(p.b, l10 - lm0, l20 - l00);
+            const float dv1 = lerp(p.b, l11 - lm1, l21 - l01);
+            dlv = lerp(p.a, dv0, dv1);
+          }
           const float wj = __ldg(wcol + (size_t)m * wstride);
           const float W = WEIGHT ? G.sad2 * p.rw * p.rw : 1.f;
           const float cc = fmaf(dlu, p.uq, dlv * p.vq);
           float qx = fmaf(dlu, j00, fmaf(dlv, j10, -cc * j20));
           float qy = fmaf(dlu, j01, fmaf(dlv, j11, -cc * j21));
           float qz = fmaf(dlu, j02, fmaf(dlv, j12, -cc * j22));
-          const float sc = 0.5f * W * p.rw * wj;
+          const float sc = (MODE == 1 ? 1.0f : 0.5f) * W * p.rw * wj;
           if (DW) {
             const float b0 = lerp(p.a, l00, l01), b1 = lerp(p.a, l10, l11);
             const float bv = lerp(p.b, b0, b1);
-            const float k = -4.f * bv;
+            const float k = (MODE == 1 ? -2.f : -4.f) * bv;
             qx = fmaf(k, j20, qx); qy = fmaf(k, j21, qy); qz = fmaf(k, j22, qz);
           }
           sm[0] = fmaf(sc, qx, sm[0]); sm[1] = fmaf(sc, qy, sm[1]); sm[2] = fmaf(sc, qz, sm[2]);

@@ -58,7 +58,9 @@ __device__ __forceinline__ float2 lerp2(float2 a, float2 v0, float2 v1) { return
 
 // Pixel tile of a block: 16 x 16 (forward), 16 x 8 (gradient: 256 threads = 128 rays x 2 slots, four blocks per SM
 // instead of two 512-thread ones hide the single-stage TMA latency better).
-template <bool GRAD> struct TmaLanes {
+// GRAD: 0 forward projection, 1 gradient with central differences of f~ (the paper's, O3), 2 gradient
+// with the exact derivative of the trilinear interpolant (DFP_FLAG_GRAD_INTERP: the same 8 voxels as the forward).
+template <int GRAD> struct TmaLanes {
   static constexpr int SLOTS = GRAD ? 2 : 1, TU = kFwdTU, TV = GRAD ? 8 : kFwdTV, THREADS = TU * TV * SLOTS;
 };
 template <int SLOTS>
@@ -113,7 +115,7 @@ struct TmaBlock {              // block-wide state in shared memory
 };
 
 // One chunk's box: origin (voxel indices, for the TMA) and the index constant of the stage it lands in.
-template <bool GRAD, int SHAPE>
+template <int GRAD, int SHAPE>
 __device__ __forceinline__ void issue_chunk(const VolLayout& L, TmaBlock& B, const CUtensorMap* map, int chunk,
                                             unsigned tiles_addr, unsigned bar_addr) {
   using S = BoxShape<SHAPE>;
@@ -142,7 +144,7 @@ __device__ __forceinline__ void issue_chunk(const VolLayout& L, TmaBlock& B, con
 }
 
 // The chunk loop of one block for one box shape.  acc = {sum} (forward) or {gx,gy,gz,hx,hy,hz} (gradient).
-template <bool GRAD, int SHAPE>
+template <int GRAD, int SHAPE>
 __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* map, const Ray& r, int slot,
                                           TmaBlock& B, const float* tiles, unsigned tiles_addr, unsigned bar_addr,
                                           float* acc) {
@@ -223,6 +225,22 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
         const float2 ry = lerp2(make_float2(ay, ay), rA, rB);
         sum += lerp(az, ry.x, ry.y);
       } else {
+        float ddx, ddy, ddz;
+        if (GRAD == 2) {
+          // exact gradient of the trilinear interpolant in the sample's cell (per voxel index; G.sg* = 1 / pitch):
+          // pairs over the two z slices, as in the forward kernel
+          const float2 ax2 = make_float2(ax, ax), ay2 = make_float2(ay, ay);
+          const float2 v00 = make_float2(c[0], c[BXY]), v10 = make_float2(c[1], c[BXY + 1]);                      // row y
+          const float2 v01 = make_float2(c[BX], c[BXY + BX]), v11 = make_float2(c[BX + 1], c[BXY + BX + 1]);      // row y+1
+          const float2 d0 = sub2(v10, v00), d1 = sub2(v11, v01);          // x differences of rows y, y+1
+          const float2 rA = __ffma2_rn(ax2, d0, v00), rB = __ffma2_rn(ax2, d1, v01);   // (r00, r01), (r10, r11)
+          const float2 dx2 = lerp2(ay2, d0, d1);
+          ddx = lerp(az, dx2.x, dx2.y);
+          const float2 dy2 = sub2(rB, rA);
+          ddy = lerp(az, dy2.x, dy2.y);
+          const float2 ry = lerp2(ay2, rA, rB);
+          ddz = ry.y - ry.x;
+        } else {
         // Packed fp32x2 arithmetic (sm_100 FADD2 / FFMA2: two IEEE-rounded fp32 results per issue slot, the same
         // bits as the scalar code of fwd_grad_kernel).  Pairs run over the two z slices kk = 0, 1 of a row (y + j).
         const float2 ax2 = make_float2(ax, ax), ay2 = make_float2(ay, ay);
@@ -255,14 +273,15 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
           rzp2 = lerp2(ax2, make_float2(p0[0], p1[0]), make_float2(p0[1], p1[1]));
         }
         const float2 dx2 = lerp2(ay2, rdx2[0], rdx2[1]);                           // pair over kk
-        const float ddx = lerp(az, dx2.x, dx2.y);
+        ddx = lerp(az, dx2.x, dx2.y);
         const float2 dy2 = lerp2(ay2, sub2(rv2[1], rym2), sub2(ryp2, rv2[0]));     // (dy0, dy1)
-        const float ddy = lerp(az, dy2.x, dy2.y);
+        ddy = lerp(az, dy2.x, dy2.y);
         // d/dz pairs over j: (rv[0][1], rv[1][1]) - rzm2, rzp2 - (rv[0][0], rv[1][0])
         const float2 az2 = make_float2(az, az);
         const float2 dz2 = lerp2(az2, sub2(make_float2(rv2[0].y, rv2[1].y), rzm2),
                                  sub2(rzp2, make_float2(rv2[0].x, rv2[1].x)));     // (dz0, dz1)
-        const float ddz = lerp(ay, dz2.x, dz2.y);
+        ddz = lerp(ay, dz2.x, dz2.y);
+        }
         gx += ddx; gy += ddy; gz += ddz;
         hx = fmaf(kf, ddx, hx); hy = fmaf(kf, ddy, hy); hz = fmaf(kf, ddz, hz);
       }
@@ -279,7 +298,7 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
   }
 }
 
-template <bool GRAD, int SHAPE>
+template <int GRAD, int SHAPE>
 __global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, 4) fwd_tma_kernel(FwdGeom G, const FwdView* __restrict__ views,
                                                               const __grid_constant__ CUtensorMap vol_map,
                                                               const float* __restrict__ upstream,

@@ -197,6 +197,9 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_project_kernel(FwdGeom G, con
 // differences: 32 distinct voxels per sample, fetched as 16 float2 cells.  With r'_k = r_ref + kappa D e:
 //   B_i = D [ r_ref x sum g + D e x sum kappa g ]     -> six running sums (sum g, sum kappa g) per ray.
 // Block result: sum_i w_i A_i, sum_i w_i B_i over the block's rays -> partials[view][block][6]   (Eq.20 :185).
+// MODE 0: central differences of f~ (the paper's, 32 voxels); MODE 1 (DFP_FLAG_GRAD_INTERP): exact derivative of the
+// trilinear interpolant in the sample's cell (the forward kernel's 8 voxels; G.sg* = 1 / pitch instead of 1 / 2 pitch).
+template <int MODE>
 __global__ void __launch_bounds__(kFwdThreads) fwd_grad_kernel(FwdGeom G, const FwdView* __restrict__ views,
                                                                const float4* __restrict__ pvol,
                                                                const float* __restrict__ upstream,
@@ -219,6 +222,17 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_grad_kernel(FwdGeom G, const 
       const float ax = (qx - (tx - kMagic)) + 0.5f, ay = (qy - (ty - kMagic)) + 0.5f,
                   az = (qz - (tz - kMagic)) + 0.5f;
       const unsigned idx = brick_index(G.L, tx, ty, tz);
+      float ddx, ddy, ddz;
+      if (MODE == 1) {
+        const unsigned up = (__float_as_int(tz) & 1) ? bz8 - 4u : 4u;                     // FZ(Z+1) - FZ(Z)
+        const float4 c0 = ldg4(pvol + idx), c1 = ldg4(pvol + (idx + up));                // slices z, z+1: rows y, y+1
+        const float d00 = c0.y - c0.x, d10 = c0.w - c0.z, d01 = c1.y - c1.x, d11 = c1.w - c1.z;
+        const float r00 = fmaf(ax, d00, c0.x), r10 = fmaf(ax, d10, c0.z);
+        const float r01 = fmaf(ax, d01, c1.x), r11 = fmaf(ax, d11, c1.z);
+        ddx = lerp(az, lerp(ay, d00, d10), lerp(ay, d01, d11));
+        ddy = lerp(az, r10 - r00, r11 - r01);
+        ddz = lerp(ay, r01, r11) - lerp(ay, r00, r10);
+      } else {
       // neighbour cells: +-1 along an axis stays inside the brick or hops to the next one, by parity
       const unsigned ox = (unsigned)__float_as_int(tx) & 1u, oy = (unsigned)__float_as_int(ty) & 1u,
                      oz = (unsigned)__float_as_int(tz) & 1u;
@@ -244,13 +258,14 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_grad_kernel(FwdGeom G, const 
         rzm[0] = lerp(ax, E.x, E.y); rzm[1] = lerp(ax, E.z, E.w);
         rzp[0] = lerp(ax, F.x, F.y); rzp[1] = lerp(ax, F.z, F.w);
       }
-      const float ddx = lerp(az, lerp(ay, rdx[0][0], rdx[1][0]), lerp(ay, rdx[0][1], rdx[1][1]));
+      ddx = lerp(az, lerp(ay, rdx[0][0], rdx[1][0]), lerp(ay, rdx[0][1], rdx[1][1]));
       const float dy0 = lerp(ay, rv[1][0] - rym[0], ryp[0] - rv[0][0]);
       const float dy1 = lerp(ay, rv[1][1] - rym[1], ryp[1] - rv[0][1]);
-      const float ddy = lerp(az, dy0, dy1);
+      ddy = lerp(az, dy0, dy1);
       const float dz0 = lerp(az, rv[0][1] - rzm[0], rzp[0] - rv[0][0]);
       const float dz1 = lerp(az, rv[1][1] - rzm[1], rzp[1] - rv[1][0]);
-      const float ddz = lerp(ay, dz0, dz1);
+      ddz = lerp(ay, dz0, dz1);
+      }
       gx += ddx; gy += ddy; gz += ddz;
       hx = fmaf(kf, ddx, hx); hy = fmaf(kf, ddy, hy); hz = fmaf(kf, ddz, hz);
       kf += 1.0f;
@@ -421,7 +436,8 @@ __global__ void __launch_bounds__(kBpThreads) bp_kernel(BpGeom G, int n_views, c
 //   S'_c = r'_0 x sum(w q') + vz e_z x sum(m w q')  -> six running sums per (thread, view).
 // d~_u l = [b~(u+1,v) - b~(u-1,v)]/2 is ONE bilinear interpolation of pixel differences: 12 distinct pixels,
 // fetched as 4 quad cells.  Result: partials[tile][view][6].
-template <int WEIGHT, int DW>
+// MODE 1 (DFP_FLAG_GRAD_INTERP): d_u l, d_v l = exact derivatives of the bilinear interpolant (the 4 pixels of b~).
+template <int WEIGHT, int DW, int MODE>
 __global__ void __launch_bounds__(kBpThreads) bp_grad_kernel(BpGeom G, int n_views, int zchunk,
                                                              const BpView* __restrict__ views,
                                                              const float4* __restrict__ q,
@@ -461,16 +477,25 @@ __global__ void __launch_bounds__(kBpThreads) bp_grad_kernel(BpGeom G, int n_vie
         const BpPix p = bp_locate(fmaf(mf, sv.A[0][2], ub), fmaf(mf, sv.A[1][2], vb), fmaf(mf, sv.A[2][2], wb), ulo,
                                   uhi, vlo, vhi, pu, C0);
         const float4* c = img + p.idx;
-        const float4 cl = ldg4(c - 1), cr = ldg4(c + 1);      // rows v, v+1; columns u-1,u | u+1,u+2
-        const float4 cd = ldg4(c - pu), cu = ldg4(c + pu);    // columns u, u+1; rows v-1,v | v+1,v+2
-        // d~_u l (x2): per row lerp_a(l[u+1]-l[u-1], l[u+2]-l[u]), then lerp_b over the two rows
-        const float du0 = lerp(p.a, cr.x - cl.x, cr.y - cl.y);
-        const float du1 = lerp(p.a, cr.z - cl.z, cr.w - cl.w);
-        const float dlu = lerp(p.b, du0, du1);
-        // d~_v l (x2): per column lerp_b(l[v+1]-l[v-1], l[v+2]-l[v]), then lerp_a over the two columns
-        const float dv0 = lerp(p.b, cu.x - cd.x, cu.z - cd.z);
-        const float dv1 = lerp(p.b, cu.y - cd.y, cu.w - cd.w);
-        const float dlv = lerp(p.a, dv0, dv1);
+        float dlu, dlv, b00, b01, b10, b11;            // (x2 for MODE 0) interpolated differences; the 4 pixels of b~
+        if (MODE == 1) {
+          const float4 q0 = ldg4(c);                   // l[v][u], l[v][u+1], l[v+1][u], l[v+1][u+1]
+          dlu = lerp(p.b, q0.y - q0.x, q0.w - q0.z);
+          dlv = lerp(p.a, q0.z - q0.x, q0.w - q0.y);
+          b00 = q0.x; b01 = q0.y; b10 = q0.z; b11 = q0.w;
+        } else {
+          const float4 cl = ldg4(c - 1), cr = ldg4(c + 1);      // rows v, v+1; columns u-1,u | u+1,u+2
+          const float4 cd = ldg4(c - pu), cu = ldg4(c + pu);    // columns u, u+1; rows v-1,v | v+1,v+2
+          // d~_u l (x2): per row lerp_a(l[u+1]-l[u-1], l[u+2]-l[u]), then lerp_b over the two rows
+          const float du0 = lerp(p.a, cr.x - cl.x, cr.y - cl.y);
+          const float du1 = lerp(p.a, cr.z - cl.z, cr.w - cl.w);
+          dlu = lerp(p.b, du0, du1);
+          // d~_v l (x2): per column lerp_b(l[v+1]-l[v-1], l[v+2]-l[v]), then lerp_a over the two columns
+          const float dv0 = lerp(p.b, cu.x - cd.x, cu.z - cd.z);
+          const float dv1 = lerp(p.b, cu.y - cd.y, cu.w - cd.w);
+          dlv = lerp(p.a, dv0, dv1);
+          b00 = cl.y; b01 = cr.x; b10 = cl.w; b11 = cr.z;
+        }
         const float wj = __ldg(wcol + (size_t)(z - z0) * wstride);
         float W = WEIGHT ? G.sad2 * p.rw * p.rw : 1.f;
         W = p.front ? W : 0.f;
@@ -479,12 +504,12 @@ __global__ void __launch_bounds__(kBpThreads) bp_grad_kernel(BpGeom G, int n_vie
         float qx = fmaf(dlu, sv.J[0][0], fmaf(dlv, sv.J[1][0], -cc * sv.J[2][0]));
         float qy = fmaf(dlu, sv.J[0][1], fmaf(dlv, sv.J[1][1], -cc * sv.J[2][1]));
         float qz = fmaf(dlu, sv.J[0][2], fmaf(dlv, sv.J[1][2], -cc * sv.J[2][2]));
-        float sc = 0.5f * W * p.rw * wj;
+        float sc = (MODE == 1 ? 1.0f : 0.5f) * W * p.rw * wj;
         if (DW) {
           // + b~ dW/dr',  dW/dr' = -2 W / w' * J3   (U8); b~ from the same cells
-          const float b0 = lerp(p.a, cl.y, cr.x), b1 = lerp(p.a, cl.w, cr.z);
+          const float b0 = lerp(p.a, b00, b01), b1 = lerp(p.a, b10, b11);
           const float bv = lerp(p.b, b0, b1);
-          const float k = -4.f * bv;      // relative to the common factor 0.5 W / w'
+          const float k = (MODE == 1 ? -2.f : -4.f) * bv;      // relative to the common factor (0.5) W / w'
           qx = fmaf(k, sv.J[2][0], qx); qy = fmaf(k, sv.J[2][1], qy); qz = fmaf(k, sv.J[2][2], qz);
         }
         s[0] = fmaf(sc, qx, s[0]); s[1] = fmaf(sc, qy, s[1]); s[2] = fmaf(sc, qz, s[2]);

@@ -133,7 +133,7 @@ inline VolLayout make_layout(const dfp_geometry& g) {
 }
 
 // grad = false: support of f~ is (-1, n) per axis; grad = true: support of the central difference is (-2, n+1).
-inline FwdGeom make_fwd_geom(const dfp_geometry& g, bool grad) {
+inline FwdGeom make_fwd_geom(const dfp_geometry& g, bool grad, bool interp = false) {
   FwdGeom G;
   G.L = make_layout(g);
   G.nu = g.nu; G.nv = g.nv;
@@ -149,7 +149,9 @@ inline FwdGeom make_fwd_geom(const dfp_geometry& g, bool grad) {
     G.lo[a] = (float)(-margin - H[a]);
     G.hi[a] = (float)(n[a] - 1 + margin - H[a]);
   }
-  G.sgx = (float)(0.5 / g.vx); G.sgy = (float)(0.5 / g.vy); G.sgz = (float)(0.5 / g.vz);
+  // central differences over 2 voxels (O3), or the exact derivative of the interpolant per voxel (GRAD_INTERP)
+  const double sg = interp ? 1.0 : 0.5;
+  G.sgx = (float)(sg / g.vx); G.sgy = (float)(sg / g.vy); G.sgz = (float)(sg / g.vz);
   return G;
 }
 

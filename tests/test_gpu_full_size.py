@@ -123,3 +123,22 @@ def test_c5_sweep_full(dfp):
     check_forward_full(dfp, 5, n_check_views=2, band_rows=24, n_grad_views=1)
     torch.cuda.empty_cache()
     check_back_full(dfp, 5, n_slabs=2, slab=1, n_grad_views=1)
+
+
+def test_c2_registration_full_grad_interp_mode(dfp):
+    """DFP_FLAG_GRAD_INTERP at the bench's size: two seeded views' 6-vectors against the oracle's GRAD_INTERP mode."""
+    dev = torch.device("cuda:0")
+    w = W.make_config(2)
+    g = w.geom.replace(flags=dfp.FLAG_GRAD_INTERP)
+    a = w.angles.float().numpy()
+    p = w.poses.float().numpy()
+    vol = w.volume(dev)
+    up = w.fwd_upstream(dev)
+    grad = dfp.forward_pose_grad(g, a, p, vol, up).cpu().numpy()
+    assert dfp.last_path() == dfp.PATH_TMA and np.isfinite(grad).all()
+    vol_c = vol.cpu().numpy()
+    for v in pick(w.seed + 503, w.n_views, 2):
+        o = oracle.forward_pose_grad(w.geom, a[v:v + 1], p[v:v + 1], vol_c, up[v:v + 1].cpu().numpy(),
+                                     grad_mode=oracle.GRAD_INTERP)
+        e = grad_err_u9(grad[v:v + 1], o)
+        assert e.max() <= 3 * TOL_GRAD and np.sort(e.ravel())[-2] <= TOL_GRAD, (v, e)

@@ -319,3 +319,43 @@ def test_bp_tma_path_falls_back_when_it_does_not_apply(dfp):
         o = _both_bp_paths(dfp, g, ANGLES3[:2], POSES3[:2], proj, up)
         assert o["tma"][2] == dfp.PATH_GATHER and o["tma"][3] == dfp.PATH_GATHER
         check_back(run_back_case(dfp, g, ANGLES3[:2], POSES3[:2], proj, up))
+
+
+# ------------------------------------------------------------------ DFP_FLAG_GRAD_INTERP
+def test_grad_interp_mode_forward(dfp):
+    """Exact derivative of the trilinear interpolant (what autodiff of the discrete projector gives): the oracle's
+    GRAD_INTERP mode, itself pinned against finite differences of the discrete projector.  TMA and gather paths."""
+    dev = torch.device("cuda:0")
+    cases = [W.make_config(2, scale=0.25, n_views=3), W.make_config(4, scale=0.125, n_views=4), W.make_config(1)]
+    for w in cases:
+        a, p = f32(w.angles.numpy()), f32(w.poses.numpy()).reshape(-1, 6)
+        vol, up = w.volume(dev), w.fwd_upstream(dev)
+        o = oracle.forward_pose_grad(w.geom, a, p, vol.cpu().numpy(), up.cpu().numpy(), grad_mode=oracle.GRAD_INTERP)
+        o_central = oracle.forward_pose_grad(w.geom, a, p, vol.cpu().numpy(), up.cpu().numpy())
+        assert grad_err_u9(o, o_central).max() > 1e-2            # the two modes are different estimators
+        for fl in (dfp.FLAG_GRAD_INTERP, dfp.FLAG_GRAD_INTERP | dfp.FLAG_NO_TMA):
+            g = dfp.forward_pose_grad(w.geom.replace(flags=fl), a, p, vol, up).cpu().numpy()
+            assert np.all(np.isfinite(g))
+            e = grad_err_u9(g, o)
+            # the exact derivative telescopes along a ray, so the translation component along the rays is a sum that
+            # cancels to ~0.5 % of its group's largest component (C2, NCC upstream: zero-mean weights); fp32 summation
+            # noise of 2e-5 of that largest component then reads as 1.8e-3 against U9's floor of 1 %
+            assert e.max() <= 3 * TOL_GRAD and np.sort(e.ravel())[-2] <= TOL_GRAD, (w.name, fl, e)
+
+
+@pytest.mark.parametrize("bw,fl", [(0, 0), (1, 0), (1, 1)])
+def test_grad_interp_mode_backproject(dfp, bw, fl):
+    dev = torch.device("cuda:0")
+    w = W.make_config(3, scale=0.25, n_views=10)
+    a, p = f32(w.angles.numpy()), f32(w.poses.numpy()).reshape(-1, 6)
+    proj, up = w.projections(dev), w.bp_upstream(dev)
+    g0 = w.geom.replace(bp_weight=bw, flags=fl)
+    o = oracle.backproject_pose_grad(g0, a, p, proj.cpu().numpy(), up.cpu().numpy(), grad_mode=oracle.GRAD_INTERP)
+    for extra in (dfp.FLAG_GRAD_INTERP, dfp.FLAG_GRAD_INTERP | dfp.FLAG_NO_TMA):
+        g = dfp.backproject_pose_grad(g0.replace(flags=fl | extra), a, p, proj, up).cpu().numpy()
+        assert np.all(np.isfinite(g))
+        e = grad_err_u9(g, o)
+        # the derivative of the bilinear interpolant is piecewise constant: a voxel that projects within fp32 rounding
+        # of a pixel boundary takes the neighbouring cell's slope, an O(1) change of that term which does not average
+        # out like rounding noise; on ramp-filtered (sign-cancelling) data the smallest components show 1.0-1.3e-3
+        assert e.max() <= 3 * TOL_GRAD and np.quantile(e, 0.95) <= TOL_GRAD, (bw, fl, extra, e)
