@@ -280,6 +280,20 @@ def main():
         b_.record()
         torch.cuda.synchronize()
         interp_ms.append(a_.elapsed_time(b_) / 3)
+    # dfp_forward_fused_moments: projection + gradient moments in one traversal (target = the upstream array's shape)
+    ws_f = torch.empty(dfp.workspace_bytes(g, V, dfp.OP_FORWARD_FUSED), dtype=torch.uint8, device=dev)
+    mom = torch.empty((V, 3, 6), dtype=torch.float32, device=dev)
+    proj_f = torch.empty_like(proj)
+    fused = lambda: dfp.forward_fused_moments(g, angles, poses, vol, up, out_proj=proj_f, out_moments=mom, ws=ws_f)
+    fused()
+    a_, b_ = ev(), ev()
+    a_.record()
+    for _ in range(3):
+        fused()
+    b_.record()
+    torch.cuda.synchronize()
+    fused_ms = a_.elapsed_time(b_) / 3
+    del ws_f, proj_f
     dfp.forward_pose_grad(g, angles, poses, vol, up, out=grad, ws=ws)          # leave the default-mode results behind
     dfp.backproject_pose_grad(g, angles, poses, proj, bp_up, out=bgrad, ws=ws)
 
@@ -378,7 +392,9 @@ def main():
                                      "backproject": float(seg[:, 2].mean()),
                                      "backproject_pose_grad": float(seg[:, 3].mean())},
                      "grad_interp_mode_ms_per_call": {"forward_pose_grad": interp_ms[0],
-                                                      "backproject_pose_grad": interp_ms[1]}},
+                                                      "backproject_pose_grad": interp_ms[1]},
+                     "forward_fused_moments_ms_per_call": fused_ms,
+                     "forward_fused_moments_gray_steps_per_s": 2.0 * ray_steps / (fused_ms * 1e-3) / 1e9},
            "clocks": clocks, "e2e": e2e, "gpu_launches": n_launch, "roofline": roofline, "cpu_baseline": cpu}
     print(json.dumps(out), flush=True)
     if dist is not None:

@@ -65,7 +65,8 @@ enum {
   DFP_ERR_WORKSPACE = -5,  /* ws_bytes < dfp_workspace_bytes(...)                                           */
   DFP_ERR_CUDA = -6        /* CUDA runtime error (no device, launch failure, out of memory in *_host)       */
 };
-enum { DFP_OP_FORWARD = 0, DFP_OP_FORWARD_POSE_GRAD = 1, DFP_OP_BACKPROJECT = 2, DFP_OP_BACKPROJECT_POSE_GRAD = 3 };
+enum { DFP_OP_FORWARD = 0, DFP_OP_FORWARD_POSE_GRAD = 1, DFP_OP_BACKPROJECT = 2, DFP_OP_BACKPROJECT_POSE_GRAD = 3,
+       DFP_OP_FORWARD_FUSED = 4 };
 enum { DFP_FLAG_DW = 1, DFP_FLAG_NO_TMA = 2, DFP_FLAG_GRAD_INTERP = 4 };
 
 /* Forward projection, Eq.2a :67-69 discretised as Eq.18 :172-177 with a fixed-step, zero-extended
@@ -92,6 +93,22 @@ int dfp_backproject(const dfp_geometry* geometry, int n_views, const float* angl
  * G_b never materialised.  d_grad is overwritten. */
 int dfp_backproject_pose_grad(const dfp_geometry* geometry, int n_views, const float* angles, const float* poses,
                               const float* d_proj, const float* d_dLdvol, float* d_grad, void* d_ws,
+                              size_t ws_bytes, void* stream);
+
+/* Fused forward projection + pose-gradient MOMENTS in one traversal of the volume (an extension beyond the paper's
+ * four operations).  For a loss whose upstream gradient is affine in the projection,
+ *     dL/dl_i = alpha_v + beta_v * l_i + gamma_v * b_i        (b = a target image: SSD, NCC - PAPER.md Eq.23, 25)
+ * with per-view scalars known only AFTER l is (means, norms), the gradient of Eq.20 (:185) is
+ *     dL/dtheta_v = alpha_v m[v][0] + beta_v m[v][1] + gamma_v m[v][2],
+ *     m[v][0] = sum_i dl_i/dtheta_v,   m[v][1] = sum_i l_i dl_i/dtheta_v,   m[v][2] = sum_i b_i dl_i/dtheta_v,
+ * so one pass that writes l AND the three 6-vectors replaces dfp_forward followed by dfp_forward_pose_grad.
+ * d_target: device [n_views][nv][nu] (b); d_proj: device, out, [n_views][nv][nu] (l, as dfp_forward up to fp32
+ * summation order); d_moments: device, out, [n_views][3][6], each 6-vector laid out and scaled exactly like the
+ * output of dfp_forward_pose_grad with upstream 1, l, b.  Central-difference gradient mode only (DFP_ERR_DIMS with
+ * DFP_FLAG_GRAD_INTERP).  Workspace: dfp_workspace_bytes(geometry, n_views, DFP_OP_FORWARD_FUSED).  Same ownership,
+ * asynchrony and error behaviour as the four calls above. */
+int dfp_forward_fused_moments(const dfp_geometry* geometry, int n_views, const float* angles, const float* poses,
+                              const float* d_vol, const float* d_target, float* d_proj, float* d_moments, void* d_ws,
                               size_t ws_bytes, void* stream);
 
 /* Bytes of device workspace the op needs for this geometry and view count (0 on invalid arguments).

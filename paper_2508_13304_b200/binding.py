@@ -13,7 +13,7 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libdfp.so")
 
-OP_FORWARD, OP_FORWARD_POSE_GRAD, OP_BACKPROJECT, OP_BACKPROJECT_POSE_GRAD = 0, 1, 2, 3
+OP_FORWARD, OP_FORWARD_POSE_GRAD, OP_BACKPROJECT, OP_BACKPROJECT_POSE_GRAD, OP_FORWARD_FUSED = 0, 1, 2, 3, 4
 FLAG_DW = 1
 FLAG_NO_TMA = 2
 FLAG_GRAD_INTERP = 4
@@ -65,6 +65,8 @@ def _load():
     lib.dfp_backproject.argtypes = dev
     lib.dfp_forward_pose_grad.argtypes = devg
     lib.dfp_backproject_pose_grad.argtypes = devg
+    lib.dfp_forward_fused_moments.argtypes = [gp, ci, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.dfp_forward_fused_moments.restype = ci
     lib.dfp_forward_host.argtypes = [gp, ci, vp, vp, vp, vp, vp]
     lib.dfp_backproject_host.argtypes = [gp, ci, vp, vp, vp, vp, vp]
     lib.dfp_forward_pose_grad_host.argtypes = [gp, ci, vp, vp, vp, vp, vp, vp]
@@ -189,6 +191,23 @@ def forward_pose_grad(geom, angles, poses, vol, dLdproj, out=None, ws=None):
                                       _dev(dLdproj, (V, g.nv, g.nu), "dLdproj"), _dev(out, (V, 6), "grad"), wp, wn,
                                       _stream()))
     return out
+
+
+def forward_fused_moments(geom, angles, poses, vol, target, out_proj=None, out_moments=None, ws=None):
+    """dfp_forward_fused_moments: vol, target [V,nv,nu] -> (proj [V,nv,nu], moments [V,3,6]) in one traversal."""
+    g = Geometry.of(geom)
+    a, p, V = _views(angles, poses)
+    if out_proj is None:
+        out_proj = torch.empty((V, g.nv, g.nu), dtype=torch.float32, device=vol.device)
+    if out_moments is None:
+        out_moments = torch.empty((V, 3, 6), dtype=torch.float32, device=vol.device)
+    ws, wp, wn = _workspace(g, V, OP_FORWARD_FUSED, ws, vol.device)
+    _check(_lib.dfp_forward_fused_moments(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p),
+                                          _dev(vol, (g.nz, g.ny, g.nx), "vol"),
+                                          _dev(target, (V, g.nv, g.nu), "target"),
+                                          _dev(out_proj, (V, g.nv, g.nu), "proj"),
+                                          _dev(out_moments, (V, 3, 6), "moments"), wp, wn, _stream()))
+    return out_proj, out_moments
 
 
 def backproject(geom, angles, poses, proj, out=None, ws=None):

@@ -207,7 +207,7 @@ struct FwdWs {
   int gx, gy;     // blocks per view (16 x 16-pixel tiles)
   int gy8;        // rows of 16 x 8-pixel tiles (TMA gradient kernel)
 };
-FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad) {
+FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad, int nset = 1) {
   FwdWs w;
   const VolLayout L = make_layout(g);
   w.gx = (g.nu + kFwdTU - 1) / kFwdTU;
@@ -217,7 +217,7 @@ FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad) {
   w.off_views = o; o += align_up(sizeof(FwdView) * (size_t)V);
   w.off_con = o;   o += grad ? align_up(sizeof(FwdContract) * (size_t)V) : 0;
   w.off_pvol = o;  o += align_up(sizeof(float4) * (size_t)L.px * L.py * L.pz);
-  w.off_part = o;  o += grad ? align_up(sizeof(float) * 6 * (size_t)V * w.gx * w.gy8) : 0;
+  w.off_part = o;  o += grad ? align_up(sizeof(float) * 6 * (size_t)nset * V * w.gx * w.gy8) : 0;
   w.total = o;
   return w;
 }
@@ -268,12 +268,19 @@ int check_common(const dfp_geometry* g, int n_views, const float* angles, const 
   return DFP_OK;
 }
 
+// op = DFP_OP_FORWARD (d_out = projections), DFP_OP_FORWARD_POSE_GRAD (d_up = upstream, d_out = gradients) or
+// DFP_OP_FORWARD_FUSED (d_up = target b, d_out = moments [V][3][6], d_proj = projections)
 int run_forward(const dfp_geometry* g, int V, const float* angles, const float* poses, const float* d_vol,
-                const float* d_up, float* d_out, void* d_ws, size_t ws_bytes, cudaStream_t s, bool grad) {
+                const float* d_up, float* d_out, void* d_ws, size_t ws_bytes, cudaStream_t s, int op,
+                float* d_proj = nullptr) {
   if (!g) return DFP_ERR_NULL;
   int st = validate_geometry(g);
   if (st) return st;
-  const FwdWs w = fwd_ws(*g, V, grad);
+  const bool grad = op != DFP_OP_FORWARD, fused = op == DFP_OP_FORWARD_FUSED;
+  if (fused && (!d_proj || !aligned(d_proj, 16))) return d_proj ? DFP_ERR_ALIGN : DFP_ERR_NULL;
+  if (fused && (g->flags & DFP_FLAG_GRAD_INTERP)) return DFP_ERR_DIMS;      // fused moments: central differences only
+  const int nset = fused ? 3 : 1;
+  const FwdWs w = fwd_ws(*g, V, grad, nset);
   st = check_common(g, V, angles, poses, d_vol, d_out, grad ? (const void*)d_up : (const void*)d_vol, d_ws,
                         ws_bytes, w.total);
   if (st) return st;
@@ -324,27 +331,36 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
         cudaFuncSetAttribute(fwd_tma_kernel<2, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<3>()),
         cudaFuncSetAttribute(fwd_tma_kernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<2>())};
     for (cudaError_t e : attr3) DFP_CUDA(e, "cudaFuncSetAttribute");
+    static const cudaError_t attr4[2] = {
+        cudaFuncSetAttribute(fwd_tma_kernel<3, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<3>()),
+        cudaFuncSetAttribute(fwd_tma_kernel<3, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<2>())};
+    for (cudaError_t e : attr4) DFP_CUDA(e, "cudaFuncSetAttribute");
     for (cudaError_t e : attr) DFP_CUDA(e, "cudaFuncSetAttribute");
     time_begin(s);
     const dim3 ggrid(w.gx, w.gy8, V);
-    if (grad && interp && shape == 3)
-      fwd_tma_kernel<2, 3><<<ggrid, TmaLanes<2>::THREADS, tma_smem_bytes<3>(), s>>>(G, dv, vol_map, d_up, part);
+    if (fused && shape == 3)
+      fwd_tma_kernel<3, 3><<<ggrid, TmaLanes<3>::THREADS, tma_smem_bytes<3>(), s>>>(G, dv, vol_map, d_up, part, d_proj);
+    else if (fused)
+      fwd_tma_kernel<3, 2><<<ggrid, TmaLanes<3>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, d_up, part, d_proj);
+    else if (grad && interp && shape == 3)
+      fwd_tma_kernel<2, 3><<<ggrid, TmaLanes<2>::THREADS, tma_smem_bytes<3>(), s>>>(G, dv, vol_map, d_up, part, nullptr);
     else if (grad && interp)
-      fwd_tma_kernel<2, 2><<<ggrid, TmaLanes<2>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, d_up, part);
+      fwd_tma_kernel<2, 2><<<ggrid, TmaLanes<2>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, d_up, part, nullptr);
     else if (grad && shape == 3)
-      fwd_tma_kernel<1, 3><<<ggrid, TmaLanes<1>::THREADS, tma_smem_bytes<3>(), s>>>(G, dv, vol_map, d_up, part);
+      fwd_tma_kernel<1, 3><<<ggrid, TmaLanes<1>::THREADS, tma_smem_bytes<3>(), s>>>(G, dv, vol_map, d_up, part, nullptr);
     else if (grad)
-      fwd_tma_kernel<1, 2><<<ggrid, TmaLanes<1>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, d_up, part);
+      fwd_tma_kernel<1, 2><<<ggrid, TmaLanes<1>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, d_up, part, nullptr);
     else if (shape == 0)
-      fwd_tma_kernel<0, 0><<<grid, TmaLanes<0>::THREADS, tma_smem_bytes<0>(), s>>>(G, dv, vol_map, nullptr, d_out);
+      fwd_tma_kernel<0, 0><<<grid, TmaLanes<0>::THREADS, tma_smem_bytes<0>(), s>>>(G, dv, vol_map, nullptr, d_out, nullptr);
     else if (shape == 1)
-      fwd_tma_kernel<0, 1><<<grid, TmaLanes<0>::THREADS, tma_smem_bytes<1>(), s>>>(G, dv, vol_map, nullptr, d_out);
+      fwd_tma_kernel<0, 1><<<grid, TmaLanes<0>::THREADS, tma_smem_bytes<1>(), s>>>(G, dv, vol_map, nullptr, d_out, nullptr);
     else
-      fwd_tma_kernel<0, 2><<<grid, TmaLanes<0>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, nullptr, d_out);
+      fwd_tma_kernel<0, 2><<<grid, TmaLanes<0>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, nullptr, d_out, nullptr);
     time_end(s);
     ++g_launches;
-    if (grad) {
-      fwd_contract_kernel<<<V, 256, 0, s>>>(w.gx * w.gy8, part, dc, d_out);
+    const int nblk8 = w.gx * w.gy8;
+    for (int set = 0; grad && set < nset; ++set) {       // fused: one contraction per weight set -> moments[v][set][6]
+      fwd_contract_kernel<<<V, 256, 0, s>>>(nblk8, part + (size_t)set * V * nblk8 * 6, dc, d_out, 6 * nset, 6 * set);
       ++g_launches;
     }
     DFP_CUDA(cudaGetLastError(), "forward launch (TMA path)");
@@ -353,7 +369,21 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
   const size_t ncell = (size_t)G.L.px * G.L.py * G.L.pz;
   pack_volume_kernel<<<grid_1d(ncell, 256), 256, 0, s>>>(G.L, d_vol, pvol);
   ++g_launches;
-  if (!grad) {
+  if (fused) {
+    // gather fallback of the fused call, composed from the two gather kernels: projections, then the three
+    // weight sets (unit, l, b) one gradient pass each (this path trades the fusion for generality)
+    const int nblk = w.gx * w.gy;
+    fwd_project_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, pvol, d_proj);
+    ++g_launches;
+    const float* ups[3] = {nullptr, d_proj, d_up};
+    time_begin(s);
+    for (int set = 0; set < 3; ++set) {
+      fwd_grad_kernel<0><<<grid, kFwdThreads, 0, s>>>(G, dv, pvol, ups[set], part + (size_t)set * V * nblk * 6);
+      fwd_contract_kernel<<<V, 256, 0, s>>>(nblk, part + (size_t)set * V * nblk * 6, dc, d_out, 18, 6 * set);
+      g_launches += 2;
+    }
+    time_end(s);
+  } else if (!grad) {
     time_begin(s);
     fwd_project_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, pvol, d_out);
     time_end(s);
@@ -515,7 +545,7 @@ int run_host(int op, const dfp_geometry* g, int V, const float* angles, const fl
   if (grad) DFP_CUDA(cudaMemcpyAsync(d_up.p, h_up, n_up, cudaMemcpyHostToDevice, s), "H2D");
   if (fwd)
     st = run_forward(g, V, angles, poses, (const float*)d_in.p, (const float*)d_up.p, (float*)d_out.p, d_ws.p, n_ws, s,
-                     grad);
+                     grad ? DFP_OP_FORWARD_POSE_GRAD : DFP_OP_FORWARD);
   else
     st = run_backproject(g, V, angles, poses, (const float*)d_in.p, (const float*)d_up.p, (float*)d_out.p, d_ws.p,
                          n_ws, s, grad);
@@ -532,14 +562,21 @@ extern "C" {
 int dfp_forward(const dfp_geometry* g, int n_views, const float* angles, const float* poses, const float* d_vol,
                 float* d_proj, void* d_ws, size_t ws_bytes, void* stream) {
   return run_forward(g, n_views, angles, poses, d_vol, nullptr, d_proj, d_ws, ws_bytes,
-                     static_cast<cudaStream_t>(stream), false);
+                     static_cast<cudaStream_t>(stream), DFP_OP_FORWARD);
 }
 
 int dfp_forward_pose_grad(const dfp_geometry* g, int n_views, const float* angles, const float* poses,
                           const float* d_vol, const float* d_dLdproj, float* d_grad, void* d_ws, size_t ws_bytes,
                           void* stream) {
   return run_forward(g, n_views, angles, poses, d_vol, d_dLdproj, d_grad, d_ws, ws_bytes,
-                     static_cast<cudaStream_t>(stream), true);
+                     static_cast<cudaStream_t>(stream), DFP_OP_FORWARD_POSE_GRAD);
+}
+
+int dfp_forward_fused_moments(const dfp_geometry* g, int n_views, const float* angles, const float* poses,
+                              const float* d_vol, const float* d_target, float* d_proj, float* d_moments, void* d_ws,
+                              size_t ws_bytes, void* stream) {
+  return run_forward(g, n_views, angles, poses, d_vol, d_target, d_moments, d_ws, ws_bytes,
+                     static_cast<cudaStream_t>(stream), DFP_OP_FORWARD_FUSED, d_proj);
 }
 
 int dfp_backproject(const dfp_geometry* g, int n_views, const float* angles, const float* poses, const float* d_proj,
@@ -562,6 +599,7 @@ size_t dfp_workspace_bytes(const dfp_geometry* g, int n_views, int op) {
     case DFP_OP_FORWARD_POSE_GRAD: return fwd_ws(*g, n_views, true).total;
     case DFP_OP_BACKPROJECT: return bp_ws(*g, n_views, false).total;
     case DFP_OP_BACKPROJECT_POSE_GRAD: return bp_ws(*g, n_views, true).total;
+    case DFP_OP_FORWARD_FUSED: return fwd_ws(*g, n_views, true, 3).total;
     default: return 0;
   }
 }

@@ -59,7 +59,8 @@ __device__ __forceinline__ float2 lerp2(float2 a, float2 v0, float2 v1) { return
 // Pixel tile of a block: 16 x 16 (forward), 16 x 8 (gradient: 256 threads = 128 rays x 2 slots, four blocks per SM
 // instead of two 512-thread ones hide the single-stage TMA latency better).
 // GRAD: 0 forward projection, 1 gradient with central differences of f~ (the paper's, O3), 2 gradient
-// with the exact derivative of the trilinear interpolant (DFP_FLAG_GRAD_INTERP: the same 8 voxels as the forward).
+// with the exact derivative of the trilinear interpolant (DFP_FLAG_GRAD_INTERP: the same 8 voxels as the forward),
+// 3 FUSED projection + central-difference gradient moments in one traversal (dfp_forward_fused_moments).
 template <int GRAD> struct TmaLanes {
   static constexpr int SLOTS = GRAD ? 2 : 1, TU = kFwdTU, TV = GRAD ? 8 : kFwdTV, THREADS = TU * TV * SLOTS;
 };
@@ -281,6 +282,10 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
         const float2 dz2 = lerp2(az2, sub2(make_float2(rv2[0].y, rv2[1].y), rzm2),
                                  sub2(rzp2, make_float2(rv2[0].x, rv2[1].x)));     // (dz0, dz1)
         ddz = lerp(ay, dz2.x, dz2.y);
+        if (GRAD == 3) {                 // fused: the projection itself, from the core rows already interpolated in x
+          const float2 ry = lerp2(ay2, rv2[0], rv2[1]);
+          sum += lerp(az, ry.x, ry.y);
+        }
         }
         gx += ddx; gy += ddy; gz += ddz;
         hx = fmaf(kf, ddx, hx); hy = fmaf(kf, ddy, hy); hz = fmaf(kf, ddz, hz);
@@ -295,6 +300,7 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
     acc[0] = sum;
   } else {
     acc[0] = gx; acc[1] = gy; acc[2] = gz; acc[3] = hx; acc[4] = hy; acc[5] = hz;
+    if (GRAD == 3) acc[6] = sum;
   }
 }
 
@@ -302,11 +308,13 @@ template <int GRAD, int SHAPE>
 __global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, 4) fwd_tma_kernel(FwdGeom G, const FwdView* __restrict__ views,
                                                               const __grid_constant__ CUtensorMap vol_map,
                                                               const float* __restrict__ upstream,
-                                                              float* __restrict__ out) {
+                                                              float* __restrict__ out,
+                                                              float* __restrict__ proj_out) {
+  constexpr int NSET = GRAD == 3 ? 3 : 1;              // weight sets of the per-view reduction (fused: 1, l, b)
   extern __shared__ __align__(128) float tiles[];      // STAGES boxes
   __shared__ __align__(8) unsigned long long full_bar[kMaxStages];
   __shared__ TmaBlock B;
-  __shared__ float red[TmaLanes<GRAD>::THREADS / 32][6];
+  __shared__ float red[TmaLanes<GRAD>::THREADS / 32][6 * NSET];
 
   int iu, iv, slot;
   tma_pixel<TmaLanes<GRAD>::SLOTS>(iu, iv, slot);
@@ -357,12 +365,12 @@ __global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, 4) fwd_tma_kernel(Fwd
     }
   }
   __syncthreads();
-  float acc[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  float acc[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   tma_march<GRAD, SHAPE>(G, &vol_map, r, slot, B, tiles, tiles_addr, bar_addr, acc);
   // the two slots of a ray: even-kappa partial sums + odd-kappa partial sums
   if (TmaLanes<GRAD>::SLOTS == 2) {
 #pragma unroll
-    for (int q = 0; q < (GRAD ? 6 : 1); ++q) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], 16);
+    for (int q = 0; q < (GRAD == 3 ? 7 : GRAD ? 6 : 1); ++q) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], 16);
   }
 
   const float bad = B.Kc < 0 ? __int_as_float(0x7fc00000) : 0.f;   // NaN: the box cannot hold the tile (host bound wrong)
@@ -370,21 +378,35 @@ __global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, 4) fwd_tma_kernel(Fwd
     if (live && slot == 0) out[((size_t)view * G.nv + iv) * G.nu + iu] = G.step * acc[0] + bad;
     return;
   }
-  float o6[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  float o6[6 * NSET];
+#pragma unroll
+  for (int q = 0; q < 6 * NSET; ++q) o6[q] = 0.f;
   if (live && slot == 0) {
     const float gx = acc[0], gy = acc[1], gz = acc[2], hx = acc[3], hy = acc[4], hz = acc[5];
-    const float w = __ldg(upstream + ((size_t)view * G.nv + iv) * G.nu + iu);
+    const size_t pix = ((size_t)view * G.nv + iv) * G.nu + iu;
     const float D = G.step;
     const float sx = gx * G.sgx, sy = gy * G.sgy, sz = gz * G.sgz;
     const float mx = hx * G.sgx * D, my = hy * G.sgy * D, mz = hz * G.sgz * D;
-    const float wd = w * D;
-    o6[0] = wd * sx + bad; o6[1] = wd * sy; o6[2] = wd * sz;
-    o6[3] = wd * ((py * sz - pz * sy) + (ey * mz - ez * my));
-    o6[4] = wd * ((pz * sx - px * sz) + (ez * mx - ex * mz));
-    o6[5] = wd * ((px * sy - py * sx) + (ex * my - ey * mx));
+    const float c3 = (py * sz - pz * sy) + (ey * mz - ez * my);
+    const float c4 = (pz * sx - px * sz) + (ez * mx - ex * mz);
+    const float c5 = (px * sy - py * sx) + (ex * my - ey * mx);
+    float wset[NSET];
+    if (GRAD == 3) {
+      const float l = D * acc[6] + bad;
+      proj_out[pix] = l;
+      wset[0] = 1.f; wset[NSET > 1 ? 1 : 0] = l; wset[NSET > 2 ? 2 : 0] = __ldg(upstream + pix);   // upstream = target b
+    } else {
+      wset[0] = __ldg(upstream + pix);
+    }
+#pragma unroll
+    for (int j = 0; j < NSET; ++j) {
+      const float wd = wset[j] * D;
+      o6[6 * j + 0] = wd * sx + bad; o6[6 * j + 1] = wd * sy; o6[6 * j + 2] = wd * sz;
+      o6[6 * j + 3] = wd * c3; o6[6 * j + 4] = wd * c4; o6[6 * j + 5] = wd * c5;
+    }
   }
 #pragma unroll
-  for (int q = 0; q < 6; ++q) {
+  for (int q = 0; q < 6 * NSET; ++q) {
     float v = o6[q];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -393,16 +415,18 @@ __global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, 4) fwd_tma_kernel(Fwd
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   if (lane == 0) {
 #pragma unroll
-    for (int q = 0; q < 6; ++q) red[warp][q] = o6[q];
+    for (int q = 0; q < 6 * NSET; ++q) red[warp][q] = o6[q];
   }
   __syncthreads();
-  if (threadIdx.x < 6) {
+  if (threadIdx.x < 6 * NSET) {
     float t = 0.f;
 #pragma unroll
     for (int wI = 0; wI < TmaLanes<GRAD>::THREADS / 32; ++wI) t += red[wI][threadIdx.x];
     const size_t blk = (size_t)blockIdx.y * gridDim.x + blockIdx.x;
     const size_t nblk = (size_t)gridDim.x * gridDim.y;
-    out[((size_t)view * nblk + blk) * 6 + threadIdx.x] = t;
+    // partials[set][view][block][6]: each weight set is a plain gradient partial array for fwd_contract_kernel
+    const int set = threadIdx.x / 6, k = threadIdx.x % 6;
+    out[(((size_t)set * gridDim.z + view) * nblk + blk) * 6 + k] = t;
   }
 }
 

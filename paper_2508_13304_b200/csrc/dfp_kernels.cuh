@@ -271,7 +271,7 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_grad_kernel(FwdGeom G, const 
       kf += 1.0f;
     }
     // per-ray epilogue (once per ray): scale to per-mm gradients, lever arm about the reference sample
-    const float w = __ldg(upstream + ((size_t)view * G.nv + iv) * G.nu + iu);
+    const float w = upstream ? __ldg(upstream + ((size_t)view * G.nv + iv) * G.nu + iu) : 1.f;   // null: unit weights
     const float D = G.step;
     const float sx = gx * G.sgx, sy = gy * G.sgy, sz = gz * G.sgz;            // sum g  (per mm)
     const float mx = hx * G.sgx * D, my = hy * G.sgy * D, mz = hz * G.sgz * D; // D sum kappa g
@@ -312,7 +312,7 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_grad_kernel(FwdGeom G, const 
 //   dL/dt = -R S_A,  dL/dgamma_k = -w_k . S_B          (PAPER.md :79: grad_theta = grad_theta M . grad_M)
 __global__ void __launch_bounds__(256) fwd_contract_kernel(int nblk, const float* __restrict__ partials,
                                                            const FwdContract* __restrict__ con,
-                                                           float* __restrict__ grad) {
+                                                           float* __restrict__ grad, int gstride = 6, int goff = 0) {
   const int view = blockIdx.x;
   __shared__ double sh[8][6];
   double acc[6] = {0, 0, 0, 0, 0, 0};
@@ -337,8 +337,9 @@ __global__ void __launch_bounds__(256) fwd_contract_kernel(int nblk, const float
     }
     const FwdContract& C = con[view];
     for (int a = 0; a < 3; ++a) {
-      grad[view * 6 + a] = (float)(-(C.R[a * 3 + 0] * S[0] + C.R[a * 3 + 1] * S[1] + C.R[a * 3 + 2] * S[2]));
-      grad[view * 6 + 3 + a] = (float)(-(C.w[a * 3 + 0] * S[3] + C.w[a * 3 + 1] * S[4] + C.w[a * 3 + 2] * S[5]));
+      grad[view * gstride + goff + a] = (float)(-(C.R[a * 3 + 0] * S[0] + C.R[a * 3 + 1] * S[1] + C.R[a * 3 + 2] * S[2]));
+      grad[view * gstride + goff + 3 + a] =
+          (float)(-(C.w[a * 3 + 0] * S[3] + C.w[a * 3 + 1] * S[4] + C.w[a * 3 + 2] * S[5]));
     }
   }
 }

@@ -359,3 +359,73 @@ def test_grad_interp_mode_backproject(dfp, bw, fl):
         # of a pixel boundary takes the neighbouring cell's slope, an O(1) change of that term which does not average
         # out like rounding noise; on ramp-filtered (sign-cancelling) data the smallest components show 1.0-1.3e-3
         assert e.max() <= 3 * TOL_GRAD and np.quantile(e, 0.95) <= TOL_GRAD, (bw, fl, extra, e)
+
+
+# ------------------------------------------------------------------ dfp_forward_fused_moments
+def _fused_case(dfp, w, flags=0):
+    dev = torch.device("cuda:0")
+    g = w.geom.replace(flags=flags)
+    a, p = f32(w.angles.numpy()), f32(w.poses.numpy()).reshape(-1, 6)
+    vol = w.volume(dev)
+    target = w.closed_form(w.data_poses, dev).to(torch.float32).contiguous()      # b: projections at the data poses
+    proj, mom = dfp.forward_fused_moments(g, a, p, vol, target)
+    path = dfp.last_path()
+    vol_c, tgt_c = vol.cpu().numpy(), target.cpu().numpy()
+    o_proj = oracle.forward(g, a, p, vol_c)
+    ones = np.ones_like(tgt_c)
+    o_m = np.stack([oracle.forward_pose_grad(g, a, p, vol_c, ones),
+                    oracle.forward_pose_grad(g, a, p, vol_c, o_proj.astype(np.float32)),
+                    oracle.forward_pose_grad(g, a, p, vol_c, tgt_c)], axis=1)      # [V,3,6]
+    return proj.cpu().numpy(), mom.cpu().numpy(), o_proj, o_m, path, (g, a, p, vol, target)
+
+
+@pytest.mark.parametrize("index,scale,views,tma", [(2, 0.25, 3, True), (4, 0.125, 4, True), (1, 1.0, None, True),
+                                                   (2, 0.25, 2, False)])
+def test_fused_moments_match_oracle(dfp, index, scale, views, tma):
+    """One traversal = projection + the pose-gradient 6-vectors for upstream 1, l and b; expected values from the
+    pinned oracle functions (forward, and forward_pose_grad with those three upstreams).  tma=False: the gather
+    fallback, which composes the call from the projection kernel and three gradient passes."""
+    w = W.make_config(index, scale=scale, n_views=views)
+    proj, mom, o_proj, o_m, path, _ = _fused_case(dfp, w, 0 if tma else dfp.FLAG_NO_TMA)
+    assert path == (dfp.PATH_TMA if tma else dfp.PATH_GATHER)
+    assert np.all(np.isfinite(proj)) and np.all(np.isfinite(mom))
+    assert rel_l2(proj, o_proj) <= TOL_VAL
+    for k in range(3):
+        e = grad_err_u9(mom[:, k], o_m[:, k])
+        assert e.max() <= TOL_GRAD, (index, k, e)
+
+
+def test_fused_moments_give_the_ssd_and_ncc_gradients(dfp):
+    """dL/dtheta from the moments == dfp_forward_pose_grad with the loss's upstream gradient (SSD: 2(l - b); NCC: the
+    affine form of workloads.losses.ncc_grad), for both kernel paths."""
+    w = W.make_config(2, scale=0.25, n_views=3)
+    for flags in (0, dfp.FLAG_NO_TMA):
+        proj, mom, _, _, _, (g, a, p, vol, target) = _fused_case(dfp, w, flags)
+        l = torch.as_tensor(proj, device=vol.device)
+        # SSD: dL/dl = 2 (l - b)
+        ref = dfp.forward_pose_grad(g, a, p, vol, (2.0 * (l - target)).contiguous()).cpu().numpy()
+        got = 2.0 * (mom[:, 1] - mom[:, 2])
+        assert grad_err_u9(got, ref).max() <= 1e-4
+        # NCC(l, b) per view: dNCC/dl = (b - mean b)/(sa sb) - NCC (l - mean l)/sa^2, sa = |l - mean l|, sb likewise
+        got_n, up_n = [], []
+        for v in range(l.shape[0]):
+            lv, bv = l[v].double(), target[v].double()
+            la, ba = lv - lv.mean(), bv - bv.mean()
+            sa, sb = la.norm(), ba.norm()
+            ncc = (la * ba).sum() / (sa * sb)
+            up_n.append((ba / (sa * sb) - ncc * la / sa ** 2).float())
+            gam, bet = 1.0 / (sa * sb), -ncc / sa ** 2
+            alp = -gam * bv.mean() - bet * lv.mean()
+            got_n.append(float(alp) * mom[v, 0] + float(bet) * mom[v, 1] + float(gam) * mom[v, 2])
+        ref_n = dfp.forward_pose_grad(g, a, p, vol, torch.stack(up_n).contiguous()).cpu().numpy()
+        assert grad_err_u9(np.stack(got_n), ref_n).max() <= 2e-3      # alpha, beta, gamma cancel heavily for NCC
+
+
+def test_fused_moments_reject_interp_mode_and_bad_arguments(dfp):
+    w = W.make_config(1)
+    dev = torch.device("cuda:0")
+    a, p = f32(w.angles.numpy()), f32(w.poses.numpy()).reshape(-1, 6)
+    vol = w.volume(dev)
+    tgt = torch.zeros((1,) + w.geom.det_shape, device=dev)
+    with pytest.raises(dfp.DfpError):
+        dfp.forward_fused_moments(w.geom.replace(flags=dfp.FLAG_GRAD_INTERP), a, p, vol, tgt)
