@@ -270,6 +270,9 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_grad_tma_kernel(BpGeom G, in
   const float* wcol = upstream + ((size_t)T.z0 * G.ny + (live ? iy : 0)) * G.nx + (live ? ix : 0);
   const size_t wstride = (size_t)G.ny * G.nx;
   const size_t tile = ((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+  float wreg[TZ];            // the thread's column of the upstream gradient: the same for every view
+#pragma unroll
+  for (int m = 0; m < TZ; ++m) wreg[m] = (live && m < T.tz) ? __ldg(wcol + (size_t)m * wstride) : 0.f;
   bool bad = false;
   const int n_groups = (n_views + kBpGradGroup - 1) / kBpGradGroup;
   for (int grp = 0; grp < n_groups; ++grp) {
@@ -290,47 +293,66 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_grad_tma_kernel(BpGeom G, in
         const float wb = fmaf(hdr[8], xf, fmaf(hdr[9], yf, fmaf(a22, zf, hdr[11])));
         const float j00 = hdr[12], j01 = hdr[13], j02 = hdr[14], j10 = hdr[15], j11 = hdr[16], j12 = hdr[17],
                     j20 = hdr[18], j21 = hdr[19], j22 = hdr[20];
-        float mf = 0.f;
-        for (int m = 0; m < T.tz; ++m) {
-          const PatchPix p = patch_locate(fmaf(mf, a02, ub), fmaf(mf, a12, vb), fmaf(mf, a22, wb), c0, BU, chk_lo, chk_hi);
-          // rows v, v+1: columns u-1 .. u+2; rows v-1, v+2: columns u, u+1
-          float dlu, dlv, l00, l01, l10, l11;
-          if (MODE == 1) {
-            const unsigned a0 = p.addr, a1 = a0 + BU;
-            l00 = lds_f32<0>(a0); l01 = lds_f32<4>(a0); l10 = lds_f32<0>(a1); l11 = lds_f32<4>(a1);
-            dlu = lerp(p.b, l01 - l00, l11 - l10);
-            dlv = lerp(p.a, l10 - l00, l11 - l01);
-          } else {
-            const unsigned a0 = p.addr, a1 = a0 + BU, am = a0 - BU, a2 = a1 + BU;
-            const float l0m = lds_f32<-4>(a0), l02 = lds_f32<8>(a0);
-            const float l1m = lds_f32<-4>(a1), l12 = lds_f32<8>(a1);
-            l00 = lds_f32<0>(a0); l01 = lds_f32<4>(a0); l10 = lds_f32<0>(a1); l11 = lds_f32<4>(a1);
-            const float lm0 = lds_f32<0>(am), lm1 = lds_f32<4>(am), l20 = lds_f32<0>(a2), l21 = lds_f32<4>(a2);
-            const float du0 = lerp(p.a, l01 - l0m, l02 - l00);
-            const float du1 = lerp(p.a, l11 - l1m, l12 - l10);
-            dlu = lerp(p.b, du0, du1);
-            const float dv0 = lerp(p.b, l10 - lm0, l20 - l00);
-            const float dv1 = lerp(p.b, l11 - lm1, l21 - l01);
-            dlv = lerp(p.a, dv0, dv1);
+        // packed fp32x2 arithmetic on (u, v) / row / column pairs (FFMA2, FADD2, FMUL2: the scalar code's roundings)
+        const float2 ab2 = make_float2(a02, a12), uvb = make_float2(ub, vb);
+        const float2 j0 = make_float2(j00, j01), j1 = make_float2(j10, j11), j2 = make_float2(j20, j21);
+        float2 s01 = make_float2(0.f, 0.f), s34 = make_float2(0.f, 0.f);
+        float s2 = 0.f, s5 = 0.f;
+#pragma unroll
+        for (int m = 0; m < TZ; ++m) {
+          if (m < T.tz) {
+            const float mf = (float)m;
+            const float rw = fast_rcp(fmaf(mf, a22, wb));
+            const float2 uvq = __fmul2_rn(__ffma2_rn(make_float2(mf, mf), ab2, uvb), make_float2(rw, rw));
+            const float2 t2 = __fadd2_rn(uvq, make_float2(kMagic, kMagic));
+            const float2 fr = __fadd2_rn(sub2(uvq, __fadd2_rn(t2, make_float2(-kMagic, -kMagic))), make_float2(0.5f, 0.5f));
+            const unsigned a0 = 4u * (unsigned)__float_as_int(t2.x) + BU * (unsigned)__float_as_int(t2.y) + c0;
+#ifdef DFP_CHECK_BOUNDS
+            if (a0 < chk_lo || a0 > chk_hi) s2 = __int_as_float(0x7fc00000);
+#endif
+            const float pa = fr.x, pb = fr.y;
+            float dlu, dlv, l00, l01, l10, l11;
+            if (MODE == 1) {
+              const unsigned a1 = a0 + BU;
+              l00 = lds_f32<0>(a0); l01 = lds_f32<4>(a0); l10 = lds_f32<0>(a1); l11 = lds_f32<4>(a1);
+              dlu = lerp(pb, l01 - l00, l11 - l10);
+              dlv = lerp(pa, l10 - l00, l11 - l01);
+            } else {
+              // rows v, v+1: columns u-1 .. u+2; rows v-1, v+2: columns u, u+1
+              const unsigned a1 = a0 + BU, am = a0 - BU, a2 = a1 + BU;
+              const float l0m = lds_f32<-4>(a0), l02 = lds_f32<8>(a0);
+              const float l1m = lds_f32<-4>(a1), l12 = lds_f32<8>(a1);
+              l00 = lds_f32<0>(a0); l01 = lds_f32<4>(a0); l10 = lds_f32<0>(a1); l11 = lds_f32<4>(a1);
+              const float lm0 = lds_f32<0>(am), lm1 = lds_f32<4>(am), l20 = lds_f32<0>(a2), l21 = lds_f32<4>(a2);
+              // (du0, du1): rows v, v+1;  (dv0, dv1): columns u, u+1
+              const float2 du = lerp2(make_float2(pa, pa), sub2(make_float2(l01, l11), make_float2(l0m, l1m)),
+                                      sub2(make_float2(l02, l12), make_float2(l00, l10)));
+              dlu = lerp(pb, du.x, du.y);
+              const float2 dv = lerp2(make_float2(pb, pb), sub2(make_float2(l10, l11), make_float2(lm0, lm1)),
+                                      sub2(make_float2(l20, l21), make_float2(l00, l01)));
+              dlv = lerp(pa, dv.x, dv.y);
+            }
+            const float W = WEIGHT ? G.sad2 * rw * rw : 1.f;
+            const float cc = fmaf(dlu, uvq.x, dlv * uvq.y);
+            const float2 dlu2 = make_float2(dlu, dlu), dlv2 = make_float2(dlv, dlv);
+            float2 q2 = __ffma2_rn(dlu2, j0, __ffma2_rn(dlv2, j1, __fmul2_rn(make_float2(-cc, -cc), j2)));
+            float qz = fmaf(dlu, j02, fmaf(dlv, j12, -cc * j22));
+            const float sc = (MODE == 1 ? 1.0f : 0.5f) * W * rw * wreg[m];
+            if (DW) {
+              const float b0 = lerp(pa, l00, l01), b1 = lerp(pa, l10, l11);
+              const float bv = lerp(pb, b0, b1);
+              const float k = (MODE == 1 ? -2.f : -4.f) * bv;
+              q2 = __ffma2_rn(make_float2(k, k), j2, q2);
+              qz = fmaf(k, j22, qz);
+            }
+            const float scm = sc * mf;
+            s01 = __ffma2_rn(make_float2(sc, sc), q2, s01);
+            s34 = __ffma2_rn(make_float2(scm, scm), q2, s34);
+            s2 = fmaf(sc, qz, s2);
+            s5 = fmaf(scm, qz, s5);
           }
-          const float wj = __ldg(wcol + (size_t)m * wstride);
-          const float W = WEIGHT ? G.sad2 * p.rw * p.rw : 1.f;
-          const float cc = fmaf(dlu, p.uq, dlv * p.vq);
-          float qx = fmaf(dlu, j00, fmaf(dlv, j10, -cc * j20));
-          float qy = fmaf(dlu, j01, fmaf(dlv, j11, -cc * j21));
-          float qz = fmaf(dlu, j02, fmaf(dlv, j12, -cc * j22));
-          const float sc = (MODE == 1 ? 1.0f : 0.5f) * W * p.rw * wj;
-          if (DW) {
-            const float b0 = lerp(p.a, l00, l01), b1 = lerp(p.a, l10, l11);
-            const float bv = lerp(p.b, b0, b1);
-            const float k = (MODE == 1 ? -2.f : -4.f) * bv;
-            qx = fmaf(k, j20, qx); qy = fmaf(k, j21, qy); qz = fmaf(k, j22, qz);
-          }
-          sm[0] = fmaf(sc, qx, sm[0]); sm[1] = fmaf(sc, qy, sm[1]); sm[2] = fmaf(sc, qz, sm[2]);
-          const float scm = sc * mf;
-          sm[3] = fmaf(scm, qx, sm[3]); sm[4] = fmaf(scm, qy, sm[4]); sm[5] = fmaf(scm, qz, sm[5]);
-          mf += 1.0f;
         }
+        sm[0] = s01.x; sm[1] = s01.y; sm[2] = s2; sm[3] = s34.x; sm[4] = s34.y; sm[5] = s5;
         const float mx = sm[3] * G.vz, my = sm[4] * G.vz;
         const float cx = ry * sm[2] - rz * sm[1] - my;
         const float cy = rz * sm[0] - rx * sm[2] + mx;
