@@ -113,29 +113,10 @@ __device__ __forceinline__ void bp_issue_view(const BpGeom& G, const BpTile& T, 
   }
 }
 
-// Pixel cell and fractions of one (voxel, view) pair inside the staged patch (no clamps: the patch holds the
-// tile's whole footprint plus the stencil halo, and out-of-detector pixels were zero-filled).
-// `addr` is the SHARED-space byte address of pixel (floor u, floor v): 4*Tu + 4*pitch*Tv + c0b, two IMADs on the
-// magic-rounded float bits (c0b folds the stage base, the patch origin and the magic bias).
-struct PatchPix {
-  float a, b, rw, uq, vq;
-  unsigned addr;
-};
-__device__ __forceinline__ PatchPix patch_locate(float up, float vp, float wp, unsigned c0b, unsigned pitch4,
-                                                 unsigned chk_lo = 0u, unsigned chk_hi = 0xffffffffu) {
-  PatchPix o;
-  o.rw = fast_rcp(wp);
-  o.uq = up * o.rw;
-  o.vq = vp * o.rw;
-  const float tu = o.uq + kMagic, tv = o.vq + kMagic;
-  o.a = (o.uq - (tu - kMagic)) + 0.5f;
-  o.b = (o.vq - (tv - kMagic)) + 0.5f;
-  o.addr = 4u * (unsigned)__float_as_int(tu) + pitch4 * (unsigned)__float_as_int(tv) + c0b;
-#ifdef DFP_CHECK_BOUNDS   // debug build: the cell and its halo must lie inside this stage's patch area (else NaN out)
-  if (o.addr < chk_lo || o.addr > chk_hi) o.a = __int_as_float(0x7fc00000);
-#endif
-  return o;
-}
+// Pixel cell of one (voxel, view) pair inside the staged patch (no clamps: the patch holds the tile's whole
+// footprint plus the stencil halo, and out-of-detector pixels were zero-filled): the SHARED-space byte address of
+// pixel (floor u, floor v) is 4*Tu + pitch_bytes*Tv + c0b, two IMADs on the magic-rounded float bits (c0b folds the
+// stage base, the patch origin and the magic bias).
 template <int OFF>
 __device__ __forceinline__ float lds_f32(unsigned addr) {
   float v;
@@ -196,15 +177,26 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_tma_kernel(BpGeom G, int n_v
       const float ub = fmaf(hdr[0], xf, fmaf(hdr[1], yf, fmaf(a02, zf, hdr[3])));
       const float vb = fmaf(hdr[4], xf, fmaf(hdr[5], yf, fmaf(a12, zf, hdr[7])));
       const float wb = fmaf(hdr[8], xf, fmaf(hdr[9], yf, fmaf(a22, zf, hdr[11])));
+      const float2 ab2 = make_float2(a02, a12), uvb = make_float2(ub, vb);
 #pragma unroll
       for (int m = 0; m < TZ; ++m) {
         if (m < T.tz) {
+          // (u, v) as one fp32x2 lane pair: advance along z, perspective divide, floor and fractions
           const float mf = (float)m;
-          const PatchPix p = patch_locate(fmaf(mf, a02, ub), fmaf(mf, a12, vb), fmaf(mf, a22, wb), c0, BU, chk_lo, chk_hi);
-          const unsigned a1 = p.addr + BU;
-          const float val = lerp(p.b, lerp(p.a, lds_f32<0>(p.addr), lds_f32<4>(p.addr)),
-                                 lerp(p.a, lds_f32<0>(a1), lds_f32<4>(a1)));
-          const float wgt = WEIGHT ? G.sad2 * p.rw * p.rw : 1.f;
+          const float rw = fast_rcp(fmaf(mf, a22, wb));
+          const float2 uvq = __fmul2_rn(__ffma2_rn(make_float2(mf, mf), ab2, uvb), make_float2(rw, rw));
+          const float2 t2 = __fadd2_rn(uvq, make_float2(kMagic, kMagic));
+          const float2 fr = __fadd2_rn(sub2(uvq, __fadd2_rn(t2, make_float2(-kMagic, -kMagic))), make_float2(0.5f, 0.5f));
+          const unsigned a0 = 4u * (unsigned)__float_as_int(t2.x) + BU * (unsigned)__float_as_int(t2.y) + c0;
+          const unsigned a1 = a0 + BU;
+          // the two rows as a pair: lerp along u on both, then along v
+          const float2 r2 = lerp2(make_float2(fr.x, fr.x), make_float2(lds_f32<0>(a0), lds_f32<0>(a1)),
+                                  make_float2(lds_f32<4>(a0), lds_f32<4>(a1)));
+          float val = lerp(fr.y, r2.x, r2.y);
+#ifdef DFP_CHECK_BOUNDS
+          if (a0 < chk_lo || a0 > chk_hi) val = __int_as_float(0x7fc00000);
+#endif
+          const float wgt = WEIGHT ? G.sad2 * rw * rw : 1.f;
           acc[m] = fmaf(wgt, val, acc[m]);
         }
       }
