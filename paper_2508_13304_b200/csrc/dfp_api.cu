@@ -201,6 +201,43 @@ int bp_view_patch(const BpGeom& G, const BpView& Vw, int tz, int halo) {
   return -1;
 }
 
+// Kernels that use more than 48 KiB of dynamic shared memory need the opt-in attribute, per device: set once per
+// (thread's current) device and remembered.
+cudaError_t ensure_smem_attributes() {
+  static bool done[64] = {false};
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev >= 0 && dev < 64 && done[dev]) return cudaSuccess;
+#define DFP_ATTR(k, bytes)                                                                  \
+  if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes)) != cudaSuccess) return e
+  DFP_ATTR((fwd_tma_kernel<0, 0>), tma_smem_bytes<0>());
+  DFP_ATTR((fwd_tma_kernel<0, 1>), tma_smem_bytes<1>());
+  DFP_ATTR((fwd_tma_kernel<0, 2>), tma_smem_bytes<2>());
+  DFP_ATTR((fwd_tma_kernel<1, 2>), tma_smem_bytes<2>());
+  DFP_ATTR((fwd_tma_kernel<1, 3>), tma_smem_bytes<3>());
+  DFP_ATTR((fwd_tma_kernel<2, 2>), tma_smem_bytes<2>());
+  DFP_ATTR((fwd_tma_kernel<2, 3>), tma_smem_bytes<3>());
+  DFP_ATTR((fwd_tma_kernel<3, 2>), tma_smem_bytes<2>());
+  DFP_ATTR((fwd_tma_kernel<3, 3>), tma_smem_bytes<3>());
+  DFP_ATTR((bp_tma_kernel<0, 16>), kBpSmemBudget);
+  DFP_ATTR((bp_tma_kernel<1, 16>), kBpSmemBudget);
+  DFP_ATTR((bp_tma_kernel<0, 8>), kBpSmemBudget);
+  DFP_ATTR((bp_tma_kernel<1, 8>), kBpSmemBudget);
+#define DFP_ATTR_G(W, D)                                      \
+  DFP_ATTR((bp_grad_tma_kernel<W, D, 16, 0>), kBpSmemBudget); \
+  DFP_ATTR((bp_grad_tma_kernel<W, D, 8, 0>), kBpSmemBudget);  \
+  DFP_ATTR((bp_grad_tma_kernel<W, D, 16, 1>), kBpSmemBudget); \
+  DFP_ATTR((bp_grad_tma_kernel<W, D, 8, 1>), kBpSmemBudget)
+  DFP_ATTR_G(0, 0);
+  DFP_ATTR_G(1, 0);
+  DFP_ATTR_G(1, 1);
+#undef DFP_ATTR_G
+#undef DFP_ATTR
+  if (dev >= 0 && dev < 64) done[dev] = true;
+  return cudaSuccess;
+}
+
 // ---- workspace carving ---------------------------------------------------------------------------
 struct FwdWs {
   size_t off_views, off_con, off_pvol, off_part, total;
@@ -321,21 +358,7 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
   const bool tma = shape >= 0 && make_volume_map(*g, d_vol, kBoxes[shape][0], kBoxes[shape][1], kBoxes[shape][2], &vol_map);
   g_path = tma ? DFP_PATH_TMA : DFP_PATH_GATHER;
   if (tma) {
-    static const cudaError_t attr[4] = {
-        cudaFuncSetAttribute(fwd_tma_kernel<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<0>()),
-        cudaFuncSetAttribute(fwd_tma_kernel<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<1>()),
-        cudaFuncSetAttribute(fwd_tma_kernel<0, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<2>()),
-        cudaFuncSetAttribute(fwd_tma_kernel<1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<2>())};
-    static const cudaError_t attr3[3] = {
-        cudaFuncSetAttribute(fwd_tma_kernel<1, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<3>()),
-        cudaFuncSetAttribute(fwd_tma_kernel<2, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<3>()),
-        cudaFuncSetAttribute(fwd_tma_kernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<2>())};
-    for (cudaError_t e : attr3) DFP_CUDA(e, "cudaFuncSetAttribute");
-    static const cudaError_t attr4[2] = {
-        cudaFuncSetAttribute(fwd_tma_kernel<3, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<3>()),
-        cudaFuncSetAttribute(fwd_tma_kernel<3, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, tma_smem_bytes<2>())};
-    for (cudaError_t e : attr4) DFP_CUDA(e, "cudaFuncSetAttribute");
-    for (cudaError_t e : attr) DFP_CUDA(e, "cudaFuncSetAttribute");
+    DFP_CUDA(ensure_smem_attributes(), "cudaFuncSetAttribute");
     time_begin(s);
     const dim3 ggrid(w.gx, w.gy8, V);
     if (fused && shape == 3)
@@ -439,15 +462,7 @@ int run_backproject(const dfp_geometry* g, int V, const float* angles, const flo
   if (kmax >= 0 && make_proj_maps(*g, V, d_proj, kmax, &maps)) {
     const int stage_words = bp_stage_words(kmax), n_stages = bp_num_stages(kmax);
     const int smem = stage_words * 4 * n_stages;
-#define DFP_BP_ATTR(k) cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, kBpSmemBudget)
-#define DFP_BP_ATTR_G(W, D) DFP_BP_ATTR((bp_grad_tma_kernel<W, D, 16, 0>)), DFP_BP_ATTR((bp_grad_tma_kernel<W, D, 8, 0>)), \
-                            DFP_BP_ATTR((bp_grad_tma_kernel<W, D, 16, 1>)), DFP_BP_ATTR((bp_grad_tma_kernel<W, D, 8, 1>))
-    static const cudaError_t attr[16] = {
-        DFP_BP_ATTR((bp_tma_kernel<0, 16>)), DFP_BP_ATTR((bp_tma_kernel<1, 16>)), DFP_BP_ATTR((bp_tma_kernel<0, 8>)),
-        DFP_BP_ATTR((bp_tma_kernel<1, 8>)), DFP_BP_ATTR_G(0, 0), DFP_BP_ATTR_G(1, 0), DFP_BP_ATTR_G(1, 1)};
-#undef DFP_BP_ATTR_G
-#undef DFP_BP_ATTR
-    for (cudaError_t e : attr) DFP_CUDA(e, "cudaFuncSetAttribute");
+    DFP_CUDA(ensure_smem_attributes(), "cudaFuncSetAttribute");
     const dim3 tgrid(w.tx, w.ty, (g->nz + TZ - 1) / TZ);
     g_path = DFP_PATH_TMA;
 #define DFP_BP_ARGS <<<tgrid, kBpTmaThreads, smem, s>>>(G, V, dv, maps, kmax, stage_words, n_stages
