@@ -148,8 +148,9 @@ int dfp_last_launch_count(void);
 
 /* Kernel path the last successful device-pointer call on this thread took: DFP_PATH_GATHER (global-memory
  * gathers from a packed copy of the input) or DFP_PATH_TMA (input staged tile by tile in shared memory by TMA;
- * forward calls only, taken when nx % 4 == 0 and every view's pixel tiles fit the staging box).  The two paths
- * give bit-identical results. */
+ * taken when nx % 4 == 0 (forward calls) / nu % 4 == 0 (back-projection calls) and every view's tiles fit the staging boxes).  The two paths
+ * do the same arithmetic per sample / voxel and agree to fp32 summation order.  Both the
+ * forward and the back-projection calls have the two paths. */
 enum { DFP_PATH_GATHER = 0, DFP_PATH_TMA = 1 };
 int dfp_last_path(void);
 

@@ -335,8 +335,8 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
   DFP_CUDA(cudaMemcpyAsync(dv, hv.data(), sizeof(FwdView) * V, cudaMemcpyHostToDevice, s), "view upload");
   if (grad) DFP_CUDA(cudaMemcpyAsync(dc, hc.data(), sizeof(FwdContract) * V, cudaMemcpyHostToDevice, s), "view upload");
   const dim3 grid(w.gx, w.gy, V);
-  // TMA-staged path when the volume admits a tensor map and every view's tiles fit the staging box
-  // the smallest staging box (dfp_fwd_tma.cuh) that holds every view's tiles; the gradient uses shape 2 only
+  // TMA-staged path when the volume admits a tensor map and every view's tiles fit a staging box: the smallest
+  // box (dfp_fwd_tma.cuh) that holds every view's tiles
   CUtensorMap vol_map;
   static const int kBoxes[kNumShapes][3] = {{BoxShape<0>::X, BoxShape<0>::Y, BoxShape<0>::Z},
                                             {BoxShape<1>::X, BoxShape<1>::Y, BoxShape<1>::Z},
