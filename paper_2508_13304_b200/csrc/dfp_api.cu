@@ -543,6 +543,17 @@ int run_host(int op, const dfp_geometry* g, int V, const float* angles, const fl
   const bool grad = op == DFP_OP_FORWARD_POSE_GRAD || op == DFP_OP_BACKPROJECT_POSE_GRAD;
   if (!h_in || !h_out || (grad && !h_up)) return DFP_ERR_NULL;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
+  {  // keep the stream-ordered pool's memory across calls (the default trims it at every synchronisation)
+    static bool pool_set[64] = {false};
+    int dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < 64 && !pool_set[dev]) {
+      cudaMemPool_t pool;
+      unsigned long long keep = ~0ull;
+      if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess)
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+      pool_set[dev] = true;
+    }
+  }
   const size_t nvol = (size_t)g->nx * g->ny * g->nz * sizeof(float);
   const size_t nproj = (size_t)V * g->nu * g->nv * sizeof(float);
   const size_t ngrad = (size_t)V * 6 * sizeof(float);
