@@ -119,7 +119,11 @@ size_t dfp_workspace_bytes(const dfp_geometry* geometry, int n_views, int op);
 
 /* Same four operations with HOST buffers (h_*: host memory, pinned or pageable).  Each allocates device
  * scratch with cudaMallocAsync on `stream`, copies inputs in, runs the device call above, copies the result
- * out, frees, and synchronises `stream` before returning. */
+ * out, frees, and synchronises `stream` before returning.  With 8 or more views every call but
+ * dfp_backproject_host moves the per-view arrays in 4 chunks on an internal second stream, overlapped with the
+ * kernels of the neighbouring chunk (results do not depend on the chunking: views are independent there).  The
+ * first host call on a device raises the release threshold of its default stream-ordered memory pool so that
+ * later calls reuse the scratch memory. */
 int dfp_forward_host(const dfp_geometry* geometry, int n_views, const float* angles, const float* poses,
                      const float* h_vol, float* h_proj, void* stream);
 int dfp_forward_pose_grad_host(const dfp_geometry* geometry, int n_views, const float* angles, const float* poses,

@@ -567,16 +567,71 @@ int run_host(int op, const dfp_geometry* g, int V, const float* angles, const fl
   DFP_CUDA(d_up.alloc(n_up), "cudaMallocAsync");
   DFP_CUDA(d_out.alloc(n_out), "cudaMallocAsync");
   DFP_CUDA(d_ws.alloc(n_ws), "cudaMallocAsync");
-  DFP_CUDA(cudaMemcpyAsync(d_in.p, h_in, n_in, cudaMemcpyHostToDevice, s), "H2D");
-  if (grad) DFP_CUDA(cudaMemcpyAsync(d_up.p, h_up, n_up, cudaMemcpyHostToDevice, s), "H2D");
-  if (fwd)
-    st = run_forward(g, V, angles, poses, (const float*)d_in.p, (const float*)d_up.p, (float*)d_out.p, d_ws.p, n_ws, s,
-                     grad ? DFP_OP_FORWARD_POSE_GRAD : DFP_OP_FORWARD);
-  else
-    st = run_backproject(g, V, angles, poses, (const float*)d_in.p, (const float*)d_up.p, (float*)d_out.p, d_ws.p,
-                         n_ws, s, grad);
-  if (st) return st;
-  DFP_CUDA(cudaMemcpyAsync(h_out, d_out.p, n_out, cudaMemcpyDeviceToHost, s), "D2H");
+  // a9, view chunking: every call but dfp_backproject is independent per view, so the per-view arrays move in
+  // chunks on a second stream while the kernels of the neighbouring chunk run (the input shared by all views - the
+  // volume, or the upstream volume of the back-projection gradient - goes first, on the caller's stream).
+  const int n_chunks = (op == DFP_OP_BACKPROJECT || V < 8) ? 1 : 4;
+  if (n_chunks == 1) {
+    DFP_CUDA(cudaMemcpyAsync(d_in.p, h_in, n_in, cudaMemcpyHostToDevice, s), "H2D");
+    if (grad) DFP_CUDA(cudaMemcpyAsync(d_up.p, h_up, n_up, cudaMemcpyHostToDevice, s), "H2D");
+    if (fwd)
+      st = run_forward(g, V, angles, poses, (const float*)d_in.p, (const float*)d_up.p, (float*)d_out.p, d_ws.p, n_ws,
+                       s, grad ? DFP_OP_FORWARD_POSE_GRAD : DFP_OP_FORWARD);
+    else
+      st = run_backproject(g, V, angles, poses, (const float*)d_in.p, (const float*)d_up.p, (float*)d_out.p, d_ws.p,
+                           n_ws, s, grad);
+    if (st) return st;
+    DFP_CUDA(cudaMemcpyAsync(h_out, d_out.p, n_out, cudaMemcpyDeviceToHost, s), "D2H");
+    DFP_CUDA(cudaStreamSynchronize(s), "stream synchronize");
+    return DFP_OK;
+  }
+  struct Side {                      // the copy stream and its events, released on every exit path
+    cudaStream_t s2 = nullptr;
+    cudaEvent_t ev[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    ~Side() {
+      for (cudaEvent_t e : ev) if (e) cudaEventDestroy(e);
+      if (s2) cudaStreamDestroy(s2);
+    }
+  } side;
+  DFP_CUDA(cudaStreamCreateWithFlags(&side.s2, cudaStreamNonBlocking), "cudaStreamCreate");
+  for (cudaEvent_t& e : side.ev) DFP_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming), "cudaEventCreate");
+  const size_t per_view = (size_t)g->nu * g->nv;            // floats of one view's projection / upstream image
+  // shared input on the caller's stream; the copy stream starts after the buffers exist (allocation is stream-ordered)
+  const float* h_shared = fwd ? h_in : h_up;                 // volume | upstream volume
+  float* d_shared = static_cast<float*>(fwd ? d_in.p : d_up.p);
+  const float* h_views = fwd ? h_up : h_in;                  // upstream images | projections (null for dfp_forward)
+  float* d_views = static_cast<float*>(fwd ? d_up.p : d_in.p);
+  DFP_CUDA(cudaEventRecord(side.ev[0], s), "cudaEventRecord");
+  DFP_CUDA(cudaStreamWaitEvent(side.s2, side.ev[0], 0), "cudaStreamWaitEvent");
+  DFP_CUDA(cudaMemcpyAsync(d_shared, h_shared, nvol, cudaMemcpyHostToDevice, s), "H2D");
+  int launches = 0;
+  for (int c = 0; c < n_chunks; ++c) {
+    const int v0 = (int)((long long)V * c / n_chunks), v1 = (int)((long long)V * (c + 1) / n_chunks), nv_c = v1 - v0;
+    const size_t off = (size_t)v0 * per_view;
+    if (h_views) {                   // this chunk's per-view input on the copy stream, then the kernels wait for it
+      DFP_CUDA(cudaMemcpyAsync(d_views + off, h_views + off, (size_t)nv_c * per_view * 4, cudaMemcpyHostToDevice,
+                               side.s2), "H2D");
+      DFP_CUDA(cudaEventRecord(side.ev[c], side.s2), "cudaEventRecord");
+      DFP_CUDA(cudaStreamWaitEvent(s, side.ev[c], 0), "cudaStreamWaitEvent");
+    }
+    float* out_c = static_cast<float*>(d_out.p) + (grad ? (size_t)v0 * 6 : off);
+    if (fwd)
+      st = run_forward(g, nv_c, angles + v0, poses + 6 * v0, d_shared, grad ? d_views + off : nullptr, out_c, d_ws.p,
+                       n_ws, s, grad ? DFP_OP_FORWARD_POSE_GRAD : DFP_OP_FORWARD);
+    else
+      st = run_backproject(g, nv_c, angles + v0, poses + 6 * v0, d_views + off, d_shared, out_c, d_ws.p, n_ws, s, true);
+    if (st) return st;
+    launches += g_launches;
+    if (!grad) {                     // dfp_forward: this chunk's projections go home while the next chunk is computed
+      DFP_CUDA(cudaEventRecord(side.ev[4 + c], s), "cudaEventRecord");
+      DFP_CUDA(cudaStreamWaitEvent(side.s2, side.ev[4 + c], 0), "cudaStreamWaitEvent");
+      DFP_CUDA(cudaMemcpyAsync(h_out + off, out_c, (size_t)nv_c * per_view * 4, cudaMemcpyDeviceToHost, side.s2),
+               "D2H");
+    }
+  }
+  g_launches = launches;
+  if (grad) DFP_CUDA(cudaMemcpyAsync(h_out, d_out.p, n_out, cudaMemcpyDeviceToHost, s), "D2H");
+  DFP_CUDA(cudaStreamSynchronize(side.s2), "stream synchronize");
   DFP_CUDA(cudaStreamSynchronize(s), "stream synchronize");
   return DFP_OK;
 }

@@ -480,3 +480,25 @@ def test_random_geometries_both_paths_agree_and_never_nan(dfp):
             check_back((bp.cpu().numpy(), bgrad.cpu().numpy(), oracle.backproject(g, angles, poses, proj.cpu().numpy()),
                         oracle.backproject_pose_grad(g, angles, poses, proj.cpu().numpy(), bup.cpu().numpy())))
     assert 40 <= n_tma <= 150, n_tma      # a healthy mix of TMA and fallback calls (4 calls per case)
+
+
+def test_host_buffer_entry_points_chunked_views(dfp):
+    """>= 8 views: the host-buffer calls move per-view arrays in 4 chunks on a second stream, overlapped with the
+    kernels (a9, view chunking); 9 views give uneven chunks (2, 2, 2, 3).  Same results as the device-pointer calls
+    on the whole batch (per-view outputs do not depend on how the views are grouped)."""
+    w = W.make_config(2, scale=0.25, n_views=9)
+    g = w.geom
+    dev = torch.device("cuda:0")
+    a, p = f32(w.angles.numpy()), f32(w.poses.numpy()).reshape(-1, 6)
+    vol, up = w.volume(), w.fwd_upstream()
+    vd, ud = vol.to(dev), up.to(dev)
+    proj = dfp.forward(g, a, p, vd)
+    assert torch.equal(dfp.forward_host(g, a, p, vol.numpy()), proj.cpu())
+    assert torch.equal(dfp.forward_pose_grad_host(g, a, p, vol.numpy(), up.numpy()),
+                       dfp.forward_pose_grad(g, a, p, vd, ud).cpu())
+    pj = proj.cpu().numpy()
+    wv = np.random.default_rng(5).standard_normal(g.vol_shape).astype(np.float32)
+    assert torch.equal(dfp.backproject_host(g, a, p, pj), dfp.backproject(g, a, p, proj).cpu())
+    got = dfp.backproject_pose_grad_host(g, a, p, pj, wv).numpy()
+    ref = dfp.backproject_pose_grad(g, a, p, proj, torch.as_tensor(wv, device=dev)).cpu().numpy()
+    assert np.array_equal(got, ref)
