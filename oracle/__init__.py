@@ -194,3 +194,55 @@ def projection_matrix(g, angle):
     P = np.empty((3, 4))
     lib.ora_projection_matrix(ctypes.byref(gg), ctypes.c_double(float(angle)), _p(P))
     return P
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# O12: Siddon's exact radiological path - the paper's own ray-driven weights (PAPER.md :213, :395)
+def forward_siddon(g, angles, poses, vol):
+    """l_i = sum_j a^ij mu_j, a^ij = length of ray i inside voxel j.  vol [nz,ny,nx] -> proj [V,nv,nu] float64."""
+    lib = _load()
+    angles, poses, V = _views(angles, poses)
+    if hasattr(vol, "detach"):
+        vol = vol.detach().cpu().numpy()
+    gg = _geom(g)
+    proj = np.empty((V, gg.nv, gg.nu), dtype=np.float64)
+    if np.asarray(vol).dtype == np.float64:
+        vol = np.ascontiguousarray(vol)
+        fn = lib.ora_forward_siddon_f64
+    else:
+        vol = _f32(vol)
+        fn = lib.ora_forward_siddon_f32
+    assert vol.shape == (gg.nz, gg.ny, gg.nx)
+    fn(ctypes.byref(gg), V, _p(angles), _p(poses), _p(vol), _p(proj))
+    return proj
+
+
+def forward_siddon_T(g, angles, poses, y):
+    """Explicit transpose of `forward_siddon` (adjointness pin).  y [V,nv,nu] -> vol float64."""
+    lib = _load()
+    angles, poses, V = _views(angles, poses)
+    gg = _geom(g)
+    y = _f64(y, (V, gg.nv, gg.nu))
+    out = np.empty((gg.nz, gg.ny, gg.nx), dtype=np.float64)
+    lib.ora_forward_siddon_T(ctypes.byref(gg), V, _p(angles), _p(poses), _p(y), _p(out))
+    return out
+
+
+def forward_pose_grad_siddon(g, angles, poses, vol, upstream, route=ROUTE_SIX):
+    """Pose gradient with Siddon weights and per-voxel G_f^j (Eq.19-20, :189).  -> [V,6] float64."""
+    lib = _load()
+    angles, poses, V = _views(angles, poses)
+    gg = _geom(g)
+    if hasattr(vol, "detach"):
+        vol = vol.detach().cpu().numpy()
+    up = _f32(upstream).reshape(V, gg.nv, gg.nu)
+    grad = np.empty((V, 6), dtype=np.float64)
+    if np.asarray(vol).dtype == np.float64:
+        vol = np.ascontiguousarray(vol)
+        fn = lib.ora_forward_pose_grad_siddon_f64
+    else:
+        vol = _f32(vol)
+        fn = lib.ora_forward_pose_grad_siddon_f32
+    assert vol.shape == (gg.nz, gg.ny, gg.nx)
+    fn(ctypes.byref(gg), V, _p(angles), _p(poses), _p(vol), _p(up), _p(grad), int(route))
+    return grad

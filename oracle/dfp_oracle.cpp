@@ -10,7 +10,10 @@
 // Pins (tests/test_oracle_*.py, all `-m "not gpu"`): closed-form ellipsoid and Gaussian line
 // integrals, explicit-transpose adjointness, central finite differences in all six pose
 // parameters, the translation invariant dL/dt = -R A[grad mu], 6-accumulator vs the paper's
-// 12-element G route, stored-G literal algorithm, brute-force back-projection on tiny grids.
+// 12-element G route, stored-G literal algorithm, brute-force back-projection on tiny grids;
+// Siddon weights (O12, tests/test_oracle_siddon.py): chord of the grid box, brute-force clipping
+// of the ray against every voxel's own box, explicit transpose, closed forms, the paper's literal
+// stored-G algorithm, finite differences of closed-form projections.
 // No function here is "parity unpinned".
 //
 // Conventions:
@@ -544,6 +547,154 @@ void backproject_grad_impl(const ora_geom& g, int n_views, const double* angles,
 
 }  // namespace
 
+// ------------------------------------------------------------------------------------------------
+// O12: Siddon's exact radiological path [28] - the weights of the paper's own ray-driven
+// projector (PAPER.md :213, ref :395): a^ij = length of the intersection of ray i with voxel j, voxels being boxes
+// of constant value mu_j (Eq.18 :172-177, "projection path length" :177).
+// Following Siddon's formulation: the parameters at which the half-line s' + t e' (t >= 0, object frame, mm)
+// crosses the planes of the three families that bound the voxels are merged into ONE sorted list; two consecutive
+// parameters delimit a segment that lies in one voxel, identified by the segment's midpoint.
+struct Seg { double len; long ix, iy, iz; };
+inline void siddon_segments(const ora_geom& g, V3 so, V3 eo, std::vector<double>& ts, std::vector<Seg>& out) {
+  out.clear(); ts.clear();
+  const double n[3] = {(double)g.nx, (double)g.ny, (double)g.nz}, v[3] = {g.vx, g.vy, g.vz}, c[3] = {g.cx, g.cy, g.cz};
+  double lo[3], tmin = 0.0, tmax = 1e300;
+  for (int a = 0; a < 3; ++a) {
+    lo[a] = c[a] - 0.5 * n[a] * v[a];
+    const double hi = c[a] + 0.5 * n[a] * v[a], o = comp(so, a), d = comp(eo, a);
+    if (fabs(d) < 1e-300) { if (o <= lo[a] || o >= hi) return; continue; }
+    double t0 = (lo[a] - o) / d, t1 = (hi - o) / d;
+    if (t0 > t1) std::swap(t0, t1);
+    tmin = std::max(tmin, t0); tmax = std::min(tmax, t1);
+  }
+  if (!(tmax > tmin)) return;
+  ts.push_back(tmin); ts.push_back(tmax);
+  for (int a = 0; a < 3; ++a) {
+    const double o = comp(so, a), d = comp(eo, a);
+    if (fabs(d) < 1e-300) continue;
+    for (long i = 0; i <= (long)n[a]; ++i) {
+      const double t = (lo[a] + i * v[a] - o) / d;
+      if (t > tmin && t < tmax) ts.push_back(t);
+    }
+  }
+  std::sort(ts.begin(), ts.end());
+  for (size_t m = 0; m + 1 < ts.size(); ++m) {
+    const double len = ts[m + 1] - ts[m];
+    if (!(len > 0)) continue;
+    const V3 mid = so + (0.5 * (ts[m] + ts[m + 1])) * eo;
+    long idx[3];
+    for (int a = 0; a < 3; ++a) {
+      idx[a] = (long)floor((comp(mid, a) - lo[a]) / v[a]);
+      idx[a] = std::min(std::max(idx[a], 0L), (long)n[a] - 1);
+    }
+    out.push_back({len, idx[0], idx[1], idx[2]});
+  }
+}
+
+// l_i = sum_j a^ij mu_j.  (transpose = true: the explicit transpose, vol_out += a^ij y_i; adjointness pin only.)
+template <typename T>
+void forward_siddon_impl(const ora_geom& g, int n_views, const double* angles, const double* poses, const T* vol,
+                         double* proj, const double* y_in, double* vol_out) {
+  Vol<T> V{vol, g.nx, g.ny, g.nz};
+  const bool transpose = vol_out != nullptr;
+  if (transpose) for (size_t i = 0; i < (size_t)g.nx * g.ny * g.nz; ++i) vol_out[i] = 0.0;
+  for (int v = 0; v < n_views; ++v) {
+    View view(g, angles[v]);
+    Pose pose(poses + 6 * v);
+    const V3 so = mulT(pose.R, view.s - pose.t);
+#pragma omp parallel for schedule(dynamic, 4) if (!transpose)
+    for (int iv = 0; iv < g.nv; ++iv) {
+      std::vector<double> ts; std::vector<Seg> segs;
+      for (int iu = 0; iu < g.nu; ++iu) {
+        V3 d = view.pixel(g, iu, iv) - view.s;
+        V3 eo = mulT(pose.R, (1.0 / sqrt(dot(d, d))) * d);
+        siddon_segments(g, so, eo, ts, segs);
+        const size_t pix = ((size_t)v * g.nv + iv) * g.nu + iu;
+        if (!transpose) {
+          double sum = 0.0;
+          for (const Seg& sg : segs) sum += sg.len * V.at(sg.ix, sg.iy, sg.iz);
+          proj[pix] = sum;
+        } else {
+          for (const Seg& sg : segs) vol_out[((size_t)sg.iz * g.ny + sg.iy) * g.nx + sg.ix] += sg.len * y_in[pix];
+        }
+      }
+    }
+  }
+}
+
+// Pose gradient with Siddon weights, the paper's discretisation taken literally (Eq.19-20 :179-191, :189
+// "Compute matrix G_f^j for each voxel"): per voxel j of the grid, g_j = central differences of the zero-extended
+// voxel values (:183), lever arm at the voxel centre r'_j;
+//   A_i = sum_j a^ij g_j,  B_i = sum_j a^ij r'_j x g_j;  S_A = sum_i w_i A_i, S_B likewise;
+//   route 0: dL/dt = -R S_A, dL/dgamma_k = -w_k.S_B;  route 1: the 12-element G_f^j = [ (R r'_j) g_j^T | -R g_j ].
+template <typename T>
+void forward_grad_siddon_impl(const ora_geom& g, int n_views, const double* angles, const double* poses, const T* vol,
+                              const float* upstream, double* grad, int route) {
+  Vol<T> V{vol, g.nx, g.ny, g.nz};
+  for (int v = 0; v < n_views; ++v) {
+    View view(g, angles[v]);
+    Pose pose(poses + 6 * v);
+    const V3 so = mulT(pose.R, view.s - pose.t);
+    std::vector<double> rowacc((size_t)g.nv * 12, 0.0);
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int iv = 0; iv < g.nv; ++iv) {
+      std::vector<double> ts; std::vector<Seg> segs;
+      double acc[12] = {0};
+      for (int iu = 0; iu < g.nu; ++iu) {
+        const double w = (double)upstream[((size_t)v * g.nv + iv) * g.nu + iu];
+        V3 d = view.pixel(g, iu, iv) - view.s;
+        V3 eo = mulT(pose.R, (1.0 / sqrt(dot(d, d))) * d);
+        siddon_segments(g, so, eo, ts, segs);
+        V3 A = {0, 0, 0}, B = {0, 0, 0};
+        double GM[3][4] = {{0}};
+        for (const Seg& sg : segs) {
+          const long X = sg.ix, Y = sg.iy, Z = sg.iz;
+          V3 gj = {(V.at(X + 1, Y, Z) - V.at(X - 1, Y, Z)) / (2 * g.vx),
+                   (V.at(X, Y + 1, Z) - V.at(X, Y - 1, Z)) / (2 * g.vy),
+                   (V.at(X, Y, Z + 1) - V.at(X, Y, Z - 1)) / (2 * g.vz)};
+          V3 rj = voxel_centre(g, (int)X, (int)Y, (int)Z);
+          if (route == 0) {
+            A = A + sg.len * gj;
+            B = B + sg.len * cross(rj, gj);
+          } else {
+            V3 lever = mul(pose.R, rj), Rg = mul(pose.R, gj);
+            for (int a = 0; a < 3; ++a) {
+              GM[a][0] += sg.len * comp(lever, a) * gj.x;
+              GM[a][1] += sg.len * comp(lever, a) * gj.y;
+              GM[a][2] += sg.len * comp(lever, a) * gj.z;
+              GM[a][3] += -sg.len * comp(Rg, a);
+            }
+          }
+        }
+        if (route == 0) {
+          acc[0] += w * A.x; acc[1] += w * A.y; acc[2] += w * A.z;
+          acc[3] += w * B.x; acc[4] += w * B.y; acc[5] += w * B.z;
+        } else {
+          for (int a = 0; a < 3; ++a) for (int b = 0; b < 4; ++b) acc[a * 4 + b] += w * GM[a][b];
+        }
+      }
+      for (int q = 0; q < 12; ++q) rowacc[(size_t)iv * 12 + q] = acc[q];
+    }
+    double tot[12] = {0};
+    for (int iv = 0; iv < g.nv; ++iv) for (int q = 0; q < 12; ++q) tot[q] += rowacc[(size_t)iv * 12 + q];
+    double* out = grad + 6 * v;
+    if (route == 0) {
+      V3 SA = {tot[0], tot[1], tot[2]}, SB = {tot[3], tot[4], tot[5]};
+      V3 dt = mul(pose.R, SA);
+      out[0] = -dt.x; out[1] = -dt.y; out[2] = -dt.z;
+      const double* th = poses + 6 * v;
+      V3 wx = {1, 0, 0};
+      V3 wy = mulT(Rx(th[3]), V3{0, 1, 0});
+      V3 wz = mulT(mul(Ry(th[4]), Rx(th[3])), V3{0, 0, 1});
+      out[3] = -dot(wx, SB); out[4] = -dot(wy, SB); out[5] = -dot(wz, SB);
+    } else {
+      double GM[3][4];
+      for (int a = 0; a < 3; ++a) for (int b = 0; b < 4; ++b) GM[a][b] = tot[a * 4 + b];
+      contract_M(pose, GM, out);
+    }
+  }
+}
+
 extern "C" {
 
 int ora_num_threads() {
@@ -607,6 +758,28 @@ void ora_rotation(const double* pose6, double* R9, double* dR27) {
 void ora_projection_matrix(const ora_geom* g, double angle, double* P12) {
   View v(*g, angle);
   for (int i = 0; i < 3; ++i) for (int j = 0; j < 4; ++j) P12[i * 4 + j] = v.P[i][j];
+}
+
+// O12: Siddon weights (forward, explicit transpose, pose gradient)
+void ora_forward_siddon_f32(const ora_geom* g, int n_views, const double* angles, const double* poses,
+                            const float* vol, double* proj) {
+  forward_siddon_impl<float>(*g, n_views, angles, poses, vol, proj, nullptr, nullptr);
+}
+void ora_forward_siddon_f64(const ora_geom* g, int n_views, const double* angles, const double* poses,
+                            const double* vol, double* proj) {
+  forward_siddon_impl<double>(*g, n_views, angles, poses, vol, proj, nullptr, nullptr);
+}
+void ora_forward_siddon_T(const ora_geom* g, int n_views, const double* angles, const double* poses, const double* y,
+                          double* vol_out) {
+  forward_siddon_impl<double>(*g, n_views, angles, poses, (const double*)nullptr, nullptr, y, vol_out);
+}
+void ora_forward_pose_grad_siddon_f32(const ora_geom* g, int n_views, const double* angles, const double* poses,
+                                      const float* vol, const float* upstream, double* grad, int route) {
+  forward_grad_siddon_impl<float>(*g, n_views, angles, poses, vol, upstream, grad, route);
+}
+void ora_forward_pose_grad_siddon_f64(const ora_geom* g, int n_views, const double* angles, const double* poses,
+                                      const double* vol, const float* upstream, double* grad, int route) {
+  forward_grad_siddon_impl<double>(*g, n_views, angles, poses, vol, upstream, grad, route);
 }
 
 }  // extern "C"
