@@ -53,7 +53,14 @@ typedef struct dfp_geometry {
                            bit2 (DFP_FLAG_GRAD_INTERP): the two *_pose_grad calls differentiate the trilinear / bilinear
                            INTERPOLANT exactly (8 voxels / 4 pixels per sample, what automatic differentiation of the
                            discrete projector gives - PAPER.md :211, :346) instead of taking the paper's central finite
-                           differences of it (32 voxels / 12 pixels; Eq.19-22, :183, :202) */
+                           differences of it (32 voxels / 12 pixels; Eq.19-22, :183, :202);
+                           bit3 (DFP_FLAG_SIDDON): dfp_forward and dfp_forward_pose_grad use SIDDON weights - a^ij =
+                           length of ray i inside voxel j, voxels as boxes of constant value: the exact radiological
+                           path of the paper's own ray-driven projector (:213, ref [28]) - with the gradient's G_f^j
+                           taken per voxel (central differences of voxel values, lever arm at the voxel centre,
+                           Eq.19 :181, :189) instead of the default fixed-step trilinear ray-march; step_mm is then
+                           unused.  Not combinable with DFP_FLAG_GRAD_INTERP or dfp_forward_fused_moments
+                           (DFP_ERR_DIMS).  The back-projection calls ignore it. */
 } dfp_geometry;
 
 enum {
@@ -67,7 +74,7 @@ enum {
 };
 enum { DFP_OP_FORWARD = 0, DFP_OP_FORWARD_POSE_GRAD = 1, DFP_OP_BACKPROJECT = 2, DFP_OP_BACKPROJECT_POSE_GRAD = 3,
        DFP_OP_FORWARD_FUSED = 4 };
-enum { DFP_FLAG_DW = 1, DFP_FLAG_NO_TMA = 2, DFP_FLAG_GRAD_INTERP = 4 };
+enum { DFP_FLAG_DW = 1, DFP_FLAG_NO_TMA = 2, DFP_FLAG_GRAD_INTERP = 4, DFP_FLAG_SIDDON = 8 };
 
 /* Forward projection, Eq.2a :67-69 discretised as Eq.18 :172-177 with a fixed-step, zero-extended
  * trilinear ray-march (U1): proj[v][iv][iu] = D * sum_k f~(R_v^T (s_v + (k+1/2) D e_i - t_v)).

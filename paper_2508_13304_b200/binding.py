@@ -17,6 +17,7 @@ OP_FORWARD, OP_FORWARD_POSE_GRAD, OP_BACKPROJECT, OP_BACKPROJECT_POSE_GRAD, OP_F
 FLAG_DW = 1
 FLAG_NO_TMA = 2
 FLAG_GRAD_INTERP = 4
+FLAG_SIDDON = 8
 PATH_GATHER, PATH_TMA = 0, 1
 
 

@@ -1,0 +1,204 @@
+// dfp_siddon.cuh - forward projection and its pose gradient with SIDDON weights (DFP_FLAG_SIDDON).
+//
+// Siddon's exact radiological path [28] is the weight model of the paper's own ray-driven projector (PAPER.md :213,
+// ref :395): a^ij = length of ray i inside voxel j, voxels being boxes of constant value (Eq.18 :172-177).  The
+// gradient follows the paper's discretisation literally (Eq.19-20 :179-191, :189): per voxel j of the grid,
+// g_j = central differences of the zero-extended voxel values (:183) and the lever arm at the voxel centre r'_j;
+//   A_i = sum_j a^ij g_j,  B_i = sum_j a^ij r'_j x g_j   -> six running sums per ray, never the 12-element G_f^j,
+// then the same per-view reduction / contraction as the trilinear kernels (dL/dt = -R S_A, dL/dgamma_k = -w_k.S_B).
+//
+// One thread per ray, incremental 3-D DDA over the voxel grid (the merged plane-crossing list of Siddon's paper,
+// generated in order instead of sorted).  The crossing parameters run in fp64: they reach ~1000 mm while a segment
+// is ~1 voxel long, and a segment length is a DIFFERENCE of two of them (fp32 would leave 1e-4 relative error per
+// segment; fp64 adds and compares run at half the fp32 rate on B200).  Values are read straight from the caller's
+// volume through L1 (one voxel per segment; the six neighbours for the gradient) - no packed copy, no staging: this
+// is a first, plain kernel for the "next" row, measured beside the trilinear ones in DESIGN.md.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "dfp_kernels.cuh"
+
+namespace dfp {
+
+struct SiddonRay {
+  double t, tmax;              // current parameter (mm from the source) and exit parameter
+  double tn[3], dt[3];         // next crossing of each plane family, spacing of the crossings
+  int i[3], step[3];           // current voxel index, +-1 per axis
+  bool hit;
+};
+
+// Per-ray set-up (fp64, once per ray): the half-line s' + t e', t >= 0, against the grid box.
+__device__ __forceinline__ SiddonRay siddon_setup(const FwdGeom& G, const FwdView& V, int iu, int iv, double* e_out) {
+  const double dx = V.d0[0] + iu * V.du[0] + iv * V.dv[0];
+  const double dy = V.d0[1] + iu * V.du[1] + iv * V.dv[1];
+  const double dz = V.d0[2] + iu * V.du[2] + iv * V.dv[2];
+  const double inv = 1.0 / sqrt(dx * dx + dy * dy + dz * dz);
+  const double e[3] = {dx * inv, dy * inv, dz * inv};
+  const int n[3] = {G.L.nx, G.L.ny, G.L.nz};
+  const double v[3] = {(double)G.vx, (double)G.vy, (double)G.vz}, c[3] = {(double)G.cx, (double)G.cy, (double)G.cz};
+  SiddonRay r;
+  r.hit = true;
+  double tmin = 0.0, tmax = 1e300, lo[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    lo[a] = c[a] - 0.5 * n[a] * v[a];
+    const double hi = c[a] + 0.5 * n[a] * v[a], o = V.src[a];
+    if (fabs(e[a]) < 1e-300) {
+      if (o <= lo[a] || o >= hi) r.hit = false;
+    } else {
+      double t0 = (lo[a] - o) / e[a], t1 = (hi - o) / e[a];
+      if (t0 > t1) { const double s = t0; t0 = t1; t1 = s; }
+      tmin = fmax(tmin, t0);
+      tmax = fmin(tmax, t1);
+    }
+  }
+  if (!(tmax > tmin)) r.hit = false;
+  r.t = tmin;
+  r.tmax = tmax;
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    const double p = V.src[a] + tmin * e[a];
+    int i = (int)floor((p - lo[a]) / v[a]);
+    i = min(max(i, 0), n[a] - 1);
+    r.i[a] = i;
+    if (fabs(e[a]) < 1e-300) {
+      r.step[a] = 0; r.dt[a] = 1e300; r.tn[a] = 1e300;
+    } else {
+      r.step[a] = e[a] > 0 ? 1 : -1;
+      r.dt[a] = v[a] / fabs(e[a]);
+      r.tn[a] = (lo[a] + (i + (e[a] > 0 ? 1 : 0)) * v[a] - V.src[a]) / e[a];
+    }
+    if (e_out) e_out[a] = e[a];
+  }
+  return r;
+}
+
+// One DDA step: returns the length of the segment inside the current voxel, then advances index, linear offset and
+// the crossed family's next parameter.  `alive` turns false once the ray has left the grid (or reached tmax).
+// Written with selects on named scalars (an array indexed by the crossed axis would live in local memory).
+struct SiddonState {
+  double t, tmax, tnx, tny, tnz, dtx, dty, dtz;
+  int ix, iy, iz, sx, sy, sz, idx;
+};
+__device__ __forceinline__ SiddonState siddon_state(const SiddonRay& r, int nx, int ny) {
+  SiddonState s;
+  s.t = r.t; s.tmax = r.tmax;
+  s.tnx = r.tn[0]; s.tny = r.tn[1]; s.tnz = r.tn[2];
+  s.dtx = r.dt[0]; s.dty = r.dt[1]; s.dtz = r.dt[2];
+  s.ix = r.i[0]; s.iy = r.i[1]; s.iz = r.i[2];
+  s.sx = r.step[0]; s.sy = r.step[1]; s.sz = r.step[2];
+  s.idx = (s.iz * ny + s.iy) * nx + s.ix;
+  return s;
+}
+__device__ __forceinline__ float siddon_step(SiddonState& s, int nx, int ny, int nz, bool& alive) {
+  const bool cx = s.tnx <= s.tny && s.tnx <= s.tnz;
+  const bool cy = !cx && s.tny <= s.tnz;
+  const double tcross = cx ? s.tnx : (cy ? s.tny : s.tnz);
+  const double tn = fmin(tcross, s.tmax);
+  const float len = (float)fmax(tn - s.t, 0.0);
+  s.t = tn;
+  bool inside;
+  if (cx) {
+    s.tnx += s.dtx; s.ix += s.sx; s.idx += s.sx;
+    inside = (unsigned)s.ix < (unsigned)nx;
+  } else if (cy) {
+    s.tny += s.dty; s.iy += s.sy; s.idx += s.sy * nx;
+    inside = (unsigned)s.iy < (unsigned)ny;
+  } else {
+    s.tnz += s.dtz; s.iz += s.sz; s.idx += s.sz * nx * ny;
+    inside = (unsigned)s.iz < (unsigned)nz;
+  }
+  alive = inside && s.t < s.tmax;
+  return len;
+}
+
+// ------------------------------------------------------------------------------------------------ forward
+__global__ void __launch_bounds__(kFwdThreads) siddon_fwd_kernel(FwdGeom G, const FwdView* __restrict__ views,
+                                                                 const float* __restrict__ vol,
+                                                                 float* __restrict__ proj) {
+  int iu, iv;
+  fwd_pixel(iu, iv);
+  const int view = blockIdx.z;
+  if (iu >= G.nu || iv >= G.nv) return;
+  const SiddonRay r = siddon_setup(G, views[view], iu, iv, nullptr);
+  const int nx = G.L.nx, ny = G.L.ny, nz = G.L.nz;
+  float sum = 0.f;
+  if (r.hit) {
+    SiddonState s = siddon_state(r, nx, ny);
+    bool alive = true;
+    while (alive) {
+      const float val = __ldg(vol + s.idx);
+      const float len = siddon_step(s, nx, ny, nz, alive);
+      sum = fmaf(len, val, sum);
+    }
+  }
+  proj[((size_t)view * G.nv + iv) * G.nu + iu] = sum;
+}
+
+// ------------------------------------------------------------------------------------------------ pose gradient
+__global__ void __launch_bounds__(kFwdThreads) siddon_grad_kernel(FwdGeom G, const FwdView* __restrict__ views,
+                                                                  const float* __restrict__ vol,
+                                                                  const float* __restrict__ upstream,
+                                                                  float* __restrict__ partials) {
+  int iu, iv;
+  fwd_pixel(iu, iv);
+  const int view = blockIdx.z;
+  const bool live = iu < G.nu && iv < G.nv;
+  float out[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  if (live) {
+    const SiddonRay r = siddon_setup(G, views[view], iu, iv, nullptr);
+    const int nx = G.L.nx, ny = G.L.ny, nz = G.L.nz;
+    const int sy_ = nx, sz_ = nx * ny;
+    // voxel centre r'_j = c + (i - (n-1)/2) v
+    const float hx = 0.5f * (float)(nx - 1), hy = 0.5f * (float)(ny - 1), hz = 0.5f * (float)(nz - 1);
+    float ax_ = 0.f, ay_ = 0.f, az_ = 0.f, bx = 0.f, by = 0.f, bz = 0.f;     // A_i, B_i
+    if (r.hit) {
+      SiddonState s = siddon_state(r, nx, ny);
+      bool alive = true;
+      while (alive) {
+        const int ix = s.ix, iy = s.iy, iz = s.iz;
+        const float* c = vol + s.idx;
+        // central differences of the zero-extended voxel values (2 v_a g_a)
+        const float gx = ((ix + 1 < nx) ? __ldg(c + 1) : 0.f) - ((ix > 0) ? __ldg(c - 1) : 0.f);
+        const float gy = ((iy + 1 < ny) ? __ldg(c + sy_) : 0.f) - ((iy > 0) ? __ldg(c - sy_) : 0.f);
+        const float gz = ((iz + 1 < nz) ? __ldg(c + sz_) : 0.f) - ((iz > 0) ? __ldg(c - sz_) : 0.f);
+        const float rx = fmaf((float)ix - hx, G.vx, G.cx), ry = fmaf((float)iy - hy, G.vy, G.cy),
+                    rz = fmaf((float)iz - hz, G.vz, G.cz);
+        const float len = siddon_step(s, nx, ny, nz, alive);
+        const float lx = len * gx * G.sgx, ly = len * gy * G.sgy, lz = len * gz * G.sgz;   // a^ij g_j  (sg = 1 / 2v)
+        ax_ += lx; ay_ += ly; az_ += lz;
+        bx += ry * lz - rz * ly;
+        by += rz * lx - rx * lz;
+        bz += rx * ly - ry * lx;
+      }
+    }
+    const float w = __ldg(upstream + ((size_t)view * G.nv + iv) * G.nu + iu);
+    out[0] = w * ax_; out[1] = w * ay_; out[2] = w * az_;
+    out[3] = w * bx; out[4] = w * by; out[5] = w * bz;
+  }
+  // a5, first stage: warp shuffle, then across the block's warps through shared memory (fixed order)
+  __shared__ float red[kFwdThreads / 32][6];
+#pragma unroll
+  for (int q = 0; q < 6; ++q) {
+    float v = out[q];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    out[q] = v;
+  }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (lane == 0) {
+#pragma unroll
+    for (int q = 0; q < 6; ++q) red[warp][q] = out[q];
+  }
+  __syncthreads();
+  if (threadIdx.x < 6) {
+    float s = 0.f;
+#pragma unroll
+    for (int wI = 0; wI < kFwdThreads / 32; ++wI) s += red[wI][threadIdx.x];
+    const size_t blk = (size_t)blockIdx.y * gridDim.x + blockIdx.x;
+    const size_t nblk = (size_t)gridDim.x * gridDim.y;
+    partials[((size_t)view * nblk + blk) * 6 + threadIdx.x] = s;
+  }
+}
+
+}  // namespace dfp

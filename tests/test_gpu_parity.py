@@ -502,3 +502,55 @@ def test_host_buffer_entry_points_chunked_views(dfp):
     got = dfp.backproject_pose_grad_host(g, a, p, pj, wv).numpy()
     ref = dfp.backproject_pose_grad(g, a, p, proj, torch.as_tensor(wv, device=dev)).cpu().numpy()
     assert np.array_equal(got, ref)
+
+
+# ------------------------------------------------------------------ DFP_FLAG_SIDDON
+def run_siddon_case(dfp, g, angles, poses, vol, up):
+    dev = torch.device("cuda:0")
+    gs = g.replace(flags=g.flags | dfp.FLAG_SIDDON)
+    angles, poses = f32(angles), f32(poses).reshape(-1, 6)
+    vol_d = torch.as_tensor(vol, dtype=torch.float32, device=dev).contiguous()
+    up_d = torch.as_tensor(up, dtype=torch.float32, device=dev).contiguous()
+    proj = dfp.forward(gs, angles, poses, vol_d).cpu().numpy()
+    grad = dfp.forward_pose_grad(gs, angles, poses, vol_d, up_d).cpu().numpy()
+    o_proj = oracle.forward_siddon(g, angles, poses, vol_d.cpu().numpy())
+    o_grad = oracle.forward_pose_grad_siddon(g, angles, poses, vol_d.cpu().numpy(), up_d.cpu().numpy())
+    return proj, grad, o_proj, o_grad
+
+
+def test_siddon_ragged_anisotropic_and_degenerate(dfp):
+    g = aniso_geom(nx=37, ny=29, nz=23, nu=45, nv=21)
+    rng = np.random.default_rng(30)
+    vol = rng.random(g.vol_shape).astype(np.float32)
+    up = rng.standard_normal((3,) + g.det_shape).astype(np.float32)
+    check_forward(run_siddon_case(dfp, g, ANGLES3, POSES3, vol, up))
+    # axis-parallel central ray (beta = 0, identity pose, odd detector: the middle ray has e_y = e_z = 0 exactly)
+    g = small_geom(n=12, nu=11, nv=9)
+    vol = rng.random(g.vol_shape).astype(np.float32)
+    up = rng.standard_normal((1,) + g.det_shape).astype(np.float32)
+    check_forward(run_siddon_case(dfp, g, [0.0], [[0] * 6], vol, up))
+    # misses and an empty volume: exact zeros
+    proj, grad, _, _ = run_siddon_case(dfp, g, [0.3], [[0, 0, 700.0, 0, 0, 0]], vol, up)
+    assert np.all(proj == 0) and np.all(grad == 0)
+    # single voxel
+    g1 = small_geom(n=1, voxel=4.0, nu=3, nv=3, pix=1.0)
+    check_forward(run_siddon_case(dfp, g1, [0.2], [[0.3, 0.2, -0.1, 0.01, 0.02, 0.03]], np.full(g1.vol_shape, 0.7, np.float32),
+                                  np.ones((1,) + g1.det_shape, np.float32)))
+
+
+@pytest.mark.parametrize("index,scale,views", [(1, 1.0, None), (2, 0.25, 3), (4, 0.125, 4), (5, 0.125, 3)])
+def test_siddon_configs_reduced(dfp, index, scale, views):
+    w = W.make_config(index, scale=scale, n_views=views)
+    check_forward(run_siddon_case(dfp, w.geom, w.angles.numpy(), w.poses.numpy(), w.volume().numpy(),
+                                  w.fwd_upstream().numpy()))
+
+
+def test_siddon_rejects_modes_it_does_not_have(dfp):
+    w = W.make_config(1)
+    dev = torch.device("cuda:0")
+    a, p = f32(w.angles.numpy()), f32(w.poses.numpy()).reshape(-1, 6)
+    vol, up = w.volume(dev), w.fwd_upstream(dev)
+    with pytest.raises(dfp.DfpError):
+        dfp.forward_pose_grad(w.geom.replace(flags=dfp.FLAG_SIDDON | dfp.FLAG_GRAD_INTERP), a, p, vol, up)
+    with pytest.raises(dfp.DfpError):
+        dfp.forward_fused_moments(w.geom.replace(flags=dfp.FLAG_SIDDON), a, p, vol, up)
