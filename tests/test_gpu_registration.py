@@ -59,3 +59,39 @@ def test_registration_by_adam_on_ncc_recovers_a_hidden_pose():
     assert t1 < 0.15 * t0 and r1 < 0.15 * r0, hist[::15]          # within 0.6 mm / 0.45 degrees from 4 mm / 3 degrees
     # and the ascent direction was right from the first step: NCC rises over the first iterations
     assert hist[10][0] > ncc0
+
+
+def test_pose_of_one_view_recovered_through_the_backprojector():
+    """The back-projection counterpart (Eq.23b :217, the building block of motion compensation, Eq.26):
+    minimise || A^T(M(theta)) l - mu_ref ||^2 over ONE view's pose with Adam, gradient from
+    dfp_backproject_pose_grad (upstream 2 (mu - mu_ref)); the other views stay at their true poses."""
+    import paper_2508_13304_b200 as dfp
+    dev = torch.device("cuda:0")
+    w = W.make_config(3, scale=0.25, n_views=8)
+    g = w.geom.replace(bp_weight=0)
+    a = w.angles.float().numpy()
+    proj = w.closed_form(w.data_poses, dev).float().contiguous()         # smooth, unfiltered projections
+    true = np.zeros((8, 6))
+    mu_ref = dfp.backproject(g, a, true.astype(np.float32), proj).double()
+    v = 3
+    hidden = true[v].copy()
+    theta = np.array([2.0, -1.5, 1.0, 1.5 * DEG, -1.0 * DEG, 1.2 * DEG])
+    m = np.zeros(6)
+    s = np.zeros(6)
+    lr = np.array([0.15, 0.15, 0.15, 0.002, 0.002, 0.002])
+    b1, b2, eps = 0.9, 0.999, 1e-8
+    hist = []
+    for it in range(1, 201):
+        poses = true.copy()
+        poses[v] = theta
+        mu = dfp.backproject(g, a, poses.astype(np.float32), proj)
+        diff = mu.double() - mu_ref
+        loss = float((diff * diff).sum())
+        up = (2.0 * diff).float().contiguous()
+        grad = dfp.backproject_pose_grad(g, a, poses.astype(np.float32), proj, up)[v].double().cpu().numpy()
+        hist.append((loss, float(np.abs(theta[:3] - hidden[:3]).max()), float(np.abs(theta[3:] - hidden[3:]).max())))
+        m = b1 * m + (1 - b1) * grad
+        s = b2 * s + (1 - b2) * grad * grad
+        theta = theta - lr * (m / (1 - b1 ** it)) / (np.sqrt(s / (1 - b2 ** it)) + eps)
+    assert hist[-1][0] < 0.02 * hist[0][0], (hist[0], hist[-1])
+    assert hist[-1][1] < 0.2 * hist[0][1] and hist[-1][2] < 0.2 * hist[0][2], hist[::20]
