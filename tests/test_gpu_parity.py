@@ -554,3 +554,24 @@ def test_siddon_rejects_modes_it_does_not_have(dfp):
         dfp.forward_pose_grad(w.geom.replace(flags=dfp.FLAG_SIDDON | dfp.FLAG_GRAD_INTERP), a, p, vol, up)
     with pytest.raises(dfp.DfpError):
         dfp.forward_fused_moments(w.geom.replace(flags=dfp.FLAG_SIDDON), a, p, vol, up)
+
+
+def test_tma_paths_axis_aligned_views_and_other_step_sizes(dfp):
+    """Gantry at 0 / 90 / 180 / 270 degrees with the identity pose (ray direction components exactly zero: chunk
+    lengths limited by one axis only), and ray-march steps of 0.45 and 1.7 voxels (longer / shorter chunks)."""
+    w = W.make_config(2, scale=0.25, n_views=4)
+    vol = w.volume().numpy()
+    up = w.fwd_upstream().numpy()
+    angles = [0.0, math.pi / 2, math.pi, 1.5 * math.pi]
+    zero = np.zeros((4, 6))
+    dev = torch.device("cuda:0")
+    for step in (0.0, 0.45 * w.geom.vx, 1.7 * w.geom.vx):
+        g = w.geom.replace(step_mm=step)
+        res = run_forward_case(dfp, g, angles, zero, vol, up)
+        assert dfp.last_path() == dfp.PATH_TMA
+        check_forward(res)
+    proj = res[0]
+    bup = np.random.default_rng(31).standard_normal(w.geom.vol_shape).astype(np.float32)
+    resb = run_back_case(dfp, w.geom, angles, zero, proj, bup)
+    assert dfp.last_path() == dfp.PATH_TMA
+    check_back(resb)
