@@ -60,7 +60,10 @@ typedef struct dfp_geometry {
                            taken per voxel (central differences of voxel values, lever arm at the voxel centre,
                            Eq.19 :181, :189) instead of the default fixed-step trilinear ray-march; step_mm is then
                            unused.  Not combinable with DFP_FLAG_GRAD_INTERP or dfp_forward_fused_moments
-                           (DFP_ERR_DIMS).  The back-projection calls ignore it. */
+                           (DFP_ERR_DIMS).  The back-projection calls ignore it;
+                           bit4 (DFP_FLAG_ACCUMULATE): dfp_backproject ADDS the views' contribution to d_vol instead of
+                           overwriting it, so that the sum over views (Eq.21) can be taken slice by slice of the view
+                           arrays (view chunking; a view-sharded multi-GPU reconstruction).  Other calls ignore it. */
 } dfp_geometry;
 
 enum {
@@ -74,7 +77,8 @@ enum {
 };
 enum { DFP_OP_FORWARD = 0, DFP_OP_FORWARD_POSE_GRAD = 1, DFP_OP_BACKPROJECT = 2, DFP_OP_BACKPROJECT_POSE_GRAD = 3,
        DFP_OP_FORWARD_FUSED = 4 };
-enum { DFP_FLAG_DW = 1, DFP_FLAG_NO_TMA = 2, DFP_FLAG_GRAD_INTERP = 4, DFP_FLAG_SIDDON = 8 };
+enum { DFP_FLAG_DW = 1, DFP_FLAG_NO_TMA = 2, DFP_FLAG_GRAD_INTERP = 4, DFP_FLAG_SIDDON = 8,
+       DFP_FLAG_ACCUMULATE = 16 };
 
 /* Forward projection, Eq.2a :67-69 discretised as Eq.18 :172-177 with a fixed-step, zero-extended
  * trilinear ray-march (U1): proj[v][iv][iu] = D * sum_k f~(R_v^T (s_v + (k+1/2) D e_i - t_v)).
@@ -126,9 +130,10 @@ size_t dfp_workspace_bytes(const dfp_geometry* geometry, int n_views, int op);
 
 /* Same four operations with HOST buffers (h_*: host memory, pinned or pageable).  Each allocates device
  * scratch with cudaMallocAsync on `stream`, copies inputs in, runs the device call above, copies the result
- * out, frees, and synchronises `stream` before returning.  With 8 or more views every call but
- * dfp_backproject_host moves the per-view arrays in 4 chunks on an internal second stream, overlapped with the
- * kernels of the neighbouring chunk (results do not depend on the chunking: views are independent there).  The
+ * out, frees, and synchronises `stream` before returning.  With 8 or more views the per-view arrays move in 4
+ * chunks on an internal second stream, overlapped with the kernels of the neighbouring chunk (per-view results do
+ * not depend on the chunking; dfp_backproject_host sums its chunks with DFP_FLAG_ACCUMULATE, which changes the
+ * fp32 summation order only).  The
  * first host call on a device raises the release threshold of its default stream-ordered memory pool so that
  * later calls reuse the scratch memory. */
 int dfp_forward_host(const dfp_geometry* geometry, int n_views, const float* angles, const float* poses,

@@ -586,10 +586,10 @@ int run_host(int op, const dfp_geometry* g, int V, const float* angles, const fl
   DFP_CUDA(d_up.alloc(n_up), "cudaMallocAsync");
   DFP_CUDA(d_out.alloc(n_out), "cudaMallocAsync");
   DFP_CUDA(d_ws.alloc(n_ws), "cudaMallocAsync");
-  // a9, view chunking: every call but dfp_backproject is independent per view, so the per-view arrays move in
-  // chunks on a second stream while the kernels of the neighbouring chunk run (the input shared by all views - the
-  // volume, or the upstream volume of the back-projection gradient - goes first, on the caller's stream).
-  const int n_chunks = (op == DFP_OP_BACKPROJECT || V < 8) ? 1 : 4;
+  // a9, view chunking: the per-view arrays move in chunks on a second stream while the kernels of the neighbouring
+  // chunk run (the input shared by all views - the volume, or the upstream volume of the back-projection gradient -
+  // goes first, on the caller's stream); dfp_backproject sums its chunks with DFP_FLAG_ACCUMULATE.
+  const int n_chunks = V < 8 ? 1 : 4;
   if (n_chunks == 1) {
     DFP_CUDA(cudaMemcpyAsync(d_in.p, h_in, n_in, cudaMemcpyHostToDevice, s), "H2D");
     if (grad) DFP_CUDA(cudaMemcpyAsync(d_up.p, h_up, n_up, cudaMemcpyHostToDevice, s), "H2D");
@@ -622,7 +622,7 @@ int run_host(int op, const dfp_geometry* g, int V, const float* angles, const fl
   float* d_views = static_cast<float*>(fwd ? d_up.p : d_in.p);
   DFP_CUDA(cudaEventRecord(side.ev[0], s), "cudaEventRecord");
   DFP_CUDA(cudaStreamWaitEvent(side.s2, side.ev[0], 0), "cudaStreamWaitEvent");
-  DFP_CUDA(cudaMemcpyAsync(d_shared, h_shared, nvol, cudaMemcpyHostToDevice, s), "H2D");
+  if (h_shared) DFP_CUDA(cudaMemcpyAsync(d_shared, h_shared, nvol, cudaMemcpyHostToDevice, s), "H2D");
   int launches = 0;
   for (int c = 0; c < n_chunks; ++c) {
     const int v0 = (int)((long long)V * c / n_chunks), v1 = (int)((long long)V * (c + 1) / n_chunks), nv_c = v1 - v0;
@@ -637,11 +637,17 @@ int run_host(int op, const dfp_geometry* g, int V, const float* angles, const fl
     if (fwd)
       st = run_forward(g, nv_c, angles + v0, poses + 6 * v0, d_shared, grad ? d_views + off : nullptr, out_c, d_ws.p,
                        n_ws, s, grad ? DFP_OP_FORWARD_POSE_GRAD : DFP_OP_FORWARD);
-    else
+    else if (grad)
       st = run_backproject(g, nv_c, angles + v0, poses + 6 * v0, d_views + off, d_shared, out_c, d_ws.p, n_ws, s, true);
+    else {                           // dfp_backproject: the first chunk overwrites the volume, the others add to it
+      dfp_geometry gc = *g;
+      gc.flags = c ? (g->flags | DFP_FLAG_ACCUMULATE) : g->flags;
+      st = run_backproject(&gc, nv_c, angles + v0, poses + 6 * v0, d_views + off, nullptr, static_cast<float*>(d_out.p),
+                           d_ws.p, n_ws, s, false);
+    }
     if (st) return st;
     launches += g_launches;
-    if (!grad) {                     // dfp_forward: this chunk's projections go home while the next chunk is computed
+    if (fwd && !grad) {              // dfp_forward: this chunk's projections go home while the next chunk is computed
       DFP_CUDA(cudaEventRecord(side.ev[4 + c], s), "cudaEventRecord");
       DFP_CUDA(cudaStreamWaitEvent(side.s2, side.ev[4 + c], 0), "cudaStreamWaitEvent");
       DFP_CUDA(cudaMemcpyAsync(h_out + off, out_c, (size_t)nv_c * per_view * 4, cudaMemcpyDeviceToHost, side.s2),
@@ -649,7 +655,7 @@ int run_host(int op, const dfp_geometry* g, int V, const float* angles, const fl
     }
   }
   g_launches = launches;
-  if (grad) DFP_CUDA(cudaMemcpyAsync(h_out, d_out.p, n_out, cudaMemcpyDeviceToHost, s), "D2H");
+  if (grad || !fwd) DFP_CUDA(cudaMemcpyAsync(h_out, d_out.p, n_out, cudaMemcpyDeviceToHost, s), "D2H");
   DFP_CUDA(cudaStreamSynchronize(side.s2), "stream synchronize");
   DFP_CUDA(cudaStreamSynchronize(s), "stream synchronize");
   return DFP_OK;

@@ -162,7 +162,8 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_tma_kernel(BpGeom G, int n_v
   const float xf = (float)ix - G.hx, yf = (float)iy - G.hy, zf = (float)T.z0 - G.hz;
   float acc[TZ];
 #pragma unroll
-  for (int m = 0; m < TZ; ++m) acc[m] = 0.f;
+  for (int m = 0; m < TZ; ++m)     // DFP_FLAG_ACCUMULATE: start from the caller's volume (a slice of the views)
+    acc[m] = ((G.flags & DFP_FLAG_ACCUMULATE) && live && m < T.tz) ? vol[((size_t)(T.z0 + m) * G.ny + iy) * G.nx + ix] : 0.f;
   bool bad = false;
   for (int view = 0; view < n_views; ++view) {
     const int s = view % n_stages;

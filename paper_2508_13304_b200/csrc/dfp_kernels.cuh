@@ -402,7 +402,9 @@ __global__ void __launch_bounds__(kBpThreads) bp_kernel(BpGeom G, int n_views, c
   const size_t per = (size_t)G.pu * G.pv;
   float acc[kBpZ];
 #pragma unroll
-  for (int m = 0; m < kBpZ; ++m) acc[m] = 0.f;
+  for (int m = 0; m < kBpZ; ++m)   // DFP_FLAG_ACCUMULATE: start from the caller's volume (a slice of the views)
+    acc[m] = ((G.flags & DFP_FLAG_ACCUMULATE) && ix < G.nx && iy < G.ny && z0 + m < G.nz)
+                 ? vol[((size_t)(z0 + m) * G.ny + iy) * G.nx + ix] : 0.f;
   for (int view = 0; view < n_views; ++view) {
     __syncthreads();
     if (threadIdx.x < sizeof(BpView) / 4) ((float*)&sv)[threadIdx.x] = ((const float*)(views + view))[threadIdx.x];

@@ -498,7 +498,8 @@ def test_host_buffer_entry_points_chunked_views(dfp):
                        dfp.forward_pose_grad(g, a, p, vd, ud).cpu())
     pj = proj.cpu().numpy()
     wv = np.random.default_rng(5).standard_normal(g.vol_shape).astype(np.float32)
-    assert torch.equal(dfp.backproject_host(g, a, p, pj), dfp.backproject(g, a, p, proj).cpu())
+    # the back-projection sums its 4 view chunks with DFP_FLAG_ACCUMULATE: same terms, another fp32 summation order
+    assert rel_l2(dfp.backproject_host(g, a, p, pj).numpy(), dfp.backproject(g, a, p, proj).cpu().numpy()) <= 1e-6
     got = dfp.backproject_pose_grad_host(g, a, p, pj, wv).numpy()
     ref = dfp.backproject_pose_grad(g, a, p, proj, torch.as_tensor(wv, device=dev)).cpu().numpy()
     assert np.array_equal(got, ref)
@@ -575,3 +576,21 @@ def test_tma_paths_axis_aligned_views_and_other_step_sizes(dfp):
     resb = run_back_case(dfp, w.geom, angles, zero, proj, bup)
     assert dfp.last_path() == dfp.PATH_TMA
     check_back(resb)
+
+
+def test_backproject_accumulate_flag_sums_view_slices(dfp):
+    """DFP_FLAG_ACCUMULATE: back-projecting views [0, k) and then adding views [k, V) equals the whole call (Eq.21 is a
+    sum over views), on both kernel paths; without the flag the second call would overwrite."""
+    w = W.make_config(3, scale=0.25, n_views=10)
+    dev = torch.device("cuda:0")
+    a, p = f32(w.angles.numpy()), f32(w.poses.numpy()).reshape(-1, 6)
+    proj = w.projections(dev)
+    for base in (0, dfp.FLAG_NO_TMA):
+        g = w.geom.replace(flags=base)
+        whole = dfp.backproject(g, a, p, proj).cpu().numpy()
+        vol = dfp.backproject(g, a[:4], p[:4], proj[:4].contiguous())
+        first = vol.cpu().numpy().copy()
+        ga = g.replace(flags=base | dfp.FLAG_ACCUMULATE)
+        dfp.backproject(ga, a[4:], p[4:], proj[4:].contiguous(), out=vol)
+        assert rel_l2(vol.cpu().numpy(), whole) <= 1e-6
+        assert rel_l2(first, whole) > 0.1                      # the first slice alone is not the answer
