@@ -246,3 +246,49 @@ def forward_pose_grad_siddon(g, angles, poses, vol, upstream, route=ROUTE_SIX):
     assert vol.shape == (gg.nz, gg.ny, gg.nx)
     fn(ctypes.byref(gg), V, _p(angles), _p(poses), _p(vol), _p(up), _p(grad), int(route))
     return grad
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# O13: Joseph's projector (plane-by-plane along the driving axis, bilinear in each plane)
+def _model_call(name, g, angles, poses, vol, extra=()):
+    lib = _load()
+    angles, poses, V = _views(angles, poses)
+    if hasattr(vol, "detach"):
+        vol = vol.detach().cpu().numpy()
+    gg = _geom(g)
+    if np.asarray(vol).dtype == np.float64:
+        vol = np.ascontiguousarray(vol)
+        fn = getattr(lib, name + "_f64")
+    else:
+        vol = _f32(vol)
+        fn = getattr(lib, name + "_f32")
+    assert vol.shape == (gg.nz, gg.ny, gg.nx)
+    return fn, gg, angles, poses, V, vol
+
+
+def forward_joseph(g, angles, poses, vol):
+    """l_i = (v_a*/|e_a*|) sum over voxel-centre planes of the bilinear interpolant.  -> proj [V,nv,nu] float64."""
+    fn, gg, angles, poses, V, vol = _model_call("ora_forward_joseph", g, angles, poses, vol)
+    proj = np.empty((V, gg.nv, gg.nu), dtype=np.float64)
+    fn(ctypes.byref(gg), V, _p(angles), _p(poses), _p(vol), _p(proj))
+    return proj
+
+
+def forward_joseph_T(g, angles, poses, y):
+    """Explicit transpose of `forward_joseph` (adjointness pin).  y [V,nv,nu] -> vol float64."""
+    lib = _load()
+    angles, poses, V = _views(angles, poses)
+    gg = _geom(g)
+    y = _f64(y, (V, gg.nv, gg.nu))
+    out = np.empty((gg.nz, gg.ny, gg.nx), dtype=np.float64)
+    lib.ora_forward_joseph_T(ctypes.byref(gg), V, _p(angles), _p(poses), _p(y), _p(out))
+    return out
+
+
+def forward_pose_grad_joseph(g, angles, poses, vol, upstream):
+    """Pose gradient with Joseph weights and per-voxel G_f^j (Eq.19-20, :189).  -> [V,6] float64."""
+    fn, gg, angles, poses, V, vol = _model_call("ora_forward_pose_grad_joseph", g, angles, poses, vol)
+    up = _f32(upstream).reshape(V, gg.nv, gg.nu)
+    grad = np.empty((V, 6), dtype=np.float64)
+    fn(ctypes.byref(gg), V, _p(angles), _p(poses), _p(vol), _p(up), _p(grad))
+    return grad

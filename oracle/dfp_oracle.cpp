@@ -13,7 +13,10 @@
 // 12-element G route, stored-G literal algorithm, brute-force back-projection on tiny grids;
 // Siddon weights (O12, tests/test_oracle_siddon.py): chord of the grid box, brute-force clipping
 // of the ray against every voxel's own box, explicit transpose, closed forms, the paper's literal
-// stored-G algorithm, finite differences of closed-form projections.
+// stored-G algorithm, finite differences of closed-form projections; Joseph weights (O13,
+// tests/test_oracle_joseph.py): hand formulas for constant and in-plane-linear volumes, explicit
+// transpose, closed forms with second-order convergence on all three driving axes, stored-G,
+// finite differences of closed-form projections.
 // No function here is "parity unpinned".
 //
 // Conventions:
@@ -695,6 +698,120 @@ void forward_grad_siddon_impl(const ora_geom& g, int n_views, const double* angl
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// O13: Joseph's projector (BASELINE.json north_star: "trilinear or Joseph interpolation").
+// The ray is stepped from voxel-centre plane to voxel-centre plane along its DRIVING axis a* = argmax_a |e'_a|
+// (object frame); in each plane the volume is interpolated bilinearly (zero-extended) at the intersection point, and
+// every plane carries the path length between consecutive planes, v_a* / |e'_a*|:
+//   l_i = (v_a* / |e'_a*|) sum_k bilin_k,   a^ij = (v_a* / |e'_a*|) x (bilinear weight of voxel j in its plane).
+// Only intersections on the half-line t > 0 from the source count (as O6).  `visit` receives (weight, ix, iy, iz) for
+// every voxel of the GRID with a non-zero weight.
+template <typename F>
+inline void joseph_weights(const ora_geom& g, V3 so, V3 eo, F visit) {
+  const int n[3] = {g.nx, g.ny, g.nz};
+  const double v[3] = {g.vx, g.vy, g.vz}, c[3] = {g.cx, g.cy, g.cz};
+  int a = 0;
+  for (int k = 1; k < 3; ++k) if (fabs(comp(eo, k)) > fabs(comp(eo, a))) a = k;
+  const int b = (a + 1) % 3, d = (a + 2) % 3;
+  const double ea = comp(eo, a);
+  if (fabs(ea) < 1e-300) return;
+  const double wlen = v[a] / fabs(ea);
+  for (int k = 0; k < n[a]; ++k) {
+    const double xa = c[a] + (k - (n[a] - 1) / 2.0) * v[a];            // plane of voxel centres (O1)
+    const double t = (xa - comp(so, a)) / ea;
+    if (!(t > 0)) continue;
+    const double pb = (comp(so, b) + t * comp(eo, b) - c[b]) / v[b] + (n[b] - 1) / 2.0;   // continuous indices
+    const double pd = (comp(so, d) + t * comp(eo, d) - c[d]) / v[d] + (n[d] - 1) / 2.0;
+    const double fb = floor(pb), fd = floor(pd), ab = pb - fb, ad = pd - fd;
+    for (int jd = 0; jd < 2; ++jd) for (int jb = 0; jb < 2; ++jb) {
+      const long ib = (long)fb + jb, id = (long)fd + jd;
+      if (ib < 0 || id < 0 || ib >= n[b] || id >= n[d]) continue;
+      const double w = wlen * (jb ? ab : 1 - ab) * (jd ? ad : 1 - ad);
+      if (w == 0.0) continue;
+      long idx[3];
+      idx[a] = k; idx[b] = ib; idx[d] = id;
+      visit(w, idx[0], idx[1], idx[2]);
+    }
+  }
+}
+
+// forward (vol_out == nullptr) or explicit transpose (adjointness pin only)
+template <typename T>
+void forward_joseph_impl(const ora_geom& g, int n_views, const double* angles, const double* poses, const T* vol,
+                         double* proj, const double* y_in, double* vol_out) {
+  Vol<T> V{vol, g.nx, g.ny, g.nz};
+  const bool transpose = vol_out != nullptr;
+  if (transpose) for (size_t i = 0; i < (size_t)g.nx * g.ny * g.nz; ++i) vol_out[i] = 0.0;
+  for (int v = 0; v < n_views; ++v) {
+    View view(g, angles[v]);
+    Pose pose(poses + 6 * v);
+    const V3 so = mulT(pose.R, view.s - pose.t);
+#pragma omp parallel for schedule(dynamic, 4) if (!transpose)
+    for (int iv = 0; iv < g.nv; ++iv) {
+      for (int iu = 0; iu < g.nu; ++iu) {
+        V3 d = view.pixel(g, iu, iv) - view.s;
+        V3 eo = mulT(pose.R, (1.0 / sqrt(dot(d, d))) * d);
+        const size_t pix = ((size_t)v * g.nv + iv) * g.nu + iu;
+        if (!transpose) {
+          double sum = 0.0;
+          joseph_weights(g, so, eo, [&](double w, long ix, long iy, long iz) { sum += w * V.at(ix, iy, iz); });
+          proj[pix] = sum;
+        } else {
+          const double yi = y_in[pix];
+          joseph_weights(g, so, eo, [&](double w, long ix, long iy, long iz) {
+            vol_out[((size_t)iz * g.ny + iy) * g.nx + ix] += w * yi;
+          });
+        }
+      }
+    }
+  }
+}
+
+// Pose gradient with Joseph weights and per-voxel G_f^j (as O12): A_i = sum_j a^ij g_j, B_i = sum_j a^ij r'_j x g_j.
+template <typename T>
+void forward_grad_joseph_impl(const ora_geom& g, int n_views, const double* angles, const double* poses, const T* vol,
+                              const float* upstream, double* grad) {
+  Vol<T> V{vol, g.nx, g.ny, g.nz};
+  for (int v = 0; v < n_views; ++v) {
+    View view(g, angles[v]);
+    Pose pose(poses + 6 * v);
+    const V3 so = mulT(pose.R, view.s - pose.t);
+    std::vector<double> rowacc((size_t)g.nv * 6, 0.0);
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int iv = 0; iv < g.nv; ++iv) {
+      double acc[6] = {0};
+      for (int iu = 0; iu < g.nu; ++iu) {
+        const double w = (double)upstream[((size_t)v * g.nv + iv) * g.nu + iu];
+        V3 d = view.pixel(g, iu, iv) - view.s;
+        V3 eo = mulT(pose.R, (1.0 / sqrt(dot(d, d))) * d);
+        V3 A = {0, 0, 0}, B = {0, 0, 0};
+        joseph_weights(g, so, eo, [&](double a, long X, long Y, long Z) {
+          V3 gj = {(V.at(X + 1, Y, Z) - V.at(X - 1, Y, Z)) / (2 * g.vx),
+                   (V.at(X, Y + 1, Z) - V.at(X, Y - 1, Z)) / (2 * g.vy),
+                   (V.at(X, Y, Z + 1) - V.at(X, Y, Z - 1)) / (2 * g.vz)};
+          V3 rj = voxel_centre(g, (int)X, (int)Y, (int)Z);
+          A = A + a * gj;
+          B = B + a * cross(rj, gj);
+        });
+        acc[0] += w * A.x; acc[1] += w * A.y; acc[2] += w * A.z;
+        acc[3] += w * B.x; acc[4] += w * B.y; acc[5] += w * B.z;
+      }
+      for (int q = 0; q < 6; ++q) rowacc[(size_t)iv * 6 + q] = acc[q];
+    }
+    double tot[6] = {0};
+    for (int iv = 0; iv < g.nv; ++iv) for (int q = 0; q < 6; ++q) tot[q] += rowacc[(size_t)iv * 6 + q];
+    V3 SA = {tot[0], tot[1], tot[2]}, SB = {tot[3], tot[4], tot[5]};
+    V3 dt = mul(pose.R, SA);
+    double* out = grad + 6 * v;
+    out[0] = -dt.x; out[1] = -dt.y; out[2] = -dt.z;
+    const double* th = poses + 6 * v;
+    V3 wx = {1, 0, 0};
+    V3 wy = mulT(Rx(th[3]), V3{0, 1, 0});
+    V3 wz = mulT(mul(Ry(th[4]), Rx(th[3])), V3{0, 0, 1});
+    out[3] = -dot(wx, SB); out[4] = -dot(wy, SB); out[5] = -dot(wz, SB);
+  }
+}
+
 extern "C" {
 
 int ora_num_threads() {
@@ -780,6 +897,28 @@ void ora_forward_pose_grad_siddon_f32(const ora_geom* g, int n_views, const doub
 void ora_forward_pose_grad_siddon_f64(const ora_geom* g, int n_views, const double* angles, const double* poses,
                                       const double* vol, const float* upstream, double* grad, int route) {
   forward_grad_siddon_impl<double>(*g, n_views, angles, poses, vol, upstream, grad, route);
+}
+
+// O13: Joseph weights (forward, explicit transpose, pose gradient)
+void ora_forward_joseph_f32(const ora_geom* g, int n_views, const double* angles, const double* poses,
+                            const float* vol, double* proj) {
+  forward_joseph_impl<float>(*g, n_views, angles, poses, vol, proj, nullptr, nullptr);
+}
+void ora_forward_joseph_f64(const ora_geom* g, int n_views, const double* angles, const double* poses,
+                            const double* vol, double* proj) {
+  forward_joseph_impl<double>(*g, n_views, angles, poses, vol, proj, nullptr, nullptr);
+}
+void ora_forward_joseph_T(const ora_geom* g, int n_views, const double* angles, const double* poses, const double* y,
+                          double* vol_out) {
+  forward_joseph_impl<double>(*g, n_views, angles, poses, (const double*)nullptr, nullptr, y, vol_out);
+}
+void ora_forward_pose_grad_joseph_f32(const ora_geom* g, int n_views, const double* angles, const double* poses,
+                                      const float* vol, const float* upstream, double* grad) {
+  forward_grad_joseph_impl<float>(*g, n_views, angles, poses, vol, upstream, grad);
+}
+void ora_forward_pose_grad_joseph_f64(const ora_geom* g, int n_views, const double* angles, const double* poses,
+                                      const double* vol, const float* upstream, double* grad) {
+  forward_grad_joseph_impl<double>(*g, n_views, angles, poses, vol, upstream, grad);
 }
 
 }  // extern "C"
