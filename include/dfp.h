@@ -61,6 +61,10 @@ typedef struct dfp_geometry {
                            Eq.19 :181, :189) instead of the default fixed-step trilinear ray-march; step_mm is then
                            unused.  Not combinable with DFP_FLAG_GRAD_INTERP or dfp_forward_fused_moments
                            (DFP_ERR_DIMS).  The back-projection calls ignore it;
+                           bit5 (DFP_FLAG_JOSEPH): as bit3 with JOSEPH weights - the ray is stepped from voxel-centre
+                           plane to voxel-centre plane along its driving axis (largest direction component), bilinear
+                           interpolation in each plane, path length v_a/|e_a| per plane; same restrictions; not
+                           together with DFP_FLAG_SIDDON;
                            bit4 (DFP_FLAG_ACCUMULATE): dfp_backproject ADDS the views' contribution to d_vol instead of
                            overwriting it, so that the sum over views (Eq.21) can be taken slice by slice of the view
                            arrays (view chunking; a view-sharded multi-GPU reconstruction).  Other calls ignore it. */
@@ -78,7 +82,7 @@ enum {
 enum { DFP_OP_FORWARD = 0, DFP_OP_FORWARD_POSE_GRAD = 1, DFP_OP_BACKPROJECT = 2, DFP_OP_BACKPROJECT_POSE_GRAD = 3,
        DFP_OP_FORWARD_FUSED = 4 };
 enum { DFP_FLAG_DW = 1, DFP_FLAG_NO_TMA = 2, DFP_FLAG_GRAD_INTERP = 4, DFP_FLAG_SIDDON = 8,
-       DFP_FLAG_ACCUMULATE = 16 };
+       DFP_FLAG_ACCUMULATE = 16, DFP_FLAG_JOSEPH = 32 };
 
 /* Forward projection, Eq.2a :67-69 discretised as Eq.18 :172-177 with a fixed-step, zero-extended
  * trilinear ray-march (U1): proj[v][iv][iu] = D * sum_k f~(R_v^T (s_v + (k+1/2) D e_i - t_v)).

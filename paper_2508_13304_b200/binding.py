@@ -19,6 +19,7 @@ FLAG_NO_TMA = 2
 FLAG_GRAD_INTERP = 4
 FLAG_SIDDON = 8
 FLAG_ACCUMULATE = 16
+FLAG_JOSEPH = 32
 PATH_GATHER, PATH_TMA = 0, 1
 
 

@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdfp.so")
 SOURCES = [os.path.join(CSRC, "dfp_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("dfp_kernels.cuh", "dfp_fwd_tma.cuh", "dfp_bp_tma.cuh", "dfp_siddon.cuh", "dfp_params.h")] + \
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("dfp_kernels.cuh", "dfp_fwd_tma.cuh", "dfp_bp_tma.cuh", "dfp_siddon.cuh", "dfp_joseph.cuh", "dfp_params.h")] + \
     [os.path.join(os.path.dirname(HERE), "include", "dfp.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]

@@ -14,6 +14,7 @@
 #include "dfp_fwd_tma.cuh"
 #include "dfp_kernels.cuh"
 #include "dfp_params.h"
+#include "dfp_joseph.cuh"
 #include "dfp_siddon.cuh"
 
 namespace {
@@ -317,8 +318,9 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
   const bool grad = op != DFP_OP_FORWARD, fused = op == DFP_OP_FORWARD_FUSED;
   if (fused && (!d_proj || !aligned(d_proj, 16))) return d_proj ? DFP_ERR_ALIGN : DFP_ERR_NULL;
   if (fused && (g->flags & DFP_FLAG_GRAD_INTERP)) return DFP_ERR_DIMS;      // fused moments: central differences only
-  const bool siddon = (g->flags & DFP_FLAG_SIDDON) != 0;
-  if (siddon && (fused || (g->flags & DFP_FLAG_GRAD_INTERP))) return DFP_ERR_DIMS;   // Siddon: the two plain calls only
+  const bool siddon = (g->flags & DFP_FLAG_SIDDON) != 0, joseph = (g->flags & DFP_FLAG_JOSEPH) != 0;
+  // Siddon / Joseph weights: the two plain calls only, one model at a time
+  if ((siddon || joseph) && (fused || (g->flags & DFP_FLAG_GRAD_INTERP) || (siddon && joseph))) return DFP_ERR_DIMS;
   const int nset = fused ? 3 : 1;
   const FwdWs w = fwd_ws(*g, V, grad, nset);
   st = check_common(g, V, angles, poses, d_vol, d_out, grad ? (const void*)d_up : (const void*)d_vol, d_ws,
@@ -338,20 +340,22 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
   DFP_CUDA(cudaMemcpyAsync(dv, hv.data(), sizeof(FwdView) * V, cudaMemcpyHostToDevice, s), "view upload");
   if (grad) DFP_CUDA(cudaMemcpyAsync(dc, hc.data(), sizeof(FwdContract) * V, cudaMemcpyHostToDevice, s), "view upload");
   const dim3 grid(w.gx, w.gy, V);
-  if (siddon) {   // Siddon weights (dfp_siddon.cuh): DDA straight over the caller's volume
+  if (siddon || joseph) {   // other weight models (dfp_siddon.cuh, dfp_joseph.cuh): straight over the caller's volume
     g_path = DFP_PATH_GATHER;
     time_begin(s);
     if (!grad) {
-      siddon_fwd_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, d_vol, d_out);
+      if (siddon) siddon_fwd_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, d_vol, d_out);
+      else joseph_fwd_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, d_vol, d_out);
       time_end(s);
       ++g_launches;
     } else {
-      siddon_grad_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, d_vol, d_up, part);
+      if (siddon) siddon_grad_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, d_vol, d_up, part);
+      else joseph_grad_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, d_vol, d_up, part);
       time_end(s);
       fwd_contract_kernel<<<V, 256, 0, s>>>(w.gx * w.gy, part, dc, d_out);
       g_launches += 2;
     }
-    DFP_CUDA(cudaGetLastError(), "forward launch (Siddon)");
+    DFP_CUDA(cudaGetLastError(), "forward launch (Siddon / Joseph weights)");
     return DFP_OK;
   }
   // TMA-staged path when the volume admits a tensor map and every view's tiles fit a staging box: the smallest

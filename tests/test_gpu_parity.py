@@ -594,3 +594,52 @@ def test_backproject_accumulate_flag_sums_view_slices(dfp):
         dfp.backproject(ga, a[4:], p[4:], proj[4:].contiguous(), out=vol)
         assert rel_l2(vol.cpu().numpy(), whole) <= 1e-6
         assert rel_l2(first, whole) > 0.1                      # the first slice alone is not the answer
+
+
+# ------------------------------------------------------------------ DFP_FLAG_JOSEPH
+def run_joseph_case(dfp, g, angles, poses, vol, up):
+    dev = torch.device("cuda:0")
+    gj = g.replace(flags=g.flags | dfp.FLAG_JOSEPH)
+    angles, poses = f32(angles), f32(poses).reshape(-1, 6)
+    vol_d = torch.as_tensor(vol, dtype=torch.float32, device=dev).contiguous()
+    up_d = torch.as_tensor(up, dtype=torch.float32, device=dev).contiguous()
+    proj = dfp.forward(gj, angles, poses, vol_d).cpu().numpy()
+    grad = dfp.forward_pose_grad(gj, angles, poses, vol_d, up_d).cpu().numpy()
+    o_proj = oracle.forward_joseph(g, angles, poses, vol_d.cpu().numpy())
+    o_grad = oracle.forward_pose_grad_joseph(g, angles, poses, vol_d.cpu().numpy(), up_d.cpu().numpy())
+    return proj, grad, o_proj, o_grad
+
+
+def test_joseph_ragged_anisotropic_all_driving_axes_and_degenerate(dfp):
+    g = aniso_geom(nx=37, ny=29, nz=23, nu=45, nv=21)
+    rng = np.random.default_rng(40)
+    vol = rng.random(g.vol_shape).astype(np.float32)
+    up = rng.standard_normal((4,) + g.det_shape).astype(np.float32)
+    # views driven along x, along y, and (tilted by 70 degrees about y) along z
+    angles = [0.4, math.pi / 2, 4.1, 0.1]
+    poses = POSES3 + [[0.5, 0.3, 0.2, 0.05, 1.2, 0.0]]
+    check_forward(run_joseph_case(dfp, g, angles, poses, vol, up))
+    g = small_geom(n=12, nu=11, nv=9)                        # axis-parallel central ray
+    vol = rng.random(g.vol_shape).astype(np.float32)
+    up = rng.standard_normal((1,) + g.det_shape).astype(np.float32)
+    check_forward(run_joseph_case(dfp, g, [0.0], [[0] * 6], vol, up))
+    proj, grad, _, _ = run_joseph_case(dfp, g, [0.3], [[0, 0, 700.0, 0, 0, 0]], vol, up)
+    assert np.all(proj == 0) and np.all(grad == 0)
+    g1 = small_geom(n=1, voxel=4.0, nu=3, nv=3, pix=1.0)
+    check_forward(run_joseph_case(dfp, g1, [0.2], [[0.3, 0.2, -0.1, 0.01, 0.02, 0.03]], np.full(g1.vol_shape, 0.7, np.float32),
+                                  np.ones((1,) + g1.det_shape, np.float32)))
+
+
+@pytest.mark.parametrize("index,scale,views", [(1, 1.0, None), (2, 0.25, 3), (4, 0.125, 4), (5, 0.125, 3)])
+def test_joseph_configs_reduced(dfp, index, scale, views):
+    w = W.make_config(index, scale=scale, n_views=views)
+    check_forward(run_joseph_case(dfp, w.geom, w.angles.numpy(), w.poses.numpy(), w.volume().numpy(),
+                                  w.fwd_upstream().numpy()))
+
+
+def test_joseph_and_siddon_flags_exclude_each_other(dfp):
+    w = W.make_config(1)
+    dev = torch.device("cuda:0")
+    a, p = f32(w.angles.numpy()), f32(w.poses.numpy()).reshape(-1, 6)
+    with pytest.raises(dfp.DfpError):
+        dfp.forward(w.geom.replace(flags=dfp.FLAG_SIDDON | dfp.FLAG_JOSEPH), a, p, w.volume(dev))
