@@ -286,19 +286,21 @@ def main():
         b_.record()
         torch.cuda.synchronize()
         interp_ms.append(a_.elapsed_time(b_) / 3)
-    # DFP_FLAG_SIDDON variants of the two forward calls
-    gsd = g.replace(flags=g.flags | dfp.FLAG_SIDDON)
-    siddon_ms = []
-    for fn in (lambda: dfp.forward(gsd, angles, poses, vol, out=proj, ws=ws),
-               lambda: dfp.forward_pose_grad(gsd, angles, poses, vol, up, out=grad, ws=ws)):
-        fn()
-        a_, b_ = ev(), ev()
-        a_.record()
-        for _ in range(3):
+    # DFP_FLAG_SIDDON / DFP_FLAG_JOSEPH variants of the two forward calls
+    model_ms = {}
+    for name, flag in (("siddon", dfp.FLAG_SIDDON), ("joseph", dfp.FLAG_JOSEPH)):
+        gm = g.replace(flags=g.flags | flag)
+        model_ms[name] = []
+        for fn in (lambda: dfp.forward(gm, angles, poses, vol, out=proj, ws=ws),
+                   lambda: dfp.forward_pose_grad(gm, angles, poses, vol, up, out=grad, ws=ws)):
             fn()
-        b_.record()
-        torch.cuda.synchronize()
-        siddon_ms.append(a_.elapsed_time(b_) / 3)
+            a_, b_ = ev(), ev()
+            a_.record()
+            for _ in range(3):
+                fn()
+            b_.record()
+            torch.cuda.synchronize()
+            model_ms[name].append(a_.elapsed_time(b_) / 3)
     dfp.forward(g, angles, poses, vol, out=proj, ws=ws)                        # restore the default-mode projections
     # dfp_forward_fused_moments: projection + gradient moments in one traversal (target = the upstream array's shape)
     ws_f = torch.empty(dfp.workspace_bytes(g, V, dfp.OP_FORWARD_FUSED), dtype=torch.uint8, device=dev)
@@ -415,7 +417,10 @@ def main():
                                      "backproject_pose_grad": float(seg[:, 3].mean())},
                      "grad_interp_mode_ms_per_call": {"forward_pose_grad": interp_ms[0],
                                                       "backproject_pose_grad": interp_ms[1]},
-                     "siddon_mode_ms_per_call": {"forward": siddon_ms[0], "forward_pose_grad": siddon_ms[1]},
+                     "siddon_mode_ms_per_call": {"forward": model_ms["siddon"][0],
+                                                 "forward_pose_grad": model_ms["siddon"][1]},
+                     "joseph_mode_ms_per_call": {"forward": model_ms["joseph"][0],
+                                                 "forward_pose_grad": model_ms["joseph"][1]},
                      "forward_fused_moments_ms_per_call": fused_ms,
                      "forward_fused_moments_gray_steps_per_s": 2.0 * ray_steps / (fused_ms * 1e-3) / 1e9},
            "clocks": clocks, "e2e": e2e, "gpu_launches": n_launch, "roofline": roofline, "cpu_baseline": cpu}

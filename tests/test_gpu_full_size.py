@@ -144,11 +144,15 @@ def test_c2_registration_full_grad_interp_mode(dfp):
         assert e.max() <= 3 * TOL_GRAD and np.sort(e.ravel())[-2] <= TOL_GRAD, (v, e)
 
 
-def test_c2_registration_full_siddon(dfp):
-    """DFP_FLAG_SIDDON at the bench's size: a row band of two seeded views and one view's 6-vector vs the oracle."""
+@pytest.mark.parametrize("model", ["siddon", "joseph"])
+def test_c2_registration_full_other_weight_models(dfp, model):
+    """DFP_FLAG_SIDDON / DFP_FLAG_JOSEPH at the bench's size: a row band of two seeded views and one view's 6-vector
+    vs the oracle."""
     dev = torch.device("cuda:0")
     w = W.make_config(2)
-    g = w.geom.replace(flags=dfp.FLAG_SIDDON)
+    g = w.geom.replace(flags=dfp.FLAG_SIDDON if model == "siddon" else dfp.FLAG_JOSEPH)
+    o_fwd = oracle.forward_siddon if model == "siddon" else oracle.forward_joseph
+    o_grad = oracle.forward_pose_grad_siddon if model == "siddon" else oracle.forward_pose_grad_joseph
     a = w.angles.float().numpy()
     p = w.poses.float().numpy()
     vol = w.volume(dev)
@@ -160,8 +164,8 @@ def test_c2_registration_full_siddon(dfp):
     views = pick(w.seed + 601, w.n_views, 2)
     for v in views:
         r0 = pick(w.seed + 611 + v, w.geom.nv - 32 + 1, 1)[0]
-        o = oracle.forward_siddon(row_band(w.geom, r0, 32), a[v:v + 1], p[v:v + 1], vol_c)[0]
+        o = o_fwd(row_band(w.geom, r0, 32), a[v:v + 1], p[v:v + 1], vol_c)[0]
         assert rel_l2(proj[v, r0:r0 + 32].cpu().numpy(), o) <= TOL_VAL
     v = views[0]
-    o = oracle.forward_pose_grad_siddon(w.geom, a[v:v + 1], p[v:v + 1], vol_c, up[v:v + 1].cpu().numpy())
+    o = o_grad(w.geom, a[v:v + 1], p[v:v + 1], vol_c, up[v:v + 1].cpu().numpy())
     assert grad_err_u9(grad[v:v + 1], o).max() <= TOL_GRAD
