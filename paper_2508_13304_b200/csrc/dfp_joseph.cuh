@@ -100,29 +100,39 @@ __device__ __forceinline__ void joseph_march(const FwdGeom& G, const JosephRay& 
       const float v01 = jload(vol, base + S[D], okb0 && okd1), v11 = jload(vol, base + S[B] + S[D], okb1 && okd1);
       sum += wd0 * (wb0 * v00 + wb1 * v10) + wd1 * (wb0 * v01 + wb1 * v11);
     } else {
+      // the in-plane 4 x 4 neighbourhood without its corners (12 voxels) and the 2 x 2 block in planes k-1, k+1
+      // (8 voxels), each loaded once; zero extension by predicate
+      const bool okbm = (unsigned)(ib - 1) < (unsigned)n[B], okb2 = (unsigned)(ib + 2) < (unsigned)n[B];
+      const bool okdm = (unsigned)(id - 1) < (unsigned)n[D], okd2 = (unsigned)(id + 2) < (unsigned)n[D];
+      const bool okam = k > 0, okap = k + 1 < n[A];
+      const bool okb[4] = {okbm, okb0, okb1, okb2}, okd[4] = {okdm, okd0, okd1, okd2};
+      float P[4][4];                                   // P[jd+1][jb+1] = voxel (ib+jb, id+jd), jb, jd in -1..2
+#pragma unroll
+      for (int jd = 0; jd < 4; ++jd)
+#pragma unroll
+        for (int jb = 0; jb < 4; ++jb) {
+          const bool corner = (jd == 0 || jd == 3) && (jb == 0 || jb == 3);
+          P[jd][jb] = corner ? 0.f : jload(vol, base + (jb - 1) * S[B] + (jd - 1) * S[D], okb[jb] && okd[jd]);
+        }
 #pragma unroll
       for (int jd = 0; jd < 2; ++jd)
 #pragma unroll
         for (int jb = 0; jb < 2; ++jb) {
-          const bool ok = (jb ? okb1 : okb0) && (jd ? okd1 : okd0);
-          const float w = (jb ? wb1 : wb0) * (jd ? wd1 : wd0);
-          if (ok && w != 0.f) {                                   // grid voxels only (O13)
-            const int ia = k, jb_i = ib + jb, jd_i = id + jd;
-            const long long o = base + jb * S[B] + jd * S[D];
-            // central differences of the zero-extended voxel values along A, B, D (times 2 v)
-            const float ga = jload(vol, o + S[A], ia + 1 < n[A]) - jload(vol, o - S[A], ia > 0);
-            const float gb = jload(vol, o + S[B], jb_i + 1 < n[B]) - jload(vol, o - S[B], jb_i > 0);
-            const float gd = jload(vol, o + S[D], jd_i + 1 < n[D]) - jload(vol, o - S[D], jd_i > 0);
-            float g3[3], r3[3];
-            g3[A] = w * ga * sg[A]; g3[B] = w * gb * sg[B]; g3[D] = w * gd * sg[D];
-            r3[A] = fmaf((float)ia - ha, vv[A], cc[A]);
-            r3[B] = fmaf((float)jb_i - hb, vv[B], cc[B]);
-            r3[D] = fmaf((float)jd_i - hd, vv[D], cc[D]);
-            a0 += g3[0]; a1 += g3[1]; a2 += g3[2];
-            b0 += r3[1] * g3[2] - r3[2] * g3[1];
-            b1 += r3[2] * g3[0] - r3[0] * g3[2];
-            b2 += r3[0] * g3[1] - r3[1] * g3[0];
-          }
+          const bool ok = okb[jb + 1] && okd[jd + 1];
+          const float w = ok ? (jb ? wb1 : wb0) * (jd ? wd1 : wd0) : 0.f;       // grid voxels only (O13)
+          const long long o = base + jb * S[B] + jd * S[D];
+          const float ga = jload(vol, o + S[A], ok && okap) - jload(vol, o - S[A], ok && okam);
+          const float gb = P[jd + 1][jb + 2] - P[jd + 1][jb];
+          const float gd = P[jd + 2][jb + 1] - P[jd][jb + 1];
+          float g3[3], r3[3];
+          g3[A] = w * ga * sg[A]; g3[B] = w * gb * sg[B]; g3[D] = w * gd * sg[D];
+          r3[A] = fmaf(kf - ha, vv[A], cc[A]);
+          r3[B] = fmaf((float)(ib + jb) - hb, vv[B], cc[B]);
+          r3[D] = fmaf((float)(id + jd) - hd, vv[D], cc[D]);
+          a0 += g3[0]; a1 += g3[1]; a2 += g3[2];
+          b0 += r3[1] * g3[2] - r3[2] * g3[1];
+          b1 += r3[2] * g3[0] - r3[0] * g3[2];
+          b2 += r3[0] * g3[1] - r3[1] * g3[0];
         }
     }
   }
