@@ -457,28 +457,33 @@ def test_random_geometries_both_paths_agree_and_never_nan(dfp):
         vol = torch.as_tensor(rng.random(g.vol_shape).astype(np.float32), device=dev)
         up = torch.as_tensor(rng.standard_normal((V,) + g.det_shape).astype(np.float32), device=dev)
         bup = torch.as_tensor(rng.standard_normal(g.vol_shape).astype(np.float32), device=dev)
+        # back-projection input: seeded smooth images (no oracle input ever comes from the CUDA path)
+        iv_, iu_ = np.meshgrid(np.arange(g.nv), np.arange(g.nu), indexing="ij")
+        pin_np = np.stack([np.sin(0.21 * iu_ + 0.13 * iv_ + k) + 0.5 * np.cos(0.07 * iu_ - 0.19 * iv_ + 2 * k)
+                           for k in range(V)]).astype(np.float32)
+        pin = torch.as_tensor(pin_np, device=dev)
         gn = g.replace(flags=dfp.FLAG_NO_TMA)
         proj = dfp.forward(g, angles, poses, vol)
         n_tma += dfp.last_path()
         grad = dfp.forward_pose_grad(g, angles, poses, vol, up)
         n_tma += dfp.last_path()
-        bp = dfp.backproject(g, angles, poses, proj)
+        bp = dfp.backproject(g, angles, poses, pin)
         n_tma += dfp.last_path()
-        bgrad = dfp.backproject_pose_grad(g, angles, poses, proj, bup)
+        bgrad = dfp.backproject_pose_grad(g, angles, poses, pin, bup)
         n_tma += dfp.last_path()
         for t in (proj, grad, bp, bgrad):
             assert torch.isfinite(t).all(), (case, g)
         assert rel_l2(proj.cpu().numpy(), dfp.forward(gn, angles, poses, vol).cpu().numpy()) <= 2e-6, case
         assert grad_err_u9(grad.cpu().numpy(),
                            dfp.forward_pose_grad(gn, angles, poses, vol, up).cpu().numpy()).max() <= 1e-4, case
-        assert rel_l2(bp.cpu().numpy(), dfp.backproject(gn, angles, poses, proj).cpu().numpy()) <= 5e-6, case
+        assert rel_l2(bp.cpu().numpy(), dfp.backproject(gn, angles, poses, pin).cpu().numpy()) <= 5e-6, case
         assert grad_err_u9(bgrad.cpu().numpy(),
-                           dfp.backproject_pose_grad(gn, angles, poses, proj, bup).cpu().numpy()).max() <= 1e-4, case
+                           dfp.backproject_pose_grad(gn, angles, poses, pin, bup).cpu().numpy()).max() <= 1e-4, case
         if case % 3 == 0:
             check_forward((proj.cpu().numpy(), grad.cpu().numpy(), oracle.forward(g, angles, poses, vol.cpu().numpy()),
                            oracle.forward_pose_grad(g, angles, poses, vol.cpu().numpy(), up.cpu().numpy())))
-            check_back((bp.cpu().numpy(), bgrad.cpu().numpy(), oracle.backproject(g, angles, poses, proj.cpu().numpy()),
-                        oracle.backproject_pose_grad(g, angles, poses, proj.cpu().numpy(), bup.cpu().numpy())))
+            check_back((bp.cpu().numpy(), bgrad.cpu().numpy(), oracle.backproject(g, angles, poses, pin_np),
+                        oracle.backproject_pose_grad(g, angles, poses, pin_np, bup.cpu().numpy())))
     assert 40 <= n_tma <= 150, n_tma      # a healthy mix of TMA and fallback calls (4 calls per case)
 
 
@@ -571,7 +576,8 @@ def test_tma_paths_axis_aligned_views_and_other_step_sizes(dfp):
         res = run_forward_case(dfp, g, angles, zero, vol, up)
         assert dfp.last_path() == dfp.PATH_TMA
         check_forward(res)
-    proj = res[0]
+    w.angles = torch.tensor(angles, dtype=torch.float64)        # closed-form projections at these four views
+    proj = w.projections().numpy()
     bup = np.random.default_rng(31).standard_normal(w.geom.vol_shape).astype(np.float32)
     resb = run_back_case(dfp, w.geom, angles, zero, proj, bup)
     assert dfp.last_path() == dfp.PATH_TMA
