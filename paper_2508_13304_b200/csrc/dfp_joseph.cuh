@@ -181,28 +181,7 @@ __global__ void __launch_bounds__(kFwdThreads) joseph_grad_kernel(FwdGeom G, con
 #pragma unroll
     for (int q = 0; q < 6; ++q) out[q] *= w;
   }
-  __shared__ float red[kFwdThreads / 32][6];
-#pragma unroll
-  for (int q = 0; q < 6; ++q) {
-    float v = out[q];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    out[q] = v;
-  }
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  if (lane == 0) {
-#pragma unroll
-    for (int q = 0; q < 6; ++q) red[warp][q] = out[q];
-  }
-  __syncthreads();
-  if (threadIdx.x < 6) {
-    float s = 0.f;
-#pragma unroll
-    for (int wI = 0; wI < kFwdThreads / 32; ++wI) s += red[wI][threadIdx.x];
-    const size_t blk = (size_t)blockIdx.y * gridDim.x + blockIdx.x;
-    const size_t nblk = (size_t)gridDim.x * gridDim.y;
-    partials[((size_t)view * nblk + blk) * 6 + threadIdx.x] = s;
-  }
+  reduce6_to_partials<kFwdThreads>(out, partials, view);
 }
 
 }  // namespace dfp

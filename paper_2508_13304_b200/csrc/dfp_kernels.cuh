@@ -190,6 +190,34 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_project_kernel(FwdGeom G, con
   proj[((size_t)view * G.nv + iv) * G.nu + iu] = G.step * sum;
 }
 
+// a5, first stage, shared by the gradient kernels that keep one 6-vector per ray: warp shuffle, then across the
+// block's warps through shared memory in fixed order -> partials[view][block][6] (deterministic, no atomics).
+template <int NTHREADS>
+__device__ __forceinline__ void reduce6_to_partials(float (&out)[6], float* __restrict__ partials, int view) {
+  __shared__ float red[NTHREADS / 32][6];
+#pragma unroll
+  for (int q = 0; q < 6; ++q) {
+    float v = out[q];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    out[q] = v;
+  }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (lane == 0) {
+#pragma unroll
+    for (int q = 0; q < 6; ++q) red[warp][q] = out[q];
+  }
+  __syncthreads();
+  if (threadIdx.x < 6) {
+    float s = 0.f;
+#pragma unroll
+    for (int wI = 0; wI < NTHREADS / 32; ++wI) s += red[wI][threadIdx.x];
+    const size_t blk = (size_t)blockIdx.y * gridDim.x + blockIdx.x;
+    const size_t nblk = (size_t)gridDim.x * gridDim.y;
+    partials[((size_t)view * nblk + blk) * 6 + threadIdx.x] = s;
+  }
+}
+
 // ------------------------------------------------------------------------------------------------ a4 gradient
 // Per ray (Eq.7-8 :101-113, Eq.19 :179-183, on the fly per :207):
 //   A_i = D sum_k g~(r'_k),  B_i = D sum_k r'_k x g~(r'_k),  g~_a = [f~(r'+v_a e_a) - f~(r'-v_a e_a)] / (2 v_a).
@@ -283,29 +311,7 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_grad_kernel(FwdGeom G, const 
     out[4] = wd * ((pz * sx - px * sz) + (ez * mx - ex * mz));
     out[5] = wd * ((px * sy - py * sx) + (ex * my - ey * mx));
   }
-  // a5, first stage: warp shuffle, then across the block's warps through shared memory (fixed order)
-  __shared__ float red[kFwdThreads / 32][6];
-#pragma unroll
-  for (int q = 0; q < 6; ++q) {
-    float v = out[q];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    out[q] = v;
-  }
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  if (lane == 0) {
-#pragma unroll
-    for (int q = 0; q < 6; ++q) red[warp][q] = out[q];
-  }
-  __syncthreads();
-  if (threadIdx.x < 6) {
-    float s = 0.f;
-#pragma unroll
-    for (int wI = 0; wI < kFwdThreads / 32; ++wI) s += red[wI][threadIdx.x];
-    const size_t blk = (size_t)blockIdx.y * gridDim.x + blockIdx.x;
-    const size_t nblk = (size_t)gridDim.x * gridDim.y;
-    partials[((size_t)view * nblk + blk) * 6 + threadIdx.x] = s;
-  }
+  reduce6_to_partials<kFwdThreads>(out, partials, view);
 }
 
 // a5, second stage: one block per view, fp64, fixed summation order (deterministic), then the 6x6 contraction
