@@ -169,3 +169,33 @@ def test_c2_registration_full_other_weight_models(dfp, model):
     v = views[0]
     o = o_grad(w.geom, a[v:v + 1], p[v:v + 1], vol_c, up[v:v + 1].cpu().numpy())
     assert grad_err_u9(grad[v:v + 1], o).max() <= TOL_GRAD
+
+
+def test_volume_1024_cubed_indices_and_sizes(dfp):
+    """Beyond the configs: a 1024^3 volume (4 GiB) with 2048x2048 views (config 5 at twice the resolution, 4 views) -
+    32-bit index arithmetic, tensor-map extents and tile counts at the upper end.  Row bands / one slab vs the oracle."""
+    dev = torch.device("cuda:0")
+    w = W.make_config(5, scale=2.0, n_views=4)
+    g = w.geom
+    assert (g.nx, g.nu) == (1024, 2048)
+    a = w.angles.float().numpy()
+    p = w.poses.float().numpy()
+    vol = w.volume(dev)
+    vol_c = vol.cpu().numpy()
+    v, r0, rows = 2, 1000, 4
+    for flags, fwd in ((0, oracle.forward), (dfp.FLAG_SIDDON, oracle.forward_siddon)):
+        proj = dfp.forward(g.replace(flags=flags), a, p, vol)
+        assert torch.isfinite(proj).all()
+        o = fwd(row_band(g, r0, rows), a[v:v + 1], p[v:v + 1], vol_c)[0]
+        assert rel_l2(proj[v, r0:r0 + rows].cpu().numpy(), o) <= TOL_VAL
+        del proj
+    up = w.fwd_upstream(dev)
+    grad = dfp.forward_pose_grad(g, a, p, vol, up).cpu().numpy()
+    assert dfp.last_path() == dfp.PATH_TMA and np.isfinite(grad).all()
+    del vol, up
+    torch.cuda.empty_cache()
+    pin = w.projections(dev)
+    bp = dfp.backproject(g, a, p, pin)
+    assert dfp.last_path() == dfp.PATH_TMA
+    o = oracle.backproject(g, a, p, pin.cpu().numpy(), 777, 778)
+    assert rel_l2(bp[777:778].cpu().numpy(), o) <= TOL_VAL
