@@ -150,9 +150,10 @@ int dfp_backproject_pose_grad_host(const dfp_geometry* geometry, int n_views, co
                                    const float* poses, const float* h_proj, const float* h_dLdvol, float* h_grad,
                                    void* stream);
 
-/* Number of ray-steps one dfp_forward / dfp_forward_pose_grad call marches (samples inside the clip box,
- * summed over rays and views), computed on the host in fp64 from the geometry alone; the unit of the
- * "Gray-steps/s" metric.  Returns -1 on invalid arguments. */
+/* Number of ray-steps one dfp_forward / dfp_forward_pose_grad call marches in the default (trilinear) mode: samples
+ * inside the gradient's clip box, summed over rays and views; the unit of the "Gray-steps/s" metric.  Counted by a small
+ * kernel that runs the same per-ray clip (fp64) as the projectors, on the default stream, synchronously; allocates
+ * and frees its own scratch.  Returns -1 on invalid arguments or CUDA failure. */
 int64_t dfp_count_ray_steps(const dfp_geometry* geometry, int n_views, const float* angles, const float* poses);
 
 /* Kernel timing for roofline accounting.  dfp_set_kernel_timing(1) makes every later device-pointer call on
