@@ -8,9 +8,9 @@
 // then the same per-view reduction / contraction as the trilinear kernels (dL/dt = -R S_A, dL/dgamma_k = -w_k.S_B).
 //
 // One thread per ray, incremental 3-D DDA over the voxel grid (the merged plane-crossing list of Siddon's paper,
-// generated in order instead of sorted).  The crossing parameters run in fp64: they reach ~1000 mm while a segment
-// is ~1 voxel long, and a segment length is a DIFFERENCE of two of them (fp32 would leave 1e-4 relative error per
-// segment; fp64 adds and compares run at half the fp32 rate on B200).  Values are read straight from the caller's
+// generated in order instead of sorted).  Crossing PARAMETERS reach ~1000 mm while a segment is ~1 voxel long, so a
+// length taken as a difference of two fp32 parameters would carry 1e-4 relative error; the set-up therefore runs in
+// fp64 and the loop tracks only the (small) distances to the next crossings.  Values are read straight from the caller's
 // volume through L1 (one voxel per segment; the six neighbours for the gradient) - no packed copy, no staging: this
 // is a first, plain kernel for the "next" row, measured beside the trilinear ones in DESIGN.md.
 #pragma once
@@ -74,41 +74,43 @@ __device__ __forceinline__ SiddonRay siddon_setup(const FwdGeom& G, const FwdVie
 }
 
 // One DDA step: returns the length of the segment inside the current voxel, then advances index, linear offset and
-// the crossed family's next parameter.  `alive` turns false once the ray has left the grid (or reached tmax).
+// the crossed family's counter.  `alive` turns false once the ray has left the grid: the grid's faces are planes of
+// the three families, so the ray ends exactly at a crossing.
+// The state keeps, per family, the distance from the CURRENT point to the next crossing (fp32, at most one crossing
+// spacing, a few mm): a segment length is then the minimum of three small numbers, known to ~1e-7 relative, and
+// the subtraction r_a - len is exact or rounds at 1e-7 of a spacing - no fp64 and no large parameter in the loop
+// (the per-ray set-up, which does subtract parameters of ~1000 mm, runs in fp64).
 // Written with selects on named scalars (an array indexed by the crossed axis would live in local memory).
 struct SiddonState {
-  double t, tmax, tnx, tny, tnz, dtx, dty, dtz;
+  float rx, ry, rz, dtx, dty, dtz;       // distance to the next x / y / z plane; spacing of the crossings
   int ix, iy, iz, sx, sy, sz, idx;
 };
 __device__ __forceinline__ SiddonState siddon_state(const SiddonRay& r, int nx, int ny) {
   SiddonState s;
-  s.t = r.t; s.tmax = r.tmax;
-  s.tnx = r.tn[0]; s.tny = r.tn[1]; s.tnz = r.tn[2];
-  s.dtx = r.dt[0]; s.dty = r.dt[1]; s.dtz = r.dt[2];
+  s.rx = (float)fmin(r.tn[0] - r.t, 1e30); s.ry = (float)fmin(r.tn[1] - r.t, 1e30); s.rz = (float)fmin(r.tn[2] - r.t, 1e30);
+  s.dtx = (float)fmin(r.dt[0], 1e30); s.dty = (float)fmin(r.dt[1], 1e30); s.dtz = (float)fmin(r.dt[2], 1e30);
   s.ix = r.i[0]; s.iy = r.i[1]; s.iz = r.i[2];
   s.sx = r.step[0]; s.sy = r.step[1]; s.sz = r.step[2];
   s.idx = (s.iz * ny + s.iy) * nx + s.ix;
   return s;
 }
 __device__ __forceinline__ float siddon_step(SiddonState& s, int nx, int ny, int nz, bool& alive) {
-  const bool cx = s.tnx <= s.tny && s.tnx <= s.tnz;
-  const bool cy = !cx && s.tny <= s.tnz;
-  const double tcross = cx ? s.tnx : (cy ? s.tny : s.tnz);
-  const double tn = fmin(tcross, s.tmax);
-  const float len = (float)fmax(tn - s.t, 0.0);
-  s.t = tn;
+  const bool cx = s.rx <= s.ry && s.rx <= s.rz;
+  const bool cy = !cx && s.ry <= s.rz;
+  const float len = fmaxf(cx ? s.rx : (cy ? s.ry : s.rz), 0.f);
+  s.rx -= len; s.ry -= len; s.rz -= len;
   bool inside;
   if (cx) {
-    s.tnx += s.dtx; s.ix += s.sx; s.idx += s.sx;
+    s.rx = s.dtx; s.ix += s.sx; s.idx += s.sx;
     inside = (unsigned)s.ix < (unsigned)nx;
   } else if (cy) {
-    s.tny += s.dty; s.iy += s.sy; s.idx += s.sy * nx;
+    s.ry = s.dty; s.iy += s.sy; s.idx += s.sy * nx;
     inside = (unsigned)s.iy < (unsigned)ny;
   } else {
-    s.tnz += s.dtz; s.iz += s.sz; s.idx += s.sz * nx * ny;
+    s.rz = s.dtz; s.iz += s.sz; s.idx += s.sz * nx * ny;
     inside = (unsigned)s.iz < (unsigned)nz;
   }
-  alive = inside && s.t < s.tmax;
+  alive = inside;
   return len;
 }
 
