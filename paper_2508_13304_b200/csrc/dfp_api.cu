@@ -345,15 +345,23 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
     time_begin(s);
     if (!grad) {
       if (siddon) siddon_fwd_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, d_vol, d_out);
-      else joseph_fwd_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, d_vol, d_out);
+      else {
+        pack_volume_kernel<<<grid_1d((size_t)G.L.px * G.L.py * G.L.pz, 256), 256, 0, s>>>(G.L, d_vol, pvol);
+        joseph_fwd_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, pvol, d_out);
+        ++g_launches;
+      }
       time_end(s);
       ++g_launches;
     } else {
-      if (siddon) siddon_grad_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, d_vol, d_up, part);
-      else joseph_grad_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, d_vol, d_up, part);
+      // per-voxel g_j once per call, into the workspace region the packed volume of the trilinear path would take
+      const GradBricks B = GradBricks::make(g->nx, g->ny, g->nz);
+      const int gb = (int)std::min<size_t>((B.cells() + 255) / 256, (size_t)148 * 64);
+      grad_volume_kernel<<<gb, 256, 0, s>>>(B, G.sgx, G.sgy, G.sgz, d_vol, pvol);
+      if (siddon) siddon_grad_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, pvol, d_up, part);
+      else joseph_grad_kernel<<<grid, kFwdThreads, 0, s>>>(G, dv, pvol, d_up, part);
       time_end(s);
       fwd_contract_kernel<<<V, 256, 0, s>>>(w.gx * w.gy, part, dc, d_out);
-      g_launches += 2;
+      g_launches += 3;
     }
     DFP_CUDA(cudaGetLastError(), "forward launch (Siddon / Joseph weights)");
     return DFP_OK;

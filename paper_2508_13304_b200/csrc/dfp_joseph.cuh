@@ -9,9 +9,11 @@
 //   A_i = sum_j a^ij g_j,  B_i = sum_j a^ij r'_j x g_j   -> six running sums per ray, then the common reduction.
 //
 // One thread per ray; per-ray set-up in fp64 (driving axis, plane range with t > 0 and the bilinear support inside
-// reach, start and increment of the two in-plane coordinates), planes marched in fp32 on centred indices.  Values
-// are read straight from the caller's volume through L1 with bound predicates: a first, plain kernel for the
-// "next" row.  The body is instantiated per driving axis so that every index is static.
+// reach, start and increment of the two in-plane coordinates), planes marched in fp32 on centred indices.  The
+// forward kernel reads the packed quad cells of the trilinear gather path (one or two 16-byte reads per plane, zero
+// border instead of bound predicates); the gradient kernel reads g_j of the
+// four voxels from the per-voxel gradient volume (dfp_kernels.cuh: grad_volume_kernel), one float4 each.  Kernels
+// for the "next" row.  The body is instantiated per driving axis so that every index is static.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -71,19 +73,13 @@ __device__ __forceinline__ JosephRay joseph_setup(const FwdGeom& G, const FwdVie
   return r;
 }
 
-// voxel value with zero extension along the two in-plane axes (the driving-axis index is always in range)
-__device__ __forceinline__ float jload(const float* __restrict__ vol, long long off, bool ok) {
-  return ok ? __ldg(vol + off) : 0.f;
-}
-
 // A = driving axis; B = (A+1)%3, D = (A+2)%3.  GRAD = false: returns the projection in acc[0].
 template <int A, bool GRAD>
-__device__ __forceinline__ void joseph_march(const FwdGeom& G, const JosephRay& r, const float* __restrict__ vol,
-                                             float* acc) {
+__device__ __forceinline__ void joseph_march(const FwdGeom& G, const JosephRay& r, const float4* __restrict__ pvol,
+                                             const float4* __restrict__ gvol, float* acc) {
   constexpr int B = (A + 1) % 3, D = (A + 2) % 3;
   const int n[3] = {G.L.nx, G.L.ny, G.L.nz};
-  const long long S[3] = {1, G.L.nx, (long long)G.L.nx * G.L.ny};
-  const float vv[3] = {G.vx, G.vy, G.vz}, cc[3] = {G.cx, G.cy, G.cz}, sg[3] = {G.sgx, G.sgy, G.sgz};
+  const float vv[3] = {G.vx, G.vy, G.vz}, cc[3] = {G.cx, G.cy, G.cz};
   const float hb = 0.5f * (float)(n[B] - 1), hd = 0.5f * (float)(n[D] - 1), ha = 0.5f * (float)(n[A] - 1);
   float sum = 0.f, a0 = 0.f, a1 = 0.f, a2 = 0.f, b0 = 0.f, b1 = 0.f, b2 = 0.f;
   for (int k = r.k0; k <= r.k1; ++k) {
@@ -92,47 +88,51 @@ __device__ __forceinline__ void joseph_march(const FwdGeom& G, const JosephRay& 
     const float fb = floorf(qb), fd = floorf(qd);
     const float wb1 = qb - fb, wd1 = qd - fd, wb0 = 1.f - wb1, wd0 = 1.f - wd1;
     const int ib = (int)fb, id = (int)fd;
-    const long long base = (long long)k * S[A] + (long long)ib * S[B] + (long long)id * S[D];
     const bool okb0 = (unsigned)ib < (unsigned)n[B], okb1 = (unsigned)(ib + 1) < (unsigned)n[B];
     const bool okd0 = (unsigned)id < (unsigned)n[D], okd1 = (unsigned)(id + 1) < (unsigned)n[D];
     if (!GRAD) {
-      const float v00 = jload(vol, base, okb0 && okd0), v10 = jload(vol, base + S[B], okb1 && okd0);
-      const float v01 = jload(vol, base + S[D], okb0 && okd1), v11 = jload(vol, base + S[B] + S[D], okb1 && okd1);
+      // the 2 x 2 in-plane voxels from the packed quad cells (pack_volume_kernel: cell (x,y,z) holds voxels
+      // (x,y), (x+1,y), (x,y+1), (x+1,y+1) of slice z; zero border of kPad cells, so no bound predicates):
+      // driving axis z: one cell; x or y: the cells of two consecutive slices, two of their four values each
+      int x, y, z;
+      if (A == 0) { x = k; y = ib; z = id; } else if (A == 1) { x = id; y = k; z = ib; } else { x = ib; y = id; z = k; }
+      const unsigned X = (unsigned)(x + G.L.lx), Y = (unsigned)(y + G.L.ly), Z = (unsigned)(z + G.L.lz);
+      const unsigned idx = X + 3u * (X & ~1u) + 2u * Y + G.L.by * (Y & ~1u) + 4u * Z + G.L.bz * (Z & ~1u);
+      const float4 c0 = ldg4(pvol + idx);
+      float v00, v10, v01, v11;                       // v[jb][jd]
+      if (A == 2) {
+        v00 = c0.x; v10 = c0.y; v01 = c0.z; v11 = c0.w;
+      } else {
+        const float4 c1 = ldg4(pvol + (idx + ((Z & 1u) ? 2u * G.L.bz + 4u : 4u)));      // slice z + 1
+        if (A == 0) { v00 = c0.x; v10 = c0.z; v01 = c1.x; v11 = c1.z; }           // B = y, D = z
+        else        { v00 = c0.x; v10 = c1.x; v01 = c0.y; v11 = c1.y; }           // B = z, D = x
+      }
       sum += wd0 * (wb0 * v00 + wb1 * v10) + wd1 * (wb0 * v01 + wb1 * v11);
     } else {
-      // the in-plane 4 x 4 neighbourhood without its corners (12 voxels) and the 2 x 2 block in planes k-1, k+1
-      // (8 voxels), each loaded once; zero extension by predicate
-      const bool okbm = (unsigned)(ib - 1) < (unsigned)n[B], okb2 = (unsigned)(ib + 2) < (unsigned)n[B];
-      const bool okdm = (unsigned)(id - 1) < (unsigned)n[D], okd2 = (unsigned)(id + 2) < (unsigned)n[D];
-      const bool okam = k > 0, okap = k + 1 < n[A];
-      const bool okb[4] = {okbm, okb0, okb1, okb2}, okd[4] = {okdm, okd0, okd1, okd2};
-      float P[4][4];                                   // P[jd+1][jb+1] = voxel (ib+jb, id+jd), jb, jd in -1..2
-#pragma unroll
-      for (int jd = 0; jd < 4; ++jd)
-#pragma unroll
-        for (int jb = 0; jb < 4; ++jb) {
-          const bool corner = (jd == 0 || jd == 3) && (jb == 0 || jb == 3);
-          P[jd][jb] = corner ? 0.f : jload(vol, base + (jb - 1) * S[B] + (jd - 1) * S[D], okb[jb] && okd[jd]);
-        }
+      // g_j of the four voxels from the per-voxel gradient volume (grad_volume_kernel); grid voxels only (O13)
+      const GradBricks Bk = GradBricks::make(G.L.nx, G.L.ny, G.L.nz);
+      int FA, FB[2], FD[2];
+      if (A == 0) { FA = Bk.FX(k); FB[0] = Bk.FY(ib); FB[1] = Bk.FY(ib + 1); FD[0] = Bk.FZ(id); FD[1] = Bk.FZ(id + 1); }
+      else if (A == 1) { FA = Bk.FY(k); FB[0] = Bk.FZ(ib); FB[1] = Bk.FZ(ib + 1); FD[0] = Bk.FX(id); FD[1] = Bk.FX(id + 1); }
+      else { FA = Bk.FZ(k); FB[0] = Bk.FX(ib); FB[1] = Bk.FX(ib + 1); FD[0] = Bk.FY(id); FD[1] = Bk.FY(id + 1); }
+      const bool okb[2] = {okb0, okb1}, okd[2] = {okd0, okd1};
+      float r3[3];
+      r3[A] = fmaf(kf - ha, vv[A], cc[A]);
 #pragma unroll
       for (int jd = 0; jd < 2; ++jd)
 #pragma unroll
         for (int jb = 0; jb < 2; ++jb) {
-          const bool ok = okb[jb + 1] && okd[jd + 1];
-          const float w = ok ? (jb ? wb1 : wb0) * (jd ? wd1 : wd0) : 0.f;       // grid voxels only (O13)
-          const long long o = base + jb * S[B] + jd * S[D];
-          const float ga = jload(vol, o + S[A], ok && okap) - jload(vol, o - S[A], ok && okam);
-          const float gb = P[jd + 1][jb + 2] - P[jd + 1][jb];
-          const float gd = P[jd + 2][jb + 1] - P[jd][jb + 1];
-          float g3[3], r3[3];
-          g3[A] = w * ga * sg[A]; g3[B] = w * gb * sg[B]; g3[D] = w * gd * sg[D];
-          r3[A] = fmaf(kf - ha, vv[A], cc[A]);
+          const bool ok = okb[jb] && okd[jd];
+          const float w = (jb ? wb1 : wb0) * (jd ? wd1 : wd0);
+          float4 g = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (ok) g = ldg4(gvol + (FA + FB[jb] + FD[jd]));
+          const float g0 = w * g.x, g1 = w * g.y, g2 = w * g.z;
           r3[B] = fmaf((float)(ib + jb) - hb, vv[B], cc[B]);
           r3[D] = fmaf((float)(id + jd) - hd, vv[D], cc[D]);
-          a0 += g3[0]; a1 += g3[1]; a2 += g3[2];
-          b0 += r3[1] * g3[2] - r3[2] * g3[1];
-          b1 += r3[2] * g3[0] - r3[0] * g3[2];
-          b2 += r3[0] * g3[1] - r3[1] * g3[0];
+          a0 += g0; a1 += g1; a2 += g2;
+          b0 += r3[1] * g2 - r3[2] * g1;
+          b1 += r3[2] * g0 - r3[0] * g2;
+          b2 += r3[0] * g1 - r3[1] * g0;
         }
     }
   }
@@ -145,15 +145,15 @@ __device__ __forceinline__ void joseph_march(const FwdGeom& G, const JosephRay& 
 }
 
 template <bool GRAD>
-__device__ __forceinline__ void joseph_ray(const FwdGeom& G, const JosephRay& r, const float* __restrict__ vol,
-                                           float* acc) {
-  if (r.axis == 0) joseph_march<0, GRAD>(G, r, vol, acc);
-  else if (r.axis == 1) joseph_march<1, GRAD>(G, r, vol, acc);
-  else joseph_march<2, GRAD>(G, r, vol, acc);
+__device__ __forceinline__ void joseph_ray(const FwdGeom& G, const JosephRay& r, const float4* __restrict__ pvol,
+                                           const float4* __restrict__ gvol, float* acc) {
+  if (r.axis == 0) joseph_march<0, GRAD>(G, r, pvol, gvol, acc);
+  else if (r.axis == 1) joseph_march<1, GRAD>(G, r, pvol, gvol, acc);
+  else joseph_march<2, GRAD>(G, r, pvol, gvol, acc);
 }
 
 __global__ void __launch_bounds__(kFwdThreads) joseph_fwd_kernel(FwdGeom G, const FwdView* __restrict__ views,
-                                                                 const float* __restrict__ vol,
+                                                                 const float4* __restrict__ pvol,
                                                                  float* __restrict__ proj) {
   int iu, iv;
   fwd_pixel(iu, iv);
@@ -161,12 +161,12 @@ __global__ void __launch_bounds__(kFwdThreads) joseph_fwd_kernel(FwdGeom G, cons
   if (iu >= G.nu || iv >= G.nv) return;
   const JosephRay r = joseph_setup(G, views[view], iu, iv);
   float acc[1] = {0.f};
-  joseph_ray<false>(G, r, vol, acc);
+  joseph_ray<false>(G, r, pvol, nullptr, acc);
   proj[((size_t)view * G.nv + iv) * G.nu + iu] = acc[0];
 }
 
 __global__ void __launch_bounds__(kFwdThreads) joseph_grad_kernel(FwdGeom G, const FwdView* __restrict__ views,
-                                                                  const float* __restrict__ vol,
+                                                                  const float4* __restrict__ gvol,
                                                                   const float* __restrict__ upstream,
                                                                   float* __restrict__ partials) {
   int iu, iv;
@@ -176,7 +176,7 @@ __global__ void __launch_bounds__(kFwdThreads) joseph_grad_kernel(FwdGeom G, con
   float out[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   if (live) {
     const JosephRay r = joseph_setup(G, views[view], iu, iv);
-    joseph_ray<true>(G, r, vol, out);
+    joseph_ray<true>(G, r, nullptr, gvol, out);
     const float w = __ldg(upstream + ((size_t)view * G.nv + iv) * G.nu + iu);
 #pragma unroll
     for (int q = 0; q < 6; ++q) out[q] *= w;

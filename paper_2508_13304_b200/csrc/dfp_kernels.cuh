@@ -71,6 +71,48 @@ __global__ void __launch_bounds__(256) pack_volume_kernel(VolLayout L, const flo
   }
 }
 
+// Per-voxel gradient volume for the weight models that follow the paper's per-voxel G_f^j (Siddon, Joseph;
+// PAPER.md :183, :189): g_j = central differences of the zero-extended voxel values times 1/(2 v_a), one float4
+// (g_x, g_y, g_z, f_j) per GRID voxel, in 2 x 2 x 2 bricks of 128 B so that the rays of a warp, which spread over a
+// few voxels in every direction, touch few lines.  GradBricks::index(x, y, z) = FX(x) + FY(y) + FZ(z).
+struct GradBricks {
+  int nx, ny, nz;
+  int fy8, fz8;                  // 8 * nbx, 8 * nbx * nby
+  __host__ __device__ static GradBricks make(int nx, int ny, int nz) {
+    GradBricks b;
+    b.nx = nx; b.ny = ny; b.nz = nz;
+    b.fy8 = 8 * ((nx + 1) / 2);
+    b.fz8 = b.fy8 * ((ny + 1) / 2);
+    return b;
+  }
+  __host__ __device__ size_t cells() const { return (size_t)fz8 * ((nz + 1) / 2); }
+  __device__ __forceinline__ int FX(int x) const { return ((x >> 1) << 3) + (x & 1); }
+  __device__ __forceinline__ int FY(int y) const { return (y >> 1) * fy8 + ((y & 1) << 1); }
+  __device__ __forceinline__ int FZ(int z) const { return (z >> 1) * fz8 + ((z & 1) << 2); }
+};
+
+__global__ void __launch_bounds__(256) grad_volume_kernel(GradBricks B, float sgx, float sgy, float sgz,
+                                                          const float* __restrict__ vol, float4* __restrict__ gvol) {
+  const size_t n = B.cells();
+  const unsigned nbx = (unsigned)B.fy8 / 8u, nbxy = (unsigned)B.fz8 / 8u;
+  const size_t sy = (size_t)B.nx, sz = (size_t)B.nx * B.ny;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const unsigned within = (unsigned)(i & 7), brick = (unsigned)(i >> 3);
+    const unsigned bz = brick / nbxy, rem = brick - bz * nbxy;
+    const unsigned by = rem / nbx, bx = rem - by * nbx;
+    const int x = (int)(2 * bx + (within & 1)), y = (int)(2 * by + ((within >> 1) & 1)), z = (int)(2 * bz + (within >> 2));
+    float4 g = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (x < B.nx && y < B.ny && z < B.nz) {
+      const float* c = vol + (size_t)z * sz + (size_t)y * sy + x;
+      g.x = sgx * ((x + 1 < B.nx ? __ldg(c + 1) : 0.f) - (x > 0 ? __ldg(c - 1) : 0.f));
+      g.y = sgy * ((y + 1 < B.ny ? __ldg(c + sy) : 0.f) - (y > 0 ? __ldg(c - sy) : 0.f));
+      g.z = sgz * ((z + 1 < B.nz ? __ldg(c + sz) : 0.f) - (z > 0 ? __ldg(c - sz) : 0.f));
+      g.w = __ldg(c);
+    }
+    gvol[i] = g;
+  }
+}
+
 __global__ void __launch_bounds__(256) pack_proj_kernel(int nu, int nv, int pu, int pv, size_t n_views,
                                                         const float* __restrict__ proj, float4* __restrict__ q) {
   const size_t per = (size_t)pu * pv, n = per * n_views;

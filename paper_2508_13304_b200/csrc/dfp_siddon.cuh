@@ -11,8 +11,9 @@
 // generated in order instead of sorted).  Crossing PARAMETERS reach ~1000 mm while a segment is ~1 voxel long, so a
 // length taken as a difference of two fp32 parameters would carry 1e-4 relative error; the set-up therefore runs in
 // fp64 and the loop tracks only the (small) distances to the next crossings.  Values are read straight from the caller's
-// volume through L1 (one voxel per segment; the six neighbours for the gradient) - no packed copy, no staging: this
-// is a first, plain kernel for the "next" row, measured beside the trilinear ones in DESIGN.md.
+// volume through L1 (forward: one voxel per segment); the gradient reads one float4 of the per-voxel gradient volume
+// (dfp_kernels.cuh: grad_volume_kernel) per segment.  No shared-memory staging: kernels for the "next" row, measured
+// beside the trilinear ones in DESIGN.md.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -83,7 +84,9 @@ __device__ __forceinline__ SiddonRay siddon_setup(const FwdGeom& G, const FwdVie
 // Written with selects on named scalars (an array indexed by the crossed axis would live in local memory).
 struct SiddonState {
   float rx, ry, rz, dtx, dty, dtz;       // distance to the next x / y / z plane; spacing of the crossings
-  int ix, iy, iz, sx, sy, sz, idx;
+  int ix, iy, iz, sx, sy, sz;
+  int idx;                               // linear offset of the voxel in the caller's volume (forward kernel)
+  int fx, fy, fz;                        // GradBricks terms of the voxel (gradient kernel)
 };
 __device__ __forceinline__ SiddonState siddon_state(const SiddonRay& r, int nx, int ny) {
   SiddonState s;
@@ -92,22 +95,27 @@ __device__ __forceinline__ SiddonState siddon_state(const SiddonRay& r, int nx, 
   s.ix = r.i[0]; s.iy = r.i[1]; s.iz = r.i[2];
   s.sx = r.step[0]; s.sy = r.step[1]; s.sz = r.step[2];
   s.idx = (s.iz * ny + s.iy) * nx + s.ix;
+  s.fx = s.fy = s.fz = 0;
   return s;
 }
-__device__ __forceinline__ float siddon_step(SiddonState& s, int nx, int ny, int nz, bool& alive) {
+template <bool BRICK>
+__device__ __forceinline__ float siddon_step(SiddonState& s, int nx, int ny, int nz, const GradBricks& B, bool& alive) {
   const bool cx = s.rx <= s.ry && s.rx <= s.rz;
   const bool cy = !cx && s.ry <= s.rz;
   const float len = fmaxf(cx ? s.rx : (cy ? s.ry : s.rz), 0.f);
   s.rx -= len; s.ry -= len; s.rz -= len;
   bool inside;
   if (cx) {
-    s.rx = s.dtx; s.ix += s.sx; s.idx += s.sx;
+    s.rx = s.dtx; s.ix += s.sx;
+    if (BRICK) s.fx = B.FX(s.ix); else s.idx += s.sx;
     inside = (unsigned)s.ix < (unsigned)nx;
   } else if (cy) {
-    s.ry = s.dty; s.iy += s.sy; s.idx += s.sy * nx;
+    s.ry = s.dty; s.iy += s.sy;
+    if (BRICK) s.fy = B.FY(s.iy); else s.idx += s.sy * nx;
     inside = (unsigned)s.iy < (unsigned)ny;
   } else {
-    s.rz = s.dtz; s.iz += s.sz; s.idx += s.sz * nx * ny;
+    s.rz = s.dtz; s.iz += s.sz;
+    if (BRICK) s.fz = B.FZ(s.iz); else s.idx += s.sz * nx * ny;
     inside = (unsigned)s.iz < (unsigned)nz;
   }
   alive = inside;
@@ -127,10 +135,11 @@ __global__ void __launch_bounds__(kFwdThreads) siddon_fwd_kernel(FwdGeom G, cons
   float sum = 0.f;
   if (r.hit) {
     SiddonState s = siddon_state(r, nx, ny);
+    const GradBricks B = GradBricks::make(nx, ny, nz);   // unused by the forward kernel
     bool alive = true;
     while (alive) {
       const float val = __ldg(vol + s.idx);
-      const float len = siddon_step(s, nx, ny, nz, alive);
+      const float len = siddon_step<false>(s, nx, ny, nz, B, alive);
       sum = fmaf(len, val, sum);
     }
   }
@@ -138,8 +147,11 @@ __global__ void __launch_bounds__(kFwdThreads) siddon_fwd_kernel(FwdGeom G, cons
 }
 
 // ------------------------------------------------------------------------------------------------ pose gradient
+// g_j comes from the per-voxel gradient volume (grad_volume_kernel, written once per call): one 16-byte read per
+// segment instead of six predicated scalar gathers - the first version, which differenced the caller's volume in the
+// loop, was L1TEX-bound.
 __global__ void __launch_bounds__(kFwdThreads) siddon_grad_kernel(FwdGeom G, const FwdView* __restrict__ views,
-                                                                  const float* __restrict__ vol,
+                                                                  const float4* __restrict__ gvol,
                                                                   const float* __restrict__ upstream,
                                                                   float* __restrict__ partials) {
   int iu, iv;
@@ -150,24 +162,20 @@ __global__ void __launch_bounds__(kFwdThreads) siddon_grad_kernel(FwdGeom G, con
   if (live) {
     const SiddonRay r = siddon_setup(G, views[view], iu, iv, nullptr);
     const int nx = G.L.nx, ny = G.L.ny, nz = G.L.nz;
-    const int sy_ = nx, sz_ = nx * ny;
+    const GradBricks B = GradBricks::make(nx, ny, nz);
     // voxel centre r'_j = c + (i - (n-1)/2) v
     const float hx = 0.5f * (float)(nx - 1), hy = 0.5f * (float)(ny - 1), hz = 0.5f * (float)(nz - 1);
     float ax_ = 0.f, ay_ = 0.f, az_ = 0.f, bx = 0.f, by = 0.f, bz = 0.f;     // A_i, B_i
     if (r.hit) {
       SiddonState s = siddon_state(r, nx, ny);
+      s.fx = B.FX(s.ix); s.fy = B.FY(s.iy); s.fz = B.FZ(s.iz);
       bool alive = true;
       while (alive) {
-        const int ix = s.ix, iy = s.iy, iz = s.iz;
-        const float* c = vol + s.idx;
-        // central differences of the zero-extended voxel values (2 v_a g_a)
-        const float gx = ((ix + 1 < nx) ? __ldg(c + 1) : 0.f) - ((ix > 0) ? __ldg(c - 1) : 0.f);
-        const float gy = ((iy + 1 < ny) ? __ldg(c + sy_) : 0.f) - ((iy > 0) ? __ldg(c - sy_) : 0.f);
-        const float gz = ((iz + 1 < nz) ? __ldg(c + sz_) : 0.f) - ((iz > 0) ? __ldg(c - sz_) : 0.f);
-        const float rx = fmaf((float)ix - hx, G.vx, G.cx), ry = fmaf((float)iy - hy, G.vy, G.cy),
-                    rz = fmaf((float)iz - hz, G.vz, G.cz);
-        const float len = siddon_step(s, nx, ny, nz, alive);
-        const float lx = len * gx * G.sgx, ly = len * gy * G.sgy, lz = len * gz * G.sgz;   // a^ij g_j  (sg = 1 / 2v)
+        const float4 g = ldg4(gvol + (s.fx + s.fy + s.fz));
+        const float rx = fmaf((float)s.ix - hx, G.vx, G.cx), ry = fmaf((float)s.iy - hy, G.vy, G.cy),
+                    rz = fmaf((float)s.iz - hz, G.vz, G.cz);
+        const float len = siddon_step<true>(s, nx, ny, nz, B, alive);
+        const float lx = len * g.x, ly = len * g.y, lz = len * g.z;          // a^ij g_j
         ax_ += lx; ay_ += ly; az_ += lz;
         bx += ry * lz - rz * ly;
         by += rz * lx - rx * lz;
