@@ -74,6 +74,9 @@ __device__ __forceinline__ JosephRay joseph_setup(const FwdGeom& G, const FwdVie
 }
 
 // A = driving axis; B = (A+1)%3, D = (A+2)%3.  GRAD = false: returns the projection in acc[0].
+// floor() of the two in-plane coordinates by the magic-number addition of the trilinear kernels (no F2I / FRND):
+// t = (q - 1/2) + 1.5 * 2^23 holds rint(q - 1/2) in its low mantissa bits, which is floor(q) except at integers,
+// where either neighbour with weight 0 / 1 gives the same interpolant.
 template <int A, bool GRAD>
 __device__ __forceinline__ void joseph_march(const FwdGeom& G, const JosephRay& r, const float4* __restrict__ pvol,
                                              const float4* __restrict__ gvol, float* acc) {
@@ -81,15 +84,17 @@ __device__ __forceinline__ void joseph_march(const FwdGeom& G, const JosephRay& 
   const int n[3] = {G.L.nx, G.L.ny, G.L.nz};
   const float vv[3] = {G.vx, G.vy, G.vz}, cc[3] = {G.cx, G.cy, G.cz};
   const float hb = 0.5f * (float)(n[B] - 1), hd = 0.5f * (float)(n[D] - 1), ha = 0.5f * (float)(n[A] - 1);
+  const float pb = r.pb0 + (hb - 0.5f), pd = r.pd0 + (hd - 0.5f);          // continuous index minus 1/2 at k = 0
   float sum = 0.f, a0 = 0.f, a1 = 0.f, a2 = 0.f, b0 = 0.f, b1 = 0.f, b2 = 0.f;
-  for (int k = r.k0; k <= r.k1; ++k) {
-    const float kf = (float)k;
-    const float qb = fmaf(kf, r.dpb, r.pb0) + hb, qd = fmaf(kf, r.dpd, r.pd0) + hd;     // continuous indices
-    const float fb = floorf(qb), fd = floorf(qd);
-    const float wb1 = qb - fb, wd1 = qd - fd, wb0 = 1.f - wb1, wd0 = 1.f - wd1;
-    const int ib = (int)fb, id = (int)fd;
-    const bool okb0 = (unsigned)ib < (unsigned)n[B], okb1 = (unsigned)(ib + 1) < (unsigned)n[B];
-    const bool okd0 = (unsigned)id < (unsigned)n[D], okd1 = (unsigned)(id + 1) < (unsigned)n[D];
+  float kf = (float)r.k0;
+  const GradBricks Bk = GradBricks::make(G.L.nx, G.L.ny, G.L.nz);
+#pragma unroll(GRAD ? 1 : 4)
+  for (int k = r.k0; k <= r.k1; ++k, kf += 1.0f) {
+    const float qb = fmaf(kf, r.dpb, pb), qd = fmaf(kf, r.dpd, pd);
+    const float tb = qb + kMagic, td = qd + kMagic;
+    const float wb1 = (qb - (tb - kMagic)) + 0.5f, wd1 = (qd - (td - kMagic)) + 0.5f;
+    const float wb0 = 1.f - wb1, wd0 = 1.f - wd1;
+    const int ib = __float_as_int(tb) - kMagicBits, id = __float_as_int(td) - kMagicBits;
     if (!GRAD) {
       // the 2 x 2 in-plane voxels from the packed quad cells (pack_volume_kernel: cell (x,y,z) holds voxels
       // (x,y), (x+1,y), (x,y+1), (x+1,y+1) of slice z; zero border of kPad cells, so no bound predicates):
@@ -103,37 +108,47 @@ __device__ __forceinline__ void joseph_march(const FwdGeom& G, const JosephRay& 
       if (A == 2) {
         v00 = c0.x; v10 = c0.y; v01 = c0.z; v11 = c0.w;
       } else {
-        const float4 c1 = ldg4(pvol + (idx + ((Z & 1u) ? 2u * G.L.bz + 4u : 4u)));      // slice z + 1
+        const float4 c1 = ldg4(pvol + (idx + ((Z & 1u) ? 2u * G.L.bz + 4u : 4u)));  // slice z + 1
         if (A == 0) { v00 = c0.x; v10 = c0.z; v01 = c1.x; v11 = c1.z; }           // B = y, D = z
         else        { v00 = c0.x; v10 = c1.x; v01 = c0.y; v11 = c1.y; }           // B = z, D = x
       }
       sum += wd0 * (wb0 * v00 + wb1 * v10) + wd1 * (wb0 * v01 + wb1 * v11);
     } else {
-      // g_j of the four voxels from the per-voxel gradient volume (grad_volume_kernel); grid voxels only (O13)
-      const GradBricks Bk = GradBricks::make(G.L.nx, G.L.ny, G.L.nz);
-      int FA, FB[2], FD[2];
-      if (A == 0) { FA = Bk.FX(k); FB[0] = Bk.FY(ib); FB[1] = Bk.FY(ib + 1); FD[0] = Bk.FZ(id); FD[1] = Bk.FZ(id + 1); }
-      else if (A == 1) { FA = Bk.FY(k); FB[0] = Bk.FZ(ib); FB[1] = Bk.FZ(ib + 1); FD[0] = Bk.FX(id); FD[1] = Bk.FX(id + 1); }
-      else { FA = Bk.FZ(k); FB[0] = Bk.FX(ib); FB[1] = Bk.FX(ib + 1); FD[0] = Bk.FY(id); FD[1] = Bk.FY(id + 1); }
-      const bool okb[2] = {okb0, okb1}, okd[2] = {okd0, okd1};
-      float r3[3];
+      // g_j of the four voxels from the per-voxel gradient volume (grad_volume_kernel); grid voxels only (O13).
+      // The four lever arms differ by one pitch along B and D:  sum_j w_j r'_j x g_j =
+      //   r'_00 x S + v_B e_B x S_b + v_D e_D x S_d,   S = sum_j w_j g_j,  S_b / S_d = the jb = 1 / jd = 1 parts.
+      const bool okb0 = (unsigned)ib < (unsigned)n[B], okb1 = (unsigned)(ib + 1) < (unsigned)n[B];
+      const bool okd0 = (unsigned)id < (unsigned)n[D], okd1 = (unsigned)(id + 1) < (unsigned)n[D];
+      int FA, FB0, FB1, FD0, FD1;
+      if (A == 0) { FA = Bk.FX(k); FB0 = Bk.FY(ib); FB1 = Bk.FY(ib + 1); FD0 = Bk.FZ(id); FD1 = Bk.FZ(id + 1); }
+      else if (A == 1) { FA = Bk.FY(k); FB0 = Bk.FZ(ib); FB1 = Bk.FZ(ib + 1); FD0 = Bk.FX(id); FD1 = Bk.FX(id + 1); }
+      else { FA = Bk.FZ(k); FB0 = Bk.FX(ib); FB1 = Bk.FX(ib + 1); FD0 = Bk.FY(id); FD1 = Bk.FY(id + 1); }
+      const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+      const float4 g00 = (okb0 && okd0) ? ldg4(gvol + (FA + FB0 + FD0)) : z4;
+      const float4 g10 = (okb1 && okd0) ? ldg4(gvol + (FA + FB1 + FD0)) : z4;
+      const float4 g01 = (okb0 && okd1) ? ldg4(gvol + (FA + FB0 + FD1)) : z4;
+      const float4 g11 = (okb1 && okd1) ? ldg4(gvol + (FA + FB1 + FD1)) : z4;
+      const float w00 = wb0 * wd0, w10 = wb1 * wd0, w01 = wb0 * wd1, w11 = wb1 * wd1;
+      float S[3], Sb[3], Sd[3], r3[3];
+      Sb[0] = fmaf(w10, g10.x, w11 * g11.x); Sb[1] = fmaf(w10, g10.y, w11 * g11.y); Sb[2] = fmaf(w10, g10.z, w11 * g11.z);
+      Sd[0] = fmaf(w01, g01.x, w11 * g11.x); Sd[1] = fmaf(w01, g01.y, w11 * g11.y); Sd[2] = fmaf(w01, g01.z, w11 * g11.z);
+      S[0] = fmaf(w00, g00.x, fmaf(w01, g01.x, Sb[0]));
+      S[1] = fmaf(w00, g00.y, fmaf(w01, g01.y, Sb[1]));
+      S[2] = fmaf(w00, g00.z, fmaf(w01, g01.z, Sb[2]));
       r3[A] = fmaf(kf - ha, vv[A], cc[A]);
-#pragma unroll
-      for (int jd = 0; jd < 2; ++jd)
-#pragma unroll
-        for (int jb = 0; jb < 2; ++jb) {
-          const bool ok = okb[jb] && okd[jd];
-          const float w = (jb ? wb1 : wb0) * (jd ? wd1 : wd0);
-          float4 g = make_float4(0.f, 0.f, 0.f, 0.f);
-          if (ok) g = ldg4(gvol + (FA + FB[jb] + FD[jd]));
-          const float g0 = w * g.x, g1 = w * g.y, g2 = w * g.z;
-          r3[B] = fmaf((float)(ib + jb) - hb, vv[B], cc[B]);
-          r3[D] = fmaf((float)(id + jd) - hd, vv[D], cc[D]);
-          a0 += g0; a1 += g1; a2 += g2;
-          b0 += r3[1] * g2 - r3[2] * g1;
-          b1 += r3[2] * g0 - r3[0] * g2;
-          b2 += r3[0] * g1 - r3[1] * g0;
-        }
+      r3[B] = fmaf((float)ib - hb, vv[B], cc[B]);
+      r3[D] = fmaf((float)id - hd, vv[D], cc[D]);
+      float bq[3];
+      bq[0] = r3[1] * S[2] - r3[2] * S[1];
+      bq[1] = r3[2] * S[0] - r3[0] * S[2];
+      bq[2] = r3[0] * S[1] - r3[1] * S[0];
+      // (A, B, D) is a cyclic permutation of (x, y, z):  e_B x S = S_D e_A - S_A e_D,   e_D x S = S_A e_B - S_B e_A
+      bq[A] = fmaf(vv[B], Sb[D], bq[A]);
+      bq[D] = fmaf(-vv[B], Sb[A], bq[D]);
+      bq[B] = fmaf(vv[D], Sd[A], bq[B]);
+      bq[A] = fmaf(-vv[D], Sd[B], bq[A]);
+      a0 += S[0]; a1 += S[1]; a2 += S[2];
+      b0 += bq[0]; b1 += bq[1]; b2 += bq[2];
     }
   }
   if (!GRAD) {

@@ -84,46 +84,68 @@ __device__ __forceinline__ SiddonRay siddon_setup(const FwdGeom& G, const FwdVie
 // Written with selects on named scalars (an array indexed by the crossed axis would live in local memory).
 struct SiddonState {
   float rx, ry, rz, dtx, dty, dtz;       // distance to the next x / y / z plane; spacing of the crossings
-  int ix, iy, iz, sx, sy, sz;
-  int idx;                               // linear offset of the voxel in the caller's volume (forward kernel)
-  int fx, fy, fz;                        // GradBricks terms of the voxel (gradient kernel)
+  int nx_, ny_, nz_;                     // crossings of each family left before the ray leaves the grid
+  int idx, stx, sty, stz;                // offset of the voxel and its step per family: linear in the caller's volume
+                                         // (forward); GradBricks index and the step of the NEXT crossing (gradient)
+  int ttx, tty, ttz;                     // gradient: step of this crossing + step of the following one (they alternate
+                                         // with the parity of the index: inside the brick, then to the next brick)
+  float px, py, pz, dpx, dpy, dpz;       // gradient: voxel centre r'_j (mm) and its step per family
 };
-__device__ __forceinline__ SiddonState siddon_state(const SiddonRay& r, int nx, int ny) {
+template <bool BRICK>
+__device__ __forceinline__ SiddonState siddon_state(const SiddonRay& r, const FwdGeom& G) {
+  const int nx = G.L.nx, ny = G.L.ny, nz = G.L.nz;
   SiddonState s;
   s.rx = (float)fmin(r.tn[0] - r.t, 1e30); s.ry = (float)fmin(r.tn[1] - r.t, 1e30); s.rz = (float)fmin(r.tn[2] - r.t, 1e30);
   s.dtx = (float)fmin(r.dt[0], 1e30); s.dty = (float)fmin(r.dt[1], 1e30); s.dtz = (float)fmin(r.dt[2], 1e30);
-  s.ix = r.i[0]; s.iy = r.i[1]; s.iz = r.i[2];
-  s.sx = r.step[0]; s.sy = r.step[1]; s.sz = r.step[2];
-  s.idx = (s.iz * ny + s.iy) * nx + s.ix;
-  s.fx = s.fy = s.fz = 0;
+  const int ix = r.i[0], iy = r.i[1], iz = r.i[2], sx = r.step[0], sy = r.step[1], sz = r.step[2];
+  s.nx_ = sx > 0 ? nx - ix : ix + 1;                // a family with step 0 is never crossed (its distance is 1e30)
+  s.ny_ = sy > 0 ? ny - iy : iy + 1;
+  s.nz_ = sz > 0 ? nz - iz : iz + 1;
+  if (!BRICK) {
+    s.idx = (iz * ny + iy) * nx + ix;
+    s.stx = sx; s.sty = sy * nx; s.stz = sz * nx * ny;
+  } else {
+    const GradBricks B = GradBricks::make(nx, ny, nz);
+    s.idx = B.FX(ix) + B.FY(iy) + B.FZ(iz);
+    s.stx = B.FX(ix + sx) - B.FX(ix); s.ttx = 8 * sx;
+    s.sty = B.FY(iy + sy) - B.FY(iy); s.tty = B.fy8 * sy;
+    s.stz = B.FZ(iz + sz) - B.FZ(iz); s.ttz = B.fz8 * sz;
+    // voxel centre r'_j = c + (i - (n-1)/2) v, stepped in fp32 (a few hundred additions of a pitch: ~1e-5 mm)
+    s.px = fmaf((float)ix - 0.5f * (float)(nx - 1), G.vx, G.cx); s.dpx = (float)sx * G.vx;
+    s.py = fmaf((float)iy - 0.5f * (float)(ny - 1), G.vy, G.cy); s.dpy = (float)sy * G.vy;
+    s.pz = fmaf((float)iz - 0.5f * (float)(nz - 1), G.vz, G.cz); s.dpz = (float)sz * G.vz;
+  }
   return s;
 }
+// Branch-free on purpose: the three families take turns within a warp, and the if / else form compiled to a
+// divergent branch with a dozen register moves per step.
 template <bool BRICK>
-__device__ __forceinline__ float siddon_step(SiddonState& s, int nx, int ny, int nz, const GradBricks& B, bool& alive) {
+__device__ __forceinline__ float siddon_step(SiddonState& s, bool& alive) {
   const bool cx = s.rx <= s.ry && s.rx <= s.rz;
   const bool cy = !cx && s.ry <= s.rz;
+  const bool cz = !cx && !cy;
   const float len = fmaxf(cx ? s.rx : (cy ? s.ry : s.rz), 0.f);
-  s.rx -= len; s.ry -= len; s.rz -= len;
-  bool inside;
-  if (cx) {
-    s.rx = s.dtx; s.ix += s.sx;
-    if (BRICK) s.fx = B.FX(s.ix); else s.idx += s.sx;
-    inside = (unsigned)s.ix < (unsigned)nx;
-  } else if (cy) {
-    s.ry = s.dty; s.iy += s.sy;
-    if (BRICK) s.fy = B.FY(s.iy); else s.idx += s.sy * nx;
-    inside = (unsigned)s.iy < (unsigned)ny;
-  } else {
-    s.rz = s.dtz; s.iz += s.sz;
-    if (BRICK) s.fz = B.FZ(s.iz); else s.idx += s.sz * nx * ny;
-    inside = (unsigned)s.iz < (unsigned)nz;
+  s.rx = cx ? s.dtx : s.rx - len;
+  s.ry = cy ? s.dty : s.ry - len;
+  s.rz = cz ? s.dtz : s.rz - len;
+  if (cx) --s.nx_;
+  if (cy) --s.ny_;
+  if (cz) --s.nz_;
+  alive = (cx ? s.nx_ : (cy ? s.ny_ : s.nz_)) != 0;
+  s.idx += cx ? s.stx : (cy ? s.sty : s.stz);
+  if (BRICK) {
+    s.stx = cx ? s.ttx - s.stx : s.stx;
+    s.sty = cy ? s.tty - s.sty : s.sty;
+    s.stz = cz ? s.ttz - s.stz : s.stz;
+    s.px += cx ? s.dpx : 0.f;
+    s.py += cy ? s.dpy : 0.f;
+    s.pz += cz ? s.dpz : 0.f;
   }
-  alive = inside;
   return len;
 }
 
 // ------------------------------------------------------------------------------------------------ forward
-__global__ void __launch_bounds__(kFwdThreads) siddon_fwd_kernel(FwdGeom G, const FwdView* __restrict__ views,
+__global__ void __launch_bounds__(kFwdThreads, 6) siddon_fwd_kernel(FwdGeom G, const FwdView* __restrict__ views,
                                                                  const float* __restrict__ vol,
                                                                  float* __restrict__ proj) {
   int iu, iv;
@@ -131,15 +153,13 @@ __global__ void __launch_bounds__(kFwdThreads) siddon_fwd_kernel(FwdGeom G, cons
   const int view = blockIdx.z;
   if (iu >= G.nu || iv >= G.nv) return;
   const SiddonRay r = siddon_setup(G, views[view], iu, iv, nullptr);
-  const int nx = G.L.nx, ny = G.L.ny, nz = G.L.nz;
   float sum = 0.f;
   if (r.hit) {
-    SiddonState s = siddon_state(r, nx, ny);
-    const GradBricks B = GradBricks::make(nx, ny, nz);   // unused by the forward kernel
+    SiddonState s = siddon_state<false>(r, G);
     bool alive = true;
     while (alive) {
       const float val = __ldg(vol + s.idx);
-      const float len = siddon_step<false>(s, nx, ny, nz, B, alive);
+      const float len = siddon_step<false>(s, alive);
       sum = fmaf(len, val, sum);
     }
   }
@@ -150,7 +170,7 @@ __global__ void __launch_bounds__(kFwdThreads) siddon_fwd_kernel(FwdGeom G, cons
 // g_j comes from the per-voxel gradient volume (grad_volume_kernel, written once per call): one 16-byte read per
 // segment instead of six predicated scalar gathers - the first version, which differenced the caller's volume in the
 // loop, was L1TEX-bound.
-__global__ void __launch_bounds__(kFwdThreads) siddon_grad_kernel(FwdGeom G, const FwdView* __restrict__ views,
+__global__ void __launch_bounds__(kFwdThreads, 5) siddon_grad_kernel(FwdGeom G, const FwdView* __restrict__ views,
                                                                   const float4* __restrict__ gvol,
                                                                   const float* __restrict__ upstream,
                                                                   float* __restrict__ partials) {
@@ -161,20 +181,14 @@ __global__ void __launch_bounds__(kFwdThreads) siddon_grad_kernel(FwdGeom G, con
   float out[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   if (live) {
     const SiddonRay r = siddon_setup(G, views[view], iu, iv, nullptr);
-    const int nx = G.L.nx, ny = G.L.ny, nz = G.L.nz;
-    const GradBricks B = GradBricks::make(nx, ny, nz);
-    // voxel centre r'_j = c + (i - (n-1)/2) v
-    const float hx = 0.5f * (float)(nx - 1), hy = 0.5f * (float)(ny - 1), hz = 0.5f * (float)(nz - 1);
     float ax_ = 0.f, ay_ = 0.f, az_ = 0.f, bx = 0.f, by = 0.f, bz = 0.f;     // A_i, B_i
     if (r.hit) {
-      SiddonState s = siddon_state(r, nx, ny);
-      s.fx = B.FX(s.ix); s.fy = B.FY(s.iy); s.fz = B.FZ(s.iz);
+      SiddonState s = siddon_state<true>(r, G);
       bool alive = true;
       while (alive) {
-        const float4 g = ldg4(gvol + (s.fx + s.fy + s.fz));
-        const float rx = fmaf((float)s.ix - hx, G.vx, G.cx), ry = fmaf((float)s.iy - hy, G.vy, G.cy),
-                    rz = fmaf((float)s.iz - hz, G.vz, G.cz);
-        const float len = siddon_step<true>(s, nx, ny, nz, B, alive);
+        const float4 g = ldg4(gvol + s.idx);
+        const float rx = s.px, ry = s.py, rz = s.pz;
+        const float len = siddon_step<true>(s, alive);
         const float lx = len * g.x, ly = len * g.y, lz = len * g.z;          // a^ij g_j
         ax_ += lx; ay_ += ly; az_ += lz;
         bx += ry * lz - rz * ly;
