@@ -25,6 +25,7 @@ struct SiddonRay {
   double t, tmax;              // current parameter (mm from the source) and exit parameter
   double tn[3], dt[3];         // next crossing of each plane family, spacing of the crossings
   int i[3], step[3];           // current voxel index, +-1 per axis
+  int nseg;                    // number of segments = plane crossings between entry and exit + 1
   bool hit;
 };
 
@@ -56,12 +57,17 @@ __device__ __forceinline__ SiddonRay siddon_setup(const FwdGeom& G, const FwdVie
   if (!(tmax > tmin)) r.hit = false;
   r.t = tmin;
   r.tmax = tmax;
+  r.nseg = 1;
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
     const double p = V.src[a] + tmin * e[a];
     int i = (int)floor((p - lo[a]) / v[a]);
     i = min(max(i, 0), n[a] - 1);
     r.i[a] = i;
+    // voxel of the exit point: every plane of family a between the two indices is crossed once
+    int ie = (int)floor((V.src[a] + fmin(tmax, 1e30) * e[a] - lo[a]) / v[a]);
+    ie = min(max(ie, 0), n[a] - 1);
+    r.nseg += abs(ie - i);
     if (fabs(e[a]) < 1e-300) {
       r.step[a] = 0; r.dt[a] = 1e300; r.tn[a] = 1e300;
     } else {
@@ -74,17 +80,20 @@ __device__ __forceinline__ SiddonRay siddon_setup(const FwdGeom& G, const FwdVie
   return r;
 }
 
-// One DDA step: returns the length of the segment inside the current voxel, then advances index, linear offset and
-// the crossed family's counter.  `alive` turns false once the ray has left the grid: the grid's faces are planes of
-// the three families, so the ray ends exactly at a crossing.
+// One DDA step: returns the length of the segment inside the current voxel, then advances the voxel offset and the
+// crossed family's distance.
 // The state keeps, per family, the distance from the CURRENT point to the next crossing (fp32, at most one crossing
 // spacing, a few mm): a segment length is then the minimum of three small numbers, known to ~1e-7 relative, and
 // the subtraction r_a - len is exact or rounds at 1e-7 of a spacing - no fp64 and no large parameter in the loop
 // (the per-ray set-up, which does subtract parameters of ~1000 mm, runs in fp64).
-// Written with selects on named scalars (an array indexed by the crossed axis would live in local memory).
+// The loop runs SiddonRay::nseg times (counted by the fp64 set-up from the entry and exit voxels).  Where two
+// crossings coincide to within the fp32 drift of the distances (~1e-5 mm) the loop may take them in the other order
+// or count one more / fewer than the set-up did; every segment this misplaces is that short, and the voxel offset
+// is clamped to the volume (clamp_offset), so such a step reads a valid voxel with a ~1e-5 mm weight.
+// Branch-free on purpose: the three families take turns within a warp, and an if / else form compiled to a
+// divergent branch with a dozen register moves per step.
 struct SiddonState {
   float rx, ry, rz, dtx, dty, dtz;       // distance to the next x / y / z plane; spacing of the crossings
-  int nx_, ny_, nz_;                     // crossings of each family left before the ray leaves the grid
   int idx, stx, sty, stz;                // offset of the voxel and its step per family: linear in the caller's volume
                                          // (forward); GradBricks index and the step of the NEXT crossing (gradient)
   int ttx, tty, ttz;                     // gradient: step of this crossing + step of the following one (they alternate
@@ -98,9 +107,6 @@ __device__ __forceinline__ SiddonState siddon_state(const SiddonRay& r, const Fw
   s.rx = (float)fmin(r.tn[0] - r.t, 1e30); s.ry = (float)fmin(r.tn[1] - r.t, 1e30); s.rz = (float)fmin(r.tn[2] - r.t, 1e30);
   s.dtx = (float)fmin(r.dt[0], 1e30); s.dty = (float)fmin(r.dt[1], 1e30); s.dtz = (float)fmin(r.dt[2], 1e30);
   const int ix = r.i[0], iy = r.i[1], iz = r.i[2], sx = r.step[0], sy = r.step[1], sz = r.step[2];
-  s.nx_ = sx > 0 ? nx - ix : ix + 1;                // a family with step 0 is never crossed (its distance is 1e30)
-  s.ny_ = sy > 0 ? ny - iy : iy + 1;
-  s.nz_ = sz > 0 ? nz - iz : iz + 1;
   if (!BRICK) {
     s.idx = (iz * ny + iy) * nx + ix;
     s.stx = sx; s.sty = sy * nx; s.stz = sz * nx * ny;
@@ -117,10 +123,11 @@ __device__ __forceinline__ SiddonState siddon_state(const SiddonRay& r, const Fw
   }
   return s;
 }
-// Branch-free on purpose: the three families take turns within a warp, and the if / else form compiled to a
-// divergent branch with a dozen register moves per step.
+// offset into [0, last]: a negative offset wraps to a large unsigned number and lands on `last`
+__device__ __forceinline__ unsigned clamp_offset(int idx, unsigned last) { return min((unsigned)idx, last); }
+
 template <bool BRICK>
-__device__ __forceinline__ float siddon_step(SiddonState& s, bool& alive) {
+__device__ __forceinline__ float siddon_step(SiddonState& s) {
   const bool cx = s.rx <= s.ry && s.rx <= s.rz;
   const bool cy = !cx && s.ry <= s.rz;
   const bool cz = !cx && !cy;
@@ -128,10 +135,6 @@ __device__ __forceinline__ float siddon_step(SiddonState& s, bool& alive) {
   s.rx = cx ? s.dtx : s.rx - len;
   s.ry = cy ? s.dty : s.ry - len;
   s.rz = cz ? s.dtz : s.rz - len;
-  if (cx) --s.nx_;
-  if (cy) --s.ny_;
-  if (cz) --s.nz_;
-  alive = (cx ? s.nx_ : (cy ? s.ny_ : s.nz_)) != 0;
   s.idx += cx ? s.stx : (cy ? s.sty : s.stz);
   if (BRICK) {
     s.stx = cx ? s.ttx - s.stx : s.stx;
@@ -156,10 +159,10 @@ __global__ void __launch_bounds__(kFwdThreads, 6) siddon_fwd_kernel(FwdGeom G, c
   float sum = 0.f;
   if (r.hit) {
     SiddonState s = siddon_state<false>(r, G);
-    bool alive = true;
-    while (alive) {
-      const float val = __ldg(vol + s.idx);
-      const float len = siddon_step<false>(s, alive);
+    const unsigned last = (unsigned)(G.L.nx * G.L.ny * G.L.nz) - 1u;
+    for (int n = r.nseg; n > 0; --n) {
+      const float val = __ldg(vol + clamp_offset(s.idx, last));
+      const float len = siddon_step<false>(s);
       sum = fmaf(len, val, sum);
     }
   }
@@ -184,11 +187,11 @@ __global__ void __launch_bounds__(kFwdThreads, 5) siddon_grad_kernel(FwdGeom G, 
     float ax_ = 0.f, ay_ = 0.f, az_ = 0.f, bx = 0.f, by = 0.f, bz = 0.f;     // A_i, B_i
     if (r.hit) {
       SiddonState s = siddon_state<true>(r, G);
-      bool alive = true;
-      while (alive) {
-        const float4 g = ldg4(gvol + s.idx);
+      const unsigned last = (unsigned)GradBricks::make(G.L.nx, G.L.ny, G.L.nz).cells() - 1u;
+      for (int n = r.nseg; n > 0; --n) {
+        const float4 g = ldg4(gvol + clamp_offset(s.idx, last));
         const float rx = s.px, ry = s.py, rz = s.pz;
-        const float len = siddon_step<true>(s, alive);
+        const float len = siddon_step<true>(s);
         const float lx = len * g.x, ly = len * g.y, lz = len * g.z;          // a^ij g_j
         ax_ += lx; ay_ += ly; az_ += lz;
         bx += ry * lz - rz * ly;
