@@ -535,8 +535,17 @@ def test_siddon_ragged_anisotropic_and_degenerate(dfp):
     vol = rng.random(g.vol_shape).astype(np.float32)
     up = rng.standard_normal((1,) + g.det_shape).astype(np.float32)
     check_forward(run_siddon_case(dfp, g, [0.0], [[0] * 6], vol, up))
+    # diagonal views of an even grid: the middle ray runs through voxel CORNERS (x and y planes crossed together, to
+    # within rounding of cos / sin) inside the plane z = 0 - coincident crossings, which the DDA may take in either
+    # order or count differently from its fp64 set-up (zero-length segments either way)
+    g = small_geom(n=16, nu=11, nv=9)
+    vol = rng.random(g.vol_shape).astype(np.float32)
+    diag = [math.pi / 4, 3 * math.pi / 4, -math.pi / 4, 5 * math.pi / 4]
+    up4 = rng.standard_normal((4,) + g.det_shape).astype(np.float32)
+    check_forward(run_siddon_case(dfp, g, diag, [[0] * 6] * 4, vol, up4))
+    g = small_geom(n=12, nu=11, nv=9)
     # misses and an empty volume: exact zeros
-    proj, grad, _, _ = run_siddon_case(dfp, g, [0.3], [[0, 0, 700.0, 0, 0, 0]], vol, up)
+    proj, grad, _, _ = run_siddon_case(dfp, g, [0.3], [[0, 0, 700.0, 0, 0, 0]], vol[:12, :12, :12].copy(), up)
     assert np.all(proj == 0) and np.all(grad == 0)
     # single voxel
     g1 = small_geom(n=1, voxel=4.0, nu=3, nv=3, pix=1.0)
