@@ -82,17 +82,21 @@ def _p(a):
     return a.ctypes.data_as(ctypes.c_void_p)
 
 
-def _views(angles, poses):
+FLAG_VIEW_FRAMES = 64    # O14: `angles` holds [V][12] view frames (s, c, U, V) instead of [V] gantry angles
+
+
+def _views(angles, poses, g):
     angles = _f64(angles).reshape(-1)
     poses = _f64(poses).reshape(-1, 6)
-    assert poses.shape[0] == angles.shape[0]
-    return angles, poses, int(angles.shape[0])
+    per_view = 12 if (int(_geom(g).flags) & FLAG_VIEW_FRAMES) else 1
+    assert angles.shape[0] == per_view * poses.shape[0]
+    return angles, poses, int(poses.shape[0])
 
 
 def forward(g, angles, poses, vol, return_steps=False):
     """O6.  vol [nz,ny,nx] float32 or float64 -> proj [V,nv,nu] float64 (and the ray-step count)."""
     lib = _load()
-    angles, poses, V = _views(angles, poses)
+    angles, poses, V = _views(angles, poses, g)
     if hasattr(vol, "detach"):
         vol = vol.detach().cpu().numpy()
     gg = _geom(g)
@@ -112,7 +116,7 @@ def forward(g, angles, poses, vol, return_steps=False):
 def forward_T(g, angles, poses, y):
     """O10: explicit transpose of `forward` (adjointness pin).  y [V,nv,nu] -> vol float64."""
     lib = _load()
-    angles, poses, V = _views(angles, poses)
+    angles, poses, V = _views(angles, poses, g)
     gg = _geom(g)
     y = _f64(y, (V, gg.nv, gg.nu))
     out = np.empty((gg.nz, gg.ny, gg.nx), dtype=np.float64)
@@ -124,7 +128,7 @@ def forward_pose_grad(g, angles, poses, vol, upstream, lever_arm=LEVER_SAMPLE, g
                       route=ROUTE_SIX):
     """O7.  upstream [V,nv,nu] float32 -> dL/dtheta [V,6] float64."""
     lib = _load()
-    angles, poses, V = _views(angles, poses)
+    angles, poses, V = _views(angles, poses, g)
     gg = _geom(g)
     if hasattr(vol, "detach"):
         vol = vol.detach().cpu().numpy()
@@ -145,7 +149,7 @@ def forward_pose_grad(g, angles, poses, vol, upstream, lever_arm=LEVER_SAMPLE, g
 def backproject(g, angles, poses, proj, iz0=0, iz1=None):
     """O8.  proj [V,nv,nu] float32 -> vol[iz0:iz1] float64."""
     lib = _load()
-    angles, poses, V = _views(angles, poses)
+    angles, poses, V = _views(angles, poses, g)
     gg = _geom(g)
     iz1 = gg.nz if iz1 is None else iz1
     proj = _f32(proj).reshape(V, gg.nv, gg.nu)
@@ -157,7 +161,7 @@ def backproject(g, angles, poses, proj, iz0=0, iz1=None):
 def backproject_T(g, angles, poses, x):
     """O10: explicit transpose of `backproject` (splat), adjointness pin.  x [nz,ny,nx] -> [V,nv,nu] float64."""
     lib = _load()
-    angles, poses, V = _views(angles, poses)
+    angles, poses, V = _views(angles, poses, g)
     gg = _geom(g)
     x = _f64(x, (gg.nz, gg.ny, gg.nx))
     out = np.empty((V, gg.nv, gg.nu), dtype=np.float64)
@@ -168,7 +172,7 @@ def backproject_T(g, angles, poses, x):
 def backproject_pose_grad(g, angles, poses, proj, upstream, grad_mode=GRAD_CENTRAL, route=ROUTE_SIX):
     """O9.  proj [V,nv,nu] float32, upstream [nz,ny,nx] float32 -> dL/dtheta [V,6] float64."""
     lib = _load()
-    angles, poses, V = _views(angles, poses)
+    angles, poses, V = _views(angles, poses, g)
     gg = _geom(g)
     proj = _f32(proj).reshape(V, gg.nv, gg.nu)
     up = _f32(upstream).reshape(gg.nz, gg.ny, gg.nx)
@@ -188,11 +192,14 @@ def rotation(pose6):
 
 
 def projection_matrix(g, angle):
-    """P [3,4] in pixel-index units (O5, Eq.1)."""
+    """P [3,4] in pixel-index units (O5 / O14, Eq.1).  `angle`: gantry angle, or a 12-number view frame
+    when the geometry carries FLAG_VIEW_FRAMES."""
     lib = _load()
     gg = _geom(g)
+    view = _f64(angle).reshape(-1)
+    assert view.shape[0] == (12 if (int(gg.flags) & FLAG_VIEW_FRAMES) else 1)
     P = np.empty((3, 4))
-    lib.ora_projection_matrix(ctypes.byref(gg), ctypes.c_double(float(angle)), _p(P))
+    lib.ora_projection_matrix(ctypes.byref(gg), _p(view), _p(P))
     return P
 
 
@@ -201,7 +208,7 @@ def projection_matrix(g, angle):
 def forward_siddon(g, angles, poses, vol):
     """l_i = sum_j a^ij mu_j, a^ij = length of ray i inside voxel j.  vol [nz,ny,nx] -> proj [V,nv,nu] float64."""
     lib = _load()
-    angles, poses, V = _views(angles, poses)
+    angles, poses, V = _views(angles, poses, g)
     if hasattr(vol, "detach"):
         vol = vol.detach().cpu().numpy()
     gg = _geom(g)
@@ -220,7 +227,7 @@ def forward_siddon(g, angles, poses, vol):
 def forward_siddon_T(g, angles, poses, y):
     """Explicit transpose of `forward_siddon` (adjointness pin).  y [V,nv,nu] -> vol float64."""
     lib = _load()
-    angles, poses, V = _views(angles, poses)
+    angles, poses, V = _views(angles, poses, g)
     gg = _geom(g)
     y = _f64(y, (V, gg.nv, gg.nu))
     out = np.empty((gg.nz, gg.ny, gg.nx), dtype=np.float64)
@@ -231,7 +238,7 @@ def forward_siddon_T(g, angles, poses, y):
 def forward_pose_grad_siddon(g, angles, poses, vol, upstream, route=ROUTE_SIX):
     """Pose gradient with Siddon weights and per-voxel G_f^j (Eq.19-20, :189).  -> [V,6] float64."""
     lib = _load()
-    angles, poses, V = _views(angles, poses)
+    angles, poses, V = _views(angles, poses, g)
     gg = _geom(g)
     if hasattr(vol, "detach"):
         vol = vol.detach().cpu().numpy()
@@ -252,7 +259,7 @@ def forward_pose_grad_siddon(g, angles, poses, vol, upstream, route=ROUTE_SIX):
 # O13: Joseph's projector (plane-by-plane along the driving axis, bilinear in each plane)
 def _model_call(name, g, angles, poses, vol, extra=()):
     lib = _load()
-    angles, poses, V = _views(angles, poses)
+    angles, poses, V = _views(angles, poses, g)
     if hasattr(vol, "detach"):
         vol = vol.detach().cpu().numpy()
     gg = _geom(g)
@@ -277,7 +284,7 @@ def forward_joseph(g, angles, poses, vol):
 def forward_joseph_T(g, angles, poses, y):
     """Explicit transpose of `forward_joseph` (adjointness pin).  y [V,nv,nu] -> vol float64."""
     lib = _load()
-    angles, poses, V = _views(angles, poses)
+    angles, poses, V = _views(angles, poses, g)
     gg = _geom(g)
     y = _f64(y, (V, gg.nv, gg.nu))
     out = np.empty((gg.nz, gg.ny, gg.nx), dtype=np.float64)

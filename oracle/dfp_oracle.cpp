@@ -16,7 +16,11 @@
 // stored-G algorithm, finite differences of closed-form projections; Joseph weights (O13,
 // tests/test_oracle_joseph.py): hand formulas for constant and in-plane-linear volumes, explicit
 // transpose, closed forms with second-order convergence on all three driving axes, stored-G,
-// finite differences of closed-form projections.
+// finite differences of closed-form projections; explicit view frames (O14,
+// tests/test_oracle_view_frames.py): Eq.1 on the source -> pixel lines of tilted / skewed / shifted
+// detectors, closed-form blobs under a general frame, the frame of a circular view against the
+// circular path, scanner and object moved together, finite differences of the discrete projector /
+// back-projector under a general frame.
 // No function here is "parity unpinned".
 //
 // Conventions:
@@ -96,17 +100,47 @@ struct Pose {
   }
 };
 
-// O5: one view of the circular cone-beam scanner.
+// O5: one view of the scanner.  Default: circular cone-beam orbit, gantry angle `views[v]`.
+// O14 (flags & 64, "view frames"; SURVEY.md 8b optional extension, PAPER.md :244 non-circular orbit): `views` holds
+// 12 numbers per view, world frame, mm: source s, detector reference point c (where the pixel index is (c_u, c_v)),
+// and the displacements U, V of one pixel step along u and along v (any flat detector; U, V need not be orthogonal).
+//   pixel (iu,iv) centre = c + (iu - c_u) U + (iv - c_v) V                                       (definition)
+//   P (Eq.1 :60-63, pixel-index units) follows from intersecting the line s -> r with the detector plane:
+//   nh = unit normal of the plane on the far side of the source, w' = (r - s).nh (depth in mm, as in the circular
+//   case), SDD_v = (c - s).nh, and with the dual vectors U* = (V x nh)/(U.(V x nh)), V* = (nh x U)/(V.(nh x U))
+//   (U*.U = 1, U*.V = 0):  u = c_u + (x - c).U*  at  x = s + (SDD_v / w')(r - s), i.e.
+//   P_3 = (nh | -nh.s),  P_1 = SDD_v (U* | -U*.s) + (c_u - (c - s).U*) P_3,  P_2 likewise with V*, c_v.
 struct View {
-  V3 n, s, dc, eu, ev; double P[3][4]; double cu, cv;
-  View(const ora_geom& g, double beta) {
-    n = {cos(beta), sin(beta), 0.0};
-    s = g.sad * n;
-    dc = -(g.sdd - g.sad) * n;
-    eu = {-sin(beta), cos(beta), 0.0};
-    ev = {0.0, 0.0, 1.0};
+  V3 s, dc, U, Vs; double P[3][4]; double cu, cv;
+  View(const ora_geom& g, const double* views, int v) {
     cu = (g.nu - 1) / 2.0 + g.u0;
     cv = (g.nv - 1) / 2.0 + g.v0;
+    if (g.flags & 64) {
+      const double* f = views + 12 * (size_t)v;
+      s = {f[0], f[1], f[2]}; dc = {f[3], f[4], f[5]}; U = {f[6], f[7], f[8]}; Vs = {f[9], f[10], f[11]};
+      V3 nh = cross(U, Vs);
+      nh = (1.0 / sqrt(dot(nh, nh))) * nh;
+      if (dot(dc - s, nh) < 0) nh = -1.0 * nh;
+      const double sddv = dot(dc - s, nh);
+      V3 Ud = cross(Vs, nh); Ud = (1.0 / dot(U, Ud)) * Ud;
+      V3 Vd = cross(nh, U); Vd = (1.0 / dot(Vs, Vd)) * Vd;
+      double P3[4] = {nh.x, nh.y, nh.z, -dot(nh, s)};
+      double e1[4] = {Ud.x, Ud.y, Ud.z, -dot(Ud, s)}, e2[4] = {Vd.x, Vd.y, Vd.z, -dot(Vd, s)};
+      const double ou = cu - dot(dc - s, Ud), ov = cv - dot(dc - s, Vd);
+      for (int k = 0; k < 4; ++k) {
+        P[2][k] = P3[k];
+        P[0][k] = sddv * e1[k] + ou * P3[k];
+        P[1][k] = sddv * e2[k] + ov * P3[k];
+      }
+      return;
+    }
+    const double beta = views[v];
+    V3 n = {cos(beta), sin(beta), 0.0};
+    s = g.sad * n;
+    dc = -(g.sdd - g.sad) * n;
+    V3 eu = {-sin(beta), cos(beta), 0.0}, ev = {0.0, 0.0, 1.0};
+    U = g.du * eu;
+    Vs = g.dv * ev;
     double P3[4] = {-n.x, -n.y, -n.z, g.sad};
     double e1[4] = {eu.x, eu.y, eu.z, 0.0}, e2[4] = {ev.x, ev.y, ev.z, 0.0};
     for (int k = 0; k < 4; ++k) {
@@ -116,7 +150,8 @@ struct View {
     }
   }
   V3 pixel(const ora_geom& g, int iu, int iv) const {
-    return dc + ((iu - cu) * g.du) * eu + ((iv - cv) * g.dv) * ev;
+    (void)g;
+    return dc + (iu - cu) * U + (iv - cv) * Vs;
   }
 };
 
@@ -216,7 +251,7 @@ void forward_impl(const ora_geom& g, int n_views, const double* angles, const do
   const double D = step_of(g);
   int64_t total_steps = 0;
   for (int v = 0; v < n_views; ++v) {
-    View view(g, angles[v]);
+    View view(g, angles, v);
     Pose pose(poses + 6 * v);
     int64_t steps_v = 0;
 #pragma omp parallel for schedule(dynamic, 4) reduction(+ : steps_v)
@@ -256,7 +291,7 @@ void forward_T_impl(const ora_geom& g, int n_views, const double* angles, const 
   size_t nvox = (size_t)g.nx * g.ny * g.nz;
   for (size_t i = 0; i < nvox; ++i) vol_out[i] = 0.0;
   for (int v = 0; v < n_views; ++v) {
-    View view(g, angles[v]);
+    View view(g, angles, v);
     Pose pose(poses + 6 * v);
     for (int iv = 0; iv < g.nv; ++iv) for (int iu = 0; iu < g.nu; ++iu) {
       double yi = (double)y[((size_t)v * g.nv + iv) * g.nu + iu];
@@ -307,7 +342,7 @@ void forward_grad_impl(const ora_geom& g, int n_views, const double* angles, con
   Vol<T> V{vol, g.nx, g.ny, g.nz};
   const double D = step_of(g);
   for (int v = 0; v < n_views; ++v) {
-    View view(g, angles[v]);
+    View view(g, angles, v);
     Pose pose(poses + 6 * v);
     // per-row partial sums, added in row order afterwards (deterministic)
     std::vector<double> rowacc((size_t)g.nv * 12, 0.0);
@@ -420,7 +455,7 @@ inline double bilin(const Img& I, double u, double v) {
 void backproject_impl(const ora_geom& g, int n_views, const double* angles, const double* poses,
                       const float* proj, double* vol_out, int iz0, int iz1) {
   std::vector<View> views; std::vector<Pose> ps;
-  for (int v = 0; v < n_views; ++v) { views.emplace_back(g, angles[v]); ps.emplace_back(poses + 6 * v); }
+  for (int v = 0; v < n_views; ++v) { views.emplace_back(g, angles, v); ps.emplace_back(poses + 6 * v); }
 #pragma omp parallel for schedule(dynamic, 1) collapse(2)
   for (int iz = iz0; iz < iz1; ++iz) for (int iy = 0; iy < g.ny; ++iy) for (int ix = 0; ix < g.nx; ++ix) {
     V3 rp = voxel_centre(g, ix, iy, iz);
@@ -446,7 +481,7 @@ void backproject_T_impl(const ora_geom& g, int n_views, const double* angles, co
   size_t np = (size_t)n_views * g.nu * g.nv;
   for (size_t i = 0; i < np; ++i) proj_out[i] = 0.0;
   for (int v = 0; v < n_views; ++v) {
-    View view(g, angles[v]); Pose pose(poses + 6 * v);
+    View view(g, angles, v); Pose pose(poses + 6 * v);
     double* out = proj_out + (size_t)v * g.nu * g.nv;
     for (int iz = 0; iz < g.nz; ++iz) for (int iy = 0; iy < g.ny; ++iy) for (int ix = 0; ix < g.nx; ++ix) {
       V3 r = mul(pose.R, voxel_centre(g, ix, iy, iz)) + pose.t;
@@ -481,7 +516,7 @@ void backproject_T_impl(const ora_geom& g, int n_views, const double* angles, co
 void backproject_grad_impl(const ora_geom& g, int n_views, const double* angles, const double* poses,
                            const float* proj, const float* upstream, double* grad, int grad_mode, int route) {
   for (int v = 0; v < n_views; ++v) {
-    View view(g, angles[v]); Pose pose(poses + 6 * v);
+    View view(g, angles, v); Pose pose(poses + 6 * v);
     Img I{proj + (size_t)v * g.nu * g.nv, g.nu, g.nv};
     const double(*P)[4] = view.P;
     std::vector<double> slab((size_t)g.nz * 12, 0.0);
@@ -602,7 +637,7 @@ void forward_siddon_impl(const ora_geom& g, int n_views, const double* angles, c
   const bool transpose = vol_out != nullptr;
   if (transpose) for (size_t i = 0; i < (size_t)g.nx * g.ny * g.nz; ++i) vol_out[i] = 0.0;
   for (int v = 0; v < n_views; ++v) {
-    View view(g, angles[v]);
+    View view(g, angles, v);
     Pose pose(poses + 6 * v);
     const V3 so = mulT(pose.R, view.s - pose.t);
 #pragma omp parallel for schedule(dynamic, 4) if (!transpose)
@@ -635,7 +670,7 @@ void forward_grad_siddon_impl(const ora_geom& g, int n_views, const double* angl
                               const float* upstream, double* grad, int route) {
   Vol<T> V{vol, g.nx, g.ny, g.nz};
   for (int v = 0; v < n_views; ++v) {
-    View view(g, angles[v]);
+    View view(g, angles, v);
     Pose pose(poses + 6 * v);
     const V3 so = mulT(pose.R, view.s - pose.t);
     std::vector<double> rowacc((size_t)g.nv * 12, 0.0);
@@ -743,7 +778,7 @@ void forward_joseph_impl(const ora_geom& g, int n_views, const double* angles, c
   const bool transpose = vol_out != nullptr;
   if (transpose) for (size_t i = 0; i < (size_t)g.nx * g.ny * g.nz; ++i) vol_out[i] = 0.0;
   for (int v = 0; v < n_views; ++v) {
-    View view(g, angles[v]);
+    View view(g, angles, v);
     Pose pose(poses + 6 * v);
     const V3 so = mulT(pose.R, view.s - pose.t);
 #pragma omp parallel for schedule(dynamic, 4) if (!transpose)
@@ -773,7 +808,7 @@ void forward_grad_joseph_impl(const ora_geom& g, int n_views, const double* angl
                               const float* upstream, double* grad) {
   Vol<T> V{vol, g.nx, g.ny, g.nz};
   for (int v = 0; v < n_views; ++v) {
-    View view(g, angles[v]);
+    View view(g, angles, v);
     Pose pose(poses + 6 * v);
     const V3 so = mulT(pose.R, view.s - pose.t);
     std::vector<double> rowacc((size_t)g.nv * 6, 0.0);
@@ -872,8 +907,9 @@ void ora_rotation(const double* pose6, double* R9, double* dR27) {
   }
 }
 // Projection matrix P (pixel-index units) of a view, exposed so the tests can pin Eq.1.
-void ora_projection_matrix(const ora_geom* g, double angle, double* P12) {
-  View v(*g, angle);
+// `view`: one gantry angle, or (flags & 64) one 12-number view frame.
+void ora_projection_matrix(const ora_geom* g, const double* view, double* P12) {
+  View v(*g, view, 0);
   for (int i = 0; i < 3; ++i) for (int j = 0; j < 4; ++j) P12[i * 4 + j] = v.P[i][j];
 }
 

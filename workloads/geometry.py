@@ -30,7 +30,7 @@ class Geometry:
     v0: float = 0.0
     step_mm: float = 0.0      # <=0: min(vx,vy,vz)
     bp_weight: int = 0        # 0 unit, 1 FDK (sad/w')^2
-    flags: int = 0            # bit0: add dW/dtheta term in backproject_pose_grad
+    flags: int = 0            # bit0: add dW/dtheta term in backproject_pose_grad; bit6 (64): views are 12-number frames
 
     def replace(self, **kw) -> "Geometry":
         return dataclasses.replace(self, **kw)
@@ -55,3 +55,24 @@ def view_angles(n_views: int, arc_deg: float = 360.0, start_deg: float = 0.0) ->
     """Gantry angles in radians, evenly spaced over `arc_deg` (end point excluded), float64."""
     k = torch.arange(n_views, dtype=torch.float64)
     return (start_deg + arc_deg * k / n_views) * (math.pi / 180.0)
+
+
+FLAG_VIEW_FRAMES = 64   # dfp_geometry.flags bit6: the view array holds [V][12] frames instead of [V] gantry angles
+
+
+def circular_frame(geom: Geometry, angle: float) -> torch.Tensor:
+    """The 12 numbers (source s, detector reference point c, pixel steps U, V; world frame, mm) that describe the
+    circular-orbit view of gantry angle `angle` (include/dfp.h conventions), float64."""
+    cb, sb = math.cos(angle), math.sin(angle)
+    n = torch.tensor([cb, sb, 0.0], dtype=torch.float64)
+    return torch.cat([geom.sad * n, -(geom.sdd - geom.sad) * n,
+                      geom.du * torch.tensor([-sb, cb, 0.0], dtype=torch.float64),
+                      geom.dv * torch.tensor([0.0, 0.0, 1.0], dtype=torch.float64)])
+
+
+def move_frame(frame, Q, tau) -> torch.Tensor:
+    """The scanner of `frame` moved rigidly as a whole: points x -> Q x + tau, directions d -> Q d."""
+    f = torch.as_tensor(frame, dtype=torch.float64).reshape(4, 3)
+    Q = torch.as_tensor(Q, dtype=torch.float64)
+    tau = torch.as_tensor(tau, dtype=torch.float64)
+    return torch.cat([Q @ f[0] + tau, Q @ f[1] + tau, Q @ f[2], Q @ f[3]])

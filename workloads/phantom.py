@@ -113,23 +113,31 @@ def voxelise_blobs(geom: Geometry, blobs: Sequence[Ellipsoid], device="cpu") -> 
     return vol.to(torch.float32)
 
 
-def _object_frame_rays(geom: Geometry, angle: float, pose, device, rows=None):
-    """Source position s' [3] and unit directions e' [nrows,nu,3] in the OBJECT frame for one view."""
+def _object_frame_rays(geom: Geometry, angle, pose, device, rows=None):
+    """Source position s' [3] and unit directions e' [nrows,nu,3] in the OBJECT frame for one view.
+    `angle`: a gantry angle (circular orbit) or a 12-number view frame (s, c, U, V; workloads.circular_frame)."""
     pose = [float(p) for p in pose]
     R = rotation_zyx(pose[3], pose[4], pose[5], device)
     t = torch.tensor(pose[:3], dtype=torch.float64, device=device)
-    cb, sb = math.cos(angle), math.sin(angle)
-    n = torch.tensor([cb, sb, 0.0], dtype=torch.float64, device=device)
-    eu = torch.tensor([-sb, cb, 0.0], dtype=torch.float64, device=device)
-    ev = torch.tensor([0.0, 0.0, 1.0], dtype=torch.float64, device=device)
-    s = geom.sad * n
-    dc = -(geom.sdd - geom.sad) * n
     cu = (geom.nu - 1) / 2.0 + geom.u0
     cv = (geom.nv - 1) / 2.0 + geom.v0
     iu = torch.arange(geom.nu, dtype=torch.float64, device=device)
     iv = torch.arange(geom.nv, dtype=torch.float64, device=device) if rows is None else \
         torch.as_tensor(rows, dtype=torch.float64, device=device)
-    pix = dc[None, None, :] + ((iu - cu) * geom.du)[None, :, None] * eu + ((iv - cv) * geom.dv)[:, None, None] * ev
+    if not isinstance(angle, (int, float)) and len(torch.as_tensor(angle).reshape(-1)) == 12:
+        f = torch.as_tensor(angle, dtype=torch.float64, device=device).reshape(4, 3)
+        s, dc = f[0], f[1]
+        pix = dc[None, None, :] + (iu - cu)[None, :, None] * f[2] + (iv - cv)[:, None, None] * f[3]
+    else:
+        angle = float(angle)
+        cb, sb = math.cos(angle), math.sin(angle)
+        n = torch.tensor([cb, sb, 0.0], dtype=torch.float64, device=device)
+        eu = torch.tensor([-sb, cb, 0.0], dtype=torch.float64, device=device)
+        ev = torch.tensor([0.0, 0.0, 1.0], dtype=torch.float64, device=device)
+        s = geom.sad * n
+        dc = -(geom.sdd - geom.sad) * n
+        pix = dc[None, None, :] + ((iu - cu) * geom.du)[None, :, None] * eu + \
+            ((iv - cv) * geom.dv)[:, None, None] * ev
     d = pix - s
     e = d / torch.linalg.norm(d, dim=-1, keepdim=True)
     s_obj = R.T @ (s - t)
