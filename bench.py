@@ -301,6 +301,23 @@ def main():
             b_.record()
             torch.cuda.synchronize()
             model_ms[name].append(a_.elapsed_time(b_) / 3)
+    # DFP_FLAG_VIEW_FRAMES: the four calls with one explicit (s, c, U, V) frame per view - the config's views on a
+    # seeded non-circular (saddle) orbit with detector wobble; same kernels, only the per-view set-up differs
+    gv = g.replace(flags=g.flags | dfp.FLAG_VIEW_FRAMES)
+    frames = W.noncircular_orbit(g, np.asarray(angles, dtype=np.float64), w.seed + 17).numpy().astype(np.float32)
+    frames_ms = []
+    for fn in (lambda: dfp.forward(gv, frames, poses, vol, out=proj, ws=ws),
+               lambda: dfp.forward_pose_grad(gv, frames, poses, vol, up, out=grad, ws=ws),
+               lambda: dfp.backproject(gv, frames, poses, proj, out=bvol, ws=ws),
+               lambda: dfp.backproject_pose_grad(gv, frames, poses, proj, bp_up, out=bgrad, ws=ws)):
+        fn()
+        a_, b_ = ev(), ev()
+        a_.record()
+        for _ in range(3):
+            fn()
+        b_.record()
+        torch.cuda.synchronize()
+        frames_ms.append(a_.elapsed_time(b_) / 3)
     dfp.forward(g, angles, poses, vol, out=proj, ws=ws)                        # restore the default-mode projections
     # dfp_forward_fused_moments: projection + gradient moments in one traversal (target = the upstream array's shape)
     ws_f = torch.empty(dfp.workspace_bytes(g, V, dfp.OP_FORWARD_FUSED), dtype=torch.uint8, device=dev)
@@ -421,6 +438,9 @@ def main():
                                                  "forward_pose_grad": model_ms["siddon"][1]},
                      "joseph_mode_ms_per_call": {"forward": model_ms["joseph"][0],
                                                  "forward_pose_grad": model_ms["joseph"][1]},
+                     "view_frames_mode_ms_per_call": {"forward": frames_ms[0], "forward_pose_grad": frames_ms[1],
+                                                      "backproject": frames_ms[2],
+                                                      "backproject_pose_grad": frames_ms[3]},
                      "forward_fused_moments_ms_per_call": fused_ms,
                      "forward_fused_moments_gray_steps_per_s": 2.0 * ray_steps / (fused_ms * 1e-3) / 1e9},
            "clocks": clocks, "e2e": e2e, "gpu_launches": n_launch, "roofline": roofline, "cpu_baseline": cpu}

@@ -14,6 +14,8 @@
  *   c_u = (nu-1)/2 + u0, c_v = (nv-1)/2 + v0;  d = p(r) of Eq.1 (:60-63) is in pixel-index units.
  *   Gradients [n_views][6] are dL/d(tx,ty,tz) per mm and dL/d(gx,gy,gz) per radian.
  *
+ *   With DFP_FLAG_VIEW_FRAMES the `angles` array holds one explicit frame (s, c, U, V: 12 floats) per view instead.
+ *
  * Pointer kinds.  `angles`, `poses`, `geometry`: HOST memory, read before the call returns.
  *   d_* : DEVICE memory owned by the caller (e.g. torch tensors), fp32, contiguous, 16-byte aligned; read /
  *   written asynchronously on `stream` (a cudaStream_t passed as void*, NULL = default stream) and must stay
@@ -67,7 +69,17 @@ typedef struct dfp_geometry {
                            together with DFP_FLAG_SIDDON;
                            bit4 (DFP_FLAG_ACCUMULATE): dfp_backproject ADDS the views' contribution to d_vol instead of
                            overwriting it, so that the sum over views (Eq.21) can be taken slice by slice of the view
-                           arrays (view chunking; a view-sharded multi-GPU reconstruction).  Other calls ignore it. */
+                           arrays (view chunking; a view-sharded multi-GPU reconstruction).  Other calls ignore it;
+                           bit6 (DFP_FLAG_VIEW_FRAMES): every call reads its `angles` argument as [n_views][12] explicit
+                           VIEW FRAMES instead of [n_views] gantry angles - per view, in the world frame and mm: the
+                           source s, the detector reference point c (where the pixel index is (c_u, c_v)), and the
+                           displacements U, V of one pixel step along u and v (a flat detector anywhere: tilted, shifted,
+                           |U| != |V|, U not orthogonal to V) - for non-circular orbits and per-view calibrated
+                           geometries (PAPER.md :244).  Pixel (iu,iv) centre = c + (iu-c_u) U + (iv-c_v) V; Eq.1's w' is
+                           the depth from the source along the detector normal in mm; du, dv and sdd are then unused and
+                           sad only scales the FDK weight (sad/w')^2.  A frame with U parallel to V or with the source
+                           in the detector plane is rejected (DFP_ERR_DIMS).  All kernels and both paths serve it
+                           (the per-view set-up is the only code that differs).                                   */
 } dfp_geometry;
 
 enum {
@@ -82,7 +94,7 @@ enum {
 enum { DFP_OP_FORWARD = 0, DFP_OP_FORWARD_POSE_GRAD = 1, DFP_OP_BACKPROJECT = 2, DFP_OP_BACKPROJECT_POSE_GRAD = 3,
        DFP_OP_FORWARD_FUSED = 4 };
 enum { DFP_FLAG_DW = 1, DFP_FLAG_NO_TMA = 2, DFP_FLAG_GRAD_INTERP = 4, DFP_FLAG_SIDDON = 8,
-       DFP_FLAG_ACCUMULATE = 16, DFP_FLAG_JOSEPH = 32 };
+       DFP_FLAG_ACCUMULATE = 16, DFP_FLAG_JOSEPH = 32, DFP_FLAG_VIEW_FRAMES = 64 };
 
 /* Forward projection, Eq.2a :67-69 discretised as Eq.18 :172-177 with a fixed-step, zero-extended
  * trilinear ray-march (U1): proj[v][iv][iu] = D * sum_k f~(R_v^T (s_v + (k+1/2) D e_i - t_v)).

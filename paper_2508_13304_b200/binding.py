@@ -20,6 +20,7 @@ FLAG_GRAD_INTERP = 4
 FLAG_SIDDON = 8
 FLAG_ACCUMULATE = 16
 FLAG_JOSEPH = 32
+FLAG_VIEW_FRAMES = 64      # `angles` arguments hold [V,12] explicit view frames (s, c, U, V), include/dfp.h
 PATH_GATHER, PATH_TMA = 0, 1
 
 
@@ -129,14 +130,16 @@ def _check(status):
         raise DfpError(status, status_string(status))
 
 
-def _views(angles, poses):
+def _views(angles, poses, geom):
+    """`angles`: [V] gantry angles, or [V,12] view frames (s, c, U, V) when geom.flags has FLAG_VIEW_FRAMES."""
     a = np.ascontiguousarray(np.asarray(torch.as_tensor(angles).cpu().numpy() if torch.is_tensor(angles) else angles,
                                         dtype=np.float32).reshape(-1))
     p = np.ascontiguousarray(np.asarray(torch.as_tensor(poses).cpu().numpy() if torch.is_tensor(poses) else poses,
                                         dtype=np.float32).reshape(-1, 6))
-    if p.shape[0] != a.shape[0]:
-        raise ValueError("angles and poses disagree on the number of views")
-    return a, p, int(a.shape[0])
+    per_view = 12 if (int(Geometry.of(geom).flags) & FLAG_VIEW_FRAMES) else 1
+    if a.shape[0] != per_view * p.shape[0]:
+        raise ValueError("angles / view frames and poses disagree on the number of views")
+    return a, p, int(p.shape[0])
 
 
 def _dev(t: torch.Tensor, shape, name):
@@ -173,7 +176,7 @@ def _np_ptr(a):
 def forward(geom, angles, poses, vol, out=None, ws=None):
     """dfp_forward: vol [nz,ny,nx] cuda fp32 -> proj [V,nv,nu]."""
     g = Geometry.of(geom)
-    a, p, V = _views(angles, poses)
+    a, p, V = _views(angles, poses, geom)
     if out is None:
         out = torch.empty((V, g.nv, g.nu), dtype=torch.float32, device=vol.device)
     ws, wp, wn = _workspace(g, V, OP_FORWARD, ws, vol.device)
@@ -185,7 +188,7 @@ def forward(geom, angles, poses, vol, out=None, ws=None):
 def forward_pose_grad(geom, angles, poses, vol, dLdproj, out=None, ws=None):
     """dfp_forward_pose_grad: vol, dL/dproj [V,nv,nu] -> dL/dtheta [V,6]."""
     g = Geometry.of(geom)
-    a, p, V = _views(angles, poses)
+    a, p, V = _views(angles, poses, geom)
     if out is None:
         out = torch.empty((V, 6), dtype=torch.float32, device=vol.device)
     ws, wp, wn = _workspace(g, V, OP_FORWARD_POSE_GRAD, ws, vol.device)
@@ -199,7 +202,7 @@ def forward_pose_grad(geom, angles, poses, vol, dLdproj, out=None, ws=None):
 def forward_fused_moments(geom, angles, poses, vol, target, out_proj=None, out_moments=None, ws=None):
     """dfp_forward_fused_moments: vol, target [V,nv,nu] -> (proj [V,nv,nu], moments [V,3,6]) in one traversal."""
     g = Geometry.of(geom)
-    a, p, V = _views(angles, poses)
+    a, p, V = _views(angles, poses, geom)
     if out_proj is None:
         out_proj = torch.empty((V, g.nv, g.nu), dtype=torch.float32, device=vol.device)
     if out_moments is None:
@@ -216,7 +219,7 @@ def forward_fused_moments(geom, angles, poses, vol, target, out_proj=None, out_m
 def backproject(geom, angles, poses, proj, out=None, ws=None):
     """dfp_backproject: proj [V,nv,nu] cuda fp32 -> vol [nz,ny,nx]."""
     g = Geometry.of(geom)
-    a, p, V = _views(angles, poses)
+    a, p, V = _views(angles, poses, geom)
     if out is None:
         out = torch.empty((g.nz, g.ny, g.nx), dtype=torch.float32, device=proj.device)
     ws, wp, wn = _workspace(g, V, OP_BACKPROJECT, ws, proj.device)
@@ -228,7 +231,7 @@ def backproject(geom, angles, poses, proj, out=None, ws=None):
 def backproject_pose_grad(geom, angles, poses, proj, dLdvol, out=None, ws=None):
     """dfp_backproject_pose_grad: proj, dL/dvol [nz,ny,nx] -> dL/dtheta [V,6]."""
     g = Geometry.of(geom)
-    a, p, V = _views(angles, poses)
+    a, p, V = _views(angles, poses, geom)
     if out is None:
         out = torch.empty((V, 6), dtype=torch.float32, device=proj.device)
     ws, wp, wn = _workspace(g, V, OP_BACKPROJECT_POSE_GRAD, ws, proj.device)
@@ -255,7 +258,7 @@ def _host(t, shape, name):
 
 def forward_host(geom, angles, poses, vol, out=None):
     g = Geometry.of(geom)
-    a, p, V = _views(angles, poses)
+    a, p, V = _views(angles, poses, geom)
     if out is None:
         out = torch.empty((V, g.nv, g.nu), dtype=torch.float32, pin_memory=True)
     _check(_lib.dfp_forward_host(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p), _host(vol, (g.nz, g.ny, g.nx), "vol"),
@@ -265,7 +268,7 @@ def forward_host(geom, angles, poses, vol, out=None):
 
 def forward_pose_grad_host(geom, angles, poses, vol, dLdproj, out=None):
     g = Geometry.of(geom)
-    a, p, V = _views(angles, poses)
+    a, p, V = _views(angles, poses, geom)
     if out is None:
         out = torch.empty((V, 6), dtype=torch.float32, pin_memory=True)
     _check(_lib.dfp_forward_pose_grad_host(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p),
@@ -277,7 +280,7 @@ def forward_pose_grad_host(geom, angles, poses, vol, dLdproj, out=None):
 
 def backproject_host(geom, angles, poses, proj, out=None):
     g = Geometry.of(geom)
-    a, p, V = _views(angles, poses)
+    a, p, V = _views(angles, poses, geom)
     if out is None:
         out = torch.empty((g.nz, g.ny, g.nx), dtype=torch.float32, pin_memory=True)
     _check(_lib.dfp_backproject_host(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p),
@@ -288,7 +291,7 @@ def backproject_host(geom, angles, poses, proj, out=None):
 
 def backproject_pose_grad_host(geom, angles, poses, proj, dLdvol, out=None):
     g = Geometry.of(geom)
-    a, p, V = _views(angles, poses)
+    a, p, V = _views(angles, poses, geom)
     if out is None:
         out = torch.empty((V, 6), dtype=torch.float32, pin_memory=True)
     _check(_lib.dfp_backproject_pose_grad_host(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p),
@@ -301,7 +304,7 @@ def backproject_pose_grad_host(geom, angles, poses, proj, dLdvol, out=None):
 def count_ray_steps(geom, angles, poses) -> int:
     """Ray-steps one forward / forward_pose_grad call marches over (the unit of the Gray-steps/s metric)."""
     g = Geometry.of(geom)
-    a, p, V = _views(angles, poses)
+    a, p, V = _views(angles, poses, geom)
     n = int(_lib.dfp_count_ray_steps(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p)))
     if n < 0:
         raise DfpError(-6, status_string(-6))

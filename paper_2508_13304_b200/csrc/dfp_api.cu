@@ -71,11 +71,14 @@ int validate_geometry(const dfp_geometry* g) {
   return DFP_OK;
 }
 
-int validate_views(int n_views, const float* angles, const float* poses) {
+int validate_views(const dfp_geometry& g, int n_views, const float* angles, const float* poses) {
   if (n_views <= 0 || n_views > 65535) return DFP_ERR_DIMS;
   if (!angles || !poses) return DFP_ERR_NULL;
+  const int stride = view_stride(g);
   for (int v = 0; v < n_views; ++v) {
-    if (!std::isfinite(angles[v])) return DFP_ERR_NONFINITE;
+    for (int k = 0; k < stride; ++k)
+      if (!std::isfinite(angles[(size_t)stride * v + k])) return DFP_ERR_NONFINITE;
+    if (stride > 1 && !make_frame(g, angles, v).ok) return DFP_ERR_DIMS;
     for (int k = 0; k < 6; ++k)
       if (!std::isfinite(poses[6 * v + k])) return DFP_ERR_NONFINITE;
   }
@@ -118,8 +121,8 @@ bool make_volume_map(const dfp_geometry& g, const float* d_vol, int bx, int by, 
 // Positions at path length tau: p = s' + tau e, so a tile's extent along axis a is tau |De_a| with
 // |De_a| <= (|Dd_a| + |e_a| (rho_max/|d|) |Dd|) / SDD  for pixel offsets Dd on a detector at distance >= SDD.
 constexpr int kMinChunk = 4;
-bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V, bool grad, const int* box, int TU,
-                   int TV) {
+bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V, const ViewFrame& F, bool grad,
+                   const int* box, int TU, int TV) {
   const double v3[3] = {g.vx, g.vy, g.vz}, c3[3] = {g.cx, g.cy, g.cz};
   const double half[3] = {0.5 * g.nx * g.vx + 3 * g.vx, 0.5 * g.ny * g.vy + 3 * g.vy, 0.5 * g.nz * g.vz + 3 * g.vz};
   double tau_max = 0;
@@ -140,10 +143,11 @@ bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V, bo
     dmax = std::fmax(dmax, n);
     for (int a = 0; a < 3; ++a) emax[a] = std::fmax(emax[a], std::fabs(d[a]) / n);
   }
-  const double sdd = g.sdd;
+  const double sdd = F.sdd;                  // perpendicular source-detector distance of this view
   const double rho = std::sqrt(std::fmax(dmax * dmax - sdd * sdd, 0.0)) / sdd;
   const double tu = TU - 1, tv = TV - 1;
-  const double dnorm = std::hypot(tu * (double)g.du, tv * (double)g.dv);
+  // the tile's longer diagonal on the detector (mm): max |tu U +- tv V|
+  const double dnorm = std::sqrt(tu * tu * F.ulen * F.ulen + tv * tv * F.vlen * F.vlen + 2.0 * tu * tv * std::fabs(F.udotv));
   for (int a = 0; a < 3; ++a) {
     const double dd = tu * std::fabs(V.du[a]) + tv * std::fabs(V.dv[a]);
     const double span = tau_max * (dd + emax[a] * rho * dnorm) / sdd / v3[a];
@@ -299,7 +303,7 @@ int check_common(const dfp_geometry* g, int n_views, const float* angles, const 
                  const void* b, const void* c, void* ws, size_t ws_bytes, size_t need) {
   int st = validate_geometry(g);
   if (st) return st;
-  st = validate_views(n_views, angles, poses);
+  st = validate_views(*g, n_views, angles, poses);
   if (st) return st;
   if (!a || !b || (!c) || !ws) return DFP_ERR_NULL;
   if (!aligned(a, 16) || !aligned(b, 16) || !aligned(c, 16) || !aligned(ws, 256)) return DFP_ERR_ALIGN;
@@ -330,7 +334,11 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
   const FwdGeom G = make_fwd_geom(*g, grad, interp);
   std::vector<FwdView> hv((size_t)V);
   std::vector<FwdContract> hc(grad ? (size_t)V : 0);
-  for (int v = 0; v < V; ++v) make_fwd_view(*g, angles[v], poses + 6 * v, &hv[v], grad ? &hc[v] : nullptr);
+  std::vector<ViewFrame> hf((size_t)V);
+  for (int v = 0; v < V; ++v) {
+    hf[v] = make_frame(*g, angles, v);
+    make_fwd_view(hf[v], poses + 6 * v, &hv[v], grad ? &hc[v] : nullptr);
+  }
   char* base = static_cast<char*>(d_ws);
   FwdView* dv = reinterpret_cast<FwdView*>(base + w.off_views);
   FwdContract* dc = reinterpret_cast<FwdContract*>(base + w.off_con);
@@ -382,7 +390,7 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
   if (!(g->flags & DFP_FLAG_NO_TMA) && (g->nx % 4) == 0) {
     for (int i = 0; i < n_order && shape < 0; ++i) {
       bool fits = true;
-      for (int v = 0; fits && v < V; ++v) fits = tma_view_fits(*g, G, hv[v], grad, kBoxes[order[i]], TU, TV);
+      for (int v = 0; fits && v < V; ++v) fits = tma_view_fits(*g, G, hv[v], hf[v], grad, kBoxes[order[i]], TU, TV);
       if (fits) shape = order[i];
     }
   }
@@ -466,7 +474,8 @@ int run_backproject(const dfp_geometry* g, int V, const float* angles, const flo
   const BpGeom G = make_bp_geom(*g);
   std::vector<BpView> hv((size_t)V);
   std::vector<BpContract> hc(grad ? (size_t)V : 0);
-  for (int v = 0; v < V; ++v) make_bp_view(*g, G, angles[v], poses + 6 * v, &hv[v], grad ? &hc[v] : nullptr);
+  for (int v = 0; v < V; ++v)
+    make_bp_view(*g, G, make_frame(*g, angles, v), poses + 6 * v, &hv[v], grad ? &hc[v] : nullptr);
   char* base = static_cast<char*>(d_ws);
   BpView* dv = reinterpret_cast<BpView*>(base + w.off_views);
   BpContract* dc = reinterpret_cast<BpContract*>(base + w.off_con);
@@ -569,7 +578,7 @@ int run_host(int op, const dfp_geometry* g, int V, const float* angles, const fl
              const float* h_up, float* h_out, void* stream) {
   int st = validate_geometry(g);
   if (st) return st;
-  st = validate_views(V, angles, poses);
+  st = validate_views(*g, V, angles, poses);
   if (st) return st;
   const bool grad = op == DFP_OP_FORWARD_POSE_GRAD || op == DFP_OP_BACKPROJECT_POSE_GRAD;
   if (!h_in || !h_out || (grad && !h_up)) return DFP_ERR_NULL;
@@ -637,7 +646,9 @@ int run_host(int op, const dfp_geometry* g, int V, const float* angles, const fl
   if (h_shared) DFP_CUDA(cudaMemcpyAsync(d_shared, h_shared, nvol, cudaMemcpyHostToDevice, s), "H2D");
   int launches = 0;
   for (int c = 0; c < n_chunks; ++c) {
-    const int v0 = (int)((long long)V * c / n_chunks), v1 = (int)((long long)V * (c + 1) / n_chunks), nv_c = v1 - v0;
+    // chunk boundaries on even views: a gradient chunk writes d_grad + 6 v0 floats, which must stay 16-byte aligned
+    const int v0 = (int)((long long)V * c / n_chunks) & ~1;
+    const int v1 = c + 1 == n_chunks ? V : (int)((long long)V * (c + 1) / n_chunks) & ~1, nv_c = v1 - v0;
     const size_t off = (size_t)v0 * per_view;
     if (h_views) {                   // this chunk's per-view input on the copy stream, then the kernels wait for it
       DFP_CUDA(cudaMemcpyAsync(d_views + off, h_views + off, (size_t)nv_c * per_view * 4, cudaMemcpyHostToDevice,
@@ -647,14 +658,14 @@ int run_host(int op, const dfp_geometry* g, int V, const float* angles, const fl
     }
     float* out_c = static_cast<float*>(d_out.p) + (grad ? (size_t)v0 * 6 : off);
     if (fwd)
-      st = run_forward(g, nv_c, angles + v0, poses + 6 * v0, d_shared, grad ? d_views + off : nullptr, out_c, d_ws.p,
+      st = run_forward(g, nv_c, angles + (size_t)view_stride(*g) * v0, poses + 6 * v0, d_shared, grad ? d_views + off : nullptr, out_c, d_ws.p,
                        n_ws, s, grad ? DFP_OP_FORWARD_POSE_GRAD : DFP_OP_FORWARD);
     else if (grad)
-      st = run_backproject(g, nv_c, angles + v0, poses + 6 * v0, d_views + off, d_shared, out_c, d_ws.p, n_ws, s, true);
+      st = run_backproject(g, nv_c, angles + (size_t)view_stride(*g) * v0, poses + 6 * v0, d_views + off, d_shared, out_c, d_ws.p, n_ws, s, true);
     else {                           // dfp_backproject: the first chunk overwrites the volume, the others add to it
       dfp_geometry gc = *g;
       gc.flags = c ? (g->flags | DFP_FLAG_ACCUMULATE) : g->flags;
-      st = run_backproject(&gc, nv_c, angles + v0, poses + 6 * v0, d_views + off, nullptr, static_cast<float*>(d_out.p),
+      st = run_backproject(&gc, nv_c, angles + (size_t)view_stride(*g) * v0, poses + 6 * v0, d_views + off, nullptr, static_cast<float*>(d_out.p),
                            d_ws.p, n_ws, s, false);
     }
     if (st) return st;
@@ -740,10 +751,10 @@ int dfp_backproject_pose_grad_host(const dfp_geometry* g, int n_views, const flo
 }
 
 int64_t dfp_count_ray_steps(const dfp_geometry* g, int n_views, const float* angles, const float* poses) {
-  if (validate_geometry(g) != DFP_OK || validate_views(n_views, angles, poses) != DFP_OK) return -1;
+  if (validate_geometry(g) != DFP_OK || validate_views(*g, n_views, angles, poses) != DFP_OK) return -1;
   const FwdGeom G = make_fwd_geom(*g, true);
   std::vector<FwdView> hv((size_t)n_views);
-  for (int v = 0; v < n_views; ++v) make_fwd_view(*g, angles[v], poses + 6 * v, &hv[v], nullptr);
+  for (int v = 0; v < n_views; ++v) make_fwd_view(make_frame(*g, angles, v), poses + 6 * v, &hv[v], nullptr);
   FwdView* dv = nullptr;
   unsigned long long* dn = nullptr;
   unsigned long long n = 0;

@@ -155,35 +155,85 @@ inline FwdGeom make_fwd_geom(const dfp_geometry& g, bool grad, bool interp = fal
   return G;
 }
 
-struct ViewFrame {      // world-frame scanner vectors of one view (O5)
-  double n[3], s[3], dc[3], eu[3], ev[3], cu, cv;
+// World-frame scanner of one view.  Pixel (iu,iv) centre = dc + (iu - cu) U + (iv - cv) V; Eq.1 (PAPER.md :60-63)
+// in pixel-index units is  u w' = pu.(r;1) + cu w',  v w' = pv.(r;1) + cv w',  w' = p3.(r;1) = depth from the source
+// along the detector normal in mm.
+struct ViewFrame {
+  double s[3], dc[3], U[3], V[3], cu, cv;
+  double pu[4], pv[4], p3[4];
+  double sdd, ulen, vlen, udotv; // perpendicular source-detector distance; |U|, |V| (mm); U.V
+  bool ok;                       // false: degenerate frame (U parallel to V, or the source in the detector plane)
 };
-inline ViewFrame make_frame(const dfp_geometry& g, double beta) {
+inline int view_stride(const dfp_geometry& g) { return (g.flags & DFP_FLAG_VIEW_FRAMES) ? 12 : 1; }
+
+// Circular orbit (O5): views[v] = gantry angle.
+inline ViewFrame make_frame_circular(const dfp_geometry& g, double beta) {
   ViewFrame f;
-  f.n[0] = std::cos(beta); f.n[1] = std::sin(beta); f.n[2] = 0;
-  f.eu[0] = -std::sin(beta); f.eu[1] = std::cos(beta); f.eu[2] = 0;
-  f.ev[0] = 0; f.ev[1] = 0; f.ev[2] = 1;
-  for (int a = 0; a < 3; ++a) { f.s[a] = (double)g.sad * f.n[a]; f.dc[a] = -((double)g.sdd - (double)g.sad) * f.n[a]; }
+  const double n[3] = {std::cos(beta), std::sin(beta), 0}, eu[3] = {-std::sin(beta), std::cos(beta), 0}, ev[3] = {0, 0, 1};
+  for (int a = 0; a < 3; ++a) {
+    f.s[a] = (double)g.sad * n[a]; f.dc[a] = -((double)g.sdd - (double)g.sad) * n[a];
+    f.U[a] = (double)g.du * eu[a]; f.V[a] = (double)g.dv * ev[a];
+    f.p3[a] = -n[a];
+    f.pu[a] = ((double)g.sdd / (double)g.du) * eu[a];
+    f.pv[a] = ((double)g.sdd / (double)g.dv) * ev[a];
+  }
+  f.p3[3] = g.sad; f.pu[3] = 0; f.pv[3] = 0;
+  f.sdd = g.sdd; f.ulen = g.du; f.vlen = g.dv; f.udotv = 0;
   f.cu = (g.nu - 1) * 0.5 + (double)g.u0;
   f.cv = (g.nv - 1) * 0.5 + (double)g.v0;
+  f.ok = true;
   return f;
 }
 
-inline void make_fwd_view(const dfp_geometry& g, float angle, const float* pose, FwdView* V, FwdContract* C) {
-  const ViewFrame f = make_frame(g, angle);
+// Explicit frame (DFP_FLAG_VIEW_FRAMES): views[12 v ..] = s, dc, U, V.  With q = r - s written in the basis
+// (U, V, D = dc - s), q = a U + b V + k D, the point s + q / k of the line lies on the detector at dc + (a/k) U + (b/k) V:
+// (a, b, k) = B^-1 q with B = [U V D] (columns), so the rows of B^-1, scaled by SDD_v = |det B| / |U x V| to make
+// w' a depth in mm, are the spatial parts of pu, pv, p3.
+inline ViewFrame make_frame_explicit(const dfp_geometry& g, const float* fr) {
+  ViewFrame f;
+  double D[3];
+  for (int a = 0; a < 3; ++a) { f.s[a] = fr[a]; f.dc[a] = fr[3 + a]; f.U[a] = fr[6 + a]; f.V[a] = fr[9 + a]; D[a] = f.dc[a] - f.s[a]; }
+  auto cross = [](const double* x, const double* y, double* o) {
+    o[0] = x[1] * y[2] - x[2] * y[1]; o[1] = x[2] * y[0] - x[0] * y[2]; o[2] = x[0] * y[1] - x[1] * y[0];
+  };
+  double VxD[3], DxU[3], UxV[3];
+  cross(f.V, D, VxD); cross(D, f.U, DxU); cross(f.U, f.V, UxV);
+  const double det = f.U[0] * VxD[0] + f.U[1] * VxD[1] + f.U[2] * VxD[2];
+  const double area = std::sqrt(UxV[0] * UxV[0] + UxV[1] * UxV[1] + UxV[2] * UxV[2]);
+  f.ulen = std::sqrt(f.U[0] * f.U[0] + f.U[1] * f.U[1] + f.U[2] * f.U[2]);
+  f.vlen = std::sqrt(f.V[0] * f.V[0] + f.V[1] * f.V[1] + f.V[2] * f.V[2]);
+  f.udotv = f.U[0] * f.V[0] + f.U[1] * f.V[1] + f.U[2] * f.V[2];
+  f.cu = (g.nu - 1) * 0.5 + (double)g.u0;
+  f.cv = (g.nv - 1) * 0.5 + (double)g.v0;
+  f.ok = std::isfinite(det) && std::isfinite(area) && area > 1e-12 * f.ulen * f.vlen && f.ulen > 0 && f.vlen > 0 &&
+         std::fabs(det) > 1e-6 * area * std::sqrt(D[0] * D[0] + D[1] * D[1] + D[2] * D[2]);
+  if (!f.ok) { f.sdd = 0; return f; }
+  f.sdd = std::fabs(det) / area;
+  const double k = f.sdd / det;                        // rows of B^-1 are (V x D, D x U, U x V) / det
+  f.pu[3] = f.pv[3] = f.p3[3] = 0;
+  for (int a = 0; a < 3; ++a) {
+    f.pu[a] = k * VxD[a]; f.pv[a] = k * DxU[a]; f.p3[a] = k * UxV[a];
+    f.pu[3] -= f.pu[a] * f.s[a]; f.pv[3] -= f.pv[a] * f.s[a]; f.p3[3] -= f.p3[a] * f.s[a];
+  }
+  return f;
+}
+inline ViewFrame make_frame(const dfp_geometry& g, const float* views, int v) {
+  return (g.flags & DFP_FLAG_VIEW_FRAMES) ? make_frame_explicit(g, views + 12 * (size_t)v)
+                                          : make_frame_circular(g, (double)views[v]);
+}
+
+inline void make_fwd_view(const ViewFrame& f, const float* pose, FwdView* V, FwdContract* C) {
   const Mat3 R = pose_rotation(pose);
   const double t[3] = {pose[0], pose[1], pose[2]};
-  double sw[3], p00[3], tmp[3];
+  double sw[3], p00[3];
   for (int a = 0; a < 3; ++a) {
     sw[a] = f.s[a] - t[a];
-    p00[a] = f.dc[a] - f.cu * (double)g.du * f.eu[a] - f.cv * (double)g.dv * f.ev[a] - f.s[a];   // pixel(0,0) - s
+    p00[a] = f.dc[a] - f.cu * f.U[a] - f.cv * f.V[a] - f.s[a];   // pixel(0,0) - s
   }
   mulT(R, sw, V->src);
   mulT(R, p00, V->d0);
-  for (int a = 0; a < 3; ++a) tmp[a] = (double)g.du * f.eu[a];
-  mulT(R, tmp, V->du);
-  for (int a = 0; a < 3; ++a) tmp[a] = (double)g.dv * f.ev[a];
-  mulT(R, tmp, V->dv);
+  mulT(R, f.U, V->du);
+  mulT(R, f.V, V->dv);
   if (C) {
     for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) C->R[i * 3 + j] = R.m[i][j];
     // axial vectors of R^T dR/dgamma_k for R = Rz Ry Rx:  w_x = e_x, w_y = Rx^T e_y, w_z = (Ry Rx)^T e_z
@@ -199,8 +249,7 @@ inline BpGeom make_bp_geom(const dfp_geometry& g) {
   BpGeom G;
   G.nx = g.nx; G.ny = g.ny; G.nz = g.nz; G.nu = g.nu; G.nv = g.nv;
   G.pu = g.nu + 2 * kPadDet; G.pv = g.nv + 2 * kPadDet;
-  const ViewFrame f = make_frame(g, 0.0);
-  G.CU = (int)std::floor(f.cu); G.CV = (int)std::floor(f.cv);
+  G.CU = (int)std::floor((g.nu - 1) * 0.5 + (double)g.u0); G.CV = (int)std::floor((g.nv - 1) * 0.5 + (double)g.v0);
   G.hx = (g.nx - 1) * 0.5f; G.hy = (g.ny - 1) * 0.5f; G.hz = (g.nz - 1) * 0.5f;
   G.vx = g.vx; G.vy = g.vy; G.vz = g.vz; G.cx = g.cx; G.cy = g.cy; G.cz = g.cz;
   G.sad2 = (float)((double)g.sad * (double)g.sad);
@@ -208,20 +257,17 @@ inline BpGeom make_bp_geom(const dfp_geometry& g) {
   return G;
 }
 
-inline void make_bp_view(const dfp_geometry& g, const BpGeom& G, float angle, const float* pose, BpView* V,
+inline void make_bp_view(const dfp_geometry& g, const BpGeom& G, const ViewFrame& f, const float* pose, BpView* V,
                          BpContract* C) {
-  const ViewFrame f = make_frame(g, angle);
   const Mat3 R = pose_rotation(pose);
   const double t[3] = {pose[0], pose[1], pose[2]};
   // world projection matrix in pixel-index units (Eq.1), principal point's integer part removed:
-  //   P3 = (-n | SAD),  P1 = (SDD/du)(e_u | 0) + (c_u - CU) P3,  P2 = (SDD/dv)(e_v | 0) + (c_v - CV) P3
+  //   circular orbit: P3 = (-n | SAD),  P1 = (SDD/du)(e_u | 0) + (c_u - CU) P3,  P2 = (SDD/dv)(e_v | 0) + (c_v - CV) P3
   double P[3][4];
-  for (int a = 0; a < 3; ++a) P[2][a] = -f.n[a];
-  P[2][3] = g.sad;
   for (int a = 0; a < 4; ++a) {
-    const double e1 = a < 3 ? f.eu[a] : 0.0, e2 = a < 3 ? f.ev[a] : 0.0;
-    P[0][a] = ((double)g.sdd / (double)g.du) * e1 + (f.cu - G.CU) * P[2][a];
-    P[1][a] = ((double)g.sdd / (double)g.dv) * e2 + (f.cv - G.CV) * P[2][a];
+    P[2][a] = f.p3[a];
+    P[0][a] = f.pu[a] + (f.cu - G.CU) * P[2][a];
+    P[1][a] = f.pv[a] + (f.cv - G.CV) * P[2][a];
   }
   // P_eff = P [R | t; 0 0 0 1]  acting on object-frame mm
   double E[3][4];

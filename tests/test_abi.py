@@ -85,6 +85,19 @@ def test_bad_arguments_are_rejected_without_a_gpu(dfp):
     assert call(ctypes.byref(g), 2, P(ang), P(nan_pose), fake, fake, fake, 1 << 30) == -3
     assert call(ctypes.byref(g), 2, P(ang), P(pose), ctypes.c_void_p(0x10004), fake, fake, 1 << 30) == -4
     assert call(ctypes.byref(g), 2, P(ang), P(pose), fake, fake, fake, 16) == -5
+    # DFP_FLAG_VIEW_FRAMES: `angles` holds 12 floats per view (s, c, U, V); degenerate frames are DFP_ERR_DIMS
+    gf = dfp.Geometry.of(_geom(flags=64))
+    fr = np.tile(np.array([100, 0, 0, -80, 0, 0, 0, 1.5, 0, 0, 0, 1.5], np.float32), (2, 1))
+    assert call(ctypes.byref(gf), 2, P(fr), P(pose), fake, fake, fake, 16) == -5          # valid frames: next check
+    par = fr.copy()
+    par[1, 9:12] = par[1, 6:9]                                                            # V parallel to U
+    assert call(ctypes.byref(gf), 2, P(par), P(pose), fake, fake, fake, 1 << 30) == -2
+    flat = fr.copy()
+    flat[0, 0:3] = [-80, 7, 3]                                                            # source in the detector plane
+    assert call(ctypes.byref(gf), 2, P(flat), P(pose), fake, fake, fake, 1 << 30) == -2
+    nanf = fr.copy()
+    nanf[1, 11] = np.inf
+    assert call(ctypes.byref(gf), 2, P(nanf), P(pose), fake, fake, fake, 1 << 30) == -3
 
 
 def test_product_package_never_imports_the_oracle():

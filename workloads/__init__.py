@@ -9,7 +9,7 @@ upstream arrays.  It holds none of the method's arithmetic (no discrete projecto
 no back-projector, no pose gradient) and imports neither `oracle` nor the package.
 """
 from .rng import SplitMix64, normal_field, uniform_field
-from .geometry import Geometry, view_angles, circular_frame, move_frame, FLAG_VIEW_FRAMES
+from .geometry import Geometry, view_angles, circular_frame, move_frame, noncircular_orbit, FLAG_VIEW_FRAMES
 from .phantom import (Ellipsoid, random_ellipsoids, voxelise_ellipsoids, voxelise_blobs,
                       ellipsoid_projection, blob_projection, rotation_zyx)
 from .losses import ncc, ncc_grad, variance_grad, ssd_grad
@@ -17,7 +17,7 @@ from .ramp import ramp_filter
 from .configs import CONFIGS, make_config, base_seed
 
 __all__ = [
-    "SplitMix64", "normal_field", "uniform_field", "Geometry", "view_angles", "circular_frame", "move_frame",
+    "SplitMix64", "normal_field", "uniform_field", "Geometry", "view_angles", "circular_frame", "move_frame", "noncircular_orbit",
     "FLAG_VIEW_FRAMES", "Ellipsoid",
     "random_ellipsoids", "voxelise_ellipsoids", "voxelise_blobs", "ellipsoid_projection",
     "blob_projection", "rotation_zyx", "ncc", "ncc_grad", "variance_grad", "ssd_grad",

@@ -76,3 +76,38 @@ def move_frame(frame, Q, tau) -> torch.Tensor:
     Q = torch.as_tensor(Q, dtype=torch.float64)
     tau = torch.as_tensor(tau, dtype=torch.float64)
     return torch.cat([Q @ f[0] + tau, Q @ f[1] + tau, Q @ f[2], Q @ f[3]])
+
+
+def _axis_rotation(axis: torch.Tensor, angle: float) -> torch.Tensor:
+    """Rotation by `angle` about the unit vector `axis` (Rodrigues), float64."""
+    k = axis / torch.linalg.norm(axis)
+    K = torch.tensor([[0.0, -k[2], k[1]], [k[2], 0.0, -k[0]], [-k[1], k[0], 0.0]], dtype=torch.float64)
+    return torch.eye(3, dtype=torch.float64) + math.sin(angle) * K + (1.0 - math.cos(angle)) * (K @ K)
+
+
+def noncircular_orbit(geom: Geometry, angles, seed: int, tilt_deg: float = 10.0, wobble_mm: float = 3.0,
+                      spin_deg: float = 1.5, sdd_mm: float = 15.0) -> torch.Tensor:
+    """[V,12] view frames of a seeded NON-CIRCULAR orbit (stands in for the calibrated non-circular geometry of
+    PAPER.md :244): the circular view of each gantry angle, then (a) source and detector tilted out of the orbit
+    plane about the view's u axis by tilt_deg * sin(2 beta + phase) (a saddle orbit), (b) the detector spun about
+    its normal, shifted in its own plane and moved along the normal by smooth seeded sinusoids of the given
+    amplitudes, (c) the source moved by up to wobble_mm in each direction.  float64; round to fp32 before use."""
+    from .rng import SplitMix64
+    rng = SplitMix64(seed)
+    ph = [rng.uniform(0.0, 2.0 * math.pi) for _ in range(8)]
+    out = []
+    for beta in [float(b) for b in torch.as_tensor(angles, dtype=torch.float64).reshape(-1)]:
+        f = circular_frame(geom, beta).reshape(4, 3)
+        eu = f[2] / torch.linalg.norm(f[2])
+        Q = _axis_rotation(eu, tilt_deg * math.pi / 180.0 * math.sin(2.0 * beta + ph[0]))
+        f = move_frame(f, Q, [0.0, 0.0, 0.0]).reshape(4, 3)
+        n = torch.linalg.cross(f[2], f[3])
+        n = n / torch.linalg.norm(n)
+        S = _axis_rotation(n, spin_deg * math.pi / 180.0 * math.sin(beta + ph[1]))
+        U, V = S @ f[2], S @ f[3]
+        c = f[1] + wobble_mm * math.sin(beta + ph[2]) * U / torch.linalg.norm(U) + \
+            wobble_mm * math.sin(3.0 * beta + ph[3]) * V / torch.linalg.norm(V) + sdd_mm * math.sin(beta + ph[4]) * n
+        s = f[0] + wobble_mm * torch.tensor([math.sin(beta + ph[5]), math.sin(2.0 * beta + ph[6]),
+                                             math.sin(beta + ph[7])], dtype=torch.float64)
+        out.append(torch.cat([s, c, U, V]))
+    return torch.stack(out)
