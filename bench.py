@@ -408,6 +408,17 @@ def main():
     roofline["lsu_floor_frac"] = lds * (units[dom] / 32.0) / (N_SM * pk.get("sm_max_mhz", 1965.0) * 1e6 *
                                                                 mean_ms[dom] * 1e-3)
 
+    # measured denominators (dfp_microbench, one resident wave each): sustained rate per clock per SM of the pipes the
+    # kernels are bound by; "lsu_measured_frac" replaces the assumed one LDS per clock by the measured LDS rate
+    per_clk_sm = 1.0 / (N_SM * pk.get("sm_max_mhz", 1965.0) * 1e6)
+    mb = {name: dfp.microbench(kind) * per_clk_sm
+          for name, kind in (("lds_warp_inst", dfp.MB_LDS), ("fadd_lane_ops", dfp.MB_FADD),
+                             ("ffma_lane_ops", dfp.MB_FFMA), ("ffma2_lane_ops", dfp.MB_FFMA2))}
+    roofline["measured_per_clk_per_sm"] = mb
+    roofline["lsu_measured_frac"] = roofline["lsu_floor_frac"] / mb["lds_warp_inst"]
+    roofline["alu_measured_frac"] = roofline["frac"] * 128.0 / max(mb["fadd_lane_ops"], mb["ffma_lane_ops"],
+                                                                   mb["ffma2_lane_ops"])
+
     # ---------------------------------------------------------------- CPU baseline: the oracle on the host cores
     cpu = None
     if world == 1 and not args.no_cpu_baseline:

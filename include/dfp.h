@@ -193,6 +193,17 @@ const char* dfp_status_string(int status);
 /* Library version (major*10000 + minor*100 + patch). */
 int dfp_version(void);
 
+/* Measured denominators for the roofline of the projector kernels, which are bound by the SM-side pipes and not by HBM
+ * (DESIGN.md "Roofline").  Runs one resident wave of a small kernel on the current device (default
+ * stream, synchronous, timed with CUDA events, allocates and frees a few MB of scratch) and writes the sustained rate
+ * of the WHOLE DEVICE PER SECOND (divide by SM count x SM clock for the rate per clock per SM):
+ *   DFP_MB_LDS   warp-wide, bank-conflict-free LDS.32 instructions (the staged gradient kernels need 32 per warp-sample
+ *                and 12 per warp-voxel-view);
+ *   DFP_MB_FADD / DFP_MB_FFMA / DFP_MB_FFMA2   fp32 results of dependent-free FADD, FFMA and packed FFMA2 streams.
+ * Returns DFP_OK, DFP_ERR_NULL, DFP_ERR_DIMS (unknown kind) or DFP_ERR_CUDA. */
+enum { DFP_MB_LDS = 0, DFP_MB_FADD = 1, DFP_MB_FFMA = 2, DFP_MB_FFMA2 = 3 };
+int dfp_microbench(int kind, double* per_second);
+
 #ifdef __cplusplus
 }
 #endif

@@ -87,6 +87,8 @@ def _load():
     lib.dfp_set_kernel_timing.restype = ci
     lib.dfp_last_kernel_ms.argtypes = []
     lib.dfp_last_kernel_ms.restype = ctypes.c_float
+    lib.dfp_microbench.argtypes = [ci, ctypes.POINTER(ctypes.c_double)]
+    lib.dfp_microbench.restype = ci
     lib.dfp_status_string.argtypes = [ci]
     lib.dfp_status_string.restype = cp
     return lib
@@ -123,6 +125,16 @@ def set_kernel_timing(enable: bool) -> None:
 def last_kernel_ms() -> float:
     """Milliseconds of the dominant kernel of the last device-pointer call (waits for it); -1 if timing is off."""
     return float(_lib.dfp_last_kernel_ms())
+
+
+MB_LDS, MB_FADD, MB_FFMA, MB_FFMA2 = 0, 1, 2, 3
+
+
+def microbench(kind: int) -> float:
+    """Sustained whole-device rate per second of one SM-side pipe (include/dfp.h: dfp_microbench) on the current device."""
+    r = ctypes.c_double(0.0)
+    _check(_lib.dfp_microbench(int(kind), ctypes.byref(r)))
+    return float(r.value)
 
 
 def _check(status):

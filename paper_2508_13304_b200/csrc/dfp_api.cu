@@ -13,6 +13,7 @@
 #include "dfp_bp_tma.cuh"
 #include "dfp_fwd_tma.cuh"
 #include "dfp_kernels.cuh"
+#include "dfp_microbench.cuh"
 #include "dfp_params.h"
 #include "dfp_joseph.cuh"
 #include "dfp_siddon.cuh"
@@ -803,5 +804,57 @@ const char* dfp_status_string(int status) {
 }
 
 int dfp_version(void) { return 100; }
+
+// One resident wave of a micro-benchmark kernel, timed with CUDA events on the default stream (the kernels' own
+// clock64() counts are kept for inspection only: on B200 that counter does not tick at the SM clock).
+int dfp_microbench(int kind, double* per_second) {
+  if (!per_second) return DFP_ERR_NULL;
+  if (kind < DFP_MB_LDS || kind > DFP_MB_FFMA2) return DFP_ERR_DIMS;
+  int dev = 0, n_sm = 0, R = 0;
+  DFP_CUDA(cudaGetDevice(&dev), "cudaGetDevice");
+  DFP_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute");
+  const void* fn = kind == DFP_MB_LDS    ? (const void*)mb_lds_kernel
+                   : kind == DFP_MB_FADD ? (const void*)mb_alu_kernel<0>
+                   : kind == DFP_MB_FFMA ? (const void*)mb_alu_kernel<1>
+                                         : (const void*)mb_alu_kernel<2>;
+  DFP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&R, fn, kMbThreads, 0), "occupancy");
+  if (R < 1 || n_sm < 1) return DFP_ERR_CUDA;
+  const int grid = n_sm * R;
+  float* sink = nullptr;
+  long long* cyc = nullptr;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  DFP_CUDA(cudaMalloc(&sink, sizeof(float) * (size_t)grid * kMbThreads), "cudaMalloc");
+  if (cudaMalloc(&cyc, sizeof(long long) * grid) != cudaSuccess || cudaEventCreate(&e0) != cudaSuccess ||
+      cudaEventCreate(&e1) != cudaSuccess) {
+    const cudaError_t e = cudaGetLastError();
+    cudaFree(sink); cudaFree(cyc);
+    if (e0) cudaEventDestroy(e0);
+    return cuda_fail(e, "microbench set-up");
+  }
+  double work = 0;        // whole grid: warp-instructions (LDS) or fp32 results (ALU)
+  for (int pass = 0; pass < 2; ++pass) {                 // warm-up, then the measured wave
+    const int iters = pass ? 8000 : 50;
+    if (pass) cudaEventRecord(e0, 0);
+    if (kind == DFP_MB_LDS) {
+      mb_lds_kernel<<<grid, kMbThreads>>>(iters, 96, sink, cyc);
+      work = (double)grid * iters * kMbLdsPerIter * (kMbThreads / 32);
+    } else {
+      if (kind == DFP_MB_FADD) mb_alu_kernel<0><<<grid, kMbThreads>>>(iters, 1.0001f, 1e-3f, sink, cyc);
+      else if (kind == DFP_MB_FFMA) mb_alu_kernel<1><<<grid, kMbThreads>>>(iters, 1.0001f, 1e-3f, sink, cyc);
+      else mb_alu_kernel<2><<<grid, kMbThreads>>>(iters, 1.0001f, 1e-3f, sink, cyc);
+      work = (double)grid * iters * 4 * kMbChains * kMbThreads * (kind == DFP_MB_FFMA2 ? 2 : 1);
+    }
+    if (pass) cudaEventRecord(e1, 0);
+  }
+  float ms = 0.f;
+  cudaError_t e = cudaEventSynchronize(e1);
+  if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+  cudaFree(sink); cudaFree(cyc);
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  if (e != cudaSuccess) return cuda_fail(e, "microbench");
+  if (!(ms > 0.f)) return DFP_ERR_CUDA;
+  *per_second = work / ((double)ms * 1e-3);
+  return DFP_OK;
+}
 
 }  // extern "C"

@@ -100,6 +100,15 @@ def test_bad_arguments_are_rejected_without_a_gpu(dfp):
     assert call(ctypes.byref(gf), 2, P(nanf), P(pose), fake, fake, fake, 1 << 30) == -3
 
 
+def test_microbench_rejects_bad_arguments(dfp):
+    lib = ctypes.CDLL(dfp.lib_path())
+    lib.dfp_microbench.restype = ctypes.c_int
+    lib.dfp_microbench.argtypes = [ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
+    r = ctypes.c_double(0.0)
+    assert lib.dfp_microbench(0, None) == -1
+    assert lib.dfp_microbench(7, ctypes.byref(r)) == -2 and lib.dfp_microbench(-1, ctypes.byref(r)) == -2
+
+
 def test_product_package_never_imports_the_oracle():
     pkg = os.path.join(ROOT, "paper_2508_13304_b200")
     for dirpath, _, files in os.walk(pkg):

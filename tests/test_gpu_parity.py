@@ -658,3 +658,14 @@ def test_joseph_and_siddon_flags_exclude_each_other(dfp):
     a, p = f32(w.angles.numpy()), f32(w.poses.numpy()).reshape(-1, 6)
     with pytest.raises(dfp.DfpError):
         dfp.forward(w.geom.replace(flags=dfp.FLAG_SIDDON | dfp.FLAG_JOSEPH), a, p, w.volume(dev))
+
+
+# ------------------------------------------------------------------ dfp_microbench (roofline denominators)
+def test_microbench_rates_are_those_of_a_b200_class_sm(dfp):
+    """One warp-wide LDS per clock per SM and 128 fp32 lanes per SM at 1-2.5 GHz on >= 100 SMs."""
+    n_sm = torch.cuda.get_device_properties(0).multi_processor_count
+    lds = dfp.microbench(dfp.MB_LDS) / n_sm
+    assert 0.8e9 < lds < 2.6e9, lds                              # ~1 per clock
+    for kind in (dfp.MB_FADD, dfp.MB_FFMA, dfp.MB_FFMA2):
+        r = dfp.microbench(kind) / n_sm
+        assert 100 * 0.9e9 < r < 130 * 2.6e9, (kind, r)          # ~128 per clock
