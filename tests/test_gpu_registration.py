@@ -95,3 +95,41 @@ def test_pose_of_one_view_recovered_through_the_backprojector():
         theta = theta - lr * (m / (1 - b1 ** it)) / (np.sqrt(s / (1 - b2 ** it)) + eps)
     assert hist[-1][0] < 0.02 * hist[0][0], (hist[0], hist[-1])
     assert hist[-1][1] < 0.2 * hist[0][1] and hist[-1][2] < 0.2 * hist[0][2], hist[::20]
+
+
+def test_online_calibration_of_a_noncircular_orbit_recovers_per_view_poses():
+    """The paper's third task (PAPER.md :244, :259-268): per-view rigid calibration of a NON-CIRCULAR orbit.  The
+    nominal scanner is a seeded saddle orbit given as explicit view frames (DFP_FLAG_VIEW_FRAMES); every view is off
+    by an unknown 6-DOF pose (config 4's +-2 mm / +-1 degree).  All views are calibrated at once by Adam on the sum of
+    squared differences, one dfp_forward_fused_moments call per iteration for the whole batch: dSSD/dl = 2 (l - b),
+    i.e. (alpha, beta, gamma) = (0, 2, -2) per view."""
+    import paper_2508_13304_b200 as dfp
+    dev = torch.device("cuda:0")
+    w = W.make_config(4, scale=0.125, n_views=8)
+    g = w.geom.replace(flags=dfp.FLAG_VIEW_FRAMES)
+    frames = W.noncircular_orbit(w.geom, w.angles, w.seed + 17).numpy().astype(np.float32)
+    vol = w.volume(dev)
+    hidden = w.data_poses.numpy().astype(np.float64)                     # seeded U(+-2 mm, +-1 degree) per view
+    V = hidden.shape[0]
+    target = dfp.forward(g, frames, hidden.astype(np.float32), vol).clone()
+    theta = np.zeros((V, 6))
+    m = np.zeros((V, 6))
+    s = np.zeros((V, 6))
+    lr = np.array([0.08, 0.08, 0.08, 0.0012, 0.0012, 0.0012])
+    b1, b2, eps = 0.9, 0.999, 1e-8
+    hist = []
+    for it in range(1, 251):
+        proj, mom = dfp.forward_fused_moments(g, frames, theta.astype(np.float32), vol, target)
+        loss = float(((proj.double() - target.double()) ** 2).sum())
+        mo = mom.double().cpu().numpy()
+        grad = 2.0 * mo[:, 1] - 2.0 * mo[:, 2]
+        et = np.linalg.norm(theta[:, :3] - hidden[:, :3], axis=1).mean()
+        er = np.linalg.norm(theta[:, 3:] - hidden[:, 3:], axis=1).mean()
+        hist.append((loss, float(et), float(er)))
+        m = b1 * m + (1 - b1) * grad
+        s = b2 * s + (1 - b2) * grad * grad
+        theta = theta - lr * (m / (1 - b1 ** it)) / (np.sqrt(s / (1 - b2 ** it)) + eps)
+    # observed: SSD 1712 -> 0.09, mean pose error 1.77 mm / 1.0 degree -> 0.05 mm / 0.001 degree
+    assert hist[-1][0] < 1e-3 * hist[0][0], (hist[0], hist[-1])
+    assert hist[-1][1] < 0.1 * hist[0][1] and hist[-1][2] < 0.05 * hist[0][2], hist[::25]
+    assert hist[10][0] < hist[0][0]
