@@ -170,8 +170,10 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_tma_kernel(BpGeom G, int n_v
     mbar_wait(full_addr + 8u * s, (unsigned)(view / n_stages) & 1u);
     const float* hdr = smem + s * stage_words;
     const unsigned c0 = __float_as_uint(hdr[24]), BU = __float_as_uint(hdr[26]);
+#ifdef DFP_CHECK_BOUNDS
     const unsigned chk_lo = smem_addr + 4u * (unsigned)(s * stage_words + kPatchHeader) + BU + 4u,
                    chk_hi = smem_addr + 4u * (unsigned)((s + 1) * stage_words) - 2u * BU - 12u;
+#endif
     bad |= __float_as_uint(hdr[25]) != 0u;
     if (live) {
       const float a02 = hdr[2], a12 = hdr[6], a22 = hdr[10];
@@ -275,8 +277,10 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_grad_tma_kernel(BpGeom G, in
       mbar_wait(full_addr + 8u * s, (unsigned)(view / n_stages) & 1u);
       const float* hdr = smem + s * stage_words;
       const unsigned c0 = __float_as_uint(hdr[24]), BU = __float_as_uint(hdr[26]);
+#ifdef DFP_CHECK_BOUNDS
       const unsigned chk_lo = smem_addr + 4u * (unsigned)(s * stage_words + kPatchHeader) + BU + 4u,
                      chk_hi = smem_addr + 4u * (unsigned)((s + 1) * stage_words) - 2u * BU - 12u;
+#endif
       bad |= __float_as_uint(hdr[25]) != 0u;
       float sm[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
       if (live) {

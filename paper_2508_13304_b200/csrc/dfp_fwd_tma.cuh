@@ -374,10 +374,10 @@ __global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, 4) fwd_tma_kernel(Fwd
   }
 
   const float bad = B.Kc < 0 ? __int_as_float(0x7fc00000) : 0.f;   // NaN: the box cannot hold the tile (host bound wrong)
-  if (!GRAD) {
+  if constexpr (!GRAD) {
     if (live && slot == 0) out[((size_t)view * G.nv + iv) * G.nu + iu] = G.step * acc[0] + bad;
     return;
-  }
+  } else {
   float o6[6 * NSET];
 #pragma unroll
   for (int q = 0; q < 6 * NSET; ++q) o6[q] = 0.f;
@@ -428,6 +428,7 @@ __global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, 4) fwd_tma_kernel(Fwd
     const int set = threadIdx.x / 6, k = threadIdx.x % 6;
     out[(((size_t)set * gridDim.z + view) * nblk + blk) * 6 + k] = t;
   }
+  }  // GRAD
 }
 
 }  // namespace dfp
