@@ -199,3 +199,51 @@ def test_volume_1024_cubed_indices_and_sizes(dfp):
     assert dfp.last_path() == dfp.PATH_TMA
     o = oracle.backproject(g, a, p, pin.cpu().numpy(), 777, 778)
     assert rel_l2(bp[777:778].cpu().numpy(), o) <= TOL_VAL
+
+
+def test_c2_view_results_do_not_depend_on_the_batch(dfp):
+    """Property that holds at any size: views are independent (Eq.18-22 sum over the rays / voxels of ONE
+    view), so a view computed alone, in a pair or inside the 64-view batch of config 2 gives the same projection
+    bit for bit and the same 6-vectors / moments up to the fp32 order of its block partial sums - whatever staging
+    box, chunking or grid the host picks for the batch.  The back-projection is the sum over the batch's views:
+    the volume of the whole batch equals the ACCUMULATE-d volumes of its two halves."""
+    dev = torch.device("cuda:0")
+    w = W.make_config(2)
+    g = w.geom
+    a = w.angles.float().numpy()
+    p = w.poses.float().numpy()
+    vol = w.volume(dev)
+    up = w.fwd_upstream(dev)
+    proj = dfp.forward(g, a, p, vol)
+    grad = dfp.forward_pose_grad(g, a, p, vol, up)
+    projf, mom = dfp.forward_fused_moments(g, a, p, vol, up)   # two lanes per ray: another fp32 order than `forward`
+    assert rel_l2(projf.cpu().numpy(), proj.cpu().numpy()) <= 1e-6
+    for sel in ([0], [63], [17, 40], [5, 6, 7]):
+        s = np.asarray(sel)
+        proj_s = dfp.forward(g, a[s], p[s], vol)
+        assert torch.equal(proj_s, proj[s]), sel
+        up_s = up[s].contiguous()
+        grad_s = dfp.forward_pose_grad(g, a[s], p[s], vol, up_s)
+        e = grad_err_u9(grad_s.cpu().numpy(), grad[s].cpu().numpy())
+        assert e.max() <= 2e-5, (sel, e)
+        proj_f, mom_s = dfp.forward_fused_moments(g, a[s], p[s], vol, up_s)
+        assert torch.equal(proj_f, projf[s]), sel
+        for k in range(3):
+            e = grad_err_u9(mom_s[:, k].cpu().numpy(), mom[s, k].cpu().numpy())
+            assert e.max() <= 2e-5, (sel, k, e)
+    del proj, projf, up, grad, mom
+    # upstream = the voxelised phantom (one sign): with config 2's N(0,1) field a view's 6-vector is the nearly
+    # cancelled sum of 1.7e7 random-sign terms and the fp32 rounding of the terms themselves shows at 1e-3 of U9
+    bup = vol
+    bproj = w.projections(dev)
+    bgrad = dfp.backproject_pose_grad(g, a, p, bproj, bup)
+    for sel in ([0], [63], [17, 40]):
+        s = np.asarray(sel)
+        bgrad_s = dfp.backproject_pose_grad(g, a[s], p[s], bproj[s].contiguous(), bup)
+        e = grad_err_u9(bgrad_s.cpu().numpy(), bgrad[s].cpu().numpy())
+        assert e.max() <= 1e-4, (sel, e)   # small batches get another tile depth / grid: fp32 partials in another order
+    whole = dfp.backproject(g, a, p, bproj)
+    halves = dfp.backproject(g, a[:32], p[:32], bproj[:32].contiguous())
+    ga = g.replace(flags=g.flags | dfp.FLAG_ACCUMULATE)
+    dfp.backproject(ga, a[32:], p[32:], bproj[32:].contiguous(), out=halves)
+    assert rel_l2(halves.cpu().numpy(), whole.cpu().numpy()) <= 2e-7
