@@ -10,7 +10,9 @@
 // Pins (tests/test_oracle_*.py, all `-m "not gpu"`): closed-form ellipsoid and Gaussian line
 // integrals, explicit-transpose adjointness, central finite differences in all six pose
 // parameters, the translation invariant dL/dt = -R A[grad mu], 6-accumulator vs the paper's
-// 12-element G route, stored-G literal algorithm, brute-force back-projection on tiny grids;
+// 12-element G route, stored-G literal algorithm on BOTH sides (forward: 12 stored G_f volumes projected;
+// back: stored central-difference images back-projected, Eq.13, G_b contracted - at general
+// non-integer (u,v)), brute-force back-projection on tiny grids;
 // Siddon weights (O12, tests/test_oracle_siddon.py): chord of the grid box, brute-force clipping
 // of the ray against every voxel's own box, explicit transpose, closed forms, the paper's literal
 // stored-G algorithm, finite differences of closed-form projections; Joseph weights (O13,

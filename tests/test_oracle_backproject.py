@@ -207,10 +207,10 @@ def test_backproject_grad_six_accumulators_equal_the_papers_twelve_element_route
             assert np.abs(a - b).max() <= 1e-11 * np.abs(b).max()
 
 
-def test_backproject_grad_central_difference_equals_backprojection_of_stored_difference_images():
-    """Structural identity (:198): with R = I the translation gradient dL/dt is the back-projection of the
-    stored central-difference images contracted with Eq.13's Jacobian; for a voxel on the central ray of a
-    view at beta=0 (J_u = (SDD/du)/w' e_y, J_v = (SDD/dv)/w' e_z) this is checked by hand."""
+def test_backproject_grad_of_one_voxel_on_the_central_ray_by_hand():
+    """One voxel on the central ray of a view at beta=0, identity pose: J_u = (SDD/du)/w' e_y, J_v = (SDD/dv)/w' e_z
+    (Eq.13 :143-146), the central differences are those of the pixel the voxel hits (a pixel CENTRE - the general,
+    non-integer (u,v) case is pinned by the stored-G_b test below), rotations move the voxel at (x0,0,0) by hand."""
     g0 = W.Geometry(nx=1, ny=1, nz=1, vx=1, vy=1, vz=1, nu=9, nv=7, du=1.5, dv=2.0, sad=100.0, sdd=160.0)
     proj = np.random.default_rng(8).standard_normal((1,) + g0.det_shape).astype(np.float32)
     x0 = 12.0                                        # voxel on the central axis, 12 mm towards the source
@@ -226,6 +226,78 @@ def test_backproject_grad_central_difference_equals_backprojection_of_stored_dif
     # rotations about the origin move the voxel at (x0,0,0): d r/d gz = (0,x0,0), d r/d gy = (0,0,-x0), d r/d gx = 0
     expect_r = np.array([0.0, -x0 * expect_t[2], x0 * expect_t[1]])
     assert np.abs(an[3:] - expect_r).max() < 1e-12
+
+
+def _dyadic(rng, shape, bits=6, span=64):
+    """Random values k / 2^bits, |k| <= span: sums, differences and halves of a few of them are exact in float32."""
+    return (rng.integers(-span, span + 1, size=shape) / float(1 << bits)).astype(np.float32)
+
+
+@pytest.mark.parametrize("bp_weight", [0, 1])
+def test_backproject_grad_central_mode_equals_the_papers_stored_Gb_algorithm(bp_weight):
+    """The paper's algorithm taken literally (PAPER.md :202-206, Eq.22 :200): "the gradient of the projection is
+    computed with central finite difference", "compute matrix G_b^i for each detector pixel", "backproject each
+    element of G_b", "accumulate" - here with STORED images instead of on-the-fly values:
+      1. the two central-difference images D_u[iv][iu] = (l[iv][iu+1] - l[iv][iu-1]) / 2, D_v likewise, of the
+         zero-extended projection, stored on the detector padded by one pixel per side (beyond it both neighbours
+         are outside the detector); shifting by exactly one pixel keeps the bilinear weights, so the interpolated
+         central difference of b~ IS the bilinear interpolation of these images;
+      2. each image back-projected with `oracle.backproject` (O8, pinned above) on a general anisotropic grid, pose
+         and view -> B[D_u]_j, B[D_v]_j (the weight W of a^ij included);
+      3. q_j = B[D_u]_j J_u(j) + B[D_v]_j J_v(j), J from Eq.13 (:143-146) built here in numpy from
+         `oracle.projection_matrix` (Eq.1, pinned by hand values) at r_j = R r'_j + t;
+      4. the 12-element G_b^j = q_j^T (x) (x', y', z', 1) (Eq.15 / 17 :155-168) summed with the upstream weights and
+         contracted with dM/dtheta (`oracle.rotation`: R, dR/dgamma_k, pinned by finite differences).
+    The projection values are dyadic rationals so that the stored difference images are exact in float32.
+    This pins `backproject_grad_impl` CENTRAL at NON-INTEGER (u, v): replacing its two difference lines
+    (0.5 * (b~(u+1,v) - b~(u-1,v)), same in v) by the half-pixel form b~(u+1/2,v) - b~(u-1/2,v) - which coincides
+    with it at pixel centres and passed every other pin - fails this test at the 1e-2 level (checked by mutation
+    when the test was written)."""
+    g = aniso_geom(bp_weight=bp_weight)
+    rng = np.random.default_rng(21)
+    angles = [0.3, 2.0]
+    poses = [POSE, [-2.0, 1.0, 0.3, -0.2, 0.15, -0.4]]
+    proj = _dyadic(rng, (2,) + g.det_shape)
+    w = rng.standard_normal(g.vol_shape).astype(np.float32)
+    # 1. stored difference images on the padded detector: index iu' = iu + 1; c_u' = c_u + 1 needs u0' = u0
+    gp = g.replace(nu=g.nu + 2, nv=g.nv + 2)
+    lp = np.zeros((2, g.nv + 4, g.nu + 4))                       # zero extension by two pixels per side
+    lp[:, 2:-2, 2:-2] = proj
+    Du = 0.5 * (lp[:, 1:-1, 2:] - lp[:, 1:-1, :-2])
+    Dv = 0.5 * (lp[:, 2:, 1:-1] - lp[:, :-2, 1:-1])
+    assert np.array_equal(Du.astype(np.float32), Du) and np.array_equal(Dv.astype(np.float32), Dv)
+    # voxel centres r'_j (O1)
+    iz, iy, ix = np.meshgrid(np.arange(g.nz), np.arange(g.ny), np.arange(g.nx), indexing="ij")
+    rp = np.stack([g.cx + (ix - (g.nx - 1) / 2) * g.vx, g.cy + (iy - (g.ny - 1) / 2) * g.vy,
+                   g.cz + (iz - (g.nz - 1) / 2) * g.vz], axis=-1)                            # [nz,ny,nx,3]
+    hom = np.concatenate([rp, np.ones(rp.shape[:-1] + (1,))], axis=-1)
+    expect = np.zeros((2, 6))
+    for v in range(2):
+        # 2. back-project each stored image
+        Bu = oracle.backproject(gp, angles[v:v + 1], poses[v:v + 1], Du[v:v + 1].astype(np.float32))
+        Bv = oracle.backproject(gp, angles[v:v + 1], poses[v:v + 1], Dv[v:v + 1].astype(np.float32))
+        # 3. Jacobian of Eq.13 at r_j = R r'_j + t
+        P = oracle.projection_matrix(g, angles[v])
+        R, dR = oracle.rotation(poses[v])
+        r = rp @ R.T + np.asarray(poses[v][:3])
+        up_ = r @ P[0, :3] + P[0, 3]
+        vp_ = r @ P[1, :3] + P[1, 3]
+        wp_ = r @ P[2, :3] + P[2, 3]
+        assert (wp_ > 0).all()
+        Ju = (P[0, :3][None, None, None, :] * wp_[..., None] - P[2, :3][None, None, None, :] * up_[..., None]) / wp_[..., None] ** 2
+        Jv = (P[1, :3][None, None, None, :] * wp_[..., None] - P[2, :3][None, None, None, :] * vp_[..., None]) / wp_[..., None] ** 2
+        q = Bu[..., None] * Ju + Bv[..., None] * Jv                                           # [nz,ny,nx,3]
+        # 4. grad_M L = sum_j w_j q_j^T (x) (x',y',z',1);  dL/dtheta_k = <dM/dtheta_k, grad_M L>
+        GM = np.einsum("zyx,zyxa,zyxb->ab", w.astype(np.float64), q, hom)                     # [3,4]
+        expect[v, :3] = GM[:, 3]                                                              # dM/dt_k = [0 | e_k]
+        for k in range(3):
+            expect[v, 3 + k] = (dR[k] * GM[:, :3]).sum()                                      # dM/dgamma_k = [dR_k | 0]
+    for route in (oracle.ROUTE_SIX, oracle.ROUTE_TWELVE):
+        an = oracle.backproject_pose_grad(g, angles, poses, proj, w, grad_mode=oracle.GRAD_CENTRAL, route=route)
+        assert np.abs(an - expect).max() <= 1e-11 * np.abs(expect).max(), (an, expect)
+    # the voxels do not sit on pixel centres: the identity is exercised at general fractional (u, v)
+    frac = np.abs((up_ / wp_) - np.rint(up_ / wp_))
+    assert np.median(frac) > 0.1
 
 
 def test_backproject_grad_zero_cases_and_linearity():
