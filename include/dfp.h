@@ -20,13 +20,18 @@
  *   d_* : DEVICE memory owned by the caller (e.g. torch tensors), fp32, contiguous, 16-byte aligned; read /
  *   written asynchronously on `stream` (a cudaStream_t passed as void*, NULL = default stream) and must stay
  *   alive until the stream reaches that point.  The library allocates no device memory in these calls and
- *   never synchronises the host; all scratch lives in the caller-provided workspace `d_ws`
- *   (>= dfp_workspace_bytes(...) bytes, 256-byte aligned).
+ *   does not wait for the GPU: all device scratch lives in the caller-provided workspace `d_ws`
+ *   (>= dfp_workspace_bytes(...) bytes, 256-byte aligned), and the per-view constants (<= 240 bytes per view, computed
+ *   on the host in fp64) reach it through a ring of 8 pinned host staging buffers owned by the calling thread (grown on
+ *   demand, freed when the thread ends), i.e. by true asynchronous copies; a call waits on the host only if the 8
+ *   previous uploads of this thread are all still pending.  Not meant for CUDA-graph capture.
+ *   n_views: 1 .. 2^24; batches of more than 65532 views are run as consecutive grid launches on `stream`.
  *   The dfp_*_host convenience calls take HOST arrays for the big buffers too, allocate and free their own
  *   device scratch on `stream` and return after the result has landed in host memory.
  *
  * Errors.  Every call returns an int status: DFP_OK (0) or a negative code; nothing is thrown, printed or
- *   exited.  On error no kernel has been launched.  Rays / voxels that miss contribute exact zeros (never NaN).
+ *   exited.  Arguments are validated for the whole call before any kernel is launched; only DFP_ERR_CUDA can be
+ *   returned after work was queued.  Rays / voxels that miss contribute exact zeros (never NaN).
  */
 #ifndef DFP_H_
 #define DFP_H_
@@ -85,7 +90,7 @@ typedef struct dfp_geometry {
 enum {
   DFP_OK = 0,
   DFP_ERR_NULL = -1,       /* a required pointer is NULL                                                    */
-  DFP_ERR_DIMS = -2,       /* non-positive size / pitch, sad <= 0, sdd <= sad, n_views <= 0, index overflow */
+  DFP_ERR_DIMS = -2,       /* non-positive size / pitch, sad <= 0, sdd <= sad, n_views <= 0 or > 2^24, index overflow */
   DFP_ERR_NONFINITE = -3,  /* NaN / Inf in geometry, angles or poses                                        */
   DFP_ERR_ALIGN = -4,      /* a device pointer is not 16-byte (workspace: 256-byte) aligned                 */
   DFP_ERR_WORKSPACE = -5,  /* ws_bytes < dfp_workspace_bytes(...)                                           */
@@ -146,8 +151,10 @@ size_t dfp_workspace_bytes(const dfp_geometry* geometry, int n_views, int op);
 
 /* Same four operations with HOST buffers (h_*: host memory, pinned or pageable).  Each allocates device
  * scratch with cudaMallocAsync on `stream`, copies inputs in, runs the device call above, copies the result
- * out, frees, and synchronises `stream` before returning.  With 8 or more views the per-view arrays move in 4
- * chunks on an internal second stream, overlapped with the kernels of the neighbouring chunk (per-view results do
+ * out, frees, and synchronises `stream` before returning (also on an error that occurs after work was queued: the
+ * caller's buffers are never touched after the call has returned).  With 8 or more views the per-view arrays move in
+ * up to 4 chunks (boundaries on multiples of 4 views, so every chunk pointer keeps its 16-byte alignment for any nu, nv)
+ * on an internal second stream, overlapped with the kernels of the neighbouring chunk (per-view results do
  * not depend on the chunking; dfp_backproject_host sums its chunks with DFP_FLAG_ACCUMULATE, which changes the
  * fp32 summation order only).  The
  * first host call on a device raises the release threshold of its default stream-ordered memory pool so that
@@ -162,10 +169,12 @@ int dfp_backproject_pose_grad_host(const dfp_geometry* geometry, int n_views, co
                                    const float* poses, const float* h_proj, const float* h_dLdvol, float* h_grad,
                                    void* stream);
 
-/* Number of ray-steps one dfp_forward / dfp_forward_pose_grad call marches in the default (trilinear) mode: samples
- * inside the gradient's clip box, summed over rays and views; the unit of the "Gray-steps/s" metric.  Counted by a small
- * kernel that runs the same per-ray clip (fp64) as the projectors, on the default stream, synchronously; allocates
- * and frees its own scratch.  Returns -1 on invalid arguments or CUDA failure. */
+/* The unit of the "Gray-steps/s" metric: the number of (ray, sample) pairs, summed over rays and
+ * views, whose sample tau_k = (k + 1/2) D lies in the volume box padded by exactly 2 voxels (continuous voxel index in
+ * [-2, n + 1] on every axis) - the set the oracle's forward projector counts; one number for both dfp_forward and
+ * dfp_forward_pose_grad in the default (trilinear) mode, whatever slightly different box each kernel marches.  Counted
+ * by a small kernel that runs the projectors' per-ray clip (fp64) against that box, on the default stream,
+ * synchronously; allocates and frees its own scratch.  Returns -1 on invalid arguments or CUDA failure. */
 int64_t dfp_count_ray_steps(const dfp_geometry* geometry, int n_views, const float* angles, const float* poses);
 
 /* Kernel timing for roofline accounting.  dfp_set_kernel_timing(1) makes every later device-pointer call on
@@ -192,17 +201,6 @@ const char* dfp_status_string(int status);
 
 /* Library version (major*10000 + minor*100 + patch). */
 int dfp_version(void);
-
-/* Measured denominators for the roofline of the projector kernels, which are bound by the SM-side pipes and not by HBM
- * (DESIGN.md "Roofline").  Runs one resident wave of a small kernel on the current device (default
- * stream, synchronous, timed with CUDA events, allocates and frees a few MB of scratch) and writes the sustained rate
- * of the WHOLE DEVICE PER SECOND (divide by SM count x SM clock for the rate per clock per SM):
- *   DFP_MB_LDS   warp-wide, bank-conflict-free LDS.32 instructions (the staged gradient kernels need 32 per warp-sample
- *                and 12 per warp-voxel-view);
- *   DFP_MB_FADD / DFP_MB_FFMA / DFP_MB_FFMA2   fp32 results of dependent-free FADD, FFMA and packed FFMA2 streams.
- * Returns DFP_OK, DFP_ERR_NULL, DFP_ERR_DIMS (unknown kind) or DFP_ERR_CUDA. */
-enum { DFP_MB_LDS = 0, DFP_MB_FADD = 1, DFP_MB_FFMA = 2, DFP_MB_FFMA2 = 3 };
-int dfp_microbench(int kind, double* per_second);
 
 #ifdef __cplusplus
 }

@@ -4,6 +4,7 @@ Device-pointer calls take torch CUDA tensors (fp32, contiguous) and run asynchro
 stream; `*_host` calls take CPU tensors / numpy arrays.  `angles` / `poses` are host arrays (any float
 sequence; rounded to fp32, which is what the C ABI takes).
 """
+import contextlib
 import ctypes
 import os
 
@@ -87,8 +88,6 @@ def _load():
     lib.dfp_set_kernel_timing.restype = ci
     lib.dfp_last_kernel_ms.argtypes = []
     lib.dfp_last_kernel_ms.restype = ctypes.c_float
-    lib.dfp_microbench.argtypes = [ci, ctypes.POINTER(ctypes.c_double)]
-    lib.dfp_microbench.restype = ci
     lib.dfp_status_string.argtypes = [ci]
     lib.dfp_status_string.restype = cp
     return lib
@@ -125,16 +124,6 @@ def set_kernel_timing(enable: bool) -> None:
 def last_kernel_ms() -> float:
     """Milliseconds of the dominant kernel of the last device-pointer call (waits for it); -1 if timing is off."""
     return float(_lib.dfp_last_kernel_ms())
-
-
-MB_LDS, MB_FADD, MB_FFMA, MB_FFMA2 = 0, 1, 2, 3
-
-
-def microbench(kind: int) -> float:
-    """Sustained whole-device rate per second of one SM-side pipe (include/dfp.h: dfp_microbench) on the current device."""
-    r = ctypes.c_double(0.0)
-    _check(_lib.dfp_microbench(int(kind), ctypes.byref(r)))
-    return float(r.value)
 
 
 def _check(status):
@@ -177,8 +166,21 @@ def _workspace(g, V, op, ws, device):
     return ws, ctypes.c_void_p(ws.data_ptr()), ctypes.c_size_t(ws.numel() * ws.element_size())
 
 
-def _stream():
-    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+def _stream(t=None):
+    """torch's current stream ON THE TENSORS' DEVICE (the library launches on the thread's current device, which the
+    device-pointer wrappers set to that device for the duration of the call)."""
+    dev = t.device if (torch.is_tensor(t) and t.is_cuda) else None
+    return ctypes.c_void_p(torch.cuda.current_stream(dev).cuda_stream)
+
+
+def _same_device(*tensors):
+    ts = [t for t in tensors if torch.is_tensor(t) and t.is_cuda]
+    if not ts:
+        return contextlib.nullcontext()          # the argument checks of the call report what is wrong
+    for t in ts:
+        if t.device != ts[0].device:
+            raise ValueError(f"all device tensors of a call must live on one device ({ts[0].device} vs {t.device})")
+    return torch.cuda.device(ts[0].device)
 
 
 def _np_ptr(a):
@@ -192,8 +194,9 @@ def forward(geom, angles, poses, vol, out=None, ws=None):
     if out is None:
         out = torch.empty((V, g.nv, g.nu), dtype=torch.float32, device=vol.device)
     ws, wp, wn = _workspace(g, V, OP_FORWARD, ws, vol.device)
-    _check(_lib.dfp_forward(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p), _dev(vol, (g.nz, g.ny, g.nx), "vol"),
-                            _dev(out, (V, g.nv, g.nu), "proj"), wp, wn, _stream()))
+    with _same_device(vol, out, ws):
+        _check(_lib.dfp_forward(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p), _dev(vol, (g.nz, g.ny, g.nx), "vol"),
+                                _dev(out, (V, g.nv, g.nu), "proj"), wp, wn, _stream(vol)))
     return out
 
 
@@ -204,10 +207,11 @@ def forward_pose_grad(geom, angles, poses, vol, dLdproj, out=None, ws=None):
     if out is None:
         out = torch.empty((V, 6), dtype=torch.float32, device=vol.device)
     ws, wp, wn = _workspace(g, V, OP_FORWARD_POSE_GRAD, ws, vol.device)
-    _check(_lib.dfp_forward_pose_grad(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p),
-                                      _dev(vol, (g.nz, g.ny, g.nx), "vol"),
-                                      _dev(dLdproj, (V, g.nv, g.nu), "dLdproj"), _dev(out, (V, 6), "grad"), wp, wn,
-                                      _stream()))
+    with _same_device(vol, dLdproj, out, ws):
+        _check(_lib.dfp_forward_pose_grad(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p),
+                                          _dev(vol, (g.nz, g.ny, g.nx), "vol"),
+                                          _dev(dLdproj, (V, g.nv, g.nu), "dLdproj"), _dev(out, (V, 6), "grad"), wp, wn,
+                                          _stream(vol)))
     return out
 
 
@@ -220,11 +224,12 @@ def forward_fused_moments(geom, angles, poses, vol, target, out_proj=None, out_m
     if out_moments is None:
         out_moments = torch.empty((V, 3, 6), dtype=torch.float32, device=vol.device)
     ws, wp, wn = _workspace(g, V, OP_FORWARD_FUSED, ws, vol.device)
-    _check(_lib.dfp_forward_fused_moments(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p),
-                                          _dev(vol, (g.nz, g.ny, g.nx), "vol"),
-                                          _dev(target, (V, g.nv, g.nu), "target"),
-                                          _dev(out_proj, (V, g.nv, g.nu), "proj"),
-                                          _dev(out_moments, (V, 3, 6), "moments"), wp, wn, _stream()))
+    with _same_device(vol, target, out_proj, out_moments, ws):
+        _check(_lib.dfp_forward_fused_moments(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p),
+                                              _dev(vol, (g.nz, g.ny, g.nx), "vol"),
+                                              _dev(target, (V, g.nv, g.nu), "target"),
+                                              _dev(out_proj, (V, g.nv, g.nu), "proj"),
+                                              _dev(out_moments, (V, 3, 6), "moments"), wp, wn, _stream(vol)))
     return out_proj, out_moments
 
 
@@ -235,8 +240,9 @@ def backproject(geom, angles, poses, proj, out=None, ws=None):
     if out is None:
         out = torch.empty((g.nz, g.ny, g.nx), dtype=torch.float32, device=proj.device)
     ws, wp, wn = _workspace(g, V, OP_BACKPROJECT, ws, proj.device)
-    _check(_lib.dfp_backproject(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p), _dev(proj, (V, g.nv, g.nu), "proj"),
-                                _dev(out, (g.nz, g.ny, g.nx), "vol"), wp, wn, _stream()))
+    with _same_device(proj, out, ws):
+        _check(_lib.dfp_backproject(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p), _dev(proj, (V, g.nv, g.nu), "proj"),
+                                    _dev(out, (g.nz, g.ny, g.nx), "vol"), wp, wn, _stream(proj)))
     return out
 
 
@@ -247,10 +253,11 @@ def backproject_pose_grad(geom, angles, poses, proj, dLdvol, out=None, ws=None):
     if out is None:
         out = torch.empty((V, 6), dtype=torch.float32, device=proj.device)
     ws, wp, wn = _workspace(g, V, OP_BACKPROJECT_POSE_GRAD, ws, proj.device)
-    _check(_lib.dfp_backproject_pose_grad(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p),
-                                          _dev(proj, (V, g.nv, g.nu), "proj"),
-                                          _dev(dLdvol, (g.nz, g.ny, g.nx), "dLdvol"), _dev(out, (V, 6), "grad"), wp,
-                                          wn, _stream()))
+    with _same_device(proj, dLdvol, out, ws):
+        _check(_lib.dfp_backproject_pose_grad(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p),
+                                              _dev(proj, (V, g.nv, g.nu), "proj"),
+                                              _dev(dLdvol, (g.nz, g.ny, g.nx), "dLdvol"), _dev(out, (V, 6), "grad"), wp,
+                                              wn, _stream(proj)))
     return out
 
 

@@ -13,7 +13,6 @@
 #include "dfp_bp_tma.cuh"
 #include "dfp_fwd_tma.cuh"
 #include "dfp_kernels.cuh"
-#include "dfp_microbench.cuh"
 #include "dfp_params.h"
 #include "dfp_joseph.cuh"
 #include "dfp_siddon.cuh"
@@ -28,17 +27,84 @@ thread_local int g_path = DFP_PATH_GATHER;
 
 thread_local bool g_timing = false;
 thread_local cudaEvent_t g_ev[2] = {nullptr, nullptr};
+thread_local int g_ev_dev = -1;              // the device the two events belong to
 thread_local bool g_ev_valid = false;
 
 void time_begin(cudaStream_t s) {
   g_ev_valid = false;
   if (!g_timing) return;
-  if (!g_ev[0] && (cudaEventCreate(&g_ev[0]) != cudaSuccess || cudaEventCreate(&g_ev[1]) != cudaSuccess)) return;
-  cudaEventRecord(g_ev[0], s);
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) return;
+  if (g_ev[0] && dev != g_ev_dev) {          // events are per device: the caller switched devices
+    cudaEventDestroy(g_ev[0]); cudaEventDestroy(g_ev[1]);
+    g_ev[0] = g_ev[1] = nullptr;
+  }
+  if (!g_ev[0]) {
+    if (cudaEventCreate(&g_ev[0]) != cudaSuccess || cudaEventCreate(&g_ev[1]) != cudaSuccess) {
+      g_ev[0] = g_ev[1] = nullptr;
+      cudaGetLastError();
+      return;
+    }
+    g_ev_dev = dev;
+  }
+  if (cudaEventRecord(g_ev[0], s) != cudaSuccess) cudaGetLastError();   // timing is best effort: never fails the call
 }
 void time_end(cudaStream_t s) {
   if (!g_timing || !g_ev[1]) return;
   g_ev_valid = cudaEventRecord(g_ev[1], s) == cudaSuccess;
+  if (!g_ev_valid) cudaGetLastError();
+}
+
+// Per-view constants go to the device through a small ring of PINNED host buffers owned by the calling thread, so
+// that the upload is a true asynchronous copy (a cudaMemcpyAsync from pageable memory is staged by the runtime and
+// may block the host).  A slot is reused only after the copy that last read it has completed (its event); with
+// kStageSlots calls in flight that wait never triggers in practice.  Slots grow on demand and live until the thread
+// ends (host memory only: the library still allocates no device memory in the device-pointer calls).
+constexpr int kStageSlots = 8;
+struct StageRing {
+  void* buf[kStageSlots] = {};
+  size_t cap[kStageSlots] = {};
+  cudaEvent_t ev[kStageSlots] = {};
+  int dev[kStageSlots] = {};
+  int next = 0;
+  ~StageRing() {
+    for (int i = 0; i < kStageSlots; ++i) {
+      if (ev[i]) cudaEventDestroy(ev[i]);
+      if (buf[i]) cudaFreeHost(buf[i]);
+    }
+  }
+};
+thread_local StageRing g_stage;
+
+// Copies `bytes` from pageable host memory `src` to device memory `dst` on stream `s` without blocking on the GPU.
+cudaError_t upload_async(void* dst, const void* src, size_t bytes, cudaStream_t s) {
+  StageRing& R = g_stage;
+  const int i = R.next;
+  R.next = (R.next + 1) % kStageSlots;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (R.ev[i] && R.dev[i] != dev) { cudaEventDestroy(R.ev[i]); R.ev[i] = nullptr; }
+  if (R.ev[i]) {
+    e = cudaEventSynchronize(R.ev[i]);       // the copy that last used this slot (kStageSlots uploads ago)
+    if (e != cudaSuccess) return e;
+  } else {
+    e = cudaEventCreateWithFlags(&R.ev[i], cudaEventDisableTiming);
+    if (e != cudaSuccess) { R.ev[i] = nullptr; return e; }
+    R.dev[i] = dev;
+  }
+  if (R.cap[i] < bytes) {
+    if (R.buf[i]) cudaFreeHost(R.buf[i]);
+    R.buf[i] = nullptr; R.cap[i] = 0;
+    const size_t want = bytes < 65536 ? 65536 : bytes + bytes / 2;
+    e = cudaHostAlloc(&R.buf[i], want, cudaHostAllocDefault);
+    if (e != cudaSuccess) { R.buf[i] = nullptr; return e; }
+    R.cap[i] = want;
+  }
+  std::memcpy(R.buf[i], src, bytes);
+  e = cudaMemcpyAsync(dst, R.buf[i], bytes, cudaMemcpyHostToDevice, s);
+  if (e != cudaSuccess) return e;
+  return cudaEventRecord(R.ev[i], s);
 }
 
 int cuda_fail(cudaError_t e, const char* where) {
@@ -72,8 +138,13 @@ int validate_geometry(const dfp_geometry* g) {
   return DFP_OK;
 }
 
+// Views ride on blockIdx.z (<= 65535): larger batches are run as consecutive slices of kMaxViewsPerLaunch views
+// (a multiple of 4, so that every slice's projection / gradient pointers keep their 16-byte alignment).
+constexpr int kMaxViewsPerLaunch = 65532;
+constexpr int kMaxViews = 1 << 24;
+
 int validate_views(const dfp_geometry& g, int n_views, const float* angles, const float* poses) {
-  if (n_views <= 0 || n_views > 65535) return DFP_ERR_DIMS;
+  if (n_views <= 0 || n_views > kMaxViews) return DFP_ERR_DIMS;
   if (!angles || !poses) return DFP_ERR_NULL;
   const int stride = view_stride(g);
   for (int v = 0; v < n_views; ++v) {
@@ -314,9 +385,9 @@ int check_common(const dfp_geometry* g, int n_views, const float* angles, const 
 
 // op = DFP_OP_FORWARD (d_out = projections), DFP_OP_FORWARD_POSE_GRAD (d_up = upstream, d_out = gradients) or
 // DFP_OP_FORWARD_FUSED (d_up = target b, d_out = moments [V][3][6], d_proj = projections)
-int run_forward(const dfp_geometry* g, int V, const float* angles, const float* poses, const float* d_vol,
-                const float* d_up, float* d_out, void* d_ws, size_t ws_bytes, cudaStream_t s, int op,
-                float* d_proj = nullptr) {
+int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const float* poses, const float* d_vol,
+                      const float* d_up, float* d_out, void* d_ws, size_t ws_bytes, cudaStream_t s, int op,
+                      float* d_proj) {
   if (!g) return DFP_ERR_NULL;
   int st = validate_geometry(g);
   if (st) return st;
@@ -346,8 +417,8 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
   float4* pvol = reinterpret_cast<float4*>(base + w.off_pvol);
   float* part = reinterpret_cast<float*>(base + w.off_part);
   g_launches = 0;
-  DFP_CUDA(cudaMemcpyAsync(dv, hv.data(), sizeof(FwdView) * V, cudaMemcpyHostToDevice, s), "view upload");
-  if (grad) DFP_CUDA(cudaMemcpyAsync(dc, hc.data(), sizeof(FwdContract) * V, cudaMemcpyHostToDevice, s), "view upload");
+  DFP_CUDA(upload_async(dv, hv.data(), sizeof(FwdView) * V, s), "view upload");
+  if (grad) DFP_CUDA(upload_async(dc, hc.data(), sizeof(FwdContract) * V, s), "view upload");
   const dim3 grid(w.gx, w.gy, V);
   if (siddon || joseph) {   // other weight models (dfp_siddon.cuh, dfp_joseph.cuh): straight over the caller's volume
     g_path = DFP_PATH_GATHER;
@@ -400,25 +471,27 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
   if (tma) {
     DFP_CUDA(ensure_smem_attributes(), "cudaFuncSetAttribute");
     time_begin(s);
-    const dim3 ggrid(w.gx, w.gy8, V);
+    // 1-D grid, one block per (view, tile), ordered view group -> tile -> view (dfp_fwd_tma.cuh: fwd_block)
+    const FwdGrid Qf{V, w.gx, w.gy}, Qg{V, w.gx, w.gy8};
+    const unsigned nbf = (unsigned)V * w.gx * w.gy, nbg = (unsigned)V * w.gx * w.gy8;
     if (fused && shape == 3)
-      fwd_tma_kernel<3, 3><<<ggrid, TmaLanes<3>::THREADS, tma_smem_bytes<3>(), s>>>(G, dv, vol_map, d_up, part, d_proj);
+      fwd_tma_kernel<3, 3><<<nbg, TmaLanes<3>::THREADS, tma_smem_bytes<3>(), s>>>(G, Qg, dv, vol_map, d_up, part, d_proj);
     else if (fused)
-      fwd_tma_kernel<3, 2><<<ggrid, TmaLanes<3>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, d_up, part, d_proj);
+      fwd_tma_kernel<3, 2><<<nbg, TmaLanes<3>::THREADS, tma_smem_bytes<2>(), s>>>(G, Qg, dv, vol_map, d_up, part, d_proj);
     else if (grad && interp && shape == 3)
-      fwd_tma_kernel<2, 3><<<ggrid, TmaLanes<2>::THREADS, tma_smem_bytes<3>(), s>>>(G, dv, vol_map, d_up, part, nullptr);
+      fwd_tma_kernel<2, 3><<<nbg, TmaLanes<2>::THREADS, tma_smem_bytes<3>(), s>>>(G, Qg, dv, vol_map, d_up, part, nullptr);
     else if (grad && interp)
-      fwd_tma_kernel<2, 2><<<ggrid, TmaLanes<2>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, d_up, part, nullptr);
+      fwd_tma_kernel<2, 2><<<nbg, TmaLanes<2>::THREADS, tma_smem_bytes<2>(), s>>>(G, Qg, dv, vol_map, d_up, part, nullptr);
     else if (grad && shape == 3)
-      fwd_tma_kernel<1, 3><<<ggrid, TmaLanes<1>::THREADS, tma_smem_bytes<3>(), s>>>(G, dv, vol_map, d_up, part, nullptr);
+      fwd_tma_kernel<1, 3><<<nbg, TmaLanes<1>::THREADS, tma_smem_bytes<3>(), s>>>(G, Qg, dv, vol_map, d_up, part, nullptr);
     else if (grad)
-      fwd_tma_kernel<1, 2><<<ggrid, TmaLanes<1>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, d_up, part, nullptr);
+      fwd_tma_kernel<1, 2><<<nbg, TmaLanes<1>::THREADS, tma_smem_bytes<2>(), s>>>(G, Qg, dv, vol_map, d_up, part, nullptr);
     else if (shape == 0)
-      fwd_tma_kernel<0, 0><<<grid, TmaLanes<0>::THREADS, tma_smem_bytes<0>(), s>>>(G, dv, vol_map, nullptr, d_out, nullptr);
+      fwd_tma_kernel<0, 0><<<nbf, TmaLanes<0>::THREADS, tma_smem_bytes<0>(), s>>>(G, Qf, dv, vol_map, nullptr, d_out, nullptr);
     else if (shape == 1)
-      fwd_tma_kernel<0, 1><<<grid, TmaLanes<0>::THREADS, tma_smem_bytes<1>(), s>>>(G, dv, vol_map, nullptr, d_out, nullptr);
+      fwd_tma_kernel<0, 1><<<nbf, TmaLanes<0>::THREADS, tma_smem_bytes<1>(), s>>>(G, Qf, dv, vol_map, nullptr, d_out, nullptr);
     else
-      fwd_tma_kernel<0, 2><<<grid, TmaLanes<0>::THREADS, tma_smem_bytes<2>(), s>>>(G, dv, vol_map, nullptr, d_out, nullptr);
+      fwd_tma_kernel<0, 2><<<nbf, TmaLanes<0>::THREADS, tma_smem_bytes<2>(), s>>>(G, Qf, dv, vol_map, nullptr, d_out, nullptr);
     time_end(s);
     ++g_launches;
     const int nblk8 = w.gx * w.gy8;
@@ -463,8 +536,8 @@ int run_forward(const dfp_geometry* g, int V, const float* angles, const float* 
   return DFP_OK;
 }
 
-int run_backproject(const dfp_geometry* g, int V, const float* angles, const float* poses, const float* d_proj,
-                    const float* d_up, float* d_out, void* d_ws, size_t ws_bytes, cudaStream_t s, bool grad) {
+int run_backproject_slice(const dfp_geometry* g, int V, const float* angles, const float* poses, const float* d_proj,
+                          const float* d_up, float* d_out, void* d_ws, size_t ws_bytes, cudaStream_t s, bool grad) {
   if (!g) return DFP_ERR_NULL;
   int st = validate_geometry(g);
   if (st) return st;
@@ -484,8 +557,8 @@ int run_backproject(const dfp_geometry* g, int V, const float* angles, const flo
   float* part = reinterpret_cast<float*>(base + w.off_part);
   g_launches = 0;
   g_path = DFP_PATH_GATHER;
-  DFP_CUDA(cudaMemcpyAsync(dv, hv.data(), sizeof(BpView) * V, cudaMemcpyHostToDevice, s), "view upload");
-  if (grad) DFP_CUDA(cudaMemcpyAsync(dc, hc.data(), sizeof(BpContract) * V, cudaMemcpyHostToDevice, s), "view upload");
+  DFP_CUDA(upload_async(dv, hv.data(), sizeof(BpView) * V, s), "view upload");
+  if (grad) DFP_CUDA(upload_async(dc, hc.data(), sizeof(BpContract) * V, s), "view upload");
   // TMA-staged path: projections admit a tensor map, every voxel in front of the source, patches fit the menu
   int kmax = -1, TZ = 16;
   if (!(g->flags & DFP_FLAG_NO_TMA) && (g->nu % 4) == 0) {
@@ -566,6 +639,56 @@ int run_backproject(const dfp_geometry* g, int V, const float* angles, const flo
   return DFP_OK;
 }
 
+// More views than one grid holds: consecutive slices on the same stream (the workspace is reused in stream order).
+// Everything is validated for the WHOLE call first, so that an error is returned before any kernel is launched.
+int run_forward(const dfp_geometry* g, int V, const float* angles, const float* poses, const float* d_vol,
+                const float* d_up, float* d_out, void* d_ws, size_t ws_bytes, cudaStream_t s, int op,
+                float* d_proj = nullptr) {
+  if (V <= kMaxViewsPerLaunch || !g) return run_forward_slice(g, V, angles, poses, d_vol, d_up, d_out, d_ws, ws_bytes, s, op, d_proj);
+  int st = validate_geometry(g);
+  if (st) return st;
+  const bool grad = op != DFP_OP_FORWARD, fused = op == DFP_OP_FORWARD_FUSED;
+  st = check_common(g, V, angles, poses, d_vol, d_out, grad ? (const void*)d_up : (const void*)d_vol, d_ws, ws_bytes,
+                    fwd_ws(*g, V, grad, fused ? 3 : 1).total);
+  if (st) return st;
+  const size_t per_view = (size_t)g->nu * g->nv, stride = (size_t)view_stride(*g);
+  const int per_out = fused ? 18 : 6;
+  int launches = 0;
+  for (int v0 = 0; v0 < V; v0 += kMaxViewsPerLaunch) {
+    const int n = V - v0 < kMaxViewsPerLaunch ? V - v0 : kMaxViewsPerLaunch;
+    st = run_forward_slice(g, n, angles + stride * v0, poses + 6 * (size_t)v0, d_vol, d_up ? d_up + per_view * v0 : nullptr,
+                           grad ? d_out + (size_t)per_out * v0 : d_out + per_view * v0, d_ws, ws_bytes, s, op,
+                           d_proj ? d_proj + per_view * v0 : nullptr);
+    if (st) return st;
+    launches += g_launches;
+  }
+  g_launches = launches;
+  return DFP_OK;
+}
+
+int run_backproject(const dfp_geometry* g, int V, const float* angles, const float* poses, const float* d_proj,
+                    const float* d_up, float* d_out, void* d_ws, size_t ws_bytes, cudaStream_t s, bool grad) {
+  if (V <= kMaxViewsPerLaunch || !g) return run_backproject_slice(g, V, angles, poses, d_proj, d_up, d_out, d_ws, ws_bytes, s, grad);
+  int st = validate_geometry(g);
+  if (st) return st;
+  st = check_common(g, V, angles, poses, d_proj, d_out, grad ? (const void*)d_up : (const void*)d_proj, d_ws, ws_bytes,
+                    bp_ws(*g, V, grad).total);
+  if (st) return st;
+  const size_t per_view = (size_t)g->nu * g->nv, stride = (size_t)view_stride(*g);
+  int launches = 0;
+  for (int v0 = 0; v0 < V; v0 += kMaxViewsPerLaunch) {
+    const int n = V - v0 < kMaxViewsPerLaunch ? V - v0 : kMaxViewsPerLaunch;
+    dfp_geometry gc = *g;                 // dfp_backproject: the first slice overwrites the volume, the others add to it
+    if (!grad && v0) gc.flags |= DFP_FLAG_ACCUMULATE;
+    st = run_backproject_slice(&gc, n, angles + stride * v0, poses + 6 * (size_t)v0, d_proj + per_view * v0, d_up,
+                               grad ? d_out + 6 * (size_t)v0 : d_out, d_ws, ws_bytes, s, grad);
+    if (st) return st;
+    launches += g_launches;
+  }
+  g_launches = launches;
+  return DFP_OK;
+}
+
 // ---- host-buffer wrappers ------------------------------------------------------------------------
 struct DevBuf {
   void* p = nullptr;
@@ -621,19 +744,24 @@ int run_host(int op, const dfp_geometry* g, int V, const float* angles, const fl
     else
       st = run_backproject(g, V, angles, poses, (const float*)d_in.p, (const float*)d_up.p, (float*)d_out.p, d_ws.p,
                            n_ws, s, grad);
-    if (st) return st;
+    if (st) { cudaStreamSynchronize(s); return st; }
     DFP_CUDA(cudaMemcpyAsync(h_out, d_out.p, n_out, cudaMemcpyDeviceToHost, s), "D2H");
     DFP_CUDA(cudaStreamSynchronize(s), "stream synchronize");
     return DFP_OK;
   }
   struct Side {                      // the copy stream and its events, released on every exit path
-    cudaStream_t s2 = nullptr;
+    cudaStream_t s = nullptr, s2 = nullptr;
+    bool ok = false;                 // set on the normal exit (which has synchronised both streams itself)
     cudaEvent_t ev[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     ~Side() {
+      // error exit in mid-loop: copies of earlier chunks may still be in flight - wait for them before the device
+      // buffers are freed and before the caller regains h_out
+      if (!ok) { if (s2) cudaStreamSynchronize(s2); cudaStreamSynchronize(s); }
       for (cudaEvent_t e : ev) if (e) cudaEventDestroy(e);
       if (s2) cudaStreamDestroy(s2);
     }
   } side;
+  side.s = s;
   DFP_CUDA(cudaStreamCreateWithFlags(&side.s2, cudaStreamNonBlocking), "cudaStreamCreate");
   for (cudaEvent_t& e : side.ev) DFP_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming), "cudaEventCreate");
   const size_t per_view = (size_t)g->nu * g->nv;            // floats of one view's projection / upstream image
@@ -647,9 +775,11 @@ int run_host(int op, const dfp_geometry* g, int V, const float* angles, const fl
   if (h_shared) DFP_CUDA(cudaMemcpyAsync(d_shared, h_shared, nvol, cudaMemcpyHostToDevice, s), "H2D");
   int launches = 0;
   for (int c = 0; c < n_chunks; ++c) {
-    // chunk boundaries on even views: a gradient chunk writes d_grad + 6 v0 floats, which must stay 16-byte aligned
-    const int v0 = (int)((long long)V * c / n_chunks) & ~1;
-    const int v1 = c + 1 == n_chunks ? V : (int)((long long)V * (c + 1) / n_chunks) & ~1, nv_c = v1 - v0;
+    // chunk boundaries on multiples of 4 views: a chunk reads / writes d_views + v0 nu nv floats and d_grad + 6 v0
+    // floats, which must stay 16-byte aligned whatever the parity of nu nv; a chunk that comes out empty is skipped
+    const int v0 = (int)((long long)V * c / n_chunks) & ~3;
+    const int v1 = c + 1 == n_chunks ? V : (int)((long long)V * (c + 1) / n_chunks) & ~3, nv_c = v1 - v0;
+    if (nv_c <= 0) continue;
     const size_t off = (size_t)v0 * per_view;
     if (h_views) {                   // this chunk's per-view input on the copy stream, then the kernels wait for it
       DFP_CUDA(cudaMemcpyAsync(d_views + off, h_views + off, (size_t)nv_c * per_view * 4, cudaMemcpyHostToDevice,
@@ -665,7 +795,7 @@ int run_host(int op, const dfp_geometry* g, int V, const float* angles, const fl
       st = run_backproject(g, nv_c, angles + (size_t)view_stride(*g) * v0, poses + 6 * v0, d_views + off, d_shared, out_c, d_ws.p, n_ws, s, true);
     else {                           // dfp_backproject: the first chunk overwrites the volume, the others add to it
       dfp_geometry gc = *g;
-      gc.flags = c ? (g->flags | DFP_FLAG_ACCUMULATE) : g->flags;
+      gc.flags = v0 ? (g->flags | DFP_FLAG_ACCUMULATE) : g->flags;
       st = run_backproject(&gc, nv_c, angles + (size_t)view_stride(*g) * v0, poses + 6 * v0, d_views + off, nullptr, static_cast<float*>(d_out.p),
                            d_ws.p, n_ws, s, false);
     }
@@ -682,6 +812,7 @@ int run_host(int op, const dfp_geometry* g, int V, const float* angles, const fl
   if (grad || !fwd) DFP_CUDA(cudaMemcpyAsync(h_out, d_out.p, n_out, cudaMemcpyDeviceToHost, s), "D2H");
   DFP_CUDA(cudaStreamSynchronize(side.s2), "stream synchronize");
   DFP_CUDA(cudaStreamSynchronize(s), "stream synchronize");
+  side.ok = true;
   return DFP_OK;
 }
 
@@ -723,7 +854,7 @@ int dfp_backproject_pose_grad(const dfp_geometry* g, int n_views, const float* a
 }
 
 size_t dfp_workspace_bytes(const dfp_geometry* g, int n_views, int op) {
-  if (validate_geometry(g) != DFP_OK || n_views <= 0 || n_views > 65535) return 0;
+  if (validate_geometry(g) != DFP_OK || n_views <= 0 || n_views > kMaxViews) return 0;
   switch (op) {
     case DFP_OP_FORWARD: return fwd_ws(*g, n_views, false).total;
     case DFP_OP_FORWARD_POSE_GRAD: return fwd_ws(*g, n_views, true).total;
@@ -753,7 +884,14 @@ int dfp_backproject_pose_grad_host(const dfp_geometry* g, int n_views, const flo
 
 int64_t dfp_count_ray_steps(const dfp_geometry* g, int n_views, const float* angles, const float* poses) {
   if (validate_geometry(g) != DFP_OK || validate_views(*g, n_views, angles, poses) != DFP_OK) return -1;
-  const FwdGeom G = make_fwd_geom(*g, true);
+  // the metric's unit: samples tau_k = (k + 1/2) D whose position lies in the volume box padded by
+  // EXACTLY 2 voxels (closed box, continuous voxel index in [-2, n + 1] per axis) - the oracle's clip; one count for
+  // both the forward and the gradient pass, whatever (slightly larger or smaller) box the kernels march
+  FwdGeom G = make_fwd_geom(*g, true);
+  {
+    const int n[3] = {g->nx, g->ny, g->nz}, H[3] = {G.L.hx, G.L.hy, G.L.hz};
+    for (int a = 0; a < 3; ++a) { G.lo[a] = (float)(-2 - H[a]); G.hi[a] = (float)(n[a] + 1 - H[a]); }
+  }
   std::vector<FwdView> hv((size_t)n_views);
   for (int v = 0; v < n_views; ++v) make_fwd_view(make_frame(*g, angles, v), poses + 6 * v, &hv[v], nullptr);
   FwdView* dv = nullptr;
@@ -763,8 +901,11 @@ int64_t dfp_count_ray_steps(const dfp_geometry* g, int n_views, const float* ang
   if (cudaMalloc(&dn, sizeof(unsigned long long)) != cudaSuccess) { cudaFree(dv); return -1; }
   cudaMemcpy(dv, hv.data(), sizeof(FwdView) * n_views, cudaMemcpyHostToDevice);
   cudaMemset(dn, 0, sizeof(unsigned long long));
-  const dim3 grid((g->nu + kFwdTU - 1) / kFwdTU, (g->nv + kFwdTV - 1) / kFwdTV, n_views);
-  count_steps_kernel<<<grid, kFwdThreads>>>(G, dv, dn);
+  for (int v0 = 0; v0 < n_views; v0 += kMaxViewsPerLaunch) {
+    const int nv = n_views - v0 < kMaxViewsPerLaunch ? n_views - v0 : kMaxViewsPerLaunch;
+    const dim3 grid((g->nu + kFwdTU - 1) / kFwdTU, (g->nv + kFwdTV - 1) / kFwdTV, nv);
+    count_steps_kernel<<<grid, kFwdThreads>>>(G, dv + v0, dn);
+  }
   const cudaError_t e = cudaMemcpy(&n, dn, sizeof(n), cudaMemcpyDeviceToHost);
   cudaFree(dv);
   cudaFree(dn);
@@ -804,57 +945,5 @@ const char* dfp_status_string(int status) {
 }
 
 int dfp_version(void) { return 100; }
-
-// One resident wave of a micro-benchmark kernel, timed with CUDA events on the default stream (the kernels' own
-// clock64() counts are kept for inspection only: on B200 that counter does not tick at the SM clock).
-int dfp_microbench(int kind, double* per_second) {
-  if (!per_second) return DFP_ERR_NULL;
-  if (kind < DFP_MB_LDS || kind > DFP_MB_FFMA2) return DFP_ERR_DIMS;
-  int dev = 0, n_sm = 0, R = 0;
-  DFP_CUDA(cudaGetDevice(&dev), "cudaGetDevice");
-  DFP_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute");
-  const void* fn = kind == DFP_MB_LDS    ? (const void*)mb_lds_kernel
-                   : kind == DFP_MB_FADD ? (const void*)mb_alu_kernel<0>
-                   : kind == DFP_MB_FFMA ? (const void*)mb_alu_kernel<1>
-                                         : (const void*)mb_alu_kernel<2>;
-  DFP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&R, fn, kMbThreads, 0), "occupancy");
-  if (R < 1 || n_sm < 1) return DFP_ERR_CUDA;
-  const int grid = n_sm * R;
-  float* sink = nullptr;
-  long long* cyc = nullptr;
-  cudaEvent_t e0 = nullptr, e1 = nullptr;
-  DFP_CUDA(cudaMalloc(&sink, sizeof(float) * (size_t)grid * kMbThreads), "cudaMalloc");
-  if (cudaMalloc(&cyc, sizeof(long long) * grid) != cudaSuccess || cudaEventCreate(&e0) != cudaSuccess ||
-      cudaEventCreate(&e1) != cudaSuccess) {
-    const cudaError_t e = cudaGetLastError();
-    cudaFree(sink); cudaFree(cyc);
-    if (e0) cudaEventDestroy(e0);
-    return cuda_fail(e, "microbench set-up");
-  }
-  double work = 0;        // whole grid: warp-instructions (LDS) or fp32 results (ALU)
-  for (int pass = 0; pass < 2; ++pass) {                 // warm-up, then the measured wave
-    const int iters = pass ? 8000 : 50;
-    if (pass) cudaEventRecord(e0, 0);
-    if (kind == DFP_MB_LDS) {
-      mb_lds_kernel<<<grid, kMbThreads>>>(iters, 96, sink, cyc);
-      work = (double)grid * iters * kMbLdsPerIter * (kMbThreads / 32);
-    } else {
-      if (kind == DFP_MB_FADD) mb_alu_kernel<0><<<grid, kMbThreads>>>(iters, 1.0001f, 1e-3f, sink, cyc);
-      else if (kind == DFP_MB_FFMA) mb_alu_kernel<1><<<grid, kMbThreads>>>(iters, 1.0001f, 1e-3f, sink, cyc);
-      else mb_alu_kernel<2><<<grid, kMbThreads>>>(iters, 1.0001f, 1e-3f, sink, cyc);
-      work = (double)grid * iters * 4 * kMbChains * kMbThreads * (kind == DFP_MB_FFMA2 ? 2 : 1);
-    }
-    if (pass) cudaEventRecord(e1, 0);
-  }
-  float ms = 0.f;
-  cudaError_t e = cudaEventSynchronize(e1);
-  if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
-  cudaFree(sink); cudaFree(cyc);
-  cudaEventDestroy(e0); cudaEventDestroy(e1);
-  if (e != cudaSuccess) return cuda_fail(e, "microbench");
-  if (!(ms > 0.f)) return DFP_ERR_CUDA;
-  *per_second = work / ((double)ms * 1e-3);
-  return DFP_OK;
-}
 
 }  // extern "C"

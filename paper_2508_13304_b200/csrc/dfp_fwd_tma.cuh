@@ -1,9 +1,8 @@
 // dfp_fwd_tma.cuh - a3 / a4 with the volume staged in shared memory by TMA (sm_100a).
 //
-// Same arithmetic, sample for sample, as fwd_project_kernel / fwd_grad_kernel (dfp_kernels.cuh) - the forward
-// results are bit-identical, the gradient's differ only by the order in which a ray's even and odd samples are
-// added - but the 8 (forward) or 32 (gradient) voxel reads of a sample are LDS from a box of the volume that the
-// block's pixel tile (16x16 forward, 16x8 gradient) crosses during one CHUNK of consecutive samples:
+// Same arithmetic per sample as fwd_project_kernel / fwd_grad_kernel (dfp_kernels.cuh), but the 8 (forward) or 32
+// (gradient) voxel reads of a sample are LDS from a box of the volume that the block's pixel tile crosses during one
+// CHUNK of consecutive samples:
 //
 //   * the block's rays share one kappa axis (sample k = kref + kappa, tau_k = (k + 1/2) D, fixed in the world:
 //     DESIGN.md O6), so a chunk [kappa0, kappa0 + Kc) is a slab of the frustum; its bounding box in voxel
@@ -15,7 +14,11 @@
 //   * one or two stages (BoxShape), mbarrier (complete_tx) as the "full" signal, __syncthreads as the "empty" one;
 //   * the box origin is rounded down to a multiple of 4 floats along x (TMA: 16-byte inner alignment);
 //   * Kc is chosen per block so that the box always fits (oblique tiles get shorter chunks);
-//   * gradient: two lanes per ray (even / odd samples) and packed fp32x2 arithmetic (FFMA2 / FADD2).
+//   * positions are BOX-LOCAL: every thread keeps its ray in fp64 (Ray) and, once per chunk, re-bases it onto the
+//     box origin, so the fp32 position of a sample is a number in [0, 28) with ~1e-6 voxel of error whatever the
+//     size of the volume; the shared-memory word index is X + BX*Y + BX*BY*Z of the magic-rounded local position;
+//   * gradient: several lanes per ray (interleaved samples) and packed fp32x2 arithmetic (FFMA2 / FADD2);
+//   * exact-interpolant mode: a sample within fp32 rounding of a cell face takes cell and fractions from fp64.
 // PAPER.md Eq.18 :172-177 (forward), Eq.7-8 :101-113, Eq.19-20 :179-191 (gradient), :207 (on the fly, weights once).
 #pragma once
 #include <cuda.h>
@@ -25,17 +28,18 @@
 
 namespace dfp {
 
-// Staging boxes (floats).  The x extent times 4 bytes must be a multiple of 16 (TMA inner box).  Pitches of
-// 20 / 28 words spread the rows of a warp's 8x4-pixel footprint over distinct banks (measured 1.4 LDS
-// wavefronts per warp load on C2).
-// The host picks, per call, the smallest shape every view's tiles fit with chunks of >= kMinChunk samples:
+// Staging boxes (floats).  The x extent times 4 bytes must be a multiple of 16 (TMA inner box).  Bank of a voxel =
+// (x + X*y + X*Y*z) mod 32: only x reaches the two low bank bits (rows are 16-byte aligned), so a warp-wide load is
+// conflict-free only if the warp's voxels spread along x as well as across (y, z) - DESIGN.md "Kernels", and the
+// simulation / measurements quoted there.
+// The host picks, per call, the first shape of the op's list that every view's tiles fit with chunks of >= kMinChunk
+// samples:
 //   shape 0  20 x 20 x 16, two stages : forward, clinical magnification and small pose angles (C2, C4)
 //   shape 1  28 x 20 x 20, two stages : forward, wider tiles / larger tilts (C5)
 //   shape 2  28 x 28 x 20, one stage  : forward fallback before the gather path; gradient fallback
 //   shape 3  28 x 28 x 16, one stage  : gradient, 16 x 8-pixel tiles (the stencil needs 2 more cells per axis and a
 //            chunk lasts 4x longer than the forward's, so one stage and four blocks per SM hide the TMA latency;
 //            long enough along x and y that views at 45 degrees in the xy plane still get ~10-sample chunks).
-// Measured on B200 (Gray-steps/s, forward): C2 625 / 591 / 557, C4 607 / 560 / 548 for shapes 0 / 1 / 2.
 template <int SHAPE> struct BoxShape;
 template <> struct BoxShape<0> { static constexpr int X = 20, Y = 20, Z = 16, STAGES = 2; };
 template <> struct BoxShape<1> { static constexpr int X = 28, Y = 20, Z = 20, STAGES = 2; };
@@ -45,40 +49,40 @@ constexpr int kNumShapes = 4;
 template <int SHAPE> constexpr int tma_smem_bytes() {
   return BoxShape<SHAPE>::X * BoxShape<SHAPE>::Y * BoxShape<SHAPE>::Z * 4 * BoxShape<SHAPE>::STAGES;
 }
-// Lane mapping.  Each ray is marched by kTmaSlots = 2 lanes (even / odd samples); a warp = 8(u) x 2(v) pixels x 2
-// consecutive samples.  The 32 lanes of a warp-wide LDS then touch voxels spread over two depth steps as well as
-// the 8 x 2 patch: with row pitches 20 / 28 (= -12 / -4 mod 32) and slab pitch = 16 mod 32 these fall on distinct
-// banks almost always (simulated 1.01 wavefronts per load on C2, 1.2 on C4; the 8 x 4-pixel single-sample warp of
-// the gather kernels gives 1.39 / 1.69, measured 1.39 on C2).  Block = 16 x 16 pixels x 2 slots = 512 threads.
-// The forward kernel is issue-bound, not LDS-bound, and keeps one lane per ray (256 threads, 8 x 4-pixel warps):
-// with two slots it ran 7.0 -> 9.0 ms on C2 (twice the per-ray set-up and loop overhead).
 __device__ __forceinline__ float2 sub2(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
 // lerp on two lanes of data at once: v0 + a (v1 - v0), rounded exactly like lerp()
 __device__ __forceinline__ float2 lerp2(float2 a, float2 v0, float2 v1) { return __ffma2_rn(a, sub2(v1, v0), v0); }
 
-// Pixel tile of a block: 16 x 16 (forward), 16 x 8 (gradient: 256 threads = 128 rays x 2 slots, four blocks per SM
-// instead of two 512-thread ones hide the single-stage TMA latency better).
-// GRAD: 0 forward projection, 1 gradient with central differences of f~ (the paper's, O3), 2 gradient
-// with the exact derivative of the trilinear interpolant (DFP_FLAG_GRAD_INTERP: the same 8 voxels as the forward),
-// 3 FUSED projection + central-difference gradient moments in one traversal (dfp_forward_fused_moments).
+// Lane mapping.  A ray is marched by SLOTS lanes (lane `slot` takes the samples kappa = slot mod SLOTS); a warp covers
+// PU x PV pixels x SLOTS consecutive samples, so that the 32 lanes of a warp-wide LDS touch voxels spread over SLOTS
+// depth steps as well as the pixel patch.  Block = TU x TV pixels x SLOTS.
+// GRAD: 0 forward projection (one lane per ray, 8 x 4-pixel warps, 16 x 16-pixel tile: the kernel is issue-bound and
+// a second lane per ray doubles the per-ray set-up), 1 gradient with central differences of f~ (the paper's,
+// DESIGN.md O3), 2 gradient with the exact derivative of the trilinear interpolant (DFP_FLAG_GRAD_INTERP: the same 8
+// voxels as the forward), 3 FUSED projection + central-difference gradient moments in one traversal
+// (dfp_forward_fused_moments).  Gradient kernels: two lanes per ray, 8 x 2-pixel warps, 16 x 8-pixel tile.
 template <int GRAD> struct TmaLanes {
   static constexpr int SLOTS = GRAD ? 2 : 1, TU = kFwdTU, TV = GRAD ? 8 : kFwdTV, THREADS = TU * TV * SLOTS;
+  static constexpr int PU = 8, PV = 32 / (PU * SLOTS);
 };
-template <int SLOTS>
-__device__ __forceinline__ void tma_pixel(int& iu, int& iv, int& slot) {
-  if (SLOTS == 1) {
-    slot = 0;
-    fwd_pixel(iu, iv);
-    return;
-  }
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;          // warps: 2 across u, TV / 2 down v
-  slot = lane >> 4;
-  iu = blockIdx.x * kFwdTU + (warp & 1) * 8 + (lane & 7);
-  iv = blockIdx.y * TmaLanes<true>::TV + (warp >> 1) * 2 + ((lane >> 3) & 1);
+template <int GRAD>
+__device__ __forceinline__ void tma_pixel(int bx, int by, int& iu, int& iv, int& slot) {
+  using T = TmaLanes<GRAD>;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  constexpr int WU = T::TU / T::PU;                     // warps across u
+  const int pix = lane % (T::PU * T::PV);
+  slot = lane / (T::PU * T::PV);
+  iu = bx * T::TU + (warp % WU) * T::PU + (pix % T::PU);
+  iv = by * T::TV + (warp / WU) * T::PV + (pix / T::PU);
 }
 constexpr int kMaxStages = 2;
 constexpr float kBoxMargin = 0.05f;                    // voxels: sagitta of the tile + fp32 rounding
 constexpr int kBoxAlignLoss = 3;                       // x cells lost to the 16-byte alignment of the box origin
+// Blocks are ordered so that the views of a GROUP of kViewGroup consecutive views run tile by tile, view fastest:
+// the blocks resident at one time then cover a few dozen neighbouring tiles of a few neighbouring views, whose frusta
+// overlap in the volume - a 512^3 volume (4x the L2) is then pulled from HBM about once per group instead of once
+// per view.
+constexpr int kViewGroup = 8;
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 
@@ -109,13 +113,13 @@ __device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap* map
 }
 
 struct TmaBlock {              // block-wide state in shared memory
-  float pm[4][3], dp[4][3];    // the tile's corner rays (centred-index coordinates, as in struct Ray)
+  float pm[4][3], dp[4][3];    // the tile's corner rays (centred-index coordinates, as in struct Ray, rounded to fp32)
   int kA, kB;                  // union of the live rays' kappa ranges [kA, kB)
   int Kc;                      // samples per chunk (0: nothing to do, -1: the box cannot hold the tile)
-  unsigned c0[kMaxStages];     // per-stage index constant: word index = Tx + X*Ty + X*Y*Tz + c0
+  int org[kMaxStages][3];      // per stage: centred index of the box's first cell (the origin of the local positions)
 };
 
-// One chunk's box: origin (voxel indices, for the TMA) and the index constant of the stage it lands in.
+// One chunk's box: origin (voxel indices, for the TMA) of the stage it lands in.
 template <int GRAD, int SHAPE>
 __device__ __forceinline__ void issue_chunk(const VolLayout& L, TmaBlock& B, const CUtensorMap* map, int chunk,
                                             unsigned tiles_addr, unsigned bar_addr) {
@@ -136,21 +140,20 @@ __device__ __forceinline__ void issue_chunk(const VolLayout& L, TmaBlock& B, con
   // the TMA unit wants the innermost coordinate on a 16-byte boundary (measured on B200: an x origin that is
   // not a multiple of 4 floats raises an illegal-instruction fault): round the x origin down, kBoxAlignLoss
   oc[0] = (((oc[0] + L.hx) >> 2) << 2) - L.hx;
-  const unsigned mb = (unsigned)kMagicBits;
-  B.c0[s] = (unsigned)(s * kWords) - ((unsigned)oc[0] + mb) - (unsigned)S::X * ((unsigned)oc[1] + mb) -
-            (unsigned)(S::X * S::Y) * ((unsigned)oc[2] + mb);
+  B.org[s][0] = oc[0]; B.org[s][1] = oc[1]; B.org[s][2] = oc[2];
   const unsigned bar = bar_addr + 8u * s;
   mbar_expect_tx(bar, kWords * 4);
   tma_load_3d(tiles_addr + (unsigned)(s * kWords * 4), map, oc[0] + L.hx, oc[1] + L.hy, oc[2] + L.hz, bar);
 }
 
-// The chunk loop of one block for one box shape.  acc = {sum} (forward) or {gx,gy,gz,hx,hy,hz} (gradient).
+// The chunk loop of one block for one box shape.  acc = {sum} (forward) or {gx,gy,gz,hx,hy,hz[,sum]} (gradient).
 template <int GRAD, int SHAPE>
 __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* map, const Ray& r, int slot,
                                           TmaBlock& B, const float* tiles, unsigned tiles_addr, unsigned bar_addr,
                                           float* acc) {
   using S = BoxShape<SHAPE>;
-  constexpr int BX = S::X, BXY = S::X * S::Y;
+  constexpr int BX = S::X, BXY = S::X * S::Y, kWords = S::X * S::Y * S::Z;
+  constexpr int SLOTS = TmaLanes<GRAD>::SLOTS;
   if (threadIdx.x == 0) {
     int Kc = 0;
     if (B.kA < B.kB) {
@@ -187,35 +190,55 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
   const int Kc = B.Kc, kA = B.kA, kB = B.kB;
   const int n_chunks = Kc > 0 ? (kB - kA + Kc - 1) / Kc : 0;
   const int kend = r.k0 + r.n;
+  const float dpx = (float)r.dp[0], dpy = (float)r.dp[1], dpz = (float)r.dp[2];
+  const float2 dpxy = make_float2(dpx, dpy);
 
   float sum = 0.f;
   float gx = 0.f, gy = 0.f, gz = 0.f, hx = 0.f, hy = 0.f, hz = 0.f;
   for (int chunk = 0; chunk < n_chunks; ++chunk) {
     const int s = chunk % S::STAGES;
     mbar_wait(bar_addr + 8u * s, (unsigned)(chunk / S::STAGES) & 1u);
-    const unsigned c0 = B.c0[s];
     const int c_lo = kA + chunk * Kc;
     const int ka = max(c_lo, r.k0), kb = min(min(c_lo + Kc, kB), kend);
-    // this lane takes the samples of its ray whose kappa has the lane's parity (the other slot takes the rest)
-    constexpr int SLOTS = TmaLanes<GRAD>::SLOTS;
-    const int kfirst = SLOTS == 1 ? ka : ka + ((ka ^ slot) & 1);
-    float kf = (float)kfirst;
+    // this lane takes the samples of its ray whose kappa is congruent to its slot (the other slots take the rest)
+    const int kfirst = SLOTS == 1 ? ka : ka + ((slot - ka) & (SLOTS - 1));
+    // re-base the ray onto the box origin (fp64, once per chunk): local position of this lane's first sample
+    const int o0 = B.org[s][0], o1 = B.org[s][1], o2 = B.org[s][2];
+    const double kd = (double)kfirst;
+    const float2 bxy = make_float2((float)(fma(kd, r.dp[0], r.pm[0]) - (double)o0),
+                                   (float)(fma(kd, r.dp[1], r.pm[1]) - (double)o1));
+    const float bz = (float)(fma(kd, r.dp[2], r.pm[2]) - (double)o2);
+    // word index of local cell (X, Y, Z) in stage s from the magic-rounded floats' bits
+    const unsigned c0 = (unsigned)(s * kWords) - (unsigned)kMagicBits * (unsigned)(1 + BX + BXY);
+    float kf = (float)kfirst, jf = 0.f;
     for (int k = kfirst; k < kb; k += SLOTS) {
-      // position, floor and fractions: x and y as one fp32x2 lane pair (same roundings as the scalar code)
-      const float2 q2 = __ffma2_rn(make_float2(kf, kf), make_float2(r.dpx, r.dpy), make_float2(r.pmx, r.pmy));
-      const float qz = fmaf(kf, r.dpz, r.pmz);
+      // position, floor and fractions: x and y as one fp32x2 lane pair
+      const float2 q2 = __ffma2_rn(make_float2(jf, jf), dpxy, bxy);
+      const float qz = fmaf(jf, dpz, bz);
       const float2 t2 = __fadd2_rn(q2, make_float2(kMagic, kMagic));
       const float tz = qz + kMagic;
       const float2 a2 = __fadd2_rn(sub2(q2, __fadd2_rn(t2, make_float2(-kMagic, -kMagic))), make_float2(0.5f, 0.5f));
-      const float ax = a2.x, ay = a2.y, az = (qz - (tz - kMagic)) + 0.5f;
-      const unsigned idx = (unsigned)__float_as_int(t2.x) + (unsigned)BX * (unsigned)__float_as_int(t2.y) +
-                           (unsigned)BXY * (unsigned)__float_as_int(tz) + c0;
+      float ax = a2.x, ay = a2.y, az = (qz - (tz - kMagic)) + 0.5f;
+      unsigned idx = (unsigned)__float_as_int(t2.x) + (unsigned)BX * (unsigned)__float_as_int(t2.y) +
+                     (unsigned)BXY * (unsigned)__float_as_int(tz) + c0;
+      if (GRAD == 2) {
+        // the derivative of the interpolant jumps at cell faces: a sample within fp32 rounding of one takes its
+        // cell (and fractions) from the fp64 position, as the oracle does
+        const float mn = fminf(fminf(fminf(ax, 1.f - ax), fminf(ay, 1.f - ay)), fminf(az, 1.f - az));
+        if (mn < kFaceEps) {
+          int cell[3];
+          float fr[3];
+          exact_cell(r, k, cell, fr);
+          idx = (unsigned)(s * kWords + (cell[0] - o0) + BX * (cell[1] - o1) + BXY * (cell[2] - o2));
+          ax = fr[0]; ay = fr[1]; az = fr[2];
+        }
+      }
       const float* c = tiles + idx;
 #ifdef DFP_CHECK_BOUNDS   // debug build: every LDS of the sample must fall inside the stage's box (else NaN out)
       {
-        const int local = (int)(idx - (unsigned)(s * BXY * S::Z)), halo = GRAD ? 1 : 0;
+        const int local = (int)(idx - (unsigned)(s * kWords)), halo = (GRAD == 1 || GRAD == 3) ? 1 : 0;
         const int lo = local - halo * (1 + BX + BXY), hi = local + (1 + halo) * (1 + BX + BXY);
-        if (lo < 0 || hi >= BXY * S::Z) sum = gx = __int_as_float(0x7fc00000);
+        if (lo < 0 || hi >= kWords) sum = gx = __int_as_float(0x7fc00000);
       }
 #endif
       if (!GRAD) {
@@ -291,6 +314,7 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
         hx = fmaf(kf, ddx, hx); hy = fmaf(kf, ddy, hy); hz = fmaf(kf, ddz, hz);
       }
       kf += (float)SLOTS;
+      jf += (float)SLOTS;
     }
     __syncthreads();                                   // every thread is done with stage s ("empty")
     if (threadIdx.x == 0 && chunk + S::STAGES < n_chunks)
@@ -304,21 +328,37 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
   }
 }
 
+// Grid: one block per (view, pixel tile), 1-D, ordered group of views -> tile -> view within the group (kViewGroup).
+struct FwdGrid {
+  int n_views, gx, gy;         // views of this launch; tiles per view along u and v
+};
+__device__ __forceinline__ void fwd_block(const FwdGrid& Q, int& view, int& bx, int& by) {
+  const unsigned nb = (unsigned)Q.gx * (unsigned)Q.gy, per = (unsigned)kViewGroup * nb;
+  const unsigned b = blockIdx.x, grp = b / per, r = b - grp * per;
+  const unsigned gsz = min((unsigned)kViewGroup, (unsigned)Q.n_views - grp * kViewGroup);
+  const unsigned tile = r / gsz, vg = r - tile * gsz;
+  view = (int)(grp * kViewGroup + vg);
+  by = (int)(tile / (unsigned)Q.gx);
+  bx = (int)(tile - (unsigned)by * (unsigned)Q.gx);
+}
+
 template <int GRAD, int SHAPE>
-__global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, 4) fwd_tma_kernel(FwdGeom G, const FwdView* __restrict__ views,
+__global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, 4) fwd_tma_kernel(FwdGeom G, FwdGrid Q,
+                                                              const FwdView* __restrict__ views,
                                                               const __grid_constant__ CUtensorMap vol_map,
                                                               const float* __restrict__ upstream,
                                                               float* __restrict__ out,
                                                               float* __restrict__ proj_out) {
   constexpr int NSET = GRAD == 3 ? 3 : 1;              // weight sets of the per-view reduction (fused: 1, l, b)
+  constexpr int SLOTS = TmaLanes<GRAD>::SLOTS;
   extern __shared__ __align__(128) float tiles[];      // STAGES boxes
   __shared__ __align__(8) unsigned long long full_bar[kMaxStages];
   __shared__ TmaBlock B;
   __shared__ float red[TmaLanes<GRAD>::THREADS / 32][6 * NSET];
 
-  int iu, iv, slot;
-  tma_pixel<TmaLanes<GRAD>::SLOTS>(iu, iv, slot);
-  const int view = blockIdx.z;
+  int view, bx, by, iu, iv, slot;
+  fwd_block(Q, view, bx, by);
+  tma_pixel<GRAD>(bx, by, iu, iv, slot);
   const bool live = iu < G.nu && iv < G.nv;
   const unsigned tiles_addr = smem_u32(tiles), bar_addr = smem_u32(full_bar);
 
@@ -344,11 +384,11 @@ __global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, 4) fwd_tma_kernel(Fwd
   }
   {  // corner rays of the tile: pixels (0,0), (TU-1,0), (0,TV-1), (TU-1,TV-1) of the block
     constexpr int TU = TmaLanes<GRAD>::TU, TV = TmaLanes<GRAD>::TV;
-    const int cu = iu - blockIdx.x * TU, cv = iv - blockIdx.y * TV;
+    const int cu = iu - bx * TU, cv = iv - by * TV;
     if (slot == 0 && (cu == 0 || cu == TU - 1) && (cv == 0 || cv == TV - 1)) {
       const int c = (cu ? 1 : 0) + (cv ? 2 : 0);
-      B.pm[c][0] = r.pmx; B.pm[c][1] = r.pmy; B.pm[c][2] = r.pmz;
-      B.dp[c][0] = r.dpx; B.dp[c][1] = r.dpy; B.dp[c][2] = r.dpz;
+#pragma unroll
+      for (int a = 0; a < 3; ++a) { B.pm[c][a] = (float)r.pm[a]; B.dp[c][a] = (float)r.dp[a]; }
     }
   }
   __syncthreads();
@@ -367,10 +407,13 @@ __global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, 4) fwd_tma_kernel(Fwd
   __syncthreads();
   float acc[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   tma_march<GRAD, SHAPE>(G, &vol_map, r, slot, B, tiles, tiles_addr, bar_addr, acc);
-  // the two slots of a ray: even-kappa partial sums + odd-kappa partial sums
-  if (TmaLanes<GRAD>::SLOTS == 2) {
+  // the slots of a ray: partial sums over the samples each lane took (slot = lane / (PU * PV): the high lane bits)
+  if (SLOTS > 1) {
 #pragma unroll
-    for (int q = 0; q < (GRAD == 3 ? 7 : GRAD ? 6 : 1); ++q) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], 16);
+    for (int q = 0; q < (GRAD == 3 ? 7 : GRAD ? 6 : 1); ++q) {
+#pragma unroll
+      for (int o = 16; o >= 32 / SLOTS; o >>= 1) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], o);
+    }
   }
 
   const float bad = B.Kc < 0 ? __int_as_float(0x7fc00000) : 0.f;   // NaN: the box cannot hold the tile (host bound wrong)
@@ -422,11 +465,11 @@ __global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, 4) fwd_tma_kernel(Fwd
     float t = 0.f;
 #pragma unroll
     for (int wI = 0; wI < TmaLanes<GRAD>::THREADS / 32; ++wI) t += red[wI][threadIdx.x];
-    const size_t blk = (size_t)blockIdx.y * gridDim.x + blockIdx.x;
-    const size_t nblk = (size_t)gridDim.x * gridDim.y;
+    const size_t blk = (size_t)by * Q.gx + bx;
+    const size_t nblk = (size_t)Q.gx * Q.gy;
     // partials[set][view][block][6]: each weight set is a plain gradient partial array for fwd_contract_kernel
     const int set = threadIdx.x / 6, k = threadIdx.x % 6;
-    out[(((size_t)set * gridDim.z + view) * nblk + blk) * 6 + k] = t;
+    out[(((size_t)set * Q.n_views + view) * nblk + blk) * 6 + k] = t;
   }
   }  // GRAD
 }

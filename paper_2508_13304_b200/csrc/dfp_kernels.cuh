@@ -136,9 +136,13 @@ __global__ void __launch_bounds__(256) pack_proj_kernel(int nu, int nv, int pu, 
 // a2 (Eq.2a :67-69: the delta selects the source->pixel line).  Runs once per ray in fp64 so that the
 // fp32 march starts from correctly rounded constants: sample kappa sits at centred-index position
 // pm + kappa*dp (+0.5, folded out for the magic floor), kappa = k - kref, tau_k = (k + 1/2) D.
+// The march keeps the ray in DOUBLE (pm, dp: 12 registers, touched once per chunk / group of samples) and re-bases it
+// every few samples onto a nearby integer origin, so that the fp32 position of a sample is a small number (|q| < 32)
+// with an error of ~1e-6 voxel - instead of 3e-5 for a 512^3 volume if the fp32 position ran over the whole grid.
+// The interpolation weights inherit that error; it is what the pose-gradient sums are most sensitive to.
 struct Ray {
-  float pmx, pmy, pmz;     // centred-index position of sample kappa = 0, minus 0.5
-  float dpx, dpy, dpz;     // centred-index step per sample
+  double pm[3];            // centred-index position of sample kappa = 0, minus 0.5
+  double dp[3];            // centred-index step per sample
   int k0, n;               // first kappa and sample count (n <= 0: the ray misses the clip box)
 };
 
@@ -178,18 +182,47 @@ __device__ __forceinline__ Ray setup_ray(const FwdGeom& G, const FwdView& V, int
   r.n = hit ? (k1 - k0 + 1) : 0;
   r.k0 = k0 - G.kref;
   const double tref = (G.kref + 0.5) * D;
-  r.pmx = (float)(ps[0] + tref * pe[0] - 0.5);
-  r.pmy = (float)(ps[1] + tref * pe[1] - 0.5);
-  r.pmz = (float)(ps[2] + tref * pe[2] - 0.5);
-  r.dpx = (float)(D * pe[0]);
-  r.dpy = (float)(D * pe[1]);
-  r.dpz = (float)(D * pe[2]);
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    r.pm[a] = ps[a] + tref * pe[a] - 0.5;
+    r.dp[a] = D * pe[a];
+  }
   if (e_mm) {
 #pragma unroll
     for (int a = 0; a < 3; ++a) { e_mm[a] = e[a]; ref_mm[a] = V.src[a] + tref * e[a]; }
   }
   return r;
 }
+
+// Re-based march of the gather kernels: groups of kRebase samples share an integer origin (the rounded position of the
+// group's first sample); inside a group the position is fma(j, dp, b) with |b| <= 1/2, j < kRebase.
+constexpr int kRebase = 16;
+struct RayGroup {
+  float bx, by, bz;        // position of the group's first sample minus the origin
+  int ox, oy, oz;          // origin (centred index)
+};
+__device__ __forceinline__ RayGroup ray_group(const Ray& r, int kappa) {
+  RayGroup g;
+  const double k = (double)kappa;
+  const double px = fma(k, r.dp[0], r.pm[0]), py = fma(k, r.dp[1], r.pm[1]), pz = fma(k, r.dp[2], r.pm[2]);
+  const double rx = rint(px), ry = rint(py), rz = rint(pz);
+  g.ox = (int)rx; g.oy = (int)ry; g.oz = (int)rz;
+  g.bx = (float)(px - rx); g.by = (float)(py - ry); g.bz = (float)(pz - rz);
+  return g;
+}
+// Exact cell and fractions of one sample (fp64): the slow path of the exact-interpolant gradient mode, whose
+// integrand is discontinuous at cell faces - a sample within fp32 rounding of a face takes its cell from here.
+__device__ __forceinline__ void exact_cell(const Ray& r, int kappa, int* cell, float* frac) {
+  const double k = (double)kappa;
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    const double p = fma(k, r.dp[a], r.pm[a]) + 0.5;        // centred-index position
+    const double f = floor(p);
+    cell[a] = (int)f;
+    frac[a] = (float)(p - f);
+  }
+}
+constexpr float kFaceEps = 6e-6f;      // |fraction - {0,1}| below this: the fp32 cell decision is not trusted
 
 // pixel of this thread: warps are 8(u) x 4(v) patches, (kFwdTU/8) x (kFwdTV/4) warps per block
 __device__ __forceinline__ void fwd_pixel(int& iu, int& iv) {
@@ -201,9 +234,22 @@ __device__ __forceinline__ void fwd_pixel(int& iu, int& iv) {
 // ------------------------------------------------------------------------------------------------ a3 forward
 // l_i = D sum_k f~(r'_k)  (Eq.18 :172-177 with a^ij = D * trilinear weight; U1).
 // Cell index of the sample's base voxel from the magic-rounded coordinates (VolLayout): 3 LOP + 6 IMAD/LEA.
-__device__ __forceinline__ unsigned brick_index(const VolLayout& L, float tx, float ty, float tz) {
-  const unsigned X = (unsigned)__float_as_int(tx), Y = (unsigned)__float_as_int(ty), Z = (unsigned)__float_as_int(tz);
+__device__ __forceinline__ unsigned brick_index(const VolLayout& L, unsigned X, unsigned Y, unsigned Z) {
   return X + 3u * (X & ~1u) + 2u * Y + L.by * (Y & ~1u) + 4u * Z + L.bz * (Z & ~1u) + L.c0;
+}
+// position, magic-rounded cell bits (kMagicBits + centred cell index) and fractions of sample j of a group
+struct SamplePos {
+  unsigned X, Y, Z;
+  float ax, ay, az;
+};
+__device__ __forceinline__ SamplePos sample_pos(const RayGroup& g, float jf, float dpx, float dpy, float dpz) {
+  SamplePos s;
+  const float qx = fmaf(jf, dpx, g.bx), qy = fmaf(jf, dpy, g.by), qz = fmaf(jf, dpz, g.bz);
+  const float tx = qx + kMagic, ty = qy + kMagic, tz = qz + kMagic;
+  s.ax = (qx - (tx - kMagic)) + 0.5f; s.ay = (qy - (ty - kMagic)) + 0.5f; s.az = (qz - (tz - kMagic)) + 0.5f;
+  s.X = (unsigned)(__float_as_int(tx) + g.ox); s.Y = (unsigned)(__float_as_int(ty) + g.oy);
+  s.Z = (unsigned)(__float_as_int(tz) + g.oz);
+  return s;
 }
 
 __global__ void __launch_bounds__(kFwdThreads) fwd_project_kernel(FwdGeom G, const FwdView* __restrict__ views,
@@ -214,20 +260,23 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_project_kernel(FwdGeom G, con
   const int view = blockIdx.z;
   if (iu >= G.nu || iv >= G.nv) return;
   const Ray r = setup_ray(G, views[view], iu, iv, nullptr, nullptr);
+  const float dpx = (float)r.dp[0], dpy = (float)r.dp[1], dpz = (float)r.dp[2];
   const unsigned dz1 = 2u * G.L.bz + 4u;     // FZ(Z+1) - FZ(Z) for odd Z (4 for even Z)
   float sum = 0.f;
-  float kf = (float)r.k0;
-  for (int i = 0; i < r.n; ++i) {
-    const float qx = fmaf(kf, r.dpx, r.pmx), qy = fmaf(kf, r.dpy, r.pmy), qz = fmaf(kf, r.dpz, r.pmz);
-    const float tx = qx + kMagic, ty = qy + kMagic, tz = qz + kMagic;
-    const float ax = (qx - (tx - kMagic)) + 0.5f, ay = (qy - (ty - kMagic)) + 0.5f, az = (qz - (tz - kMagic)) + 0.5f;
-    const unsigned idx = brick_index(G.L, tx, ty, tz);
-    const unsigned up = (__float_as_int(tz) & 1) ? dz1 : 4u;
-    const float4 c0 = ldg4(pvol + idx), c1 = ldg4(pvol + (idx + up));
-    const float r00 = lerp(ax, c0.x, c0.y), r10 = lerp(ax, c0.z, c0.w);
-    const float r01 = lerp(ax, c1.x, c1.y), r11 = lerp(ax, c1.z, c1.w);
-    sum += lerp(az, lerp(ay, r00, r10), lerp(ay, r01, r11));
-    kf += 1.0f;
+  for (int g0 = 0; g0 < r.n; g0 += kRebase) {
+    const RayGroup grp = ray_group(r, r.k0 + g0);
+    const int m = min(kRebase, r.n - g0);
+    float jf = 0.f;
+    for (int j = 0; j < m; ++j) {
+      const SamplePos sp = sample_pos(grp, jf, dpx, dpy, dpz);
+      const unsigned idx = brick_index(G.L, sp.X, sp.Y, sp.Z);
+      const unsigned up = (sp.Z & 1u) ? dz1 : 4u;
+      const float4 c0 = ldg4(pvol + idx), c1 = ldg4(pvol + (idx + up));
+      const float r00 = lerp(sp.ax, c0.x, c0.y), r10 = lerp(sp.ax, c0.z, c0.w);
+      const float r01 = lerp(sp.ax, c1.x, c1.y), r11 = lerp(sp.ax, c1.z, c1.w);
+      sum += lerp(sp.az, lerp(sp.ay, r00, r10), lerp(sp.ay, r01, r11));
+      jf += 1.0f;
+    }
   }
   proj[((size_t)view * G.nv + iv) * G.nu + iu] = G.step * sum;
 }
@@ -282,19 +331,33 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_grad_kernel(FwdGeom G, const 
   if (live) {
     double e_mm[3], ref_mm[3];
     const Ray r = setup_ray(G, views[view], iu, iv, e_mm, ref_mm);
+    const float dpx = (float)r.dp[0], dpy = (float)r.dp[1], dpz = (float)r.dp[2];
     const unsigned by8 = 2u * G.L.by + 4u;          // 8*nbx:     FY(Y+2) - FY(Y)
     const unsigned bz8 = 2u * G.L.bz + 8u;          // 8*nbx*nby: FZ(Z+2) - FZ(Z)
     float gx = 0.f, gy = 0.f, gz = 0.f, hx = 0.f, hy = 0.f, hz = 0.f;
-    float kf = (float)r.k0;
-    for (int i = 0; i < r.n; ++i) {
-      const float qx = fmaf(kf, r.dpx, r.pmx), qy = fmaf(kf, r.dpy, r.pmy), qz = fmaf(kf, r.dpz, r.pmz);
-      const float tx = qx + kMagic, ty = qy + kMagic, tz = qz + kMagic;
-      const float ax = (qx - (tx - kMagic)) + 0.5f, ay = (qy - (ty - kMagic)) + 0.5f,
-                  az = (qz - (tz - kMagic)) + 0.5f;
-      const unsigned idx = brick_index(G.L, tx, ty, tz);
+    for (int g0 = 0; g0 < r.n; g0 += kRebase) {
+    const RayGroup grp = ray_group(r, r.k0 + g0);
+    const int m = min(kRebase, r.n - g0);
+    float jf = 0.f, kf = (float)(r.k0 + g0);
+    for (int j = 0; j < m; ++j) {
+      SamplePos sp = sample_pos(grp, jf, dpx, dpy, dpz);
+      if (MODE == 1) {
+        // the derivative of the interpolant jumps at cell faces: a sample within fp32 rounding of one takes its cell
+        // (and fractions) from the fp64 position, as the oracle does
+        const float mn = fminf(fminf(fminf(sp.ax, 1.f - sp.ax), fminf(sp.ay, 1.f - sp.ay)), fminf(sp.az, 1.f - sp.az));
+        if (mn < kFaceEps) {
+          int cell[3];
+          float fr[3];
+          exact_cell(r, r.k0 + g0 + j, cell, fr);
+          sp.X = (unsigned)(kMagicBits + cell[0]); sp.Y = (unsigned)(kMagicBits + cell[1]); sp.Z = (unsigned)(kMagicBits + cell[2]);
+          sp.ax = fr[0]; sp.ay = fr[1]; sp.az = fr[2];
+        }
+      }
+      const float ax = sp.ax, ay = sp.ay, az = sp.az;
+      const unsigned idx = brick_index(G.L, sp.X, sp.Y, sp.Z);
       float ddx, ddy, ddz;
       if (MODE == 1) {
-        const unsigned up = (__float_as_int(tz) & 1) ? bz8 - 4u : 4u;                     // FZ(Z+1) - FZ(Z)
+        const unsigned up = (sp.Z & 1u) ? bz8 - 4u : 4u;                                  // FZ(Z+1) - FZ(Z)
         const float4 c0 = ldg4(pvol + idx), c1 = ldg4(pvol + (idx + up));                // slices z, z+1: rows y, y+1
         const float d00 = c0.y - c0.x, d10 = c0.w - c0.z, d01 = c1.y - c1.x, d11 = c1.w - c1.z;
         const float r00 = fmaf(ax, d00, c0.x), r10 = fmaf(ax, d10, c0.z);
@@ -304,8 +367,7 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_grad_kernel(FwdGeom G, const 
         ddz = lerp(ay, r01, r11) - lerp(ay, r00, r10);
       } else {
       // neighbour cells: +-1 along an axis stays inside the brick or hops to the next one, by parity
-      const unsigned ox = (unsigned)__float_as_int(tx) & 1u, oy = (unsigned)__float_as_int(ty) & 1u,
-                     oz = (unsigned)__float_as_int(tz) & 1u;
+      const unsigned ox = sp.X & 1u, oy = sp.Y & 1u, oz = sp.Z & 1u;
       const unsigned dxp = 1u + 6u * ox, dxm = dxp - 8u;
       const unsigned dyp = 2u + (by8 - 4u) * oy, dym = dyp - by8;
       const unsigned dzp = 4u + (bz8 - 8u) * oz, dzm = dzp - bz8;
@@ -339,6 +401,8 @@ __global__ void __launch_bounds__(kFwdThreads) fwd_grad_kernel(FwdGeom G, const 
       gx += ddx; gy += ddy; gz += ddz;
       hx = fmaf(kf, ddx, hx); hy = fmaf(kf, ddy, hy); hz = fmaf(kf, ddz, hz);
       kf += 1.0f;
+      jf += 1.0f;
+    }
     }
     // per-ray epilogue (once per ray): scale to per-mm gradients, lever arm about the reference sample
     const float w = upstream ? __ldg(upstream + ((size_t)view * G.nv + iv) * G.nu + iu) : 1.f;   // null: unit weights

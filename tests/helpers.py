@@ -60,3 +60,29 @@ def grad_err_u9(g, ref):
 
 def t64(a):
     return torch.as_tensor(np.asarray(a), dtype=torch.float64)
+
+
+def check_values(got, ref, tol_l2=1e-5, tol_abs=5e-5, zero_border=True):
+    """Values (projections, back-projections) against the oracle: the stated metric (relative L2 <= 1e-5), backed by a
+    per-element bound - max |got - ref| <= 5e-5 max|ref|, five times the L2 tolerance (an fp32
+    result carries ~1e-6 of its own magnitude, so only a wrong element - a tile edge, a missed sample - can exceed it) -
+    and by the zero pattern: where the oracle is exactly zero (rays / voxels that miss) the CUDA result is exactly zero
+    too (`zero_border`: inputs whose outermost voxels / pixels are zero, all workloads' phantoms) or below 1e-6 of the
+    largest value (white-noise inputs: a sample within fp32 rounding of the support's edge may pick up a last voxel)."""
+    got = np.asarray(got, dtype=np.float64)
+    ref = np.asarray(ref, dtype=np.float64)
+    assert got.shape == ref.shape and np.all(np.isfinite(got))
+    scale = np.abs(ref).max()
+    if scale == 0.0:
+        assert not got.any(), "oracle is all zero, the CUDA result is not"
+        return 0.0
+    e = rel_l2(got, ref)
+    assert e <= tol_l2, e
+    assert np.abs(got - ref).max() <= tol_abs * scale, (np.abs(got - ref).max() / scale)
+    z = ref == 0
+    if z.any():
+        if zero_border:
+            assert not got[z].any(), "non-zero where the oracle is exactly zero"
+        else:
+            assert np.abs(got[z]).max() <= 1e-6 * scale
+    return e

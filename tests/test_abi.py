@@ -18,15 +18,29 @@ def dfp():
     return m
 
 
-def test_every_declared_symbol_is_exported(dfp):
-    hdr = open(os.path.join(ROOT, "include", "dfp.h")).read()
+def _declared(header):
+    hdr = open(os.path.join(ROOT, "include", header)).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    names = set(re.findall(r"\b(dfp_[a-z_]+)\s*\(", hdr))
+    return set(re.findall(r"\b(dfp_[a-z_]+)\s*\(", hdr))
+
+
+def test_every_declared_symbol_is_exported(dfp):
+    """include/dfp.h -> libdfp.so (the product); include/dfp_bench.h -> libdfp_bench.so (the roofline probes, kept out
+    of the product library and header)."""
+    names = _declared("dfp.h")
     assert {"dfp_forward", "dfp_forward_pose_grad", "dfp_backproject", "dfp_backproject_pose_grad",
             "dfp_workspace_bytes", "dfp_status_string"} <= names
+    assert "dfp_microbench" not in names
     lib = ctypes.CDLL(dfp.lib_path())
     for n in names:
         assert hasattr(lib, n), n
+    assert not hasattr(lib, "dfp_microbench")
+    from paper_2508_13304_b200 import microbench
+    bench_names = _declared("dfp_bench.h")
+    assert bench_names == {"dfp_microbench"}
+    blib = ctypes.CDLL(microbench.lib_path())
+    for n in bench_names:
+        assert hasattr(blib, n), n
 
 
 def test_geometry_struct_matches_the_header(dfp):
@@ -100,8 +114,9 @@ def test_bad_arguments_are_rejected_without_a_gpu(dfp):
     assert call(ctypes.byref(gf), 2, P(nanf), P(pose), fake, fake, fake, 1 << 30) == -3
 
 
-def test_microbench_rejects_bad_arguments(dfp):
-    lib = ctypes.CDLL(dfp.lib_path())
+def test_microbench_rejects_bad_arguments():
+    from paper_2508_13304_b200 import microbench
+    lib = ctypes.CDLL(microbench.lib_path())
     lib.dfp_microbench.restype = ctypes.c_int
     lib.dfp_microbench.argtypes = [ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
     r = ctypes.c_double(0.0)

@@ -15,7 +15,7 @@ import torch
 
 import oracle
 import workloads as W
-from helpers import grad_err_u9, rel_l2
+from helpers import check_values, grad_err_u9, rel_l2
 
 pytestmark = pytest.mark.gpu
 
@@ -65,14 +65,20 @@ def check_forward_full(dfp, index, n_check_views, band_rows, n_grad_views):
         o = oracle.forward(gb, a[v:v + 1], p[v:v + 1], vol_c)[0]
         got = proj[v, r0:r0 + band_rows].cpu().numpy()
         assert np.linalg.norm(o) > 0
-        e = rel_l2(got, o)
-        assert e <= TOL_VAL, (index, v, r0, e)
-        assert np.array_equal(got == 0, o == 0) or e <= TOL_VAL
-    for v in views[:n_grad_views]:
-        o = oracle.forward_pose_grad(g, a[v:v + 1], p[v:v + 1], vol_c, up[v:v + 1].cpu().numpy())
-        e = grad_err_u9(grad[v:v + 1], o)
-        assert e.max() <= TOL_GRAD, (index, v, e)
+        check_values(got, o, TOL_VAL, zero_border=True)
+    gviews = pick(w.seed + 131, w.n_views, n_grad_views)
+    o = oracle.forward_pose_grad(g, a[gviews], p[gviews], vol_c, up[gviews].cpu().numpy())
+    e = grad_err_u9(grad[gviews], o)
+    report(f"C{index} forward_pose_grad, {len(gviews)} seeded views", e)
+    assert e.max() <= TOL_GRAD, (index, gviews, e)
     return w
+
+
+def report(what, e):
+    """Error quantiles of a [views, 6] table of U9 errors, into the test log (pytest -s / -rP shows it)."""
+    q = np.quantile(e, [0.5, 0.9, 1.0])
+    print(f"{what}: U9 error median {q[0]:.2e}  p90 {q[1]:.2e}  max {q[2]:.2e}  (tolerance {TOL_GRAD:.0e}); "
+          f"per-view max " + " ".join(f"{x:.1e}" for x in e.max(axis=1)))
 
 
 def check_back_full(dfp, index, n_slabs, slab, n_grad_views):
@@ -95,34 +101,36 @@ def check_back_full(dfp, index, n_slabs, slab, n_grad_views):
         d = vol[z0:z0 + slab].cpu().numpy().astype(np.float64) - o
         num += float((d * d).sum())
         den += float((o * o).sum())
+        assert np.abs(d).max() <= 5e-5 * np.abs(o).max(), (index, z0)      # per element: no wrong voxel hides in the L2
     assert den > 0 and (num / den) ** 0.5 <= TOL_VAL, (index, (num / den) ** 0.5)
     up_c = up.cpu().numpy()
-    for v in pick(w.seed + 401, w.n_views, n_grad_views):
-        o = oracle.backproject_pose_grad(g, a[v:v + 1], p[v:v + 1], proj_c[v:v + 1], up_c)
-        e = grad_err_u9(grad[v:v + 1], o)
-        assert e.max() <= TOL_GRAD, (index, v, e)
+    gviews = pick(w.seed + 401, w.n_views, n_grad_views)
+    o = oracle.backproject_pose_grad(g, a[gviews], p[gviews], proj_c[gviews], up_c)
+    e = grad_err_u9(grad[gviews], o)
+    report(f"C{index} backproject_pose_grad, {len(gviews)} seeded views", e)
+    assert e.max() <= TOL_GRAD, (index, gviews, e)
 
 
 def test_c2_registration_full(dfp):
     """The workload bench.py times: 256^3, 64 candidate poses, 512x512 detector."""
-    check_forward_full(dfp, 2, n_check_views=3, band_rows=64, n_grad_views=2)
+    check_forward_full(dfp, 2, n_check_views=3, band_rows=64, n_grad_views=8)
 
 
 def test_c3_mcfdk_full(dfp):
     """256^3, 360 ramp-filtered views of 512x384, FDK weight."""
-    check_back_full(dfp, 3, n_slabs=3, slab=2, n_grad_views=2)
+    check_back_full(dfp, 3, n_slabs=3, slab=2, n_grad_views=8)
 
 
 def test_c4_calibration_full(dfp):
     """512^3, 720 views of 768x768."""
-    check_forward_full(dfp, 4, n_check_views=2, band_rows=32, n_grad_views=1)
+    check_forward_full(dfp, 4, n_check_views=2, band_rows=32, n_grad_views=8)
 
 
 def test_c5_sweep_full(dfp):
     """512^3, 360 views of 1024x1024: all four calls (the largest config; everything resident at once)."""
-    check_forward_full(dfp, 5, n_check_views=2, band_rows=24, n_grad_views=1)
+    check_forward_full(dfp, 5, n_check_views=2, band_rows=24, n_grad_views=8)
     torch.cuda.empty_cache()
-    check_back_full(dfp, 5, n_slabs=2, slab=1, n_grad_views=1)
+    check_back_full(dfp, 5, n_slabs=2, slab=1, n_grad_views=8)
 
 
 def test_c2_registration_full_grad_interp_mode(dfp):

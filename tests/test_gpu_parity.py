@@ -12,7 +12,7 @@ import torch
 
 import oracle
 import workloads as W
-from helpers import aniso_geom, grad_err_u9, rel_l2, small_geom
+from helpers import aniso_geom, check_values, grad_err_u9, rel_l2, small_geom
 
 pytestmark = pytest.mark.gpu
 
@@ -54,19 +54,18 @@ def run_back_case(dfp, g, angles, poses, proj, up):
     return vol, grad, o_vol, o_grad
 
 
-def check_forward(res):
+def check_forward(res, zero_border=False):
     proj, grad, o_proj, o_grad = res
     assert np.all(np.isfinite(proj)) and np.all(np.isfinite(grad))
-    assert rel_l2(proj, o_proj) <= TOL_VAL, rel_l2(proj, o_proj)
-    assert np.array_equal(proj == 0, o_proj == 0) or rel_l2(proj, o_proj) <= TOL_VAL
+    check_values(proj, o_proj, TOL_VAL, zero_border=zero_border)
     e = grad_err_u9(grad, o_grad)
     assert e.max() <= TOL_GRAD, e
 
 
-def check_back(res):
+def check_back(res, zero_border=False):
     vol, grad, o_vol, o_grad = res
     assert np.all(np.isfinite(vol)) and np.all(np.isfinite(grad))
-    assert rel_l2(vol, o_vol) <= TOL_VAL, rel_l2(vol, o_vol)
+    check_values(vol, o_vol, TOL_VAL, zero_border=zero_border)
     e = grad_err_u9(grad, o_grad)
     assert e.max() <= TOL_GRAD, e
 
@@ -172,12 +171,16 @@ def test_results_are_deterministic(dfp):
     assert torch.equal(b1, b2)
 
 
-def test_ray_step_count_matches_oracle(dfp):
-    w = W.make_config(1)
+@pytest.mark.parametrize("index,scale,views", [(1, 1.0, None), (2, 0.25, 5), (4, 0.125, 6), (5, 0.125, 6)])
+def test_ray_step_count_matches_oracle(dfp, index, scale, views):
+    """The metric's unit (SURVEY.md 8d) is defined by the ORACLE's clip - samples inside the 2-voxel-padded box;
+    dfp_count_ray_steps counts the same set (both in fp64: they may differ only on samples within rounding of the
+    box faces)."""
+    w = W.make_config(index, scale=scale, n_views=views)
     a, p = f32(w.angles), f32(w.poses)
     n_gpu = dfp.count_ray_steps(w.geom, a, p)
     _, n_ora = oracle.forward(w.geom, a, p, w.volume().numpy(), return_steps=True)
-    assert abs(n_gpu - n_ora) <= 1e-2 * n_ora, (n_gpu, n_ora)   # the clip box carries a 1/16-voxel safety margin
+    assert n_ora > 0 and abs(n_gpu - n_ora) <= max(2, 1e-6 * n_ora), (n_gpu, n_ora)
 
 
 # ------------------------------------------------------------------ the five configs, reduced so the oracle takes seconds
@@ -185,7 +188,7 @@ def test_ray_step_count_matches_oracle(dfp):
 def test_forward_configs_reduced(dfp, index, scale, views):
     w = W.make_config(index, scale=scale, n_views=views)
     check_forward(run_forward_case(dfp, w.geom, w.angles.numpy(), w.poses.numpy(), w.volume().numpy(),
-                                   w.fwd_upstream().numpy()))
+                                   w.fwd_upstream().numpy()), zero_border=True)
 
 
 @pytest.mark.parametrize("index,scale,views", [(3, 0.25, 12), (5, 0.125, 6)])
@@ -211,8 +214,9 @@ def _both_paths(dfp, g, angles, poses, vol, up):
 
 
 def _same(o):
-    """The two forward paths do the same arithmetic per sample; the TMA kernels split a ray's samples between two
-    lanes (even / odd) and add the two partial sums, so the results agree to fp32 summation order."""
+    """The two forward paths do the same arithmetic per sample on positions re-based at different places (per chunk of
+    the block / per 16 samples of the ray), and the TMA gradient kernels split a ray's samples between lanes: the results
+    agree to fp32 rounding."""
     pt, pg = o["tma"][0].numpy(), o["gather"][0].numpy()
     return (rel_l2(pt, pg) <= 2e-6 and np.array_equal(pt == 0, pg == 0) and
             grad_err_u9(o["tma"][1].numpy(), o["gather"][1].numpy()).max() <= 2e-5)
@@ -510,6 +514,61 @@ def test_host_buffer_entry_points_chunked_views(dfp):
     assert np.array_equal(got, ref)
 
 
+def test_host_buffer_chunks_keep_alignment_on_odd_detectors(dfp):
+    """nu * nv odd (21 x 17) with 9..11 views: a chunk that started at view 2 had an image offset of 8 mod 16 bytes
+    (DFP_ERR_ALIGN after chunk 0 was queued).  Chunk boundaries are multiples of 4 views; all four host calls."""
+    g = aniso_geom()
+    assert (g.nu * g.nv) % 2 == 1
+    rng = np.random.default_rng(11)
+    dev = torch.device("cuda:0")
+    for V in (9, 10, 11, 13):
+        a = f32(np.linspace(0.0, 5.0, V))
+        p = f32(np.concatenate([rng.uniform(-3, 3, (V, 3)), rng.uniform(-0.2, 0.2, (V, 3))], axis=1))
+        vol = rng.standard_normal(g.vol_shape).astype(np.float32)
+        up = rng.standard_normal((V,) + g.det_shape).astype(np.float32)
+        wv = rng.standard_normal(g.vol_shape).astype(np.float32)
+        vd, ud, wd = (torch.as_tensor(x, device=dev) for x in (vol, up, wv))
+        proj = dfp.forward(g, a, p, vd)
+        assert torch.equal(dfp.forward_host(g, a, p, vol), proj.cpu())
+        assert torch.equal(dfp.forward_pose_grad_host(g, a, p, vol, up), dfp.forward_pose_grad(g, a, p, vd, ud).cpu())
+        pj = proj.cpu().numpy()
+        assert rel_l2(dfp.backproject_host(g, a, p, pj).numpy(), dfp.backproject(g, a, p, proj).cpu().numpy()) <= 1e-6
+        assert torch.equal(dfp.backproject_pose_grad_host(g, a, p, pj, wv),
+                           dfp.backproject_pose_grad(g, a, p, proj, wd).cpu())
+
+
+def test_more_views_than_one_grid_holds(dfp):
+    """70 000 views (> 65 535, the grid-z limit): the library slices the batch internally; every view's result equals
+    the one it has in a small batch.  All four calls and the unit counter, on a tiny scanner."""
+    g = W.Geometry(nx=8, ny=8, nz=8, vx=1.0, vy=1.0, vz=1.0, nu=8, nv=4, du=1.5, dv=1.5, sad=60.0, sdd=90.0)
+    V = 70000
+    rng = np.random.default_rng(12)
+    dev = torch.device("cuda:0")
+    a = f32(rng.uniform(0, 6.28, V))
+    p = f32(np.concatenate([rng.uniform(-1, 1, (V, 3)), rng.uniform(-0.1, 0.1, (V, 3))], axis=1))
+    vol = torch.as_tensor(rng.random(g.vol_shape).astype(np.float32), device=dev)
+    up = torch.as_tensor(rng.standard_normal((V,) + g.det_shape).astype(np.float32), device=dev)
+    wv = torch.as_tensor(rng.standard_normal(g.vol_shape).astype(np.float32), device=dev)
+    proj = dfp.forward(g, a, p, vol)
+    grad = dfp.forward_pose_grad(g, a, p, vol, up)
+    bgrad = dfp.backproject_pose_grad(g, a, p, proj, wv)
+    bp = dfp.backproject(g, a, p, proj)
+    assert all(torch.isfinite(t).all() for t in (proj, grad, bgrad, bp))
+    sel = np.array([0, 1, 65531, 65532, 65535, 65536, 69999])
+    ps, us = proj[sel].contiguous(), up[sel].contiguous()
+    # (another batch may get another staging box / tile depth: the same terms in another fp32 order)
+    assert rel_l2(dfp.forward(g, a[sel], p[sel], vol).cpu().numpy(), ps.cpu().numpy()) <= 1e-6
+    assert grad_err_u9(dfp.forward_pose_grad(g, a[sel], p[sel], vol, us).cpu().numpy(), grad[sel].cpu().numpy()).max() <= 1e-4
+    assert grad_err_u9(dfp.backproject_pose_grad(g, a[sel], p[sel], ps, wv).cpu().numpy(),
+                       bgrad[sel].cpu().numpy()).max() <= 1e-4
+    # the volume is the sum over all views: two halves accumulated == the whole, up to the fp32 order of the sum
+    h = dfp.backproject(g, a[:35000], p[:35000], proj[:35000].contiguous())
+    dfp.backproject(g.replace(flags=dfp.FLAG_ACCUMULATE), a[35000:], p[35000:], proj[35000:].contiguous(), out=h)
+    assert rel_l2(h.cpu().numpy(), bp.cpu().numpy()) <= 1e-5
+    n_all = dfp.count_ray_steps(g, a, p)
+    assert n_all == dfp.count_ray_steps(g, a[:65532], p[:65532]) + dfp.count_ray_steps(g, a[65532:], p[65532:])
+
+
 # ------------------------------------------------------------------ DFP_FLAG_SIDDON (SURVEY section 8f-3)
 def run_siddon_case(dfp, g, angles, poses, vol, up):
     dev = torch.device("cuda:0")
@@ -661,11 +720,13 @@ def test_joseph_and_siddon_flags_exclude_each_other(dfp):
 
 
 # ------------------------------------------------------------------ dfp_microbench (roofline denominators)
-def test_microbench_rates_are_those_of_a_b200_class_sm(dfp):
-    """One warp-wide LDS per clock per SM and 128 fp32 lanes per SM at 1-2.5 GHz on >= 100 SMs."""
+def test_microbench_rates_are_those_of_a_b200_class_sm():
+    """One warp-wide LDS per clock per SM and 128 fp32 lanes per SM at 1-2.5 GHz on >= 100 SMs.
+    The probes live in libdfp_bench.so (include/dfp_bench.h), outside the product library."""
+    from paper_2508_13304_b200 import microbench as mb
     n_sm = torch.cuda.get_device_properties(0).multi_processor_count
-    lds = dfp.microbench(dfp.MB_LDS) / n_sm
+    lds = mb.run(mb.MB_LDS) / n_sm
     assert 0.8e9 < lds < 2.6e9, lds                              # ~1 per clock
-    for kind in (dfp.MB_FADD, dfp.MB_FFMA, dfp.MB_FFMA2):
-        r = dfp.microbench(kind) / n_sm
+    for kind in (mb.MB_FADD, mb.MB_FFMA, mb.MB_FFMA2):
+        r = mb.run(kind) / n_sm
         assert 100 * 0.9e9 < r < 130 * 2.6e9, (kind, r)          # ~128 per clock

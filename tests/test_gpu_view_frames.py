@@ -11,7 +11,7 @@ import torch
 
 import oracle
 import workloads as W
-from helpers import aniso_geom, grad_err_u9, rel_l2, small_geom
+from helpers import check_values, aniso_geom, grad_err_u9, rel_l2, small_geom
 from test_gpu_parity import POSES3, check_back, check_forward, f32, run_back_case, run_forward_case
 from test_oracle_view_frames import _general_frame
 
@@ -57,7 +57,7 @@ def test_general_frames_tma_paths_and_other_modes(dfp):
     check_forward(res)
     res_g = run_forward_case(dfp, g.replace(flags=VF | dfp.FLAG_NO_TMA), F, POSES3, vol, up)
     assert dfp.last_path() == dfp.PATH_GATHER
-    assert np.array_equal(res[0], res_g[0])                       # same arithmetic sample for sample
+    assert rel_l2(res[0], res_g[0]) <= 2e-6                        # same arithmetic per sample, positions re-based elsewhere
     proj = rng.random((3,) + g.det_shape).astype(np.float32)
     upv = rng.standard_normal(g.vol_shape).astype(np.float32)
     for bw, fl in ((0, 0), (1, 1)):
@@ -278,8 +278,8 @@ def test_random_frames_both_paths_agree_and_never_nan(dfp):
                            dfp.backproject_pose_grad(gn, F, poses, pin, bup).cpu().numpy()).max() <= 1e-4, case
         if case % 3 == 0:
             o_proj, o_bp = oracle.forward(g, F, poses, vol.cpu().numpy()), oracle.backproject(g, F, poses, pin_np)
-            assert rel_l2(proj.cpu().numpy(), o_proj) <= 1e-5 or not o_proj.any(), case
-            assert rel_l2(bp.cpu().numpy(), o_bp) <= 1e-5 or not o_bp.any(), case
+            check_values(proj.cpu().numpy(), o_proj, 1e-5, zero_border=False)    # all-zero oracle => all-zero result
+            check_values(bp.cpu().numpy(), o_bp, 1e-5, zero_border=False)
             check_grad(grad.cpu().numpy(), oracle.forward_pose_grad(g, F, poses, vol.cpu().numpy(), up.cpu().numpy()), case)
             check_grad(bgrad.cpu().numpy(), oracle.backproject_pose_grad(g, F, poses, pin_np, bup.cpu().numpy()), case)
     print("TMA calls", n_tma)
