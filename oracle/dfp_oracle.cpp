@@ -849,6 +849,222 @@ void forward_grad_joseph_impl(const ora_geom& g, int n_views, const double* angl
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// O15: distance-driven projector pair [44] (PAPER.md :213, Tables III / IV rows DD) under a rigid
+// pose and a general flat detector.  The paper cites the method and gives no formula; reading taken (U14):
+//   * everything in the OBJECT frame: source s' = R^T (s - t), detector points X(u, v) = R^T (c + (u - c_u) U +
+//     (v - c_v) V - t) for real (u, v) - pixel (iu, iv) covers [iu - 1/2, iu + 1/2] x [iv - 1/2, iv + 1/2];
+//   * per VIEW the driving axis a* = argmax_a |n'_a|, n' = direction from s' to the detector's central point
+//     ((nu-1)/2, (nv-1)/2); the other two axes (b, d) = ((a*+1)%3, (a*+2)%3); the detector's u pairs with the in-plane
+//     axis along which the pixel step U' = R^T U is longer (|U'_b| >= |U'_d|: u<->b, v<->d; else u<->d, v<->b);
+//   * per plane k of voxel centres along a* (x_a = c_a + (k - (n_a - 1)/2) v_a): the pixel's boundary mid-points
+//     (iu -+ 1/2, iv) and (iu, iv -+ 1/2) are projected from the source onto the plane; in continuous voxel indices
+//     they bound the pixel's footprint [B0, B1] along u's axis and [D0, D1] along v's axis (the distance-driven
+//     separable footprint, taken per pixel so that in-plane rotations of the pose are followed);
+//   * a^ij = L (|[B0,B1] n cell_B(j)| / (B1 - B0)) (|[D0,D1] n cell_D(j)| / (D1 - D0)),  cell(j) = [j - 1/2, j + 1/2],
+//     L = v_a* / |e'_a*| with e' the unit direction of the pixel-centre ray: normalised overlap x slab path length
+//     (a uniform volume gives the chord); planes behind the source (any of the five rays with t <= 0) are skipped.
+// Forward l_i = sum_j a^ij mu_j; the back-projector is its EXACT transpose mu_j = sum_i a^ij l_i (Eq.21 :193-196: DD
+// is a matched pair), unit weight only.  `visit(w, ix, iy, iz)` for every grid voxel with a non-zero weight.
+struct DDView {
+  V3 so, X00, Uo, Vo;          // object frame: source, detector point of index (0, 0), steps per pixel along u and v
+  int a, b, d;                 // driving axis and the two in-plane axes
+  bool u_is_b;
+  DDView(const ora_geom& g, const View& view, const Pose& pose) {
+    so = mulT(pose.R, view.s - pose.t);
+    Uo = mulT(pose.R, view.U); Vo = mulT(pose.R, view.Vs);
+    X00 = mulT(pose.R, view.dc - pose.t) - view.cu * Uo - view.cv * Vo;
+    V3 n = X00 + ((g.nu - 1) / 2.0) * Uo + ((g.nv - 1) / 2.0) * Vo - so;
+    a = 0;
+    for (int k = 1; k < 3; ++k) if (fabs(comp(n, k)) > fabs(comp(n, a))) a = k;
+    b = (a + 1) % 3; d = (a + 2) % 3;
+    u_is_b = fabs(comp(Uo, b)) >= fabs(comp(Uo, d));
+  }
+  V3 det(double u, double v) const { return X00 + u * Uo + v * Vo; }
+};
+template <typename F>
+inline void dd_weights(const ora_geom& g, const DDView& W, int iu, int iv, F visit) {
+  const int n[3] = {g.nx, g.ny, g.nz};
+  const double v[3] = {g.vx, g.vy, g.vz}, c[3] = {g.cx, g.cy, g.cz};
+  const int a = W.a, ub = W.u_is_b ? W.b : W.d, vb = W.u_is_b ? W.d : W.b;   // axis paired with u, with v
+  const V3 pts[5] = {W.det(iu, iv), W.det(iu - 0.5, iv), W.det(iu + 0.5, iv), W.det(iu, iv - 0.5), W.det(iu, iv + 0.5)};
+  V3 dir[5];
+  for (int q = 0; q < 5; ++q) dir[q] = pts[q] - W.so;
+  const double elen = sqrt(dot(dir[0], dir[0]));
+  const double ea = comp(dir[0], a) / elen;
+  if (fabs(ea) < 1e-300) return;
+  const double L = v[a] / fabs(ea);
+  for (int k = 0; k < n[a]; ++k) {
+    const double xa = c[a] + (k - (n[a] - 1) / 2.0) * v[a];
+    double t[5];
+    bool front = true;
+    for (int q = 0; q < 5; ++q) {
+      const double da = comp(dir[q], a);
+      if (fabs(da) < 1e-300) { front = false; break; }
+      t[q] = (xa - comp(W.so, a)) / da;
+      if (!(t[q] > 0)) { front = false; break; }
+    }
+    if (!front) continue;
+    auto idx = [&](int q, int ax) { return (comp(W.so, ax) + t[q] * comp(dir[q], ax) - c[ax]) / v[ax] + (n[ax] - 1) / 2.0; };
+    double B0 = idx(1, ub), B1 = idx(2, ub), D0 = idx(3, vb), D1 = idx(4, vb);
+    if (B0 > B1) std::swap(B0, B1);
+    if (D0 > D1) std::swap(D0, D1);
+    if (!(B1 > B0) || !(D1 > D0)) continue;
+    const long jb0 = (long)floor(B0 + 0.5), jb1 = (long)floor(B1 + 0.5);
+    const long jd0 = (long)floor(D0 + 0.5), jd1 = (long)floor(D1 + 0.5);
+    for (long jd = jd0; jd <= jd1; ++jd) {
+      if (jd < 0 || jd >= n[vb]) continue;
+      const double od = std::min(D1, jd + 0.5) - std::max(D0, jd - 0.5);
+      if (!(od > 0)) continue;
+      for (long jb = jb0; jb <= jb1; ++jb) {
+        if (jb < 0 || jb >= n[ub]) continue;
+        const double ob = std::min(B1, jb + 0.5) - std::max(B0, jb - 0.5);
+        if (!(ob > 0)) continue;
+        long id[3];
+        id[a] = k; id[ub] = jb; id[vb] = jd;
+        visit(L * (ob / (B1 - B0)) * (od / (D1 - D0)), id[0], id[1], id[2]);
+      }
+    }
+  }
+}
+
+// forward (vol_out == nullptr) or explicit transpose = the DD back-projector, slab [iz0, iz1) of the volume
+template <typename T>
+void forward_dd_impl(const ora_geom& g, int n_views, const double* angles, const double* poses, const T* vol,
+                     double* proj, const float* y_in, double* vol_out, int iz0, int iz1) {
+  Vol<T> V{vol, g.nx, g.ny, g.nz};
+  const bool transpose = vol_out != nullptr;
+  const size_t nslab = transpose ? (size_t)(iz1 - iz0) * g.ny * g.nx : 0;
+  for (size_t i = 0; i < nslab; ++i) vol_out[i] = 0.0;
+  int nthr = 1;
+#ifdef _OPENMP
+  nthr = omp_get_max_threads();
+#endif
+  std::vector<std::vector<double>> priv(transpose ? nthr : 0);
+  for (auto& p : priv) p.assign(nslab, 0.0);
+  for (int v = 0; v < n_views; ++v) {
+    View view(g, angles, v);
+    Pose pose(poses + 6 * v);
+    const DDView W(g, view, pose);
+#pragma omp parallel for schedule(static)      // fixed row -> thread map: the transpose's sums have one order
+    for (int iv = 0; iv < g.nv; ++iv) {
+      int me = 0;
+#ifdef _OPENMP
+      me = omp_get_thread_num();
+#endif
+      for (int iu = 0; iu < g.nu; ++iu) {
+        const size_t pix = ((size_t)v * g.nv + iv) * g.nu + iu;
+        if (!transpose) {
+          double sum = 0.0;
+          dd_weights(g, W, iu, iv, [&](double w, long ix, long iy, long iz) { sum += w * V.at(ix, iy, iz); });
+          proj[pix] = sum;
+        } else {
+          const double yi = (double)y_in[pix];
+          double* out = priv[me].data();
+          dd_weights(g, W, iu, iv, [&](double w, long ix, long iy, long iz) {
+            if (iz >= iz0 && iz < iz1) out[((size_t)(iz - iz0) * g.ny + iy) * g.nx + ix] += w * yi;
+          });
+        }
+      }
+    }
+  }
+  for (auto& p : priv) for (size_t i = 0; i < nslab; ++i) vol_out[i] += p[i];      // thread order: fixed
+}
+
+// Pose gradient through the DD forward projector: per-voxel G_f^j with the weights a^ij (Eq.19-20 :179-191), as O12.
+template <typename T>
+void forward_grad_dd_impl(const ora_geom& g, int n_views, const double* angles, const double* poses, const T* vol,
+                          const float* upstream, double* grad) {
+  Vol<T> V{vol, g.nx, g.ny, g.nz};
+  for (int v = 0; v < n_views; ++v) {
+    View view(g, angles, v);
+    Pose pose(poses + 6 * v);
+    const DDView W(g, view, pose);
+    std::vector<double> rowacc((size_t)g.nv * 6, 0.0);
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int iv = 0; iv < g.nv; ++iv) {
+      double acc[6] = {0};
+      for (int iu = 0; iu < g.nu; ++iu) {
+        const double w = (double)upstream[((size_t)v * g.nv + iv) * g.nu + iu];
+        V3 A = {0, 0, 0}, B = {0, 0, 0};
+        dd_weights(g, W, iu, iv, [&](double a, long X, long Y, long Z) {
+          V3 gj = {(V.at(X + 1, Y, Z) - V.at(X - 1, Y, Z)) / (2 * g.vx),
+                   (V.at(X, Y + 1, Z) - V.at(X, Y - 1, Z)) / (2 * g.vy),
+                   (V.at(X, Y, Z + 1) - V.at(X, Y, Z - 1)) / (2 * g.vz)};
+          V3 rj = voxel_centre(g, (int)X, (int)Y, (int)Z);
+          A = A + a * gj;
+          B = B + a * cross(rj, gj);
+        });
+        acc[0] += w * A.x; acc[1] += w * A.y; acc[2] += w * A.z;
+        acc[3] += w * B.x; acc[4] += w * B.y; acc[5] += w * B.z;
+      }
+      for (int q = 0; q < 6; ++q) rowacc[(size_t)iv * 6 + q] = acc[q];
+    }
+    double tot[6] = {0};
+    for (int iv = 0; iv < g.nv; ++iv) for (int q = 0; q < 6; ++q) tot[q] += rowacc[(size_t)iv * 6 + q];
+    V3 SA = {tot[0], tot[1], tot[2]}, SB = {tot[3], tot[4], tot[5]};
+    V3 dt = mul(pose.R, SA);
+    double* out = grad + 6 * v;
+    out[0] = -dt.x; out[1] = -dt.y; out[2] = -dt.z;
+    const double* th = poses + 6 * v;
+    V3 wx = {1, 0, 0};
+    V3 wy = mulT(Rx(th[3]), V3{0, 1, 0});
+    V3 wz = mulT(mul(Ry(th[4]), Rx(th[3])), V3{0, 0, 1});
+    out[3] = -dot(wx, SB); out[4] = -dot(wy, SB); out[5] = -dot(wz, SB);
+  }
+}
+
+// Pose gradient through the DD back-projector, Eq.22 (:198-206) with the DD weights: per detector PIXEL i the
+// central differences of the zero-extended projection, D_u^i = (l[iv][iu+1] - l[iv][iu-1]) / 2, D_v^i likewise ("the
+// projection gradient is approximated by a central finite difference", "compute G_b^i for each detector pixel"; i runs
+// over the detector's pixels); per pair (i, j): a^ij w_j (D_u^i J_u(r_j) + D_v^i J_v(r_j)), J from Eq.13 at the voxel
+// centre r_j = R r'_j + t; S_q, S_c and the contraction as O9.
+void backproject_grad_dd_impl(const ora_geom& g, int n_views, const double* angles, const double* poses,
+                              const float* proj, const float* upstream, double* grad) {
+  for (int v = 0; v < n_views; ++v) {
+    View view(g, angles, v);
+    Pose pose(poses + 6 * v);
+    const DDView W(g, view, pose);
+    Img I{proj + (size_t)v * g.nu * g.nv, g.nu, g.nv};
+    const double(*P)[4] = view.P;
+    std::vector<double> rowacc((size_t)g.nv * 6, 0.0);
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int iv = 0; iv < g.nv; ++iv) {
+      double acc[6] = {0};
+      for (int iu = 0; iu < g.nu; ++iu) {
+        const double Du = 0.5 * (I.at(iu + 1, iv) - I.at(iu - 1, iv)), Dv = 0.5 * (I.at(iu, iv + 1) - I.at(iu, iv - 1));
+        if (Du == 0.0 && Dv == 0.0) continue;
+        dd_weights(g, W, iu, iv, [&](double a, long X, long Y, long Z) {
+          const double wj = (double)upstream[((size_t)Z * g.ny + Y) * g.nx + X];
+          V3 r = mul(pose.R, voxel_centre(g, (int)X, (int)Y, (int)Z)) + pose.t;
+          double up = P[0][0] * r.x + P[0][1] * r.y + P[0][2] * r.z + P[0][3];
+          double vp = P[1][0] * r.x + P[1][1] * r.y + P[1][2] * r.z + P[1][3];
+          double wp = P[2][0] * r.x + P[2][1] * r.y + P[2][2] * r.z + P[2][3];
+          V3 Ju = {(P[0][0] * wp - P[2][0] * up) / (wp * wp), (P[0][1] * wp - P[2][1] * up) / (wp * wp),
+                   (P[0][2] * wp - P[2][2] * up) / (wp * wp)};
+          V3 Jv = {(P[1][0] * wp - P[2][0] * vp) / (wp * wp), (P[1][1] * wp - P[2][1] * vp) / (wp * wp),
+                   (P[1][2] * wp - P[2][2] * vp) / (wp * wp)};
+          V3 q = (a * wj) * ((Du * Ju) + (Dv * Jv));
+          V3 cq = cross(r - pose.t, q);
+          acc[0] += q.x; acc[1] += q.y; acc[2] += q.z;
+          acc[3] += cq.x; acc[4] += cq.y; acc[5] += cq.z;
+        });
+      }
+      for (int k = 0; k < 6; ++k) rowacc[(size_t)iv * 6 + k] = acc[k];
+    }
+    double tot[6] = {0};
+    for (int iv = 0; iv < g.nv; ++iv) for (int k = 0; k < 6; ++k) tot[k] += rowacc[(size_t)iv * 6 + k];
+    const double* th = poses + 6 * v;
+    V3 Sq = {tot[0], tot[1], tot[2]}, Sc = {tot[3], tot[4], tot[5]};
+    V3 ax = mul(pose.R, V3{1, 0, 0});
+    V3 ay = mul(Rz(th[5]), V3{0, 1, 0});
+    V3 az = {0, 0, 1};
+    double* out = grad + 6 * v;
+    out[0] = Sq.x; out[1] = Sq.y; out[2] = Sq.z;
+    out[3] = dot(ax, Sc); out[4] = dot(ay, Sc); out[5] = dot(az, Sc);
+  }
+}
+
 extern "C" {
 
 int ora_num_threads() {
@@ -957,6 +1173,32 @@ void ora_forward_pose_grad_joseph_f32(const ora_geom* g, int n_views, const doub
 void ora_forward_pose_grad_joseph_f64(const ora_geom* g, int n_views, const double* angles, const double* poses,
                                       const double* vol, const float* upstream, double* grad) {
   forward_grad_joseph_impl<double>(*g, n_views, angles, poses, vol, upstream, grad);
+}
+
+// O15: distance-driven pair (forward, back-projector = exact transpose, both pose gradients)
+void ora_forward_dd_f32(const ora_geom* g, int n_views, const double* angles, const double* poses, const float* vol,
+                        double* proj) {
+  forward_dd_impl<float>(*g, n_views, angles, poses, vol, proj, nullptr, nullptr, 0, 0);
+}
+void ora_forward_dd_f64(const ora_geom* g, int n_views, const double* angles, const double* poses, const double* vol,
+                        double* proj) {
+  forward_dd_impl<double>(*g, n_views, angles, poses, vol, proj, nullptr, nullptr, 0, 0);
+}
+void ora_backproject_dd(const ora_geom* g, int n_views, const double* angles, const double* poses, const float* proj,
+                        double* vol_out, int iz0, int iz1) {
+  forward_dd_impl<float>(*g, n_views, angles, poses, (const float*)nullptr, nullptr, proj, vol_out, iz0, iz1);
+}
+void ora_forward_pose_grad_dd_f32(const ora_geom* g, int n_views, const double* angles, const double* poses,
+                                  const float* vol, const float* upstream, double* grad) {
+  forward_grad_dd_impl<float>(*g, n_views, angles, poses, vol, upstream, grad);
+}
+void ora_forward_pose_grad_dd_f64(const ora_geom* g, int n_views, const double* angles, const double* poses,
+                                  const double* vol, const float* upstream, double* grad) {
+  forward_grad_dd_impl<double>(*g, n_views, angles, poses, vol, upstream, grad);
+}
+void ora_backproject_pose_grad_dd(const ora_geom* g, int n_views, const double* angles, const double* poses,
+                                  const float* proj, const float* upstream, double* grad) {
+  backproject_grad_dd_impl(*g, n_views, angles, poses, proj, upstream, grad);
 }
 
 }  // extern "C"

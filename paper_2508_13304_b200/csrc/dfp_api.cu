@@ -339,7 +339,7 @@ FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad, int nset = 1) {
 
 constexpr int kBpGradZChunk = 16;
 struct BpWs {
-  size_t off_views, off_con, off_q, off_part, total;
+  size_t off_views, off_viewsd, off_con, off_q, off_part, total;
   int gx, gy, gz;  // voxel tiles (gather path)
   int tx, ty, tz;  // voxel tiles (TMA path)
 };
@@ -354,6 +354,7 @@ BpWs bp_ws(const dfp_geometry& g, int V, bool grad) {
   w.tz = (g.nz + 7) / 8;
   size_t o = 0;
   w.off_views = o; o += align_up(sizeof(BpView) * (size_t)V);
+  w.off_viewsd = o; o += align_up(sizeof(BpViewD) * (size_t)V);
   w.off_con = o;   o += grad ? align_up(sizeof(BpContract) * (size_t)V) : 0;
   w.off_q = o;     o += align_up(sizeof(float4) * (size_t)V * (g.nu + 2 * kPadDet) * (g.nv + 2 * kPadDet));
   w.off_part = o;
@@ -547,17 +548,20 @@ int run_backproject_slice(const dfp_geometry* g, int V, const float* angles, con
   if (st) return st;
   const BpGeom G = make_bp_geom(*g);
   std::vector<BpView> hv((size_t)V);
+  std::vector<BpViewD> hvd((size_t)V);
   std::vector<BpContract> hc(grad ? (size_t)V : 0);
   for (int v = 0; v < V; ++v)
-    make_bp_view(*g, G, make_frame(*g, angles, v), poses + 6 * v, &hv[v], grad ? &hc[v] : nullptr);
+    make_bp_view(*g, G, make_frame(*g, angles, v), poses + 6 * v, &hv[v], grad ? &hc[v] : nullptr, &hvd[v]);
   char* base = static_cast<char*>(d_ws);
   BpView* dv = reinterpret_cast<BpView*>(base + w.off_views);
+  BpViewD* dvd = reinterpret_cast<BpViewD*>(base + w.off_viewsd);
   BpContract* dc = reinterpret_cast<BpContract*>(base + w.off_con);
   float4* q = reinterpret_cast<float4*>(base + w.off_q);
   float* part = reinterpret_cast<float*>(base + w.off_part);
   g_launches = 0;
   g_path = DFP_PATH_GATHER;
   DFP_CUDA(upload_async(dv, hv.data(), sizeof(BpView) * V, s), "view upload");
+  DFP_CUDA(upload_async(dvd, hvd.data(), sizeof(BpViewD) * V, s), "view upload");
   if (grad) DFP_CUDA(upload_async(dc, hc.data(), sizeof(BpContract) * V, s), "view upload");
   // TMA-staged path: projections admit a tensor map, every voxel in front of the source, patches fit the menu
   int kmax = -1, TZ = 16;
@@ -579,7 +583,7 @@ int run_backproject_slice(const dfp_geometry* g, int V, const float* angles, con
     DFP_CUDA(ensure_smem_attributes(), "cudaFuncSetAttribute");
     const dim3 tgrid(w.tx, w.ty, (g->nz + TZ - 1) / TZ);
     g_path = DFP_PATH_TMA;
-#define DFP_BP_ARGS <<<tgrid, kBpTmaThreads, smem, s>>>(G, V, dv, maps, kmax, stage_words, n_stages
+#define DFP_BP_ARGS <<<tgrid, kBpTmaThreads, smem, s>>>(G, V, dvd, maps, kmax, stage_words, n_stages
     time_begin(s);
     if (!grad) {
       if (G.bp_weight) { if (TZ == 16) bp_tma_kernel<1, 16> DFP_BP_ARGS, d_out); else bp_tma_kernel<1, 8> DFP_BP_ARGS, d_out); }
@@ -624,8 +628,8 @@ int run_backproject_slice(const dfp_geometry* g, int V, const float* angles, con
     const bool interp = (G.flags & DFP_FLAG_GRAD_INTERP) != 0;
 #define DFP_BP_GRAD(W, D)                                                                                       \
   do {                                                                                                          \
-    if (interp) bp_grad_kernel<W, D, 1><<<grid, kBpThreads, 0, s>>>(G, V, kBpGradZChunk, dv, q, d_up, part);    \
-    else bp_grad_kernel<W, D, 0><<<grid, kBpThreads, 0, s>>>(G, V, kBpGradZChunk, dv, q, d_up, part);           \
+    if (interp) bp_grad_kernel<W, D, 1><<<grid, kBpThreads, 0, s>>>(G, V, kBpGradZChunk, dv, dvd, q, d_up, part);    \
+    else bp_grad_kernel<W, D, 0><<<grid, kBpThreads, 0, s>>>(G, V, kBpGradZChunk, dv, dvd, q, d_up, part);           \
   } while (0)
     if (!G.bp_weight) DFP_BP_GRAD(0, 0);
     else if (!dw) DFP_BP_GRAD(1, 0);

@@ -39,7 +39,7 @@ __device__ __constant__ int kPatchV[kNumPatches] = {16, 24, 32, 48, 64, 80};
 static const int kPatchUHost[kNumPatches] = {36, 52, 68, 68, 100, 100};
 static const int kPatchVHost[kNumPatches] = {16, 24, 32, 48, 64, 80};
 struct alignas(64) PatchMaps { CUtensorMap m[kNumPatches]; };
-constexpr int kPatchHeader = 32;                 // floats per stage in front of the patch: P_eff rows, c0, pitch, status
+constexpr int kPatchHeader = 64;                 // floats per stage in front of the patch: local P_eff rows, c0, pitch, status, fp64 rows
 constexpr int kBpMaxStages = 4;
 constexpr int kBpSmemBudget = 72 * 1024;         // dynamic shared memory per block: 3 blocks per SM
 inline int bp_stage_words(int kmax) { return kPatchUHost[kmax] * kPatchVHost[kmax] + kPatchHeader; }
@@ -53,32 +53,42 @@ __device__ __forceinline__ void mbar_arrive(unsigned bar) {
 }
 __device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kBpConsumers) : "memory"); }
 
-// Stage header layout (floats): [0..11] A rows (P_eff on centred voxel indices, u and v rows minus half the w row),
-// [12..20] J rows (gradient only), [24] c0b (as bits; see patch_locate), [25] status (as bits: 0 ok, 1 no patch
-// of the menu fits), [26] row pitch of the patch in BYTES (as bits).
+// Stage header layout (floats).  All rows are LOCAL to the (tile, view): they act on (lx, ly, lz) = voxel index minus
+// the tile's first voxel and yield (u, v) relative to the staged patch's first pixel (minus 1/2, for the magic floor):
+// [0..11] A rows, [12..20] J rows re-based likewise (gradient only; Eq.13 is invariant under a common shift of u),
+// [24] c0b (as bits; see below), [25] status (as bits: 0 ok, 1 no patch of the menu fits), [26] row pitch of the patch
+// in BYTES (as bits), [32..55] the A rows again in DOUBLE (12 values; the exact-interpolant mode's slow path).
+// The producer derives them in fp64 from BpViewD and rounds once.
 struct BpTile {
   int x0, y0, z0, tz;          // first voxel of the tile and its z extent (<= TZ)
 };
 
 // Producer: footprint of the tile in view `view`, header, TMA.  Called by the whole producer warp.
 template <int HALO>
-__device__ __forceinline__ void bp_issue_view(const BpGeom& G, const BpTile& T, const BpView* __restrict__ views,
+__device__ __forceinline__ void bp_issue_view(const BpGeom& G, const BpTile& T, const BpViewD* __restrict__ viewsd,
                                               const PatchMaps* maps, int kmax, int stage_words, int view, int stage,
                                               float* smem, unsigned smem_addr, unsigned full_addr) {
   const int lane = threadIdx.x & 31;
   float* hdr = smem + stage * stage_words;
-  const float* src = reinterpret_cast<const float*>(views + view);
-  if (lane < (int)(sizeof(BpView) / 4)) hdr[lane] = __ldg(src + lane);
-  // corner (lane & 7) of the tile, centred voxel indices
-  const int cx = T.x0 + ((lane & 1) ? kBpT - 1 : 0), cy = T.y0 + ((lane & 2) ? kBpT - 1 : 0),
-            cz = T.z0 + ((lane & 4) ? T.tz - 1 : 0);
-  const float xf = (float)min(cx, G.nx - 1) - G.hx, yf = (float)min(cy, G.ny - 1) - G.hy, zf = (float)cz - G.hz;
-  const float* A = src;
-  const float up = fmaf(__ldg(A + 0), xf, fmaf(__ldg(A + 1), yf, fmaf(__ldg(A + 2), zf, __ldg(A + 3))));
-  const float vp = fmaf(__ldg(A + 4), xf, fmaf(__ldg(A + 5), yf, fmaf(__ldg(A + 6), zf, __ldg(A + 7))));
-  const float wp = fmaf(__ldg(A + 8), xf, fmaf(__ldg(A + 9), yf, fmaf(__ldg(A + 10), zf, __ldg(A + 11))));
-  const float rw = fast_rcp(wp);
-  float ulo = up * rw, vlo = vp * rw, uhi = ulo, vhi = vlo;
+  const double* src = reinterpret_cast<const double*>(viewsd + view);       // A[3][4] then J[3][3]
+  // tile origin in centred voxel indices (exact in double); rows with the origin folded into the constant term
+  const double X0 = (double)T.x0 - (double)G.hx, Y0 = (double)T.y0 - (double)G.hy, Z0 = (double)T.z0 - (double)G.hz;
+  double A[3][4];
+#pragma unroll
+  for (int r = 0; r < 3; ++r) {
+#pragma unroll
+    for (int c = 0; c < 4; ++c) A[r][c] = __ldg(src + 4 * r + c);
+    A[r][3] = fma(A[r][0], X0, fma(A[r][1], Y0, fma(A[r][2], Z0, A[r][3])));
+  }
+  // corner (lane & 7) of the tile, local voxel indices
+  const double cx = (lane & 1) ? (double)(min(T.x0 + kBpT - 1, G.nx - 1) - T.x0) : 0.0,
+               cy = (lane & 2) ? (double)(min(T.y0 + kBpT - 1, G.ny - 1) - T.y0) : 0.0,
+               cz = (lane & 4) ? (double)(T.tz - 1) : 0.0;
+  const double wp = fma(A[2][0], cx, fma(A[2][1], cy, fma(A[2][2], cz, A[2][3])));
+  const double rw = 1.0 / wp;
+  float ulo = (float)(fma(A[0][0], cx, fma(A[0][1], cy, fma(A[0][2], cz, A[0][3]))) * rw);
+  float vlo = (float)(fma(A[1][0], cx, fma(A[1][1], cy, fma(A[1][2], cz, A[1][3]))) * rw);
+  float uhi = ulo, vhi = vlo;
 #pragma unroll
   for (int o = 4; o > 0; o >>= 1) {
     ulo = fminf(ulo, __shfl_xor_sync(0xffffffffu, ulo, o));
@@ -86,21 +96,33 @@ __device__ __forceinline__ void bp_issue_view(const BpGeom& G, const BpTile& T, 
     vlo = fminf(vlo, __shfl_xor_sync(0xffffffffu, vlo, o));
     vhi = fmaxf(vhi, __shfl_xor_sync(0xffffffffu, vhi, o));
   }
+  // cells floor(u - CU) = rint(uq) in [rint(lo), rint(hi)], stencil [-HALO, 1 + HALO]  (the same on every lane)
+  int ou = (int)floorf(ulo - 0.5f - kPatchMargin) - HALO, ov = (int)floorf(vlo - 0.5f - kPatchMargin) - HALO;
+  ou = (((ou + G.CU) >> 2) << 2) - G.CU;                       // 16-byte alignment of the TMA inner coordinate
+  const int eu = (int)floorf(uhi + 0.5f + kPatchMargin) + 1 + HALO - ou + 1;
+  const int ev = (int)floorf(vhi + 0.5f + kPatchMargin) + 1 + HALO - ov + 1;
+  int k = 0;
+  while (k <= kmax && (eu > kPatchU[k] || ev > kPatchV[k])) ++k;
+  const bool ok = k <= kmax && ulo == ulo && vlo == vlo;
+  if (!ok) k = 0;
+  // local rows: (u - ou) w' = (A0 - ou A2).(l;1), likewise v; J rows likewise
+  if (lane < 12) {
+    const int r = lane >> 2, c = lane & 3;
+    const double o = r == 0 ? (double)ou : (r == 1 ? (double)ov : 0.0);
+    const double a = A[r][c] - o * A[2][c];
+    hdr[lane] = (float)a;
+    reinterpret_cast<double*>(hdr + 32)[lane] = a;
+  } else if (lane < 21) {
+    const int r = (lane - 12) / 3, c = (lane - 12) - 3 * r;
+    const double o = r == 0 ? (double)ou : (r == 1 ? (double)ov : 0.0);
+    hdr[lane] = (float)(__ldg(src + 12 + 3 * r + c) - o * __ldg(src + 12 + 6 + c));
+  }
   __syncwarp();                                                  // header words written by lanes 0..20
   if (lane == 0) {
-    // cells floor(u - CU) = rint(uq) in [rint(lo), rint(hi)], stencil [-HALO, 1 + HALO]
-    int ou = (int)floorf(ulo - 0.5f - kPatchMargin) - HALO, ov = (int)floorf(vlo - 0.5f - kPatchMargin) - HALO;
-    ou = (((ou + G.CU) >> 2) << 2) - G.CU;                       // 16-byte alignment of the TMA inner coordinate
-    const int eu = (int)floorf(uhi + 0.5f + kPatchMargin) + 1 + HALO - ou + 1;
-    const int ev = (int)floorf(vhi + 0.5f + kPatchMargin) + 1 + HALO - ov + 1;
-    int k = 0;
-    while (k <= kmax && (eu > kPatchU[k] || ev > kPatchV[k])) ++k;
-    const bool ok = k <= kmax && ulo == ulo && vlo == vlo;
-    if (!ok) k = 0;
     const int U = kPatchU[k], V = kPatchV[k];
-    const unsigned mb = (unsigned)kMagicBits;
-    const unsigned c0b = smem_addr + 4u * ((unsigned)(stage * stage_words + kPatchHeader) - ((unsigned)ou + mb) -
-                                           (unsigned)U * ((unsigned)ov + mb));
+    // SHARED-space byte address of local pixel cell (X, Y) from the magic-rounded floats' bits: 4 X + 4 U Y + c0b
+    const unsigned c0b = smem_addr + 4u * (unsigned)(stage * stage_words + kPatchHeader) -
+                         (unsigned)kMagicBits * (4u + 4u * (unsigned)U);
     hdr[24] = __uint_as_float(c0b);
     hdr[25] = __uint_as_float(ok ? 0u : 1u);
     hdr[26] = __uint_as_float(4u * (unsigned)U);
@@ -115,8 +137,8 @@ __device__ __forceinline__ void bp_issue_view(const BpGeom& G, const BpTile& T, 
 
 // Pixel cell of one (voxel, view) pair inside the staged patch (no clamps: the patch holds the tile's whole
 // footprint plus the stencil halo, and out-of-detector pixels were zero-filled): the SHARED-space byte address of
-// pixel (floor u, floor v) is 4*Tu + pitch_bytes*Tv + c0b, two IMADs on the magic-rounded float bits (c0b folds the
-// stage base, the patch origin and the magic bias).
+// local pixel (floor u, floor v) is 4*Tu + pitch_bytes*Tv + c0b, two IMADs on the magic-rounded float bits (c0b folds
+// the stage base and the magic bias).
 template <int OFF>
 __device__ __forceinline__ float lds_f32(unsigned addr) {
   float v;
@@ -128,7 +150,7 @@ __device__ __forceinline__ float lds_f32(unsigned addr) {
 // TZ = voxels along z per thread (register accumulators): 16, or 8 where the magnification is so large that a
 // 16-deep tile's footprint exceeds the patch menu (C2: 2.5-3 pixels per voxel).
 template <int WEIGHT, int TZ>
-__global__ void __launch_bounds__(kBpTmaThreads) bp_tma_kernel(BpGeom G, int n_views, const BpView* __restrict__ views,
+__global__ void __launch_bounds__(kBpTmaThreads) bp_tma_kernel(BpGeom G, int n_views, const BpViewD* __restrict__ views,
                                                                const __grid_constant__ PatchMaps maps, int kmax,
                                                                int stage_words, int n_stages, float* __restrict__ vol) {
   extern __shared__ __align__(128) float smem[];
@@ -159,7 +181,7 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_tma_kernel(BpGeom G, int n_v
   // ---- consumers: thread = one (x, y) column of the tile, TZ voxels along z in registers
   const int ix = T.x0 + (threadIdx.x & (kBpT - 1)), iy = T.y0 + threadIdx.x / kBpT;
   const bool live = ix < G.nx && iy < G.ny;
-  const float xf = (float)ix - G.hx, yf = (float)iy - G.hy, zf = (float)T.z0 - G.hz;
+  const float xf = (float)(threadIdx.x & (kBpT - 1)), yf = (float)(threadIdx.x / kBpT);   // tile-local voxel index
   float acc[TZ];
 #pragma unroll
   for (int m = 0; m < TZ; ++m)     // DFP_FLAG_ACCUMULATE: start from the caller's volume (a slice of the views)
@@ -177,9 +199,9 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_tma_kernel(BpGeom G, int n_v
     bad |= __float_as_uint(hdr[25]) != 0u;
     if (live) {
       const float a02 = hdr[2], a12 = hdr[6], a22 = hdr[10];
-      const float ub = fmaf(hdr[0], xf, fmaf(hdr[1], yf, fmaf(a02, zf, hdr[3])));
-      const float vb = fmaf(hdr[4], xf, fmaf(hdr[5], yf, fmaf(a12, zf, hdr[7])));
-      const float wb = fmaf(hdr[8], xf, fmaf(hdr[9], yf, fmaf(a22, zf, hdr[11])));
+      const float ub = fmaf(hdr[0], xf, fmaf(hdr[1], yf, hdr[3]));
+      const float vb = fmaf(hdr[4], xf, fmaf(hdr[5], yf, hdr[7]));
+      const float wb = fmaf(hdr[8], xf, fmaf(hdr[9], yf, hdr[11]));
       const float2 ab2 = make_float2(a02, a12), uvb = make_float2(ub, vb);
 #pragma unroll
       for (int m = 0; m < TZ; ++m) {
@@ -221,11 +243,12 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_tma_kernel(BpGeom G, int n_v
 // warp's sums are shuffled together; the 8 warps' results wait in shared memory (two buffers of kBpGradGroup views)
 // and are added in fixed order once per group -> partials[tile][view][6]: one consumer barrier per group, not per view.
 constexpr int kBpGradGroup = 8;                  // views per cross-warp reduction
+constexpr float kFaceEpsBp = 2e-5f;              // |fraction - {0,1}| below this: the fp32 pixel-cell decision is not trusted
 
 // MODE 1 (DFP_FLAG_GRAD_INTERP): exact derivatives of the bilinear interpolant, 4 LDS instead of 12.
 template <int WEIGHT, int DW, int TZ, int MODE>
 __global__ void __launch_bounds__(kBpTmaThreads) bp_grad_tma_kernel(BpGeom G, int n_views,
-                                                                    const BpView* __restrict__ views,
+                                                                    const BpViewD* __restrict__ views,
                                                                     const __grid_constant__ PatchMaps maps, int kmax,
                                                                     int stage_words, int n_stages,
                                                                     const float* __restrict__ upstream,
@@ -260,8 +283,10 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_grad_tma_kernel(BpGeom G, in
   // ---- consumers
   const int ix = T.x0 + (threadIdx.x & (kBpT - 1)), iy = T.y0 + threadIdx.x / kBpT;
   const bool live = ix < G.nx && iy < G.ny;
-  const float xf = (float)ix - G.hx, yf = (float)iy - G.hy, zf = (float)T.z0 - G.hz;
-  const float rx = G.cx + xf * G.vx, ry = G.cy + yf * G.vy, rz = G.cz + zf * G.vz;   // object-frame mm, first voxel
+  const float xf = (float)(threadIdx.x & (kBpT - 1)), yf = (float)(threadIdx.x / kBpT);   // tile-local voxel index
+  // object-frame mm of the column's first voxel
+  const float rx = G.cx + ((float)ix - G.hx) * G.vx, ry = G.cy + ((float)iy - G.hy) * G.vy,
+              rz = G.cz + ((float)T.z0 - G.hz) * G.vz;
   const float* wcol = upstream + ((size_t)T.z0 * G.ny + (live ? iy : 0)) * G.nx + (live ? ix : 0);
   const size_t wstride = (size_t)G.ny * G.nx;
   const size_t tile = ((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
@@ -285,9 +310,9 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_grad_tma_kernel(BpGeom G, in
       float sm[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
       if (live) {
         const float a02 = hdr[2], a12 = hdr[6], a22 = hdr[10];
-        const float ub = fmaf(hdr[0], xf, fmaf(hdr[1], yf, fmaf(a02, zf, hdr[3])));
-        const float vb = fmaf(hdr[4], xf, fmaf(hdr[5], yf, fmaf(a12, zf, hdr[7])));
-        const float wb = fmaf(hdr[8], xf, fmaf(hdr[9], yf, fmaf(a22, zf, hdr[11])));
+        const float ub = fmaf(hdr[0], xf, fmaf(hdr[1], yf, hdr[3]));
+        const float vb = fmaf(hdr[4], xf, fmaf(hdr[5], yf, hdr[7]));
+        const float wb = fmaf(hdr[8], xf, fmaf(hdr[9], yf, hdr[11]));
         const float j00 = hdr[12], j01 = hdr[13], j02 = hdr[14], j10 = hdr[15], j11 = hdr[16], j12 = hdr[17],
                     j20 = hdr[18], j21 = hdr[19], j22 = hdr[20];
         // packed fp32x2 arithmetic on (u, v) / row / column pairs (FFMA2, FADD2, FMUL2: the scalar code's roundings)
@@ -303,13 +328,25 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_grad_tma_kernel(BpGeom G, in
             const float2 uvq = __fmul2_rn(__ffma2_rn(make_float2(mf, mf), ab2, uvb), make_float2(rw, rw));
             const float2 t2 = __fadd2_rn(uvq, make_float2(kMagic, kMagic));
             const float2 fr = __fadd2_rn(sub2(uvq, __fadd2_rn(t2, make_float2(-kMagic, -kMagic))), make_float2(0.5f, 0.5f));
-            const unsigned a0 = 4u * (unsigned)__float_as_int(t2.x) + BU * (unsigned)__float_as_int(t2.y) + c0;
+            unsigned a0 = 4u * (unsigned)__float_as_int(t2.x) + BU * (unsigned)__float_as_int(t2.y) + c0;
 #ifdef DFP_CHECK_BOUNDS
             if (a0 < chk_lo || a0 > chk_hi) s2 = __int_as_float(0x7fc00000);
 #endif
-            const float pa = fr.x, pb = fr.y;
+            float pa = fr.x, pb = fr.y;
             float dlu, dlv, l00, l01, l10, l11;
             if (MODE == 1) {
+              // the derivative of the bilinear interpolant jumps at pixel boundaries: a voxel that projects within
+              // fp32 rounding of one takes its cell and fractions from the fp64 rows, as the oracle does
+              if (fminf(fminf(pa, 1.f - pa), fminf(pb, 1.f - pb)) < kFaceEpsBp) {
+                const double* Ad = reinterpret_cast<const double*>(hdr + 32);
+                const double lx = (double)xf, ly = (double)yf, lz = (double)m;
+                const double wd = fma(Ad[8], lx, fma(Ad[9], ly, fma(Ad[10], lz, Ad[11])));
+                const double ud = fma(Ad[0], lx, fma(Ad[1], ly, fma(Ad[2], lz, Ad[3]))) / wd + 0.5;
+                const double vd = fma(Ad[4], lx, fma(Ad[5], ly, fma(Ad[6], lz, Ad[7]))) / wd + 0.5;
+                const double fu = floor(ud), fv = floor(vd);
+                pa = (float)(ud - fu); pb = (float)(vd - fv);
+                a0 = smem_addr + 4u * (unsigned)(s * stage_words + kPatchHeader) + 4u * (unsigned)(int)fu + BU * (unsigned)(int)fv;
+              }
               const unsigned a1 = a0 + BU;
               l00 = lds_f32<0>(a0); l01 = lds_f32<4>(a0); l10 = lds_f32<0>(a1); l11 = lds_f32<4>(a1);
               dlu = lerp(pb, l01 - l00, l11 - l10);

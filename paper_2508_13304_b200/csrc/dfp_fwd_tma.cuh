@@ -82,7 +82,10 @@ constexpr int kBoxAlignLoss = 3;                       // x cells lost to the 16
 // the blocks resident at one time then cover a few dozen neighbouring tiles of a few neighbouring views, whose frusta
 // overlap in the volume - a 512^3 volume (4x the L2) is then pulled from HBM about once per group instead of once
 // per view.
-constexpr int kViewGroup = 8;
+#ifndef DFP_VIEW_GROUP
+#define DFP_VIEW_GROUP 8
+#endif
+constexpr int kViewGroup = DFP_VIEW_GROUP;
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 

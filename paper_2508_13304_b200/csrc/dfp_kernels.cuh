@@ -555,6 +555,7 @@ __global__ void __launch_bounds__(kBpThreads) bp_kernel(BpGeom G, int n_views, c
 template <int WEIGHT, int DW, int MODE>
 __global__ void __launch_bounds__(kBpThreads) bp_grad_kernel(BpGeom G, int n_views, int zchunk,
                                                              const BpView* __restrict__ views,
+                                                             const BpViewD* __restrict__ viewsd,
                                                              const float4* __restrict__ q,
                                                              const float* __restrict__ upstream,
                                                              float* __restrict__ partials) {
@@ -589,8 +590,23 @@ __global__ void __launch_bounds__(kBpThreads) bp_grad_kernel(BpGeom G, int n_vie
       const float4* img = q + (size_t)view * per;
       float mf = 0.f;
       for (int z = z0; z < z1; ++z) {
-        const BpPix p = bp_locate(fmaf(mf, sv.A[0][2], ub), fmaf(mf, sv.A[1][2], vb), fmaf(mf, sv.A[2][2], wb), ulo,
-                                  uhi, vlo, vhi, pu, C0);
+        BpPix p = bp_locate(fmaf(mf, sv.A[0][2], ub), fmaf(mf, sv.A[1][2], vb), fmaf(mf, sv.A[2][2], wb), ulo,
+                            uhi, vlo, vhi, pu, C0);
+        if (MODE == 1 && fminf(fminf(p.a, 1.f - p.a), fminf(p.b, 1.f - p.b)) < 1e-4f) {
+          // the derivative of the bilinear interpolant jumps at pixel boundaries: a voxel that projects within fp32
+          // rounding of one (|u - c_u| <= n/2 pixels in fp32: up to 3e-5 pixel) takes its cell and fractions from the
+          // fp64 rows, as the oracle does
+          const double* Ad = reinterpret_cast<const double*>(viewsd + view);
+          const double X = (double)xf, Y = (double)yf, Z = (double)zf + (double)mf;
+          const double wd = fma(__ldg(Ad + 8), X, fma(__ldg(Ad + 9), Y, fma(__ldg(Ad + 10), Z, __ldg(Ad + 11))));
+          double ud = fma(__ldg(Ad + 0), X, fma(__ldg(Ad + 1), Y, fma(__ldg(Ad + 2), Z, __ldg(Ad + 3)))) / wd;
+          double vd = fma(__ldg(Ad + 4), X, fma(__ldg(Ad + 5), Y, fma(__ldg(Ad + 6), Z, __ldg(Ad + 7)))) / wd;
+          ud = fmin(fmax(ud, (double)ulo), (double)uhi) + 0.5;
+          vd = fmin(fmax(vd, (double)vlo), (double)vhi) + 0.5;
+          const double fu = floor(ud), fv = floor(vd);
+          p.a = (float)(ud - fu); p.b = (float)(vd - fv);
+          p.idx = (unsigned)((int)fv + G.CV + kPadDet) * pu + (unsigned)((int)fu + G.CU + kPadDet);
+        }
         const float4* c = img + p.idx;
         float dlu, dlv, b00, b01, b10, b11;            // (x2 for MODE 0) interpolated differences; the 4 pixels of b~
         if (MODE == 1) {

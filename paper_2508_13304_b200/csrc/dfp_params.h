@@ -81,6 +81,14 @@ struct BpView {
   float J[3][3];                 // P_eff rows (centred), spatial part, per mm in the object frame
 };
 
+// The same rows in DOUBLE, for the TMA kernels' producer warp: per (voxel tile, view) it re-bases the rows onto the
+// tile's first voxel and the staged patch's first pixel (fp64) and only then rounds to fp32, so that the consumers'
+// fp32 (u, v) are patch-local numbers (< 100 pixels) with ~3e-6 pixel of error whatever the detector size.
+struct BpViewD {
+  double A[3][4];
+  double J[3][3];
+};
+
 // Final contraction of the back-projection gradient (a8): dL/dt = R S'_q, dL/dgamma_k = (R^T a_k) . S'_c.
 struct BpContract {
   double R[9];
@@ -258,7 +266,7 @@ inline BpGeom make_bp_geom(const dfp_geometry& g) {
 }
 
 inline void make_bp_view(const dfp_geometry& g, const BpGeom& G, const ViewFrame& f, const float* pose, BpView* V,
-                         BpContract* C) {
+                         BpContract* C, BpViewD* VD = nullptr) {
   const Mat3 R = pose_rotation(pose);
   const double t[3] = {pose[0], pose[1], pose[2]};
   // world projection matrix in pixel-index units (Eq.1), principal point's integer part removed:
@@ -285,6 +293,11 @@ inline void make_bp_view(const dfp_geometry& g, const BpGeom& G, const ViewFrame
     V->A[r][2] = (float)(E[r][2] * (double)g.vz);
     V->A[r][3] = (float)(E[r][0] * (double)g.cx + E[r][1] * (double)g.cy + E[r][2] * (double)g.cz + E[r][3]);
     for (int c = 0; c < 3; ++c) V->J[r][c] = (float)E[r][c];
+    if (VD) {
+      VD->A[r][0] = E[r][0] * (double)g.vx; VD->A[r][1] = E[r][1] * (double)g.vy; VD->A[r][2] = E[r][2] * (double)g.vz;
+      VD->A[r][3] = E[r][0] * (double)g.cx + E[r][1] * (double)g.cy + E[r][2] * (double)g.cz + E[r][3];
+      for (int c = 0; c < 3; ++c) VD->J[r][c] = E[r][c];
+    }
   }
   if (C) {
     for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) C->R[i * 3 + j] = R.m[i][j];

@@ -12,7 +12,7 @@ DEG = math.pi / 180.0
 def small_geom(n=24, voxel=1.25, nu=20, nv=18, pix=2.4, sad=120.0, sdd=200.0, **kw) -> W.Geometry:
     """A toy cone-beam scanner with a wide cone (stresses the geometry more than the clinical ones)."""
     return W.Geometry(nx=n, ny=n, nz=n, vx=voxel, vy=voxel, vz=voxel, nu=nu, nv=nv, du=pix, dv=pix,
-                      sad=sad, sdd=sdd, **kw)
+                      sad=sad, sdd=sdd, **kw).f32()
 
 
 def aniso_geom(**kw) -> W.Geometry:
@@ -20,7 +20,7 @@ def aniso_geom(**kw) -> W.Geometry:
     d = dict(nx=22, ny=18, nz=14, vx=1.1, vy=1.4, vz=1.9, nu=21, nv=17, du=2.1, dv=2.7, sad=130.0, sdd=210.0,
              cx=1.5, cy=-2.0, cz=0.7, u0=0.8, v0=-1.3)
     d.update(kw)
-    return W.Geometry(**d)
+    return W.Geometry(**d).f32()
 
 
 def blobs(seed=3, n=3, half=10.0, sig=(2.0, 4.0), amp=(0.01, 0.04)):

@@ -454,7 +454,7 @@ def test_random_geometries_both_paths_agree_and_never_nan(dfp):
         du, dv = (vox.mean() * sdd / sad * rng.uniform(0.3, 2.0) for _ in range(2))
         g = W.Geometry(nx=nx, ny=ny, nz=nz, vx=vox[0], vy=vox[1], vz=vox[2], nu=nu, nv=nv, du=du, dv=dv, sad=sad,
                        sdd=sdd, cx=rng.uniform(-3, 3), cy=rng.uniform(-3, 3), cz=rng.uniform(-3, 3),
-                       u0=rng.uniform(-2, 2), v0=rng.uniform(-2, 2), bp_weight=int(case % 2))
+                       u0=rng.uniform(-2, 2), v0=rng.uniform(-2, 2), bp_weight=int(case % 2)).f32()
         V = int(rng.integers(1, 6))
         angles = f32(rng.uniform(0, 2 * math.pi, V))
         poses = f32(np.concatenate([rng.uniform(-8, 8, (V, 3)), rng.uniform(-0.35, 0.35, (V, 3))], axis=1))

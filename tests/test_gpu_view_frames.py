@@ -248,7 +248,7 @@ def test_random_frames_both_paths_agree_and_never_nan(dfp):
         du, dv = (vox.mean() * sdd / sad * rng.uniform(0.3, 1.5) for _ in range(2))
         g = W.Geometry(nx=nx, ny=ny, nz=nz, vx=vox[0], vy=vox[1], vz=vox[2], nu=nu, nv=nv, du=du, dv=dv, sad=sad,
                        sdd=sdd, cx=rng.uniform(-3, 3), cy=rng.uniform(-3, 3), cz=rng.uniform(-3, 3),
-                       u0=rng.uniform(-2, 2), v0=rng.uniform(-2, 2), bp_weight=int((case // 2) % 2), flags=VF)
+                       u0=rng.uniform(-2, 2), v0=rng.uniform(-2, 2), bp_weight=int((case // 2) % 2), flags=VF).f32()
         V = int(rng.integers(1, 6))
         F = f32(np.stack([_random_frame(rng, g, wild=case % 2 == 1) for _ in range(V)]))
         poses = f32(np.concatenate([rng.uniform(-8, 8, (V, 3)), rng.uniform(-0.35, 0.35, (V, 3))], axis=1))

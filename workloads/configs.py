@@ -136,7 +136,7 @@ def make_config(index: int, scale: float = 1.0, n_views: Optional[int] = None) -
     du = c["pix"] * c["nu"] / nu
     dv = c["pix"] * c["nv"] / nv
     geom = Geometry(nx=n, ny=n, nz=n, vx=voxel, vy=voxel, vz=voxel, nu=nu, nv=nv, du=du, dv=dv,
-                    sad=c["sad"], sdd=c["sdd"], bp_weight=1 if index == 3 else 0)
+                    sad=c["sad"], sdd=c["sdd"], bp_weight=1 if index == 3 else 0).f32()
     half = 0.5 * c["n"] * c["voxel"]
     # 1) phantom (always drawn at full-resolution margins so every scale shows the same object)
     ells = random_ellipsoids(rng, c["n_ell"], c["semi"], c["dens"], half, 2.0 * c["voxel"])

@@ -35,6 +35,14 @@ class Geometry:
     def replace(self, **kw) -> "Geometry":
         return dataclasses.replace(self, **kw)
 
+    def f32(self) -> "Geometry":
+        """The same scanner with every real number rounded to float32 - the precision of `dfp_geometry` (the C ABI takes
+        fp32).  Workloads are emitted this way so that the oracle (fp64 fields) and the CUDA path see the SAME numbers:
+        a pitch such as 0.388 mm otherwise differs by 3e-8 relative between the two, which moves a ray by ~1e-5 voxel."""
+        import numpy as np
+        kw = {f.name: float(np.float32(getattr(self, f.name))) for f in dataclasses.fields(self) if f.type is float}
+        return dataclasses.replace(self, **kw)
+
     def as_dict(self) -> dict:
         return dataclasses.asdict(self)
 
