@@ -334,6 +334,7 @@ def main():
             c = dict(job.calls(g.replace(flags=g.flags | flag)))
             ms = job.time_calls([c["forward"], c["forward_pose_grad"]], reps)
             extra[f"{name}_mode_ms_per_call"] = {"forward": ms[0], "forward_pose_grad": ms[1]}
+        # DFP_FLAG_DD: the distance-driven pair, all four calls (back-projector = exact transpose of the forward one)
         # DFP_FLAG_VIEW_FRAMES: the four calls with one explicit (s, c, U, V) frame per view - the config's views on a
         # seeded non-circular (saddle) orbit with detector wobble; same kernels, only the per-view set-up differs
         gv = g.replace(flags=g.flags | dfp.FLAG_VIEW_FRAMES)
@@ -413,10 +414,35 @@ def main():
     if not args.no_extras and world == 1 and args.config == 5 and args.debug_views is None:
         del job.up, job.proj, job.bp_up, job.ws, job.vol, job.bvol
         torch.cuda.empty_cache()
+        # the paper's first task as a loop (PAPER.md :228-235): one view of C2, Adam on NCC, per iteration
+        # dfp_forward_fused_moments + dfp_ncc_pose_grad + a 28-byte read-back (registration.register_view)
+        from paper_2508_13304_b200.registration import register_view
+        wr = W.make_config(2, n_views=1)
+        volr = wr.volume(dev)
+        ar = wr.angles.float().numpy()
+        hidden = wr.data_poses[0].float().numpy()
+        tgt = dfp.forward(wr.geom, ar, hidden[None] * 0.25, volr).clone()          # 5 mm / 2.5 degrees off
+        register_view(wr.geom, ar, volr, tgt, max_iters=5, ncc_stop=2.0, dloss_stop=-1.0)     # warm-up
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        rr = register_view(wr.geom, ar, volr, tgt, max_iters=100, ncc_stop=2.0, dloss_stop=-1.0)
+        dt = time.perf_counter() - t0
+        rs = register_view(wr.geom, ar, volr, tgt, max_iters=300)
+        other["registration_loop_C2"] = {"iterations_per_s": rr["iterations"] / dt, "ms_per_iteration": dt / rr["iterations"] * 1e3,
+                                         "timed_iterations": rr["iterations"], "with_stop_rule": {"iterations": rs["iterations"],
+                                         "ncc": rs["ncc"], "stop": rs["stop"]},
+                                         "what": "256^3 volume, one 512x512 view, Adam on NCC (Eq.25), stop rule of PAPER.md :235"}
+        del volr, tgt
         for idx in (2, 4):
             j2 = Job(dfp, idx, dev)
             seg2, _ = j2.timed(3, 3, flush, barrier)
             other[f"C{idx}"] = dict(rates(j2, seg2), workload=workload_name(j2.w, j2.V))
+            if idx == 2:      # DFP_FLAG_DD: the distance-driven pair, all four calls, on the C2 workload
+                gdd = j2.g.replace(flags=j2.g.flags | dfp.FLAG_DD)
+                j2.ws = torch.empty(max(dfp.workspace_bytes(gdd, j2.V, op) for op in range(4)), dtype=torch.uint8, device=dev)
+                ms = j2.time_calls([fn for _, fn in j2.calls(gdd)], 1)
+                other["C2"]["dd_mode_ms_per_call"] = dict(zip(("forward", "forward_pose_grad", "backproject",
+                                                               "backproject_pose_grad"), ms))
             del j2
             torch.cuda.empty_cache()
 

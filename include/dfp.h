@@ -84,7 +84,14 @@ typedef struct dfp_geometry {
                            the depth from the source along the detector normal in mm; du, dv and sdd are then unused and
                            sad only scales the FDK weight (sad/w')^2.  A frame with U parallel to V or with the source
                            in the detector plane is rejected (DFP_ERR_DIMS).  All kernels and both paths serve it
-                           (the per-view set-up is the only code that differs).                                   */
+                           (the per-view set-up is the only code that differs);
+                           bit7 (DFP_FLAG_DD): all four calls use the DISTANCE-DRIVEN weights (PAPER.md :213, ref [44]) - per
+                           view a driving axis, per plane of voxel centres the pixel's boundaries projected from the source,
+                           a^ij = slab path length x normalised overlap of the pixel's footprint with the voxel's cell along
+                           the two in-plane axes (U14).  dfp_backproject is then the EXACT transpose of dfp_forward
+                           (a matched pair, Eq.21), dfp_forward_pose_grad takes G_f^j per voxel and dfp_backproject_pose_grad
+                           G_b^i per detector pixel (Eq.19-22).  bp_weight must be 0; not combinable with bits 2, 3, 5 or
+                           dfp_forward_fused_moments (DFP_ERR_DIMS); step_mm is unused.                            */
 } dfp_geometry;
 
 enum {
@@ -97,9 +104,9 @@ enum {
   DFP_ERR_CUDA = -6        /* CUDA runtime error (no device, launch failure, out of memory in *_host)       */
 };
 enum { DFP_OP_FORWARD = 0, DFP_OP_FORWARD_POSE_GRAD = 1, DFP_OP_BACKPROJECT = 2, DFP_OP_BACKPROJECT_POSE_GRAD = 3,
-       DFP_OP_FORWARD_FUSED = 4 };
+       DFP_OP_FORWARD_FUSED = 4, DFP_OP_NCC = 5 };
 enum { DFP_FLAG_DW = 1, DFP_FLAG_NO_TMA = 2, DFP_FLAG_GRAD_INTERP = 4, DFP_FLAG_SIDDON = 8,
-       DFP_FLAG_ACCUMULATE = 16, DFP_FLAG_JOSEPH = 32, DFP_FLAG_VIEW_FRAMES = 64 };
+       DFP_FLAG_ACCUMULATE = 16, DFP_FLAG_JOSEPH = 32, DFP_FLAG_VIEW_FRAMES = 64, DFP_FLAG_DD = 128 };
 
 /* Forward projection, Eq.2a :67-69 discretised as Eq.18 :172-177 with a fixed-step, zero-extended
  * trilinear ray-march (U1): proj[v][iv][iu] = D * sum_k f~(R_v^T (s_v + (k+1/2) D e_i - t_v)).
@@ -142,6 +149,18 @@ int dfp_backproject_pose_grad(const dfp_geometry* geometry, int n_views, const f
 int dfp_forward_fused_moments(const dfp_geometry* geometry, int n_views, const float* angles, const float* poses,
                               const float* d_vol, const float* d_target, float* d_proj, float* d_moments, void* d_ws,
                               size_t ws_bytes, void* stream);
+
+/* The loss of the paper's 2D/3D registration task on the device (Eq.25 :230-235; an extension beyond the four
+ * operations): for every view the normalised cross-correlation NCC(l_v, b_v) of its projection
+ * with its measured image, and dNCC/dtheta_v = alpha m[v][0] + beta m[v][1] + gamma m[v][2] from the moments of
+ * dfp_forward_fused_moments (alpha, beta, gamma: the coefficients of dNCC/dl_i = alpha + beta l_i + gamma b_i) - so that
+ * an iteration of the registration loop is two asynchronous calls on one stream and one 28-byte read-back.
+ * d_proj, d_target: device [n_views][nv][nu]; d_moments: device [n_views][3][6]; d_ncc: device, out, [n_views];
+ * d_grad: device, out, [n_views][6], laid out like the output of dfp_forward_pose_grad.  Sums in fp64, fixed order.
+ * A view whose projection or target is constant gets NCC 0 and a zero gradient.  Workspace:
+ * dfp_workspace_bytes(geometry, n_views, DFP_OP_NCC).  Same ownership, asynchrony and error behaviour as above. */
+int dfp_ncc_pose_grad(const dfp_geometry* geometry, int n_views, const float* d_proj, const float* d_target,
+                      const float* d_moments, float* d_ncc, float* d_grad, void* d_ws, size_t ws_bytes, void* stream);
 
 /* Bytes of device workspace the op needs for this geometry and view count (0 on invalid arguments).
  * View chunking: any n_views may be passed to the calls above; to bound the workspace (and the size of

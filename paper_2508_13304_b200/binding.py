@@ -14,13 +14,14 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libdfp.so")
 
-OP_FORWARD, OP_FORWARD_POSE_GRAD, OP_BACKPROJECT, OP_BACKPROJECT_POSE_GRAD, OP_FORWARD_FUSED = 0, 1, 2, 3, 4
+OP_FORWARD, OP_FORWARD_POSE_GRAD, OP_BACKPROJECT, OP_BACKPROJECT_POSE_GRAD, OP_FORWARD_FUSED, OP_NCC = 0, 1, 2, 3, 4, 5
 FLAG_DW = 1
 FLAG_NO_TMA = 2
 FLAG_GRAD_INTERP = 4
 FLAG_SIDDON = 8
 FLAG_ACCUMULATE = 16
 FLAG_JOSEPH = 32
+FLAG_DD = 128              # distance-driven weights in all four calls (include/dfp.h)
 FLAG_VIEW_FRAMES = 64      # `angles` arguments hold [V,12] explicit view frames (s, c, U, V), include/dfp.h
 PATH_GATHER, PATH_TMA = 0, 1
 
@@ -72,6 +73,8 @@ def _load():
     lib.dfp_backproject_pose_grad.argtypes = devg
     lib.dfp_forward_fused_moments.argtypes = [gp, ci, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.dfp_forward_fused_moments.restype = ci
+    lib.dfp_ncc_pose_grad.argtypes = [gp, ci, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.dfp_ncc_pose_grad.restype = ci
     lib.dfp_forward_host.argtypes = [gp, ci, vp, vp, vp, vp, vp]
     lib.dfp_backproject_host.argtypes = [gp, ci, vp, vp, vp, vp, vp]
     lib.dfp_forward_pose_grad_host.argtypes = [gp, ci, vp, vp, vp, vp, vp, vp]
@@ -231,6 +234,22 @@ def forward_fused_moments(geom, angles, poses, vol, target, out_proj=None, out_m
                                               _dev(out_proj, (V, g.nv, g.nu), "proj"),
                                               _dev(out_moments, (V, 3, 6), "moments"), wp, wn, _stream(vol)))
     return out_proj, out_moments
+
+
+def ncc_pose_grad(geom, proj, target, moments, out_ncc=None, out_grad=None, ws=None):
+    """dfp_ncc_pose_grad: NCC(l_v, b_v) [V] and dNCC/dtheta_v [V,6] from the outputs of forward_fused_moments."""
+    g = Geometry.of(geom)
+    V = int(proj.shape[0])
+    if out_ncc is None:
+        out_ncc = torch.empty((V,), dtype=torch.float32, device=proj.device)
+    if out_grad is None:
+        out_grad = torch.empty((V, 6), dtype=torch.float32, device=proj.device)
+    ws, wp, wn = _workspace(g, V, OP_NCC, ws, proj.device)
+    with _same_device(proj, target, moments, out_ncc, out_grad, ws):
+        _check(_lib.dfp_ncc_pose_grad(ctypes.byref(g), V, _dev(proj, (V, g.nv, g.nu), "proj"),
+                                      _dev(target, (V, g.nv, g.nu), "target"), _dev(moments, (V, 3, 6), "moments"),
+                                      _dev(out_ncc, (V,), "ncc"), _dev(out_grad, (V, 6), "grad"), wp, wn, _stream(proj)))
+    return out_ncc, out_grad
 
 
 def backproject(geom, angles, poses, proj, out=None, ws=None):

@@ -14,7 +14,9 @@
 #include "dfp_fwd_tma.cuh"
 #include "dfp_kernels.cuh"
 #include "dfp_params.h"
+#include "dfp_dd.cuh"
 #include "dfp_joseph.cuh"
+#include "dfp_loss.cuh"
 #include "dfp_siddon.cuh"
 
 namespace {
@@ -292,6 +294,8 @@ cudaError_t ensure_smem_attributes() {
   DFP_ATTR((fwd_tma_kernel<0, 0>), tma_smem_bytes<0>());
   DFP_ATTR((fwd_tma_kernel<0, 1>), tma_smem_bytes<1>());
   DFP_ATTR((fwd_tma_kernel<0, 2>), tma_smem_bytes<2>());
+  DFP_ATTR((fwd_tma_kernel<0, 4>), tma_smem_bytes<4>());
+  DFP_ATTR((fwd_tma_kernel<0, 5>), tma_smem_bytes<5>());
   DFP_ATTR((fwd_tma_kernel<1, 2>), tma_smem_bytes<2>());
   DFP_ATTR((fwd_tma_kernel<1, 3>), tma_smem_bytes<3>());
   DFP_ATTR((fwd_tma_kernel<2, 2>), tma_smem_bytes<2>());
@@ -318,7 +322,7 @@ cudaError_t ensure_smem_attributes() {
 
 // ---- workspace carving ---------------------------------------------------------------------------
 struct FwdWs {
-  size_t off_views, off_con, off_pvol, off_part, total;
+  size_t off_views, off_dd, off_con, off_pvol, off_part, total;
   int gx, gy;     // blocks per view (16 x 16-pixel tiles)
   int gy8;        // rows of 16 x 8-pixel tiles (TMA gradient kernel)
 };
@@ -330,6 +334,7 @@ FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad, int nset = 1) {
   w.gy8 = (g.nv + TmaLanes<1>::TV - 1) / TmaLanes<1>::TV;
   size_t o = 0;
   w.off_views = o; o += align_up(sizeof(FwdView) * (size_t)V);
+  w.off_dd = o;    o += (g.flags & DFP_FLAG_DD) ? align_up(sizeof(DdView) * (size_t)V) : 0;
   w.off_con = o;   o += grad ? align_up(sizeof(FwdContract) * (size_t)V) : 0;
   w.off_pvol = o;  o += align_up(sizeof(float4) * (size_t)L.px * L.py * L.pz);
   w.off_part = o;  o += grad ? align_up(sizeof(float) * 6 * (size_t)nset * V * w.gx * w.gy8) : 0;
@@ -339,7 +344,7 @@ FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad, int nset = 1) {
 
 constexpr int kBpGradZChunk = 16;
 struct BpWs {
-  size_t off_views, off_viewsd, off_con, off_q, off_part, total;
+  size_t off_views, off_viewsd, off_dd, off_con, off_q, off_part, total;
   int gx, gy, gz;  // voxel tiles (gather path)
   int tx, ty, tz;  // voxel tiles (TMA path)
 };
@@ -355,12 +360,15 @@ BpWs bp_ws(const dfp_geometry& g, int V, bool grad) {
   size_t o = 0;
   w.off_views = o; o += align_up(sizeof(BpView) * (size_t)V);
   w.off_viewsd = o; o += align_up(sizeof(BpViewD) * (size_t)V);
+  w.off_dd = o;    o += (g.flags & DFP_FLAG_DD) ? align_up(sizeof(DdView) * (size_t)V) : 0;
   w.off_con = o;   o += grad ? align_up(sizeof(BpContract) * (size_t)V) : 0;
   w.off_q = o;     o += align_up(sizeof(float4) * (size_t)V * (g.nu + 2 * kPadDet) * (g.nv + 2 * kPadDet));
   w.off_part = o;
   {
     const size_t t_gather = (size_t)w.gx * w.gy * w.gz, t_tma = (size_t)w.tx * w.ty * w.tz;
-    o += grad ? align_up(sizeof(float) * 6 * (size_t)V * (t_gather > t_tma ? t_gather : t_tma)) : 0;
+    size_t tiles = t_gather > t_tma ? t_gather : t_tma;
+    if (g.flags & DFP_FLAG_DD) tiles = ((size_t)g.nx * g.ny * g.nz + kDdBpThreads - 1) / kDdBpThreads;   // dd_bp_kernel blocks
+    o += grad ? align_up(sizeof(float) * 6 * (size_t)V * tiles) : 0;
   }
   w.total = o;
   return w;
@@ -395,9 +403,11 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
   const bool grad = op != DFP_OP_FORWARD, fused = op == DFP_OP_FORWARD_FUSED;
   if (fused && (!d_proj || !aligned(d_proj, 16))) return d_proj ? DFP_ERR_ALIGN : DFP_ERR_NULL;
   if (fused && (g->flags & DFP_FLAG_GRAD_INTERP)) return DFP_ERR_DIMS;      // fused moments: central differences only
-  const bool siddon = (g->flags & DFP_FLAG_SIDDON) != 0, joseph = (g->flags & DFP_FLAG_JOSEPH) != 0;
-  // Siddon / Joseph weights: the two plain calls only, one model at a time
-  if ((siddon || joseph) && (fused || (g->flags & DFP_FLAG_GRAD_INTERP) || (siddon && joseph))) return DFP_ERR_DIMS;
+  const bool siddon = (g->flags & DFP_FLAG_SIDDON) != 0, joseph = (g->flags & DFP_FLAG_JOSEPH) != 0,
+             dd = (g->flags & DFP_FLAG_DD) != 0;
+  // Siddon / Joseph / distance-driven weights: the two plain calls only, one model at a time
+  if ((siddon || joseph || dd) && (fused || (g->flags & DFP_FLAG_GRAD_INTERP) || (int)siddon + (int)joseph + (int)dd > 1))
+    return DFP_ERR_DIMS;
   const int nset = fused ? 3 : 1;
   const FwdWs w = fwd_ws(*g, V, grad, nset);
   st = check_common(g, V, angles, poses, d_vol, d_out, grad ? (const void*)d_up : (const void*)d_vol, d_ws,
@@ -421,6 +431,30 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
   DFP_CUDA(upload_async(dv, hv.data(), sizeof(FwdView) * V, s), "view upload");
   if (grad) DFP_CUDA(upload_async(dc, hc.data(), sizeof(FwdContract) * V, s), "view upload");
   const dim3 grid(w.gx, w.gy, V);
+  if (dd) {                 // distance-driven weights (dfp_dd.cuh)
+    std::vector<DdView> hd((size_t)V);
+    for (int v = 0; v < V; ++v) make_dd_view(*g, hf[v], poses + 6 * v, &hd[v]);
+    DdView* ddv = reinterpret_cast<DdView*>(base + w.off_dd);
+    DFP_CUDA(upload_async(ddv, hd.data(), sizeof(DdView) * V, s), "view upload");
+    const DdGeom DG = make_dd_geom(*g);
+    const GradBricks GB = GradBricks::make(g->nx, g->ny, g->nz);
+    g_path = DFP_PATH_GATHER;
+    time_begin(s);
+    if (!grad) {
+      dd_fwd_kernel<0><<<grid, kFwdThreads, 0, s>>>(DG, ddv, d_vol, nullptr, GB, nullptr, d_out);
+      time_end(s);
+      g_launches = 1;
+    } else {
+      const int gb = (int)std::min<size_t>((GB.cells() + 255) / 256, (size_t)148 * 64);
+      grad_volume_kernel<<<gb, 256, 0, s>>>(GB, G.sgx, G.sgy, G.sgz, d_vol, pvol);
+      dd_fwd_kernel<1><<<grid, kFwdThreads, 0, s>>>(DG, ddv, d_vol, pvol, GB, d_up, part);
+      time_end(s);
+      fwd_contract_kernel<<<V, 256, 0, s>>>(w.gx * w.gy, part, dc, d_out);
+      g_launches = 3;
+    }
+    DFP_CUDA(cudaGetLastError(), "forward launch (distance-driven weights)");
+    return DFP_OK;
+  }
   if (siddon || joseph) {   // other weight models (dfp_siddon.cuh, dfp_joseph.cuh): straight over the caller's volume
     g_path = DFP_PATH_GATHER;
     time_begin(s);
@@ -453,11 +487,15 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
   static const int kBoxes[kNumShapes][3] = {{BoxShape<0>::X, BoxShape<0>::Y, BoxShape<0>::Z},
                                             {BoxShape<1>::X, BoxShape<1>::Y, BoxShape<1>::Z},
                                             {BoxShape<2>::X, BoxShape<2>::Y, BoxShape<2>::Z},
-                                            {BoxShape<3>::X, BoxShape<3>::Y, BoxShape<3>::Z}};
-  // forward: shapes 0, 1, 2 (16 x 16-pixel tiles); gradient: shapes 3, 2 (16 x 8-pixel tiles)
-  static const int kOrderFwd[3] = {0, 1, 2}, kOrderGrad[2] = {3, 2};
-  const int* order = grad ? kOrderGrad : kOrderFwd;
-  const int n_order = grad ? 2 : 3;
+                                            {BoxShape<3>::X, BoxShape<3>::Y, BoxShape<3>::Z},
+                                            {BoxShape<4>::X, BoxShape<4>::Y, BoxShape<4>::Z},
+                                            {BoxShape<5>::X, BoxShape<5>::Y, BoxShape<5>::Z}};
+  // forward: shapes 0, 1, 2 (16 x 16-pixel tiles) - with the odd-extent boxes 4, 5 first where a pixel spans >= 0.45
+  // voxel along z (bank conflicts, dfp_fwd_tma.cuh); gradient: shapes 3, 2 (16 x 8-pixel tiles)
+  static const int kOrderFwd[3] = {0, 1, 2}, kOrderFwdWide[5] = {4, 5, 0, 1, 2}, kOrderGrad[2] = {3, 2};
+  const bool wide = hf[0].vlen * ((double)g->sad / hf[0].sdd) / (double)g->vz >= 0.45;
+  const int* order = grad ? kOrderGrad : (wide ? kOrderFwdWide : kOrderFwd);
+  const int n_order = grad ? 2 : (wide ? 5 : 3);
   const int TU = grad ? TmaLanes<1>::TU : TmaLanes<0>::TU, TV = grad ? TmaLanes<1>::TV : TmaLanes<0>::TV;
   int shape = -1;
   if (!(g->flags & DFP_FLAG_NO_TMA) && (g->nx % 4) == 0) {
@@ -491,6 +529,10 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
       fwd_tma_kernel<0, 0><<<nbf, TmaLanes<0>::THREADS, tma_smem_bytes<0>(), s>>>(G, Qf, dv, vol_map, nullptr, d_out, nullptr);
     else if (shape == 1)
       fwd_tma_kernel<0, 1><<<nbf, TmaLanes<0>::THREADS, tma_smem_bytes<1>(), s>>>(G, Qf, dv, vol_map, nullptr, d_out, nullptr);
+    else if (shape == 4)
+      fwd_tma_kernel<0, 4><<<nbf, TmaLanes<0>::THREADS, tma_smem_bytes<4>(), s>>>(G, Qf, dv, vol_map, nullptr, d_out, nullptr);
+    else if (shape == 5)
+      fwd_tma_kernel<0, 5><<<nbf, TmaLanes<0>::THREADS, tma_smem_bytes<5>(), s>>>(G, Qf, dv, vol_map, nullptr, d_out, nullptr);
     else
       fwd_tma_kernel<0, 2><<<nbf, TmaLanes<0>::THREADS, tma_smem_bytes<2>(), s>>>(G, Qf, dv, vol_map, nullptr, d_out, nullptr);
     time_end(s);
@@ -542,6 +584,8 @@ int run_backproject_slice(const dfp_geometry* g, int V, const float* angles, con
   if (!g) return DFP_ERR_NULL;
   int st = validate_geometry(g);
   if (st) return st;
+  if ((g->flags & DFP_FLAG_DD) && (g->bp_weight != 0 || (g->flags & (DFP_FLAG_GRAD_INTERP | DFP_FLAG_SIDDON | DFP_FLAG_JOSEPH))))
+    return DFP_ERR_DIMS;     // the DD back-projector is the plain transpose: unit weight, central differences only
   const BpWs w = bp_ws(*g, V, grad);
   st = check_common(g, V, angles, poses, d_proj, d_out, grad ? (const void*)d_up : (const void*)d_proj, d_ws,
                         ws_bytes, w.total);
@@ -563,6 +607,27 @@ int run_backproject_slice(const dfp_geometry* g, int V, const float* angles, con
   DFP_CUDA(upload_async(dv, hv.data(), sizeof(BpView) * V, s), "view upload");
   DFP_CUDA(upload_async(dvd, hvd.data(), sizeof(BpViewD) * V, s), "view upload");
   if (grad) DFP_CUDA(upload_async(dc, hc.data(), sizeof(BpContract) * V, s), "view upload");
+  if (g->flags & DFP_FLAG_DD) {   // distance-driven weights (dfp_dd.cuh): the exact transpose of the DD forward projector
+    std::vector<DdView> hd((size_t)V);
+    for (int v = 0; v < V; ++v) make_dd_view(*g, make_frame(*g, angles, v), poses + 6 * v, &hd[v]);
+    DdView* ddv = reinterpret_cast<DdView*>(base + w.off_dd);
+    DFP_CUDA(upload_async(ddv, hd.data(), sizeof(DdView) * V, s), "view upload");
+    const DdGeom DG = make_dd_geom(*g);
+    const unsigned nblk = (unsigned)(((size_t)g->nx * g->ny * g->nz + kDdBpThreads - 1) / kDdBpThreads);
+    time_begin(s);
+    if (!grad) {
+      dd_bp_kernel<0><<<nblk, kDdBpThreads, 0, s>>>(DG, V, (g->flags & DFP_FLAG_ACCUMULATE) ? 1 : 0, ddv, dv, d_proj, nullptr, d_out);
+      time_end(s);
+      g_launches = 1;
+    } else {
+      dd_bp_kernel<1><<<nblk, kDdBpThreads, 0, s>>>(DG, V, 0, ddv, dv, d_proj, d_up, part);
+      time_end(s);
+      bp_contract_kernel<<<V, 256, 0, s>>>((int)nblk, V, part, dc, d_out);
+      g_launches = 2;
+    }
+    DFP_CUDA(cudaGetLastError(), "back-projection launch (distance-driven weights)");
+    return DFP_OK;
+  }
   // TMA-staged path: projections admit a tensor map, every voxel in front of the source, patches fit the menu
   int kmax = -1, TZ = 16;
   if (!(g->flags & DFP_FLAG_NO_TMA) && (g->nu % 4) == 0) {
@@ -857,6 +922,27 @@ int dfp_backproject_pose_grad(const dfp_geometry* g, int n_views, const float* a
                          static_cast<cudaStream_t>(stream), true);
 }
 
+int dfp_ncc_pose_grad(const dfp_geometry* g, int n_views, const float* d_proj, const float* d_target,
+                      const float* d_moments, float* d_ncc, float* d_grad, void* d_ws, size_t ws_bytes, void* stream) {
+  int st = validate_geometry(g);
+  if (st) return st;
+  if (n_views <= 0 || n_views > kMaxViewsPerLaunch) return DFP_ERR_DIMS;
+  if (!d_proj || !d_target || !d_moments || !d_ncc || !d_grad || !d_ws) return DFP_ERR_NULL;
+  if (!aligned(d_proj, 16) || !aligned(d_target, 16) || !aligned(d_moments, 8) || !aligned(d_ncc, 4) || !aligned(d_grad, 8) ||
+      !aligned(d_ws, 256))
+    return DFP_ERR_ALIGN;
+  if (ws_bytes < dfp_workspace_bytes(g, n_views, DFP_OP_NCC)) return DFP_ERR_WORKSPACE;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const size_t npix = (size_t)g->nu * g->nv;
+  const int nblk = (int)std::min<size_t>(kNccBlocks, (npix + 4 * kNccThreads - 1) / (4 * kNccThreads));
+  double* partial = static_cast<double*>(d_ws);
+  ncc_partial_kernel<<<dim3(nblk, n_views), kNccThreads, 0, s>>>(npix, d_proj, d_target, partial);
+  ncc_finish_kernel<<<n_views, 32, 0, s>>>(npix, nblk, partial, d_moments, d_ncc, d_grad);
+  g_launches = 2;
+  DFP_CUDA(cudaGetLastError(), "NCC launch");
+  return DFP_OK;
+}
+
 size_t dfp_workspace_bytes(const dfp_geometry* g, int n_views, int op) {
   if (validate_geometry(g) != DFP_OK || n_views <= 0 || n_views > kMaxViews) return 0;
   switch (op) {
@@ -865,6 +951,7 @@ size_t dfp_workspace_bytes(const dfp_geometry* g, int n_views, int op) {
     case DFP_OP_BACKPROJECT: return bp_ws(*g, n_views, false).total;
     case DFP_OP_BACKPROJECT_POSE_GRAD: return bp_ws(*g, n_views, true).total;
     case DFP_OP_FORWARD_FUSED: return fwd_ws(*g, n_views, true, 3).total;
+    case DFP_OP_NCC: return align_up(sizeof(double) * 5 * (size_t)kNccBlocks * (size_t)n_views);
     default: return 0;
   }
 }

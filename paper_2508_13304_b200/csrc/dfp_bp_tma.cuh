@@ -208,10 +208,16 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_tma_kernel(BpGeom G, int n_v
         if (m < T.tz) {
           // (u, v) as one fp32x2 lane pair: advance along z, perspective divide, floor and fractions
           const float mf = (float)m;
-          const float rw = fast_rcp(fmaf(mf, a22, wb));
-          const float2 uvq = __fmul2_rn(__ffma2_rn(make_float2(mf, mf), ab2, uvb), make_float2(rw, rw));
+          const float wz = fmaf(mf, a22, wb);
+          const float rw = fast_rcp(wz);
+          const float2 uvp = __ffma2_rn(make_float2(mf, mf), ab2, uvb);                 // (u', v')
+          const float2 uvq = __fmul2_rn(uvp, make_float2(rw, rw));
           const float2 t2 = __fadd2_rn(uvq, make_float2(kMagic, kMagic));
-          const float2 fr = __fadd2_rn(sub2(uvq, __fadd2_rn(t2, make_float2(-kMagic, -kMagic))), make_float2(0.5f, 0.5f));
+          // fractions from the residual (u' - rint(u) w') / w': the residual is a small number, so neither the rounding of
+          // the quotient u = u'/w' (|u| up to 100 pixels) nor that of 1/w' reaches the interpolation weights
+          const float2 tr = __fadd2_rn(t2, make_float2(-kMagic, -kMagic));
+          const float2 fr = __ffma2_rn(__ffma2_rn(make_float2(-tr.x, -tr.y), make_float2(wz, wz), uvp), make_float2(rw, rw),
+                                       make_float2(0.5f, 0.5f));
           const unsigned a0 = 4u * (unsigned)__float_as_int(t2.x) + BU * (unsigned)__float_as_int(t2.y) + c0;
           const unsigned a1 = a0 + BU;
           // the two rows as a pair: lerp along u on both, then along v
@@ -324,10 +330,16 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_grad_tma_kernel(BpGeom G, in
         for (int m = 0; m < TZ; ++m) {
           if (m < T.tz) {
             const float mf = (float)m;
-            const float rw = fast_rcp(fmaf(mf, a22, wb));
-            const float2 uvq = __fmul2_rn(__ffma2_rn(make_float2(mf, mf), ab2, uvb), make_float2(rw, rw));
+            const float wz = fmaf(mf, a22, wb);
+            const float rw = fast_rcp(wz);
+            const float2 uvp = __ffma2_rn(make_float2(mf, mf), ab2, uvb);                 // (u', v')
+            const float2 uvq = __fmul2_rn(uvp, make_float2(rw, rw));
             const float2 t2 = __fadd2_rn(uvq, make_float2(kMagic, kMagic));
-            const float2 fr = __fadd2_rn(sub2(uvq, __fadd2_rn(t2, make_float2(-kMagic, -kMagic))), make_float2(0.5f, 0.5f));
+            // fractions from the residual (u' - rint(u) w') / w': the residual is a small number, so neither the rounding of
+            // the quotient u = u'/w' (|u| up to 100 pixels) nor that of 1/w' reaches the interpolation weights
+            const float2 tr = __fadd2_rn(t2, make_float2(-kMagic, -kMagic));
+            const float2 fr = __ffma2_rn(__ffma2_rn(make_float2(-tr.x, -tr.y), make_float2(wz, wz), uvp), make_float2(rw, rw),
+                                         make_float2(0.5f, 0.5f));
             unsigned a0 = 4u * (unsigned)__float_as_int(t2.x) + BU * (unsigned)__float_as_int(t2.y) + c0;
 #ifdef DFP_CHECK_BOUNDS
             if (a0 < chk_lo || a0 > chk_hi) s2 = __int_as_float(0x7fc00000);

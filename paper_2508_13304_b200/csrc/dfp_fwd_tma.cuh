@@ -44,11 +44,28 @@ template <int SHAPE> struct BoxShape;
 template <> struct BoxShape<0> { static constexpr int X = 20, Y = 20, Z = 16, STAGES = 2; };
 template <> struct BoxShape<1> { static constexpr int X = 28, Y = 20, Z = 20, STAGES = 2; };
 template <> struct BoxShape<2> { static constexpr int X = 28, Y = 28, Z = 20, STAGES = 1; };
-template <> struct BoxShape<3> { static constexpr int X = 28, Y = 28, Z = 16, STAGES = 1; };   // gradient, 16 x 8 tiles
-constexpr int kNumShapes = 4;
-template <int SHAPE> constexpr int tma_smem_bytes() {
-  return BoxShape<SHAPE>::X * BoxShape<SHAPE>::Y * BoxShape<SHAPE>::Z * 4 * BoxShape<SHAPE>::STAGES;
+#ifndef DFP_GRAD_STAGES
+#define DFP_GRAD_STAGES 1
+#endif
+#ifndef DFP_GRAD_SLOTS
+#define DFP_GRAD_SLOTS 2
+#endif
+#ifndef DFP_GRAD_TV
+#define DFP_GRAD_TV 8
+#endif
+template <> struct BoxShape<3> { static constexpr int X = 28, Y = 28, Z = 16, STAGES = DFP_GRAD_STAGES; };   // gradient, 16 x 8 tiles
+// Forward boxes with an ODD y extent (slab pitch = 12 / 20 mod 32 instead of 16): where a warp's 8 x 4-pixel patch spans
+// three z slices (>= 0.45 voxel per pixel: the 512^3 configs), slab pitch 16 puts slices z and z + 2 on the same banks;
+// 1.76 -> 1.38 wavefronts per load on C5, 1.62 -> 1.36 on C4 (simulated, _and measured_ in DESIGN.md); at C2's 0.39
+// voxel per pixel the even extents are the better ones (1.37 against 1.64).
+template <> struct BoxShape<4> { static constexpr int X = 20, Y = 19, Z = 16, STAGES = 2; };
+template <> struct BoxShape<5> { static constexpr int X = 28, Y = 19, Z = 20, STAGES = 2; };
+constexpr int kNumShapes = 6;
+// words between the stages of a box: the box rounded up to 128 bytes (alignment of a TMA destination)
+template <int SHAPE> __host__ __device__ constexpr int tma_stage_words() {
+  return (BoxShape<SHAPE>::X * BoxShape<SHAPE>::Y * BoxShape<SHAPE>::Z + 31) / 32 * 32;
 }
+template <int SHAPE> constexpr int tma_smem_bytes() { return tma_stage_words<SHAPE>() * 4 * BoxShape<SHAPE>::STAGES; }
 __device__ __forceinline__ float2 sub2(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
 // lerp on two lanes of data at once: v0 + a (v1 - v0), rounded exactly like lerp()
 __device__ __forceinline__ float2 lerp2(float2 a, float2 v0, float2 v1) { return __ffma2_rn(a, sub2(v1, v0), v0); }
@@ -62,8 +79,9 @@ __device__ __forceinline__ float2 lerp2(float2 a, float2 v0, float2 v1) { return
 // voxels as the forward), 3 FUSED projection + central-difference gradient moments in one traversal
 // (dfp_forward_fused_moments).  Gradient kernels: two lanes per ray, 8 x 2-pixel warps, 16 x 8-pixel tile.
 template <int GRAD> struct TmaLanes {
-  static constexpr int SLOTS = GRAD ? 2 : 1, TU = kFwdTU, TV = GRAD ? 8 : kFwdTV, THREADS = TU * TV * SLOTS;
-  static constexpr int PU = 8, PV = 32 / (PU * SLOTS);
+  static constexpr int SLOTS = GRAD ? DFP_GRAD_SLOTS : 1, TU = kFwdTU, TV = GRAD ? DFP_GRAD_TV : kFwdTV, THREADS = TU * TV * SLOTS;
+  static constexpr int PU = SLOTS == 4 ? 4 : 8, PV = 32 / (PU * SLOTS);
+  static constexpr int MINB = THREADS > 256 ? 2 : 4;
 };
 template <int GRAD>
 __device__ __forceinline__ void tma_pixel(int bx, int by, int& iu, int& iv, int& slot) {
@@ -146,7 +164,7 @@ __device__ __forceinline__ void issue_chunk(const VolLayout& L, TmaBlock& B, con
   B.org[s][0] = oc[0]; B.org[s][1] = oc[1]; B.org[s][2] = oc[2];
   const unsigned bar = bar_addr + 8u * s;
   mbar_expect_tx(bar, kWords * 4);
-  tma_load_3d(tiles_addr + (unsigned)(s * kWords * 4), map, oc[0] + L.hx, oc[1] + L.hy, oc[2] + L.hz, bar);
+  tma_load_3d(tiles_addr + (unsigned)(s * tma_stage_words<SHAPE>() * 4), map, oc[0] + L.hx, oc[1] + L.hy, oc[2] + L.hz, bar);
 }
 
 // The chunk loop of one block for one box shape.  acc = {sum} (forward) or {gx,gy,gz,hx,hy,hz[,sum]} (gradient).
@@ -155,7 +173,7 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
                                           TmaBlock& B, const float* tiles, unsigned tiles_addr, unsigned bar_addr,
                                           float* acc) {
   using S = BoxShape<SHAPE>;
-  constexpr int BX = S::X, BXY = S::X * S::Y, kWords = S::X * S::Y * S::Z;
+  constexpr int BX = S::X, BXY = S::X * S::Y, kBox = S::X * S::Y * S::Z, kWords = tma_stage_words<SHAPE>();
   constexpr int SLOTS = TmaLanes<GRAD>::SLOTS;
   if (threadIdx.x == 0) {
     int Kc = 0;
@@ -195,6 +213,14 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
   const int kend = r.k0 + r.n;
   const float dpx = (float)r.dp[0], dpy = (float)r.dp[1], dpz = (float)r.dp[2];
   const float2 dpxy = make_float2(dpx, dpy);
+  // The fp64 ray is touched once per chunk (and in the rare exact-cell path): it is parked in LOCAL memory - an array
+  // read through an index the compiler cannot see through - so that its 12 registers stay free for the sample loop
+  // (with them live the loop lost 10-20 %: fewer loads in flight at the 64-register budget of four blocks per SM).
+  double rd[6];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) { rd[a] = r.pm[a]; rd[3 + a] = r.dp[a]; }
+  int zi;
+  asm volatile("mov.u32 %0, 0;" : "=r"(zi));
 
   float sum = 0.f;
   float gx = 0.f, gy = 0.f, gz = 0.f, hx = 0.f, hy = 0.f, hz = 0.f;
@@ -208,11 +234,14 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
     // re-base the ray onto the box origin (fp64, once per chunk): local position of this lane's first sample
     const int o0 = B.org[s][0], o1 = B.org[s][1], o2 = B.org[s][2];
     const double kd = (double)kfirst;
-    const float2 bxy = make_float2((float)(fma(kd, r.dp[0], r.pm[0]) - (double)o0),
-                                   (float)(fma(kd, r.dp[1], r.pm[1]) - (double)o1));
-    const float bz = (float)(fma(kd, r.dp[2], r.pm[2]) - (double)o2);
+    const float2 bxy = make_float2((float)(fma(kd, rd[zi + 3], rd[zi + 0]) - (double)o0),
+                                   (float)(fma(kd, rd[zi + 4], rd[zi + 1]) - (double)o1));
+    const float bz = (float)(fma(kd, rd[zi + 5], rd[zi + 2]) - (double)o2);
     // word index of local cell (X, Y, Z) in stage s from the magic-rounded floats' bits
-    const unsigned c0 = (unsigned)(s * kWords) - (unsigned)kMagicBits * (unsigned)(1 + BX + BXY);
+    unsigned c0 = (unsigned)(s * kWords) - (unsigned)kMagicBits * (unsigned)(1 + BX + BXY);
+    // keep the constant out of the optimiser's sight: folded into every load's offset it no longer fits the LDS
+    // immediate field and each of the 8 / 32 loads of a sample gets its own address add (measured: +20 % time)
+    asm volatile("" : "+r"(c0));
     float kf = (float)kfirst, jf = 0.f;
     for (int k = kfirst; k < kb; k += SLOTS) {
       // position, floor and fractions: x and y as one fp32x2 lane pair
@@ -231,7 +260,10 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
         if (mn < kFaceEps) {
           int cell[3];
           float fr[3];
-          exact_cell(r, k, cell, fr);
+          Ray rr;
+#pragma unroll
+          for (int a = 0; a < 3; ++a) { rr.pm[a] = rd[zi + a]; rr.dp[a] = rd[zi + 3 + a]; }
+          exact_cell(rr, k, cell, fr);
           idx = (unsigned)(s * kWords + (cell[0] - o0) + BX * (cell[1] - o1) + BXY * (cell[2] - o2));
           ax = fr[0]; ay = fr[1]; az = fr[2];
         }
@@ -241,7 +273,7 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
       {
         const int local = (int)(idx - (unsigned)(s * kWords)), halo = (GRAD == 1 || GRAD == 3) ? 1 : 0;
         const int lo = local - halo * (1 + BX + BXY), hi = local + (1 + halo) * (1 + BX + BXY);
-        if (lo < 0 || hi >= kWords) sum = gx = __int_as_float(0x7fc00000);
+        if (lo < 0 || hi >= kBox) sum = gx = __int_as_float(0x7fc00000);
       }
 #endif
       if (!GRAD) {
@@ -346,7 +378,7 @@ __device__ __forceinline__ void fwd_block(const FwdGrid& Q, int& view, int& bx, 
 }
 
 template <int GRAD, int SHAPE>
-__global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, 4) fwd_tma_kernel(FwdGeom G, FwdGrid Q,
+__global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, TmaLanes<GRAD>::MINB) fwd_tma_kernel(FwdGeom G, FwdGrid Q,
                                                               const FwdView* __restrict__ views,
                                                               const __grid_constant__ CUtensorMap vol_map,
                                                               const float* __restrict__ upstream,

@@ -253,6 +253,47 @@ inline void make_fwd_view(const ViewFrame& f, const float* pose, FwdView* V, Fwd
   }
 }
 
+// One view of the distance-driven kernels (dfp_dd.cuh), object frame, mm, fp64: source, detector point of pixel index
+// (0, 0), displacement of one pixel step along u and v; P maps an object-frame point to pixel indices,
+// (u', v', w') = P (r'; 1), u = u'/w' (Eq.1 with the pose folded in; used to find the pixels a voxel cell can meet);
+// a = driving axis of the view, ub / vb = the in-plane axes paired with the detector's u / v.
+struct DdView {
+  double so[3], X00[3], Uo[3], Vo[3];
+  double P[3][4];
+  int a, ub, vb, pad;
+};
+inline void make_dd_view(const dfp_geometry& g, const ViewFrame& f, const float* pose, DdView* D) {
+  const Mat3 R = pose_rotation(pose);
+  const double t[3] = {pose[0], pose[1], pose[2]};
+  double sw[3], x00[3];
+  for (int a = 0; a < 3; ++a) {
+    sw[a] = f.s[a] - t[a];
+    x00[a] = f.dc[a] - f.cu * f.U[a] - f.cv * f.V[a] - t[a];
+  }
+  mulT(R, sw, D->so);
+  mulT(R, x00, D->X00);
+  mulT(R, f.U, D->Uo);
+  mulT(R, f.V, D->Vo);
+  double n[3];
+  for (int a = 0; a < 3; ++a)
+    n[a] = D->X00[a] + 0.5 * (g.nu - 1) * D->Uo[a] + 0.5 * (g.nv - 1) * D->Vo[a] - D->so[a];
+  int a = 0;
+  for (int k = 1; k < 3; ++k) if (std::fabs(n[k]) > std::fabs(n[a])) a = k;
+  const int b = (a + 1) % 3, d = (a + 2) % 3;
+  const bool u_is_b = std::fabs(D->Uo[b]) >= std::fabs(D->Uo[d]);
+  D->a = a; D->ub = u_is_b ? b : d; D->vb = u_is_b ? d : b; D->pad = 0;
+  double P[3][4];
+  for (int c = 0; c < 4; ++c) {
+    P[2][c] = f.p3[c];
+    P[0][c] = f.pu[c] + f.cu * f.p3[c];
+    P[1][c] = f.pv[c] + f.cv * f.p3[c];
+  }
+  for (int r = 0; r < 3; ++r) {
+    for (int c = 0; c < 3; ++c) D->P[r][c] = P[r][0] * R.m[0][c] + P[r][1] * R.m[1][c] + P[r][2] * R.m[2][c];
+    D->P[r][3] = P[r][0] * t[0] + P[r][1] * t[1] + P[r][2] * t[2] + P[r][3];
+  }
+}
+
 inline BpGeom make_bp_geom(const dfp_geometry& g) {
   BpGeom G;
   G.nx = g.nx; G.ny = g.ny; G.nz = g.nz; G.nu = g.nu; G.nv = g.nv;

@@ -134,7 +134,7 @@ def test_c5_sweep_full(dfp):
 
 
 def test_c2_registration_full_grad_interp_mode(dfp):
-    """DFP_FLAG_GRAD_INTERP at the bench's size: two seeded views' 6-vectors against the oracle's GRAD_INTERP mode."""
+    """DFP_FLAG_GRAD_INTERP at full C2 size: eight seeded views' 6-vectors against the oracle's GRAD_INTERP mode."""
     dev = torch.device("cuda:0")
     w = W.make_config(2)
     g = w.geom.replace(flags=dfp.FLAG_GRAD_INTERP)
@@ -145,11 +145,11 @@ def test_c2_registration_full_grad_interp_mode(dfp):
     grad = dfp.forward_pose_grad(g, a, p, vol, up).cpu().numpy()
     assert dfp.last_path() == dfp.PATH_TMA and np.isfinite(grad).all()
     vol_c = vol.cpu().numpy()
-    for v in pick(w.seed + 503, w.n_views, 2):
+    for v in pick(w.seed + 503, w.n_views, 8):
         o = oracle.forward_pose_grad(w.geom, a[v:v + 1], p[v:v + 1], vol_c, up[v:v + 1].cpu().numpy(),
                                      grad_mode=oracle.GRAD_INTERP)
         e = grad_err_u9(grad[v:v + 1], o)
-        assert e.max() <= 3 * TOL_GRAD and np.sort(e.ravel())[-2] <= TOL_GRAD, (v, e)
+        assert e.max() <= TOL_GRAD, (v, e)
 
 
 @pytest.mark.parametrize("model", ["siddon", "joseph"])
@@ -255,3 +255,44 @@ def test_c2_view_results_do_not_depend_on_the_batch(dfp):
     ga = g.replace(flags=g.flags | dfp.FLAG_ACCUMULATE)
     dfp.backproject(ga, a[32:], p[32:], bproj[32:].contiguous(), out=halves)
     assert rel_l2(halves.cpu().numpy(), whole.cpu().numpy()) <= 2e-7
+
+
+def test_c2_registration_full_distance_driven(dfp):
+    """DFP_FLAG_DD at full C2 size (256^3, 64 views of 512x512): a row band of two seeded views, one z-slab of the
+    back-projection (all 64 views) and one view's 6-vectors of both gradients against the oracle's O15."""
+    dev = torch.device("cuda:0")
+    w = W.make_config(2)
+    g0 = w.geom
+    g = g0.replace(flags=dfp.FLAG_DD)
+    a = w.angles.float().numpy()
+    p = w.poses.float().numpy()
+    vol = w.volume(dev)
+    up = w.fwd_upstream(dev)
+    proj = dfp.forward(g, a, p, vol)
+    grad = dfp.forward_pose_grad(g, a, p, vol, up).cpu().numpy()
+    assert torch.isfinite(proj).all() and np.isfinite(grad).all()
+    vol_c = vol.cpu().numpy()
+    views = pick(w.seed + 701, w.n_views, 2)
+    for v in views:
+        r0 = pick(w.seed + 711 + v, g0.nv - 32 + 1, 1)[0]
+        o = oracle.forward_dd(row_band(g0, r0, 32), a[v:v + 1], p[v:v + 1], vol_c)[0]
+        check_values(proj[v, r0:r0 + 32].cpu().numpy(), o, TOL_VAL, zero_border=True)
+    v = views[0]
+    o = oracle.forward_pose_grad_dd(g0, a[v:v + 1], p[v:v + 1], vol_c, up[v:v + 1].cpu().numpy())
+    e = grad_err_u9(grad[v:v + 1], o)
+    report("C2 DD forward_pose_grad, 1 view", e)
+    assert e.max() <= TOL_GRAD
+    del up, proj
+    pin = w.projections(dev)
+    bup = w.bp_upstream(dev)
+    bp = dfp.backproject(g, a, p, pin)
+    bgrad = dfp.backproject_pose_grad(g, a, p, pin, bup).cpu().numpy()
+    assert torch.isfinite(bp).all() and np.isfinite(bgrad).all()
+    pin_c = pin.cpu().numpy()
+    z0 = pick(w.seed + 721, g0.nz - 1, 1)[0]
+    o = oracle.backproject_dd(g0, a, p, pin_c, z0, z0 + 1)
+    check_values(bp[z0:z0 + 1].cpu().numpy(), o, TOL_VAL, zero_border=False)
+    o = oracle.backproject_pose_grad_dd(g0, a[v:v + 1], p[v:v + 1], pin_c[v:v + 1], bup.cpu().numpy())
+    e = grad_err_u9(bgrad[v:v + 1], o)
+    report("C2 DD backproject_pose_grad, 1 view", e)
+    assert e.max() <= TOL_GRAD

