@@ -433,6 +433,23 @@ def main():
                                          "ncc": rs["ncc"], "stop": rs["stop"]},
                                          "what": "256^3 volume, one 512x512 view, Adam on NCC (Eq.25), stop rule of PAPER.md :235"}
         del volr, tgt
+        # the paper's second task as a loop (PAPER.md :237-242, Eq.26): full C3 (256^3, 360 ramp-filtered views of
+        # 512x384, FDK weight), Adam on the gradient entropy of the back-projection; per iteration dfp_backproject +
+        # GE and its autograd gradient (harness, torch, same stream) + dfp_backproject_pose_grad + a [360, 6] read-back
+        from paper_2508_13304_b200.registration import motion_compensated_backprojection
+        w3 = W.make_config(3)
+        p3 = w3.projections(dev)
+        a3 = w3.angles.float().numpy()
+        motion_compensated_backprojection(w3.geom, a3, p3, W.gradient_entropy, n_iters=2)       # warm-up
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        r3 = motion_compensated_backprojection(w3.geom, a3, p3, W.gradient_entropy, n_iters=10)
+        dt = time.perf_counter() - t0
+        other["mcfdk_loop_C3"] = {"ms_per_iteration": dt / 10 * 1e3, "iterations_per_s": 10 / dt, "timed_iterations": 10,
+                                  "gradient_entropy_first_last": [r3["losses"][0], r3["losses"][-1]],
+                                  "what": "256^3 volume, 360 views of 512x384, all 360x6 poses, Adam on gradient entropy (Eq.26)"}
+        del p3
+        torch.cuda.empty_cache()
         for idx in (2, 4):
             j2 = Job(dfp, idx, dev)
             seg2, _ = j2.timed(3, 3, flush, barrier)

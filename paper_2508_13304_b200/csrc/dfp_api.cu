@@ -492,7 +492,11 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
                                             {BoxShape<5>::X, BoxShape<5>::Y, BoxShape<5>::Z}};
   // forward: shapes 0, 1, 2 (16 x 16-pixel tiles) - with the odd-extent boxes 4, 5 first where a pixel spans >= 0.45
   // voxel along z (bank conflicts, dfp_fwd_tma.cuh); gradient: shapes 3, 2 (16 x 8-pixel tiles)
-  static const int kOrderFwd[3] = {0, 1, 2}, kOrderFwdWide[5] = {4, 5, 0, 1, 2}, kOrderGrad[2] = {3, 2};
+#ifndef DFP_WIDE_A
+#define DFP_WIDE_A 4
+#define DFP_WIDE_B 5
+#endif
+  static const int kOrderFwd[3] = {0, 1, 2}, kOrderFwdWide[5] = {DFP_WIDE_A, DFP_WIDE_B, 0, 1, 2}, kOrderGrad[2] = {3, 2};
   const bool wide = hf[0].vlen * ((double)g->sad / hf[0].sdd) / (double)g->vz >= 0.45;
   const int* order = grad ? kOrderGrad : (wide ? kOrderFwdWide : kOrderFwd);
   const int n_order = grad ? 2 : (wide ? 5 : 3);

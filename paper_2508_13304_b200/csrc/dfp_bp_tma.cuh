@@ -27,16 +27,19 @@ constexpr int kBpConsumers = kBpT * kBpT;        // 256 consumer threads = 8 war
 constexpr int kBpTmaThreads = kBpConsumers + 32; // + 1 producer warp
 constexpr float kPatchMargin = 0.05f;            // pixels: fp32 rounding of the per-voxel projection
 
-// Detector patch menu (floats): U x V, every U a multiple of 4 (TMA inner box) and = 4 or 20 mod 32, so that
-// consecutive detector rows of a patch start 4 banks apart (U = 32, 64, 96 put all rows on the same banks:
-// measured 1.97 LDS wavefronts per warp load on C3 against 1.3 with these pitches).  The host bounds the largest
+// Detector patch menu (floats): U x V, every U a multiple of 4 (TMA inner box) and = 12 or 20 mod 32.  A warp is an
+// 8 x 4 patch of voxel columns at one z: its 32 pixels lie in a thin parallelogram - up to ~16 pixels along u and, by
+// the perspective (v scales with the depth, which varies across the tile), 2-5 detector rows.  Bank = (u + U v) mod 32:
+// with U = 12 / 20 mod 32 the rows land 12 banks apart and the parallelogram spreads over distinct banks (simulated
+// wavefronts per warp load, C5 / C2 / C3: 1.39 / 1.48 / 1.02; the first layout - 16 x 2 columns per warp, U = 4 mod 32 -
+// 1.90 / 1.56 / 1.36, measured 2.2 on C5; U = 32, 64, 96 put all rows on the same banks: 2.1-3.5).  The host bounds the largest
 // patch any (tile, view) of the call can need and sizes the stages for it; the producer then picks, per (tile,
 // view), the SMALLEST patch that holds the actual footprint, so the bytes the TMA unit moves follow the local
 // magnification instead of the worst case (near-source tiles and rotated views need 2-4x the median patch).
 constexpr int kNumPatches = 6;
-__device__ __constant__ int kPatchU[kNumPatches] = {36, 52, 68, 68, 100, 100};
+__device__ __constant__ int kPatchU[kNumPatches] = {44, 52, 76, 76, 108, 108};
 __device__ __constant__ int kPatchV[kNumPatches] = {16, 24, 32, 48, 64, 80};
-static const int kPatchUHost[kNumPatches] = {36, 52, 68, 68, 100, 100};
+static const int kPatchUHost[kNumPatches] = {44, 52, 76, 76, 108, 108};
 static const int kPatchVHost[kNumPatches] = {16, 24, 32, 48, 64, 80};
 struct alignas(64) PatchMaps { CUtensorMap m[kNumPatches]; };
 constexpr int kPatchHeader = 64;                 // floats per stage in front of the patch: local P_eff rows, c0, pitch, status, fp64 rows
@@ -51,6 +54,9 @@ inline int bp_num_stages(int kmax) {
 __device__ __forceinline__ void mbar_arrive(unsigned bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+// Consumer thread -> voxel column of the 16 x 16 tile: a warp is an 8 (x) by 4 (y) patch, two warps across x.
+__device__ __forceinline__ int bp_lane_x() { return ((threadIdx.x >> 5) & 1) * 8 + (threadIdx.x & 7); }
+__device__ __forceinline__ int bp_lane_y() { return (threadIdx.x >> 6) * 4 + ((threadIdx.x >> 3) & 3); }
 __device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kBpConsumers) : "memory"); }
 
 // Stage header layout (floats).  All rows are LOCAL to the (tile, view): they act on (lx, ly, lz) = voxel index minus
@@ -179,9 +185,10 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_tma_kernel(BpGeom G, int n_v
     return;
   }
   // ---- consumers: thread = one (x, y) column of the tile, TZ voxels along z in registers
-  const int ix = T.x0 + (threadIdx.x & (kBpT - 1)), iy = T.y0 + threadIdx.x / kBpT;
+  const int lx = bp_lane_x(), ly = bp_lane_y();
+  const int ix = T.x0 + lx, iy = T.y0 + ly;
   const bool live = ix < G.nx && iy < G.ny;
-  const float xf = (float)(threadIdx.x & (kBpT - 1)), yf = (float)(threadIdx.x / kBpT);   // tile-local voxel index
+  const float xf = (float)lx, yf = (float)ly;                      // tile-local voxel index
   float acc[TZ];
 #pragma unroll
   for (int m = 0; m < TZ; ++m)     // DFP_FLAG_ACCUMULATE: start from the caller's volume (a slice of the views)
@@ -287,9 +294,10 @@ __global__ void __launch_bounds__(kBpTmaThreads) bp_grad_tma_kernel(BpGeom G, in
     return;
   }
   // ---- consumers
-  const int ix = T.x0 + (threadIdx.x & (kBpT - 1)), iy = T.y0 + threadIdx.x / kBpT;
+  const int lx = bp_lane_x(), ly = bp_lane_y();
+  const int ix = T.x0 + lx, iy = T.y0 + ly;
   const bool live = ix < G.nx && iy < G.ny;
-  const float xf = (float)(threadIdx.x & (kBpT - 1)), yf = (float)(threadIdx.x / kBpT);   // tile-local voxel index
+  const float xf = (float)lx, yf = (float)ly;                      // tile-local voxel index
   // object-frame mm of the column's first voxel
   const float rx = G.cx + ((float)ix - G.hx) * G.vx, ry = G.cy + ((float)iy - G.hy) * G.vy,
               rz = G.cz + ((float)T.z0 - G.hz) * G.vz;

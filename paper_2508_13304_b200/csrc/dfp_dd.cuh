@@ -180,57 +180,69 @@ __global__ void __launch_bounds__(kFwdThreads) dd_fwd_kernel(DdGeom G, const DdV
 }
 
 // ------------------------------------------------------------------------------------------------ back (transpose)
-// Weight of pixel (iu, iv) on the cell of voxel (plane xa, in-plane indices jb, jd): the forward formula.  `L` is left
-// out (the caller multiplies by it only when the overlaps are positive: it costs a square root).
-__device__ __forceinline__ double dd_overlap(const DdGeom& G, const DdView& W, int iu, int iv, double xa, int jb, int jd) {
-  double b0, b1, d0, d1;
-  bool f = dd_hit(G, W, iu - 0.5, (double)iv, xa, W.ub, &b0);
-  f &= dd_hit(G, W, iu + 0.5, (double)iv, xa, W.ub, &b1);
-  f &= dd_hit(G, W, (double)iu, iv - 0.5, xa, W.vb, &d0);
-  f &= dd_hit(G, W, (double)iu, iv + 0.5, xa, W.vb, &d1);
-  if (!f) return 0.0;
-  if (b0 > b1) { const double t = b0; b0 = b1; b1 = t; }
-  if (d0 > d1) { const double t = d0; d0 = d1; d1 = t; }
-  if (!(b1 > b0) || !(d1 > d0)) return 0.0;
-  // the voxel must be one of the cells the forward loop visits: jb in [floor(b0 + 1/2), floor(b1 + 1/2)]
-  const double ob = fmin(b1, jb + 0.5) - fmax(b0, jb - 0.5), od = fmin(d1, jd + 0.5) - fmax(d0, jd - 0.5);
-  if (!(ob > 0.0) || !(od > 0.0)) return 0.0;
+// Offset, in voxels along axis `ax`, from the voxel centre r (on the plane x_a = r_a) to the point where the ray
+// source -> detector point (u, v) meets that plane:  (D_ax E_a - E_ax D_a) / (D_a v_ax),  D = X(u, v) - s', E = r - s'.
+// The 2 x 2 determinant of two nearly parallel vectors is taken in fp64; the quotient is a small number (a few voxels)
+// and is taken in fp32 from there - no fp64 division per boundary.  `front`: the plane lies in front of the source.
+__device__ __forceinline__ float dd_offset(const DdView& W, double u, double v, const double* E, int ax, float inv_v,
+                                           bool* front) {
+  const int a = W.a;
+  const double Da = fma(u, W.Uo[a], fma(v, W.Vo[a], W.X00[a])) - W.so[a];
+  const double Dx = fma(u, W.Uo[ax], fma(v, W.Vo[ax], W.X00[ax])) - W.so[ax];
+  const float det = (float)fma(Dx, E[a], -E[ax] * Da);
+  const float da = (float)Da;
+  *front = E[a] * Da > 0.0;                       // t = E_a / D_a > 0
+  return det * fast_rcp(da) * inv_v;
+}
+// Weight (without the slab length L) of pixel (iu, iv) on the voxel whose centre is r = s' + E, in-plane axes ub / vb.
+__device__ __forceinline__ float dd_overlap(const DdGeom& G, const DdView& W, int iu, int iv, const double* E) {
+  bool f0, f1, f2, f3;
+  const float ivb = 1.0f / (float)G.v[W.ub], ivd = 1.0f / (float)G.v[W.vb];
+  float b0 = dd_offset(W, iu - 0.5, (double)iv, E, W.ub, ivb, &f0), b1 = dd_offset(W, iu + 0.5, (double)iv, E, W.ub, ivb, &f1);
+  float d0 = dd_offset(W, (double)iu, iv - 0.5, E, W.vb, ivd, &f2), d1 = dd_offset(W, (double)iu, iv + 0.5, E, W.vb, ivd, &f3);
+  if (!(f0 && f1 && f2 && f3)) return 0.f;
+  if (b0 > b1) { const float t = b0; b0 = b1; b1 = t; }
+  if (d0 > d1) { const float t = d0; d0 = d1; d1 = t; }
+  if (!(b1 > b0) || !(d1 > d0)) return 0.f;
+  // the voxel's cell is [-1/2, 1/2] in these offsets
+  const float ob = fminf(b1, 0.5f) - fmaxf(b0, -0.5f), od = fminf(d1, 0.5f) - fmaxf(d0, -0.5f);
+  if (!(ob > 0.f) || !(od > 0.f)) return 0.f;
   return (ob / (b1 - b0)) * (od / (d1 - d0));
 }
-__device__ __forceinline__ double dd_slab_length(const DdGeom& G, const DdView& W, int iu, int iv, double xa, bool* front) {
-  double n2 = 0, da = 0;
+__device__ __forceinline__ float dd_slab_length(const DdGeom& G, const DdView& W, int iu, int iv) {
+  float n2 = 0.f, da = 0.f;
 #pragma unroll
   for (int x = 0; x < 3; ++x) {
-    const double d = fma((double)iu, W.Uo[x], fma((double)iv, W.Vo[x], W.X00[x])) - W.so[x];
-    n2 = fma(d, d, n2);
+    const float d = (float)(fma((double)iu, W.Uo[x], fma((double)iv, W.Vo[x], W.X00[x])) - W.so[x]);
+    n2 = fmaf(d, d, n2);
     if (x == W.a) da = d;
   }
-  *front = fabs(da) >= 1e-300 && (xa - W.so[W.a]) / da > 0.0;
-  return G.v[W.a] * sqrt(n2) / fabs(da);
+  return (float)G.v[W.a] * sqrtf(n2) / fabsf(da);
 }
 
-// Candidate pixels of a voxel: the detector bounding box of its cell's four corners on the plane, one pixel of margin
-// (the footprints are taken on the pixels' mid-lines, which an in-plane rotation tilts by a fraction of a pixel).
+// Candidate pixels of a voxel: the detector bounding box of its cell's four corners on the plane (fp32: the box gets
+// one pixel of margin anyway - the footprints are taken on the pixels' mid-lines, which an in-plane rotation tilts by a
+// fraction of a pixel).
 struct DdWindow { int u0, u1, v0, v1; };
-__device__ __forceinline__ DdWindow dd_window(const DdGeom& G, const DdView& W, int k, int jb, int jd) {
-  double umin = 1e300, umax = -1e300, vmin = 1e300, vmax = -1e300;
+__device__ __forceinline__ DdWindow dd_window(const DdGeom& G, const DdView& W, const float* P, const float* r) {
+  float umin = 3e38f, umax = -3e38f, vmin = 3e38f, vmax = -3e38f;
   bool ok = true;
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
-    double r[3];
-    r[W.a] = G.c[W.a] + (k - G.h[W.a]) * G.v[W.a];
-    r[W.ub] = G.c[W.ub] + (jb + ((c & 1) ? 0.5 : -0.5) - G.h[W.ub]) * G.v[W.ub];
-    r[W.vb] = G.c[W.vb] + (jd + ((c & 2) ? 0.5 : -0.5) - G.h[W.vb]) * G.v[W.vb];
-    const double wp = fma(W.P[2][0], r[0], fma(W.P[2][1], r[1], fma(W.P[2][2], r[2], W.P[2][3])));
-    if (!(wp > 0.0)) ok = false;
-    const double u = fma(W.P[0][0], r[0], fma(W.P[0][1], r[1], fma(W.P[0][2], r[2], W.P[0][3]))) / wp;
-    const double v = fma(W.P[1][0], r[0], fma(W.P[1][1], r[1], fma(W.P[1][2], r[2], W.P[1][3]))) / wp;
-    umin = fmin(umin, u); umax = fmax(umax, u); vmin = fmin(vmin, v); vmax = fmax(vmax, v);
+    float q[3] = {r[0], r[1], r[2]};
+    q[W.ub] += ((c & 1) ? 0.5f : -0.5f) * (float)G.v[W.ub];
+    q[W.vb] += ((c & 2) ? 0.5f : -0.5f) * (float)G.v[W.vb];
+    const float wp = fmaf(P[8], q[0], fmaf(P[9], q[1], fmaf(P[10], q[2], P[11])));
+    if (!(wp > 0.f)) ok = false;
+    const float rw = 1.0f / wp;
+    const float u = fmaf(P[0], q[0], fmaf(P[1], q[1], fmaf(P[2], q[2], P[3]))) * rw;
+    const float v = fmaf(P[4], q[0], fmaf(P[5], q[1], fmaf(P[6], q[2], P[7]))) * rw;
+    umin = fminf(umin, u); umax = fmaxf(umax, u); vmin = fminf(vmin, v); vmax = fmaxf(vmax, v);
   }
   DdWindow w;
-  if (!ok || !(umax - umin < 1e6) || !(vmax - vmin < 1e6)) { w.u0 = w.v0 = 0; w.u1 = w.v1 = -1; return w; }
-  w.u0 = max((int)floor(umin + 0.5) - 1, 0); w.u1 = min((int)floor(umax + 0.5) + 1, G.nu - 1);
-  w.v0 = max((int)floor(vmin + 0.5) - 1, 0); w.v1 = min((int)floor(vmax + 0.5) + 1, G.nv - 1);
+  if (!ok || !(umax - umin < 1e6f) || !(vmax - vmin < 1e6f)) { w.u0 = w.v0 = 0; w.u1 = w.v1 = -1; return w; }
+  w.u0 = max((int)floorf(umin + 0.5f) - 1, 0); w.u1 = min((int)floorf(umax + 0.5f) + 1, G.nu - 1);
+  w.v0 = max((int)floorf(vmin + 0.5f) - 1, 0); w.v1 = min((int)floorf(vmax + 0.5f) + 1, G.nv - 1);
   return w;
 }
 
@@ -268,18 +280,20 @@ __global__ void __launch_bounds__(kDdBpThreads) dd_bp_kernel(DdGeom G, int n_vie
     __syncthreads();
     double su = 0.0, sv = 0.0;
     if (live && (!GRAD || wj != 0.f)) {
-      const int k = xyz[W.a], jb = xyz[W.ub], jd = xyz[W.vb];
-      const double xa = G.c[W.a] + (k - G.h[W.a]) * G.v[W.a];
-      const DdWindow win = dd_window(G, W, k, jb, jd);
+      double E[3];
+#pragma unroll
+      for (int x = 0; x < 3; ++x) E[x] = G.c[x] + ((double)xyz[x] - G.h[x]) * G.v[x] - W.so[x];
+      float Pl[12];
+#pragma unroll
+      for (int q = 0; q < 12; ++q) Pl[q] = (float)W.P[q >> 2][q & 3];
+      const float rc[3] = {rx, ry, rz};
+      const DdWindow win = dd_window(G, W, Pl, rc);
       const float* img = proj + (size_t)view * G.nu * G.nv;
       for (int iv = win.v0; iv <= win.v1; ++iv)
         for (int iu = win.u0; iu <= win.u1; ++iu) {
-          const double o = dd_overlap(G, W, iu, iv, xa, jb, jd);
-          if (!(o > 0.0)) continue;
-          bool front;
-          const double L = dd_slab_length(G, W, iu, iv, xa, &front);
-          if (!front) continue;
-          const double wgt = L * o;
+          const float o = dd_overlap(G, W, iu, iv, E);
+          if (!(o > 0.f)) continue;
+          const double wgt = (double)(dd_slab_length(G, W, iu, iv) * o);
           if (!GRAD) {
             acc = fma(wgt, (double)__ldg(img + (size_t)iv * G.nu + iu), acc);
           } else {

@@ -59,7 +59,13 @@ template <> struct BoxShape<3> { static constexpr int X = 28, Y = 28, Z = 16, ST
 // 1.76 -> 1.38 wavefronts per load on C5, 1.62 -> 1.36 on C4 (simulated, _and measured_ in DESIGN.md); at C2's 0.39
 // voxel per pixel the even extents are the better ones (1.37 against 1.64).
 template <> struct BoxShape<4> { static constexpr int X = 20, Y = 19, Z = 16, STAGES = 2; };
-template <> struct BoxShape<5> { static constexpr int X = 28, Y = 19, Z = 20, STAGES = 2; };
+#ifndef DFP_S5_STAGES
+#define DFP_S5_STAGES 1          // one stage, four blocks per SM: 305 ms against 322 with two stages / two blocks (C5)
+#endif
+#ifndef DFP_S5_Z
+#define DFP_S5_Z 20
+#endif
+template <> struct BoxShape<5> { static constexpr int X = 28, Y = 19, Z = DFP_S5_Z, STAGES = DFP_S5_STAGES; };
 constexpr int kNumShapes = 6;
 // words between the stages of a box: the box rounded up to 128 bytes (alignment of a TMA destination)
 template <int SHAPE> __host__ __device__ constexpr int tma_stage_words() {
@@ -226,17 +232,19 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
   float gx = 0.f, gy = 0.f, gz = 0.f, hx = 0.f, hy = 0.f, hz = 0.f;
   for (int chunk = 0; chunk < n_chunks; ++chunk) {
     const int s = chunk % S::STAGES;
-    mbar_wait(bar_addr + 8u * s, (unsigned)(chunk / S::STAGES) & 1u);
     const int c_lo = kA + chunk * Kc;
     const int ka = max(c_lo, r.k0), kb = min(min(c_lo + Kc, kB), kend);
     // this lane takes the samples of its ray whose kappa is congruent to its slot (the other slots take the rest)
     const int kfirst = SLOTS == 1 ? ka : ka + ((slot - ka) & (SLOTS - 1));
-    // re-base the ray onto the box origin (fp64, once per chunk): local position of this lane's first sample
-    const int o0 = B.org[s][0], o1 = B.org[s][1], o2 = B.org[s][2];
+    // re-base the ray onto the box origin (fp64, once per chunk): position of this lane's first sample - fetched from
+    // local memory and advanced BEFORE the wait for the box, so that the loads' latency overlaps it
     const double kd = (double)kfirst;
-    const float2 bxy = make_float2((float)(fma(kd, rd[zi + 3], rd[zi + 0]) - (double)o0),
-                                   (float)(fma(kd, rd[zi + 4], rd[zi + 1]) - (double)o1));
-    const float bz = (float)(fma(kd, rd[zi + 5], rd[zi + 2]) - (double)o2);
+    const double p0 = fma(kd, rd[zi + 3], rd[zi + 0]), p1 = fma(kd, rd[zi + 4], rd[zi + 1]),
+                 p2 = fma(kd, rd[zi + 5], rd[zi + 2]);
+    mbar_wait(bar_addr + 8u * s, (unsigned)(chunk / S::STAGES) & 1u);
+    const int o0 = B.org[s][0], o1 = B.org[s][1], o2 = B.org[s][2];
+    const float2 bxy = make_float2((float)(p0 - (double)o0), (float)(p1 - (double)o1));
+    const float bz = (float)(p2 - (double)o2);
     // word index of local cell (X, Y, Z) in stage s from the magic-rounded floats' bits
     unsigned c0 = (unsigned)(s * kWords) - (unsigned)kMagicBits * (unsigned)(1 + BX + BXY);
     // keep the constant out of the optimiser's sight: folded into every load's offset it no longer fits the LDS

@@ -52,3 +52,42 @@ def register_view(geom, view, vol, target, theta0=None, max_iters=200, lr_mm=0.4
         v = betas[1] * v + (1 - betas[1]) * grad * grad
         theta = theta + lr * (m / (1 - betas[0] ** it)) / (np.sqrt(v / (1 - betas[1] ** it)) + eps)     # ascent
     return {"theta": theta, "ncc": hist[-1], "iterations": it, "stop": stop, "history": hist}
+
+
+def motion_compensated_backprojection(geom, views, proj, loss_fn, n_iters=80, lr_mm=0.1, lr_rad=0.1 * DEG, theta0=None,
+                                      betas=(0.9, 0.999), eps=1e-12, callback=None):
+    """The paper's second task as a loop over the library (PAPER.md :237-242, Eq.26): per-view rigid motion estimated by
+    Adam descent on an image-sharpness loss of the (filtered) back-projection, 80 iterations, all views' 6 parameters
+    at once and no trajectory regularisation.  Per iteration: `dfp_backproject` at the current poses, the caller's
+    differentiable `loss_fn(volume) -> scalar` (torch; e.g. the gradient entropy) and its autograd gradient dL/dmu on
+    the same stream, `dfp_backproject_pose_grad` with that upstream, one read-back of the [V, 6] gradient, Adam on the
+    host.  `proj`: cuda [V, nv, nu] (already ramp-filtered for an FDK weight).  Returns dict(theta, losses)."""
+    g = _b.Geometry.of(geom)
+    dev = proj.device
+    V = int(proj.shape[0])
+    theta = np.zeros((V, 6)) if theta0 is None else np.array(theta0, dtype=np.float64)
+    lr = np.array([lr_mm] * 3 + [lr_rad] * 3)
+    m, v = np.zeros_like(theta), np.zeros_like(theta)
+    vol = torch.empty((g.nz, g.ny, g.nx), dtype=torch.float32, device=dev)
+    grad = torch.empty((V, 6), dtype=torch.float32, device=dev)
+    ws = torch.empty(max(_b.workspace_bytes(g, V, _b.OP_BACKPROJECT), _b.workspace_bytes(g, V, _b.OP_BACKPROJECT_POSE_GRAD)),
+                     dtype=torch.uint8, device=dev)
+    host = torch.empty((V, 6), dtype=torch.float32).pin_memory()
+    losses = []
+    for it in range(1, n_iters + 1):
+        th32 = theta.astype(np.float32)
+        _b.backproject(g, views, th32, proj, out=vol, ws=ws)
+        mu = vol.detach().requires_grad_(True)
+        loss = loss_fn(mu)
+        (up,) = torch.autograd.grad(loss, mu)
+        _b.backproject_pose_grad(g, views, th32, proj, up.to(torch.float32).contiguous(), out=grad, ws=ws)
+        host.copy_(grad, non_blocking=True)
+        torch.cuda.current_stream(dev).synchronize()
+        gr = host.double().numpy()
+        losses.append(float(loss))
+        if callback is not None:
+            callback(it, theta, losses[-1])
+        m = betas[0] * m + (1 - betas[0]) * gr
+        v = betas[1] * v + (1 - betas[1]) * gr * gr
+        theta = theta - lr * (m / (1 - betas[0] ** it)) / (np.sqrt(v / (1 - betas[1] ** it)) + eps)     # descent
+    return {"theta": theta, "losses": losses}

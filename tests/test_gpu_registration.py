@@ -181,3 +181,33 @@ def test_registration_loop_on_the_device_meets_the_papers_stop_rule():
     assert res["iterations"] < 400
     # the stop rule ends the search at NCC 0.999, not at the optimum: within a quarter of the initial 4 mm / 3 degrees
     assert np.abs(res["theta"][:3] - hidden[:3]).max() < 1.0 and np.abs(res["theta"][3:] - hidden[3:]).max() < 0.75 * DEG, res
+
+
+def test_motion_compensated_fdk_with_gradient_entropy_recovers_the_per_view_motion():
+    """The paper's second task (PAPER.md :237-242, Eq.26): 90 ramp-filtered views of config 3 (quarter scale) of an object
+    that moved smoothly during the scan (up to 4 mm / 2 degrees); all 90 x 6 pose parameters start at 0 and follow 80
+    Adam steps on the gradient entropy of the FDK back-projection, through dfp_backproject + dfp_backproject_pose_grad.
+    GE falls to its value at the true motion and the motion error (a rigid offset common to all views does not change
+    the sharpness and is removed) falls from 1.6 mm / 0.85 degrees to under 0.6 mm / 0.2 degrees."""
+    import paper_2508_13304_b200 as dfp
+    from paper_2508_13304_b200.registration import motion_compensated_backprojection
+    dev = torch.device("cuda:0")
+    w = W.make_config(3, scale=0.25, n_views=90)
+    g = w.geom
+    a = w.angles.float().numpy()
+    true = w.data_poses.numpy()
+    proj = w.projections(dev)
+
+    def err(th):
+        d = th - true
+        d = d - d.mean(axis=0, keepdims=True)
+        return float(np.abs(d[:, :3]).mean()), float(np.abs(d[:, 3:]).mean() / DEG)
+
+    ge_at = lambda th: float(W.gradient_entropy(dfp.backproject(g, a, th.astype(np.float32), proj)))
+    ge_true, ge_zero = ge_at(true), ge_at(np.zeros_like(true))
+    res = motion_compensated_backprojection(g, a, proj, W.gradient_entropy, n_iters=80)
+    e0, e1 = err(np.zeros_like(true)), err(res["theta"])
+    ge_end = ge_at(res["theta"])
+    assert ge_true < ge_zero and res["losses"][0] == pytest.approx(ge_zero, rel=1e-6)
+    assert (ge_zero - ge_end) >= 0.9 * (ge_zero - ge_true), (ge_zero, ge_end, ge_true)
+    assert e1[0] < 0.4 * e0[0] and e1[1] < 0.3 * e0[1], (e0, e1)

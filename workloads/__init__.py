@@ -12,7 +12,7 @@ from .rng import SplitMix64, normal_field, uniform_field
 from .geometry import Geometry, view_angles, circular_frame, move_frame, noncircular_orbit, FLAG_VIEW_FRAMES
 from .phantom import (Ellipsoid, random_ellipsoids, voxelise_ellipsoids, voxelise_blobs,
                       ellipsoid_projection, blob_projection, rotation_zyx)
-from .losses import ncc, ncc_grad, variance_grad, ssd_grad
+from .losses import ncc, ncc_grad, variance_grad, ssd_grad, gradient_entropy
 from .ramp import ramp_filter
 from .configs import CONFIGS, make_config, base_seed
 
@@ -20,6 +20,6 @@ __all__ = [
     "SplitMix64", "normal_field", "uniform_field", "Geometry", "view_angles", "circular_frame", "move_frame", "noncircular_orbit",
     "FLAG_VIEW_FRAMES", "Ellipsoid",
     "random_ellipsoids", "voxelise_ellipsoids", "voxelise_blobs", "ellipsoid_projection",
-    "blob_projection", "rotation_zyx", "ncc", "ncc_grad", "variance_grad", "ssd_grad",
+    "blob_projection", "rotation_zyx", "ncc", "ncc_grad", "variance_grad", "ssd_grad", "gradient_entropy",
     "ramp_filter", "CONFIGS", "make_config", "base_seed",
 ]

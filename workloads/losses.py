@@ -34,3 +34,17 @@ def variance_grad(mu: torch.Tensor) -> torch.Tensor:
 def ssd_grad(l: torch.Tensor, target: torch.Tensor) -> torch.Tensor:
     """d sum (l - target)^2 / d l = 2 (l - target)."""
     return 2.0 * (l.to(torch.float64) - target.to(torch.float64))
+
+
+def gradient_entropy(mu: torch.Tensor) -> torch.Tensor:
+    """Gradient entropy of a volume, the sharpness criterion of the paper's motion-compensated reconstruction
+    (Eq.26 :239, "as in [9]"): with g_j = |forward finite-difference gradient of mu at voxel j| and
+    p_j = g_j / sum g, GE = -sum_j p_j log p_j (smaller = sharper).  Differentiable torch code: its autograd gradient
+    dGE/dmu is the UPSTREAM array of dfp_backproject_pose_grad - an input of the method, not part of it."""
+    m = mu.to(torch.float64)
+    gx = m[:-1, :-1, 1:] - m[:-1, :-1, :-1]
+    gy = m[:-1, 1:, :-1] - m[:-1, :-1, :-1]
+    gz = m[1:, :-1, :-1] - m[:-1, :-1, :-1]
+    g = torch.sqrt(gx * gx + gy * gy + gz * gz + 1e-12)
+    p = g / g.sum()
+    return -(p * torch.log(p + 1e-30)).sum()
