@@ -342,3 +342,46 @@ def backproject_pose_grad_dd(g, angles, poses, proj, upstream):
     grad = np.empty((V, 6), dtype=np.float64)
     lib.ora_backproject_pose_grad_dd(ctypes.byref(gg), V, _p(angles), _p(poses), _p(proj), _p(up), _p(grad))
     return grad
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# O16: separable-footprint projector pair SF-TR (PAPER.md :213 [29]; reading DESIGN.md U16)
+def forward_sf(g, angles, poses, vol):
+    """l_i = sum_j a^ij mu_j with separable-footprint weights (voxel-driven).  -> proj [V,nv,nu] float64."""
+    fn, gg, angles, poses, V, vol = _model_call("ora_forward_sf", g, angles, poses, vol)
+    proj = np.empty((V, gg.nv, gg.nu), dtype=np.float64)
+    fn(ctypes.byref(gg), V, _p(angles), _p(poses), _p(vol), _p(proj))
+    return proj
+
+
+def backproject_sf(g, angles, poses, proj, iz0=0, iz1=None):
+    """The SF back-projector = the exact transpose of `forward_sf`.  proj [V,nv,nu] float32 -> vol[iz0:iz1] float64."""
+    lib = _load()
+    angles, poses, V = _views(angles, poses, g)
+    gg = _geom(g)
+    iz1 = gg.nz if iz1 is None else iz1
+    proj = _f32(proj).reshape(V, gg.nv, gg.nu)
+    out = np.empty((iz1 - iz0, gg.ny, gg.nx), dtype=np.float64)
+    lib.ora_backproject_sf(ctypes.byref(gg), V, _p(angles), _p(poses), _p(proj), _p(out), int(iz0), int(iz1))
+    return out
+
+
+def forward_pose_grad_sf(g, angles, poses, vol, upstream):
+    """Pose gradient through the SF forward projector, per-voxel G_f^j (Eq.19-20).  -> [V,6] float64."""
+    fn, gg, angles, poses, V, vol = _model_call("ora_forward_pose_grad_sf", g, angles, poses, vol)
+    up = _f32(upstream).reshape(V, gg.nv, gg.nu)
+    grad = np.empty((V, 6), dtype=np.float64)
+    fn(ctypes.byref(gg), V, _p(angles), _p(poses), _p(vol), _p(up), _p(grad))
+    return grad
+
+
+def backproject_pose_grad_sf(g, angles, poses, proj, upstream):
+    """Pose gradient through the SF back-projector, per-pixel G_b^i (Eq.22).  -> [V,6] float64."""
+    lib = _load()
+    angles, poses, V = _views(angles, poses, g)
+    gg = _geom(g)
+    proj = _f32(proj).reshape(V, gg.nv, gg.nu)
+    up = _f32(upstream).reshape(gg.nz, gg.ny, gg.nx)
+    grad = np.empty((V, 6), dtype=np.float64)
+    lib.ora_backproject_pose_grad_sf(ctypes.byref(gg), V, _p(angles), _p(poses), _p(proj), _p(up), _p(grad))
+    return grad

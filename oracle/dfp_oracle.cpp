@@ -1065,6 +1065,202 @@ void backproject_grad_dd_impl(const ora_geom& g, int n_views, const double* angl
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// O16 (last item): separable-footprint projector pair [29] (PAPER.md :213, Tables III / IV rows SF)
+// under a rigid pose.  The paper cites the method and gives no formula; [29] builds its trapezoids from the corners of
+// a voxel whose axes are aligned with the detector's, which a 6-DOF pose breaks (taken literally under an in-plane
+// rotation psi the footprint loses a factor cos^2 psi of its mass and the projector no longer converges - tried).
+// Reading taken (U16), voxel-driven, everything from Eq.13's Jacobian at the voxel centre:
+//   * (u_j, v_j) = p(r_j) and J = d(u, v)/d r' (2 x 3, pixel-index units per mm; Eq.13 :143-146 with P_eff = P [R | t]);
+//   * widths of the voxel along the detector axes: wu_k = |J_uk| v_k, wv_k = |J_vk| v_k, k = x', y', z';
+//   * T(u) = the unit-area TRAPEZOID that is the convolution of the two widest rects among wu (base w1 + w2, top
+//     w1 - w2), centred at u_j; R(v) likewise from wv, centred at v_j  (SF's separable footprint with trapezoids
+//     along both axes, "SF-TT", linearised about the voxel centre; the third, narrowest rect of each axis is dropped);
+//   * mass M_j = v_x v_y v_z sqrt(det(J J^T)): the integral of the voxel's chord-length image over the detector in
+//     pixel units (J annihilates the ray direction, so sqrt(det J J^T) is the area magnification of the plane
+//     perpendicular to the ray);
+//   * a^ij = M_j * int_{iu-1/2}^{iu+1/2} T(u) du * int_{iv-1/2}^{iv+1/2} R(v) dv   (detector blur = the pixel's rect).
+// Voxels behind the source (w' <= 0) contribute nothing.  `visit(w, iu, iv)` for the view's pixels.
+struct SFView {
+  double E[3][4];               // P_eff: (u', v', w') = E (r'; 1), pixel-index units, object-frame mm
+  SFView(const ora_geom& g, const View& view, const Pose& pose) {
+    (void)g;
+    for (int r = 0; r < 3; ++r) {
+      for (int c = 0; c < 3; ++c)
+        E[r][c] = view.P[r][0] * pose.R.m[0][c] + view.P[r][1] * pose.R.m[1][c] + view.P[r][2] * pose.R.m[2][c];
+      E[r][3] = view.P[r][0] * pose.t.x + view.P[r][1] * pose.t.y + view.P[r][2] * pose.t.z + view.P[r][3];
+    }
+  }
+};
+// int_{-inf}^{x} of the unit-area trapezoid centred at c with base b >= top t >= 0
+inline double trap_cdf(double c, double b, double t, double x) {
+  const double h = 2.0 / (b + t);                   // height: area = h (b + t) / 2 = 1
+  const double x0 = c - 0.5 * b, x1 = c - 0.5 * t, x2 = c + 0.5 * t, x3 = c + 0.5 * b;
+  double s = 0.0;
+  if (x1 > x0) { const double r = std::min(std::max(x, x0), x1) - x0; s += h * r * r / (2.0 * (x1 - x0)); }
+  s += h * (std::min(std::max(x, x1), x2) - x1);
+  if (x3 > x2) { const double r = std::min(std::max(x, x2), x3) - x2; s += h * (r - r * r / (2.0 * (x3 - x2))); }
+  return s;
+}
+inline void two_widest(const double* w, double* base, double* top) {
+  double a = w[0], b = w[1], c = w[2];
+  if (a < b) std::swap(a, b);
+  if (b < c) std::swap(b, c);
+  if (a < b) std::swap(a, b);
+  *base = a + b; *top = a - b;
+}
+template <typename F>
+inline void sf_weights(const ora_geom& g, const SFView& S, int ix, int iy, int iz, F visit) {
+  const double v[3] = {g.vx, g.vy, g.vz};
+  const V3 rc = voxel_centre(g, ix, iy, iz);
+  const double up = S.E[0][0] * rc.x + S.E[0][1] * rc.y + S.E[0][2] * rc.z + S.E[0][3];
+  const double vp = S.E[1][0] * rc.x + S.E[1][1] * rc.y + S.E[1][2] * rc.z + S.E[1][3];
+  const double wp = S.E[2][0] * rc.x + S.E[2][1] * rc.y + S.E[2][2] * rc.z + S.E[2][3];
+  if (!(wp > 0)) return;
+  const double uj = up / wp, vj = vp / wp;
+  double Ju[3], Jv[3], wu[3], wv[3];
+  for (int k = 0; k < 3; ++k) {
+    Ju[k] = (S.E[0][k] * wp - S.E[2][k] * up) / (wp * wp);      // Eq.13
+    Jv[k] = (S.E[1][k] * wp - S.E[2][k] * vp) / (wp * wp);
+    wu[k] = fabs(Ju[k]) * v[k]; wv[k] = fabs(Jv[k]) * v[k];
+  }
+  const double guu = Ju[0] * Ju[0] + Ju[1] * Ju[1] + Ju[2] * Ju[2], gvv = Jv[0] * Jv[0] + Jv[1] * Jv[1] + Jv[2] * Jv[2],
+               guv = Ju[0] * Jv[0] + Ju[1] * Jv[1] + Ju[2] * Jv[2];
+  const double M = v[0] * v[1] * v[2] * sqrt(std::max(guu * gvv - guv * guv, 0.0));
+  double bu, tu, bv, tv;
+  two_widest(wu, &bu, &tu);
+  two_widest(wv, &bv, &tv);
+  if (!(bu > 0) || !(bv > 0) || !(M > 0)) return;
+  const long iu0 = std::max((long)floor(uj - 0.5 * bu + 0.5), 0L), iu1 = std::min((long)floor(uj + 0.5 * bu + 0.5), (long)g.nu - 1);
+  const long iv0 = std::max((long)floor(vj - 0.5 * bv + 0.5), 0L), iv1 = std::min((long)floor(vj + 0.5 * bv + 0.5), (long)g.nv - 1);
+  for (long iv = iv0; iv <= iv1; ++iv) {
+    const double fv = trap_cdf(vj, bv, tv, iv + 0.5) - trap_cdf(vj, bv, tv, iv - 0.5);
+    if (!(fv > 0)) continue;
+    for (long iu = iu0; iu <= iu1; ++iu) {
+      const double fu = trap_cdf(uj, bu, tu, iu + 0.5) - trap_cdf(uj, bu, tu, iu - 0.5);
+      if (!(fu > 0)) continue;
+      visit(M * fu * fv, iu, iv);
+    }
+  }
+}
+
+// mode 0: forward l_i = sum_j a^ij mu_j;  mode 1: back-projection mu_j = sum_i a^ij l_i (exact transpose), slab [iz0, iz1)
+template <typename T>
+void sf_project_impl(const ora_geom& g, int n_views, const double* angles, const double* poses, const T* vol,
+                     double* proj, const float* y_in, double* vol_out, int iz0, int iz1) {
+  const bool back = vol_out != nullptr;
+  const size_t npix = (size_t)g.nu * g.nv;
+  if (back) for (size_t i = 0; i < (size_t)(iz1 - iz0) * g.ny * g.nx; ++i) vol_out[i] = 0.0;
+  int nthr = 1;
+#ifdef _OPENMP
+  nthr = omp_get_max_threads();
+#endif
+  for (int v = 0; v < n_views; ++v) {
+    View view(g, angles, v);
+    Pose pose(poses + 6 * v);
+    const SFView S(g, view, pose);
+    if (back) {
+#pragma omp parallel for schedule(dynamic, 1) collapse(2)
+      for (int iz = iz0; iz < iz1; ++iz) for (int iy = 0; iy < g.ny; ++iy) for (int ix = 0; ix < g.nx; ++ix) {
+        double s = 0.0;
+        sf_weights(g, S, ix, iy, iz, [&](double w, long iu, long iv) { s += w * (double)y_in[(size_t)v * npix + (size_t)iv * g.nu + iu]; });
+        vol_out[((size_t)(iz - iz0) * g.ny + iy) * g.nx + ix] += s;
+      }
+    } else {
+      std::vector<std::vector<double>> priv(nthr, std::vector<double>(npix, 0.0));
+#pragma omp parallel for schedule(static)
+      for (int iz = 0; iz < g.nz; ++iz) {
+        int me = 0;
+#ifdef _OPENMP
+        me = omp_get_thread_num();
+#endif
+        double* out = priv[me].data();
+        for (int iy = 0; iy < g.ny; ++iy) for (int ix = 0; ix < g.nx; ++ix) {
+          const double mu = (double)vol[((size_t)iz * g.ny + iy) * g.nx + ix];
+          if (mu == 0.0) continue;
+          sf_weights(g, S, ix, iy, iz, [&](double w, long iu, long iv) { out[(size_t)iv * g.nu + iu] += w * mu; });
+        }
+      }
+      double* dst = proj + (size_t)v * npix;
+      for (size_t i = 0; i < npix; ++i) { double s = 0.0; for (int t = 0; t < nthr; ++t) s += priv[t][i]; dst[i] = s; }
+    }
+  }
+}
+
+// mode 0: forward pose gradient  sum_ij w_i a^ij G_f^j = sum_j (A^T w)_j G_f^j  (per-voxel G_f^j, Eq.19-20);
+// mode 1: back-projection pose gradient  sum_ij a^ij w_j (D_u^i J_u(r_j) + D_v^i J_v(r_j))  (per-pixel G_b^i, Eq.22; as O15).
+template <typename T>
+void sf_grad_impl(const ora_geom& g, int n_views, const double* angles, const double* poses, const T* vol,
+                  const float* img, const float* upvol, double* grad, int mode) {
+  Vol<T> V{vol, g.nx, g.ny, g.nz};
+  const size_t npix = (size_t)g.nu * g.nv;
+  for (int v = 0; v < n_views; ++v) {
+    View view(g, angles, v);
+    Pose pose(poses + 6 * v);
+    const SFView S(g, view, pose);
+    Img I{img + (size_t)v * npix, g.nu, g.nv};
+    const double(*P)[4] = view.P;
+    std::vector<double> slab((size_t)g.nz * 6, 0.0);
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int iz = 0; iz < g.nz; ++iz) {
+      double acc[6] = {0};
+      for (int iy = 0; iy < g.ny; ++iy) for (int ix = 0; ix < g.nx; ++ix) {
+        if (mode == 0) {
+          double s = 0.0;
+          sf_weights(g, S, ix, iy, iz, [&](double w, long iu, long iv) { s += w * I.at(iu, iv); });
+          if (s == 0.0) continue;
+          V3 gj = {(V.at(ix + 1, iy, iz) - V.at(ix - 1, iy, iz)) / (2 * g.vx),
+                   (V.at(ix, iy + 1, iz) - V.at(ix, iy - 1, iz)) / (2 * g.vy),
+                   (V.at(ix, iy, iz + 1) - V.at(ix, iy, iz - 1)) / (2 * g.vz)};
+          V3 rj = voxel_centre(g, ix, iy, iz), c = cross(rj, gj);
+          acc[0] += s * gj.x; acc[1] += s * gj.y; acc[2] += s * gj.z;
+          acc[3] += s * c.x; acc[4] += s * c.y; acc[5] += s * c.z;
+        } else {
+          const double wj = (double)upvol[((size_t)iz * g.ny + iy) * g.nx + ix];
+          double su = 0.0, sv = 0.0;
+          sf_weights(g, S, ix, iy, iz, [&](double w, long iu, long iv) {
+            su += w * 0.5 * (I.at(iu + 1, iv) - I.at(iu - 1, iv));
+            sv += w * 0.5 * (I.at(iu, iv + 1) - I.at(iu, iv - 1));
+          });
+          if (su == 0.0 && sv == 0.0) continue;
+          V3 r = mul(pose.R, voxel_centre(g, ix, iy, iz)) + pose.t;
+          double up = P[0][0] * r.x + P[0][1] * r.y + P[0][2] * r.z + P[0][3];
+          double vp = P[1][0] * r.x + P[1][1] * r.y + P[1][2] * r.z + P[1][3];
+          double wp = P[2][0] * r.x + P[2][1] * r.y + P[2][2] * r.z + P[2][3];
+          V3 Ju = {(P[0][0] * wp - P[2][0] * up) / (wp * wp), (P[0][1] * wp - P[2][1] * up) / (wp * wp),
+                   (P[0][2] * wp - P[2][2] * up) / (wp * wp)};
+          V3 Jv = {(P[1][0] * wp - P[2][0] * vp) / (wp * wp), (P[1][1] * wp - P[2][1] * vp) / (wp * wp),
+                   (P[1][2] * wp - P[2][2] * vp) / (wp * wp)};
+          V3 q = wj * ((su * Ju) + (sv * Jv));
+          V3 cq = cross(r - pose.t, q);
+          acc[0] += q.x; acc[1] += q.y; acc[2] += q.z; acc[3] += cq.x; acc[4] += cq.y; acc[5] += cq.z;
+        }
+      }
+      for (int k = 0; k < 6; ++k) slab[(size_t)iz * 6 + k] = acc[k];
+    }
+    double tot[6] = {0};
+    for (int iz = 0; iz < g.nz; ++iz) for (int k = 0; k < 6; ++k) tot[k] += slab[(size_t)iz * 6 + k];
+    const double* th = poses + 6 * v;
+    double* out = grad + 6 * v;
+    if (mode == 0) {
+      V3 SA = {tot[0], tot[1], tot[2]}, SB = {tot[3], tot[4], tot[5]};
+      V3 dt = mul(pose.R, SA);
+      out[0] = -dt.x; out[1] = -dt.y; out[2] = -dt.z;
+      V3 wx = {1, 0, 0};
+      V3 wy = mulT(Rx(th[3]), V3{0, 1, 0});
+      V3 wz = mulT(mul(Ry(th[4]), Rx(th[3])), V3{0, 0, 1});
+      out[3] = -dot(wx, SB); out[4] = -dot(wy, SB); out[5] = -dot(wz, SB);
+    } else {
+      V3 Sq = {tot[0], tot[1], tot[2]}, Sc = {tot[3], tot[4], tot[5]};
+      V3 ax = mul(pose.R, V3{1, 0, 0});
+      V3 ay = mul(Rz(th[5]), V3{0, 1, 0});
+      V3 az = {0, 0, 1};
+      out[0] = Sq.x; out[1] = Sq.y; out[2] = Sq.z;
+      out[3] = dot(ax, Sc); out[4] = dot(ay, Sc); out[5] = dot(az, Sc);
+    }
+  }
+}
+
 extern "C" {
 
 int ora_num_threads() {
@@ -1199,6 +1395,32 @@ void ora_forward_pose_grad_dd_f64(const ora_geom* g, int n_views, const double* 
 void ora_backproject_pose_grad_dd(const ora_geom* g, int n_views, const double* angles, const double* poses,
                                   const float* proj, const float* upstream, double* grad) {
   backproject_grad_dd_impl(*g, n_views, angles, poses, proj, upstream, grad);
+}
+
+// O16: separable-footprint pair (forward, back-projector = exact transpose, both pose gradients)
+void ora_forward_sf_f32(const ora_geom* g, int n_views, const double* angles, const double* poses, const float* vol,
+                        double* proj) {
+  sf_project_impl<float>(*g, n_views, angles, poses, vol, proj, nullptr, nullptr, 0, 0);
+}
+void ora_forward_sf_f64(const ora_geom* g, int n_views, const double* angles, const double* poses, const double* vol,
+                        double* proj) {
+  sf_project_impl<double>(*g, n_views, angles, poses, vol, proj, nullptr, nullptr, 0, 0);
+}
+void ora_backproject_sf(const ora_geom* g, int n_views, const double* angles, const double* poses, const float* proj,
+                        double* vol_out, int iz0, int iz1) {
+  sf_project_impl<float>(*g, n_views, angles, poses, (const float*)nullptr, nullptr, proj, vol_out, iz0, iz1);
+}
+void ora_forward_pose_grad_sf_f32(const ora_geom* g, int n_views, const double* angles, const double* poses,
+                                  const float* vol, const float* upstream, double* grad) {
+  sf_grad_impl<float>(*g, n_views, angles, poses, vol, upstream, nullptr, grad, 0);
+}
+void ora_forward_pose_grad_sf_f64(const ora_geom* g, int n_views, const double* angles, const double* poses,
+                                  const double* vol, const float* upstream, double* grad) {
+  sf_grad_impl<double>(*g, n_views, angles, poses, vol, upstream, nullptr, grad, 0);
+}
+void ora_backproject_pose_grad_sf(const ora_geom* g, int n_views, const double* angles, const double* poses,
+                                  const float* proj, const float* upstream, double* grad) {
+  sf_grad_impl<float>(*g, n_views, angles, poses, (const float*)nullptr, proj, upstream, grad, 1);
 }
 
 }  // extern "C"

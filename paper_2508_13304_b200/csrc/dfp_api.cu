@@ -196,7 +196,7 @@ bool make_volume_map(const dfp_geometry& g, const float* d_vol, int bx, int by, 
 // |De_a| <= (|Dd_a| + |e_a| (rho_max/|d|) |Dd|) / SDD  for pixel offsets Dd on a detector at distance >= SDD.
 constexpr int kMinChunk = 4;
 bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V, const ViewFrame& F, bool grad,
-                   const int* box, int TU, int TV) {
+                   const int* box, int TU, int TV, int min_chunk = kMinChunk) {
   const double v3[3] = {g.vx, g.vy, g.vz}, c3[3] = {g.cx, g.cy, g.cz};
   const double half[3] = {0.5 * g.nx * g.vx + 3 * g.vx, 0.5 * g.ny * g.vy + 3 * g.vy, 0.5 * g.nz * g.vz + 3 * g.vz};
   double tau_max = 0;
@@ -227,7 +227,7 @@ bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V, co
     const double span = tau_max * (dd + emax[a] * rho * dnorm) / sdd / v3[a];
     const double slope = (double)G.step * emax[a] / v3[a];
     const double avail = box[a] - 4 - (grad ? 2 : 0) - (a == 0 ? kBoxAlignLoss : 0) - 2.0 * kBoxMargin - 1.05 * span - 0.05;
-    if (avail < (kMinChunk - 1) * slope) return false;
+    if (avail < (min_chunk - 1) * slope) return false;
   }
   return true;
 }
@@ -507,6 +507,13 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
       bool fits = true;
       for (int v = 0; fits && v < V; ++v) fits = tma_view_fits(*g, G, hv[v], hf[v], grad, kBoxes[order[i]], TU, TV);
       if (fits) shape = order[i];
+    }
+    // last resort before the gather kernels (coarse pixels on fine voxels, e.g. C1's forward call: 1.2 voxels per
+    // pixel): the largest box with chunks of two samples - short chunks, but no packed copy of the volume
+    if (shape < 0) {
+      bool fits = true;
+      for (int v = 0; fits && v < V; ++v) fits = tma_view_fits(*g, G, hv[v], hf[v], grad, kBoxes[2], TU, TV, 2);
+      if (fits) shape = 2;
     }
   }
   const bool tma = shape >= 0 && make_volume_map(*g, d_vol, kBoxes[shape][0], kBoxes[shape][1], kBoxes[shape][2], &vol_map);

@@ -126,9 +126,10 @@ def test_missed_and_empty_inputs_give_exact_zeros():
 
 
 # ---------------------------------------------------------------- forward pose gradient (Eq.19-20 :179-191)
-def stored_Gf_gradient(g, beta, pose, vol, up):
+def stored_Gf_gradient(g, beta, pose, vol, up, forward=None):
     """The paper's algorithm as printed (:189-191) with DD weights: 12 volumes G_f^j = [ (R r'_j) g_j^T | -R g_j ]
     built with numpy, each projected by the (separately pinned) forward_dd, weighted, contracted with dM/dtheta."""
+    forward = oracle.forward_dd if forward is None else forward
     R, dR = oracle.rotation(pose)
     pad = np.pad(vol, 1)
     gj = np.stack([(pad[1:-1, 1:-1, 2:] - pad[1:-1, 1:-1, :-2]) / (2 * g.vx),
@@ -142,8 +143,8 @@ def stored_Gf_gradient(g, beta, pose, vol, up):
     GM = np.zeros((3, 4))
     for a in range(3):
         for b in range(3):
-            GM[a, b] = float((oracle.forward_dd(g, [beta], [pose], lever[a] * gj[b])[0] * up).sum())
-        GM[a, 3] = float((oracle.forward_dd(g, [beta], [pose], -Rg[a])[0] * up).sum())
+            GM[a, b] = float((forward(g, [beta], [pose], lever[a] * gj[b])[0] * up).sum())
+        GM[a, 3] = float((forward(g, [beta], [pose], -Rg[a])[0] * up).sum())
     out = np.zeros(6)
     out[:3] = GM[:, 3]
     for k in range(3):
@@ -199,12 +200,19 @@ def test_back_gradient_equals_the_papers_stored_Gb_algorithm(beta, pose):
     rng = np.random.default_rng(23)
     proj = (rng.integers(-64, 65, size=(1,) + g.det_shape) / 64.0).astype(np.float32)
     w = rng.standard_normal(g.vol_shape).astype(np.float32)
+    expect = stored_Gb_gradient(g, beta, pose, proj, w, backproject=oracle.backproject_dd)
+    got = oracle.backproject_pose_grad_dd(g, [beta], [pose], proj, w)[0]
+    assert np.abs(got - expect).max() <= 1e-11 * np.abs(expect).max(), (got, expect)
+
+
+def stored_Gb_gradient(g, beta, pose, proj, w, backproject):
+    """The paper's stored-G_b algorithm (:202-206) for a matched projector pair given by its `backproject`."""
     lp = np.pad(proj[0].astype(np.float64), 1)
     Du = 0.5 * (lp[1:-1, 2:] - lp[1:-1, :-2])
     Dv = 0.5 * (lp[2:, 1:-1] - lp[:-2, 1:-1])
     assert np.array_equal(Du.astype(np.float32), Du) and np.array_equal(Dv.astype(np.float32), Dv)
-    Bu = oracle.backproject_dd(g, [beta], [pose], Du[None].astype(np.float32))
-    Bv = oracle.backproject_dd(g, [beta], [pose], Dv[None].astype(np.float32))
+    Bu = backproject(g, [beta], [pose], Du[None].astype(np.float32))
+    Bv = backproject(g, [beta], [pose], Dv[None].astype(np.float32))
     iz, iy, ix = np.meshgrid(np.arange(g.nz), np.arange(g.ny), np.arange(g.nx), indexing="ij")
     rp = np.stack([g.cx + (ix - (g.nx - 1) / 2) * g.vx, g.cy + (iy - (g.ny - 1) / 2) * g.vy,
                    g.cz + (iz - (g.nz - 1) / 2) * g.vz], axis=-1)
@@ -217,9 +225,7 @@ def test_back_gradient_equals_the_papers_stored_Gb_algorithm(beta, pose):
     Jv = (P[1, :3] * wp_[..., None] - P[2, :3] * vp_[..., None]) / wp_[..., None] ** 2
     q = Bu[..., None] * Ju + Bv[..., None] * Jv
     GM = np.einsum("zyx,zyxa,zyxb->ab", w.astype(np.float64), q, hom)
-    expect = np.concatenate([GM[:, 3], [(dR[k] * GM[:, :3]).sum() for k in range(3)]])
-    got = oracle.backproject_pose_grad_dd(g, [beta], [pose], proj, w)[0]
-    assert np.abs(got - expect).max() <= 1e-11 * np.abs(expect).max(), (got, expect)
+    return np.concatenate([GM[:, 3], [(dR[k] * GM[:, :3]).sum() for k in range(3)]])
 
 
 def test_back_gradient_vs_finite_differences_of_the_discrete_dd_backprojector():
