@@ -91,7 +91,13 @@ typedef struct dfp_geometry {
                            the two in-plane axes (U14).  dfp_backproject is then the EXACT transpose of dfp_forward
                            (a matched pair, Eq.21), dfp_forward_pose_grad takes G_f^j per voxel and dfp_backproject_pose_grad
                            G_b^i per detector pixel (Eq.19-22).  bp_weight must be 0; not combinable with bits 2, 3, 5 or
-                           dfp_forward_fused_moments (DFP_ERR_DIMS); step_mm is unused.                            */
+                           dfp_forward_fused_moments (DFP_ERR_DIMS); step_mm is unused;
+                           bit8 (DFP_FLAG_SF): as bit7 with SEPARABLE-FOOTPRINT weights (PAPER.md :213, ref [29]) - per
+                           (voxel, view) a separable footprint on the detector, trapezoids along u and v built from the
+                           Jacobian of Eq.13 at the voxel centre, mass = voxel volume x area magnification (U16).
+                           dfp_forward accumulates with fp32 atomics (its results vary at the 1e-7 level from run to run;
+                           every other call of the library is bit-reproducible).  Same restrictions as bit7; not together
+                           with it.                                                                              */
 } dfp_geometry;
 
 enum {
@@ -106,7 +112,7 @@ enum {
 enum { DFP_OP_FORWARD = 0, DFP_OP_FORWARD_POSE_GRAD = 1, DFP_OP_BACKPROJECT = 2, DFP_OP_BACKPROJECT_POSE_GRAD = 3,
        DFP_OP_FORWARD_FUSED = 4, DFP_OP_NCC = 5 };
 enum { DFP_FLAG_DW = 1, DFP_FLAG_NO_TMA = 2, DFP_FLAG_GRAD_INTERP = 4, DFP_FLAG_SIDDON = 8,
-       DFP_FLAG_ACCUMULATE = 16, DFP_FLAG_JOSEPH = 32, DFP_FLAG_VIEW_FRAMES = 64, DFP_FLAG_DD = 128 };
+       DFP_FLAG_ACCUMULATE = 16, DFP_FLAG_JOSEPH = 32, DFP_FLAG_VIEW_FRAMES = 64, DFP_FLAG_DD = 128, DFP_FLAG_SF = 256 };
 
 /* Forward projection, Eq.2a :67-69 discretised as Eq.18 :172-177 with a fixed-step, zero-extended
  * trilinear ray-march (U1): proj[v][iv][iu] = D * sum_k f~(R_v^T (s_v + (k+1/2) D e_i - t_v)).

@@ -22,6 +22,7 @@ FLAG_SIDDON = 8
 FLAG_ACCUMULATE = 16
 FLAG_JOSEPH = 32
 FLAG_DD = 128              # distance-driven weights in all four calls (include/dfp.h)
+FLAG_SF = 256              # separable-footprint weights in all four calls
 FLAG_VIEW_FRAMES = 64      # `angles` arguments hold [V,12] explicit view frames (s, c, U, V), include/dfp.h
 PATH_GATHER, PATH_TMA = 0, 1
 

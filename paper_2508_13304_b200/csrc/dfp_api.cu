@@ -15,6 +15,7 @@
 #include "dfp_kernels.cuh"
 #include "dfp_params.h"
 #include "dfp_dd.cuh"
+#include "dfp_sf.cuh"
 #include "dfp_joseph.cuh"
 #include "dfp_loss.cuh"
 #include "dfp_siddon.cuh"
@@ -334,10 +335,14 @@ FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad, int nset = 1) {
   w.gy8 = (g.nv + TmaLanes<1>::TV - 1) / TmaLanes<1>::TV;
   size_t o = 0;
   w.off_views = o; o += align_up(sizeof(FwdView) * (size_t)V);
-  w.off_dd = o;    o += (g.flags & DFP_FLAG_DD) ? align_up(sizeof(DdView) * (size_t)V) : 0;
+  w.off_dd = o;    o += (g.flags & (DFP_FLAG_DD | DFP_FLAG_SF)) ? align_up(sizeof(DdView) * (size_t)V) : 0;
   w.off_con = o;   o += grad ? align_up(sizeof(FwdContract) * (size_t)V) : 0;
   w.off_pvol = o;  o += align_up(sizeof(float4) * (size_t)L.px * L.py * L.pz);
-  w.off_part = o;  o += grad ? align_up(sizeof(float) * 6 * (size_t)nset * V * w.gx * w.gy8) : 0;
+  {
+    size_t nblk = (size_t)w.gx * w.gy8;
+    if (g.flags & DFP_FLAG_SF) nblk = ((size_t)g.nx * g.ny * g.nz + kSfThreads - 1) / kSfThreads;   // sf_kernel blocks
+    w.off_part = o;  o += grad ? align_up(sizeof(float) * 6 * (size_t)nset * V * nblk) : 0;
+  }
   w.total = o;
   return w;
 }
@@ -360,14 +365,14 @@ BpWs bp_ws(const dfp_geometry& g, int V, bool grad) {
   size_t o = 0;
   w.off_views = o; o += align_up(sizeof(BpView) * (size_t)V);
   w.off_viewsd = o; o += align_up(sizeof(BpViewD) * (size_t)V);
-  w.off_dd = o;    o += (g.flags & DFP_FLAG_DD) ? align_up(sizeof(DdView) * (size_t)V) : 0;
+  w.off_dd = o;    o += (g.flags & (DFP_FLAG_DD | DFP_FLAG_SF)) ? align_up(sizeof(DdView) * (size_t)V) : 0;
   w.off_con = o;   o += grad ? align_up(sizeof(BpContract) * (size_t)V) : 0;
   w.off_q = o;     o += align_up(sizeof(float4) * (size_t)V * (g.nu + 2 * kPadDet) * (g.nv + 2 * kPadDet));
   w.off_part = o;
   {
     const size_t t_gather = (size_t)w.gx * w.gy * w.gz, t_tma = (size_t)w.tx * w.ty * w.tz;
     size_t tiles = t_gather > t_tma ? t_gather : t_tma;
-    if (g.flags & DFP_FLAG_DD) tiles = ((size_t)g.nx * g.ny * g.nz + kDdBpThreads - 1) / kDdBpThreads;   // dd_bp_kernel blocks
+    if (g.flags & (DFP_FLAG_DD | DFP_FLAG_SF)) tiles = ((size_t)g.nx * g.ny * g.nz + kDdBpThreads - 1) / kDdBpThreads;   // dd_bp / sf blocks
     o += grad ? align_up(sizeof(float) * 6 * (size_t)V * tiles) : 0;
   }
   w.total = o;
@@ -404,9 +409,10 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
   if (fused && (!d_proj || !aligned(d_proj, 16))) return d_proj ? DFP_ERR_ALIGN : DFP_ERR_NULL;
   if (fused && (g->flags & DFP_FLAG_GRAD_INTERP)) return DFP_ERR_DIMS;      // fused moments: central differences only
   const bool siddon = (g->flags & DFP_FLAG_SIDDON) != 0, joseph = (g->flags & DFP_FLAG_JOSEPH) != 0,
-             dd = (g->flags & DFP_FLAG_DD) != 0;
-  // Siddon / Joseph / distance-driven weights: the two plain calls only, one model at a time
-  if ((siddon || joseph || dd) && (fused || (g->flags & DFP_FLAG_GRAD_INTERP) || (int)siddon + (int)joseph + (int)dd > 1))
+             dd = (g->flags & DFP_FLAG_DD) != 0, sf = (g->flags & DFP_FLAG_SF) != 0;
+  // Siddon / Joseph / distance-driven / separable-footprint weights: the two plain calls only, one model at a time
+  if ((siddon || joseph || dd || sf) &&
+      (fused || (g->flags & DFP_FLAG_GRAD_INTERP) || (int)siddon + (int)joseph + (int)dd + (int)sf > 1))
     return DFP_ERR_DIMS;
   const int nset = fused ? 3 : 1;
   const FwdWs w = fwd_ws(*g, V, grad, nset);
@@ -431,6 +437,30 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
   DFP_CUDA(upload_async(dv, hv.data(), sizeof(FwdView) * V, s), "view upload");
   if (grad) DFP_CUDA(upload_async(dc, hc.data(), sizeof(FwdContract) * V, s), "view upload");
   const dim3 grid(w.gx, w.gy, V);
+  if (sf) {                 // separable-footprint weights (dfp_sf.cuh): voxel-driven
+    std::vector<DdView> hd((size_t)V);
+    for (int v = 0; v < V; ++v) make_dd_view(*g, hf[v], poses + 6 * v, &hd[v]);
+    DdView* ddv = reinterpret_cast<DdView*>(base + w.off_dd);
+    DFP_CUDA(upload_async(ddv, hd.data(), sizeof(DdView) * V, s), "view upload");
+    const DdGeom DG = make_dd_geom(*g);
+    const unsigned nblk = (unsigned)(((size_t)g->nx * g->ny * g->nz + kSfThreads - 1) / kSfThreads);
+    g_path = DFP_PATH_GATHER;
+    if (!grad) {
+      DFP_CUDA(cudaMemsetAsync(d_out, 0, sizeof(float) * (size_t)V * g->nu * g->nv, s), "cudaMemsetAsync");
+      time_begin(s);
+      sf_kernel<0><<<nblk, kSfThreads, 0, s>>>(DG, V, 0, ddv, d_vol, nullptr, nullptr, d_out);
+      time_end(s);
+      g_launches = 1;
+    } else {
+      time_begin(s);
+      sf_kernel<2><<<nblk, kSfThreads, 0, s>>>(DG, V, 0, ddv, d_vol, d_up, nullptr, part);
+      time_end(s);
+      fwd_contract_kernel<<<V, 256, 0, s>>>((int)nblk, part, dc, d_out);
+      g_launches = 2;
+    }
+    DFP_CUDA(cudaGetLastError(), "forward launch (separable-footprint weights)");
+    return DFP_OK;
+  }
   if (dd) {                 // distance-driven weights (dfp_dd.cuh)
     std::vector<DdView> hd((size_t)V);
     for (int v = 0; v < V; ++v) make_dd_view(*g, hf[v], poses + 6 * v, &hd[v]);
@@ -595,8 +625,10 @@ int run_backproject_slice(const dfp_geometry* g, int V, const float* angles, con
   if (!g) return DFP_ERR_NULL;
   int st = validate_geometry(g);
   if (st) return st;
-  if ((g->flags & DFP_FLAG_DD) && (g->bp_weight != 0 || (g->flags & (DFP_FLAG_GRAD_INTERP | DFP_FLAG_SIDDON | DFP_FLAG_JOSEPH))))
-    return DFP_ERR_DIMS;     // the DD back-projector is the plain transpose: unit weight, central differences only
+  if ((g->flags & (DFP_FLAG_DD | DFP_FLAG_SF)) &&
+      (g->bp_weight != 0 || (g->flags & (DFP_FLAG_GRAD_INTERP | DFP_FLAG_SIDDON | DFP_FLAG_JOSEPH)) ||
+       (g->flags & (DFP_FLAG_DD | DFP_FLAG_SF)) == (DFP_FLAG_DD | DFP_FLAG_SF)))
+    return DFP_ERR_DIMS;     // the DD / SF back-projectors are plain transposes: unit weight, central differences only
   const BpWs w = bp_ws(*g, V, grad);
   st = check_common(g, V, angles, poses, d_proj, d_out, grad ? (const void*)d_up : (const void*)d_proj, d_ws,
                         ws_bytes, w.total);
@@ -618,6 +650,27 @@ int run_backproject_slice(const dfp_geometry* g, int V, const float* angles, con
   DFP_CUDA(upload_async(dv, hv.data(), sizeof(BpView) * V, s), "view upload");
   DFP_CUDA(upload_async(dvd, hvd.data(), sizeof(BpViewD) * V, s), "view upload");
   if (grad) DFP_CUDA(upload_async(dc, hc.data(), sizeof(BpContract) * V, s), "view upload");
+  if (g->flags & DFP_FLAG_SF) {   // separable-footprint weights (dfp_sf.cuh): the exact transpose of the SF forward projector
+    std::vector<DdView> hd((size_t)V);
+    for (int v = 0; v < V; ++v) make_dd_view(*g, make_frame(*g, angles, v), poses + 6 * v, &hd[v]);
+    DdView* ddv = reinterpret_cast<DdView*>(base + w.off_dd);
+    DFP_CUDA(upload_async(ddv, hd.data(), sizeof(DdView) * V, s), "view upload");
+    const DdGeom DG = make_dd_geom(*g);
+    const unsigned nblk = (unsigned)(((size_t)g->nx * g->ny * g->nz + kSfThreads - 1) / kSfThreads);
+    time_begin(s);
+    if (!grad) {
+      sf_kernel<1><<<nblk, kSfThreads, 0, s>>>(DG, V, (g->flags & DFP_FLAG_ACCUMULATE) ? 1 : 0, ddv, nullptr, d_proj, nullptr, d_out);
+      time_end(s);
+      g_launches = 1;
+    } else {
+      sf_kernel<3><<<nblk, kSfThreads, 0, s>>>(DG, V, 0, ddv, nullptr, d_proj, d_up, part);
+      time_end(s);
+      bp_contract_kernel<<<V, 256, 0, s>>>((int)nblk, V, part, dc, d_out);
+      g_launches = 2;
+    }
+    DFP_CUDA(cudaGetLastError(), "back-projection launch (separable-footprint weights)");
+    return DFP_OK;
+  }
   if (g->flags & DFP_FLAG_DD) {   // distance-driven weights (dfp_dd.cuh): the exact transpose of the DD forward projector
     std::vector<DdView> hd((size_t)V);
     for (int v = 0; v < V; ++v) make_dd_view(*g, make_frame(*g, angles, v), poses + 6 * v, &hd[v]);

@@ -257,13 +257,15 @@ def test_c2_view_results_do_not_depend_on_the_batch(dfp):
     assert rel_l2(halves.cpu().numpy(), whole.cpu().numpy()) <= 2e-7
 
 
-def test_c2_registration_full_distance_driven(dfp):
-    """DFP_FLAG_DD at full C2 size (256^3, 64 views of 512x512): a row band of two seeded views, one z-slab of the
-    back-projection (all 64 views) and one view's 6-vectors of both gradients against the oracle's O15."""
+@pytest.mark.parametrize("model", ["dd", "sf"])
+def test_c2_registration_full_distance_driven(dfp, model):
+    """DFP_FLAG_DD / DFP_FLAG_SF at full C2 size (256^3, 64 views of 512x512): a row band of two seeded views, one z-slab
+    of the back-projection (all 64 views) and one view's 6-vectors of both gradients against the oracle's O15 / O16."""
     dev = torch.device("cuda:0")
     w = W.make_config(2)
     g0 = w.geom
-    g = g0.replace(flags=dfp.FLAG_DD)
+    g = g0.replace(flags=dfp.FLAG_DD if model == "dd" else dfp.FLAG_SF)
+    ora = {k: getattr(oracle, k + "_" + model) for k in ("forward", "forward_pose_grad", "backproject", "backproject_pose_grad")}
     a = w.angles.float().numpy()
     p = w.poses.float().numpy()
     vol = w.volume(dev)
@@ -275,12 +277,12 @@ def test_c2_registration_full_distance_driven(dfp):
     views = pick(w.seed + 701, w.n_views, 2)
     for v in views:
         r0 = pick(w.seed + 711 + v, g0.nv - 32 + 1, 1)[0]
-        o = oracle.forward_dd(row_band(g0, r0, 32), a[v:v + 1], p[v:v + 1], vol_c)[0]
+        o = ora["forward"](row_band(g0, r0, 32), a[v:v + 1], p[v:v + 1], vol_c)[0]
         check_values(proj[v, r0:r0 + 32].cpu().numpy(), o, TOL_VAL, zero_border=True)
     v = views[0]
-    o = oracle.forward_pose_grad_dd(g0, a[v:v + 1], p[v:v + 1], vol_c, up[v:v + 1].cpu().numpy())
+    o = ora["forward_pose_grad"](g0, a[v:v + 1], p[v:v + 1], vol_c, up[v:v + 1].cpu().numpy())
     e = grad_err_u9(grad[v:v + 1], o)
-    report("C2 DD forward_pose_grad, 1 view", e)
+    report(f"C2 {model} forward_pose_grad, 1 view", e)
     assert e.max() <= TOL_GRAD
     del up, proj
     pin = w.projections(dev)
@@ -290,9 +292,9 @@ def test_c2_registration_full_distance_driven(dfp):
     assert torch.isfinite(bp).all() and np.isfinite(bgrad).all()
     pin_c = pin.cpu().numpy()
     z0 = pick(w.seed + 721, g0.nz - 1, 1)[0]
-    o = oracle.backproject_dd(g0, a, p, pin_c, z0, z0 + 1)
+    o = ora["backproject"](g0, a, p, pin_c, z0, z0 + 1)
     check_values(bp[z0:z0 + 1].cpu().numpy(), o, TOL_VAL, zero_border=False)
-    o = oracle.backproject_pose_grad_dd(g0, a[v:v + 1], p[v:v + 1], pin_c[v:v + 1], bup.cpu().numpy())
+    o = ora["backproject_pose_grad"](g0, a[v:v + 1], p[v:v + 1], pin_c[v:v + 1], bup.cpu().numpy())
     e = grad_err_u9(bgrad[v:v + 1], o)
-    report("C2 DD backproject_pose_grad, 1 view", e)
+    report(f"C2 {model} backproject_pose_grad, 1 view", e)
     assert e.max() <= TOL_GRAD

@@ -732,10 +732,10 @@ def test_microbench_rates_are_those_of_a_b200_class_sm():
 
 
 # ------------------------------------------------------------------ DFP_FLAG_DD (distance-driven pair)
-def run_dd_case(dfp, g, angles, poses, vol, up, proj, bup):
-    """All four calls with distance-driven weights against the oracle's O15."""
+def run_dd_case(dfp, g, angles, poses, vol, up, proj, bup, model="dd"):
+    """All four calls with distance-driven (O15) or separable-footprint (O16) weights against the oracle."""
     dev = torch.device("cuda:0")
-    gd = g.replace(flags=g.flags | dfp.FLAG_DD)
+    gd = g.replace(flags=g.flags | (dfp.FLAG_DD if model == "dd" else dfp.FLAG_SF))
     angles, poses = f32(angles), f32(poses).reshape(-1, 6)
     t = lambda x: torch.as_tensor(np.asarray(x), dtype=torch.float32, device=dev).contiguous()
     vol_d, up_d, proj_d, bup_d = t(vol), t(up), t(proj), t(bup)
@@ -744,8 +744,9 @@ def run_dd_case(dfp, g, angles, poses, vol, up, proj, bup):
            dfp.backproject(gd, angles, poses, proj_d).cpu().numpy(),
            dfp.backproject_pose_grad(gd, angles, poses, proj_d, bup_d).cpu().numpy())
     vol_c, up_c, proj_c, bup_c = (x.cpu().numpy() for x in (vol_d, up_d, proj_d, bup_d))
-    ref = (oracle.forward_dd(g, angles, poses, vol_c), oracle.forward_pose_grad_dd(g, angles, poses, vol_c, up_c),
-           oracle.backproject_dd(g, angles, poses, proj_c), oracle.backproject_pose_grad_dd(g, angles, poses, proj_c, bup_c))
+    o = {k: getattr(oracle, k + "_" + model) for k in ("forward", "forward_pose_grad", "backproject", "backproject_pose_grad")}
+    ref = (o["forward"](g, angles, poses, vol_c), o["forward_pose_grad"](g, angles, poses, vol_c, up_c),
+           o["backproject"](g, angles, poses, proj_c), o["backproject_pose_grad"](g, angles, poses, proj_c, bup_c))
     return got, ref
 
 
@@ -808,3 +809,50 @@ def test_dd_is_a_matched_pair_and_rejects_what_it_does_not_have(dfp):
         dfp.backproject(g.replace(bp_weight=1), a, p, y)
     with pytest.raises(dfp.DfpError):
         dfp.forward_fused_moments(g, a, p, x, y)
+
+
+# ------------------------------------------------------------------ DFP_FLAG_SF (separable-footprint pair)
+def test_sf_ragged_anisotropic_general_poses_and_degenerate(dfp):
+    g = aniso_geom(nx=37, ny=29, nz=23, nu=45, nv=21)
+    rng = np.random.default_rng(50)
+    vol = rng.random(g.vol_shape).astype(np.float32)
+    angles = [0.4, math.pi / 2, 4.1, 0.1, 0.3]
+    poses = POSES3 + [[0.5, 0.3, 0.2, 0.05, 1.2, 0.0], [1.0, -1.0, 0.5, 0.9, 0.1, -0.1]]
+    up = rng.standard_normal((5,) + g.det_shape).astype(np.float32)
+    iv, iu = np.meshgrid(np.arange(g.nv), np.arange(g.nu), indexing="ij")
+    proj = np.stack([np.sin(0.21 * iu + 0.13 * iv + k) + 0.5 * np.cos(0.07 * iu - 0.19 * iv + 2 * k) for k in range(5)])
+    bup = rng.standard_normal(g.vol_shape).astype(np.float32)
+    check_dd(run_dd_case(dfp, g, angles, poses, vol, up, proj, bup, model="sf"))
+    got, _ = run_dd_case(dfp, g, [0.2], [[0, 0, 400.0, 0, 0, 0]], vol, up[:1], proj[:1], bup, model="sf")
+    assert not got[0].any() and not got[1].any() and not got[2].any() and not got[3].any()
+
+
+@pytest.mark.parametrize("index,scale,views", [(1, 1.0, None), (2, 0.25, 3), (3, 0.25, 6), (5, 0.125, 4)])
+def test_sf_configs_reduced(dfp, index, scale, views):
+    w = W.make_config(index, scale=scale, n_views=views)
+    g = w.geom.replace(bp_weight=0)
+    check_dd(run_dd_case(dfp, g, w.angles.numpy(), w.poses.numpy(), w.volume().numpy(), w.fwd_upstream().numpy(),
+                         w.projections().numpy(), w.bp_upstream().numpy(), model="sf"), zero_border=True)
+
+
+def test_sf_is_a_matched_pair_and_rejects_what_it_does_not_have(dfp):
+    dev = torch.device("cuda:0")
+    w = W.make_config(2, scale=0.25, n_views=4)
+    g = w.geom.replace(flags=dfp.FLAG_SF)
+    a, p = f32(w.angles.numpy()), f32(w.poses.numpy()).reshape(-1, 6)
+    rng = np.random.default_rng(51)
+    x = torch.as_tensor(rng.standard_normal(g.vol_shape).astype(np.float32), device=dev)
+    y = torch.as_tensor(rng.standard_normal((4,) + g.det_shape).astype(np.float32), device=dev)
+    Ax, ATy = dfp.forward(g, a, p, x), dfp.backproject(g, a, p, y)
+    lhs, rhs = float((Ax.double() * y.double()).sum()), float((x.double() * ATy.double()).sum())
+    assert abs(lhs - rhs) <= 2e-6 * abs(lhs), (lhs, rhs)
+    half = dfp.backproject(g, a[:2], p[:2], y[:2].contiguous())
+    dfp.backproject(g.replace(flags=dfp.FLAG_SF | dfp.FLAG_ACCUMULATE), a[2:], p[2:], y[2:].contiguous(), out=half)
+    assert rel_l2(half.cpu().numpy(), ATy.cpu().numpy()) <= 1e-6
+    for bad in (g.replace(flags=dfp.FLAG_SF | dfp.FLAG_DD), g.replace(flags=dfp.FLAG_SF | dfp.FLAG_GRAD_INTERP)):
+        with pytest.raises(dfp.DfpError):
+            dfp.forward_pose_grad(bad, a, p, x, y)
+        with pytest.raises(dfp.DfpError):
+            dfp.backproject(bad, a, p, y)
+    with pytest.raises(dfp.DfpError):
+        dfp.backproject(g.replace(bp_weight=1), a, p, y)
