@@ -454,12 +454,14 @@ def main():
             j2 = Job(dfp, idx, dev)
             seg2, _ = j2.timed(3, 3, flush, barrier)
             other[f"C{idx}"] = dict(rates(j2, seg2), workload=workload_name(j2.w, j2.V))
-            if idx == 2:      # DFP_FLAG_DD: the distance-driven pair, all four calls, on the C2 workload
-                gdd = j2.g.replace(flags=j2.g.flags | dfp.FLAG_DD)
-                j2.ws = torch.empty(max(dfp.workspace_bytes(gdd, j2.V, op) for op in range(4)), dtype=torch.uint8, device=dev)
-                ms = j2.time_calls([fn for _, fn in j2.calls(gdd)], 1)
-                other["C2"]["dd_mode_ms_per_call"] = dict(zip(("forward", "forward_pose_grad", "backproject",
-                                                               "backproject_pose_grad"), ms))
+            if idx == 2:      # DFP_FLAG_DD / DFP_FLAG_SF: the other matched pairs, all four calls, on the C2 workload
+                for name, flag in (("dd", dfp.FLAG_DD), ("sf", dfp.FLAG_SF)):
+                    gm = j2.g.replace(flags=j2.g.flags | flag)
+                    j2.ws = torch.empty(max(dfp.workspace_bytes(gm, j2.V, op) for op in range(4)), dtype=torch.uint8,
+                                        device=dev)
+                    ms = j2.time_calls([fn for _, fn in j2.calls(gm)], 1)
+                    other["C2"][f"{name}_mode_ms_per_call"] = dict(zip(("forward", "forward_pose_grad", "backproject",
+                                                                       "backproject_pose_grad"), ms))
             del j2
             torch.cuda.empty_cache()
 

@@ -23,6 +23,9 @@
 // detectors, closed-form blobs under a general frame, the frame of a circular view against the
 // circular path, scanner and object moved together, finite differences of the discrete projector /
 // back-projector under a general frame.
+// Distance-driven pair (O15, tests/test_oracle_dd.py) and separable-footprint pair (O16, tests/test_oracle_sf.py):
+// textbook weights on the standard views, footprint mass vs the brute-force integral of exact chords, exact
+// transposes, closed forms with convergence, stored-G on both sides, finite differences.
 // No function here is "parity unpinned".
 //
 // Conventions:

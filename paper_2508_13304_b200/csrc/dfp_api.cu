@@ -295,6 +295,7 @@ cudaError_t ensure_smem_attributes() {
   DFP_ATTR((fwd_tma_kernel<0, 0>), tma_smem_bytes<0>());
   DFP_ATTR((fwd_tma_kernel<0, 1>), tma_smem_bytes<1>());
   DFP_ATTR((fwd_tma_kernel<0, 2>), tma_smem_bytes<2>());
+  DFP_ATTR((fwd_tma_kernel<4, 2>), tma_smem_bytes<2>());
   DFP_ATTR((fwd_tma_kernel<0, 4>), tma_smem_bytes<4>());
   DFP_ATTR((fwd_tma_kernel<0, 5>), tma_smem_bytes<5>());
   DFP_ATTR((fwd_tma_kernel<1, 2>), tma_smem_bytes<2>());
@@ -532,6 +533,7 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
   const int n_order = grad ? 2 : (wide ? 5 : 3);
   const int TU = grad ? TmaLanes<1>::TU : TmaLanes<0>::TU, TV = grad ? TmaLanes<1>::TV : TmaLanes<0>::TV;
   int shape = -1;
+  bool half_tile = false;
   if (!(g->flags & DFP_FLAG_NO_TMA) && (g->nx % 4) == 0) {
     for (int i = 0; i < n_order && shape < 0; ++i) {
       bool fits = true;
@@ -544,6 +546,12 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
       bool fits = true;
       for (int v = 0; fits && v < V; ++v) fits = tma_view_fits(*g, G, hv[v], hf[v], grad, kBoxes[2], TU, TV, 2);
       if (fits) shape = 2;
+    }
+    if (shape < 0 && !grad) {          // forward only: the same box under a 16 x 8-pixel tile (MODE 4)
+      bool fits = true;
+      for (int v = 0; fits && v < V; ++v)
+        fits = tma_view_fits(*g, G, hv[v], hf[v], false, kBoxes[2], TmaLanes<4>::TU, TmaLanes<4>::TV, 2);
+      if (fits) { shape = 2; half_tile = true; }
     }
   }
   const bool tma = shape >= 0 && make_volume_map(*g, d_vol, kBoxes[shape][0], kBoxes[shape][1], kBoxes[shape][2], &vol_map);
@@ -566,6 +574,9 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
       fwd_tma_kernel<1, 3><<<nbg, TmaLanes<1>::THREADS, tma_smem_bytes<3>(), s>>>(G, Qg, dv, vol_map, d_up, part, nullptr);
     else if (grad)
       fwd_tma_kernel<1, 2><<<nbg, TmaLanes<1>::THREADS, tma_smem_bytes<2>(), s>>>(G, Qg, dv, vol_map, d_up, part, nullptr);
+    else if (half_tile)
+      fwd_tma_kernel<4, 2><<<(unsigned)V * w.gx * ((g->nv + 7) / 8), TmaLanes<4>::THREADS, tma_smem_bytes<2>(), s>>>(
+          G, FwdGrid{V, w.gx, (g->nv + 7) / 8}, dv, vol_map, nullptr, d_out, nullptr);
     else if (shape == 0)
       fwd_tma_kernel<0, 0><<<nbf, TmaLanes<0>::THREADS, tma_smem_bytes<0>(), s>>>(G, Qf, dv, vol_map, nullptr, d_out, nullptr);
     else if (shape == 1)

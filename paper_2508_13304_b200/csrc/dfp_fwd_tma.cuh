@@ -84,8 +84,11 @@ __device__ __forceinline__ float2 lerp2(float2 a, float2 v0, float2 v1) { return
 // DESIGN.md O3), 2 gradient with the exact derivative of the trilinear interpolant (DFP_FLAG_GRAD_INTERP: the same 8
 // voxels as the forward), 3 FUSED projection + central-difference gradient moments in one traversal
 // (dfp_forward_fused_moments).  Gradient kernels: two lanes per ray, 8 x 2-pixel warps, 16 x 8-pixel tile.
+// MODE 4 = GRAD 0 on a 16 x 8-pixel tile (128 threads): the forward projector's last resort before the gather kernels,
+// for coarse pixels on fine voxels (C1's forward call, 1.2 voxels per pixel: a 16 x 16 tile's frustum holds no box).
 template <int GRAD> struct TmaLanes {
-  static constexpr int SLOTS = GRAD ? DFP_GRAD_SLOTS : 1, TU = kFwdTU, TV = GRAD ? DFP_GRAD_TV : kFwdTV, THREADS = TU * TV * SLOTS;
+  static constexpr int SLOTS = (GRAD && GRAD != 4) ? DFP_GRAD_SLOTS : 1, TU = kFwdTU,
+                       TV = GRAD == 0 ? kFwdTV : (GRAD == 4 ? 8 : DFP_GRAD_TV), THREADS = TU * TV * SLOTS;
   static constexpr int PU = SLOTS == 4 ? 4 : 8, PV = 32 / (PU * SLOTS);
   static constexpr int MINB = THREADS > 256 ? 2 : 4;
 };
@@ -147,10 +150,11 @@ struct TmaBlock {              // block-wide state in shared memory
 };
 
 // One chunk's box: origin (voxel indices, for the TMA) of the stage it lands in.
-template <int GRAD, int SHAPE>
+template <int MODE, int SHAPE>
 __device__ __forceinline__ void issue_chunk(const VolLayout& L, TmaBlock& B, const CUtensorMap* map, int chunk,
                                             unsigned tiles_addr, unsigned bar_addr) {
   using S = BoxShape<SHAPE>;
+  constexpr int GRAD = MODE == 4 ? 0 : MODE;
   constexpr int kWords = S::X * S::Y * S::Z;
   const int s = chunk % S::STAGES;
   const int k0 = B.kA + chunk * B.Kc;
@@ -174,13 +178,14 @@ __device__ __forceinline__ void issue_chunk(const VolLayout& L, TmaBlock& B, con
 }
 
 // The chunk loop of one block for one box shape.  acc = {sum} (forward) or {gx,gy,gz,hx,hy,hz[,sum]} (gradient).
-template <int GRAD, int SHAPE>
+template <int MODE, int SHAPE>
 __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* map, const Ray& r, int slot,
                                           TmaBlock& B, const float* tiles, unsigned tiles_addr, unsigned bar_addr,
                                           float* acc) {
   using S = BoxShape<SHAPE>;
+  constexpr int GRAD = MODE == 4 ? 0 : MODE;
   constexpr int BX = S::X, BXY = S::X * S::Y, kBox = S::X * S::Y * S::Z, kWords = tma_stage_words<SHAPE>();
-  constexpr int SLOTS = TmaLanes<GRAD>::SLOTS;
+  constexpr int SLOTS = TmaLanes<MODE>::SLOTS;
   if (threadIdx.x == 0) {
     int Kc = 0;
     if (B.kA < B.kB) {
@@ -210,7 +215,7 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
       const int n_chunks = (B.kB - B.kA + Kc - 1) / Kc;
 #pragma unroll
       for (int c = 0; c < S::STAGES; ++c)
-        if (c < n_chunks) issue_chunk<GRAD, SHAPE>(G.L, B, map, c, tiles_addr, bar_addr);
+        if (c < n_chunks) issue_chunk<MODE, SHAPE>(G.L, B, map, c, tiles_addr, bar_addr);
     }
   }
   __syncthreads();
@@ -361,7 +366,7 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
     }
     __syncthreads();                                   // every thread is done with stage s ("empty")
     if (threadIdx.x == 0 && chunk + S::STAGES < n_chunks)
-      issue_chunk<GRAD, SHAPE>(G.L, B, map, chunk + S::STAGES, tiles_addr, bar_addr);
+      issue_chunk<MODE, SHAPE>(G.L, B, map, chunk + S::STAGES, tiles_addr, bar_addr);
   }
   if (!GRAD) {
     acc[0] = sum;
@@ -385,23 +390,24 @@ __device__ __forceinline__ void fwd_block(const FwdGrid& Q, int& view, int& bx, 
   bx = (int)(tile - (unsigned)by * (unsigned)Q.gx);
 }
 
-template <int GRAD, int SHAPE>
-__global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, TmaLanes<GRAD>::MINB) fwd_tma_kernel(FwdGeom G, FwdGrid Q,
+template <int MODE, int SHAPE>
+__global__ void __launch_bounds__(TmaLanes<MODE>::THREADS, TmaLanes<MODE>::MINB) fwd_tma_kernel(FwdGeom G, FwdGrid Q,
                                                               const FwdView* __restrict__ views,
                                                               const __grid_constant__ CUtensorMap vol_map,
                                                               const float* __restrict__ upstream,
                                                               float* __restrict__ out,
                                                               float* __restrict__ proj_out) {
+  constexpr int GRAD = MODE == 4 ? 0 : MODE;
   constexpr int NSET = GRAD == 3 ? 3 : 1;              // weight sets of the per-view reduction (fused: 1, l, b)
-  constexpr int SLOTS = TmaLanes<GRAD>::SLOTS;
+  constexpr int SLOTS = TmaLanes<MODE>::SLOTS;
   extern __shared__ __align__(128) float tiles[];      // STAGES boxes
   __shared__ __align__(8) unsigned long long full_bar[kMaxStages];
   __shared__ TmaBlock B;
-  __shared__ float red[TmaLanes<GRAD>::THREADS / 32][6 * NSET];
+  __shared__ float red[TmaLanes<MODE>::THREADS / 32][6 * NSET];
 
   int view, bx, by, iu, iv, slot;
   fwd_block(Q, view, bx, by);
-  tma_pixel<GRAD>(bx, by, iu, iv, slot);
+  tma_pixel<MODE>(bx, by, iu, iv, slot);
   const bool live = iu < G.nu && iv < G.nv;
   const unsigned tiles_addr = smem_u32(tiles), bar_addr = smem_u32(full_bar);
 
@@ -426,7 +432,7 @@ __global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, TmaLanes<GRAD>::MINB)
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   {  // corner rays of the tile: pixels (0,0), (TU-1,0), (0,TV-1), (TU-1,TV-1) of the block
-    constexpr int TU = TmaLanes<GRAD>::TU, TV = TmaLanes<GRAD>::TV;
+    constexpr int TU = TmaLanes<MODE>::TU, TV = TmaLanes<MODE>::TV;
     const int cu = iu - bx * TU, cv = iv - by * TV;
     if (slot == 0 && (cu == 0 || cu == TU - 1) && (cv == 0 || cv == TV - 1)) {
       const int c = (cu ? 1 : 0) + (cv ? 2 : 0);
@@ -449,7 +455,7 @@ __global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, TmaLanes<GRAD>::MINB)
   }
   __syncthreads();
   float acc[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-  tma_march<GRAD, SHAPE>(G, &vol_map, r, slot, B, tiles, tiles_addr, bar_addr, acc);
+  tma_march<MODE, SHAPE>(G, &vol_map, r, slot, B, tiles, tiles_addr, bar_addr, acc);
   // the slots of a ray: partial sums over the samples each lane took (slot = lane / (PU * PV): the high lane bits)
   if (SLOTS > 1) {
 #pragma unroll
@@ -507,7 +513,7 @@ __global__ void __launch_bounds__(TmaLanes<GRAD>::THREADS, TmaLanes<GRAD>::MINB)
   if (threadIdx.x < 6 * NSET) {
     float t = 0.f;
 #pragma unroll
-    for (int wI = 0; wI < TmaLanes<GRAD>::THREADS / 32; ++wI) t += red[wI][threadIdx.x];
+    for (int wI = 0; wI < TmaLanes<MODE>::THREADS / 32; ++wI) t += red[wI][threadIdx.x];
     const size_t blk = (size_t)by * Q.gx + bx;
     const size_t nblk = (size_t)Q.gx * Q.gy;
     // partials[set][view][block][6]: each weight set is a plain gradient partial array for fwd_contract_kernel

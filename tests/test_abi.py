@@ -137,3 +137,32 @@ def test_product_package_never_imports_the_oracle():
             assert "import paper_2508_13304_b200" not in src and "csrc/" not in src.replace(
                 "paper_2508_13304_b200/csrc", "") or True
             assert "import paper_2508_13304_b200" not in src
+
+
+def test_new_flags_and_the_ncc_call_reject_bad_arguments_without_a_gpu(dfp):
+    """DFP_FLAG_DD / DFP_FLAG_SF exclude each other, the other weight models, the exact-interpolant mode and an FDK
+    weight; dfp_ncc_pose_grad validates pointers, alignment and workspace before any launch."""
+    lib = ctypes.CDLL(dfp.lib_path())
+    lib.dfp_forward.restype = lib.dfp_backproject.restype = lib.dfp_ncc_pose_grad.restype = ctypes.c_int
+    dev = [ctypes.c_void_p, ctypes.c_int] + [ctypes.c_void_p] * 5 + [ctypes.c_size_t, ctypes.c_void_p]
+    lib.dfp_forward.argtypes = lib.dfp_backproject.argtypes = dev
+    lib.dfp_ncc_pose_grad.argtypes = [ctypes.c_void_p, ctypes.c_int] + [ctypes.c_void_p] * 6 + [ctypes.c_size_t, ctypes.c_void_p]
+    ang, pose = np.zeros(2, np.float32), np.zeros((2, 6), np.float32)
+    P = lambda a: a.ctypes.data_as(ctypes.c_void_p)
+    fake = ctypes.c_void_p(0x10000)
+    for flags in (128 | 256, 128 | 8, 256 | 32, 128 | 4, 256 | 4):
+        g = dfp.Geometry.of(_geom(flags=flags))
+        assert lib.dfp_forward(ctypes.byref(g), 2, P(ang), P(pose), fake, fake, fake, 1 << 30, None) == -2, flags
+    for kw in (dict(flags=128, bp_weight=1), dict(flags=256, bp_weight=1), dict(flags=128 | 256)):
+        g = dfp.Geometry.of(_geom(**kw))
+        assert lib.dfp_backproject(ctypes.byref(g), 2, P(ang), P(pose), fake, fake, fake, 1 << 30, None) == -2, kw
+    g = dfp.Geometry.of(_geom())
+    ncc = lambda gg, n, a, b, c, d, e, ws, nb: lib.dfp_ncc_pose_grad(gg, n, a, b, c, d, e, ws, nb, None)
+    assert ncc(None, 2, fake, fake, fake, fake, fake, fake, 1 << 20) == -1
+    assert ncc(ctypes.byref(g), 2, None, fake, fake, fake, fake, fake, 1 << 20) == -1
+    assert ncc(ctypes.byref(g), 0, fake, fake, fake, fake, fake, fake, 1 << 20) == -2
+    assert ncc(ctypes.byref(g), 2, ctypes.c_void_p(0x10004), fake, fake, fake, fake, fake, 1 << 20) == -4
+    assert ncc(ctypes.byref(g), 2, fake, fake, fake, fake, fake, fake, 16) == -5
+    assert dfp.workspace_bytes(g, 2, dfp.OP_NCC) > 0
+    # the other matched pairs need room for their per-view blocks and finer partial sums
+    assert dfp.workspace_bytes(dfp.Geometry.of(_geom(flags=128)), 3, 3) > dfp.workspace_bytes(g, 3, 3)
