@@ -147,6 +147,7 @@ struct TmaBlock {              // block-wide state in shared memory
   int kA, kB;                  // union of the live rays' kappa ranges [kA, kB)
   int Kc;                      // samples per chunk (0: nothing to do, -1: the box cannot hold the tile)
   int org[kMaxStages][3];      // per stage: centred index of the box's first cell (the origin of the local positions)
+  double orgd[kMaxStages][3];  // the same as doubles (one conversion by the issuing thread instead of one per thread)
 };
 
 // One chunk's box: origin (voxel indices, for the TMA) of the stage it lands in.
@@ -172,6 +173,7 @@ __device__ __forceinline__ void issue_chunk(const VolLayout& L, TmaBlock& B, con
   // not a multiple of 4 floats raises an illegal-instruction fault): round the x origin down, kBoxAlignLoss
   oc[0] = (((oc[0] + L.hx) >> 2) << 2) - L.hx;
   B.org[s][0] = oc[0]; B.org[s][1] = oc[1]; B.org[s][2] = oc[2];
+  B.orgd[s][0] = (double)oc[0]; B.orgd[s][1] = (double)oc[1]; B.orgd[s][2] = (double)oc[2];
   const unsigned bar = bar_addr + 8u * s;
   mbar_expect_tx(bar, kWords * 4);
   tma_load_3d(tiles_addr + (unsigned)(s * tma_stage_words<SHAPE>() * 4), map, oc[0] + L.hx, oc[1] + L.hy, oc[2] + L.hz, bar);
@@ -247,9 +249,8 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
     const double p0 = fma(kd, rd[zi + 3], rd[zi + 0]), p1 = fma(kd, rd[zi + 4], rd[zi + 1]),
                  p2 = fma(kd, rd[zi + 5], rd[zi + 2]);
     mbar_wait(bar_addr + 8u * s, (unsigned)(chunk / S::STAGES) & 1u);
-    const int o0 = B.org[s][0], o1 = B.org[s][1], o2 = B.org[s][2];
-    const float2 bxy = make_float2((float)(p0 - (double)o0), (float)(p1 - (double)o1));
-    const float bz = (float)(p2 - (double)o2);
+    const float2 bxy = make_float2((float)(p0 - B.orgd[s][0]), (float)(p1 - B.orgd[s][1]));
+    const float bz = (float)(p2 - B.orgd[s][2]);
     // word index of local cell (X, Y, Z) in stage s from the magic-rounded floats' bits
     unsigned c0 = (unsigned)(s * kWords) - (unsigned)kMagicBits * (unsigned)(1 + BX + BXY);
     // keep the constant out of the optimiser's sight: folded into every load's offset it no longer fits the LDS
@@ -277,7 +278,7 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
 #pragma unroll
           for (int a = 0; a < 3; ++a) { rr.pm[a] = rd[zi + a]; rr.dp[a] = rd[zi + 3 + a]; }
           exact_cell(rr, k, cell, fr);
-          idx = (unsigned)(s * kWords + (cell[0] - o0) + BX * (cell[1] - o1) + BXY * (cell[2] - o2));
+          idx = (unsigned)(s * kWords + (cell[0] - B.org[s][0]) + BX * (cell[1] - B.org[s][1]) + BXY * (cell[2] - B.org[s][2]));
           ax = fr[0]; ay = fr[1]; az = fr[2];
         }
       }
