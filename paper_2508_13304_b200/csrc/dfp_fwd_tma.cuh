@@ -90,7 +90,10 @@ template <int GRAD> struct TmaLanes {
   static constexpr int SLOTS = (GRAD && GRAD != 4) ? DFP_GRAD_SLOTS : 1, TU = kFwdTU,
                        TV = GRAD == 0 ? kFwdTV : (GRAD == 4 ? 8 : DFP_GRAD_TV), THREADS = TU * TV * SLOTS;
   static constexpr int PU = SLOTS == 4 ? 4 : 8, PV = 32 / (PU * SLOTS);
-  static constexpr int MINB = THREADS > 256 ? 2 : 4;
+#ifndef DFP_FWD_MINB
+#define DFP_FWD_MINB 4
+#endif
+  static constexpr int MINB = THREADS > 256 ? 2 : (GRAD == 0 ? DFP_FWD_MINB : 4);
 };
 template <int GRAD>
 __device__ __forceinline__ void tma_pixel(int bx, int by, int& iu, int& iv, int& slot) {
