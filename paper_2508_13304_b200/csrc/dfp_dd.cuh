@@ -180,44 +180,58 @@ __global__ void __launch_bounds__(kFwdThreads) dd_fwd_kernel(DdGeom G, const DdV
 }
 
 // ------------------------------------------------------------------------------------------------ back (transpose)
-// Offset, in voxels along axis `ax`, from the voxel centre r (on the plane x_a = r_a) to the point where the ray
-// source -> detector point (u, v) meets that plane:  (D_ax E_a - E_ax D_a) / (D_a v_ax),  D = X(u, v) - s', E = r - s'.
-// The 2 x 2 determinant of two nearly parallel vectors is taken in fp64; the quotient is a small number (a few voxels)
-// and is taken in fp32 from there - no fp64 division per boundary.  `front`: the plane lies in front of the source.
-__device__ __forceinline__ float dd_offset(const DdView& W, double u, double v, const double* E, int ax, float inv_v,
-                                           bool* front) {
-  const int a = W.a;
-  const double Da = fma(u, W.Uo[a], fma(v, W.Vo[a], W.X00[a])) - W.so[a];
-  const double Dx = fma(u, W.Uo[ax], fma(v, W.Vo[ax], W.X00[ax])) - W.so[ax];
-  const float det = (float)fma(Dx, E[a], -E[ax] * Da);
-  const float da = (float)Da;
-  *front = E[a] * Da > 0.0;                       // t = E_a / D_a > 0
-  return det * fast_rcp(da) * inv_v;
-}
-// Weight (without the slab length L) of pixel (iu, iv) on the voxel whose centre is r = s' + E, in-plane axes ub / vb.
-__device__ __forceinline__ float dd_overlap(const DdGeom& G, const DdView& W, int iu, int iv, const double* E) {
-  bool f0, f1, f2, f3;
-  const float ivb = 1.0f / (float)G.v[W.ub], ivd = 1.0f / (float)G.v[W.vb];
-  float b0 = dd_offset(W, iu - 0.5, (double)iv, E, W.ub, ivb, &f0), b1 = dd_offset(W, iu + 0.5, (double)iv, E, W.ub, ivb, &f1);
-  float d0 = dd_offset(W, (double)iu, iv - 0.5, E, W.vb, ivd, &f2), d1 = dd_offset(W, (double)iu, iv + 0.5, E, W.vb, ivd, &f3);
-  if (!(f0 && f1 && f2 && f3)) return 0.f;
-  if (b0 > b1) { const float t = b0; b0 = b1; b1 = t; }
-  if (d0 > d1) { const float t = d0; d0 = d1; d1 = t; }
-  if (!(b1 > b0) || !(d1 > d0)) return 0.f;
-  // the voxel's cell is [-1/2, 1/2] in these offsets
-  const float ob = fminf(b1, 0.5f) - fmaxf(b0, -0.5f), od = fminf(d1, 0.5f) - fmaxf(d0, -0.5f);
-  if (!(ob > 0.f) || !(od > 0.f)) return 0.f;
-  return (ob / (b1 - b0)) * (od / (d1 - d0));
-}
-__device__ __forceinline__ float dd_slab_length(const DdGeom& G, const DdView& W, int iu, int iv) {
-  float n2 = 0.f, da = 0.f;
+// Offsets, in voxels, from the voxel centre r (on the plane x_a = r_a) to the points where the rays source -> detector
+// point (u, v) meet that plane:  off_x(u, v) = (D_x E_a - E_x D_a) / (D_a v_x),  D = X(u, v) - s' (affine in u, v),
+// E = r - s'.  The 2 x 2 determinant of two nearly parallel vectors of ~1000 mm is a few hundred: it is expanded ONCE per
+// (voxel, view), in fp64, about a reference pixel (uc, vc) inside the voxel's window -
+//   det_x(u, v) = c_x + (u - uc) p_x + (v - vc) q_x,   D_a(u, v) = D_a(uc, vc) + (u - uc) U_a + (v - vc) V_a -
+// and its three coefficients are small numbers without cancellation left in them, so every boundary of every
+// candidate pixel is then two fp32 FMAs per function, a reciprocal and a product (no fp64 per pixel).
+struct DdLocal {
+  float Dc[3];            // D(uc, vc) along a, ub, vb
+  float U[3], V[3];       // detector steps along a, ub, vb
+  float cb, pb, qb;       // det along ub
+  float cd, pd, qd;       // det along vb
+  float Ea, ivb, ivd, va; // E_a; 1 / pitch along ub, vb; pitch along a
+};
+__device__ __forceinline__ DdLocal dd_local(const DdGeom& G, const DdView& W, const double* E, int uc, int vc) {
+  DdLocal q;
+  const int ax[3] = {W.a, W.ub, W.vb};
+  double D[3];
 #pragma unroll
-  for (int x = 0; x < 3; ++x) {
-    const float d = (float)(fma((double)iu, W.Uo[x], fma((double)iv, W.Vo[x], W.X00[x])) - W.so[x]);
-    n2 = fmaf(d, d, n2);
-    if (x == W.a) da = d;
+  for (int i = 0; i < 3; ++i) {
+    D[i] = fma((double)uc, W.Uo[ax[i]], fma((double)vc, W.Vo[ax[i]], W.X00[ax[i]])) - W.so[ax[i]];
+    q.Dc[i] = (float)D[i]; q.U[i] = (float)W.Uo[ax[i]]; q.V[i] = (float)W.Vo[ax[i]];
   }
-  return (float)G.v[W.a] * sqrtf(n2) / fabsf(da);
+  const double Ea = E[W.a], Eb = E[W.ub], Ed = E[W.vb];
+  q.cb = (float)fma(D[1], Ea, -Eb * D[0]);
+  q.pb = (float)fma(W.Uo[W.ub], Ea, -Eb * W.Uo[W.a]);
+  q.qb = (float)fma(W.Vo[W.ub], Ea, -Eb * W.Vo[W.a]);
+  q.cd = (float)fma(D[2], Ea, -Ed * D[0]);
+  q.pd = (float)fma(W.Uo[W.vb], Ea, -Ed * W.Uo[W.a]);
+  q.qd = (float)fma(W.Vo[W.vb], Ea, -Ed * W.Vo[W.a]);
+  q.Ea = (float)Ea; q.ivb = 1.0f / (float)G.v[W.ub]; q.ivd = 1.0f / (float)G.v[W.vb]; q.va = (float)G.v[W.a];
+  return q;
+}
+// offset along ub (AXIS 0) or vb (AXIS 1) at the detector point (uc + du, vc + dv); *front: t = E_a / D_a > 0
+template <int AXIS>
+__device__ __forceinline__ float dd_off(const DdLocal& q, float du, float dv, bool* front) {
+  const float Da = fmaf(du, q.U[0], fmaf(dv, q.V[0], q.Dc[0]));
+  const float det = AXIS == 0 ? fmaf(du, q.pb, fmaf(dv, q.qb, q.cb)) : fmaf(du, q.pd, fmaf(dv, q.qd, q.cd));
+  *front = q.Ea * Da > 0.f;
+  return det * fast_rcp(Da) * (AXIS == 0 ? q.ivb : q.ivd);
+}
+// normalised overlap of the footprint [x0, x1] (either order) with the voxel's cell [-1/2, 1/2]; 0 if none
+__device__ __forceinline__ float dd_cell_overlap(float x0, float x1) {
+  const float lo = fminf(x0, x1), hi = fmaxf(x0, x1);
+  const float o = fminf(hi, 0.5f) - fmaxf(lo, -0.5f);
+  return (o > 0.f && hi > lo) ? o / (hi - lo) : 0.f;
+}
+// slab length v_a / |e_a| of the pixel-centre ray at (uc + du, vc + dv)
+__device__ __forceinline__ float dd_slab_length(const DdLocal& q, float du, float dv) {
+  const float d0 = fmaf(du, q.U[0], fmaf(dv, q.V[0], q.Dc[0])), d1 = fmaf(du, q.U[1], fmaf(dv, q.V[1], q.Dc[1])),
+              d2 = fmaf(du, q.U[2], fmaf(dv, q.V[2], q.Dc[2]));
+  return q.va * sqrtf(fmaf(d0, d0, fmaf(d1, d1, d2 * d2))) * fast_rcp(fabsf(d0));
 }
 
 // Candidate pixels of a voxel: the detector bounding box of its cell's four corners on the plane (fp32: the box gets
@@ -289,22 +303,37 @@ __global__ void __launch_bounds__(kDdBpThreads) dd_bp_kernel(DdGeom G, int n_vie
       const float rc[3] = {rx, ry, rz};
       const DdWindow win = dd_window(G, W, Pl, rc);
       const float* img = proj + (size_t)view * G.nu * G.nv;
-      for (int iv = win.v0; iv <= win.v1; ++iv)
-        for (int iu = win.u0; iu <= win.u1; ++iu) {
-          const float o = dd_overlap(G, W, iu, iv, E);
-          if (!(o > 0.f)) continue;
-          const double wgt = (double)(dd_slab_length(G, W, iu, iv) * o);
-          if (!GRAD) {
-            acc = fma(wgt, (double)__ldg(img + (size_t)iv * G.nu + iu), acc);
-          } else {
-            const float lp = iu + 1 < G.nu ? __ldg(img + (size_t)iv * G.nu + iu + 1) : 0.f;
-            const float lm = iu > 0 ? __ldg(img + (size_t)iv * G.nu + iu - 1) : 0.f;
-            const float tp = iv + 1 < G.nv ? __ldg(img + (size_t)(iv + 1) * G.nu + iu) : 0.f;
-            const float tm = iv > 0 ? __ldg(img + (size_t)(iv - 1) * G.nu + iu) : 0.f;
-            su = fma(wgt, 0.5 * ((double)lp - (double)lm), su);
-            sv = fma(wgt, 0.5 * ((double)tp - (double)tm), sv);
+      if (win.u0 <= win.u1 && win.v0 <= win.v1) {
+        const int uc = (win.u0 + win.u1) >> 1, vc = (win.v0 + win.v1) >> 1;
+        const DdLocal q = dd_local(G, W, E, uc, vc);
+        for (int iv = win.v0; iv <= win.v1; ++iv) {
+          const float dv = (float)(iv - vc);
+          bool fl, fr, f2, f3;
+          float bl = dd_off<0>(q, (float)(win.u0 - uc) - 0.5f, dv, &fl);      // the left boundary of the row's first pixel
+          for (int iu = win.u0; iu <= win.u1; ++iu) {
+            const float du = (float)(iu - uc);
+            const float br = dd_off<0>(q, du + 0.5f, dv, &fr);                // shared with the next pixel
+            const float ob = dd_cell_overlap(bl, br);
+            const bool fb = fl && fr;
+            bl = br; fl = fr;
+            if (!(ob > 0.f) || !fb) continue;
+            const float d0 = dd_off<1>(q, du, dv - 0.5f, &f2), d1 = dd_off<1>(q, du, dv + 0.5f, &f3);
+            const float od = dd_cell_overlap(d0, d1);
+            if (!(od > 0.f) || !(f2 && f3)) continue;
+            const double wgt = (double)(dd_slab_length(q, du, dv) * ob * od);
+            if (!GRAD) {
+              acc = fma(wgt, (double)__ldg(img + (size_t)iv * G.nu + iu), acc);
+            } else {
+              const float lp = iu + 1 < G.nu ? __ldg(img + (size_t)iv * G.nu + iu + 1) : 0.f;
+              const float lm = iu > 0 ? __ldg(img + (size_t)iv * G.nu + iu - 1) : 0.f;
+              const float tp = iv + 1 < G.nv ? __ldg(img + (size_t)(iv + 1) * G.nu + iu) : 0.f;
+              const float tm = iv > 0 ? __ldg(img + (size_t)(iv - 1) * G.nu + iu) : 0.f;
+              su = fma(wgt, 0.5 * ((double)lp - (double)lm), su);
+              sv = fma(wgt, 0.5 * ((double)tp - (double)tm), sv);
+            }
           }
         }
+      }
     }
     if (GRAD) {
       float s6[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};

@@ -105,6 +105,9 @@ __device__ __forceinline__ void tma_pixel(int bx, int by, int& iu, int& iv, int&
   iu = bx * T::TU + (warp % WU) * T::PU + (pix % T::PU);
   iv = by * T::TV + (warp / WU) * T::PV + (pix / T::PU);
 }
+#ifndef DFP_ORIGIN_PRE
+#define DFP_ORIGIN_PRE 2         // bit 0: forward, bit 1: gradient kernels take the next box origin before the barrier
+#endif
 constexpr int kMaxStages = 2;
 constexpr float kBoxMargin = 0.05f;                    // voxels: sagitta of the tile + fp32 rounding
 constexpr int kBoxAlignLoss = 3;                       // x cells lost to the 16-byte alignment of the box origin
@@ -153,28 +156,51 @@ struct TmaBlock {              // block-wide state in shared memory
   double orgd[kMaxStages][3];  // the same as doubles (one conversion by the issuing thread instead of one per thread)
 };
 
-// One chunk's box: origin (voxel indices, for the TMA) of the stage it lands in.
+// One chunk's box: centred index of its first cell along each axis, from the tile's four corner rays at the chunk's
+// first and last sample.  Called by ALL 32 LANES of a warp (lane -> axis, corner ray, end of the chunk; shuffles for the
+// minimum): the origin of the next chunk is then ready in lane 0's registers BEFORE the block's "empty" barrier, and
+// the serial section between the barrier and the TMA issue shrinks to the six stores and the issue itself.
 template <int MODE, int SHAPE>
-__device__ __forceinline__ void issue_chunk(const VolLayout& L, TmaBlock& B, const CUtensorMap* map, int chunk,
-                                            unsigned tiles_addr, unsigned bar_addr) {
-  using S = BoxShape<SHAPE>;
+__device__ __forceinline__ void chunk_origin(const VolLayout& L, const TmaBlock& B, int chunk, int* oc) {
   constexpr int GRAD = MODE == 4 ? 0 : MODE;
-  constexpr int kWords = S::X * S::Y * S::Z;
-  const int s = chunk % S::STAGES;
+  const int lane = threadIdx.x & 31;
+  const int a = min(lane >> 3, 2), r = (lane >> 1) & 3;
+  const int k0 = B.kA + chunk * B.Kc;
+  const int k1 = min(k0 + B.Kc, B.kB) - 1;
+  float lo = fmaf((float)((lane & 1) ? k1 : k0), B.dp[r][a], B.pm[r][a]);
+#pragma unroll
+  for (int o = 1; o < 8; o <<= 1) lo = fminf(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+  const int o_ = (int)floorf(lo - 0.5f - kBoxMargin) - (GRAD ? 1 : 0);      // centred index of the box's first cell
+  oc[0] = __shfl_sync(0xffffffffu, o_, 0);
+  oc[1] = __shfl_sync(0xffffffffu, o_, 8);
+  oc[2] = __shfl_sync(0xffffffffu, o_, 16);
+  // the TMA unit wants the innermost coordinate on a 16-byte boundary (measured on B200: an x origin that is
+  // not a multiple of 4 floats raises an illegal-instruction fault): round the x origin down, kBoxAlignLoss
+  oc[0] = (((oc[0] + L.hx) >> 2) << 2) - L.hx;
+}
+// The same by ONE thread (forward kernels: after the barrier, measured faster there than the warp-wide version).
+template <int MODE, int SHAPE>
+__device__ __forceinline__ void chunk_origin_serial(const VolLayout& L, const TmaBlock& B, int chunk, int* oc) {
+  constexpr int GRAD = MODE == 4 ? 0 : MODE;
   const int k0 = B.kA + chunk * B.Kc;
   const int k1 = min(k0 + B.Kc, B.kB) - 1;
   const float f0 = (float)k0, f1 = (float)k1;
-  int oc[3];
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
     float lo = 3.0e38f;
 #pragma unroll
     for (int r = 0; r < 4; ++r) lo = fminf(lo, fminf(fmaf(f0, B.dp[r][a], B.pm[r][a]), fmaf(f1, B.dp[r][a], B.pm[r][a])));
-    oc[a] = (int)floorf(lo - 0.5f - kBoxMargin) - (GRAD ? 1 : 0);      // centred index of the box's first cell
+    oc[a] = (int)floorf(lo - 0.5f - kBoxMargin) - (GRAD ? 1 : 0);
   }
-  // the TMA unit wants the innermost coordinate on a 16-byte boundary (measured on B200: an x origin that is
-  // not a multiple of 4 floats raises an illegal-instruction fault): round the x origin down, kBoxAlignLoss
   oc[0] = (((oc[0] + L.hx) >> 2) << 2) - L.hx;
+}
+// One thread: publish the origin of the stage the chunk lands in and issue its TMA load.
+template <int SHAPE>
+__device__ __forceinline__ void issue_chunk(const VolLayout& L, TmaBlock& B, const CUtensorMap* map, int chunk,
+                                            const int* oc, unsigned tiles_addr, unsigned bar_addr) {
+  using S = BoxShape<SHAPE>;
+  constexpr int kWords = S::X * S::Y * S::Z;
+  const int s = chunk % S::STAGES;
   B.org[s][0] = oc[0]; B.org[s][1] = oc[1]; B.org[s][2] = oc[2];
   B.orgd[s][0] = (double)oc[0]; B.orgd[s][1] = (double)oc[1]; B.orgd[s][2] = (double)oc[2];
   const unsigned bar = bar_addr + 8u * s;
@@ -220,12 +246,17 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
       const int n_chunks = (B.kB - B.kA + Kc - 1) / Kc;
 #pragma unroll
       for (int c = 0; c < S::STAGES; ++c)
-        if (c < n_chunks) issue_chunk<MODE, SHAPE>(G.L, B, map, c, tiles_addr, bar_addr);
+        if (c < n_chunks) {
+          int oc[3];
+          chunk_origin_serial<MODE, SHAPE>(G.L, B, c, oc);
+          issue_chunk<SHAPE>(G.L, B, map, c, oc, tiles_addr, bar_addr);
+        }
     }
   }
   __syncthreads();
   const int Kc = B.Kc, kA = B.kA, kB = B.kB;
   const int n_chunks = Kc > 0 ? (kB - kA + Kc - 1) / Kc : 0;
+  const bool warp0 = threadIdx.x < 32;
   const int kend = r.k0 + r.n;
   const float dpx = (float)r.dp[0], dpy = (float)r.dp[1], dpz = (float)r.dp[2];
   const float2 dpxy = make_float2(dpx, dpy);
@@ -368,9 +399,19 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
       kf += (float)SLOTS;
       jf += (float)SLOTS;
     }
+    // The origin of the chunk that will reuse this stage.  Gradient kernels: warp 0 works it out BEFORE it joins the
+    // barrier (the serial section after the barrier is then the six stores and the issue: C5 903 -> 893 ms); forward
+    // kernels: thread 0, after the barrier (a chunk is 4x shorter there, and 20 more instructions in one warp ahead of
+    // the barrier hold up the other seven: 305 against 295 ms).
+    constexpr bool kPre = (DFP_ORIGIN_PRE >> (GRAD ? 1 : 0)) & 1;
+    int oc[3] = {0, 0, 0};
+    const bool more = chunk + S::STAGES < n_chunks;
+    if (kPre && warp0 && more) chunk_origin<MODE, SHAPE>(G.L, B, chunk + S::STAGES, oc);
     __syncthreads();                                   // every thread is done with stage s ("empty")
-    if (threadIdx.x == 0 && chunk + S::STAGES < n_chunks)
-      issue_chunk<MODE, SHAPE>(G.L, B, map, chunk + S::STAGES, tiles_addr, bar_addr);
+    if (threadIdx.x == 0 && more) {
+      if (!kPre) chunk_origin_serial<MODE, SHAPE>(G.L, B, chunk + S::STAGES, oc);
+      issue_chunk<SHAPE>(G.L, B, map, chunk + S::STAGES, oc, tiles_addr, bar_addr);
+    }
   }
   if (!GRAD) {
     acc[0] = sum;
