@@ -324,7 +324,7 @@ cudaError_t ensure_smem_attributes() {
 
 // ---- workspace carving ---------------------------------------------------------------------------
 struct FwdWs {
-  size_t off_views, off_dd, off_con, off_pvol, off_part, total;
+  size_t off_views, off_dd, off_con, off_pvol, off_part, off_fixed, total;
   int gx, gy;     // blocks per view (16 x 16-pixel tiles)
   int gy8;        // rows of 16 x 8-pixel tiles (TMA gradient kernel)
 };
@@ -344,6 +344,8 @@ FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad, int nset = 1) {
     if (g.flags & DFP_FLAG_SF) nblk = ((size_t)g.nx * g.ny * g.nz + kSfThreads - 1) / kSfThreads;   // sf_kernel blocks
     w.off_part = o;  o += grad ? align_up(sizeof(float) * 6 * (size_t)nset * V * nblk) : 0;
   }
+  // sf_kernel<0>: SfFixed (256 bytes) + the 64-bit fixed-point accumulator image
+  w.off_fixed = o; o += ((g.flags & DFP_FLAG_SF) && !grad) ? align_up(256 + sizeof(long long) * (size_t)V * g.nu * g.nv) : 0;
   w.total = o;
   return w;
 }
@@ -447,14 +449,19 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
     const unsigned nblk = (unsigned)(((size_t)g->nx * g->ny * g->nz + kSfThreads - 1) / kSfThreads);
     g_path = DFP_PATH_GATHER;
     if (!grad) {
-      DFP_CUDA(cudaMemsetAsync(d_out, 0, sizeof(float) * (size_t)V * g->nu * g->nv, s), "cudaMemsetAsync");
+      const size_t npix = (size_t)V * g->nu * g->nv, nvox = (size_t)g->nx * g->ny * g->nz;
+      SfFixed* fx = reinterpret_cast<SfFixed*>(base + w.off_fixed);
+      long long* acc = reinterpret_cast<long long*>(base + w.off_fixed + 256);
+      DFP_CUDA(cudaMemsetAsync(fx, 0, 256 + sizeof(long long) * npix, s), "cudaMemsetAsync");
+      sf_maxabs_kernel<<<grid_1d(nvox, 256), 256, 0, s>>>(d_vol, nvox, fx);
       time_begin(s);
-      sf_kernel<0><<<nblk, kSfThreads, 0, s>>>(DG, V, 0, ddv, d_vol, nullptr, nullptr, d_out);
+      sf_kernel<0><<<nblk, kSfThreads, 0, s>>>(DG, V, 0, ddv, d_vol, nullptr, nullptr, fx, reinterpret_cast<float*>(acc));
       time_end(s);
-      g_launches = 1;
+      sf_fixed_to_float_kernel<<<grid_1d(npix, 256), 256, 0, s>>>(DG, acc, fx, npix, d_out);
+      g_launches = 3;
     } else {
       time_begin(s);
-      sf_kernel<2><<<nblk, kSfThreads, 0, s>>>(DG, V, 0, ddv, d_vol, d_up, nullptr, part);
+      sf_kernel<2><<<nblk, kSfThreads, 0, s>>>(DG, V, 0, ddv, d_vol, d_up, nullptr, nullptr, part);
       time_end(s);
       fwd_contract_kernel<<<V, 256, 0, s>>>((int)nblk, part, dc, d_out);
       g_launches = 2;
@@ -670,11 +677,11 @@ int run_backproject_slice(const dfp_geometry* g, int V, const float* angles, con
     const unsigned nblk = (unsigned)(((size_t)g->nx * g->ny * g->nz + kSfThreads - 1) / kSfThreads);
     time_begin(s);
     if (!grad) {
-      sf_kernel<1><<<nblk, kSfThreads, 0, s>>>(DG, V, (g->flags & DFP_FLAG_ACCUMULATE) ? 1 : 0, ddv, nullptr, d_proj, nullptr, d_out);
+      sf_kernel<1><<<nblk, kSfThreads, 0, s>>>(DG, V, (g->flags & DFP_FLAG_ACCUMULATE) ? 1 : 0, ddv, nullptr, d_proj, nullptr, nullptr, d_out);
       time_end(s);
       g_launches = 1;
     } else {
-      sf_kernel<3><<<nblk, kSfThreads, 0, s>>>(DG, V, 0, ddv, nullptr, d_proj, d_up, part);
+      sf_kernel<3><<<nblk, kSfThreads, 0, s>>>(DG, V, 0, ddv, nullptr, d_proj, d_up, nullptr, part);
       time_end(s);
       bp_contract_kernel<<<V, 256, 0, s>>>((int)nblk, V, part, dc, d_out);
       g_launches = 2;

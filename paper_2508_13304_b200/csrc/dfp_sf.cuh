@@ -4,11 +4,12 @@
 //   widths wu_k = |J_uk| v_k, wv_k = |J_vk| v_k;  T(u), R(v) = unit-area trapezoids from the two widest rects of each axis;
 //   a^ij = v_x v_y v_z sqrt(det J J^T) * int_pixel T du * int_pixel R dv.
 // One thread per voxel, the views inside (the footprint of a (voxel, view) is computed once and serves every pixel it
-// covers; the volume is written once; per-view 6-vectors are reduced per block).  fp64 for the footprint (a weight is
-// a difference of trapezoid integrals at u_j -+ a few pixels).
-//   MODE 0  forward     l_i += a^ij mu_j         scatter with atomicAdd (fp32; the paper's own kernels accumulate with
-//                                                atomics, :207) into the zeroed projections - the one non-deterministic
-//                                                summation order of the library, at the 1e-7 level
+// covers; the volume is written once; per-view 6-vectors are reduced per block).  The projected centre is taken in
+// fp64 and split into a reference pixel + an offset; the trapezoid integrals are fp32 about that origin.
+//   MODE 0  forward     l_i += a^ij mu_j         scatter (the paper's own kernels accumulate with atomics, :207) as
+//                                                64-bit FIXED-POINT integer atomics into a zeroed accumulator image:
+//                                                integer sums do not depend on the order, so the call is deterministic
+//                                                like the rest of the library; sf_fixed_to_float_kernel finishes it
 //   MODE 1  back        mu_j = sum_i a^ij l_i    gather: the exact transpose
 //   MODE 2  forward pose gradient  sum_j (A^T w)_j G_f^j, G_f^j per voxel (Eq.19-20): gather the upstream image
 //   MODE 3  back pose gradient     sum_ij a^ij w_j (D_u^i J_u(r_j) + D_v^i J_v(r_j))   (Eq.22, per-pixel G_b^i)
@@ -19,55 +20,99 @@
 
 namespace dfp {
 
-// int_{-inf}^{x} of the unit-area trapezoid centred at c with base b >= top t >= 0
-__device__ __forceinline__ double sf_cdf(double c, double b, double t, double x) {
-  const double h = 2.0 / (b + t);
-  const double x0 = c - 0.5 * b, x1 = c - 0.5 * t, x2 = c + 0.5 * t, x3 = c + 0.5 * b;
-  double s = h * (fmin(fmax(x, x1), x2) - x1);
-  if (x1 > x0) { const double r = fmin(fmax(x, x0), x1) - x0; s += h * r * r / (2.0 * (x1 - x0)); }
-  if (x3 > x2) { const double r = fmin(fmax(x, x2), x3) - x2; s += h * (r - r * r / (2.0 * (x3 - x2))); }
-  return s;
+// Unit-area trapezoid with base b >= top t >= 0 about its centre: half widths, height 2 / (b + t), 1 / (b - t).
+struct SfTrap { float hb, ht, h, rr; };
+__device__ __forceinline__ SfTrap sf_trap(float w0, float w1, float w2) {
+  // base = sum, top = difference of the two widest of the three rects' widths
+  const float hi = fmaxf(w0, fmaxf(w1, w2)), lo = fminf(w0, fminf(w1, w2)), mid = (w0 + w1 + w2) - hi - lo;
+  SfTrap T;
+  T.hb = 0.5f * (hi + mid); T.ht = 0.5f * (hi - mid);
+  T.h = fast_rcp(T.hb + T.ht);
+  T.rr = mid > 0.f ? fast_rcp(2.f * mid) : 0.f;          // 1 / (2 (x1 - x0)) = 1 / (b - t), b - t = 2 mid
+  return T;
 }
-__device__ __forceinline__ void sf_two_widest(double a, double b, double c, double* base, double* top) {
-  const double hi = fmax(a, fmax(b, c)), lo = fmin(a, fmin(b, c)), mid = a + b + c - hi - lo;
-  *base = hi + mid; *top = hi - mid;
+// int_{-inf}^{x} of the trapezoid, x measured from its centre
+__device__ __forceinline__ float sf_cdf(const SfTrap& T, float x) {
+  const float c = fminf(fmaxf(x, -T.ht), T.ht) + T.ht;           // flat top
+  const float r = fminf(fmaxf(x, -T.hb), -T.ht) + T.hb;          // rising ramp
+  const float q = fminf(fmaxf(x, T.ht), T.hb) - T.ht;            // falling ramp
+  return T.h * (c + fmaf(r * r, T.rr, fmaf(-q * q, T.rr, q)));
 }
 
-struct SfFoot {                 // footprint of one (voxel, view)
-  double uj, vj, bu, tu, bv, tv, M;
-  double Ju[3], Jv[3];
+// Footprint of one (voxel, view).  The projected centre is taken in fp64 and kept as a reference pixel (uc, vc) plus
+// an offset |.| <= 1/2 (a weight is a difference of trapezoid integrals a few pixels from the centre: with the centre
+// as the origin everything after it is fp32 at ~1e-7 of the weight).
+struct SfFoot {
+  float du, dv;           // (u_j - uc, v_j - vc)
+  int uc, vc;
+  SfTrap Tu, Tv;
+  float M;
+  float Ju[3], Jv[3];
   int iu0, iu1, iv0, iv1;
   bool ok;
 };
-__device__ __forceinline__ SfFoot sf_footprint(const DdGeom& G, const double (*E)[4], const double* r) {
+__device__ __forceinline__ SfFoot sf_footprint(const DdGeom& G, const double (*E)[4], const float (*Ef)[4], const double* r) {
   SfFoot f;
   const double up = fma(E[0][0], r[0], fma(E[0][1], r[1], fma(E[0][2], r[2], E[0][3])));
   const double vp = fma(E[1][0], r[0], fma(E[1][1], r[1], fma(E[1][2], r[2], E[1][3])));
   const double wp = fma(E[2][0], r[0], fma(E[2][1], r[1], fma(E[2][2], r[2], E[2][3])));
-  f.ok = wp > 0.0;
-  const double rw = 1.0 / wp;
-  f.uj = up * rw; f.vj = vp * rw;
-  double wu[3], wv[3];
+  const float wf = (float)wp;
+  f.ok = wf > 0.f;
+  const float rw = fast_rcp(wf);
+  const float ucf = rintf((float)up * rw), vcf = rintf((float)vp * rw);
+  f.ok = f.ok && fabsf(ucf) < 1e9f && fabsf(vcf) < 1e9f;
+  f.uc = f.ok ? (int)ucf : 0; f.vc = f.ok ? (int)vcf : 0;
+  f.du = (float)fma(-(double)f.uc, wp, up) * rw;
+  f.dv = (float)fma(-(double)f.vc, wp, vp) * rw;
+  const float uj = (float)f.uc + f.du, vj = (float)f.vc + f.dv;
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
-    f.Ju[k] = (E[0][k] - E[2][k] * f.uj) * rw;          // Eq.13: (P_1k w' - P_3k u') / w'^2
-    f.Jv[k] = (E[1][k] - E[2][k] * f.vj) * rw;
-    wu[k] = fabs(f.Ju[k]) * G.v[k]; wv[k] = fabs(f.Jv[k]) * G.v[k];
+    f.Ju[k] = (Ef[0][k] - Ef[2][k] * uj) * rw;          // Eq.13: (P_1k w' - P_3k u') / w'^2
+    f.Jv[k] = (Ef[1][k] - Ef[2][k] * vj) * rw;
   }
-  const double guu = f.Ju[0] * f.Ju[0] + f.Ju[1] * f.Ju[1] + f.Ju[2] * f.Ju[2];
-  const double gvv = f.Jv[0] * f.Jv[0] + f.Jv[1] * f.Jv[1] + f.Jv[2] * f.Jv[2];
-  const double guv = f.Ju[0] * f.Jv[0] + f.Ju[1] * f.Jv[1] + f.Ju[2] * f.Jv[2];
-  f.M = G.v[0] * G.v[1] * G.v[2] * sqrt(fmax(guu * gvv - guv * guv, 0.0));
-  sf_two_widest(wu[0], wu[1], wu[2], &f.bu, &f.tu);
-  sf_two_widest(wv[0], wv[1], wv[2], &f.bv, &f.tv);
-  if (!(f.bu > 0.0) || !(f.bv > 0.0) || !(f.M > 0.0) || !(f.bu < 1e6) || !(f.bv < 1e6)) f.ok = false;
+  const float guu = f.Ju[0] * f.Ju[0] + f.Ju[1] * f.Ju[1] + f.Ju[2] * f.Ju[2];
+  const float gvv = f.Jv[0] * f.Jv[0] + f.Jv[1] * f.Jv[1] + f.Jv[2] * f.Jv[2];
+  const float guv = f.Ju[0] * f.Jv[0] + f.Ju[1] * f.Jv[1] + f.Ju[2] * f.Jv[2];
+  f.M = G.vx * G.vy * G.vz * sqrtf(fmaxf(fmaf(guu, gvv, -guv * guv), 0.f));
+  f.Tu = sf_trap(fabsf(f.Ju[0]) * G.vx, fabsf(f.Ju[1]) * G.vy, fabsf(f.Ju[2]) * G.vz);
+  f.Tv = sf_trap(fabsf(f.Jv[0]) * G.vx, fabsf(f.Jv[1]) * G.vy, fabsf(f.Jv[2]) * G.vz);
+  if (!(f.Tu.hb > 0.f) || !(f.Tv.hb > 0.f) || !(f.M > 0.f) || !(f.Tu.hb < 1e6f) || !(f.Tv.hb < 1e6f)) f.ok = false;
   if (f.ok) {
-    f.iu0 = max((int)floor(f.uj - 0.5 * f.bu + 0.5), 0); f.iu1 = min((int)floor(f.uj + 0.5 * f.bu + 0.5), G.nu - 1);
-    f.iv0 = max((int)floor(f.vj - 0.5 * f.bv + 0.5), 0); f.iv1 = min((int)floor(f.vj + 0.5 * f.bv + 0.5), G.nv - 1);
+    f.iu0 = max(f.uc + (int)floorf(f.du - f.Tu.hb + 0.5f), 0); f.iu1 = min(f.uc + (int)floorf(f.du + f.Tu.hb + 0.5f), G.nu - 1);
+    f.iv0 = max(f.vc + (int)floorf(f.dv - f.Tv.hb + 0.5f), 0); f.iv1 = min(f.vc + (int)floorf(f.dv + f.Tv.hb + 0.5f), G.nv - 1);
   } else {
     f.iu0 = f.iv0 = 0; f.iu1 = f.iv1 = -1;
   }
   return f;
+}
+
+// MODE 0 sums its projections as 64-bit FIXED-POINT integers (integer addition is associative: the result does not
+// depend on the order the atomics land in, unlike an fp32 atomicAdd).  The scale 2^e is chosen on the device from the
+// largest |mu| (sf_maxabs_kernel) and the longest chord of the grid so that no pixel can overflow:
+//   |l_i| <= max|mu| sum_j a^ij,  sum_j a^ij ~ the chord of the pixel's ray <= the grid's diagonal (8x head-room).
+struct SfFixed { unsigned max_bits; unsigned pad; };
+__global__ void sf_maxabs_kernel(const float* __restrict__ vol, size_t n, SfFixed* __restrict__ fx) {
+  unsigned m = 0;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    m = max(m, __float_as_uint(fabsf(__ldg(vol + i))));          // |x| as bits: monotone, NaN above everything
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0 && m) atomicMax(&fx->max_bits, m);
+}
+__device__ __forceinline__ int sf_fixed_exponent(const DdGeom& G, unsigned max_bits) {
+  const float diag = sqrtf((float)G.n[0] * G.vx * (float)G.n[0] * G.vx + (float)G.n[1] * G.vy * (float)G.n[1] * G.vy +
+                           (float)G.n[2] * G.vz * (float)G.n[2] * G.vz);
+  int eb;
+  frexpf(__uint_as_float(max_bits) * diag * 8.f, &eb);           // bound < 2^eb
+  return 61 - eb;
+}
+__global__ void sf_fixed_to_float_kernel(DdGeom G, const long long* __restrict__ acc, const SfFixed* __restrict__ fx,
+                                         size_t n, float* __restrict__ out) {
+  const unsigned mb = fx->max_bits;
+  const bool bad = mb >= 0x7f800000u;                             // Inf / NaN in the volume
+  const double inv = mb && !bad ? scalbn(1.0, -sf_fixed_exponent(G, mb)) : 0.0;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    out[i] = bad ? __int_as_float(0x7fc00000) : (float)((double)acc[i] * inv);
 }
 
 constexpr int kSfThreads = 256;
@@ -77,6 +122,7 @@ __global__ void __launch_bounds__(kSfThreads) sf_kernel(DdGeom G, int n_views, i
                                                         const float* __restrict__ vol,      // MODE 0, 2: the volume
                                                         const float* __restrict__ img,      // MODE 1, 3: projections; 2: upstream
                                                         const float* __restrict__ upvol,    // MODE 3: upstream volume
+                                                        const SfFixed* __restrict__ fx,     // MODE 0: fixed-point scale
                                                         float* __restrict__ out) {
   const size_t nvox = (size_t)G.n[0] * G.n[1] * G.n[2];
   const size_t j = (size_t)blockIdx.x * kSfThreads + threadIdx.x;
@@ -84,7 +130,13 @@ __global__ void __launch_bounds__(kSfThreads) sf_kernel(DdGeom G, int n_views, i
   int xyz[3] = {0, 0, 0};
   if (live) { xyz[0] = (int)(j % G.n[0]); xyz[1] = (int)((j / G.n[0]) % G.n[1]); xyz[2] = (int)(j / ((size_t)G.n[0] * G.n[1])); }
   __shared__ double E[3][4];
+  __shared__ float Ef[3][4];
   __shared__ float red[kSfThreads / 32][6];
+  double fscale = 0.0;
+  if (MODE == 0) {
+    const unsigned mb = fx->max_bits;
+    if (mb && mb < 0x7f800000u) fscale = scalbn(1.0, sf_fixed_exponent(G, mb));
+  }
   double r[3];
 #pragma unroll
   for (int k = 0; k < 3; ++k) r[k] = G.c[k] + ((double)xyz[k] - G.h[k]) * G.v[k];
@@ -107,32 +159,44 @@ __global__ void __launch_bounds__(kSfThreads) sf_kernel(DdGeom G, int n_views, i
   double acc = (MODE == 1 && accumulate && live) ? (double)out[j] : 0.0;
   for (int view = 0; view < n_views; ++view) {
     __syncthreads();
-    if (threadIdx.x < 12) E[threadIdx.x >> 2][threadIdx.x & 3] = views[view].P[threadIdx.x >> 2][threadIdx.x & 3];
+    if (threadIdx.x < 12) {
+      const double e = views[view].P[threadIdx.x >> 2][threadIdx.x & 3];
+      E[threadIdx.x >> 2][threadIdx.x & 3] = e;
+      Ef[threadIdx.x >> 2][threadIdx.x & 3] = (float)e;
+    }
     __syncthreads();
     double s0 = 0.0, s1 = 0.0;
     SfFoot f;
     f.ok = false;
     if (work) {
-      f = sf_footprint(G, E, r);
+      f = sf_footprint(G, E, Ef, r);
       const size_t base = (size_t)view * G.nu * G.nv;
+      float cv0 = sf_cdf(f.Tv, (float)(f.iv0 - f.vc) - 0.5f - f.dv);          // rolling: the lower edge of the first row
       for (int iv = f.iv0; iv <= f.iv1; ++iv) {
-        const double fv = sf_cdf(f.vj, f.bv, f.tv, iv + 0.5) - sf_cdf(f.vj, f.bv, f.tv, iv - 0.5);
-        if (!(fv > 0.0)) continue;
+        const float cv1 = sf_cdf(f.Tv, (float)(iv - f.vc) + 0.5f - f.dv);
+        const float fv = cv1 - cv0;
+        cv0 = cv1;
+        if (!(fv > 0.f)) continue;
+        const float mv = f.M * fv;
+        float cu0 = sf_cdf(f.Tu, (float)(f.iu0 - f.uc) - 0.5f - f.du);
         for (int iu = f.iu0; iu <= f.iu1; ++iu) {
-          const double fu = sf_cdf(f.uj, f.bu, f.tu, iu + 0.5) - sf_cdf(f.uj, f.bu, f.tu, iu - 0.5);
-          if (!(fu > 0.0)) continue;
-          const double w = f.M * fu * fv;
+          const float cu1 = sf_cdf(f.Tu, (float)(iu - f.uc) + 0.5f - f.du);
+          const float fu = cu1 - cu0;
+          cu0 = cu1;
+          if (!(fu > 0.f)) continue;
+          const float w = mv * fu;
           const size_t pix = base + (size_t)iv * G.nu + iu;
           if (MODE == 0) {
-            atomicAdd(out + pix, (float)(w * (double)mu));
+            const long long q = __double2ll_rn((double)w * (double)mu * fscale);
+            atomicAdd(reinterpret_cast<unsigned long long*>(out) + pix, (unsigned long long)q);
           } else if (MODE == 1 || MODE == 2) {
-            s0 = fma(w, (double)__ldg(img + pix), s0);
+            s0 = fma((double)w, (double)__ldg(img + pix), s0);
           } else {
             const float* p = img + pix;
             const float lp = iu + 1 < G.nu ? __ldg(p + 1) : 0.f, lm = iu > 0 ? __ldg(p - 1) : 0.f;
             const float tp = iv + 1 < G.nv ? __ldg(p + G.nu) : 0.f, tm = iv > 0 ? __ldg(p - G.nu) : 0.f;
-            s0 = fma(w, 0.5 * ((double)lp - (double)lm), s0);
-            s1 = fma(w, 0.5 * ((double)tp - (double)tm), s1);
+            s0 = fma((double)w, 0.5 * ((double)lp - (double)lm), s0);
+            s1 = fma((double)w, 0.5 * ((double)tp - (double)tm), s1);
           }
         }
       }
@@ -146,9 +210,10 @@ __global__ void __launch_bounds__(kSfThreads) sf_kernel(DdGeom G, int n_views, i
           const float s = (float)s0;
           qx = s * gx; qy = s * gy; qz = s * gz;
         } else {                // w_j (su J_u + sv J_v), object frame
-          qx = wj * (float)(s0 * f.Ju[0] + s1 * f.Jv[0]);
-          qy = wj * (float)(s0 * f.Ju[1] + s1 * f.Jv[1]);
-          qz = wj * (float)(s0 * f.Ju[2] + s1 * f.Jv[2]);
+          const float a0 = (float)s0, a1 = (float)s1;
+          qx = wj * fmaf(a0, f.Ju[0], a1 * f.Jv[0]);
+          qy = wj * fmaf(a0, f.Ju[1], a1 * f.Jv[1]);
+          qz = wj * fmaf(a0, f.Ju[2], a1 * f.Jv[2]);
         }
         s6[0] = qx; s6[1] = qy; s6[2] = qz;
         s6[3] = ry * qz - rz * qy; s6[4] = rz * qx - rx * qz; s6[5] = rx * qy - ry * qx;
