@@ -95,9 +95,11 @@ typedef struct dfp_geometry {
                            bit8 (DFP_FLAG_SF): as bit7 with SEPARABLE-FOOTPRINT weights (PAPER.md :213, ref [29]) - per
                            (voxel, view) a separable footprint on the detector, trapezoids along u and v built from the
                            Jacobian of Eq.13 at the voxel centre, mass = voxel volume x area magnification (U16).
-                           dfp_forward accumulates with fp32 atomics (its results vary at the 1e-7 level from run to run;
-                           every other call of the library is bit-reproducible).  Same restrictions as bit7; not together
-                           with it.                                                                              */
+                           Same restrictions as bit7; not together with it.
+                           The two scattering calls (dfp_backproject with bit7, dfp_forward with bit8) add 64-bit
+                           fixed-point integers, whose sum does not depend on the order: like every other call of the
+                           library they are bit-reproducible.  A NaN / Inf in their input makes every element of
+                           their output NaN.                                                                     */
 } dfp_geometry;
 
 enum {

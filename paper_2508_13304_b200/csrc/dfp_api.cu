@@ -352,7 +352,7 @@ FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad, int nset = 1) {
 
 constexpr int kBpGradZChunk = 16;
 struct BpWs {
-  size_t off_views, off_viewsd, off_dd, off_con, off_q, off_part, total;
+  size_t off_views, off_viewsd, off_dd, off_con, off_q, off_part, off_fixed, total;
   int gx, gy, gz;  // voxel tiles (gather path)
   int tx, ty, tz;  // voxel tiles (TMA path)
 };
@@ -375,9 +375,12 @@ BpWs bp_ws(const dfp_geometry& g, int V, bool grad) {
   {
     const size_t t_gather = (size_t)w.gx * w.gy * w.gz, t_tma = (size_t)w.tx * w.ty * w.tz;
     size_t tiles = t_gather > t_tma ? t_gather : t_tma;
-    if (g.flags & (DFP_FLAG_DD | DFP_FLAG_SF)) tiles = ((size_t)g.nx * g.ny * g.nz + kDdBpThreads - 1) / kDdBpThreads;   // dd_bp / sf blocks
+    if (g.flags & DFP_FLAG_SF) tiles = ((size_t)g.nx * g.ny * g.nz + kSfThreads - 1) / kSfThreads;          // sf_kernel blocks
+    if (g.flags & DFP_FLAG_DD) tiles = (size_t)((g.nu + kFwdTU - 1) / kFwdTU) * ((g.nv + kFwdTV - 1) / kFwdTV);   // dd_kernel<3>: pixel tiles
     o += grad ? align_up(sizeof(float) * 6 * (size_t)V * tiles) : 0;
   }
+  // dd_kernel<2>: DdFixed (256 bytes) + the 64-bit fixed-point accumulator volume
+  w.off_fixed = o; o += ((g.flags & DFP_FLAG_DD) && !grad) ? align_up(256 + sizeof(long long) * (size_t)g.nx * g.ny * g.nz) : 0;
   w.total = o;
   return w;
 }
@@ -479,13 +482,13 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
     g_path = DFP_PATH_GATHER;
     time_begin(s);
     if (!grad) {
-      dd_fwd_kernel<0><<<grid, kFwdThreads, 0, s>>>(DG, ddv, d_vol, nullptr, GB, nullptr, d_out);
+      dd_kernel<0><<<grid, kFwdThreads, 0, s>>>(DG, ddv, d_vol, nullptr, GB, nullptr, nullptr, 0, d_out);
       time_end(s);
       g_launches = 1;
     } else {
       const int gb = (int)std::min<size_t>((GB.cells() + 255) / 256, (size_t)148 * 64);
       grad_volume_kernel<<<gb, 256, 0, s>>>(GB, G.sgx, G.sgy, G.sgz, d_vol, pvol);
-      dd_fwd_kernel<1><<<grid, kFwdThreads, 0, s>>>(DG, ddv, d_vol, pvol, GB, d_up, part);
+      dd_kernel<1><<<grid, kFwdThreads, 0, s>>>(DG, ddv, d_vol, pvol, GB, d_up, nullptr, 0, part);
       time_end(s);
       fwd_contract_kernel<<<V, 256, 0, s>>>(w.gx * w.gy, part, dc, d_out);
       g_launches = 3;
@@ -695,16 +698,40 @@ int run_backproject_slice(const dfp_geometry* g, int V, const float* angles, con
     DdView* ddv = reinterpret_cast<DdView*>(base + w.off_dd);
     DFP_CUDA(upload_async(ddv, hd.data(), sizeof(DdView) * V, s), "view upload");
     const DdGeom DG = make_dd_geom(*g);
-    const unsigned nblk = (unsigned)(((size_t)g->nx * g->ny * g->nz + kDdBpThreads - 1) / kDdBpThreads);
-    time_begin(s);
+    const dim3 grid((g->nu + kFwdTU - 1) / kFwdTU, (g->nv + kFwdTV - 1) / kFwdTV, V);
+    const GradBricks GB{};
     if (!grad) {
-      dd_bp_kernel<0><<<nblk, kDdBpThreads, 0, s>>>(DG, V, (g->flags & DFP_FLAG_ACCUMULATE) ? 1 : 0, ddv, dv, d_proj, nullptr, d_out);
+      // fixed-point head-room: sum_i a^ij <= (pixels of the call) x the longest slab length v_a / |e_a| (a normalised
+      // overlap is <= 1); |e_a| is smallest at a detector corner
+      double Lmax = 0.0;
+      for (int v = 0; v < V; ++v) {
+        const DdView& D = hd[v];
+        double cmin = 1.0;
+        for (int c = 0; c < 4; ++c) {
+          const double u = (c & 1) ? g->nu - 0.5 : -0.5, vv = (c & 2) ? g->nv - 0.5 : -0.5;
+          double d[3], n2 = 0.0;
+          for (int x = 0; x < 3; ++x) { d[x] = D.X00[x] + u * D.Uo[x] + vv * D.Vo[x] - D.so[x]; n2 += d[x] * d[x]; }
+          cmin = std::min(cmin, std::fabs(d[D.a]) / std::sqrt(n2 > 0 ? n2 : 1.0));
+        }
+        const double va = D.a == 0 ? g->vx : (D.a == 1 ? g->vy : g->vz);
+        Lmax = std::max(Lmax, va / std::max(cmin, 1e-6));
+      }
+      const int hb = (int)std::ceil(std::log2(Lmax * (double)g->nu * g->nv * V)) + 1;
+      const size_t npix = (size_t)V * g->nu * g->nv, nvox = (size_t)g->nx * g->ny * g->nz;
+      DdFixed* fx = reinterpret_cast<DdFixed*>(base + w.off_fixed);
+      long long* acc = reinterpret_cast<long long*>(base + w.off_fixed + 256);
+      DFP_CUDA(cudaMemsetAsync(fx, 0, 256 + sizeof(long long) * nvox, s), "cudaMemsetAsync");
+      dd_maxabs_kernel<<<grid_1d(npix, 256), 256, 0, s>>>(d_proj, npix, fx);
+      time_begin(s);
+      dd_kernel<2><<<grid, kFwdThreads, 0, s>>>(DG, ddv, nullptr, nullptr, GB, d_proj, fx, hb, reinterpret_cast<float*>(acc));
       time_end(s);
-      g_launches = 1;
+      dd_fixed_to_float_kernel<<<grid_1d(nvox, 256), 256, 0, s>>>(acc, fx, hb, nvox, (g->flags & DFP_FLAG_ACCUMULATE) ? 1 : 0, d_out);
+      g_launches = 3;
     } else {
-      dd_bp_kernel<1><<<nblk, kDdBpThreads, 0, s>>>(DG, V, 0, ddv, dv, d_proj, d_up, part);
+      time_begin(s);
+      dd_kernel<3><<<grid, kFwdThreads, 0, s>>>(DG, ddv, d_up, nullptr, GB, d_proj, nullptr, 0, part);
       time_end(s);
-      bp_contract_kernel<<<V, 256, 0, s>>>((int)nblk, V, part, dc, d_out);
+      bp_contract_kernel<<<V, 256, 0, s>>>((int)(grid.x * grid.y), V, part, dc, d_out);
       g_launches = 2;
     }
     DFP_CUDA(cudaGetLastError(), "back-projection launch (distance-driven weights)");

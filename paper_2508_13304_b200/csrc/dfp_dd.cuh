@@ -7,17 +7,21 @@
 // continuous voxel indices they bound the pixel's footprint [B0, B1] x [D0, D1];
 //   a^ij = L (|[B0,B1] n cell(jb)| / (B1 - B0)) (|[D0,D1] n cell(jd)| / (D1 - D0)),  L = v_a / |e'_a| (pixel-centre ray).
 // A boundary position is AFFINE in the plane index k (position = s' + (x_a - s'_a) dir / dir_a), so a pixel carries
-// four (start, increment) pairs; they and the overlaps are taken in fp64 (a weight is a difference of positions of
-// magnitude n/2: fp32 would leave 1e-5 relative error per weight) - the kernels of this "next" row are arithmetic-light
-// per voxel read and are measured beside the trilinear ones in DESIGN.md.
-//   dd_fwd_kernel        l_i = sum_j a^ij mu_j                                  one thread per pixel
-//   dd_fwd_grad_kernel   A_i = sum_j a^ij g_j, B_i = sum_j a^ij r'_j x g_j      per-voxel G_f^j (Eq.19-20), g_j from the
-//                        per-voxel gradient volume of grad_volume_kernel
-//   dd_bp_kernel         mu_j = sum_i a^ij l_i, the EXACT transpose (Eq.21)     one thread per voxel: the pixels whose
-//                        footprint can meet the voxel's cell are found by projecting the cell's corners onto the
-//                        detector, each candidate's weight is then the forward formula
-//   dd_bp_grad_kernel    sum_ij a^ij w_j (D_u^i J_u(r_j) + D_v^i J_v(r_j))      per-pixel G_b^i (Eq.22), D = central
-//                        differences of the zero-extended projection, J = Eq.13 at the voxel centre
+// four (start, increment) pairs in fp64 (a weight is a difference of positions of magnitude n/2: fp32 would leave 1e-5
+// relative error per weight); per plane the four positions are re-based onto the first cell they touch and the overlaps
+// are fp32 on numbers of order one.
+// ALL FOUR operations are pixel-driven and share one traversal (dd_kernel<MODE>: one thread per pixel, the planes
+// inside; a footprint narrower than a voxel - every BASELINE config - takes a loop-free 2 x 2 path):
+//   MODE 0  l_i = sum_j a^ij mu_j
+//   MODE 1  A_i = sum_j a^ij g_j, B_i = sum_j a^ij r'_j x g_j       per-voxel G_f^j (Eq.19-20), g_j from the per-voxel
+//           gradient volume of grad_volume_kernel
+//   MODE 2  mu_j = sum_i a^ij l_i, the EXACT transpose (Eq.21): the forward traversal with the read turned into a
+//           SCATTER (the same a^ij by construction).  The scatter adds 64-bit FIXED-POINT integers (as the SF forward
+//           projector, dfp_sf.cuh): integer sums do not depend on the order, so the call is deterministic; the scale
+//           follows max|l| (found on the device) and a host bound on sum_i a^ij
+//   MODE 3  sum_ij a^ij w_j (D_u^i J_u(r_j) + D_v^i J_v(r_j))       per-pixel G_b^i (Eq.22), D = central differences of
+//           the zero-extended projection, J = Eq.13 at the voxel centre; a sum over (i, j) pairs, taken per pixel in
+//           registers like MODE 1 - no scatter
 #pragma once
 #include <cuda_runtime.h>
 
@@ -40,20 +44,7 @@ inline DdGeom make_dd_geom(const dfp_geometry& g) {
   return G;
 }
 
-// Continuous voxel index, along axis `ax`, of the point where the ray source -> detector point (u, v) meets the plane
-// x_a = xa; false if the plane is not in front of the source along that ray.
-__device__ __forceinline__ bool dd_hit(const DdGeom& G, const DdView& W, double u, double v, double xa, int ax,
-                                       double* idx) {
-  const int a = W.a;
-  const double da = fma(u, W.Uo[a], fma(v, W.Vo[a], W.X00[a])) - W.so[a];
-  const double dx = fma(u, W.Uo[ax], fma(v, W.Vo[ax], W.X00[ax])) - W.so[ax];
-  if (fabs(da) < 1e-300) return false;
-  const double t = (xa - W.so[a]) / da;
-  *idx = (fma(t, dx, W.so[ax]) - G.c[ax]) / G.v[ax] + G.h[ax];
-  return t > 0.0;
-}
-
-// A pixel of the forward kernels: the four boundary positions as affine functions of the plane index k.
+// A pixel: the four boundary positions as affine functions of the plane index k.
 struct DdPixel {
   double b0, db0, b1, db1, d0, dd0, d1, dd1;
   double L;
@@ -101,280 +92,193 @@ __device__ __forceinline__ DdPixel dd_pixel(const DdGeom& G, const DdView& W, in
   return p;
 }
 
-// Voxel offset of (plane k, in-plane indices jb along W.ub, jd along W.vb) in vol[z][y][x].
-__device__ __forceinline__ void dd_voxel(const DdView& W, int k, int jb, int jd, int* xyz) {
-  xyz[W.a] = k; xyz[W.ub] = jb; xyz[W.vb] = jd;
+// ------------------------------------------------------------------------------------------------ the four operations
+struct DdFixed { unsigned max_bits; unsigned pad; };     // largest |l| of the call as float bits (dd_maxabs_kernel)
+__global__ void dd_maxabs_kernel(const float* __restrict__ x, size_t n, DdFixed* __restrict__ fx) {
+  unsigned m = 0;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    m = max(m, __float_as_uint(fabsf(__ldg(x + i))));            // |x| as bits: monotone, NaN above everything
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0 && m) atomicMax(&fx->max_bits, m);
+}
+// Fixed-point exponent: |sum| < 2^eb 2^hb with max|l| < 2^eb and the host's bound sum_i a^ij <= 2^hb.
+__device__ __forceinline__ int dd_fixed_exponent(unsigned max_bits, int hb) {
+  int eb;
+  frexpf(__uint_as_float(max_bits), &eb);
+  return 61 - eb - hb;
+}
+__global__ void dd_fixed_to_float_kernel(const long long* __restrict__ acc, const DdFixed* __restrict__ fx, int hb,
+                                         size_t n, int accumulate, float* __restrict__ out) {
+  const unsigned mb = fx->max_bits;
+  const bool bad = mb >= 0x7f800000u;                             // Inf / NaN in the projections
+  const double inv = mb && !bad ? scalbn(1.0, -dd_fixed_exponent(mb, hb)) : 0.0;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const float v = bad ? __int_as_float(0x7fc00000) : (float)((double)acc[i] * inv);
+    out[i] = accumulate ? out[i] + v : v;
+  }
 }
 
-// ------------------------------------------------------------------------------------------------ forward
-// GRAD 0: l_i = sum_j a^ij mu_j (reads the caller's volume); GRAD 1: the six sums of Eq.19-20 times the upstream weight.
-template <int GRAD>
-__global__ void __launch_bounds__(kFwdThreads) dd_fwd_kernel(DdGeom G, const DdView* __restrict__ views,
-                                                            const float* __restrict__ vol,
-                                                            const float4* __restrict__ gvol, GradBricks GB,
-                                                            const float* __restrict__ upstream,
-                                                            float* __restrict__ out) {
+template <int MODE>
+__global__ void __launch_bounds__(kFwdThreads) dd_kernel(DdGeom G, const DdView* __restrict__ views,
+                                                        const float* __restrict__ vol,     // 0: volume; 3: upstream volume
+                                                        const float4* __restrict__ gvol, GradBricks GB,   // 1
+                                                        const float* __restrict__ img,     // 1: upstream; 2, 3: projections
+                                                        const DdFixed* __restrict__ fx, int hb,            // 2
+                                                        float* __restrict__ out) {
   int iu, iv;
   fwd_pixel(iu, iv);
   const int view = blockIdx.z;
   const bool live = iu < G.nu && iv < G.nv;
   __shared__ DdView W;
+  __shared__ float Pf[3][4];
   for (int i = threadIdx.x; i < (int)(sizeof(DdView) / 4); i += blockDim.x)
     reinterpret_cast<int*>(&W)[i] = reinterpret_cast<const int*>(views + view)[i];
   __syncthreads();
+  if (MODE == 3 && threadIdx.x < 12) Pf[threadIdx.x >> 2][threadIdx.x & 3] = (float)W.P[threadIdx.x >> 2][threadIdx.x & 3];
+  if (MODE == 3) __syncthreads();
+  const size_t pix = ((size_t)view * G.nv + iv) * G.nu + iu;
   double sum = 0.0;
   float A0 = 0.f, A1 = 0.f, A2 = 0.f, B0 = 0.f, B1 = 0.f, B2 = 0.f;
-  if (live) {
+  // per-pixel inputs of the back-projection modes
+  float li = 0.f, Du = 0.f, Dv = 0.f, T0 = 0.f, T1 = 0.f, T2 = 0.f;
+  double fscale = 0.0;
+  bool work = live;
+  if (MODE == 2) {
+    li = live ? __ldg(img + pix) : 0.f;
+    const unsigned mb = fx->max_bits;
+    if (mb && mb < 0x7f800000u) fscale = scalbn(1.0, dd_fixed_exponent(mb, hb));
+    work = live && li != 0.f;
+  }
+  if (MODE == 3 && live) {     // central differences of the zero-extended projection (:202)
+    const float* p = img + pix;
+    Du = 0.5f * ((iu + 1 < G.nu ? __ldg(p + 1) : 0.f) - (iu > 0 ? __ldg(p - 1) : 0.f));
+    Dv = 0.5f * ((iv + 1 < G.nv ? __ldg(p + G.nu) : 0.f) - (iv > 0 ? __ldg(p - G.nu) : 0.f));
+    T0 = fmaf(Du, Pf[0][0], Dv * Pf[1][0]); T1 = fmaf(Du, Pf[0][1], Dv * Pf[1][1]); T2 = fmaf(Du, Pf[0][2], Dv * Pf[1][2]);
+    work = Du != 0.f || Dv != 0.f;
+  }
+  if (work) {
     const DdPixel p = dd_pixel(G, W, iu, iv);
     const int a = W.a, nb = G.n[W.ub], nd = G.n[W.vb];
     const size_t sx = 1, sy = (size_t)G.n[0], sz = (size_t)G.n[0] * G.n[1];
-    const size_t st[3] = {sx, sy, sz};
-    const size_t sa = st[a], sb = st[W.ub], sd = st[W.vb];
-    for (int k = 0; p.ok && k < G.n[a]; ++k) {
-      const double xa_rel = (G.c[a] + (k - G.h[a]) * G.v[a] - W.so[a]) * p.front_sign;
-      if (!(xa_rel > 0.0)) continue;
+    const size_t sa = a == 0 ? sx : (a == 1 ? sy : sz), sb = W.ub == 0 ? sx : (W.ub == 1 ? sy : sz),
+                 sd = W.vb == 0 ? sx : (W.vb == 1 ? sy : sz);
+    // planes in front of the source: (x_a(k) - s'_a) front_sign > 0, x_a(k) = c_a + (k - h_a) v_a - the bound on k once
+    int k_lo = 0, k_hi = G.n[a] - 1;
+    {
+      const double kz = (W.so[a] - G.c[a]) / G.v[a] + G.h[a];          // plane index of the source
+      if (p.front_sign > 0) k_lo = max(k_lo, (int)floor(kz) + 1); else k_hi = min(k_hi, (int)ceil(kz) - 1);
+    }
+    const float Lf = (float)p.L;
+    for (int k = k_lo; p.ok && k <= k_hi; ++k) {
       const double kd = (double)k;
       double b0 = fma(kd, p.db0, p.b0), b1 = fma(kd, p.db1, p.b1), d0 = fma(kd, p.dd0, p.d0), d1 = fma(kd, p.dd1, p.d1);
       if (b0 > b1) { const double t = b0; b0 = b1; b1 = t; }
       if (d0 > d1) { const double t = d0; d0 = d1; d1 = t; }
       if (!(b1 > b0) || !(d1 > d0)) continue;
-      const int jb0 = max((int)floor(b0 + 0.5), 0), jb1 = min((int)floor(b1 + 0.5), nb - 1);
-      const int jd0 = max((int)floor(d0 + 0.5), 0), jd1 = min((int)floor(d1 + 0.5), nd - 1);
-      const double wl = p.L / ((b1 - b0) * (d1 - d0));
-      for (int jd = jd0; jd <= jd1; ++jd) {
-        const double od = fmin(d1, jd + 0.5) - fmax(d0, jd - 0.5);
-        if (!(od > 0.0)) continue;
-        for (int jb = jb0; jb <= jb1; ++jb) {
-          const double ob = fmin(b1, jb + 0.5) - fmax(b0, jb - 0.5);
-          if (!(ob > 0.0)) continue;
-          const double wgt = wl * ob * od;
-          if (!GRAD) {
-            sum = fma(wgt, (double)__ldg(vol + (size_t)k * sa + (size_t)jb * sb + (size_t)jd * sd), sum);
-          } else {
-            int xyz[3];
-            dd_voxel(W, k, jb, jd, xyz);
-            const float4 g = ldg4(gvol + (GB.FX(xyz[0]) + GB.FY(xyz[1]) + GB.FZ(xyz[2])));
-            const float wf = (float)wgt;
-            const float rx = G.cx + ((float)xyz[0] - (float)G.h[0]) * G.vx, ry = G.cy + ((float)xyz[1] - (float)G.h[1]) * G.vy,
-                        rz = G.cz + ((float)xyz[2] - (float)G.h[2]) * G.vz;
-            const float lx = wf * g.x, ly = wf * g.y, lz = wf * g.z;
-            A0 += lx; A1 += ly; A2 += lz;
-            B0 += ry * lz - rz * ly;
-            B1 += rz * lx - rx * lz;
-            B2 += rx * ly - ry * lx;
+      // the first cell each interval touches becomes the origin: the overlaps are then fp32 on numbers of order one
+      const double jbf = floor(b0 + 0.5), jdf = floor(d0 + 0.5);
+      if (!(fabs(jbf) < 1e9) || !(fabs(jdf) < 1e9) || !(b1 - jbf < 1e6) || !(d1 - jdf < 1e6)) continue;
+      const int jbo = (int)jbf, jdo = (int)jdf;
+      const float fb0 = (float)(b0 - jbf), fb1 = (float)(b1 - jbf), fd0 = (float)(d0 - jdf), fd1 = (float)(d1 - jdf);
+      const float wl = Lf * fast_rcp((fb1 - fb0) * (fd1 - fd0));
+      float plane = 0.f;
+      // one voxel of the plane: weight wf on voxel (k, jb, jd)
+      auto add = [&](float wf, int jb, int jd) {
+        const size_t lin = (size_t)k * sa + (size_t)jb * sb + (size_t)jd * sd;
+        if (MODE == 0) {
+          plane = fmaf(wf, __ldg(vol + lin), plane);
+        } else if (MODE == 2) {
+          const long long q = __double2ll_rn((double)(wf * li) * fscale);
+          atomicAdd(reinterpret_cast<unsigned long long*>(out) + lin, (unsigned long long)q);
+        } else {
+          // (k, jb, jd) -> (x, y, z) by selects (an array indexed by W.a would live in local memory)
+          const int X = a == 0 ? k : (W.ub == 0 ? jb : jd), Y = a == 1 ? k : (W.ub == 1 ? jb : jd),
+                    Z = a == 2 ? k : (W.ub == 2 ? jb : jd);
+          const float rx = G.cx + ((float)X - (float)G.h[0]) * G.vx, ry = G.cy + ((float)Y - (float)G.h[1]) * G.vy,
+                      rz = G.cz + ((float)Z - (float)G.h[2]) * G.vz;
+          float lx, ly, lz;
+          if (MODE == 1) {
+            const float4 g = ldg4(gvol + (GB.FX(X) + GB.FY(Y) + GB.FZ(Z)));
+            lx = wf * g.x; ly = wf * g.y; lz = wf * g.z;
+          } else {             // Eq.13 at the voxel centre: q = a^ij w_j (D_u J_u + D_v J_v)
+            const float wj = __ldg(vol + lin);
+            const float up = fmaf(Pf[0][0], rx, fmaf(Pf[0][1], ry, fmaf(Pf[0][2], rz, Pf[0][3])));
+            const float vp = fmaf(Pf[1][0], rx, fmaf(Pf[1][1], ry, fmaf(Pf[1][2], rz, Pf[1][3])));
+            const float wp = fmaf(Pf[2][0], rx, fmaf(Pf[2][1], ry, fmaf(Pf[2][2], rz, Pf[2][3])));
+            const float rw = fast_rcp(wp);
+            const float cc = fmaf(Du, up, Dv * vp) * rw;
+            const float sc = wf * wj * rw;
+            lx = sc * fmaf(-cc, Pf[2][0], T0); ly = sc * fmaf(-cc, Pf[2][1], T1); lz = sc * fmaf(-cc, Pf[2][2], T2);
+          }
+          A0 += lx; A1 += ly; A2 += lz;
+          B0 += ry * lz - rz * ly;
+          B1 += rz * lx - rx * lz;
+          B2 += rx * ly - ry * lx;
+        }
+      };
+      if (fb1 < 1.5f && fd1 < 1.5f) {
+        // footprint narrower than a voxel (fine detectors: every BASELINE config): at most 2 x 2 cells, no loops
+        const float ob[2] = {fminf(fb1, 0.5f) - fb0, fmaxf(fb1 - 0.5f, 0.f)};
+        const float od[2] = {fminf(fd1, 0.5f) - fd0, fmaxf(fd1 - 0.5f, 0.f)};
+#pragma unroll
+        for (int qd = 0; qd < 2; ++qd) {
+#pragma unroll
+          for (int qb = 0; qb < 2; ++qb) {
+            const int jb = jbo + qb, jd = jdo + qd;
+            const float wf = wl * ob[qb] * od[qd];
+            if (wf > 0.f && jb >= 0 && jb < nb && jd >= 0 && jd < nd) add(wf, jb, jd);
+          }
+        }
+      } else {
+        const int nbj = min((int)floorf(fb1 + 0.5f), nb - 1 - jbo), ndj = min((int)floorf(fd1 + 0.5f), nd - 1 - jdo);
+        for (int qd = max(0, -jdo); qd <= ndj; ++qd) {
+          const float od = fminf(fd1, (float)qd + 0.5f) - fmaxf(fd0, (float)qd - 0.5f);
+          if (!(od > 0.f)) continue;
+          for (int qb = max(0, -jbo); qb <= nbj; ++qb) {
+            const float ob = fminf(fb1, (float)qb + 0.5f) - fmaxf(fb0, (float)qb - 0.5f);
+            if (!(ob > 0.f)) continue;
+            add(wl * ob * od, jbo + qb, jdo + qd);
           }
         }
       }
+      if (MODE == 0) sum += (double)plane;
     }
   }
-  if (!GRAD) {
-    if (live) out[((size_t)view * G.nv + iv) * G.nu + iu] = (float)sum;
-  } else {
+  if (MODE == 0) {
+    if (live) out[pix] = (float)sum;
+  } else if (MODE == 1) {
     float o6[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     if (live) {
-      const float w = __ldg(upstream + ((size_t)view * G.nv + iv) * G.nu + iu);
+      const float w = __ldg(img + pix);
       o6[0] = w * A0; o6[1] = w * A1; o6[2] = w * A2; o6[3] = w * B0; o6[4] = w * B1; o6[5] = w * B2;
     }
     reduce6_to_partials<kFwdThreads>(o6, out, view);
-  }
-}
-
-// ------------------------------------------------------------------------------------------------ back (transpose)
-// Offsets, in voxels, from the voxel centre r (on the plane x_a = r_a) to the points where the rays source -> detector
-// point (u, v) meet that plane:  off_x(u, v) = (D_x E_a - E_x D_a) / (D_a v_x),  D = X(u, v) - s' (affine in u, v),
-// E = r - s'.  The 2 x 2 determinant of two nearly parallel vectors of ~1000 mm is a few hundred: it is expanded ONCE per
-// (voxel, view), in fp64, about a reference pixel (uc, vc) inside the voxel's window -
-//   det_x(u, v) = c_x + (u - uc) p_x + (v - vc) q_x,   D_a(u, v) = D_a(uc, vc) + (u - uc) U_a + (v - vc) V_a -
-// and its three coefficients are small numbers without cancellation left in them, so every boundary of every
-// candidate pixel is then two fp32 FMAs per function, a reciprocal and a product (no fp64 per pixel).
-struct DdLocal {
-  float Dc[3];            // D(uc, vc) along a, ub, vb
-  float U[3], V[3];       // detector steps along a, ub, vb
-  float cb, pb, qb;       // det along ub
-  float cd, pd, qd;       // det along vb
-  float Ea, ivb, ivd, va; // E_a; 1 / pitch along ub, vb; pitch along a
-};
-__device__ __forceinline__ DdLocal dd_local(const DdGeom& G, const DdView& W, const double* E, int uc, int vc) {
-  DdLocal q;
-  const int ax[3] = {W.a, W.ub, W.vb};
-  double D[3];
+  } else if (MODE == 3) {
+    // partials[tile][view][6] (S'_q, S'_c of dfp_kernels.cuh: bp_grad_kernel; bp_contract_kernel finishes the job)
+    __shared__ float red[kFwdThreads / 32][6];
+    float o6[6] = {A0, A1, A2, B0, B1, B2};
 #pragma unroll
-  for (int i = 0; i < 3; ++i) {
-    D[i] = fma((double)uc, W.Uo[ax[i]], fma((double)vc, W.Vo[ax[i]], W.X00[ax[i]])) - W.so[ax[i]];
-    q.Dc[i] = (float)D[i]; q.U[i] = (float)W.Uo[ax[i]]; q.V[i] = (float)W.Vo[ax[i]];
-  }
-  const double Ea = E[W.a], Eb = E[W.ub], Ed = E[W.vb];
-  q.cb = (float)fma(D[1], Ea, -Eb * D[0]);
-  q.pb = (float)fma(W.Uo[W.ub], Ea, -Eb * W.Uo[W.a]);
-  q.qb = (float)fma(W.Vo[W.ub], Ea, -Eb * W.Vo[W.a]);
-  q.cd = (float)fma(D[2], Ea, -Ed * D[0]);
-  q.pd = (float)fma(W.Uo[W.vb], Ea, -Ed * W.Uo[W.a]);
-  q.qd = (float)fma(W.Vo[W.vb], Ea, -Ed * W.Vo[W.a]);
-  q.Ea = (float)Ea; q.ivb = 1.0f / (float)G.v[W.ub]; q.ivd = 1.0f / (float)G.v[W.vb]; q.va = (float)G.v[W.a];
-  return q;
-}
-// offset along ub (AXIS 0) or vb (AXIS 1) at the detector point (uc + du, vc + dv); *front: t = E_a / D_a > 0
-template <int AXIS>
-__device__ __forceinline__ float dd_off(const DdLocal& q, float du, float dv, bool* front) {
-  const float Da = fmaf(du, q.U[0], fmaf(dv, q.V[0], q.Dc[0]));
-  const float det = AXIS == 0 ? fmaf(du, q.pb, fmaf(dv, q.qb, q.cb)) : fmaf(du, q.pd, fmaf(dv, q.qd, q.cd));
-  *front = q.Ea * Da > 0.f;
-  return det * fast_rcp(Da) * (AXIS == 0 ? q.ivb : q.ivd);
-}
-// normalised overlap of the footprint [x0, x1] (either order) with the voxel's cell [-1/2, 1/2]; 0 if none
-__device__ __forceinline__ float dd_cell_overlap(float x0, float x1) {
-  const float lo = fminf(x0, x1), hi = fmaxf(x0, x1);
-  const float o = fminf(hi, 0.5f) - fmaxf(lo, -0.5f);
-  return (o > 0.f && hi > lo) ? o / (hi - lo) : 0.f;
-}
-// slab length v_a / |e_a| of the pixel-centre ray at (uc + du, vc + dv)
-__device__ __forceinline__ float dd_slab_length(const DdLocal& q, float du, float dv) {
-  const float d0 = fmaf(du, q.U[0], fmaf(dv, q.V[0], q.Dc[0])), d1 = fmaf(du, q.U[1], fmaf(dv, q.V[1], q.Dc[1])),
-              d2 = fmaf(du, q.U[2], fmaf(dv, q.V[2], q.Dc[2]));
-  return q.va * sqrtf(fmaf(d0, d0, fmaf(d1, d1, d2 * d2))) * fast_rcp(fabsf(d0));
-}
-
-// Candidate pixels of a voxel: the detector bounding box of its cell's four corners on the plane (fp32: the box gets
-// one pixel of margin anyway - the footprints are taken on the pixels' mid-lines, which an in-plane rotation tilts by a
-// fraction of a pixel).
-struct DdWindow { int u0, u1, v0, v1; };
-__device__ __forceinline__ DdWindow dd_window(const DdGeom& G, const DdView& W, const float* P, const float* r) {
-  float umin = 3e38f, umax = -3e38f, vmin = 3e38f, vmax = -3e38f;
-  bool ok = true;
+    for (int q = 0; q < 6; ++q) {
+      float v = o6[q];
 #pragma unroll
-  for (int c = 0; c < 4; ++c) {
-    float q[3] = {r[0], r[1], r[2]};
-    q[W.ub] += ((c & 1) ? 0.5f : -0.5f) * (float)G.v[W.ub];
-    q[W.vb] += ((c & 2) ? 0.5f : -0.5f) * (float)G.v[W.vb];
-    const float wp = fmaf(P[8], q[0], fmaf(P[9], q[1], fmaf(P[10], q[2], P[11])));
-    if (!(wp > 0.f)) ok = false;
-    const float rw = 1.0f / wp;
-    const float u = fmaf(P[0], q[0], fmaf(P[1], q[1], fmaf(P[2], q[2], P[3]))) * rw;
-    const float v = fmaf(P[4], q[0], fmaf(P[5], q[1], fmaf(P[6], q[2], P[7]))) * rw;
-    umin = fminf(umin, u); umax = fmaxf(umax, u); vmin = fminf(vmin, v); vmax = fmaxf(vmax, v);
-  }
-  DdWindow w;
-  if (!ok || !(umax - umin < 1e6f) || !(vmax - vmin < 1e6f)) { w.u0 = w.v0 = 0; w.u1 = w.v1 = -1; return w; }
-  w.u0 = max((int)floorf(umin + 0.5f) - 1, 0); w.u1 = min((int)floorf(umax + 0.5f) + 1, G.nu - 1);
-  w.v0 = max((int)floorf(vmin + 0.5f) - 1, 0); w.v1 = min((int)floorf(vmax + 0.5f) + 1, G.nv - 1);
-  return w;
-}
-
-constexpr int kDdBpThreads = 256;
-// GRAD 0: vol[j] (+)= sum_views sum_i a^ij l_i.  One thread per voxel, x fastest; the view loop is inside the thread
-// so that the volume is written once and the sum over views has a fixed order.
-// GRAD 1: partials[tile][view][6] of sum_ij a^ij w_j (D_u^i J_u(r_j) + D_v^i J_v(r_j)) and its moment about the origin
-// of the object frame (S'_q, S'_c of dfp_kernels.cuh: bp_grad_kernel; the same bp_contract_kernel finishes the job).
-template <int GRAD>
-__global__ void __launch_bounds__(kDdBpThreads) dd_bp_kernel(DdGeom G, int n_views, int accumulate,
-                                                            const DdView* __restrict__ views,
-                                                            const BpView* __restrict__ bviews,
-                                                            const float* __restrict__ proj,
-                                                            const float* __restrict__ upstream,
-                                                            float* __restrict__ out) {
-  const size_t nvox = (size_t)G.n[0] * G.n[1] * G.n[2];
-  const size_t j = (size_t)blockIdx.x * kDdBpThreads + threadIdx.x;
-  const bool live = j < nvox;
-  int xyz[3] = {0, 0, 0};
-  if (live) { xyz[0] = (int)(j % G.n[0]); xyz[1] = (int)((j / G.n[0]) % G.n[1]); xyz[2] = (int)(j / ((size_t)G.n[0] * G.n[1])); }
-  __shared__ DdView W;
-  __shared__ BpView BV;
-  __shared__ float red[kDdBpThreads / 32][6];
-  const float wj = (GRAD && live) ? __ldg(upstream + j) : 0.f;
-  // object-frame mm of the voxel centre
-  const float rx = G.cx + ((float)xyz[0] - (float)G.h[0]) * G.vx, ry = G.cy + ((float)xyz[1] - (float)G.h[1]) * G.vy,
-              rz = G.cz + ((float)xyz[2] - (float)G.h[2]) * G.vz;
-  double acc = (!GRAD && accumulate && live) ? (double)out[j] : 0.0;
-  for (int view = 0; view < n_views; ++view) {
-    __syncthreads();
-    for (int i = threadIdx.x; i < (int)(sizeof(DdView) / 4); i += blockDim.x)
-      reinterpret_cast<int*>(&W)[i] = reinterpret_cast<const int*>(views + view)[i];
-    if (GRAD && threadIdx.x < (int)(sizeof(BpView) / 4))
-      reinterpret_cast<float*>(&BV)[threadIdx.x] = reinterpret_cast<const float*>(bviews + view)[threadIdx.x];
-    __syncthreads();
-    double su = 0.0, sv = 0.0;
-    if (live && (!GRAD || wj != 0.f)) {
-      double E[3];
-#pragma unroll
-      for (int x = 0; x < 3; ++x) E[x] = G.c[x] + ((double)xyz[x] - G.h[x]) * G.v[x] - W.so[x];
-      float Pl[12];
-#pragma unroll
-      for (int q = 0; q < 12; ++q) Pl[q] = (float)W.P[q >> 2][q & 3];
-      const float rc[3] = {rx, ry, rz};
-      const DdWindow win = dd_window(G, W, Pl, rc);
-      const float* img = proj + (size_t)view * G.nu * G.nv;
-      if (win.u0 <= win.u1 && win.v0 <= win.v1) {
-        const int uc = (win.u0 + win.u1) >> 1, vc = (win.v0 + win.v1) >> 1;
-        const DdLocal q = dd_local(G, W, E, uc, vc);
-        for (int iv = win.v0; iv <= win.v1; ++iv) {
-          const float dv = (float)(iv - vc);
-          bool fl, fr, f2, f3;
-          float bl = dd_off<0>(q, (float)(win.u0 - uc) - 0.5f, dv, &fl);      // the left boundary of the row's first pixel
-          for (int iu = win.u0; iu <= win.u1; ++iu) {
-            const float du = (float)(iu - uc);
-            const float br = dd_off<0>(q, du + 0.5f, dv, &fr);                // shared with the next pixel
-            const float ob = dd_cell_overlap(bl, br);
-            const bool fb = fl && fr;
-            bl = br; fl = fr;
-            if (!(ob > 0.f) || !fb) continue;
-            const float d0 = dd_off<1>(q, du, dv - 0.5f, &f2), d1 = dd_off<1>(q, du, dv + 0.5f, &f3);
-            const float od = dd_cell_overlap(d0, d1);
-            if (!(od > 0.f) || !(f2 && f3)) continue;
-            const double wgt = (double)(dd_slab_length(q, du, dv) * ob * od);
-            if (!GRAD) {
-              acc = fma(wgt, (double)__ldg(img + (size_t)iv * G.nu + iu), acc);
-            } else {
-              const float lp = iu + 1 < G.nu ? __ldg(img + (size_t)iv * G.nu + iu + 1) : 0.f;
-              const float lm = iu > 0 ? __ldg(img + (size_t)iv * G.nu + iu - 1) : 0.f;
-              const float tp = iv + 1 < G.nv ? __ldg(img + (size_t)(iv + 1) * G.nu + iu) : 0.f;
-              const float tm = iv > 0 ? __ldg(img + (size_t)(iv - 1) * G.nu + iu) : 0.f;
-              su = fma(wgt, 0.5 * ((double)lp - (double)lm), su);
-              sv = fma(wgt, 0.5 * ((double)tp - (double)tm), sv);
-            }
-          }
-        }
-      }
+      for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+      o6[q] = v;
     }
-    if (GRAD) {
-      float s6[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-      if (live && wj != 0.f) {
-        // Eq.13 at the voxel centre from the folded P_eff rows of BpView (u, v in the rows' own shifted units)
-        const float xf = (float)xyz[0] - (float)G.h[0], yf = (float)xyz[1] - (float)G.h[1], zf = (float)xyz[2] - (float)G.h[2];
-        const float up = fmaf(BV.A[0][0], xf, fmaf(BV.A[0][1], yf, fmaf(BV.A[0][2], zf, BV.A[0][3])));
-        const float vp = fmaf(BV.A[1][0], xf, fmaf(BV.A[1][1], yf, fmaf(BV.A[1][2], zf, BV.A[1][3])));
-        const float wp = fmaf(BV.A[2][0], xf, fmaf(BV.A[2][1], yf, fmaf(BV.A[2][2], zf, BV.A[2][3])));
-        const float rw = 1.0f / wp, uq = up * rw, vq = vp * rw;
-        const float dlu = (float)su, dlv = (float)sv;
-        const float cc = fmaf(dlu, uq, dlv * vq);
-        const float sc = wj * rw;
-        const float qx = sc * fmaf(dlu, BV.J[0][0], fmaf(dlv, BV.J[1][0], -cc * BV.J[2][0]));
-        const float qy = sc * fmaf(dlu, BV.J[0][1], fmaf(dlv, BV.J[1][1], -cc * BV.J[2][1]));
-        const float qz = sc * fmaf(dlu, BV.J[0][2], fmaf(dlv, BV.J[1][2], -cc * BV.J[2][2]));
-        s6[0] = qx; s6[1] = qy; s6[2] = qz;
-        s6[3] = ry * qz - rz * qy; s6[4] = rz * qx - rx * qz; s6[5] = rx * qy - ry * qx;
-      }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane == 0) {
 #pragma unroll
-      for (int q = 0; q < 6; ++q) {
-        float v = s6[q];
+      for (int q = 0; q < 6; ++q) red[warp][q] = o6[q];
+    }
+    __syncthreads();
+    if (threadIdx.x < 6) {
+      float s = 0.f;
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        s6[q] = v;
-      }
-      const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-      if (lane == 0) {
-#pragma unroll
-        for (int q = 0; q < 6; ++q) red[warp][q] = s6[q];
-      }
-      __syncthreads();
-      if (threadIdx.x < 6) {
-        float t = 0.f;
-#pragma unroll
-        for (int wI = 0; wI < kDdBpThreads / 32; ++wI) t += red[wI][threadIdx.x];
-        out[((size_t)blockIdx.x * n_views + view) * 6 + threadIdx.x] = t;
-      }
+      for (int wI = 0; wI < kFwdThreads / 32; ++wI) s += red[wI][threadIdx.x];
+      const size_t tile = (size_t)blockIdx.y * gridDim.x + blockIdx.x;
+      out[(tile * gridDim.z + view) * 6 + threadIdx.x] = s;
     }
   }
-  if (!GRAD && live) out[j] = (float)acc;
 }
 
 }  // namespace dfp
