@@ -165,12 +165,12 @@ def workload_name(w, V):
 class Job:
     """One workload resident in HBM and the four calls on it."""
 
-    def __init__(self, dfp, index, dev, rank=0, world=1, views=None):
+    def __init__(self, dfp, index, dev, rank=0, world=1, views=None, flags=0):
         from paper_2508_13304_b200.sharding import shard_range
         self.dfp, self.dev = dfp, dev
         V1 = views if views is not None else W.CONFIGS[index]["views"]
         self.w = w = W.make_config(index, n_views=V1 * world)
-        self.g = g = w.geom
+        self.g = g = w.geom.replace(flags=w.geom.flags | flags) if flags else w.geom
         lo, hi = shard_range(w.n_views, rank, world)
         self.V = V = hi - lo
         self.angles = np.ascontiguousarray(w.angles.float().numpy()[lo:hi])
@@ -265,11 +265,16 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=5, help="BASELINE.json config index 1..5 (default 5, the largest)")
     ap.add_argument("--debug-views", type=int, default=None, help="override the view count (profiling runs only)")
+    ap.add_argument("--weights", default="rd", choices=["rd", "dd", "sf"],
+                    help="profiling runs only: the four calls with the distance-driven / separable-footprint weights "
+                         "(DFP_FLAG_DD / DFP_FLAG_SF) instead of the paper's ray-driven trilinear / voxel-driven pair")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the other modes / configs reported in `extra`")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.weights != "rd":      # another weight model: the four calls only (unit, roofline and baselines are the RD path's)
+        args.no_cpu_baseline = args.no_e2e = args.no_extras = True
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -299,7 +304,8 @@ def main():
     # ---------------------------------------------------------------- workload, resident in HBM
     # N ranks: a global batch of N x (the config's views), sharded by views, one shard per GPU (weak scaling);
     # rank 0's shard is exactly the N=1 workload.  No data-path collective.
-    job = Job(dfp, args.config, dev, rank, world, args.debug_views)
+    job = Job(dfp, args.config, dev, rank, world, args.debug_views,
+              {"rd": 0, "dd": dfp.FLAG_DD, "sf": dfp.FLAG_SF}[args.weights])
     w, g, V = job.w, job.g, job.V
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)        # > 126 MB L2
     dfp.set_kernel_timing(True)
@@ -334,7 +340,17 @@ def main():
             c = dict(job.calls(g.replace(flags=g.flags | flag)))
             ms = job.time_calls([c["forward"], c["forward_pose_grad"]], reps)
             extra[f"{name}_mode_ms_per_call"] = {"forward": ms[0], "forward_pose_grad": ms[1]}
-        # DFP_FLAG_DD: the distance-driven pair, all four calls (back-projector = exact transpose of the forward one)
+        # DFP_FLAG_DD / DFP_FLAG_SF: the other matched pairs, all four calls (back-projector = exact transpose of the
+        # forward one)
+        ws0 = job.ws
+        for name, flag in (("dd", dfp.FLAG_DD), ("sf", dfp.FLAG_SF)):
+            gm = g.replace(flags=g.flags | flag)
+            job.ws = torch.empty(max(dfp.workspace_bytes(gm, V, op) for op in range(4)), dtype=torch.uint8, device=dev)
+            ms = job.time_calls([fn for _, fn in job.calls(gm)], 1)
+            extra[f"{name}_mode_ms_per_call"] = dict(zip(("forward", "forward_pose_grad", "backproject",
+                                                         "backproject_pose_grad"), ms))
+        job.ws = ws0
+        torch.cuda.empty_cache()
         # DFP_FLAG_VIEW_FRAMES: the four calls with one explicit (s, c, U, V) frame per view - the config's views on a
         # seeded non-circular (saddle) orbit with detector wobble; same kernels, only the per-view set-up differs
         gv = g.replace(flags=g.flags | dfp.FLAG_VIEW_FRAMES)
@@ -520,7 +536,10 @@ def main():
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
            "ms_per_step": t_all / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f32", "data": "synthetic",
-           "config": {"workload": workload_name(w, V), "ray_steps_per_pass": int(job_ray_steps),
+           "config": {"workload": workload_name(w, V) + ("" if args.weights == "rd" else
+                                                          f" - {args.weights.upper()} weights (profiling run: unit and "
+                                                          "roofline figures are those of the ray-driven path)"),
+                      "ray_steps_per_pass": int(job_ray_steps),
                       "voxel_views_per_pass": int(job_voxel_views), "l2": "256 MiB flush write between timed steps",
                       "parallelism": f"views sharded over {world} rank(s), {V} views per GPU, no data-path collective"},
            "extra": extra, "other_configs": other, "clocks": clocks, "e2e": e2e, "gpu_launches": n_launch,
