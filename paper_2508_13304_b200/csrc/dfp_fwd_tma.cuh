@@ -153,7 +153,7 @@ struct TmaBlock {              // block-wide state in shared memory
   int kA, kB;                  // union of the live rays' kappa ranges [kA, kB)
   int Kc;                      // samples per chunk (0: nothing to do, -1: the box cannot hold the tile)
   int org[kMaxStages][3];      // per stage: centred index of the box's first cell (the origin of the local positions)
-  double orgd[kMaxStages][3];  // the same as doubles (one conversion by the issuing thread instead of one per thread)
+  double orgd[kMaxStages][3];  // the same minus 1/2, as doubles: Ray::pm (position - 1/2) minus it = local position
 };
 
 // One chunk's box: centred index of its first cell along each axis, from the tile's four corner rays at the chunk's
@@ -202,7 +202,7 @@ __device__ __forceinline__ void issue_chunk(const VolLayout& L, TmaBlock& B, con
   constexpr int kWords = S::X * S::Y * S::Z;
   const int s = chunk % S::STAGES;
   B.org[s][0] = oc[0]; B.org[s][1] = oc[1]; B.org[s][2] = oc[2];
-  B.orgd[s][0] = (double)oc[0]; B.orgd[s][1] = (double)oc[1]; B.orgd[s][2] = (double)oc[2];
+  B.orgd[s][0] = (double)oc[0] - 0.5; B.orgd[s][1] = (double)oc[1] - 0.5; B.orgd[s][2] = (double)oc[2] - 0.5;
   const unsigned bar = bar_addr + 8u * s;
   mbar_expect_tx(bar, kWords * 4);
   tma_load_3d(tiles_addr + (unsigned)(s * tma_stage_words<SHAPE>() * 4), map, oc[0] + L.hx, oc[1] + L.hy, oc[2] + L.hz, bar);
@@ -283,10 +283,11 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
     const double p0 = fma(kd, rd[zi + 3], rd[zi + 0]), p1 = fma(kd, rd[zi + 4], rd[zi + 1]),
                  p2 = fma(kd, rd[zi + 5], rd[zi + 2]);
     mbar_wait(bar_addr + 8u * s, (unsigned)(chunk / S::STAGES) & 1u);
+    // (B.orgd holds the origin minus 1/2: Ray::pm is the position minus 1/2, the local position below is the position)
     const float2 bxy = make_float2((float)(p0 - B.orgd[s][0]), (float)(p1 - B.orgd[s][1]));
     const float bz = (float)(p2 - B.orgd[s][2]);
-    // word index of local cell (X, Y, Z) in stage s from the magic-rounded floats' bits
-    unsigned c0 = (unsigned)(s * kWords) - (unsigned)kMagicBits * (unsigned)(1 + BX + BXY);
+    // BYTE offset of local cell (X, Y, Z) in stage s from the magic-rounded floats' bits
+    unsigned c0 = 4u * ((unsigned)(s * kWords) - (unsigned)kMagicBits * (unsigned)(1 + BX + BXY));
     // keep the constant out of the optimiser's sight: folded into every load's offset it no longer fits the LDS
     // immediate field and each of the 8 / 32 loads of a sample gets its own address add (measured: +20 % time)
     asm volatile("" : "+r"(c0));
@@ -295,12 +296,13 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
       // position, floor and fractions: x and y as one fp32x2 lane pair
       const float2 q2 = __ffma2_rn(make_float2(jf, jf), dpxy, bxy);
       const float qz = fmaf(jf, dpz, bz);
-      const float2 t2 = __fadd2_rn(q2, make_float2(kMagic, kMagic));
-      const float tz = qz + kMagic;
-      const float2 a2 = __fadd2_rn(sub2(q2, __fadd2_rn(t2, make_float2(-kMagic, -kMagic))), make_float2(0.5f, 0.5f));
-      float ax = a2.x, ay = a2.y, az = (qz - (tz - kMagic)) + 0.5f;
-      unsigned idx = (unsigned)__float_as_int(t2.x) + (unsigned)BX * (unsigned)__float_as_int(t2.y) +
-                     (unsigned)BXY * (unsigned)__float_as_int(tz) + c0;
+      // floor by the magic add ROUNDED DOWN (t = kMagic + floor(q) exactly), fraction = q - floor(q)
+      const float2 t2 = __fadd2_rd(q2, make_float2(kMagic, kMagic));
+      const float tz = __fadd_rd(qz, kMagic);
+      const float2 a2 = sub2(q2, __fadd2_rn(t2, make_float2(-kMagic, -kMagic)));
+      float ax = a2.x, ay = a2.y, az = qz - (tz - kMagic);
+      unsigned off = 4u * (unsigned)__float_as_int(t2.x) + (unsigned)(4 * BX) * (unsigned)__float_as_int(t2.y) +
+                     (unsigned)(4 * BXY) * (unsigned)__float_as_int(tz) + c0;
       if (GRAD == 2) {
         // the derivative of the interpolant jumps at cell faces: a sample within fp32 rounding of one takes its
         // cell (and fractions) from the fp64 position, as the oracle does
@@ -312,14 +314,14 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
 #pragma unroll
           for (int a = 0; a < 3; ++a) { rr.pm[a] = rd[zi + a]; rr.dp[a] = rd[zi + 3 + a]; }
           exact_cell(rr, k, cell, fr);
-          idx = (unsigned)(s * kWords + (cell[0] - B.org[s][0]) + BX * (cell[1] - B.org[s][1]) + BXY * (cell[2] - B.org[s][2]));
+          off = 4u * (unsigned)(s * kWords + (cell[0] - B.org[s][0]) + BX * (cell[1] - B.org[s][1]) + BXY * (cell[2] - B.org[s][2]));
           ax = fr[0]; ay = fr[1]; az = fr[2];
         }
       }
-      const float* c = tiles + idx;
+      const float* c = reinterpret_cast<const float*>(reinterpret_cast<const char*>(tiles) + off);
 #ifdef DFP_CHECK_BOUNDS   // debug build: every LDS of the sample must fall inside the stage's box (else NaN out)
       {
-        const int local = (int)(idx - (unsigned)(s * kWords)), halo = (GRAD == 1 || GRAD == 3) ? 1 : 0;
+        const int local = (int)(off / 4u - (unsigned)(s * kWords)), halo = (GRAD == 1 || GRAD == 3) ? 1 : 0;
         const int lo = local - halo * (1 + BX + BXY), hi = local + (1 + halo) * (1 + BX + BXY);
         if (lo < 0 || hi >= kBox) sum = gx = __int_as_float(0x7fc00000);
       }

