@@ -196,8 +196,27 @@ bool make_volume_map(const dfp_geometry& g, const float* d_vol, int bx, int by, 
 // Positions at path length tau: p = s' + tau e, so a tile's extent along axis a is tau |De_a| with
 // |De_a| <= (|Dd_a| + |e_a| (rho_max/|d|) |Dd|) / SDD  for pixel offsets Dd on a detector at distance >= SDD.
 constexpr int kMinChunk = 4;
+#ifndef DFP_CLASS_TAN
+#define DFP_CLASS_TAN 0.5774      // tan(30 deg): a view is "along y" when |e_x| < tan(30 deg) |e_y| (voxel-index units)
+#endif
+constexpr double kClassTan = DFP_CLASS_TAN;
+// volt[z][x][y] = vol[z][y][x]: the volume with y fastest, for the gradient kernel of the views along x (MODE 6)
+__global__ void __launch_bounds__(256) transpose_xy_kernel(int nx, int ny, const float* __restrict__ vol, float* __restrict__ volt) {
+  __shared__ float tile[32][33];
+  const size_t slab = (size_t)blockIdx.z * nx * ny;
+  const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
+  for (int j = threadIdx.y; j < 32; j += 8) {
+    const int x = x0 + threadIdx.x, y = y0 + j;
+    if (x < nx && y < ny) tile[j][threadIdx.x] = vol[slab + (size_t)y * nx + x];
+  }
+  __syncthreads();
+  for (int j = threadIdx.y; j < 32; j += 8) {
+    const int y = y0 + threadIdx.x, x = x0 + j;
+    if (x < nx && y < ny) volt[slab + (size_t)x * ny + y] = tile[threadIdx.x][j];
+  }
+}
 bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V, const ViewFrame& F, bool grad,
-                   const int* box, int TU, int TV, int min_chunk = kMinChunk) {
+                   const int* box, int TU, int TV, int min_chunk = kMinChunk, int align_axis = 0) {
   const double v3[3] = {g.vx, g.vy, g.vz}, c3[3] = {g.cx, g.cy, g.cz};
   const double half[3] = {0.5 * g.nx * g.vx + 3 * g.vx, 0.5 * g.ny * g.vy + 3 * g.vy, 0.5 * g.nz * g.vz + 3 * g.vz};
   double tau_max = 0;
@@ -227,7 +246,7 @@ bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V, co
     const double dd = tu * std::fabs(V.du[a]) + tv * std::fabs(V.dv[a]);
     const double span = tau_max * (dd + emax[a] * rho * dnorm) / sdd / v3[a];
     const double slope = (double)G.step * emax[a] / v3[a];
-    const double avail = box[a] - 4 - (grad ? 2 : 0) - (a == 0 ? kBoxAlignLoss : 0) - 2.0 * kBoxMargin - 1.05 * span - 0.05;
+    const double avail = box[a] - 4 - (grad ? 2 : 0) - (a == align_axis ? kBoxAlignLoss : 0) - 2.0 * kBoxMargin - 1.05 * span - 0.05;
     if (avail < (min_chunk - 1) * slope) return false;
   }
   return true;
@@ -300,6 +319,8 @@ cudaError_t ensure_smem_attributes() {
   DFP_ATTR((fwd_tma_kernel<0, 5>), tma_smem_bytes<5>());
   DFP_ATTR((fwd_tma_kernel<1, 2>), tma_smem_bytes<2>());
   DFP_ATTR((fwd_tma_kernel<1, 3>), tma_smem_bytes<3>());
+  DFP_ATTR((fwd_tma_kernel<5, 6>), tma_smem_bytes<6>());
+  DFP_ATTR((fwd_tma_kernel<6, 6>), tma_smem_bytes<6>());
   DFP_ATTR((fwd_tma_kernel<2, 2>), tma_smem_bytes<2>());
   DFP_ATTR((fwd_tma_kernel<2, 3>), tma_smem_bytes<3>());
   DFP_ATTR((fwd_tma_kernel<3, 2>), tma_smem_bytes<2>());
@@ -324,7 +345,7 @@ cudaError_t ensure_smem_attributes() {
 
 // ---- workspace carving ---------------------------------------------------------------------------
 struct FwdWs {
-  size_t off_views, off_dd, off_con, off_pvol, off_part, off_fixed, total;
+  size_t off_views, off_dd, off_con, off_pvol, off_part, off_fixed, off_volt, off_ids, total;
   int gx, gy;     // blocks per view (16 x 16-pixel tiles)
   int gy8;        // rows of 16 x 8-pixel tiles (TMA gradient kernel)
 };
@@ -344,6 +365,12 @@ FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad, int nset = 1) {
     if (g.flags & DFP_FLAG_SF) nblk = ((size_t)g.nx * g.ny * g.nz + kSfThreads - 1) / kSfThreads;   // sf_kernel blocks
     w.off_part = o;  o += grad ? align_up(sizeof(float) * 6 * (size_t)nset * V * nblk) : 0;
   }
+  // the paper's gradient mode on the TMA path, >= 0.45 voxel per pixel: view lists of the three ray-direction classes and
+  // the transposed volume of the views along x (dfp_fwd_tma.cuh, MODE 5 / 6)
+  const bool classes = grad && nset == 1 && !(g.flags & (DFP_FLAG_GRAD_INTERP | DFP_FLAG_SIDDON | DFP_FLAG_JOSEPH | DFP_FLAG_DD |
+                                                         DFP_FLAG_SF | DFP_FLAG_NO_TMA));
+  w.off_ids = o;  o += classes ? align_up(sizeof(int) * 3 * (size_t)V) : 0;
+  w.off_volt = o; o += classes ? align_up(sizeof(float) * (size_t)g.nx * g.ny * g.nz) : 0;
   // sf_kernel<0>: SfFixed (256 bytes) + the 64-bit fixed-point accumulator image
   w.off_fixed = o; o += ((g.flags & DFP_FLAG_SF) && !grad) ? align_up(256 + sizeof(long long) * (size_t)V * g.nu * g.nv) : 0;
   w.total = o;
@@ -530,7 +557,8 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
                                             {BoxShape<2>::X, BoxShape<2>::Y, BoxShape<2>::Z},
                                             {BoxShape<3>::X, BoxShape<3>::Y, BoxShape<3>::Z},
                                             {BoxShape<4>::X, BoxShape<4>::Y, BoxShape<4>::Z},
-                                            {BoxShape<5>::X, BoxShape<5>::Y, BoxShape<5>::Z}};
+                                            {BoxShape<5>::X, BoxShape<5>::Y, BoxShape<5>::Z},
+                                            {BoxShape<6>::X, BoxShape<6>::Y, BoxShape<6>::Z}};
   // forward: shapes 0, 1, 2 (16 x 16-pixel tiles) - with the odd-extent boxes 4, 5 first where a pixel spans >= 0.45
   // voxel along z (bank conflicts, dfp_fwd_tma.cuh); gradient: shapes 3, 2 (16 x 8-pixel tiles)
 #ifndef DFP_WIDE_A
@@ -570,7 +598,7 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
     DFP_CUDA(ensure_smem_attributes(), "cudaFuncSetAttribute");
     time_begin(s);
     // 1-D grid, one block per (view, tile), ordered view group -> tile -> view (dfp_fwd_tma.cuh: fwd_block)
-    const FwdGrid Qf{V, w.gx, w.gy}, Qg{V, w.gx, w.gy8};
+    const FwdGrid Qf{V, w.gx, w.gy, V, nullptr}, Qg{V, w.gx, w.gy8, V, nullptr};
     const unsigned nbf = (unsigned)V * w.gx * w.gy, nbg = (unsigned)V * w.gx * w.gy8;
     if (fused && shape == 3)
       fwd_tma_kernel<3, 3><<<nbg, TmaLanes<3>::THREADS, tma_smem_bytes<3>(), s>>>(G, Qg, dv, vol_map, d_up, part, d_proj);
@@ -580,13 +608,57 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
       fwd_tma_kernel<2, 3><<<nbg, TmaLanes<2>::THREADS, tma_smem_bytes<3>(), s>>>(G, Qg, dv, vol_map, d_up, part, nullptr);
     else if (grad && interp)
       fwd_tma_kernel<2, 2><<<nbg, TmaLanes<2>::THREADS, tma_smem_bytes<2>(), s>>>(G, Qg, dv, vol_map, d_up, part, nullptr);
-    else if (grad && shape == 3)
+    else if (grad && shape == 3 && wide) {
+      // Views by the in-plane direction of their central ray (voxel-index units): along y -> MODE 5, along x -> MODE 6 on
+      // the transposed volume, near the diagonals (or where the MODE 5 / 6 box does not hold the view's tiles) -> MODE 1.
+      std::vector<int> ids[3];
+      CUtensorMap map_y, map_x;
+      const bool ok_y = make_volume_map(*g, d_vol, kBoxes[6][0], kBoxes[6][1], kBoxes[6][2], &map_y);
+      float* volt = reinterpret_cast<float*>(base + w.off_volt);
+      bool ok_x = (g->ny % 4) == 0;
+      if (ok_x) {
+        dfp_geometry gt = *g;
+        gt.nx = g->ny; gt.ny = g->nx;
+        ok_x = make_volume_map(gt, volt, kBoxes[6][0], kBoxes[6][1], kBoxes[6][2], &map_x);
+      }
+      const int box_y[3] = {kBoxes[6][0], kBoxes[6][1], kBoxes[6][2]}, box_x[3] = {kBoxes[6][1], kBoxes[6][0], kBoxes[6][2]};
+      for (int v = 0; v < V; ++v) {
+        const double cu = 0.5 * (g->nu - 1), cv = 0.5 * (g->nv - 1);
+        const double ex = std::fabs(hv[v].d0[0] + cu * hv[v].du[0] + cv * hv[v].dv[0]) / g->vx;
+        const double ey = std::fabs(hv[v].d0[1] + cu * hv[v].du[1] + cv * hv[v].dv[1]) / g->vy;
+        int c = 0;
+        if (ok_y && ey * kClassTan > ex && tma_view_fits(*g, G, hv[v], hf[v], true, box_y, TU, TV)) c = 1;
+        if (ok_x && ex * kClassTan > ey && tma_view_fits(*g, G, hv[v], hf[v], true, box_x, TU, TV, kMinChunk, 1)) c = 2;
+        ids[c].push_back(v);
+      }
+      int* dids = reinterpret_cast<int*>(base + w.off_ids);
+      std::vector<int> all;
+      for (int c = 0; c < 3; ++c) all.insert(all.end(), ids[c].begin(), ids[c].end());
+      DFP_CUDA(upload_async(dids, all.data(), sizeof(int) * all.size(), s), "view upload");
+      const int* d0 = dids, *d1 = dids + ids[0].size(), *d2 = d1 + ids[1].size();
+      const unsigned tiles = (unsigned)w.gx * w.gy8;
+      if (!ids[0].empty())
+        fwd_tma_kernel<1, 3><<<(unsigned)ids[0].size() * tiles, TmaLanes<1>::THREADS, tma_smem_bytes<3>(), s>>>(
+            G, FwdGrid{(int)ids[0].size(), w.gx, w.gy8, V, d0}, dv, vol_map, d_up, part, nullptr);
+      if (!ids[1].empty()) {
+        fwd_tma_kernel<5, 6><<<(unsigned)ids[1].size() * tiles, TmaLanes<5>::THREADS, tma_smem_bytes<6>(), s>>>(
+            G, FwdGrid{(int)ids[1].size(), w.gx, w.gy8, V, d1}, dv, map_y, d_up, part, nullptr);
+        ++g_launches;
+      }
+      if (!ids[2].empty()) {
+        transpose_xy_kernel<<<dim3((g->nx + 31) / 32, (g->ny + 31) / 32, g->nz), dim3(32, 8), 0, s>>>(g->nx, g->ny, d_vol, volt);
+        fwd_tma_kernel<6, 6><<<(unsigned)ids[2].size() * tiles, TmaLanes<6>::THREADS, tma_smem_bytes<6>(), s>>>(
+            G, FwdGrid{(int)ids[2].size(), w.gx, w.gy8, V, d2}, dv, map_x, d_up, part, nullptr);
+        g_launches += 2;
+      }
+      if (ids[0].empty()) --g_launches;        // (the common count below adds one launch)
+    } else if (grad && shape == 3)
       fwd_tma_kernel<1, 3><<<nbg, TmaLanes<1>::THREADS, tma_smem_bytes<3>(), s>>>(G, Qg, dv, vol_map, d_up, part, nullptr);
     else if (grad)
       fwd_tma_kernel<1, 2><<<nbg, TmaLanes<1>::THREADS, tma_smem_bytes<2>(), s>>>(G, Qg, dv, vol_map, d_up, part, nullptr);
     else if (half_tile)
       fwd_tma_kernel<4, 2><<<(unsigned)V * w.gx * ((g->nv + 7) / 8), TmaLanes<4>::THREADS, tma_smem_bytes<2>(), s>>>(
-          G, FwdGrid{V, w.gx, (g->nv + 7) / 8}, dv, vol_map, nullptr, d_out, nullptr);
+          G, FwdGrid{V, w.gx, (g->nv + 7) / 8, V, nullptr}, dv, vol_map, nullptr, d_out, nullptr);
     else if (shape == 0)
       fwd_tma_kernel<0, 0><<<nbf, TmaLanes<0>::THREADS, tma_smem_bytes<0>(), s>>>(G, Qf, dv, vol_map, nullptr, d_out, nullptr);
     else if (shape == 1)

@@ -53,7 +53,13 @@ template <> struct BoxShape<2> { static constexpr int X = 28, Y = 28, Z = 20, ST
 #ifndef DFP_GRAD_TV
 #define DFP_GRAD_TV 8
 #endif
-template <> struct BoxShape<3> { static constexpr int X = 28, Y = 28, Z = 16, STAGES = DFP_GRAD_STAGES; };   // gradient, 16 x 8 tiles
+#ifndef DFP_GRAD_BY
+#define DFP_GRAD_BY 28
+#endif
+#ifndef DFP_GRAD_PU
+#define DFP_GRAD_PU 8
+#endif
+template <> struct BoxShape<3> { static constexpr int X = 28, Y = DFP_GRAD_BY, Z = 16, STAGES = DFP_GRAD_STAGES; };   // gradient, 16 x 8 tiles
 // Forward boxes with an ODD y extent (slab pitch = 12 / 20 mod 32 instead of 16): where a warp's 8 x 4-pixel patch spans
 // three z slices (>= 0.45 voxel per pixel: the 512^3 configs), slab pitch 16 puts slices z and z + 2 on the same banks;
 // 1.76 -> 1.38 wavefronts per load on C5, 1.62 -> 1.36 on C4 (simulated, _and measured_ in DESIGN.md); at C2's 0.39
@@ -66,7 +72,8 @@ template <> struct BoxShape<4> { static constexpr int X = 20, Y = 19, Z = 16, ST
 #define DFP_S5_Z 20
 #endif
 template <> struct BoxShape<5> { static constexpr int X = 28, Y = 19, Z = DFP_S5_Z, STAGES = DFP_S5_STAGES; };
-constexpr int kNumShapes = 6;
+template <> struct BoxShape<6> { static constexpr int X = 28, Y = 27, Z = 16, STAGES = 1; };   // MODE 5 / 6 (above)
+constexpr int kNumShapes = 7;
 // words between the stages of a box: the box rounded up to 128 bytes (alignment of a TMA destination)
 template <int SHAPE> __host__ __device__ constexpr int tma_stage_words() {
   return (BoxShape<SHAPE>::X * BoxShape<SHAPE>::Y * BoxShape<SHAPE>::Z + 31) / 32 * 32;
@@ -86,18 +93,27 @@ __device__ __forceinline__ float2 lerp2(float2 a, float2 v0, float2 v1) { return
 // (dfp_forward_fused_moments).  Gradient kernels: two lanes per ray, 8 x 2-pixel warps, 16 x 8-pixel tile.
 // MODE 4 = GRAD 0 on a 16 x 8-pixel tile (128 threads): the forward projector's last resort before the gather kernels,
 // for coarse pixels on fine voxels (C1's forward call, 1.2 voxels per pixel: a 16 x 16 tile's frustum holds no box).
-template <int GRAD> struct TmaLanes {
-  static constexpr int SLOTS = (GRAD && GRAD != 4) ? DFP_GRAD_SLOTS : 1, TU = kFwdTU,
-                       TV = GRAD == 0 ? kFwdTV : (GRAD == 4 ? 8 : DFP_GRAD_TV), THREADS = TU * TV * SLOTS;
-  static constexpr int PU = SLOTS == 4 ? 4 : 8, PV = 32 / (PU * SLOTS);
+// MODE 5 / 6 = GRAD 1 for views whose rays run along ONE in-plane axis, at >= 0.45 voxel per pixel (the 512^3 configs).
+// There a warp of 8 x 2 pixels x 2 samples holds ~5 voxels across the rays, 2 along z and only 2 along the rays: when
+// the rays run along x, only two x values reach the low bank bits and 15-20 distinct words share 16 banks (1.38
+// wavefronts per load whatever the pitches); a warp of 4 x 4 pixels x 2 samples on a box with an ODD y extent (slab pitch
+// = 20 mod 32) measures 1.10 when the rays run along y.  MODE 5 is that kernel for the views along y; MODE 6 is the same
+// kernel on the TRANSPOSED volume ([z][x][y], x and y of the ray swapped on entry, of the sums on exit) for the views along
+// x; views near the diagonals keep MODE 1 (1.10 as it is).  C5: 188 -> 218 Gray-steps/s on the axis-aligned views.
+__host__ __device__ constexpr int tma_grad_of(int MODE) { return MODE == 4 ? 0 : (MODE >= 5 ? 1 : MODE); }
+template <int MODE> struct TmaLanes {
+  static constexpr int GRAD = tma_grad_of(MODE);
+  static constexpr int SLOTS = GRAD ? DFP_GRAD_SLOTS : 1, TU = kFwdTU,
+                       TV = MODE == 0 ? kFwdTV : (MODE == 4 ? 8 : DFP_GRAD_TV), THREADS = TU * TV * SLOTS;
+  static constexpr int PU = SLOTS == 4 ? 4 : (MODE >= 5 ? 4 : (SLOTS == 2 ? DFP_GRAD_PU : 8)), PV = 32 / (PU * SLOTS);
 #ifndef DFP_FWD_MINB
 #define DFP_FWD_MINB 4
 #endif
-  static constexpr int MINB = THREADS > 256 ? 2 : (GRAD == 0 ? DFP_FWD_MINB : 4);
+  static constexpr int MINB = THREADS > 256 ? 2 : (MODE == 0 ? DFP_FWD_MINB : 4);
 };
-template <int GRAD>
+template <int MODE>
 __device__ __forceinline__ void tma_pixel(int bx, int by, int& iu, int& iv, int& slot) {
-  using T = TmaLanes<GRAD>;
+  using T = TmaLanes<MODE>;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   constexpr int WU = T::TU / T::PU;                     // warps across u
   const int pix = lane % (T::PU * T::PV);
@@ -162,7 +178,7 @@ struct TmaBlock {              // block-wide state in shared memory
 // the serial section between the barrier and the TMA issue shrinks to the six stores and the issue itself.
 template <int MODE, int SHAPE>
 __device__ __forceinline__ void chunk_origin(const VolLayout& L, const TmaBlock& B, int chunk, int* oc) {
-  constexpr int GRAD = MODE == 4 ? 0 : MODE;
+  constexpr int GRAD = tma_grad_of(MODE);
   const int lane = threadIdx.x & 31;
   const int a = min(lane >> 3, 2), r = (lane >> 1) & 3;
   const int k0 = B.kA + chunk * B.Kc;
@@ -181,7 +197,7 @@ __device__ __forceinline__ void chunk_origin(const VolLayout& L, const TmaBlock&
 // The same by ONE thread (forward kernels: after the barrier, measured faster there than the warp-wide version).
 template <int MODE, int SHAPE>
 __device__ __forceinline__ void chunk_origin_serial(const VolLayout& L, const TmaBlock& B, int chunk, int* oc) {
-  constexpr int GRAD = MODE == 4 ? 0 : MODE;
+  constexpr int GRAD = tma_grad_of(MODE);
   const int k0 = B.kA + chunk * B.Kc;
   const int k1 = min(k0 + B.Kc, B.kB) - 1;
   const float f0 = (float)k0, f1 = (float)k1;
@@ -210,11 +226,11 @@ __device__ __forceinline__ void issue_chunk(const VolLayout& L, TmaBlock& B, con
 
 // The chunk loop of one block for one box shape.  acc = {sum} (forward) or {gx,gy,gz,hx,hy,hz[,sum]} (gradient).
 template <int MODE, int SHAPE>
-__device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* map, const Ray& r, int slot,
+__device__ __forceinline__ void tma_march(const VolLayout& L, const CUtensorMap* map, const Ray& r, int slot,
                                           TmaBlock& B, const float* tiles, unsigned tiles_addr, unsigned bar_addr,
                                           float* acc) {
   using S = BoxShape<SHAPE>;
-  constexpr int GRAD = MODE == 4 ? 0 : MODE;
+  constexpr int GRAD = tma_grad_of(MODE);
   constexpr int BX = S::X, BXY = S::X * S::Y, kBox = S::X * S::Y * S::Z, kWords = tma_stage_words<SHAPE>();
   constexpr int SLOTS = TmaLanes<MODE>::SLOTS;
   if (threadIdx.x == 0) {
@@ -248,8 +264,8 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
       for (int c = 0; c < S::STAGES; ++c)
         if (c < n_chunks) {
           int oc[3];
-          chunk_origin_serial<MODE, SHAPE>(G.L, B, c, oc);
-          issue_chunk<SHAPE>(G.L, B, map, c, oc, tiles_addr, bar_addr);
+          chunk_origin_serial<MODE, SHAPE>(L, B, c, oc);
+          issue_chunk<SHAPE>(L, B, map, c, oc, tiles_addr, bar_addr);
         }
     }
   }
@@ -408,11 +424,11 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
     constexpr bool kPre = (DFP_ORIGIN_PRE >> (GRAD ? 1 : 0)) & 1;
     int oc[3] = {0, 0, 0};
     const bool more = chunk + S::STAGES < n_chunks;
-    if (kPre && warp0 && more) chunk_origin<MODE, SHAPE>(G.L, B, chunk + S::STAGES, oc);
+    if (kPre && warp0 && more) chunk_origin<MODE, SHAPE>(L, B, chunk + S::STAGES, oc);
     __syncthreads();                                   // every thread is done with stage s ("empty")
     if (threadIdx.x == 0 && more) {
-      if (!kPre) chunk_origin_serial<MODE, SHAPE>(G.L, B, chunk + S::STAGES, oc);
-      issue_chunk<SHAPE>(G.L, B, map, chunk + S::STAGES, oc, tiles_addr, bar_addr);
+      if (!kPre) chunk_origin_serial<MODE, SHAPE>(L, B, chunk + S::STAGES, oc);
+      issue_chunk<SHAPE>(L, B, map, chunk + S::STAGES, oc, tiles_addr, bar_addr);
     }
   }
   if (!GRAD) {
@@ -426,6 +442,8 @@ __device__ __forceinline__ void tma_march(const FwdGeom& G, const CUtensorMap* m
 // Grid: one block per (view, pixel tile), 1-D, ordered group of views -> tile -> view within the group (kViewGroup).
 struct FwdGrid {
   int n_views, gx, gy;         // views of this launch; tiles per view along u and v
+  int n_total;                 // views of the call (layout of the partials)
+  const int* ids;              // view index of each of the launch's views, or nullptr: the views 0 .. n_views - 1
 };
 __device__ __forceinline__ void fwd_block(const FwdGrid& Q, int& view, int& bx, int& by) {
   const unsigned nb = (unsigned)Q.gx * (unsigned)Q.gy, per = (unsigned)kViewGroup * nb;
@@ -433,6 +451,7 @@ __device__ __forceinline__ void fwd_block(const FwdGrid& Q, int& view, int& bx, 
   const unsigned gsz = min((unsigned)kViewGroup, (unsigned)Q.n_views - grp * kViewGroup);
   const unsigned tile = r / gsz, vg = r - tile * gsz;
   view = (int)(grp * kViewGroup + vg);
+  if (Q.ids) view = __ldg(Q.ids + view);
   by = (int)(tile / (unsigned)Q.gx);
   bx = (int)(tile - (unsigned)by * (unsigned)Q.gx);
 }
@@ -444,7 +463,7 @@ __global__ void __launch_bounds__(TmaLanes<MODE>::THREADS, TmaLanes<MODE>::MINB)
                                                               const float* __restrict__ upstream,
                                                               float* __restrict__ out,
                                                               float* __restrict__ proj_out) {
-  constexpr int GRAD = MODE == 4 ? 0 : MODE;
+  constexpr int GRAD = tma_grad_of(MODE);
   constexpr int NSET = GRAD == 3 ? 3 : 1;              // weight sets of the per-view reduction (fused: 1, l, b)
   constexpr int SLOTS = TmaLanes<MODE>::SLOTS;
   extern __shared__ __align__(128) float tiles[];      // STAGES boxes
@@ -469,6 +488,12 @@ __global__ void __launch_bounds__(TmaLanes<MODE>::THREADS, TmaLanes<MODE>::MINB)
     }
   }
   if (!live) r.n = 0;
+  VolLayout L = G.L;
+  if (MODE == 6) {             // the transposed volume: the ray in (y, x, z)
+    double sw = r.pm[0]; r.pm[0] = r.pm[1]; r.pm[1] = sw;
+    sw = r.dp[0]; r.dp[0] = r.dp[1]; r.dp[1] = sw;
+    const int h = L.hx; L.hx = L.hy; L.hy = h;
+  }
 
   if (threadIdx.x == 0) {
     B.kA = 0x7fffffff;
@@ -502,7 +527,11 @@ __global__ void __launch_bounds__(TmaLanes<MODE>::THREADS, TmaLanes<MODE>::MINB)
   }
   __syncthreads();
   float acc[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-  tma_march<MODE, SHAPE>(G, &vol_map, r, slot, B, tiles, tiles_addr, bar_addr, acc);
+  tma_march<MODE, SHAPE>(L, &vol_map, r, slot, B, tiles, tiles_addr, bar_addr, acc);
+  if (MODE == 6) {             // back to (x, y, z): the sums of d/dx and d/dy
+    float sw = acc[0]; acc[0] = acc[1]; acc[1] = sw;
+    sw = acc[3]; acc[3] = acc[4]; acc[4] = sw;
+  }
   // the slots of a ray: partial sums over the samples each lane took (slot = lane / (PU * PV): the high lane bits)
   if (SLOTS > 1) {
 #pragma unroll
@@ -565,7 +594,7 @@ __global__ void __launch_bounds__(TmaLanes<MODE>::THREADS, TmaLanes<MODE>::MINB)
     const size_t nblk = (size_t)Q.gx * Q.gy;
     // partials[set][view][block][6]: each weight set is a plain gradient partial array for fwd_contract_kernel
     const int set = threadIdx.x / 6, k = threadIdx.x % 6;
-    out[(((size_t)set * Q.n_views + view) * nblk + blk) * 6 + k] = t;
+    out[(((size_t)set * Q.n_total + view) * nblk + blk) * 6 + k] = t;
   }
   }  // GRAD
 }

@@ -115,7 +115,7 @@ __global__ void sf_fixed_to_float_kernel(DdGeom G, const long long* __restrict__
     out[i] = bad ? __int_as_float(0x7fc00000) : (float)((double)acc[i] * inv);
 }
 
-constexpr int kSfThreads = 256;
+constexpr int kSfThreads = 256, kSfBatch = 8;
 template <int MODE>
 __global__ void __launch_bounds__(kSfThreads) sf_kernel(DdGeom G, int n_views, int accumulate,
                                                         const DdView* __restrict__ views,
@@ -129,9 +129,11 @@ __global__ void __launch_bounds__(kSfThreads) sf_kernel(DdGeom G, int n_views, i
   const bool live = j < nvox;
   int xyz[3] = {0, 0, 0};
   if (live) { xyz[0] = (int)(j % G.n[0]); xyz[1] = (int)((j / G.n[0]) % G.n[1]); xyz[2] = (int)(j / ((size_t)G.n[0] * G.n[1])); }
-  __shared__ double E[3][4];
-  __shared__ float Ef[3][4];
-  __shared__ float red[kSfThreads / 32][6];
+  // the views run in batches of kSfBatch: their matrices are staged together and the per-view block reductions of the
+  // gradient modes wait for the end of the batch - three barriers per batch instead of three per view
+  __shared__ double Eb[kSfBatch][3][4];
+  __shared__ float Efb[kSfBatch][3][4];
+  __shared__ float red[kSfBatch][kSfThreads / 32][6];
   double fscale = 0.0;
   if (MODE == 0) {
     const unsigned mb = fx->max_bits;
@@ -157,14 +159,20 @@ __global__ void __launch_bounds__(kSfThreads) sf_kernel(DdGeom G, int n_views, i
   if (MODE == 2) work = live && (gx != 0.f || gy != 0.f || gz != 0.f);
   if (MODE == 3) work = live && wj != 0.f;
   double acc = (MODE == 1 && accumulate && live) ? (double)out[j] : 0.0;
-  for (int view = 0; view < n_views; ++view) {
-    __syncthreads();
-    if (threadIdx.x < 12) {
-      const double e = views[view].P[threadIdx.x >> 2][threadIdx.x & 3];
-      E[threadIdx.x >> 2][threadIdx.x & 3] = e;
-      Ef[threadIdx.x >> 2][threadIdx.x & 3] = (float)e;
-    }
-    __syncthreads();
+  for (int view0 = 0; view0 < n_views; view0 += kSfBatch) {
+   const int nb = min(kSfBatch, n_views - view0);
+   __syncthreads();
+   if (threadIdx.x < 12 * nb) {
+     const int b = threadIdx.x / 12, q = threadIdx.x % 12;
+     const double e = views[view0 + b].P[q >> 2][q & 3];
+     Eb[b][q >> 2][q & 3] = e;
+     Efb[b][q >> 2][q & 3] = (float)e;
+   }
+   __syncthreads();
+   for (int vb = 0; vb < nb; ++vb) {
+    const int view = view0 + vb;
+    const double (*E)[4] = Eb[vb];
+    const float (*Ef)[4] = Efb[vb];
     double s0 = 0.0, s1 = 0.0;
     SfFoot f;
     f.ok = false;
@@ -228,18 +236,22 @@ __global__ void __launch_bounds__(kSfThreads) sf_kernel(DdGeom G, int n_views, i
       const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
       if (lane == 0) {
 #pragma unroll
-        for (int q = 0; q < 6; ++q) red[warp][q] = s6[q];
-      }
-      __syncthreads();
-      if (threadIdx.x < 6) {
-        float t = 0.f;
-#pragma unroll
-        for (int wI = 0; wI < kSfThreads / 32; ++wI) t += red[wI][threadIdx.x];
-        // MODE 2: partials[view][block][6] (fwd_contract_kernel); MODE 3: partials[block][view][6] (bp_contract_kernel)
-        const size_t at = MODE == 2 ? ((size_t)view * gridDim.x + blockIdx.x) : ((size_t)blockIdx.x * n_views + view);
-        out[at * 6 + threadIdx.x] = t;
+        for (int q = 0; q < 6; ++q) red[vb][warp][q] = s6[q];
       }
     }
+   }
+   if (MODE == 2 || MODE == 3) {
+     __syncthreads();
+     if (threadIdx.x < 6 * nb) {
+       const int vb = threadIdx.x / 6, q = threadIdx.x % 6, view = view0 + vb;
+       float t = 0.f;
+#pragma unroll
+       for (int wI = 0; wI < kSfThreads / 32; ++wI) t += red[vb][wI][q];
+       // MODE 2: partials[view][block][6] (fwd_contract_kernel); MODE 3: partials[block][view][6] (bp_contract_kernel)
+       const size_t at = MODE == 2 ? ((size_t)view * gridDim.x + blockIdx.x) : ((size_t)blockIdx.x * n_views + view);
+       out[at * 6 + q] = t;
+     }
+   }
   }
   if (MODE == 1 && live) out[j] = (float)acc;
 }
