@@ -109,7 +109,8 @@ enum {
   DFP_ERR_NONFINITE = -3,  /* NaN / Inf in geometry, angles or poses                                        */
   DFP_ERR_ALIGN = -4,      /* a device pointer is not 16-byte (workspace: 256-byte) aligned                 */
   DFP_ERR_WORKSPACE = -5,  /* ws_bytes < dfp_workspace_bytes(...)                                           */
-  DFP_ERR_CUDA = -6        /* CUDA runtime error (no device, launch failure, out of memory in *_host)       */
+  DFP_ERR_CUDA = -6,       /* CUDA runtime error (no device, launch failure, out of memory in *_host)       */
+  DFP_ERR_STATIC_LIMIT = -7 /* n_views > DFP_NCC_STATIC_MAX_VIEWS in dfp_ncc_pose_grad_static               */
 };
 enum { DFP_OP_FORWARD = 0, DFP_OP_FORWARD_POSE_GRAD = 1, DFP_OP_BACKPROJECT = 2, DFP_OP_BACKPROJECT_POSE_GRAD = 3,
        DFP_OP_FORWARD_FUSED = 4, DFP_OP_NCC = 5 };
@@ -169,6 +170,22 @@ int dfp_forward_fused_moments(const dfp_geometry* geometry, int n_views, const f
  * dfp_workspace_bytes(geometry, n_views, DFP_OP_NCC).  Same ownership, asynchrony and error behaviour as above. */
 int dfp_ncc_pose_grad(const dfp_geometry* geometry, int n_views, const float* d_proj, const float* d_target,
                       const float* d_moments, float* d_ncc, float* d_grad, void* d_ws, size_t ws_bytes, void* stream);
+
+/* dfp_ncc_pose_grad for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): the same two kernels, the same arguments without the workspace, the same results bit for bit -
+ * the per-view partial sums live in a fixed array in the library's own device image instead
+ * (static __device__, 5 x 64 x DFP_NCC_STATIC_MAX_VIEWS doubles = 640 KiB, held by every GPU that loads the library
+ * until the process exits).  The call allocates and frees nothing, on the host or the device, and synchronises
+ * nothing; the first call on a device looks the array's address up (cudaGetSymbolAddress, with that device current).
+ * n_views > DFP_NCC_STATIC_MAX_VIEWS is rejected with DFP_ERR_STATIC_LIMIT before any launch (slice the views, or use
+ * dfp_ncc_pose_grad with a caller-owned workspace); every other argument is checked as in dfp_ncc_pose_grad.
+ * ALL calls on a device share the one array: calls queued on the same stream are ordered and safe; two calls that can
+ * overlap on the GPU (different streams, or different host threads on different streams) RACE on it - order them with an
+ * event, or give all but one a workspace through dfp_ncc_pose_grad.  The array keeps the last call's partial sums;
+ * nothing in it has to start at zero (every element a call reads, it has written first). */
+#define DFP_NCC_STATIC_MAX_VIEWS 256
+int dfp_ncc_pose_grad_static(const dfp_geometry* geometry, int n_views, const float* d_proj, const float* d_target,
+                             const float* d_moments, float* d_ncc, float* d_grad, void* stream);
 
 /* Bytes of device workspace the op needs for this geometry and view count (0 on invalid arguments).
  * View chunking: any n_views may be passed to the calls above; to bound the workspace (and the size of

@@ -76,6 +76,8 @@ def _load():
     lib.dfp_forward_fused_moments.restype = ci
     lib.dfp_ncc_pose_grad.argtypes = [gp, ci, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.dfp_ncc_pose_grad.restype = ci
+    lib.dfp_ncc_pose_grad_static.argtypes = [gp, ci, vp, vp, vp, vp, vp, vp]
+    lib.dfp_ncc_pose_grad_static.restype = ci
     lib.dfp_forward_host.argtypes = [gp, ci, vp, vp, vp, vp, vp]
     lib.dfp_backproject_host.argtypes = [gp, ci, vp, vp, vp, vp, vp]
     lib.dfp_forward_pose_grad_host.argtypes = [gp, ci, vp, vp, vp, vp, vp, vp]
@@ -250,6 +252,23 @@ def ncc_pose_grad(geom, proj, target, moments, out_ncc=None, out_grad=None, ws=N
         _check(_lib.dfp_ncc_pose_grad(ctypes.byref(g), V, _dev(proj, (V, g.nv, g.nu), "proj"),
                                       _dev(target, (V, g.nv, g.nu), "target"), _dev(moments, (V, 3, 6), "moments"),
                                       _dev(out_ncc, (V,), "ncc"), _dev(out_grad, (V, 6), "grad"), wp, wn, _stream(proj)))
+    return out_ncc, out_grad
+
+
+NCC_STATIC_MAX_VIEWS = 256      # DFP_NCC_STATIC_MAX_VIEWS (include/dfp.h)
+
+
+def ncc_pose_grad_static(geom, proj, target, moments, out_ncc, out_grad):
+    """dfp_ncc_pose_grad_static: dfp_ncc_pose_grad without a workspace - the partial sums live in a fixed device array
+    of the library, the call allocates nothing (the caller passes BOTH outputs).  At most NCC_STATIC_MAX_VIEWS views;
+    calls that can overlap on the GPU race on the shared array (include/dfp.h)."""
+    g = Geometry.of(geom)
+    V = int(proj.shape[0])
+    with _same_device(proj, target, moments, out_ncc, out_grad):
+        _check(_lib.dfp_ncc_pose_grad_static(ctypes.byref(g), V, _dev(proj, (V, g.nv, g.nu), "proj"),
+                                             _dev(target, (V, g.nv, g.nu), "target"),
+                                             _dev(moments, (V, 3, 6), "moments"), _dev(out_ncc, (V,), "ncc"),
+                                             _dev(out_grad, (V, 6), "grad"), _stream(proj)))
     return out_ncc, out_grad
 
 

@@ -1,6 +1,7 @@
 // dfp_api.cu - the C ABI of libdfp (include/dfp.h): argument validation, per-view set-up (fp64 on the host,
 // dfp_params.h), workspace carving and kernel launches (dfp_kernels.cuh).  No torch types, no exceptions, no
 // printing, no host synchronisation in the device-pointer calls.
+#include <atomic>
 #include <cuda_runtime.h>
 
 #include <cmath>
@@ -1124,6 +1125,57 @@ int dfp_ncc_pose_grad(const dfp_geometry* g, int n_views, const float* d_proj, c
   return DFP_OK;
 }
 
+// The allocation-free variant (include/dfp.h): the partial sums of ncc_partial_kernel in a file-scope device array.
+// In HOST code `g_ncc_static` is only the symbol's host-side stand-in, not a device address: its address on the
+// current device is looked up once per device, below, and THAT pointer goes to the kernels.
+}  // extern "C"
+static __device__ __align__(256) double g_ncc_static[5 * (size_t)dfp::kNccBlocks * DFP_NCC_STATIC_MAX_VIEWS];
+namespace {
+constexpr int kMaxDevices = 64;
+std::atomic<double*> g_ncc_static_ptr[kMaxDevices];      // per device; nullptr until the first call on it
+// Device address of g_ncc_static on the CURRENT device (no allocation: the array is part of the loaded module).
+cudaError_t ncc_static_scratch(double** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+  double* p = g_ncc_static_ptr[dev].load(std::memory_order_acquire);
+  if (!p) {
+    void* sym = nullptr;
+    e = cudaGetSymbolAddress(&sym, g_ncc_static);      // with device `dev` current: that device's copy of the array
+    if (e != cudaSuccess) return e;
+    p = static_cast<double*>(sym);
+    g_ncc_static_ptr[dev].store(p, std::memory_order_release);      // two racing first calls store the same address
+  }
+  *out = p;
+  return cudaSuccess;
+}
+}  // namespace
+extern "C" {
+
+int dfp_ncc_pose_grad_static(const dfp_geometry* g, int n_views, const float* d_proj, const float* d_target,
+                             const float* d_moments, float* d_ncc, float* d_grad, void* stream) {
+  int st = validate_geometry(g);
+  if (st) return st;
+  if (n_views <= 0) return DFP_ERR_DIMS;
+  if (n_views > DFP_NCC_STATIC_MAX_VIEWS) return DFP_ERR_STATIC_LIMIT;
+  if (!d_proj || !d_target || !d_moments || !d_ncc || !d_grad) return DFP_ERR_NULL;
+  if (!aligned(d_proj, 16) || !aligned(d_target, 16) || !aligned(d_moments, 8) || !aligned(d_ncc, 4) || !aligned(d_grad, 8))
+    return DFP_ERR_ALIGN;
+  double* partial = nullptr;
+  DFP_CUDA(ncc_static_scratch(&partial), "cudaGetSymbolAddress (static NCC scratch)");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const size_t npix = (size_t)g->nu * g->nv;
+  const int nblk = (int)std::min<size_t>(kNccBlocks, (npix + 4 * kNccThreads - 1) / (4 * kNccThreads));
+  // every element ncc_finish_kernel reads ([view < n_views][block < nblk][5]) is written by ncc_partial_kernel first:
+  // nothing of the previous call's contents is used, nothing has to be cleared
+  ncc_partial_kernel<<<dim3(nblk, n_views), kNccThreads, 0, s>>>(npix, d_proj, d_target, partial);
+  ncc_finish_kernel<<<n_views, 32, 0, s>>>(npix, nblk, partial, d_moments, d_ncc, d_grad);
+  g_launches = 2;
+  DFP_CUDA(cudaGetLastError(), "NCC launch (static scratch)");
+  return DFP_OK;
+}
+
 size_t dfp_workspace_bytes(const dfp_geometry* g, int n_views, int op) {
   if (validate_geometry(g) != DFP_OK || n_views <= 0 || n_views > kMaxViews) return 0;
   switch (op) {
@@ -1212,6 +1264,9 @@ const char* dfp_status_string(int status) {
     case DFP_ERR_ALIGN: return "device pointer not 16-byte aligned (workspace: 256-byte)";
     case DFP_ERR_WORKSPACE: return "workspace too small (see dfp_workspace_bytes)";
     case DFP_ERR_CUDA: return g_cuda_msg;
+    case DFP_ERR_STATIC_LIMIT:
+      return "n_views exceeds DFP_NCC_STATIC_MAX_VIEWS (256), the fixed scratch of dfp_ncc_pose_grad_static: slice the "
+             "views or use dfp_ncc_pose_grad with a workspace";
     default: return "unknown status";
   }
 }

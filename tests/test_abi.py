@@ -72,7 +72,7 @@ def test_workspace_bytes_and_status_strings(dfp):
     assert dfp.workspace_bytes(_geom(nx=0), 3, 0) == 0
     assert dfp.workspace_bytes(_geom(sdd=50.0), 3, 0) == 0
     assert dfp.status_string(0) == "ok"
-    for s in range(-6, 0):
+    for s in range(-7, 0):
         assert dfp.status_string(s) not in ("ok", "unknown status")
     assert dfp.version() >= 100
 
@@ -166,3 +166,21 @@ def test_new_flags_and_the_ncc_call_reject_bad_arguments_without_a_gpu(dfp):
     assert dfp.workspace_bytes(g, 2, dfp.OP_NCC) > 0
     # the other matched pairs need room for their per-view blocks and finer partial sums
     assert dfp.workspace_bytes(dfp.Geometry.of(_geom(flags=128)), 3, 3) > dfp.workspace_bytes(g, 3, 3)
+
+
+def test_static_ncc_entry_point_checks_its_arguments_without_a_gpu(dfp):
+    """dfp_ncc_pose_grad_static: the view limit of its fixed scratch array and the other argument checks come before
+    any CUDA call (the GPU test of the entry point itself: tests/test_zz_no_alloc.py)."""
+    lib = ctypes.CDLL(dfp.lib_path())
+    f = lib.dfp_ncc_pose_grad_static
+    f.restype = ctypes.c_int
+    f.argtypes = [ctypes.c_void_p, ctypes.c_int] + [ctypes.c_void_p] * 6
+    g = dfp.Geometry.of(_geom())
+    fake = ctypes.c_void_p(0x10000)
+    assert dfp.NCC_STATIC_MAX_VIEWS == 256
+    assert f(ctypes.byref(g), 257, fake, fake, fake, fake, fake, None) == -7
+    assert "256" in dfp.status_string(-7)
+    assert f(ctypes.byref(g), 0, fake, fake, fake, fake, fake, None) == -2
+    assert f(None, 4, fake, fake, fake, fake, fake, None) == -1
+    assert f(ctypes.byref(g), 4, fake, None, fake, fake, fake, None) == -1
+    assert f(ctypes.byref(g), 4, ctypes.c_void_p(0x10004), fake, fake, fake, fake, None) == -4
