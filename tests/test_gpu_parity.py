@@ -907,3 +907,31 @@ def test_dd_backprojector_is_deterministic_scale_free_and_accumulates(dfp):
     half = dfp.backproject(g, a[:2], p[:2], y[:2].contiguous())
     dfp.backproject(g.replace(flags=dfp.FLAG_DD | dfp.FLAG_ACCUMULATE), a[2:], p[2:], y[2:].contiguous(), out=half)
     assert rel_l2(half.cpu().numpy(), ref.cpu().numpy()) <= 1e-6
+
+
+# ------------------------------------------------------------------ gradient kernels by view class
+@pytest.mark.parametrize("ny,launches", [(40, 5), (42, 3)])
+def test_gradient_kernels_by_view_class_non_cubic_grid(dfp, ny, launches):
+    """At >= 0.45 voxel per pixel dfp_forward_pose_grad sorts its views by the in-plane direction of their central ray:
+    near the diagonals -> fwd_tma_kernel<1, 3>, along y -> <5, 6>, along x -> <6, 6> on a TRANSPOSED copy of the volume.
+    A non-cubic, anisotropic grid (the transposed tensor map, the swapped centre indices and the swapped sums would all
+    show), views of all three classes in one call in mixed order, general poses; the launch count proves that the three
+    kernels ran (3 + transpose + contraction).  ny % 4 != 0 admits no tensor map over the transposed volume: the views
+    along x then stay with the first kernel (2 + contraction)."""
+    g = W.Geometry(nx=48, ny=ny, nz=28, vx=0.5, vy=0.55, vz=0.5, nu=64, nv=40, du=0.4, dv=0.4, sad=400.0, sdd=600.0,
+                   cx=0.7, cy=-0.4, cz=0.3, u0=0.6, v0=-0.8).f32()
+    angles = [0.05, 0.8, 1.6, 3.1, 2.4, 4.75, 5.5, 6.2, 1.45]
+    rng = np.random.default_rng(77)
+    poses = np.concatenate([rng.uniform(-1.5, 1.5, (len(angles), 3)), rng.uniform(-0.06, 0.06, (len(angles), 3))], axis=1)
+    vol = rng.random(g.vol_shape).astype(np.float32)
+    up = rng.standard_normal((len(angles),) + g.det_shape).astype(np.float32)
+    res = run_forward_case(dfp, g, angles, poses, vol, up)
+    dev = torch.device("cuda:0")
+    dfp.forward_pose_grad(g, f32(angles), f32(poses), torch.as_tensor(vol, device=dev), torch.as_tensor(up, device=dev))
+    assert dfp.last_path() == dfp.PATH_TMA and dfp.last_launch_count() == launches
+    check_forward(res)
+    # and the same numbers as the gather path to fp32 rounding
+    gg = g.replace(flags=dfp.FLAG_NO_TMA)
+    ref = dfp.forward_pose_grad(gg, f32(angles), f32(poses), torch.as_tensor(vol, device=dev),
+                                torch.as_tensor(up, device=dev)).cpu().numpy()
+    assert grad_err_u9(res[1], ref).max() <= 1e-4
