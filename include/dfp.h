@@ -234,7 +234,8 @@ int dfp_last_launch_count(void);
 
 /* Kernel path the last successful device-pointer call on this thread took: DFP_PATH_GATHER (global-memory
  * gathers from a packed copy of the input) or DFP_PATH_TMA (input staged tile by tile in shared memory by TMA;
- * taken when nx % 4 == 0 (forward calls) / nu % 4 == 0 (back-projection calls) and every view's tiles fit the staging boxes).  The two paths
+ * taken when every view's tiles fit the staging boxes; with nx % 4 != 0 (forward calls) / nu % 4 != 0 (back-projection
+ * calls) it reads a copy of the input with its rows padded to 16 bytes, made per call in the workspace).  The two paths
  * do the same arithmetic per sample / voxel and agree to fp32 summation order.  Both the
  * forward and the back-projection calls have the two paths. */
 enum { DFP_PATH_GATHER = 0, DFP_PATH_TMA = 1 };

@@ -180,11 +180,15 @@ EncodeTiledFn encode_tiled_fn() {
 
 // Tensor map over the caller's volume [nz][ny][nx] fp32 with the staging box of dfp_fwd_tma.cuh; elements
 // outside the volume read as zero (the zero extension of f~, U7).
-bool make_volume_map(const dfp_geometry& g, const float* d_vol, int bx, int by, int bz, CUtensorMap* map) {
+// `pitch`: floats between rows of the array the map is made over - the caller's volume when nx % 4 == 0, else a copy
+// with its rows padded to a multiple of 4 floats (global strides must be multiples of 16 bytes); the map's extent stays
+// nx, so the padding is out of range like everything else beyond the volume.
+inline int pitch4(int n) { return (n + 3) / 4 * 4; }
+bool make_volume_map(const dfp_geometry& g, const float* d_vol, int pitch, int bx, int by, int bz, CUtensorMap* map) {
   EncodeTiledFn enc = encode_tiled_fn();
-  if (!enc || (g.nx % 4) != 0) return false;           // global strides must be multiples of 16 bytes
+  if (!enc || (pitch % 4) != 0 || pitch < g.nx) return false;
   const cuuint64_t dims[3] = {(cuuint64_t)g.nx, (cuuint64_t)g.ny, (cuuint64_t)g.nz};
-  const cuuint64_t strides[2] = {(cuuint64_t)g.nx * 4, (cuuint64_t)g.nx * g.ny * 4};
+  const cuuint64_t strides[2] = {(cuuint64_t)pitch * 4, (cuuint64_t)pitch * g.ny * 4};
   const cuuint32_t box[3] = {(cuuint32_t)bx, (cuuint32_t)by, (cuuint32_t)bz};
   const cuuint32_t es[3] = {1, 1, 1};
   return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(d_vol), dims, strides, box, es,
@@ -202,9 +206,10 @@ constexpr int kMinChunk = 4;
 #endif
 constexpr double kClassTan = DFP_CLASS_TAN;
 // volt[z][x][y] = vol[z][y][x]: the volume with y fastest, for the gradient kernel of the views along x (MODE 6)
-__global__ void __launch_bounds__(256) transpose_xy_kernel(int nx, int ny, const float* __restrict__ vol, float* __restrict__ volt) {
+__global__ void __launch_bounds__(256) transpose_xy_kernel(int nx, int ny, int tpitch, const float* __restrict__ vol,
+                                                           float* __restrict__ volt) {
   __shared__ float tile[32][33];
-  const size_t slab = (size_t)blockIdx.z * nx * ny;
+  const size_t slab = (size_t)blockIdx.z * nx * ny, tslab = (size_t)blockIdx.z * nx * tpitch;
   const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
   for (int j = threadIdx.y; j < 32; j += 8) {
     const int x = x0 + threadIdx.x, y = y0 + j;
@@ -213,7 +218,7 @@ __global__ void __launch_bounds__(256) transpose_xy_kernel(int nx, int ny, const
   __syncthreads();
   for (int j = threadIdx.y; j < 32; j += 8) {
     const int y = y0 + threadIdx.x, x = x0 + j;
-    if (x < nx && y < ny) volt[slab + (size_t)x * ny + y] = tile[threadIdx.x][j];
+    if (x < nx && y < ny) volt[tslab + (size_t)x * tpitch + y] = tile[threadIdx.x][j];
   }
 }
 bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V, const ViewFrame& F, bool grad,
@@ -255,11 +260,11 @@ bool tma_view_fits(const dfp_geometry& g, const FwdGeom& G, const FwdView& V, co
 
 // ---- TMA path of the back-projection kernels (dfp_bp_tma.cuh) -----------------------------------
 // Tensor maps over the caller's projections [V][nv][nu] fp32, one per patch of the menu up to kmax.
-bool make_proj_maps(const dfp_geometry& g, int V, const float* d_proj, int kmax, PatchMaps* maps) {
+bool make_proj_maps(const dfp_geometry& g, int V, const float* d_proj, int pitch, int kmax, PatchMaps* maps) {
   EncodeTiledFn enc = encode_tiled_fn();
-  if (!enc || (g.nu % 4) != 0) return false;
+  if (!enc || (pitch % 4) != 0 || pitch < g.nu) return false;
   const cuuint64_t dims[3] = {(cuuint64_t)g.nu, (cuuint64_t)g.nv, (cuuint64_t)V};
-  const cuuint64_t strides[2] = {(cuuint64_t)g.nu * 4, (cuuint64_t)g.nu * g.nv * 4};
+  const cuuint64_t strides[2] = {(cuuint64_t)pitch * 4, (cuuint64_t)pitch * g.nv * 4};
   const cuuint32_t es[3] = {1, 1, 1};
   for (int k = 0; k < kNumPatches; ++k) {
     const int kk = k <= kmax ? k : kmax;                 // unused slots repeat the largest map
@@ -371,7 +376,7 @@ FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad, int nset = 1) {
   const bool classes = grad && nset == 1 && !(g.flags & (DFP_FLAG_GRAD_INTERP | DFP_FLAG_SIDDON | DFP_FLAG_JOSEPH | DFP_FLAG_DD |
                                                          DFP_FLAG_SF | DFP_FLAG_NO_TMA));
   w.off_ids = o;  o += classes ? align_up(sizeof(int) * 3 * (size_t)V) : 0;
-  w.off_volt = o; o += classes ? align_up(sizeof(float) * (size_t)g.nx * g.ny * g.nz) : 0;
+  w.off_volt = o; o += classes ? align_up(sizeof(float) * (size_t)g.nx * ((g.ny + 3) / 4 * 4) * g.nz) : 0;
   // sf_kernel<0>: SfFixed (256 bytes) + the 64-bit fixed-point accumulator image
   w.off_fixed = o; o += ((g.flags & DFP_FLAG_SF) && !grad) ? align_up(256 + sizeof(long long) * (size_t)V * g.nu * g.nv) : 0;
   w.total = o;
@@ -573,7 +578,7 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
   const int TU = grad ? TmaLanes<1>::TU : TmaLanes<0>::TU, TV = grad ? TmaLanes<1>::TV : TmaLanes<0>::TV;
   int shape = -1;
   bool half_tile = false;
-  if (!(g->flags & DFP_FLAG_NO_TMA) && (g->nx % 4) == 0) {
+  if (!(g->flags & DFP_FLAG_NO_TMA)) {
     for (int i = 0; i < n_order && shape < 0; ++i) {
       bool fits = true;
       for (int v = 0; fits && v < V; ++v) fits = tma_view_fits(*g, G, hv[v], hf[v], grad, kBoxes[order[i]], TU, TV);
@@ -593,10 +598,18 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
       if (fits) { shape = 2; half_tile = true; }
     }
   }
-  const bool tma = shape >= 0 && make_volume_map(*g, d_vol, kBoxes[shape][0], kBoxes[shape][1], kBoxes[shape][2], &vol_map);
+  // nx % 4 != 0: the TMA kernels read a copy of the volume with 16-byte-aligned rows (1x the volume, in the workspace
+  // region of the gather path's 4x packed copy, which is then not built)
+  const int vpitch = pitch4(g->nx);
+  const float* tma_vol = vpitch == g->nx ? d_vol : reinterpret_cast<const float*>(pvol);
+  const bool tma = shape >= 0 && make_volume_map(*g, tma_vol, vpitch, kBoxes[shape][0], kBoxes[shape][1], kBoxes[shape][2], &vol_map);
   g_path = tma ? DFP_PATH_TMA : DFP_PATH_GATHER;
   if (tma) {
     DFP_CUDA(ensure_smem_attributes(), "cudaFuncSetAttribute");
+    if (tma_vol != d_vol) {
+      DFP_CUDA(cudaMemcpy2DAsync(pvol, (size_t)vpitch * 4, d_vol, (size_t)g->nx * 4, (size_t)g->nx * 4, (size_t)g->ny * g->nz,
+                                 cudaMemcpyDeviceToDevice, s), "cudaMemcpy2DAsync (row-aligned volume)");
+    }
     time_begin(s);
     // 1-D grid, one block per (view, tile), ordered view group -> tile -> view (dfp_fwd_tma.cuh: fwd_block)
     const FwdGrid Qf{V, w.gx, w.gy, V, nullptr}, Qg{V, w.gx, w.gy8, V, nullptr};
@@ -614,13 +627,14 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
       // the transposed volume, near the diagonals (or where the MODE 5 / 6 box does not hold the view's tiles) -> MODE 1.
       std::vector<int> ids[3];
       CUtensorMap map_y, map_x;
-      const bool ok_y = make_volume_map(*g, d_vol, kBoxes[6][0], kBoxes[6][1], kBoxes[6][2], &map_y);
+      const bool ok_y = make_volume_map(*g, tma_vol, vpitch, kBoxes[6][0], kBoxes[6][1], kBoxes[6][2], &map_y);
       float* volt = reinterpret_cast<float*>(base + w.off_volt);
-      bool ok_x = (g->ny % 4) == 0;
-      if (ok_x) {
+      const int tpitch = pitch4(g->ny);               // rows of the transposed volume [z][x][y], 16-byte aligned
+      bool ok_x;
+      {
         dfp_geometry gt = *g;
         gt.nx = g->ny; gt.ny = g->nx;
-        ok_x = make_volume_map(gt, volt, kBoxes[6][0], kBoxes[6][1], kBoxes[6][2], &map_x);
+        ok_x = make_volume_map(gt, volt, tpitch, kBoxes[6][0], kBoxes[6][1], kBoxes[6][2], &map_x);
       }
       const int box_y[3] = {kBoxes[6][0], kBoxes[6][1], kBoxes[6][2]}, box_x[3] = {kBoxes[6][1], kBoxes[6][0], kBoxes[6][2]};
       for (int v = 0; v < V; ++v) {
@@ -647,7 +661,7 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
         ++g_launches;
       }
       if (!ids[2].empty()) {
-        transpose_xy_kernel<<<dim3((g->nx + 31) / 32, (g->ny + 31) / 32, g->nz), dim3(32, 8), 0, s>>>(g->nx, g->ny, d_vol, volt);
+        transpose_xy_kernel<<<dim3((g->nx + 31) / 32, (g->ny + 31) / 32, g->nz), dim3(32, 8), 0, s>>>(g->nx, g->ny, tpitch, d_vol, volt);
         fwd_tma_kernel<6, 6><<<(unsigned)ids[2].size() * tiles, TmaLanes<6>::THREADS, tma_smem_bytes<6>(), s>>>(
             G, FwdGrid{(int)ids[2].size(), w.gx, w.gy8, V, d2}, dv, map_x, d_up, part, nullptr);
         g_launches += 2;
@@ -812,7 +826,7 @@ int run_backproject_slice(const dfp_geometry* g, int V, const float* angles, con
   }
   // TMA-staged path: projections admit a tensor map, every voxel in front of the source, patches fit the menu
   int kmax = -1, TZ = 16;
-  if (!(g->flags & DFP_FLAG_NO_TMA) && (g->nu % 4) == 0) {
+  if (!(g->flags & DFP_FLAG_NO_TMA)) {
     for (TZ = 16; TZ >= 8 && kmax < 0; TZ >>= 1) {
       kmax = 0;
       for (int v = 0; v < V && kmax >= 0; ++v) {
@@ -824,10 +838,18 @@ int run_backproject_slice(const dfp_geometry* g, int V, const float* angles, con
     }
   }
   PatchMaps maps;
-  if (kmax >= 0 && make_proj_maps(*g, V, d_proj, kmax, &maps)) {
+  // nu % 4 != 0: the TMA kernels read a copy of the projections with 16-byte-aligned rows (in the workspace region of the
+  // gather path's 4x packed copy, which is then not built)
+  const int ppitch = pitch4(g->nu);
+  const float* tma_proj = ppitch == g->nu ? d_proj : reinterpret_cast<const float*>(base + w.off_q);
+  if (kmax >= 0 && make_proj_maps(*g, V, tma_proj, ppitch, kmax, &maps)) {
     const int stage_words = bp_stage_words(kmax), n_stages = bp_num_stages(kmax);
     const int smem = stage_words * 4 * n_stages;
     DFP_CUDA(ensure_smem_attributes(), "cudaFuncSetAttribute");
+    if (tma_proj != d_proj) {
+      DFP_CUDA(cudaMemcpy2DAsync(base + w.off_q, (size_t)ppitch * 4, d_proj, (size_t)g->nu * 4, (size_t)g->nu * 4,
+                                 (size_t)g->nv * V, cudaMemcpyDeviceToDevice, s), "cudaMemcpy2DAsync (row-aligned projections)");
+    }
     const dim3 tgrid(w.tx, w.ty, (g->nz + TZ - 1) / TZ);
     g_path = DFP_PATH_TMA;
 #define DFP_BP_ARGS <<<tgrid, kBpTmaThreads, smem, s>>>(G, V, dvd, maps, kmax, stage_words, n_stages

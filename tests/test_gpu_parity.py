@@ -249,16 +249,22 @@ def test_tma_path_ragged_detector_and_partial_misses(dfp):
     check_forward(run_forward_case(dfp, g, ANGLES3, POSES3, vol, up))
 
 
-def test_tma_path_falls_back_when_it_does_not_apply(dfp):
-    """nx % 4 != 0 (no tensor map) or coarse pixels on fine voxels (a tile's frustum exceeds the staging box)."""
+def test_tma_path_odd_row_length_and_fallback(dfp):
+    """nx % 4 != 0: a tensor map needs 16-byte-aligned rows, so the TMA kernels read a row-padded copy of the volume (1x,
+    in the workspace) - same results, TMA path.  Coarse pixels on fine voxels (a tile's frustum exceeds every staging
+    box): the gather kernels."""
     rng = np.random.default_rng(12)
-    for g in (aniso_geom(nx=37, ny=29, nz=23), small_geom(n=64, voxel=0.25, nu=20, nv=18, pix=2.4)):
-        vol = rng.standard_normal(g.vol_shape).astype(np.float32)
-        up = rng.standard_normal((1,) + g.det_shape).astype(np.float32)
-        dev = torch.device("cuda:0")
-        dfp.forward(g, f32([0.3]), f32([POSES3[0]]), torch.as_tensor(vol, device=dev))
-        assert dfp.last_path() == dfp.PATH_GATHER
-        check_forward(run_forward_case(dfp, g, [0.3], [POSES3[0]], vol, up))
+    dev = torch.device("cuda:0")
+    cases = ((aniso_geom(nx=37, ny=29, nz=23, nu=44, nv=36, du=1.0, dv=1.2), dfp.PATH_TMA),
+             (aniso_geom(nx=38, ny=30, nz=22, nu=40, nv=32, du=1.0, dv=1.2), dfp.PATH_TMA),
+             (small_geom(n=64, voxel=0.25, nu=20, nv=18, pix=2.4), dfp.PATH_GATHER))
+    for g, path in cases:
+        vol = rng.random(g.vol_shape).astype(np.float32)
+        up = rng.standard_normal((3,) + g.det_shape).astype(np.float32)
+        o = _both_paths(dfp, g, ANGLES3, POSES3, vol, up)
+        assert o["tma"][2] == path and o["tma"][3] == path, (g.nx, o["tma"][2:])
+        assert o["gather"][2] == dfp.PATH_GATHER and _same(o)
+        check_forward(run_forward_case(dfp, g, ANGLES3, POSES3, vol, up))
 
 
 # ------------------------------------------------------------------ the two back-projection kernel paths
@@ -313,10 +319,12 @@ def test_bp_tma_path_ragged_volume_off_detector_voxels_and_many_views(dfp):
         check_back(run_back_case(dfp, gg, angles, poses, proj, up))
 
 
-def test_bp_tma_path_falls_back_when_it_does_not_apply(dfp):
-    """nu % 4 != 0 (no tensor map), or a magnification so large that a tile's footprint exceeds the patch menu."""
+def test_bp_tma_path_odd_row_length_and_fallback(dfp):
+    """nu % 4 != 0: the TMA kernels read a row-padded copy of the projections (tensor maps need 16-byte-aligned rows) -
+    TMA path, same results.  A magnification so large that a tile's footprint exceeds the patch menu: the gather kernels."""
     rng = np.random.default_rng(22)
-    for g in (aniso_geom(nu=21, nv=17), small_geom(n=24, voxel=4.0, nu=400, nv=40, pix=0.1, sad=300.0, sdd=900.0)):
+    for g, path in ((aniso_geom(nu=21, nv=17), 1), (aniso_geom(nu=22, nv=19), 1),
+                    (small_geom(n=24, voxel=4.0, nu=400, nv=40, pix=0.1, sad=300.0, sdd=900.0), 0)):
         # smooth projections: at 120 pixels per voxel, white noise would measure the fp32 resolution of u (|u| <= 200
         # pixels -> 2e-5 pixel) rather than the kernel
         iv, iu = np.meshgrid(np.arange(g.nv), np.arange(g.nu), indexing="ij")
@@ -324,7 +332,9 @@ def test_bp_tma_path_falls_back_when_it_does_not_apply(dfp):
         proj = proj.astype(np.float32)
         up = rng.standard_normal(g.vol_shape).astype(np.float32)
         o = _both_bp_paths(dfp, g, ANGLES3[:2], POSES3[:2], proj, up)
-        assert o["tma"][2] == dfp.PATH_GATHER and o["tma"][3] == dfp.PATH_GATHER
+        want = dfp.PATH_TMA if path else dfp.PATH_GATHER
+        assert o["tma"][2] == want and o["tma"][3] == want, (g.nu, o["tma"][2:])
+        assert rel_l2(o["tma"][0], o["gather"][0]) <= 1e-5 and grad_err_u9(o["tma"][1], o["gather"][1]).max() <= 2e-3
         check_back(run_back_case(dfp, g, ANGLES3[:2], POSES3[:2], proj, up))
 
 
@@ -910,15 +920,16 @@ def test_dd_backprojector_is_deterministic_scale_free_and_accumulates(dfp):
 
 
 # ------------------------------------------------------------------ gradient kernels by view class
-@pytest.mark.parametrize("ny,launches", [(40, 5), (42, 3)])
-def test_gradient_kernels_by_view_class_non_cubic_grid(dfp, ny, launches):
+@pytest.mark.parametrize("nx,ny", [(48, 40), (48, 42), (46, 41)])
+def test_gradient_kernels_by_view_class_non_cubic_grid(dfp, nx, ny):
     """At >= 0.45 voxel per pixel dfp_forward_pose_grad sorts its views by the in-plane direction of their central ray:
     near the diagonals -> fwd_tma_kernel<1, 3>, along y -> <5, 6>, along x -> <6, 6> on a TRANSPOSED copy of the volume.
     A non-cubic, anisotropic grid (the transposed tensor map, the swapped centre indices and the swapped sums would all
     show), views of all three classes in one call in mixed order, general poses; the launch count proves that the three
-    kernels ran (3 + transpose + contraction).  ny % 4 != 0 admits no tensor map over the transposed volume: the views
-    along x then stay with the first kernel (2 + contraction)."""
-    g = W.Geometry(nx=48, ny=ny, nz=28, vx=0.5, vy=0.55, vz=0.5, nu=64, nv=40, du=0.4, dv=0.4, sad=400.0, sdd=600.0,
+    kernels ran (3 + transpose + contraction).  nx % 4 != 0 / ny % 4 != 0: the row-padded copy of the volume and the
+    row-padded transposed volume."""
+    launches = 5
+    g = W.Geometry(nx=nx, ny=ny, nz=28, vx=0.5, vy=0.55, vz=0.5, nu=64, nv=40, du=0.4, dv=0.4, sad=400.0, sdd=600.0,
                    cx=0.7, cy=-0.4, cz=0.3, u0=0.6, v0=-0.8).f32()
     angles = [0.05, 0.8, 1.6, 3.1, 2.4, 4.75, 5.5, 6.2, 1.45]
     rng = np.random.default_rng(77)
