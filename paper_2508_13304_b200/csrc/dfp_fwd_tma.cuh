@@ -121,6 +121,9 @@ __device__ __forceinline__ void tma_pixel(int bx, int by, int& iu, int& iv, int&
   iu = bx * T::TU + (warp % WU) * T::PU + (pix % T::PU);
   iv = by * T::TV + (warp / WU) * T::PV + (pix / T::PU);
 }
+#ifndef DFP_FWD_UNROLL
+#define DFP_FWD_UNROLL 0         // unroll factor of the forward kernels' sample loop (0: per box shape, see tma_march)
+#endif
 #ifndef DFP_ORIGIN_PRE
 #define DFP_ORIGIN_PRE 2         // bit 0: forward, bit 1: gradient kernels take the next box origin before the barrier
 #endif
@@ -308,6 +311,11 @@ __device__ __forceinline__ void tma_march(const VolLayout& L, const CUtensorMap*
     // immediate field and each of the 8 / 32 loads of a sample gets its own address add (measured: +20 % time)
     asm volatile("" : "+r"(c0));
     float kf = (float)kfirst, jf = 0.f;
+    // forward kernels: the sample loop unrolled by 2 (loop overhead, two samples' loads in flight: C2 7.15 -> 6.70 ms,
+    // C4 370 -> 349 ms), by 4 on C5's single-stage box (288 -> 283 ms; by 2 it gains nothing there); the gradient
+    // kernels are bound by the shared-memory pipe and keep the plain loop
+    constexpr int kUnroll = GRAD != 0 ? 1 : (DFP_FWD_UNROLL ? DFP_FWD_UNROLL : (SHAPE == 5 ? 4 : 2));
+#pragma unroll kUnroll
     for (int k = kfirst; k < kb; k += SLOTS) {
       // position, floor and fractions: x and y as one fp32x2 lane pair
       const float2 q2 = __ffma2_rn(make_float2(jf, jf), dpxy, bxy);
