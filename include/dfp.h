@@ -108,7 +108,7 @@ enum {
   DFP_ERR_DIMS = -2,       /* non-positive size / pitch, sad <= 0, sdd <= sad, n_views <= 0 or > 2^24, index overflow */
   DFP_ERR_NONFINITE = -3,  /* NaN / Inf in geometry, angles or poses                                        */
   DFP_ERR_ALIGN = -4,      /* a device pointer is not 16-byte (workspace: 256-byte) aligned                 */
-  DFP_ERR_WORKSPACE = -5,  /* ws_bytes < dfp_workspace_bytes(...)                                           */
+  DFP_ERR_WORKSPACE = -5,  /* ws_bytes < dfp_workspace_bytes_for_views(...) (<= dfp_workspace_bytes(...))           */
   DFP_ERR_CUDA = -6,       /* CUDA runtime error (no device, launch failure, out of memory in *_host)       */
   DFP_ERR_STATIC_LIMIT = -7 /* n_views > DFP_NCC_STATIC_MAX_VIEWS in dfp_ncc_pose_grad_static               */
 };
@@ -192,6 +192,19 @@ int dfp_ncc_pose_grad_static(const dfp_geometry* geometry, int n_views, const fl
  * d_proj) call them on consecutive slices of the view arrays - views are independent in forward /
  * forward_pose_grad / *_pose_grad, and dfp_backproject of a slice can be summed by the caller. */
 size_t dfp_workspace_bytes(const dfp_geometry* geometry, int n_views, int op);
+
+/* The bytes of workspace the op needs for THESE views (host arrays, as passed to the call; 0 on invalid arguments):
+ * dfp_workspace_bytes is the size that serves any views - it reserves the gather kernels' 4x packed copy of the volume
+ * (forward calls) or of the projections (back-projection calls), which only views whose tiles fit no staging box take
+ * (DFP_PATH_GATHER; none of BASELINE.json's configs).  When these views take the TMA-staged kernels the size returned
+ * here leaves that copy out (512^3 volume: 2.1 GiB -> 0.1 GiB for dfp_forward; 360 views of 1024^2: 5.7 -> 0.01 GiB for
+ * dfp_backproject); otherwise, and for the other weight models, n_views > 65532 and DFP_OP_NCC, it equals
+ * dfp_workspace_bytes.  A call checks ws_bytes against exactly this size for its own views (always <=
+ * dfp_workspace_bytes) and returns DFP_ERR_WORKSPACE, before any launch, if it is smaller.  The size depends on the
+ * views only through the kernel path they take: a workspace sized for one set of poses serves every other set that
+ * takes the same path, and dfp_workspace_bytes serves all. */
+size_t dfp_workspace_bytes_for_views(const dfp_geometry* geometry, int n_views, const float* angles, const float* poses,
+                                     int op);
 
 /* Same four operations with HOST buffers (h_*: host memory, pinned or pageable).  Each allocates device
  * scratch with cudaMallocAsync on `stream`, copies inputs in, runs the device call above, copies the result

@@ -88,6 +88,8 @@ def _load():
         f.restype = ci
     lib.dfp_workspace_bytes.argtypes = [gp, ci, ci]
     lib.dfp_workspace_bytes.restype = sz
+    lib.dfp_workspace_bytes_for_views.argtypes = [gp, ci, vp, vp, ci]
+    lib.dfp_workspace_bytes_for_views.restype = sz
     lib.dfp_count_ray_steps.argtypes = [gp, ci, vp, vp]
     lib.dfp_count_ray_steps.restype = ctypes.c_int64
     lib.dfp_set_kernel_timing.argtypes = [ci]
@@ -161,14 +163,25 @@ def workspace_bytes(geom, n_views: int, op: int) -> int:
     return int(_lib.dfp_workspace_bytes(ctypes.byref(Geometry.of(geom)), int(n_views), int(op)))
 
 
-def _workspace(g, V, op, ws, device):
-    need = workspace_bytes(g, V, op)
-    if need == 0:
-        _check(-2)
+def workspace_bytes_for_views(geom, angles, poses, op: int) -> int:
+    """dfp_workspace_bytes_for_views: the bytes the op needs for THESE views (<= workspace_bytes; without the gather
+    path's 4x packed copy when the views take the TMA-staged kernels)."""
+    g = Geometry.of(geom)
+    a, p, V = _views(angles, poses, geom)
+    return int(_lib.dfp_workspace_bytes_for_views(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p), int(op)))
+
+
+def _workspace(g, V, op, ws, device, a=None, p=None):
+    """The caller's workspace as (tensor, pointer, bytes) - its size is checked by the library - or, if none was given, a
+    new one of the size these views need."""
     if ws is None:
+        if a is None:
+            need = workspace_bytes(g, V, op)
+        else:
+            need = int(_lib.dfp_workspace_bytes_for_views(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p), int(op)))
+        if need == 0:
+            _check(-2)
         ws = torch.empty(need, dtype=torch.uint8, device=device)
-    elif ws.numel() * ws.element_size() < need:
-        _check(-5)
     return ws, ctypes.c_void_p(ws.data_ptr()), ctypes.c_size_t(ws.numel() * ws.element_size())
 
 
@@ -199,7 +212,7 @@ def forward(geom, angles, poses, vol, out=None, ws=None):
     a, p, V = _views(angles, poses, geom)
     if out is None:
         out = torch.empty((V, g.nv, g.nu), dtype=torch.float32, device=vol.device)
-    ws, wp, wn = _workspace(g, V, OP_FORWARD, ws, vol.device)
+    ws, wp, wn = _workspace(g, V, OP_FORWARD, ws, vol.device, a, p)
     with _same_device(vol, out, ws):
         _check(_lib.dfp_forward(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p), _dev(vol, (g.nz, g.ny, g.nx), "vol"),
                                 _dev(out, (V, g.nv, g.nu), "proj"), wp, wn, _stream(vol)))
@@ -212,7 +225,7 @@ def forward_pose_grad(geom, angles, poses, vol, dLdproj, out=None, ws=None):
     a, p, V = _views(angles, poses, geom)
     if out is None:
         out = torch.empty((V, 6), dtype=torch.float32, device=vol.device)
-    ws, wp, wn = _workspace(g, V, OP_FORWARD_POSE_GRAD, ws, vol.device)
+    ws, wp, wn = _workspace(g, V, OP_FORWARD_POSE_GRAD, ws, vol.device, a, p)
     with _same_device(vol, dLdproj, out, ws):
         _check(_lib.dfp_forward_pose_grad(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p),
                                           _dev(vol, (g.nz, g.ny, g.nx), "vol"),
@@ -229,7 +242,7 @@ def forward_fused_moments(geom, angles, poses, vol, target, out_proj=None, out_m
         out_proj = torch.empty((V, g.nv, g.nu), dtype=torch.float32, device=vol.device)
     if out_moments is None:
         out_moments = torch.empty((V, 3, 6), dtype=torch.float32, device=vol.device)
-    ws, wp, wn = _workspace(g, V, OP_FORWARD_FUSED, ws, vol.device)
+    ws, wp, wn = _workspace(g, V, OP_FORWARD_FUSED, ws, vol.device, a, p)
     with _same_device(vol, target, out_proj, out_moments, ws):
         _check(_lib.dfp_forward_fused_moments(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p),
                                               _dev(vol, (g.nz, g.ny, g.nx), "vol"),
@@ -278,7 +291,7 @@ def backproject(geom, angles, poses, proj, out=None, ws=None):
     a, p, V = _views(angles, poses, geom)
     if out is None:
         out = torch.empty((g.nz, g.ny, g.nx), dtype=torch.float32, device=proj.device)
-    ws, wp, wn = _workspace(g, V, OP_BACKPROJECT, ws, proj.device)
+    ws, wp, wn = _workspace(g, V, OP_BACKPROJECT, ws, proj.device, a, p)
     with _same_device(proj, out, ws):
         _check(_lib.dfp_backproject(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p), _dev(proj, (V, g.nv, g.nu), "proj"),
                                     _dev(out, (g.nz, g.ny, g.nx), "vol"), wp, wn, _stream(proj)))
@@ -291,7 +304,7 @@ def backproject_pose_grad(geom, angles, poses, proj, dLdvol, out=None, ws=None):
     a, p, V = _views(angles, poses, geom)
     if out is None:
         out = torch.empty((V, 6), dtype=torch.float32, device=proj.device)
-    ws, wp, wn = _workspace(g, V, OP_BACKPROJECT_POSE_GRAD, ws, proj.device)
+    ws, wp, wn = _workspace(g, V, OP_BACKPROJECT_POSE_GRAD, ws, proj.device, a, p)
     with _same_device(proj, dLdvol, out, ws):
         _check(_lib.dfp_backproject_pose_grad(ctypes.byref(g), V, _np_ptr(a), _np_ptr(p),
                                               _dev(proj, (V, g.nv, g.nu), "proj"),

@@ -355,7 +355,10 @@ struct FwdWs {
   int gx, gy;     // blocks per view (16 x 16-pixel tiles)
   int gy8;        // rows of 16 x 8-pixel tiles (TMA gradient kernel)
 };
-FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad, int nset = 1) {
+// `packed`: reserve the gather path's 4x packed copy of the volume (and, for the weight models that use it, the per-voxel
+// gradient volume).  packed = false is the layout of a trilinear call that takes the TMA path: only the row-padded
+// copy for nx % 4 != 0 lives there.
+FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad, int nset = 1, bool packed = true) {
   FwdWs w;
   const VolLayout L = make_layout(g);
   w.gx = (g.nu + kFwdTU - 1) / kFwdTU;
@@ -365,7 +368,10 @@ FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad, int nset = 1) {
   w.off_views = o; o += align_up(sizeof(FwdView) * (size_t)V);
   w.off_dd = o;    o += (g.flags & (DFP_FLAG_DD | DFP_FLAG_SF)) ? align_up(sizeof(DdView) * (size_t)V) : 0;
   w.off_con = o;   o += grad ? align_up(sizeof(FwdContract) * (size_t)V) : 0;
-  w.off_pvol = o;  o += align_up(sizeof(float4) * (size_t)L.px * L.py * L.pz);
+  if (g.flags & (DFP_FLAG_SIDDON | DFP_FLAG_JOSEPH | DFP_FLAG_DD | DFP_FLAG_SF)) packed = true;
+  w.off_pvol = o;
+  o += packed ? align_up(sizeof(float4) * (size_t)L.px * L.py * L.pz)
+              : ((g.nx % 4) ? align_up(sizeof(float) * (size_t)((g.nx + 3) / 4 * 4) * g.ny * g.nz) : 0);
   {
     size_t nblk = (size_t)w.gx * w.gy8;
     if (g.flags & DFP_FLAG_SF) nblk = ((size_t)g.nx * g.ny * g.nz + kSfThreads - 1) / kSfThreads;   // sf_kernel blocks
@@ -373,8 +379,11 @@ FwdWs fwd_ws(const dfp_geometry& g, int V, bool grad, int nset = 1) {
   }
   // the paper's gradient mode on the TMA path, >= 0.45 voxel per pixel: view lists of the three ray-direction classes and
   // the transposed volume of the views along x (dfp_fwd_tma.cuh, MODE 5 / 6)
+  // (taken where a pixel spans >= 0.45 voxel along z; reserved from 0.40 on, and always with explicit view frames, whose
+  // pixel pitch is per view)
   const bool classes = grad && nset == 1 && !(g.flags & (DFP_FLAG_GRAD_INTERP | DFP_FLAG_SIDDON | DFP_FLAG_JOSEPH | DFP_FLAG_DD |
-                                                         DFP_FLAG_SF | DFP_FLAG_NO_TMA));
+                                                         DFP_FLAG_SF | DFP_FLAG_NO_TMA)) &&
+                       ((g.flags & DFP_FLAG_VIEW_FRAMES) || (double)g.dv * ((double)g.sad / (double)g.sdd) / (double)g.vz >= 0.40);
   w.off_ids = o;  o += classes ? align_up(sizeof(int) * 3 * (size_t)V) : 0;
   w.off_volt = o; o += classes ? align_up(sizeof(float) * (size_t)g.nx * ((g.ny + 3) / 4 * 4) * g.nz) : 0;
   // sf_kernel<0>: SfFixed (256 bytes) + the 64-bit fixed-point accumulator image
@@ -389,7 +398,9 @@ struct BpWs {
   int gx, gy, gz;  // voxel tiles (gather path)
   int tx, ty, tz;  // voxel tiles (TMA path)
 };
-BpWs bp_ws(const dfp_geometry& g, int V, bool grad) {
+// `packed`: reserve the gather path's 4x packed copy of the projections (false: the layout of a call on the TMA path - only
+// the row-padded copy for nu % 4 != 0 lives there; the DD / SF models use neither).
+BpWs bp_ws(const dfp_geometry& g, int V, bool grad, bool packed = true) {
   BpWs w;
   w.gx = (g.nx + kBpTX - 1) / kBpTX;
   w.gy = (g.ny + kBpTY - 1) / kBpTY;
@@ -403,7 +414,10 @@ BpWs bp_ws(const dfp_geometry& g, int V, bool grad) {
   w.off_viewsd = o; o += align_up(sizeof(BpViewD) * (size_t)V);
   w.off_dd = o;    o += (g.flags & (DFP_FLAG_DD | DFP_FLAG_SF)) ? align_up(sizeof(DdView) * (size_t)V) : 0;
   w.off_con = o;   o += grad ? align_up(sizeof(BpContract) * (size_t)V) : 0;
-  w.off_q = o;     o += align_up(sizeof(float4) * (size_t)V * (g.nu + 2 * kPadDet) * (g.nv + 2 * kPadDet));
+  w.off_q = o;
+  if (g.flags & (DFP_FLAG_DD | DFP_FLAG_SF)) o += 0;
+  else if (packed) o += align_up(sizeof(float4) * (size_t)V * (g.nu + 2 * kPadDet) * (g.nv + 2 * kPadDet));
+  else o += (g.nu % 4) ? align_up(sizeof(float) * (size_t)V * ((g.nu + 3) / 4 * 4) * g.nv) : 0;
   w.off_part = o;
   {
     const size_t t_gather = (size_t)w.gx * w.gy * w.gz, t_tma = (size_t)w.tx * w.ty * w.tz;
@@ -436,6 +450,49 @@ int check_common(const dfp_geometry* g, int n_views, const float* angles, const 
   return DFP_OK;
 }
 
+// Which staging box (dfp_fwd_tma.cuh) a trilinear forward call takes for these views: -1 = none, the gather kernels.
+// Purely geometric (host): dfp_workspace_bytes_for_views and the call itself must agree on it.
+struct FwdChoice { int shape; bool half_tile, wide; };
+const int kBoxes[kNumShapes][3] = {{BoxShape<0>::X, BoxShape<0>::Y, BoxShape<0>::Z}, {BoxShape<1>::X, BoxShape<1>::Y, BoxShape<1>::Z},
+                                   {BoxShape<2>::X, BoxShape<2>::Y, BoxShape<2>::Z}, {BoxShape<3>::X, BoxShape<3>::Y, BoxShape<3>::Z},
+                                   {BoxShape<4>::X, BoxShape<4>::Y, BoxShape<4>::Z}, {BoxShape<5>::X, BoxShape<5>::Y, BoxShape<5>::Z},
+                                   {BoxShape<6>::X, BoxShape<6>::Y, BoxShape<6>::Z}};
+FwdChoice fwd_choice(const dfp_geometry& g, const FwdGeom& G, const std::vector<FwdView>& hv, const std::vector<ViewFrame>& hf,
+                     int V, bool grad) {
+  // forward: shapes 0, 1, 2 (16 x 16-pixel tiles) - with the odd-extent boxes 4, 5 first where a pixel spans >= 0.45
+  // voxel along z (bank conflicts, dfp_fwd_tma.cuh); gradient: shapes 3, 2 (16 x 8-pixel tiles)
+#ifndef DFP_WIDE_A
+#define DFP_WIDE_A 4
+#define DFP_WIDE_B 5
+#endif
+  static const int kOrderFwd[3] = {0, 1, 2}, kOrderFwdWide[5] = {DFP_WIDE_A, DFP_WIDE_B, 0, 1, 2}, kOrderGrad[2] = {3, 2};
+  FwdChoice c{-1, false, false};
+  c.wide = hf[0].vlen * ((double)g.sad / hf[0].sdd) / (double)g.vz >= 0.45;
+  if (g.flags & DFP_FLAG_NO_TMA) return c;
+  const int* order = grad ? kOrderGrad : (c.wide ? kOrderFwdWide : kOrderFwd);
+  const int n_order = grad ? 2 : (c.wide ? 5 : 3);
+  const int TU = grad ? TmaLanes<1>::TU : TmaLanes<0>::TU, TV = grad ? TmaLanes<1>::TV : TmaLanes<0>::TV;
+  for (int i = 0; i < n_order && c.shape < 0; ++i) {
+    bool fits = true;
+    for (int v = 0; fits && v < V; ++v) fits = tma_view_fits(g, G, hv[v], hf[v], grad, kBoxes[order[i]], TU, TV);
+    if (fits) c.shape = order[i];
+  }
+  // last resort before the gather kernels (coarse pixels on fine voxels, e.g. C1's forward call: 1.2 voxels per
+  // pixel): the largest box with chunks of two samples - short chunks, but no packed copy of the volume
+  if (c.shape < 0) {
+    bool fits = true;
+    for (int v = 0; fits && v < V; ++v) fits = tma_view_fits(g, G, hv[v], hf[v], grad, kBoxes[2], TU, TV, 2);
+    if (fits) c.shape = 2;
+  }
+  if (c.shape < 0 && !grad) {          // forward only: the same box under a 16 x 8-pixel tile (MODE 4)
+    bool fits = true;
+    for (int v = 0; fits && v < V; ++v)
+      fits = tma_view_fits(g, G, hv[v], hf[v], false, kBoxes[2], TmaLanes<4>::TU, TmaLanes<4>::TV, 2);
+    if (fits) { c.shape = 2; c.half_tile = true; }
+  }
+  return c;
+}
+
 // op = DFP_OP_FORWARD (d_out = projections), DFP_OP_FORWARD_POSE_GRAD (d_up = upstream, d_out = gradients) or
 // DFP_OP_FORWARD_FUSED (d_up = target b, d_out = moments [V][3][6], d_proj = projections)
 int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const float* poses, const float* d_vol,
@@ -454,9 +511,8 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
       (fused || (g->flags & DFP_FLAG_GRAD_INTERP) || (int)siddon + (int)joseph + (int)dd + (int)sf > 1))
     return DFP_ERR_DIMS;
   const int nset = fused ? 3 : 1;
-  const FwdWs w = fwd_ws(*g, V, grad, nset);
   st = check_common(g, V, angles, poses, d_vol, d_out, grad ? (const void*)d_up : (const void*)d_vol, d_ws,
-                        ws_bytes, w.total);
+                        ws_bytes, 0);          // everything but the workspace size, which depends on the path
   if (st) return st;
   const bool interp = grad && (g->flags & DFP_FLAG_GRAD_INTERP);
   const FwdGeom G = make_fwd_geom(*g, grad, interp);
@@ -468,6 +524,20 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
     make_fwd_view(hf[v], poses + 6 * v, &hv[v], grad ? &hc[v] : nullptr);
   }
   char* base = static_cast<char*>(d_ws);
+  // The kernel path first (host geometry only): a trilinear call whose views fit a staging box needs no packed copy of
+  // the volume, and its workspace is laid out without one (dfp_workspace_bytes_for_views returns that size).
+  const bool plain = !(siddon || joseph || dd || sf);
+  const FwdChoice choice = plain ? fwd_choice(*g, G, hv, hf, V, grad) : FwdChoice{-1, false, false};
+  const FwdWs w_tma = fwd_ws(*g, V, grad, nset, false);
+  CUtensorMap vol_map;
+  // nx % 4 != 0: the TMA kernels read a copy of the volume with 16-byte-aligned rows (1x the volume, at off_pvol - the
+  // same offset in both layouts)
+  const int vpitch = pitch4(g->nx);
+  const float* tma_vol = vpitch == g->nx ? d_vol : reinterpret_cast<const float*>(base + w_tma.off_pvol);
+  const bool tma = choice.shape >= 0 && make_volume_map(*g, tma_vol, vpitch, kBoxes[choice.shape][0], kBoxes[choice.shape][1],
+                                                        kBoxes[choice.shape][2], &vol_map);
+  const FwdWs w = tma ? w_tma : fwd_ws(*g, V, grad, nset, true);
+  if (ws_bytes < w.total) return DFP_ERR_WORKSPACE;
   FwdView* dv = reinterpret_cast<FwdView*>(base + w.off_views);
   FwdContract* dc = reinterpret_cast<FwdContract*>(base + w.off_con);
   float4* pvol = reinterpret_cast<float4*>(base + w.off_pvol);
@@ -555,54 +625,10 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
     DFP_CUDA(cudaGetLastError(), "forward launch (Siddon / Joseph weights)");
     return DFP_OK;
   }
-  // TMA-staged path when the volume admits a tensor map and every view's tiles fit a staging box: the smallest
-  // box (dfp_fwd_tma.cuh) that holds every view's tiles
-  CUtensorMap vol_map;
-  static const int kBoxes[kNumShapes][3] = {{BoxShape<0>::X, BoxShape<0>::Y, BoxShape<0>::Z},
-                                            {BoxShape<1>::X, BoxShape<1>::Y, BoxShape<1>::Z},
-                                            {BoxShape<2>::X, BoxShape<2>::Y, BoxShape<2>::Z},
-                                            {BoxShape<3>::X, BoxShape<3>::Y, BoxShape<3>::Z},
-                                            {BoxShape<4>::X, BoxShape<4>::Y, BoxShape<4>::Z},
-                                            {BoxShape<5>::X, BoxShape<5>::Y, BoxShape<5>::Z},
-                                            {BoxShape<6>::X, BoxShape<6>::Y, BoxShape<6>::Z}};
-  // forward: shapes 0, 1, 2 (16 x 16-pixel tiles) - with the odd-extent boxes 4, 5 first where a pixel spans >= 0.45
-  // voxel along z (bank conflicts, dfp_fwd_tma.cuh); gradient: shapes 3, 2 (16 x 8-pixel tiles)
-#ifndef DFP_WIDE_A
-#define DFP_WIDE_A 4
-#define DFP_WIDE_B 5
-#endif
-  static const int kOrderFwd[3] = {0, 1, 2}, kOrderFwdWide[5] = {DFP_WIDE_A, DFP_WIDE_B, 0, 1, 2}, kOrderGrad[2] = {3, 2};
-  const bool wide = hf[0].vlen * ((double)g->sad / hf[0].sdd) / (double)g->vz >= 0.45;
-  const int* order = grad ? kOrderGrad : (wide ? kOrderFwdWide : kOrderFwd);
-  const int n_order = grad ? 2 : (wide ? 5 : 3);
+  // TMA-staged path when every view's tiles fit a staging box: the first box of the op's list that holds them (fwd_choice)
+  const int shape = choice.shape;
+  const bool half_tile = choice.half_tile, wide = choice.wide;
   const int TU = grad ? TmaLanes<1>::TU : TmaLanes<0>::TU, TV = grad ? TmaLanes<1>::TV : TmaLanes<0>::TV;
-  int shape = -1;
-  bool half_tile = false;
-  if (!(g->flags & DFP_FLAG_NO_TMA)) {
-    for (int i = 0; i < n_order && shape < 0; ++i) {
-      bool fits = true;
-      for (int v = 0; fits && v < V; ++v) fits = tma_view_fits(*g, G, hv[v], hf[v], grad, kBoxes[order[i]], TU, TV);
-      if (fits) shape = order[i];
-    }
-    // last resort before the gather kernels (coarse pixels on fine voxels, e.g. C1's forward call: 1.2 voxels per
-    // pixel): the largest box with chunks of two samples - short chunks, but no packed copy of the volume
-    if (shape < 0) {
-      bool fits = true;
-      for (int v = 0; fits && v < V; ++v) fits = tma_view_fits(*g, G, hv[v], hf[v], grad, kBoxes[2], TU, TV, 2);
-      if (fits) shape = 2;
-    }
-    if (shape < 0 && !grad) {          // forward only: the same box under a 16 x 8-pixel tile (MODE 4)
-      bool fits = true;
-      for (int v = 0; fits && v < V; ++v)
-        fits = tma_view_fits(*g, G, hv[v], hf[v], false, kBoxes[2], TmaLanes<4>::TU, TmaLanes<4>::TV, 2);
-      if (fits) { shape = 2; half_tile = true; }
-    }
-  }
-  // nx % 4 != 0: the TMA kernels read a copy of the volume with 16-byte-aligned rows (1x the volume, in the workspace
-  // region of the gather path's 4x packed copy, which is then not built)
-  const int vpitch = pitch4(g->nx);
-  const float* tma_vol = vpitch == g->nx ? d_vol : reinterpret_cast<const float*>(pvol);
-  const bool tma = shape >= 0 && make_volume_map(*g, tma_vol, vpitch, kBoxes[shape][0], kBoxes[shape][1], kBoxes[shape][2], &vol_map);
   g_path = tma ? DFP_PATH_TMA : DFP_PATH_GATHER;
   if (tma) {
     DFP_CUDA(ensure_smem_attributes(), "cudaFuncSetAttribute");
@@ -728,6 +754,24 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
   return DFP_OK;
 }
 
+// Which patch menu entry (dfp_bp_tma.cuh) and tile depth a voxel-driven back-projection call takes for these views:
+// kmax < 0 = the gather kernels.  Host geometry only (dfp_workspace_bytes_for_views and the call must agree).
+struct BpChoice { int kmax, TZ; };
+BpChoice bp_choice(const dfp_geometry& g, const BpGeom& G, const std::vector<BpView>& hv, int V, bool grad) {
+  BpChoice c{-1, 16};
+  if (g.flags & DFP_FLAG_NO_TMA) return c;
+  for (c.TZ = 16; c.TZ >= 8 && c.kmax < 0; c.TZ >>= 1) {
+    c.kmax = 0;
+    for (int v = 0; v < V && c.kmax >= 0; ++v) {
+      const int k = bp_view_patch(G, hv[v], c.TZ, grad ? 1 : 0);
+      c.kmax = k < 0 ? -1 : (k > c.kmax ? k : c.kmax);
+    }
+    if (c.kmax >= 0 && bp_num_stages(c.kmax) < 2) c.kmax = -1;      // a single stage would serialise TMA and compute
+    if (c.kmax >= 0) break;
+  }
+  return c;
+}
+
 int run_backproject_slice(const dfp_geometry* g, int V, const float* angles, const float* poses, const float* d_proj,
                           const float* d_up, float* d_out, void* d_ws, size_t ws_bytes, cudaStream_t s, bool grad) {
   if (!g) return DFP_ERR_NULL;
@@ -737,9 +781,8 @@ int run_backproject_slice(const dfp_geometry* g, int V, const float* angles, con
       (g->bp_weight != 0 || (g->flags & (DFP_FLAG_GRAD_INTERP | DFP_FLAG_SIDDON | DFP_FLAG_JOSEPH)) ||
        (g->flags & (DFP_FLAG_DD | DFP_FLAG_SF)) == (DFP_FLAG_DD | DFP_FLAG_SF)))
     return DFP_ERR_DIMS;     // the DD / SF back-projectors are plain transposes: unit weight, central differences only
-  const BpWs w = bp_ws(*g, V, grad);
   st = check_common(g, V, angles, poses, d_proj, d_out, grad ? (const void*)d_up : (const void*)d_proj, d_ws,
-                        ws_bytes, w.total);
+                        ws_bytes, 0);          // everything but the workspace size, which depends on the path
   if (st) return st;
   const BpGeom G = make_bp_geom(*g);
   std::vector<BpView> hv((size_t)V);
@@ -748,6 +791,18 @@ int run_backproject_slice(const dfp_geometry* g, int V, const float* angles, con
   for (int v = 0; v < V; ++v)
     make_bp_view(*g, G, make_frame(*g, angles, v), poses + 6 * v, &hv[v], grad ? &hc[v] : nullptr, &hvd[v]);
   char* base = static_cast<char*>(d_ws);
+  // The kernel path first (host geometry only): on the TMA path the workspace holds no packed copy of the projections
+  const bool vd = !(g->flags & (DFP_FLAG_DD | DFP_FLAG_SF));
+  const BpChoice choice = vd ? bp_choice(*g, G, hv, V, grad) : BpChoice{-1, 16};
+  const BpWs w_tma = bp_ws(*g, V, grad, false);
+  PatchMaps maps;
+  // nu % 4 != 0: the TMA kernels read a copy of the projections with 16-byte-aligned rows (at off_q, the same offset in
+  // both layouts)
+  const int ppitch = pitch4(g->nu);
+  const float* tma_proj = ppitch == g->nu ? d_proj : reinterpret_cast<const float*>(base + w_tma.off_q);
+  const bool tma = choice.kmax >= 0 && make_proj_maps(*g, V, tma_proj, ppitch, choice.kmax, &maps);
+  const BpWs w = tma ? w_tma : bp_ws(*g, V, grad, true);
+  if (ws_bytes < w.total) return DFP_ERR_WORKSPACE;
   BpView* dv = reinterpret_cast<BpView*>(base + w.off_views);
   BpViewD* dvd = reinterpret_cast<BpViewD*>(base + w.off_viewsd);
   BpContract* dc = reinterpret_cast<BpContract*>(base + w.off_con);
@@ -824,25 +879,9 @@ int run_backproject_slice(const dfp_geometry* g, int V, const float* angles, con
     DFP_CUDA(cudaGetLastError(), "back-projection launch (distance-driven weights)");
     return DFP_OK;
   }
-  // TMA-staged path: projections admit a tensor map, every voxel in front of the source, patches fit the menu
-  int kmax = -1, TZ = 16;
-  if (!(g->flags & DFP_FLAG_NO_TMA)) {
-    for (TZ = 16; TZ >= 8 && kmax < 0; TZ >>= 1) {
-      kmax = 0;
-      for (int v = 0; v < V && kmax >= 0; ++v) {
-        const int k = bp_view_patch(G, hv[v], TZ, grad ? 1 : 0);
-        kmax = k < 0 ? -1 : (k > kmax ? k : kmax);
-      }
-      if (kmax >= 0 && bp_num_stages(kmax) < 2) kmax = -1;      // a single stage would serialise TMA and compute
-      if (kmax >= 0) break;
-    }
-  }
-  PatchMaps maps;
-  // nu % 4 != 0: the TMA kernels read a copy of the projections with 16-byte-aligned rows (in the workspace region of the
-  // gather path's 4x packed copy, which is then not built)
-  const int ppitch = pitch4(g->nu);
-  const float* tma_proj = ppitch == g->nu ? d_proj : reinterpret_cast<const float*>(base + w.off_q);
-  if (kmax >= 0 && make_proj_maps(*g, V, tma_proj, ppitch, kmax, &maps)) {
+  // TMA-staged path: every voxel in front of the source, patches fit the menu (bp_choice)
+  const int kmax = choice.kmax, TZ = choice.TZ;
+  if (tma) {
     const int stage_words = bp_stage_words(kmax), n_stages = bp_num_stages(kmax);
     const int smem = stage_words * 4 * n_stages;
     DFP_CUDA(ensure_smem_attributes(), "cudaFuncSetAttribute");
@@ -998,7 +1037,10 @@ int run_host(int op, const dfp_geometry* g, int V, const float* angles, const fl
   const size_t n_in = fwd ? nvol : nproj;
   const size_t n_up = grad ? (fwd ? nproj : nvol) : 0;
   const size_t n_out = grad ? ngrad : (fwd ? nproj : nvol);
-  const size_t n_ws = dfp_workspace_bytes(g, V, op);
+  // what these views need (a subset of views that take the TMA path takes it too, with a smaller layout): no 4x packed
+  // copy on the TMA path
+  size_t n_ws = dfp_workspace_bytes_for_views(g, V, angles, poses, op);
+  if (n_ws == 0) n_ws = dfp_workspace_bytes(g, V, op);
   DevBuf d_in(s), d_up(s), d_out(s), d_ws(s);
   DFP_CUDA(d_in.alloc(n_in), "cudaMallocAsync");
   DFP_CUDA(d_up.alloc(n_up), "cudaMallocAsync");
@@ -1209,6 +1251,32 @@ size_t dfp_workspace_bytes(const dfp_geometry* g, int n_views, int op) {
     case DFP_OP_NCC: return align_up(sizeof(double) * 5 * (size_t)kNccBlocks * (size_t)n_views);
     default: return 0;
   }
+}
+
+size_t dfp_workspace_bytes_for_views(const dfp_geometry* g, int n_views, const float* angles, const float* poses, int op) {
+  const size_t full = dfp_workspace_bytes(g, n_views, op);
+  if (full == 0 || op == DFP_OP_NCC || n_views > kMaxViewsPerLaunch) return full;
+  if (validate_views(*g, n_views, angles, poses) != DFP_OK) return 0;
+  const int V = n_views;
+  if (op == DFP_OP_FORWARD || op == DFP_OP_FORWARD_POSE_GRAD || op == DFP_OP_FORWARD_FUSED) {
+    if (g->flags & (DFP_FLAG_SIDDON | DFP_FLAG_JOSEPH | DFP_FLAG_DD | DFP_FLAG_SF)) return full;
+    const bool grad = op != DFP_OP_FORWARD, interp = grad && (g->flags & DFP_FLAG_GRAD_INTERP);
+    const FwdGeom G = make_fwd_geom(*g, grad, interp);
+    std::vector<FwdView> hv((size_t)V);
+    std::vector<ViewFrame> hf((size_t)V);
+    for (int v = 0; v < V; ++v) {
+      hf[v] = make_frame(*g, angles, v);
+      make_fwd_view(hf[v], poses + 6 * v, &hv[v], nullptr);
+    }
+    return fwd_choice(*g, G, hv, hf, V, grad).shape >= 0 ? fwd_ws(*g, V, grad, op == DFP_OP_FORWARD_FUSED ? 3 : 1, false).total : full;
+  }
+  if (g->flags & (DFP_FLAG_DD | DFP_FLAG_SF)) return full;
+  const bool grad = op == DFP_OP_BACKPROJECT_POSE_GRAD;
+  const BpGeom G = make_bp_geom(*g);
+  std::vector<BpView> hv((size_t)V);
+  BpViewD scratch;
+  for (int v = 0; v < V; ++v) make_bp_view(*g, G, make_frame(*g, angles, v), poses + 6 * v, &hv[v], nullptr, &scratch);
+  return bp_choice(*g, G, hv, V, grad).kmax >= 0 ? bp_ws(*g, V, grad, false).total : full;
 }
 
 int dfp_forward_host(const dfp_geometry* g, int n_views, const float* angles, const float* poses, const float* h_vol,

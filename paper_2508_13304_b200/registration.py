@@ -84,7 +84,7 @@ def motion_compensated_backprojection(geom, views, proj, loss_fn, n_iters=80, lr
         host.copy_(grad, non_blocking=True)
         torch.cuda.current_stream(dev).synchronize()
         gr = host.double().numpy()
-        losses.append(float(loss))
+        losses.append(float(loss.detach()))
         if callback is not None:
             callback(it, theta, losses[-1])
         m = betas[0] * m + (1 - betas[0]) * gr

@@ -164,8 +164,39 @@ def test_new_flags_and_the_ncc_call_reject_bad_arguments_without_a_gpu(dfp):
     assert ncc(ctypes.byref(g), 2, ctypes.c_void_p(0x10004), fake, fake, fake, fake, fake, 1 << 20) == -4
     assert ncc(ctypes.byref(g), 2, fake, fake, fake, fake, fake, fake, 16) == -5
     assert dfp.workspace_bytes(g, 2, dfp.OP_NCC) > 0
-    # the other matched pairs need room for their per-view blocks and finer partial sums
-    assert dfp.workspace_bytes(dfp.Geometry.of(_geom(flags=128)), 3, 3) > dfp.workspace_bytes(g, 3, 3)
+    # the other matched pairs: per-view blocks, partial sums per pixel tile / voxel block, fixed-point accumulators - and
+    # no packed copy of the input
+    gd = dfp.Geometry.of(_geom(flags=128))
+    assert 0 < dfp.workspace_bytes(gd, 3, 3) < dfp.workspace_bytes(gd, 6, 3)
+    assert dfp.workspace_bytes(gd, 3, 2) >= 8 * 8 * 8 * 8                  # the 64-bit accumulator volume
+
+
+def test_workspace_bytes_for_views_without_a_gpu(dfp):
+    """dfp_workspace_bytes_for_views runs the host-side path choice: views whose tiles fit the staging boxes need no 4x
+    packed copy of the volume / projections; views that fit none, the other weight models and DFP_FLAG_NO_TMA need the
+    full size; invalid arguments give 0; and a call checks its workspace against exactly that size."""
+    ang, pose = np.array([0.3, 1.9, 4.0], np.float32), np.zeros((3, 6), np.float32)
+    d = dict(nx=64, ny=64, nz=64, vx=1.0, vy=1.0, vz=1.0, nu=128, nv=128, du=0.6, dv=0.6, sad=785.0, sdd=1200.0)
+    g = dfp.Geometry.of(_geom(**d))
+    for op in range(5):
+        full, exact = dfp.workspace_bytes(g, 3, op), dfp.workspace_bytes_for_views(g, ang, pose, op)
+        assert 0 < exact < full and exact % 256 == 0, (op, exact, full)
+        assert full - exact >= 12 * (64 ** 3 if op in (0, 1, 4) else 3 * 128 * 128)      # the 16-byte-per-element packed copy
+        forced = dfp.workspace_bytes_for_views(dfp.Geometry.of(_geom(flags=2, **d)), ang, pose, op)      # DFP_FLAG_NO_TMA
+        assert forced == dfp.workspace_bytes(dfp.Geometry.of(_geom(flags=2, **d)), 3, op)
+    coarse = dfp.Geometry.of(_geom(nx=64, ny=64, nz=64, vx=0.25, vy=0.25, vz=0.25, nu=20, nv=18, du=2.4, dv=2.4))
+    assert dfp.workspace_bytes_for_views(coarse, ang, pose, 0) == dfp.workspace_bytes(coarse, 3, 0)
+    for flags in (8, 32, 128, 256):
+        gm = dfp.Geometry.of(_geom(flags=flags, **d))
+        assert dfp.workspace_bytes_for_views(gm, ang, pose, 1) == dfp.workspace_bytes(gm, 3, 1)
+    assert dfp.workspace_bytes_for_views(g, ang, pose, dfp.OP_NCC) == dfp.workspace_bytes(g, 3, dfp.OP_NCC)
+    bad = pose.copy()
+    bad[1, 2] = np.inf
+    assert dfp.workspace_bytes_for_views(g, ang, bad, 0) == 0 and dfp.workspace_bytes_for_views(g, ang, pose, 9) == 0
+    # odd row length: the exact size holds the row-padded 1x copy
+    g_odd = dfp.Geometry.of(_geom(**dict(d, nx=62)))
+    e0, e1 = dfp.workspace_bytes_for_views(g, ang, pose, 0), dfp.workspace_bytes_for_views(g_odd, ang, pose, 0)
+    assert 64 * 64 * 64 * 4 <= e1 - e0 + 4096 and e1 < dfp.workspace_bytes(g_odd, 3, 0)
 
 
 def test_static_ncc_entry_point_checks_its_arguments_without_a_gpu(dfp):

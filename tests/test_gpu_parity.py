@@ -946,3 +946,38 @@ def test_gradient_kernels_by_view_class_non_cubic_grid(dfp, nx, ny):
     ref = dfp.forward_pose_grad(gg, f32(angles), f32(poses), torch.as_tensor(vol, device=dev),
                                 torch.as_tensor(up, device=dev)).cpu().numpy()
     assert grad_err_u9(res[1], ref).max() <= 1e-4
+
+
+# ------------------------------------------------------------------ dfp_workspace_bytes_for_views
+def test_exact_size_workspace_serves_the_call_and_one_byte_less_does_not(dfp):
+    """A workspace of dfp_workspace_bytes_for_views bytes (no 4x packed copy: the views take the TMA path) gives the
+    same results, bit for bit, as the any-views size; 256 bytes less is DFP_ERR_WORKSPACE before any launch (the output
+    stays untouched).  Odd row lengths: the exact size holds the row-padded copy.  A geometry on the gather path: the
+    two sizes coincide."""
+    dev = torch.device("cuda:0")
+    for kw in (dict(), dict(nx=62, nu=126)):
+        w = W.make_config(2, scale=0.25, n_views=4)
+        g = w.geom.replace(**kw)
+        a, p = f32(w.angles.numpy()), f32(w.poses.numpy()).reshape(-1, 6)
+        rng = np.random.default_rng(61)
+        vol = torch.as_tensor(rng.random(g.vol_shape).astype(np.float32), device=dev)
+        up = torch.as_tensor(rng.standard_normal((4,) + g.det_shape).astype(np.float32), device=dev)
+        upv = torch.as_tensor(rng.standard_normal(g.vol_shape).astype(np.float32), device=dev)
+        calls = ((dfp.OP_FORWARD, lambda ws, out: dfp.forward(g, a, p, vol, out=out, ws=ws), (4,) + g.det_shape),
+                 (dfp.OP_FORWARD_POSE_GRAD, lambda ws, out: dfp.forward_pose_grad(g, a, p, vol, up, out=out, ws=ws), (4, 6)),
+                 (dfp.OP_BACKPROJECT, lambda ws, out: dfp.backproject(g, a, p, up, out=out, ws=ws), g.vol_shape),
+                 (dfp.OP_BACKPROJECT_POSE_GRAD, lambda ws, out: dfp.backproject_pose_grad(g, a, p, up, upv, out=out, ws=ws), (4, 6)))
+        for op, fn, shape in calls:
+            full, exact = dfp.workspace_bytes(g, 4, op), dfp.workspace_bytes_for_views(g, a, p, op)
+            assert 0 < exact < full // 2, (op, exact, full)
+            ref = fn(torch.empty(full, dtype=torch.uint8, device=dev), torch.empty(shape, device=dev)).clone()
+            assert dfp.last_path() == dfp.PATH_TMA
+            got = fn(torch.empty(exact, dtype=torch.uint8, device=dev), torch.empty(shape, device=dev))
+            assert dfp.last_path() == dfp.PATH_TMA and torch.equal(got, ref), op
+            untouched = torch.full(shape, 7.0, device=dev)
+            with pytest.raises(dfp.DfpError) as e:
+                fn(torch.empty(exact - 256, dtype=torch.uint8, device=dev), untouched)
+            assert e.value.status == -5 and bool((untouched == 7.0).all())
+    gg = small_geom(n=64, voxel=0.25, nu=20, nv=18, pix=2.4)
+    a1, p1 = f32([0.3]), f32([POSES3[0]])
+    assert dfp.workspace_bytes_for_views(gg, a1, p1, dfp.OP_FORWARD) == dfp.workspace_bytes(gg, 1, dfp.OP_FORWARD)
