@@ -981,3 +981,40 @@ def test_exact_size_workspace_serves_the_call_and_one_byte_less_does_not(dfp):
     gg = small_geom(n=64, voxel=0.25, nu=20, nv=18, pix=2.4)
     a1, p1 = f32([0.3]), f32([POSES3[0]])
     assert dfp.workspace_bytes_for_views(gg, a1, p1, dfp.OP_FORWARD) == dfp.workspace_bytes(gg, 1, dfp.OP_FORWARD)
+
+
+def test_exact_size_workspace_is_enough_for_random_geometries(dfp):
+    """dfp_workspace_bytes_for_views and the calls decide the kernel path with the same host code: over random grids,
+    detectors, magnifications, poses, weights and modes a workspace of exactly that size is never too small, whichever
+    path the call then takes, and the results do not depend on the workspace size."""
+    dev = torch.device("cuda:0")
+    rng = np.random.default_rng(97)
+    seen = set()
+    for trial in range(24):
+        n = [int(rng.integers(9, 41)) for _ in range(3)]
+        nu, nv = int(rng.integers(8, 70)), int(rng.integers(8, 50))
+        vox = float(rng.uniform(0.4, 1.5))
+        sad = float(rng.uniform(150.0, 600.0))
+        sdd = sad * float(rng.uniform(1.2, 2.0))
+        pix = vox * sdd / sad * float(rng.uniform(0.3, 2.5))
+        flags = int(rng.choice([0, 0, dfp.FLAG_GRAD_INTERP, dfp.FLAG_NO_TMA]))
+        g = W.Geometry(nx=n[0], ny=n[1], nz=n[2], vx=vox, vy=vox * 1.1, vz=vox * 0.9, nu=nu, nv=nv, du=pix, dv=pix * 1.05,
+                       sad=sad, sdd=sdd, bp_weight=int(rng.integers(0, 2)), flags=flags).f32()
+        V = int(rng.integers(1, 6))
+        a = f32(rng.uniform(0, 2 * np.pi, V))
+        p = f32(np.concatenate([rng.uniform(-2, 2, (V, 3)), rng.uniform(-0.1, 0.1, (V, 3))], axis=1))
+        vol = torch.as_tensor(rng.random(g.vol_shape).astype(np.float32), device=dev)
+        img = torch.as_tensor(rng.random((V,) + g.det_shape).astype(np.float32), device=dev)
+        for op, fn in ((dfp.OP_FORWARD, lambda ws: dfp.forward(g, a, p, vol, ws=ws)),
+                       (dfp.OP_FORWARD_POSE_GRAD, lambda ws: dfp.forward_pose_grad(g, a, p, vol, img, ws=ws)),
+                       (dfp.OP_BACKPROJECT, lambda ws: dfp.backproject(g, a, p, img, ws=ws)),
+                       (dfp.OP_BACKPROJECT_POSE_GRAD, lambda ws: dfp.backproject_pose_grad(g, a, p, img, vol, ws=ws))):
+            exact, full = dfp.workspace_bytes_for_views(g, a, p, op), dfp.workspace_bytes(g, V, op)
+            assert 0 < exact <= full
+            got = fn(torch.empty(exact, dtype=torch.uint8, device=dev)).clone()
+            path = dfp.last_path()
+            assert (exact < full) == (path == dfp.PATH_TMA), (trial, op, exact, full, path)
+            ref = fn(torch.empty(full + 4096, dtype=torch.uint8, device=dev))
+            assert dfp.last_path() == path and torch.equal(got, ref), (trial, op)
+            seen.add((op, path))
+    assert len(seen) == 8, seen          # both paths of all four calls were exercised
