@@ -53,13 +53,7 @@ template <> struct BoxShape<2> { static constexpr int X = 28, Y = 28, Z = 20, ST
 #ifndef DFP_GRAD_TV
 #define DFP_GRAD_TV 8
 #endif
-#ifndef DFP_GRAD_BY
-#define DFP_GRAD_BY 28
-#endif
-#ifndef DFP_GRAD_PU
-#define DFP_GRAD_PU 8
-#endif
-template <> struct BoxShape<3> { static constexpr int X = 28, Y = DFP_GRAD_BY, Z = 16, STAGES = DFP_GRAD_STAGES; };   // gradient, 16 x 8 tiles
+template <> struct BoxShape<3> { static constexpr int X = 28, Y = 28, Z = 16, STAGES = DFP_GRAD_STAGES; };   // gradient, 16 x 8 tiles
 // Forward boxes with an ODD y extent (slab pitch = 12 / 20 mod 32 instead of 16): where a warp's 8 x 4-pixel patch spans
 // three z slices (>= 0.45 voxel per pixel: the 512^3 configs), slab pitch 16 puts slices z and z + 2 on the same banks;
 // 1.76 -> 1.38 wavefronts per load on C5, 1.62 -> 1.36 on C4 (simulated, _and measured_ in DESIGN.md); at C2's 0.39
@@ -105,7 +99,7 @@ template <int MODE> struct TmaLanes {
   static constexpr int GRAD = tma_grad_of(MODE);
   static constexpr int SLOTS = GRAD ? DFP_GRAD_SLOTS : 1, TU = kFwdTU,
                        TV = MODE == 0 ? kFwdTV : (MODE == 4 ? 8 : DFP_GRAD_TV), THREADS = TU * TV * SLOTS;
-  static constexpr int PU = SLOTS == 4 ? 4 : (MODE >= 5 ? 4 : (SLOTS == 2 ? DFP_GRAD_PU : 8)), PV = 32 / (PU * SLOTS);
+  static constexpr int PU = SLOTS == 4 ? 4 : (MODE >= 5 ? 4 : 8), PV = 32 / (PU * SLOTS);
 #ifndef DFP_FWD_MINB
 #define DFP_FWD_MINB 4
 #endif
