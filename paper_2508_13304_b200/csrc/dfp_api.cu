@@ -325,6 +325,7 @@ cudaError_t ensure_smem_attributes() {
   DFP_ATTR((fwd_tma_kernel<0, 5>), tma_smem_bytes<5>());
   DFP_ATTR((fwd_tma_kernel<1, 2>), tma_smem_bytes<2>());
   DFP_ATTR((fwd_tma_kernel<1, 3>), tma_smem_bytes<3>());
+  DFP_ATTR((fwd_tma_kernel<1, 7>), tma_smem_bytes<7>());
   DFP_ATTR((fwd_tma_kernel<5, 6>), tma_smem_bytes<6>());
   DFP_ATTR((fwd_tma_kernel<6, 6>), tma_smem_bytes<6>());
   DFP_ATTR((fwd_tma_kernel<2, 2>), tma_smem_bytes<2>());
@@ -456,21 +457,23 @@ struct FwdChoice { int shape; bool half_tile, wide; };
 const int kBoxes[kNumShapes][3] = {{BoxShape<0>::X, BoxShape<0>::Y, BoxShape<0>::Z}, {BoxShape<1>::X, BoxShape<1>::Y, BoxShape<1>::Z},
                                    {BoxShape<2>::X, BoxShape<2>::Y, BoxShape<2>::Z}, {BoxShape<3>::X, BoxShape<3>::Y, BoxShape<3>::Z},
                                    {BoxShape<4>::X, BoxShape<4>::Y, BoxShape<4>::Z}, {BoxShape<5>::X, BoxShape<5>::Y, BoxShape<5>::Z},
-                                   {BoxShape<6>::X, BoxShape<6>::Y, BoxShape<6>::Z}};
+                                   {BoxShape<6>::X, BoxShape<6>::Y, BoxShape<6>::Z}, {BoxShape<7>::X, BoxShape<7>::Y, BoxShape<7>::Z}};
 FwdChoice fwd_choice(const dfp_geometry& g, const FwdGeom& G, const std::vector<FwdView>& hv, const std::vector<ViewFrame>& hf,
-                     int V, bool grad) {
+                     int V, bool grad, bool plain_grad = false) {
   // forward: shapes 0, 1, 2 (16 x 16-pixel tiles) - with the odd-extent boxes 4, 5 first where a pixel spans >= 0.45
   // voxel along z (bank conflicts, dfp_fwd_tma.cuh); gradient: shapes 3, 2 (16 x 8-pixel tiles)
 #ifndef DFP_WIDE_A
 #define DFP_WIDE_A 4
 #define DFP_WIDE_B 5
 #endif
-  static const int kOrderFwd[3] = {0, 1, 2}, kOrderFwdWide[5] = {DFP_WIDE_A, DFP_WIDE_B, 0, 1, 2}, kOrderGrad[2] = {3, 2};
+  // (the paper's gradient mode: the 14-slice box 7, five blocks per SM, before the 16-slice box 3)
+  static const int kOrderFwd[3] = {0, 1, 2}, kOrderFwdWide[5] = {DFP_WIDE_A, DFP_WIDE_B, 0, 1, 2}, kOrderGrad[2] = {3, 2},
+                   kOrderGradPlain[3] = {7, 3, 2};
   FwdChoice c{-1, false, false};
   c.wide = hf[0].vlen * ((double)g.sad / hf[0].sdd) / (double)g.vz >= 0.45;
   if (g.flags & DFP_FLAG_NO_TMA) return c;
-  const int* order = grad ? kOrderGrad : (c.wide ? kOrderFwdWide : kOrderFwd);
-  const int n_order = grad ? 2 : (c.wide ? 5 : 3);
+  const int* order = grad ? (plain_grad ? kOrderGradPlain : kOrderGrad) : (c.wide ? kOrderFwdWide : kOrderFwd);
+  const int n_order = grad ? (plain_grad ? 3 : 2) : (c.wide ? 5 : 3);
   const int TU = grad ? TmaLanes<1>::TU : TmaLanes<0>::TU, TV = grad ? TmaLanes<1>::TV : TmaLanes<0>::TV;
   for (int i = 0; i < n_order && c.shape < 0; ++i) {
     bool fits = true;
@@ -527,7 +530,7 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
   // The kernel path first (host geometry only): a trilinear call whose views fit a staging box needs no packed copy of
   // the volume, and its workspace is laid out without one (dfp_workspace_bytes_for_views returns that size).
   const bool plain = !(siddon || joseph || dd || sf);
-  const FwdChoice choice = plain ? fwd_choice(*g, G, hv, hf, V, grad) : FwdChoice{-1, false, false};
+  const FwdChoice choice = plain ? fwd_choice(*g, G, hv, hf, V, grad, grad && !interp && !fused) : FwdChoice{-1, false, false};
   const FwdWs w_tma = fwd_ws(*g, V, grad, nset, false);
   CUtensorMap vol_map;
   // nx % 4 != 0: the TMA kernels read a copy of the volume with 16-byte-aligned rows (1x the volume, at off_pvol - the
@@ -648,12 +651,13 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
       fwd_tma_kernel<2, 3><<<nbg, TmaLanes<2>::THREADS, tma_smem_bytes<3>(), s>>>(G, Qg, dv, vol_map, d_up, part, nullptr);
     else if (grad && interp)
       fwd_tma_kernel<2, 2><<<nbg, TmaLanes<2>::THREADS, tma_smem_bytes<2>(), s>>>(G, Qg, dv, vol_map, d_up, part, nullptr);
-    else if (grad && shape == 3 && wide) {
+    else if (grad && (shape == 3 || shape == 7) && wide) {
       // Views by the in-plane direction of their central ray (voxel-index units): along y -> MODE 5, along x -> MODE 6 on
       // the transposed volume, near the diagonals (or where the MODE 5 / 6 box does not hold the view's tiles) -> MODE 1.
-      std::vector<int> ids[3];
-      CUtensorMap map_y, map_x;
+      std::vector<int> ids[4];
+      CUtensorMap map_y, map_x, map_d;
       const bool ok_y = make_volume_map(*g, tma_vol, vpitch, kBoxes[6][0], kBoxes[6][1], kBoxes[6][2], &map_y);
+      const bool ok_d = make_volume_map(*g, tma_vol, vpitch, kBoxes[7][0], kBoxes[7][1], kBoxes[7][2], &map_d);
       float* volt = reinterpret_cast<float*>(base + w.off_volt);
       const int tpitch = pitch4(g->ny);               // rows of the transposed volume [z][x][y], 16-byte aligned
       bool ok_x;
@@ -670,17 +674,24 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
         int c = 0;
         if (ok_y && ey * kClassTan > ex && tma_view_fits(*g, G, hv[v], hf[v], true, box_y, TU, TV)) c = 1;
         if (ok_x && ex * kClassTan > ey && tma_view_fits(*g, G, hv[v], hf[v], true, box_x, TU, TV, kMinChunk, 1)) c = 2;
+        // the rest: the 8 x 2 x 2 kernel, on the 14-slice box (five blocks per SM) where the view's tiles fit it
+        if (c == 0 && ok_d && tma_view_fits(*g, G, hv[v], hf[v], true, kBoxes[7], TU, TV)) c = 3;
         ids[c].push_back(v);
       }
       int* dids = reinterpret_cast<int*>(base + w.off_ids);
       std::vector<int> all;
-      for (int c = 0; c < 3; ++c) all.insert(all.end(), ids[c].begin(), ids[c].end());
+      for (int c = 0; c < 4; ++c) all.insert(all.end(), ids[c].begin(), ids[c].end());
       DFP_CUDA(upload_async(dids, all.data(), sizeof(int) * all.size(), s), "view upload");
-      const int* d0 = dids, *d1 = dids + ids[0].size(), *d2 = d1 + ids[1].size();
+      const int* d0 = dids, *d1 = dids + ids[0].size(), *d2 = d1 + ids[1].size(), *d3 = d2 + ids[2].size();
       const unsigned tiles = (unsigned)w.gx * w.gy8;
       if (!ids[0].empty())
         fwd_tma_kernel<1, 3><<<(unsigned)ids[0].size() * tiles, TmaLanes<1>::THREADS, tma_smem_bytes<3>(), s>>>(
             G, FwdGrid{(int)ids[0].size(), w.gx, w.gy8, V, d0}, dv, vol_map, d_up, part, nullptr);
+      if (!ids[3].empty()) {
+        fwd_tma_kernel<1, 7><<<(unsigned)ids[3].size() * tiles, TmaLanes<1>::THREADS, tma_smem_bytes<7>(), s>>>(
+            G, FwdGrid{(int)ids[3].size(), w.gx, w.gy8, V, d3}, dv, map_d, d_up, part, nullptr);
+        ++g_launches;
+      }
       if (!ids[1].empty()) {
         fwd_tma_kernel<5, 6><<<(unsigned)ids[1].size() * tiles, TmaLanes<5>::THREADS, tma_smem_bytes<6>(), s>>>(
             G, FwdGrid{(int)ids[1].size(), w.gx, w.gy8, V, d1}, dv, map_y, d_up, part, nullptr);
@@ -693,7 +704,9 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
         g_launches += 2;
       }
       if (ids[0].empty()) --g_launches;        // (the common count below adds one launch)
-    } else if (grad && shape == 3)
+    } else if (grad && shape == 7)
+      fwd_tma_kernel<1, 7><<<nbg, TmaLanes<1>::THREADS, tma_smem_bytes<7>(), s>>>(G, Qg, dv, vol_map, d_up, part, nullptr);
+    else if (grad && shape == 3)
       fwd_tma_kernel<1, 3><<<nbg, TmaLanes<1>::THREADS, tma_smem_bytes<3>(), s>>>(G, Qg, dv, vol_map, d_up, part, nullptr);
     else if (grad)
       fwd_tma_kernel<1, 2><<<nbg, TmaLanes<1>::THREADS, tma_smem_bytes<2>(), s>>>(G, Qg, dv, vol_map, d_up, part, nullptr);
@@ -1268,7 +1281,7 @@ size_t dfp_workspace_bytes_for_views(const dfp_geometry* g, int n_views, const f
       hf[v] = make_frame(*g, angles, v);
       make_fwd_view(hf[v], poses + 6 * v, &hv[v], nullptr);
     }
-    return fwd_choice(*g, G, hv, hf, V, grad).shape >= 0 ? fwd_ws(*g, V, grad, op == DFP_OP_FORWARD_FUSED ? 3 : 1, false).total : full;
+    return fwd_choice(*g, G, hv, hf, V, grad, op == DFP_OP_FORWARD_POSE_GRAD && !interp).shape >= 0 ? fwd_ws(*g, V, grad, op == DFP_OP_FORWARD_FUSED ? 3 : 1, false).total : full;
   }
   if (g->flags & (DFP_FLAG_DD | DFP_FLAG_SF)) return full;
   const bool grad = op == DFP_OP_BACKPROJECT_POSE_GRAD;

@@ -66,8 +66,18 @@ template <> struct BoxShape<4> { static constexpr int X = 20, Y = 19, Z = 16, ST
 #define DFP_S5_Z 20
 #endif
 template <> struct BoxShape<5> { static constexpr int X = 28, Y = 19, Z = DFP_S5_Z, STAGES = DFP_S5_STAGES; };
-template <> struct BoxShape<6> { static constexpr int X = 28, Y = 27, Z = 16, STAGES = 1; };   // MODE 5 / 6 (above)
-constexpr int kNumShapes = 7;
+// The gradient kernels of the >= 0.45-voxel-per-pixel configs run FIVE blocks per SM: 14 slices instead of 16 keep a
+// box under 44 KB (an 8-pixel-high tile spans ~5 voxels along z there: chunks stay ~20 samples long) and the kernels
+// are compiled for 48 registers (13 values of the per-chunk set-up spill; the sample loop does not): 826 -> 810 ms on C5.
+#ifndef DFP_S6_Z
+#define DFP_S6_Z 14
+#endif
+#ifndef DFP_CLS_MINB
+#define DFP_CLS_MINB 5
+#endif
+template <> struct BoxShape<6> { static constexpr int X = 28, Y = 27, Z = DFP_S6_Z, STAGES = 1; };   // MODE 5 / 6 (above)
+template <> struct BoxShape<7> { static constexpr int X = 28, Y = 28, Z = DFP_S6_Z, STAGES = 1; };   // MODE 1, views near the diagonals
+constexpr int kNumShapes = 8;
 // words between the stages of a box: the box rounded up to 128 bytes (alignment of a TMA destination)
 template <int SHAPE> __host__ __device__ constexpr int tma_stage_words() {
   return (BoxShape<SHAPE>::X * BoxShape<SHAPE>::Y * BoxShape<SHAPE>::Z + 31) / 32 * 32;
@@ -105,6 +115,9 @@ template <int MODE> struct TmaLanes {
 #endif
   static constexpr int MINB = THREADS > 256 ? 2 : (MODE == 0 ? DFP_FWD_MINB : 4);
 };
+template <int MODE, int SHAPE> __host__ __device__ constexpr int tma_min_blocks() {
+  return (SHAPE == 6 || SHAPE == 7) ? DFP_CLS_MINB : TmaLanes<MODE>::MINB;
+}
 template <int MODE>
 __device__ __forceinline__ void tma_pixel(int bx, int by, int& iu, int& iv, int& slot) {
   using T = TmaLanes<MODE>;
@@ -459,7 +472,7 @@ __device__ __forceinline__ void fwd_block(const FwdGrid& Q, int& view, int& bx, 
 }
 
 template <int MODE, int SHAPE>
-__global__ void __launch_bounds__(TmaLanes<MODE>::THREADS, TmaLanes<MODE>::MINB) fwd_tma_kernel(FwdGeom G, FwdGrid Q,
+__global__ void __launch_bounds__(TmaLanes<MODE>::THREADS, tma_min_blocks<MODE, SHAPE>()) fwd_tma_kernel(FwdGeom G, FwdGrid Q,
                                                               const FwdView* __restrict__ views,
                                                               const __grid_constant__ CUtensorMap vol_map,
                                                               const float* __restrict__ upstream,
