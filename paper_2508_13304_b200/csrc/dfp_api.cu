@@ -327,6 +327,7 @@ cudaError_t ensure_smem_attributes() {
   DFP_ATTR((fwd_tma_kernel<1, 3>), tma_smem_bytes<3>());
   DFP_ATTR((fwd_tma_kernel<1, 7>), tma_smem_bytes<7>());
   DFP_ATTR((fwd_tma_kernel<2, 7>), tma_smem_bytes<7>());
+  DFP_ATTR((fwd_tma_kernel<3, 7>), tma_smem_bytes<7>());
   DFP_ATTR((fwd_tma_kernel<5, 6>), tma_smem_bytes<6>());
   DFP_ATTR((fwd_tma_kernel<6, 6>), tma_smem_bytes<6>());
   DFP_ATTR((fwd_tma_kernel<2, 2>), tma_smem_bytes<2>());
@@ -531,7 +532,7 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
   // The kernel path first (host geometry only): a trilinear call whose views fit a staging box needs no packed copy of
   // the volume, and its workspace is laid out without one (dfp_workspace_bytes_for_views returns that size).
   const bool plain = !(siddon || joseph || dd || sf);
-  const FwdChoice choice = plain ? fwd_choice(*g, G, hv, hf, V, grad, grad && !fused) : FwdChoice{-1, false, false};
+  const FwdChoice choice = plain ? fwd_choice(*g, G, hv, hf, V, grad, grad) : FwdChoice{-1, false, false};
   const FwdWs w_tma = fwd_ws(*g, V, grad, nset, false);
   CUtensorMap vol_map;
   // nx % 4 != 0: the TMA kernels read a copy of the volume with 16-byte-aligned rows (1x the volume, at off_pvol - the
@@ -644,7 +645,9 @@ int run_forward_slice(const dfp_geometry* g, int V, const float* angles, const f
     // 1-D grid, one block per (view, tile), ordered view group -> tile -> view (dfp_fwd_tma.cuh: fwd_block)
     const FwdGrid Qf{V, w.gx, w.gy, V, nullptr}, Qg{V, w.gx, w.gy8, V, nullptr};
     const unsigned nbf = (unsigned)V * w.gx * w.gy, nbg = (unsigned)V * w.gx * w.gy8;
-    if (fused && shape == 3)
+    if (fused && shape == 7)
+      fwd_tma_kernel<3, 7><<<nbg, TmaLanes<3>::THREADS, tma_smem_bytes<7>(), s>>>(G, Qg, dv, vol_map, d_up, part, d_proj);
+    else if (fused && shape == 3)
       fwd_tma_kernel<3, 3><<<nbg, TmaLanes<3>::THREADS, tma_smem_bytes<3>(), s>>>(G, Qg, dv, vol_map, d_up, part, d_proj);
     else if (fused)
       fwd_tma_kernel<3, 2><<<nbg, TmaLanes<3>::THREADS, tma_smem_bytes<2>(), s>>>(G, Qg, dv, vol_map, d_up, part, d_proj);
@@ -1284,7 +1287,7 @@ size_t dfp_workspace_bytes_for_views(const dfp_geometry* g, int n_views, const f
       hf[v] = make_frame(*g, angles, v);
       make_fwd_view(hf[v], poses + 6 * v, &hv[v], nullptr);
     }
-    return fwd_choice(*g, G, hv, hf, V, grad, op == DFP_OP_FORWARD_POSE_GRAD).shape >= 0 ? fwd_ws(*g, V, grad, op == DFP_OP_FORWARD_FUSED ? 3 : 1, false).total : full;
+    return fwd_choice(*g, G, hv, hf, V, grad, grad).shape >= 0 ? fwd_ws(*g, V, grad, op == DFP_OP_FORWARD_FUSED ? 3 : 1, false).total : full;
   }
   if (g->flags & (DFP_FLAG_DD | DFP_FLAG_SF)) return full;
   const bool grad = op == DFP_OP_BACKPROJECT_POSE_GRAD;
