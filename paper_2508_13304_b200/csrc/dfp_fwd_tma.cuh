@@ -34,12 +34,16 @@ namespace dfp {
 // simulation / measurements quoted there.
 // The host picks, per call, the first shape of the op's list that every view's tiles fit with chunks of >= kMinChunk
 // samples:
-//   shape 0  20 x 20 x 16, two stages : forward, clinical magnification and small pose angles (C2, C4)
-//   shape 1  28 x 20 x 20, two stages : forward, wider tiles / larger tilts (C5)
+//   shape 0  20 x 20 x 16, two stages : forward, clinical magnification and small pose angles (C2)
+//   shape 1  28 x 20 x 20, two stages : forward, wider tiles / larger tilts
 //   shape 2  28 x 28 x 20, one stage  : forward fallback before the gather path; gradient fallback
-//   shape 3  28 x 28 x 16, one stage  : gradient, 16 x 8-pixel tiles (the stencil needs 2 more cells per axis and a
-//            chunk lasts 4x longer than the forward's, so one stage and four blocks per SM hide the TMA latency;
-//            long enough along x and y that views at 45 degrees in the xy plane still get ~10-sample chunks).
+//   shape 3  28 x 28 x 16, one stage  : gradient kernels, 16 x 8-pixel tiles (the stencil needs 2 more cells per axis and
+//            a chunk lasts 4x longer than the forward's, so one stage and four blocks per SM hide the TMA latency;
+//            long enough along x and y that views at 45 degrees in the xy plane still get ~10-sample chunks) - taken
+//            where a view's tiles do not fit shape 7
+//   shape 4  20 x 19 x 16, two stages / shape 5  28 x 19 x 20, one stage : forward at >= 0.45 voxel per pixel (C4 / C5)
+//   shape 6  28 x 27 x 14, one stage  : gradient, views along one in-plane axis (MODE 5 / 6), five blocks per SM
+//   shape 7  28 x 28 x 14, one stage  : gradient kernels (all modes), five blocks per SM - the first choice
 template <int SHAPE> struct BoxShape;
 template <> struct BoxShape<0> { static constexpr int X = 20, Y = 20, Z = 16, STAGES = 2; };
 template <> struct BoxShape<1> { static constexpr int X = 28, Y = 20, Z = 20, STAGES = 2; };
